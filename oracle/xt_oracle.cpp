@@ -1,0 +1,401 @@
+// =====================================================================================
+// xt_oracle.cpp -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, slow, single-threaded FP64 CPU tracker that DEFINES what the CUDA path must
+// compute.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// --impl reference legs may load this library.  It shares no code, header, table or
+// constant generator with paper_2310_00317_b200/ (it has its own parser of the packed
+// lattice buffer and its own particle struct) and must be compiled with
+//     g++ -O2 -ffp-contract=off      (no FMA contraction, no fast-math)
+// so that every expression below is evaluated exactly in the order written.
+//
+// What it follows.  The paper (PAPER.md = /root/reference/PAPER.md at survey time)
+// prints no equations.  It states the structure:
+//   * PAPER.md:70  "The beam line is represented as a sequence of ... objects ... each
+//                   corresponding to an accelerator element ... (e.g. magnets, cavities,
+//                   aperture restrictions ...)"; tilts and misalignments "are handled as
+//                   changes of the reference system"; "multipolar errors".
+//   * PAPER.md:72  "a 'thin' lattice integration method is adopted" (Sixtrack lineage;
+//                   thin-lens formalism, ref [13] PAPER.md:255).
+//   * PAPER.md:74  one kernel tracks "the entire beamline"  -> per particle: turns x elements.
+//   * PAPER.md:178 aperture elements "check the particle positions with respect to the
+//                   defined aperture and stop the tracking for the particles found to be outside".
+//   * PAPER.md:184 non-collective tracking of different particles is independent.
+// The maps themselves are the standard thin-lens symplectic maps of that formalism, in the
+// reading fixed by SURVEY.md §8(c) / DESIGN.md §5 (every "paper is silent" point is listed
+// there).  Since the map sequence IS the definition, this file is the algorithm written
+// out element by element, turn by turn; no blocking, fusion or reordering.
+//
+// Pins (tests/test_oracle_pins.py, all -m "not gpu"): P1 exact-drift closed form in
+// 60-digit arithmetic; P2 thin-FODO one-cell matrix / tune (closed form); P3 symplecticity
+// of the one-turn Jacobian; P4 reversibility; P5 worked examples W1/W2 (60-digit textbook
+// evaluation, tests/golden/); P6 Horner vs direct complex power sum; P7 Courant-Snyder
+// invariant; P8 aperture edges; P9 structural invariants; P10 energy identities;
+// small-amplitude synchrotron tune for the cavity.
+// =====================================================================================
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+
+namespace {
+
+constexpr double C_LIGHT = 299792458.0;       // m/s (exact, SI)
+constexpr double PI = 3.14159265358979323846264338327950288;
+constexpr int MAX_ORDER = 20;
+
+enum ElemType : uint32_t {
+  MARKER = 0, DRIFT = 1, MULTIPOLE = 2, CAVITY = 3,
+  SROTATION = 4, XYSHIFT = 5, LIMITRECT = 6, LIMITELLIPSE = 7
+};
+
+struct Element {
+  uint32_t type = 0;
+  int order = 0;
+  double s_pos = 0.0;           // s at the element entrance (sum of preceding drift lengths)
+  // DRIFT
+  double length = 0.0;
+  // MULTIPOLE: c[n] = knl[n]/n!, sn[n] = ksl[n]/n!;  with curvature c[0] = knl[0] - hxl
+  std::vector<double> c, sn;
+  double hxl = 0.0, wf = 0.0;
+  // CAVITY
+  double lag_rad = 0.0, kz = 0.0, vn = 0.0;
+  // SROTATION
+  double cz = 1.0, sz = 0.0;
+  // XYSHIFT
+  double dx = 0.0, dy = 0.0;
+  // LIMITRECT
+  double min_x = 0.0, max_x = 0.0, min_y = 0.0, max_y = 0.0;
+  // LIMITELLIPSE
+  double a = 0.0, b = 0.0, a2 = 0.0, b2 = 0.0, a2b2 = 0.0;
+};
+
+struct Lattice {
+  double p0c = 0, mass0 = 0, q0 = 0;
+  double beta0 = 0, gamma0 = 0;
+  double tib = 0;      // 2/beta0
+  double igam2 = 0;    // 1/gamma0^2
+  std::vector<Element> el;
+};
+
+double factorial(int n) {               // exact in FP64 for n <= 22
+  double f = 1.0;
+  for (int i = 2; i <= n; ++i) f = f * static_cast<double>(i);
+  return f;
+}
+
+// Parse the packed lattice buffer (layout: xt_inputs/packed.py docstring).  Own parser;
+// the CUDA library has a different one.  Returns 0 or a negative error code.
+int parse(const void* packed, size_t nbytes, Lattice& L) {
+  const unsigned char* p = static_cast<const unsigned char*>(packed);
+  if (!p || nbytes < 48) return -2;
+  if (std::memcmp(p, "XTLAT001", 8) != 0) return -2;
+  uint32_t version, n_el;
+  uint64_t total;
+  std::memcpy(&version, p + 8, 4);
+  std::memcpy(&n_el, p + 12, 4);
+  std::memcpy(&L.p0c, p + 16, 8);
+  std::memcpy(&L.mass0, p + 24, 8);
+  std::memcpy(&L.q0, p + 32, 8);
+  std::memcpy(&total, p + 40, 8);
+  if (version != 1 || total != nbytes) return -2;
+  if (!(L.p0c > 0.0) || !(L.mass0 > 0.0) || !std::isfinite(L.p0c) || !std::isfinite(L.mass0) ||
+      !std::isfinite(L.q0))
+    return -2;
+  // Reference particle: E0 = sqrt(p0c^2 + mass0^2), beta0 = p0c/E0, gamma0 = E0/mass0.
+  const double e0 = std::sqrt(L.p0c * L.p0c + L.mass0 * L.mass0);
+  L.beta0 = L.p0c / e0;
+  L.gamma0 = e0 / L.mass0;
+  L.tib = 2.0 / L.beta0;
+  L.igam2 = 1.0 / (L.gamma0 * L.gamma0);
+
+  size_t off = 48;
+  double s = 0.0;
+  auto rd = [&](double& v) -> bool {
+    if (off + 8 > nbytes) return false;
+    std::memcpy(&v, p + off, 8);
+    off += 8;
+    return std::isfinite(v);
+  };
+  L.el.clear();
+  L.el.reserve(n_el);
+  for (uint32_t i = 0; i < n_el; ++i) {
+    if (off + 8 > nbytes) return -2;
+    Element e;
+    uint32_t aux;
+    std::memcpy(&e.type, p + off, 4);
+    std::memcpy(&aux, p + off + 4, 4);
+    off += 8;
+    e.s_pos = s;
+    switch (e.type) {
+      case MARKER: break;
+      case DRIFT:
+        if (!rd(e.length)) return -2;
+        s = s + e.length;
+        break;
+      case MULTIPOLE: {
+        if (aux > static_cast<uint32_t>(MAX_ORDER)) return -2;
+        e.order = static_cast<int>(aux);
+        double length;
+        if (!rd(e.hxl) || !rd(length)) return -2;
+        std::vector<double> knl(e.order + 1), ksl(e.order + 1);
+        for (int n = 0; n <= e.order; ++n) if (!rd(knl[n])) return -2;
+        for (int n = 0; n <= e.order; ++n) if (!rd(ksl[n])) return -2;
+        e.c.resize(e.order + 1);
+        e.sn.resize(e.order + 1);
+        for (int n = 0; n <= e.order; ++n) {
+          e.c[n] = knl[n] / factorial(n);
+          e.sn[n] = ksl[n] / factorial(n);
+        }
+        e.wf = 0.0;
+        if (e.hxl != 0.0) {
+          // Curvature folded into the dipole coefficient (cancellation-free form,
+          // DESIGN.md §5 "Multipole"): -k0l + hxl(1+delta) = -(k0l - hxl) + hxl*delta.
+          e.c[0] = knl[0] - e.hxl;
+          if (length != 0.0) e.wf = (knl[0] * e.hxl) / length;   // weak focusing k0*h*L
+        }
+        break;
+      }
+      case CAVITY: {
+        double volt, freq, lag_deg;
+        if (!rd(volt) || !rd(freq) || !rd(lag_deg)) return -2;
+        e.lag_rad = lag_deg * (PI / 180.0);
+        e.kz = (2.0 * PI * freq) / (L.beta0 * C_LIGHT);
+        e.vn = (L.q0 * volt) / L.p0c;
+        break;
+      }
+      case SROTATION:
+        if (!rd(e.cz) || !rd(e.sz)) return -2;
+        break;
+      case XYSHIFT:
+        if (!rd(e.dx) || !rd(e.dy)) return -2;
+        break;
+      case LIMITRECT:
+        if (!rd(e.min_x) || !rd(e.max_x) || !rd(e.min_y) || !rd(e.max_y)) return -2;
+        break;
+      case LIMITELLIPSE:
+        if (!rd(e.a) || !rd(e.b)) return -2;
+        e.a2 = e.a * e.a;
+        e.b2 = e.b * e.b;
+        e.a2b2 = e.a2 * e.b2;
+        break;
+      default: return -2;
+    }
+    L.el.push_back(std::move(e));
+  }
+  if (off != nbytes) return -2;
+  return 0;
+}
+
+// Per-particle cached constants: pure functions of the stored delta, ptau; recomputed
+// only after a cavity (DESIGN.md §5 "Per-particle cached constants").
+struct Cached {
+  double opd2, b, g, rv0v;
+};
+
+inline Cached derive_cached(const Lattice& L, double delta, double ptau) {
+  Cached k;
+  const double opd = 1.0 + delta;
+  k.opd2 = opd * opd;
+  k.b = 1.0 + L.beta0 * ptau;
+  const double t = ptau * (ptau + L.tib);
+  k.g = t * L.igam2;
+  k.rv0v = k.b / opd;
+  return k;
+}
+
+}  // namespace
+
+extern "C" {
+
+// Host pointers, all of length n_part.  at_element and min_margin may be NULL.
+struct xo_particles {
+  double *x, *px, *y, *py, *zeta, *delta, *ptau, *rpp, *rvv, *s;
+  int64_t *at_turn, *state, *at_element;
+  double* min_margin;   // out (if non-NULL): min over all aperture checks passed through of
+                        // the distance [m] to the aperture edge (reading A3); +inf if none
+};
+
+// delta -> ptau, rpp, rvv (DESIGN.md §5 "Init helper"):
+//   t = delta*(delta+2); ptau = t/(sqrt(t + 1/beta0^2) + 1/beta0)   [= sqrt((1+delta)^2 + 1/(b0 g0)^2)... energy identity]
+int xo_init_derived(const void* packed, size_t nbytes, const double* delta, double* ptau,
+                    double* rpp, double* rvv, int64_t n) {
+  Lattice L;
+  int rc = parse(packed, nbytes, L);
+  if (rc) return rc;
+  const double ib = 1.0 / L.beta0;
+  const double ib2 = ib * ib;
+  for (int64_t i = 0; i < n; ++i) {
+    const double d = delta[i];
+    const double t = d * (d + 2.0);
+    const double pt = t / (std::sqrt(t + ib2) + ib);
+    const double opd = 1.0 + d;
+    const double b = 1.0 + L.beta0 * pt;
+    ptau[i] = pt;
+    rpp[i] = 1.0 / opd;
+    rvv[i] = opd / b;
+  }
+  return 0;
+}
+
+// Reference-particle quantities as the oracle derives them (for tests / input scaling).
+int xo_reference(const void* packed, size_t nbytes, double* beta0, double* gamma0) {
+  Lattice L;
+  int rc = parse(packed, nbytes, L);
+  if (rc) return rc;
+  *beta0 = L.beta0;
+  *gamma0 = L.gamma0;
+  return 0;
+}
+
+// s position (entrance) of every element; out has n_elements entries.  Returns n_elements.
+int64_t xo_s_table(const void* packed, size_t nbytes, double* out, int64_t cap) {
+  Lattice L;
+  int rc = parse(packed, nbytes, L);
+  if (rc) return rc;
+  const int64_t n = static_cast<int64_t>(L.el.size());
+  for (int64_t i = 0; i < n && i < cap; ++i) out[i] = L.el[i].s_pos;
+  return n;
+}
+
+// Track n_part particles for n_turns turns through the whole line.
+// In/out arrays as in xo_particles.  Lost particles (state == 0) are skipped entirely.
+int xo_track(const void* packed, size_t nbytes, const xo_particles* P, int64_t n_part,
+             int64_t n_turns) {
+  if (!P || n_part < 0 || n_turns < 0) return -1;
+  Lattice L;
+  int rc = parse(packed, nbytes, L);
+  if (rc) return rc;
+  const int64_t n_el = static_cast<int64_t>(L.el.size());
+
+  for (int64_t ip = 0; ip < n_part; ++ip) {
+    double x = P->x[ip], px = P->px[ip], y = P->y[ip], py = P->py[ip];
+    double zeta = P->zeta[ip], delta = P->delta[ip], ptau = P->ptau[ip];
+    double rpp = P->rpp[ip], rvv = P->rvv[ip], s = P->s[ip];
+    int64_t at_turn = P->at_turn[ip], state = P->state[ip];
+    int64_t at_element = P->at_element ? P->at_element[ip] : 0;
+    double margin = std::numeric_limits<double>::infinity();
+    Cached k = derive_cached(L, delta, ptau);
+
+    for (int64_t turn = 0; turn < n_turns && state == 1; ++turn) {
+      for (int64_t ie = 0; ie < n_el && state == 1; ++ie) {
+        const Element& e = L.el[ie];
+        switch (e.type) {
+          case MARKER: break;
+
+          case DRIFT: {
+            // Exact drift (thin-lattice integration):
+            //   x += L px/pz, y += L py/pz, zeta += L (1 - (1+beta0 ptau)/pz),
+            //   pz = sqrt((1+delta)^2 - px^2 - py^2),
+            // with the zeta increment rewritten cancellation-free through
+            //   pz^2 - b^2 = g - px^2 - py^2   (DESIGN.md §5 "Drift").
+            const double t1 = px * px;
+            const double pxy2 = py * py + t1;
+            const double pz = std::sqrt(k.opd2 - pxy2);
+            const double s1 = pz + k.b;
+            const double den = pz * s1;
+            const double rr = 1.0 / den;
+            const double lr = e.length * rr;
+            const double lpz = lr * s1;
+            x = px * lpz + x;
+            y = py * lpz + y;
+            zeta = (k.g - pxy2) * lr + zeta;
+            break;
+          }
+
+          case MULTIPOLE: {
+            // Thin multipole kick ("multipolar errors", PAPER.md:72 thin maps):
+            //   dpx - i dpy = -sum_n (knl[n] + i ksl[n]) (x + i y)^n / n!   by complex Horner,
+            // highest order first.
+            const int N = e.order;
+            double re = e.c[N];
+            double im = e.sn[N];
+            for (int n = N - 1; n >= 0; --n) {
+              const double nre = re * x + (e.c[n] - im * y);
+              const double nim = re * y + (e.sn[n] + im * x);
+              re = nre;
+              im = nim;
+            }
+            px = px - re;
+            py = py + im;
+            if (e.hxl != 0.0) {
+              // Horizontal curvature: dpx = hxl (1+delta) [the hxl*1 part is folded into c[0]],
+              // weak focusing -k0 h L x, path length dzeta = -hxl x beta0/beta.
+              px = e.hxl * delta + px;
+              px = px - e.wf * x;
+              zeta = zeta - (e.hxl * x) * k.rv0v;
+            }
+            break;
+          }
+
+          case CAVITY: {
+            // Thin RF cavity: energy kick, transverse normalised momenta unchanged.
+            const double phase = e.lag_rad - e.kz * zeta;
+            ptau = e.vn * std::sin(phase) + ptau;
+            const double t = ptau * (ptau + L.tib);
+            delta = t / (std::sqrt(t + 1.0) + 1.0);     // = sqrt(1+t) - 1 without cancellation
+            const double opd = 1.0 + delta;
+            rpp = 1.0 / opd;
+            const double b = 1.0 + L.beta0 * ptau;
+            rvv = opd / b;
+            k.opd2 = opd * opd;
+            k.b = b;
+            k.g = t * L.igam2;
+            k.rv0v = b / opd;
+            break;
+          }
+
+          case SROTATION: {
+            // Rotation of the reference system about s ("tilts").
+            const double nx = e.cz * x + e.sz * y;
+            const double ny = e.cz * y - e.sz * x;
+            const double npx = e.cz * px + e.sz * py;
+            const double npy = e.cz * py - e.sz * px;
+            x = nx; y = ny; px = npx; py = npy;
+            break;
+          }
+
+          case XYSHIFT:
+            // Transverse shift of the reference system ("misalignments").
+            x = x - e.dx;
+            y = y - e.dy;
+            break;
+
+          case LIMITRECT: {
+            // PAPER.md:178; edges inclusive, NaN -> lost (reading A3, A4).
+            const bool inside = (x >= e.min_x) && (x <= e.max_x) && (y >= e.min_y) && (y <= e.max_y);
+            double m = std::fmin(std::fmin(x - e.min_x, e.max_x - x), std::fmin(y - e.min_y, e.max_y - y));
+            m = std::fabs(m);
+            if (m < margin) margin = m;
+            if (!inside) { state = 0; at_element = ie; s = e.s_pos; }
+            break;
+          }
+
+          case LIMITELLIPSE: {
+            const double tt = (x * x) * e.b2 + (y * y) * e.a2;
+            const bool inside = (tt <= e.a2b2);
+            double m = std::fabs(std::sqrt((x * x) / e.a2 + (y * y) / e.b2) - 1.0) * std::fmin(e.a, e.b);
+            if (m < margin) margin = m;
+            if (!inside) { state = 0; at_element = ie; s = e.s_pos; }
+            break;
+          }
+        }
+      }
+      if (state == 1) {      // turn completed
+        at_turn = at_turn + 1;
+        s = 0.0;
+      }
+    }
+
+    P->x[ip] = x; P->px[ip] = px; P->y[ip] = y; P->py[ip] = py;
+    P->zeta[ip] = zeta; P->delta[ip] = delta; P->ptau[ip] = ptau;
+    P->rpp[ip] = rpp; P->rvv[ip] = rvv; P->s[ip] = s;
+    P->at_turn[ip] = at_turn; P->state[ip] = state;
+    if (P->at_element) P->at_element[ip] = at_element;
+    if (P->min_margin) P->min_margin[ip] = margin;
+  }
+  return 0;
+}
+
+}  // extern "C"
