@@ -1,0 +1,349 @@
+#!/usr/bin/env python
+"""Benchmark of the tracking hot path (contract: see the task statement / DESIGN.md section 8).
+
+A step = one pass of the whole hot path over one batch: restore the seeded synthetic
+ensemble (device copy), then ``xt_track`` it for the config's number of turns through the
+config's lattice.  Default workload: BASELINE.json configs[3] (LHC-sized lattice with
+misalignments, 10^7 particles, 100 turns, SoA FP64 ~1 GB).  ``value`` is
+particle*element*turns/s over all ranks with inputs resident in HBM; ``e2e`` is the same
+metric through ``xt_track_host`` with pinned HOST buffers (H2D + D2H inside the timed
+region).  The roofline is the FP64 ALU pipe: peak = the library's own DFMA microbenchmark
+measured in this run.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from xt_inputs import configs as C  # noqa: E402
+
+METRIC = "particle*element*turns/s (FP64)"
+UNIT = "particle*element*turns/s"
+WORKLOADS = {
+    2: "configs[2]: synthetic LHC-sized ring, 8606 elements (order-15 multipole errors, elliptical "
+       "apertures, 8 cavities), 100000 particles (6D Gaussian 1 sigma), 1000 turns",
+    3: "configs[3]: LHC-sized ring with SRotation/XYShift misalignments, 10366 elements, "
+       "10000000 particles (6D Gaussian 2 sigma, SoA FP64 ~1 GB), 100 turns",
+    1: "configs[1]: FODO ring with sextupoles and rectangular apertures, 71 elements, 1000000 "
+       "particles (polar grid), 1000 turns",
+    0: "configs[0]: thin-lens FODO ring, 41 elements, 1000 particles, 100 turns",
+}
+
+# Algorithmic FP64 flops per element visit (minimal arithmetic of the
+# canonical forms; FMA = 2, add/mul/sqrt/div = 1, compares = 0, sin = 1) ...
+FLOPS_MIN = dict(drift=17, mult_base=2, mult_per_order=8, curved_extra=7, cavity=19, srot=12,
+                 shift=2, rect=0, ellipse=5)
+# ... and FP64 flops as executed by the sm_100a kernel (IEEE sqrt / div / sin expansions
+# counted; from the SASS of libxt_b200.so, profiles/sass_fp64_counts_r01.md)
+FLOPS_EXEC = dict(drift=43, mult_base=2, mult_per_order=8, curved_extra=7, cavity=110, srot=12,
+                  shift=2, rect=0, ellipse=5)
+
+
+def flops_per_particle_turn(info: dict, table: dict) -> float:
+    t = info["n_by_type"]
+    n_mult = t[2]
+    return (t[1] * table["drift"] + n_mult * table["mult_base"] + info["sum_order"] * table["mult_per_order"]
+            + info["n_curved"] * table["curved_extra"] + t[3] * table["cavity"] + t[4] * table["srot"]
+            + t[5] * table["shift"] + t[6] * table["rect"] + t[7] * table["ellipse"])
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with nvidia-smi while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_inputs(cfg: int, rank: int):
+    """Seeded synthetic lattice + ensemble of config ``cfg``."""
+    buf = C.pack(C.lattice(cfg))
+    if cfg in (0, 2, 3) and rank:
+        coords = {0: C.particles_cfg0, 2: C.particles_cfg2, 3: C.particles_cfg3}[cfg](seed=1000 + cfg + 100 * rank)
+    else:
+        coords = C.particles(cfg)
+    return buf, coords
+
+
+def oracle_sample(cfg: int, buf: bytes, coords: dict, budget_s: float = 15.0):
+    """The oracle, as it stands, single-threaded, on a bounded sample of the same workload."""
+    from oracle import oracle as O
+    import struct
+    turns_full = C.n_turns(cfg)
+    n_el = struct.unpack_from("<I", buf, 12)[0]          # header field n_elements
+    # calibrate on a tiny run, then size the sample for ~budget_s
+    cal_n = 8
+    cal = O.new_particles(buf, C.subsample(coords, slice(0, cal_n)))
+    cal_turns = max(1, min(turns_full, 200000 // max(n_el, 1)))
+    t0 = time.perf_counter()
+    O.track(buf, cal, cal_turns)
+    rate = cal_n * cal_turns * n_el / max(time.perf_counter() - t0, 1e-6)
+    turns = min(turns_full, 100)
+    n = int(max(8, min(len(coords["x"]), rate * budget_s / (turns * n_el))))
+    p = O.new_particles(buf, C.subsample(coords, slice(0, n)))
+    t0 = time.perf_counter()
+    O.track(buf, p, turns)
+    dt = time.perf_counter() - t0
+    return {"value": n * turns * n_el / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "first %d particles of the workload x %d turns x %d elements, 1 thread, %.1f s"
+                      % (n, turns, n_el, dt), "seconds": dt}
+
+
+def run_reference(args):
+    """--impl reference: the oracle (a deliberately plain CPU program) on the same workload,
+    each step a bounded sample.  Rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = args.config
+    buf, coords = make_inputs(cfg, 0)
+    budget = 8.0
+    for _ in range(args.warmup):
+        oracle_sample(cfg, buf, coords, budget_s=0.5)
+    vals, secs, last = [], [], None
+    for _ in range(args.steps):
+        last = oracle_sample(cfg, buf, coords, budget_s=budget)
+        vals.append(last["value"]); secs.append(last["seconds"])
+    value = float(np.mean(vals))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(secs)),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": WORKLOADS[cfg], "sampled": True},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                             "sample": last["sample"]},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
+    ap.add_argument("--turns", type=int, default=0, help="override the config's turns (testing only)")
+    ap.add_argument("--particles", type=int, default=0, help="override the particle count (testing only)")
+    ap.add_argument("--block", type=int, default=0)
+    ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and configs[2] legs")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    import paper_2310_00317_b200 as X
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = args.config
+    turns = args.turns or C.n_turns(cfg)
+    buf, coords = make_inputs(cfg, rank)
+    if args.particles:
+        coords = C.subsample(coords, slice(0, args.particles))
+    lat = X.xt_lattice_create(buf)
+    info = lat.info
+    n_el = info["n_elements"]
+    n_part = len(coords["x"])
+    pristine = X.new_particles(lat, coords)
+    work = {k: torch.empty_like(v) for k, v in pristine.items()}
+    stream = torch.cuda.current_stream()
+
+    def step(ev0=None, ev1=None):
+        for k in work:
+            work[k].copy_(pristine[k])
+        if ev0 is not None:
+            ev0.record(stream)
+        X.xt_track_ex(lat, work, turns, block_size=args.block)
+        if ev1 is not None:
+            ev1.record(stream)
+
+    peak_flops, peak_ms = X.xt_fp64_fma_peak()
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = X.xt_launch_count()
+    kev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_begin.record(stream)
+    for i in range(args.steps):
+        step(*kev[i])
+    t_end.record(stream)
+    barrier()
+    launches = X.xt_launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = t_begin.elapsed_time(t_end)
+    kernel_ms = float(np.mean([a.elapsed_time(b) for a, b in kev]))
+    alive = int((work["state"] == 1).sum().item())
+    tm = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+    total_ms = float(tm.item())
+    ms_per_step = total_ms / args.steps
+    units_per_step = float(n_part) * n_el * turns            # per rank (nominal: lost ones included)
+    value = world * units_per_step / (ms_per_step * 1e-3)
+
+    line = None
+    if rank == 0:
+        f_min = flops_per_particle_turn(info, FLOPS_MIN)
+        f_exec = flops_per_particle_turn(info, FLOPS_EXEC)
+        pt_per_s = n_part * turns / (kernel_ms * 1e-3)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOADS[cfg], "n_particles_per_gpu": n_part, "n_elements": n_el,
+                       "n_turns": turns, "l2": "inputs (%.2f GB SoA per GPU) larger than L2" %
+                                              (n_part * 13 * 8 / 1e9),
+                       "alive_after_step": alive, "block_size": args.block or 128,
+                       "lattice_image_bytes": info["image_bytes"], "tma_chunks_per_turn": info["n_chunks"]},
+            "particle_turns_per_s": world * n_part * turns / (ms_per_step * 1e-3),
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "roofline": {
+                "bound": "alu", "unit": "TFLOP/s",
+                "achieved": f_min * pt_per_s / 1e12, "peak": peak_flops / 1e12,
+                "frac": f_min * pt_per_s / peak_flops,
+                "achieved_executed": f_exec * pt_per_s / 1e12, "frac_executed": f_exec * pt_per_s / peak_flops,
+                "peak_source": "xt_fp64_fma_peak: DFMA microbenchmark in this run (%.2f ms), burst; "
+                               "nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2 TFLOP/s" % peak_ms,
+                "kernel": "xt_track_kernel", "kernel_ms": kernel_ms,
+                "flops_per_particle_turn": {"algorithmic": f_min, "executed": f_exec},
+                "traffic": None,
+            },
+        }
+
+    if not args.no_extras:
+        # ---- e2e: the same step through xt_track_host with pinned HOST buffers
+        host = {k: torch.empty(v.shape, dtype=v.dtype, pin_memory=True) for k, v in pristine.items()}
+        host0 = {k: v.cpu() for k, v in pristine.items()}
+        for k in host:
+            host[k].copy_(host0[k])
+        barrier()
+        t0 = time.perf_counter()
+        X.xt_track_host(lat, host, turns, block_size=args.block)     # synchronises the stream itself
+        barrier()
+        e2e_s = time.perf_counter() - t0
+        te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        if rank == 0:
+            nbytes = sum(v.numel() * 8 for v in host.values())
+            line["e2e"] = {"value": world * units_per_step / float(te.item()), "unit": UNIT,
+                           "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                           "seconds": float(te.item()), "api": "xt_track_host (pinned host SoA)",
+                           "alive_after_step": int((host["state"] == 1).sum().item())}
+        del host, host0
+    del work, pristine
+    lat.close()
+    torch.cuda.empty_cache()
+
+    if rank == 0 and not args.no_extras:
+        # ---- configs[2] (the other configuration the north_star's target names), same run
+        if cfg == 3 and world == 1:
+            b2, c2 = make_inputs(2, 0)
+            l2 = X.xt_lattice_create(b2)
+            pr2 = X.new_particles(l2, c2)
+            w2 = {k: torch.empty_like(v) for k, v in pr2.items()}
+            t2 = C.n_turns(2)
+            ms2 = []
+            for it in range(3):
+                for k in w2:
+                    w2[k].copy_(pr2[k])
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                X.xt_track_ex(l2, w2, t2, block_size=args.block)
+                b.record(stream)
+                torch.cuda.synchronize()
+                ms2.append(a.elapsed_time(b))
+            k2 = min(ms2[1:])
+            pt2 = len(c2["x"]) * t2 / (k2 * 1e-3)
+            line["also"] = {"workload": WORKLOADS[2], "value": pt2 * l2.info["n_elements"], "unit": UNIT,
+                            "kernel_ms": k2,
+                            "frac": flops_per_particle_turn(l2.info, FLOPS_MIN) * pt2 / peak_flops,
+                            "frac_executed": flops_per_particle_turn(l2.info, FLOPS_EXEC) * pt2 / peak_flops,
+                            "alive_after_step": int((w2["state"] == 1).sum().item())}
+            l2.close()
+        # ---- cpu_baseline: the oracle as it stands on a bounded sample of the same workload
+        line["cpu_baseline"] = {k: v for k, v in oracle_sample(cfg, buf, coords).items() if k != "seconds"}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,167 @@
+/* =====================================================================================
+ * xt.h -- C ABI of the B200-native multi-turn single-particle tracking engine.
+ *
+ * What the library computes.  "The beam line is represented as a sequence of ... objects
+ * ..., each corresponding to an accelerator element" (section "Lattice
+ * modelling and single particle tracking"); "a 'thin' lattice integration method is
+ * adopted"; one compiled kernel is "able to track the entire beamline"
+ * for "particles ensembles"; aperture elements "check the
+ * particle positions with respect to the defined aperture and stop the tracking for the
+ * particles found to be outside"; particles are independent on
+ * non-collective lines.  The paper prints no map formulas; the maps are
+ * those fixed in DESIGN.md section 5 (canonical arithmetic order included).
+ *
+ * Conventions.  Plain pointers and sizes only.  Every particle pointer is a DEVICE pointer
+ * unless the function name ends in _host.  All calls that take a stream are asynchronous on
+ * that stream and never synchronise the host (the _host variants do, once, at the end).
+ * Return value: 0 (XT_OK) or a negative xt_status; on failure no output is written and
+ * xt_last_error() holds a thread-local message.  No exceptions, no abort().
+ * There is no CPU fallback: without a CUDA device every compute entry point fails with
+ * XT_ERR_CUDA.
+ * ===================================================================================== */
+#ifndef XT_H_
+#define XT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  XT_OK = 0,
+  XT_ERR_INVALID_ARG = -1, /* NULL pointer, negative count, bad option                       */
+  XT_ERR_BAD_LATTICE = -2, /* bad magic/version/size, unknown type, truncated buffer,         */
+                           /* order > XT_MAX_ORDER, non-finite parameter, p0c/mass0 <= 0      */
+  XT_ERR_CUDA = -3,        /* CUDA runtime failure (message in xt_last_error)                 */
+  XT_ERR_NOMEM = -4        /* host or device allocation failed                                */
+} xt_status;
+
+#define XT_MAX_ORDER 20
+
+/* Element type ids of the packed lattice buffer (magnets, cavities, aperture
+ * restrictions; tilts / misalignments as changes of the reference system). */
+enum {
+  XT_MARKER = 0,
+  XT_DRIFT = 1,       /* length                                                  (map M1)   */
+  XT_MULTIPOLE = 2,   /* aux = order N; hxl, length, knl[0..N], ksl[0..N] (raw)  (map M2)   */
+  XT_CAVITY = 3,      /* voltage [V], frequency [Hz], lag [deg]                  (map M3)   */
+  XT_SROTATION = 4,   /* cos_z, sin_z                                            (map M4)   */
+  XT_XYSHIFT = 5,     /* dx, dy                                                  (map M4)   */
+  XT_LIMITRECT = 6,   /* min_x, max_x, min_y, max_y (edges inclusive)            (step A)   */
+  XT_LIMITELLIPSE = 7 /* a, b (edge inclusive)                                   (step A)   */
+};
+
+/* Packed lattice buffer (HOST memory, little-endian, 8-byte aligned records):
+ *   header, 48 B: char magic[8] = "XTLAT001"; uint32 version = 1; uint32 n_elements;
+ *                 double p0c [eV]; double mass0 [eV]; double q0 [e]; uint64 total_bytes
+ *   n_elements records: uint32 type; uint32 aux; double params[...] as listed above.
+ * beta0, gamma0 are derived inside: E0 = sqrt(p0c^2 + mass0^2), beta0 = p0c/E0,
+ * gamma0 = E0/mass0.  Multipole strengths follow the MAD-X convention (PAPER.md:70,
+ * "imported from MAD-X"): knl[n] = integrated d^n By/dx^n / (P0/q0), NOT divided by n!. */
+
+typedef struct xt_lattice xt_lattice; /* opaque; immutable after create; owns its device image */
+
+/* Particle ensemble, structure of arrays, each of length n_part, caller-owned.
+ * x, y, zeta [m]; px = Px/P0, py = Py/P0; delta = (P-P0)/P0; ptau = (E-E0)/(P0 c);
+ * rpp = P0/P; rvv = beta/beta0.  delta AND ptau are both state (reading A7): they
+ * are loaded and stored verbatim so that n calls of k turns equal one call of n*k turns
+ * bit for bit.  state: 1 alive, 0 lost on an aperture.  For a lost particle the coordinates
+ * are those AT the aperture that stopped it, at_element is that element's index in the
+ * packed buffer, s the sum of drift lengths before it, at_turn the number of COMPLETED
+ * turns.  For survivors s = 0 and at_turn has advanced by n_turns.
+ * particle_id and at_element may be NULL.  particle_id is never written. */
+typedef struct {
+  double *x, *px, *y, *py, *zeta, *delta;
+  double *ptau, *rpp, *rvv;
+  double *s;
+  int64_t *at_turn, *state;
+  int64_t *particle_id, *at_element;
+} xt_particles;
+
+/* Options of xt_track_ex.  Zero-initialise for the defaults. */
+typedef struct {
+  int64_t turns_per_launch; /* 0: auto (= compact_every when compaction is active, else all)  */
+  int64_t compact_every;    /* 0: auto (1000 turns if the lattice has apertures and n_turns   */
+                            /*    exceeds it); < 0: never compact; > 0: period in turns       */
+  int32_t block_size;       /* 0: auto (128); else a multiple of 32 in [32, 512]              */
+  int32_t reserved;
+} xt_track_opts;
+
+/* Static description of a lattice image; counts are per turn. */
+typedef struct {
+  int64_t n_elements;       /* records in the packed buffer (markers included)                */
+  int64_t n_records;        /* records in the device image (markers dropped)                  */
+  int64_t n_chunks;         /* TMA chunks per turn                                            */
+  int64_t image_bytes;      /* bytes of the device image                                      */
+  int64_t chunk_bytes;      /* shared-memory bytes of one staging buffer                      */
+  int64_t n_by_type[8];     /* elements per XT_* type id                                      */
+  int64_t sum_order;        /* sum of N over all multipoles                                   */
+  int64_t n_curved;         /* multipoles with hxl != 0                                       */
+  int64_t has_aperture;     /* 1 if any LimitRect / LimitEllipse                              */
+  double beta0, gamma0;     /* reference particle as derived by the packer                    */
+  double circumference;     /* sum of drift lengths [m]                                       */
+} xt_lattice_info;
+
+/* Step P: parse + validate the packed buffer, pre-scale the multipole
+ * coefficients, fold curvature into the dipole term, lay out 16-byte-aligned records in
+ * Horner order, cut them into TMA chunks and copy the image to the current CUDA device.
+ * The caller may free `packed` as soon as the call returns.  *out untouched on failure. */
+int xt_lattice_create(const void *packed, size_t nbytes, xt_lattice **out);
+int xt_lattice_destroy(xt_lattice *lat);
+int xt_lattice_get_info(const xt_lattice *lat, xt_lattice_info *info);
+/* s position (entrance) of every element; `out` is a HOST array of `cap` doubles; returns
+ * n_elements (>= 0) or a negative xt_status. */
+int64_t xt_lattice_s_table(const xt_lattice *lat, double *out, int64_t cap);
+
+/* Host-only form of step P for tests and tools (makes NO CUDA call): packs the image exactly
+ * as xt_lattice_create would upload it.  Copies min(image size, cap) bytes to `image` (HOST;
+ * may be NULL when cap == 0), fills *info if non-NULL, returns the image size in bytes or a
+ * negative xt_status. */
+int64_t xt_lattice_pack_host(const void *packed, size_t nbytes, void *image, size_t cap,
+                             xt_lattice_info *info);
+
+/* Steps L, S, D, M1-M4, A, T, W (+ C when compaction is active): track every particle with
+ * state == 1 for n_turns turns through the whole line.  DEVICE pointers.
+ * On (stream-ordered) return the arrays are in their ORIGINAL order even if the alive
+ * particles were compacted internally.  n_part == 0 or n_turns == 0 is a successful no-op.
+ * Calling it again continues the run. */
+int xt_track(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
+             void *cuda_stream);
+int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
+                void *cuda_stream, const xt_track_opts *opts);
+
+/* End-to-end variant: the SAME call with HOST arrays.  Copies the ensemble to the device
+ * (stream-ordered allocation), tracks, copies everything back and synchronises the stream.
+ * Pinned host memory makes the copies asynchronous; pageable memory also works. */
+int xt_track_host(const xt_lattice *lat, const xt_particles *host_p, int64_t n_part,
+                  int64_t n_turns, void *cuda_stream, const xt_track_opts *opts);
+
+/* Init helper: delta -> ptau, rpp, rvv for n particles (DEVICE). */
+int xt_particles_init_derived(const xt_lattice *lat, const xt_particles *p, int64_t n_part,
+                              void *cuda_stream);
+
+/* Step H: survival-turn histogram (BASELINE.json configs[4]).  hist (DEVICE, int64[n_bins+1])
+ * is OVERWRITTEN: hist[b] = #{state == 0 and bin_width*b <= at_turn < bin_width*(b+1)},
+ * lost particles with at_turn beyond the last bin go to bin n_bins-1, and
+ * hist[n_bins] = #{state == 1} (survivors). */
+int xt_survival_histogram(const int64_t *at_turn, const int64_t *state, int64_t n_part,
+                          int64_t bin_width, int64_t n_bins, int64_t *hist, void *cuda_stream);
+
+/* FP64 FMA microbenchmark (roofline denominator, north_star: "measured by an FMA
+ * microbenchmark in the same run"): runs a register-resident DFMA kernel on the whole chip,
+ * times it with CUDA events on `cuda_stream`, synchronises, and returns FLOP/s (2 per FMA)
+ * in *flops_per_s and the kernel time in *ms (either may be NULL). */
+int xt_fp64_fma_peak(double *flops_per_s, double *ms, void *cuda_stream);
+
+/* Number of kernels the library has launched from this process so far (bench bookkeeping). */
+int64_t xt_launch_count(void);
+
+const char *xt_last_error(void); /* thread-local, never NULL */
+const char *xt_build_info(void); /* e.g. "sm_100a fmad=true" / "sm_100a fmad=false"          */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XT_H_ */

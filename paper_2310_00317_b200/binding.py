@@ -1,0 +1,302 @@
+"""Thin ctypes binding of ``include/xt.h`` -- argument marshalling only.
+
+Every step of the tracking path runs inside ``libxt_b200.so`` (hand-written CUDA for
+sm_100a).  PyTorch is used for device memory and streams, nothing else.  There is no CPU
+fallback: if the library is missing it is built with nvcc, and if that fails, or no CUDA
+device is present when a compute entry point is called, an exception is raised.
+
+The functions carry the names of the C entry points they wrap.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Dict, Optional
+
+import numpy as np
+
+from . import _build
+
+F64_FIELDS = ("x", "px", "y", "py", "zeta", "delta", "ptau", "rpp", "rvv", "s")
+I64_FIELDS = ("at_turn", "state", "particle_id", "at_element")
+ALL_FIELDS = F64_FIELDS + I64_FIELDS
+
+XT_OK, XT_ERR_INVALID_ARG, XT_ERR_BAD_LATTICE, XT_ERR_CUDA, XT_ERR_NOMEM = 0, -1, -2, -3, -4
+
+
+class XtError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__("xt error %d: %s" % (code, msg))
+        self.code = code
+
+
+class xt_particles(ctypes.Structure):
+    _fields_ = ([(k, ctypes.c_void_p) for k in F64_FIELDS] + [(k, ctypes.c_void_p) for k in I64_FIELDS])
+
+
+class xt_track_opts(ctypes.Structure):
+    _fields_ = [("turns_per_launch", ctypes.c_int64), ("compact_every", ctypes.c_int64),
+                ("block_size", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+class xt_lattice_info(ctypes.Structure):
+    _fields_ = [("n_elements", ctypes.c_int64), ("n_records", ctypes.c_int64),
+                ("n_chunks", ctypes.c_int64), ("image_bytes", ctypes.c_int64),
+                ("chunk_bytes", ctypes.c_int64), ("n_by_type", ctypes.c_int64 * 8),
+                ("sum_order", ctypes.c_int64), ("n_curved", ctypes.c_int64),
+                ("has_aperture", ctypes.c_int64), ("beta0", ctypes.c_double),
+                ("gamma0", ctypes.c_double), ("circumference", ctypes.c_double)]
+
+    def as_dict(self) -> Dict:
+        d = {k: getattr(self, k) for k, _ in self._fields_ if k != "n_by_type"}
+        d["n_by_type"] = list(self.n_by_type)
+        return d
+
+
+# name -> (restype, argtypes): every symbol include/xt.h declares
+_VP, _I64, _SZ = ctypes.c_void_p, ctypes.c_int64, ctypes.c_size_t
+SIGNATURES = {
+    "xt_lattice_create": (ctypes.c_int, [ctypes.c_char_p, _SZ, ctypes.POINTER(_VP)]),
+    "xt_lattice_destroy": (ctypes.c_int, [_VP]),
+    "xt_lattice_get_info": (ctypes.c_int, [_VP, ctypes.POINTER(xt_lattice_info)]),
+    "xt_lattice_s_table": (_I64, [_VP, _VP, _I64]),
+    "xt_lattice_pack_host": (_I64, [ctypes.c_char_p, _SZ, _VP, _SZ, ctypes.POINTER(xt_lattice_info)]),
+    "xt_track": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _VP]),
+    "xt_track_ex": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _VP,
+                                   ctypes.POINTER(xt_track_opts)]),
+    "xt_track_host": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _VP,
+                                     ctypes.POINTER(xt_track_opts)]),
+    "xt_particles_init_derived": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _VP]),
+    "xt_survival_histogram": (ctypes.c_int, [_VP, _VP, _I64, _I64, _I64, _VP, _VP]),
+    "xt_fp64_fma_peak": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), _VP]),
+    "xt_launch_count": (_I64, []),
+    "xt_last_error": (ctypes.c_char_p, []),
+    "xt_build_info": (ctypes.c_char_p, []),
+}
+
+_libs: Dict[str, ctypes.CDLL] = {}
+
+
+def load_library(kind: str = "prod") -> ctypes.CDLL:
+    """Load (building first if stale/missing) ``libxt_b200.so`` (kind='prod') or the
+    ``--fmad=false`` validation build (kind='nofma').  Fails loudly; no fallback."""
+    if kind not in _libs:
+        _build.build(kinds=(kind,))
+        path = _build.LIBS[kind]["path"]
+        if not os.path.exists(path):
+            raise RuntimeError("CUDA extension %s is missing and could not be built" % path)
+        lib = ctypes.CDLL(path)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)        # AttributeError if the symbol is not exported
+            fn.restype, fn.argtypes = res, args
+        _libs[kind] = lib
+    return _libs[kind]
+
+
+def _check(lib, rc: int) -> None:
+    if rc != XT_OK:
+        raise XtError(rc, lib.xt_last_error().decode("utf-8", "replace"))
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(int(stream.cuda_stream))
+
+
+# ------------------------------------------------------------------------------ lattice
+class Lattice:
+    """Owner of an ``xt_lattice*`` (device image of a beam line)."""
+
+    def __init__(self, handle: int, lib: ctypes.CDLL, kind: str):
+        self._h, self._lib, self.kind = handle, lib, kind
+        info = xt_lattice_info()
+        _check(lib, lib.xt_lattice_get_info(_VP(handle), ctypes.byref(info)))
+        self.info = info.as_dict()
+
+    @property
+    def handle(self) -> ctypes.c_void_p:
+        if not self._h:
+            raise ValueError("lattice already destroyed")
+        return _VP(self._h)
+
+    def close(self) -> None:
+        if self._h:
+            self._lib.xt_lattice_destroy(_VP(self._h))
+            self._h = 0
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def xt_lattice_create(packed: bytes, kind: str = "prod") -> Lattice:
+    lib = load_library(kind)
+    out = _VP()
+    _check(lib, lib.xt_lattice_create(packed, len(packed), ctypes.byref(out)))
+    return Lattice(out.value, lib, kind)
+
+
+def xt_lattice_destroy(lat: Lattice) -> None:
+    lat.close()
+
+
+def xt_lattice_get_info(lat: Lattice) -> Dict:
+    return dict(lat.info)
+
+
+def xt_lattice_s_table(lat: Lattice) -> np.ndarray:
+    n = lat._lib.xt_lattice_s_table(lat.handle, None, 0)
+    if n < 0:
+        _check(lat._lib, int(n))
+    out = np.zeros(n, dtype=np.float64)
+    lat._lib.xt_lattice_s_table(lat.handle, out.ctypes.data_as(_VP), n)
+    return out
+
+
+def xt_lattice_pack_host(packed: bytes, kind: str = "prod"):
+    """(image bytes, info dict) of the device image; makes no CUDA call."""
+    lib = load_library(kind)
+    info = xt_lattice_info()
+    n = lib.xt_lattice_pack_host(packed, len(packed), None, 0, ctypes.byref(info))
+    if n < 0:
+        _check(lib, int(n))
+    buf = ctypes.create_string_buffer(int(n))
+    lib.xt_lattice_pack_host(packed, len(packed), buf, int(n), ctypes.byref(info))
+    return buf.raw, info.as_dict()
+
+
+# ---------------------------------------------------------------------------- particles
+def _struct_from_tensors(p: Dict) -> xt_particles:
+    st = xt_particles()
+    n = None
+    for k in ALL_FIELDS:
+        t = p.get(k)
+        if t is None:
+            setattr(st, k, None)
+            continue
+        import torch
+        want = torch.float64 if k in F64_FIELDS else torch.int64
+        if not (t.is_cuda and t.dtype == want and t.is_contiguous() and t.dim() == 1):
+            raise ValueError("particle array %r must be a contiguous 1-D CUDA %s tensor" % (k, want))
+        if n is None:
+            n = t.numel()
+        elif t.numel() != n:
+            raise ValueError("particle array %r has a different length" % k)
+        setattr(st, k, t.data_ptr())
+    return st
+
+
+def _struct_from_numpy(p: Dict) -> xt_particles:
+    st = xt_particles()
+    for k in ALL_FIELDS:
+        a = p.get(k)
+        if a is None:
+            setattr(st, k, None)
+            continue
+        if hasattr(a, "data_ptr"):          # pinned torch CPU tensor
+            if a.is_cuda or not a.is_contiguous():
+                raise ValueError("host array %r must be a contiguous CPU tensor" % k)
+            setattr(st, k, a.data_ptr())
+        else:
+            want = np.float64 if k in F64_FIELDS else np.int64
+            if not (a.dtype == want and a.flags.c_contiguous and a.ndim == 1):
+                raise ValueError("host array %r must be a contiguous 1-D %s array" % (k, want))
+            setattr(st, k, a.ctypes.data)
+    return st
+
+
+def new_particles(lat: Lattice, coords: Dict[str, np.ndarray], device="cuda", stream=None) -> Dict:
+    """Device SoA (dict of torch tensors) from the six primary coordinates; the derived
+    ptau, rpp, rvv come from the library's own kernel (``xt_particles_init_derived``)."""
+    import torch
+    n = len(coords["x"])
+    p = {}
+    for k in ("x", "px", "y", "py", "zeta", "delta"):
+        p[k] = torch.from_numpy(np.ascontiguousarray(coords[k], dtype=np.float64)).to(device)
+    for k in ("ptau", "rpp", "rvv", "s"):
+        p[k] = torch.zeros(n, dtype=torch.float64, device=device)
+    p["at_turn"] = torch.zeros(n, dtype=torch.int64, device=device)
+    p["state"] = torch.ones(n, dtype=torch.int64, device=device)
+    p["at_element"] = torch.zeros(n, dtype=torch.int64, device=device)
+    xt_particles_init_derived(lat, p, stream=stream)
+    return p
+
+
+def particles_to_device(p_host: Dict[str, np.ndarray], device="cuda") -> Dict:
+    import torch
+    return {k: torch.from_numpy(np.ascontiguousarray(v)).to(device) for k, v in p_host.items()
+            if k in ALL_FIELDS}
+
+
+def particles_to_host(p: Dict) -> Dict[str, np.ndarray]:
+    return {k: v.cpu().numpy() for k, v in p.items()}
+
+
+def _n_part(p: Dict) -> int:
+    return int(p["x"].shape[0])
+
+
+def _opts(turns_per_launch=0, compact_every=0, block_size=0):
+    if not (turns_per_launch or compact_every or block_size):
+        return None
+    return xt_track_opts(int(turns_per_launch), int(compact_every), int(block_size), 0)
+
+
+def xt_particles_init_derived(lat: Lattice, p: Dict, stream=None) -> None:
+    st = _struct_from_tensors(p)
+    _check(lat._lib, lat._lib.xt_particles_init_derived(lat.handle, ctypes.byref(st), _n_part(p),
+                                                        _stream_ptr(stream)))
+
+
+def xt_track(lat: Lattice, p: Dict, n_turns: int, stream=None) -> None:
+    """Track the device SoA ``p`` in place for ``n_turns`` turns (asynchronous on ``stream``)."""
+    st = _struct_from_tensors(p)
+    _check(lat._lib, lat._lib.xt_track(lat.handle, ctypes.byref(st), _n_part(p), int(n_turns),
+                                       _stream_ptr(stream)))
+
+
+def xt_track_ex(lat: Lattice, p: Dict, n_turns: int, stream=None, *, turns_per_launch: int = 0,
+                compact_every: int = 0, block_size: int = 0) -> None:
+    st = _struct_from_tensors(p)
+    o = _opts(turns_per_launch, compact_every, block_size)
+    _check(lat._lib, lat._lib.xt_track_ex(lat.handle, ctypes.byref(st), _n_part(p), int(n_turns),
+                                          _stream_ptr(stream), ctypes.byref(o) if o else None))
+
+
+def xt_track_host(lat: Lattice, p_host: Dict, n_turns: int, stream=None, *, turns_per_launch: int = 0,
+                  compact_every: int = 0, block_size: int = 0) -> None:
+    """End to end with HOST arrays (numpy or pinned torch CPU tensors): H2D, track, D2H, sync."""
+    st = _struct_from_numpy(p_host)
+    o = _opts(turns_per_launch, compact_every, block_size)
+    _check(lat._lib, lat._lib.xt_track_host(lat.handle, ctypes.byref(st), _n_part(p_host), int(n_turns),
+                                            _stream_ptr(stream), ctypes.byref(o) if o else None))
+
+
+def xt_survival_histogram(p: Dict, bin_width: int, n_bins: int, stream=None, kind: str = "prod"):
+    """int64[n_bins+1] device tensor: lost-turn histogram, last entry = survivors."""
+    import torch
+    lib = load_library(kind)
+    hist = torch.empty(n_bins + 1, dtype=torch.int64, device=p["state"].device)
+    _check(lib, lib.xt_survival_histogram(p["at_turn"].data_ptr(), p["state"].data_ptr(), _n_part(p),
+                                          int(bin_width), int(n_bins), hist.data_ptr(), _stream_ptr(stream)))
+    return hist
+
+
+def xt_fp64_fma_peak(stream=None, kind: str = "prod"):
+    """(FLOP/s, kernel ms) of the library's FP64 FMA microbenchmark on the current device."""
+    lib = load_library(kind)
+    f, ms = ctypes.c_double(), ctypes.c_double()
+    _check(lib, lib.xt_fp64_fma_peak(ctypes.byref(f), ctypes.byref(ms), _stream_ptr(stream)))
+    return f.value, ms.value
+
+
+def xt_launch_count(kind: str = "prod") -> int:
+    return int(load_library(kind).xt_launch_count())
+
+
+def xt_build_info(kind: str = "prod") -> str:
+    return load_library(kind).xt_build_info().decode()

@@ -1,0 +1,213 @@
+// C-ABI entry points that orchestrate the kernels (include/xt.h): xt_track / xt_track_ex
+// (launch chunking + periodic compaction), xt_track_host (end-to-end with host buffers),
+// the init helper, the survival histogram, the FMA microbenchmark and error reporting.
+#include <atomic>
+#include <string>
+
+#include "xt_internal.h"
+
+namespace xt {
+namespace {
+thread_local std::string g_error;
+std::atomic<int64_t> g_launches{0};
+}  // namespace
+
+void set_error(const std::string &msg) { g_error = msg; }
+
+int cuda_fail(cudaError_t e, const char *what) {
+  g_error = std::string(what) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")";
+  return e == cudaErrorMemoryAllocation ? XT_ERR_NOMEM : XT_ERR_CUDA;
+}
+
+void count_launch(int64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+namespace {
+
+int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p, int64_t n_part) {
+  if (!lat || !p || n_part < 0) {
+    set_error(std::string(fn) + ": NULL lattice/particles or negative n_part");
+    return XT_ERR_INVALID_ARG;
+  }
+  if (n_part > 0 && (!p->x || !p->px || !p->y || !p->py || !p->zeta || !p->delta || !p->ptau || !p->rpp ||
+                     !p->rvv || !p->s || !p->at_turn || !p->state)) {
+    set_error(std::string(fn) + ": a required particle array is NULL (only particle_id, at_element may be)");
+    return XT_ERR_INVALID_ARG;
+  }
+  return XT_OK;
+}
+
+int resolve_block(const xt_track_opts *o, int *block) {
+  *block = (o && o->block_size) ? o->block_size : 128;
+  if (*block < 32 || *block > 512 || (*block % 32) != 0) {
+    set_error("xt_track_ex: block_size must be a multiple of 32 in [32, 512]");
+    return XT_ERR_INVALID_ARG;
+  }
+  return XT_OK;
+}
+
+}  // namespace
+}  // namespace xt
+
+extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
+                           void *cuda_stream, const xt_track_opts *opts) {
+  int rc = xt::check_particles("xt_track", lat, p, n_part);
+  if (rc != XT_OK) return rc;
+  if (n_turns < 0) {
+    xt::set_error("xt_track: negative n_turns");
+    return XT_ERR_INVALID_ARG;
+  }
+  int block = 0;
+  if ((rc = xt::resolve_block(opts, &block)) != XT_OK) return rc;
+  if (opts && opts->turns_per_launch < 0) {
+    xt::set_error("xt_track_ex: negative turns_per_launch");
+    return XT_ERR_INVALID_ARG;
+  }
+  if (n_part == 0 || n_turns == 0) return XT_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+
+  // compaction period (step C): only lattices with apertures can lose particles
+  int64_t period = 0;
+  const int64_t want = opts ? opts->compact_every : 0;
+  if (lat->info.has_aperture && want >= 0) {
+    const int64_t pr = want > 0 ? want : 1000;
+    if (n_turns > pr) period = pr;
+  }
+  const int64_t tpl_opt = opts ? opts->turns_per_launch : 0;
+
+  if (period == 0) {
+    const int64_t tpl = tpl_opt > 0 ? tpl_opt : n_turns;
+    for (int64_t done = 0; done < n_turns;) {
+      const int64_t k = (n_turns - done < tpl) ? n_turns - done : tpl;
+      if ((rc = xt::launch_track(lat, *p, n_part, nullptr, k, block, st)) != XT_OK) return rc;
+      done += k;
+    }
+    return XT_OK;
+  }
+
+  void *ws = nullptr;
+  const size_t ws_bytes = xt::compaction_workspace_bytes(n_part);
+  XT_CUDA(cudaMallocAsync(&ws, ws_bytes, st));
+  xt::CompactPlan plan;
+  xt::plan_compaction(ws, n_part, plan);
+  auto bail = [&](int code) {
+    cudaFreeAsync(ws, st);
+    return code;
+  };
+  // initial partition: alive particles of the caller's arrays -> working set 0
+  if ((rc = xt::launch_partition(plan, *p, nullptr, true, n_part, plan.w[0], *p, st)) != XT_OK) return bail(rc);
+  int cur = 0;
+  const int64_t tpl = (tpl_opt > 0 && tpl_opt < period) ? tpl_opt : period;
+  int64_t since = 0;
+  for (int64_t done = 0; done < n_turns;) {
+    int64_t k = n_turns - done;
+    if (k > tpl) k = tpl;
+    if (k > period - since) k = period - since;
+    if ((rc = xt::launch_track(lat, plan.w[cur].p, n_part, plan.n_active, k, block, st)) != XT_OK) return bail(rc);
+    done += k;
+    since += k;
+    if (since == period && done < n_turns) {
+      if ((rc = xt::launch_partition(plan, plan.w[cur].p, plan.w[cur].origin, false, n_part, plan.w[1 - cur], *p,
+                                     st)) != XT_OK)
+        return bail(rc);
+      cur = 1 - cur;
+      since = 0;
+    }
+  }
+  if ((rc = xt::launch_scatter_back(plan, plan.w[cur], n_part, *p, st)) != XT_OK) return bail(rc);
+  XT_CUDA(cudaFreeAsync(ws, st));
+  return XT_OK;
+}
+
+extern "C" int xt_track(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
+                        void *cuda_stream) {
+  return xt_track_ex(lat, p, n_part, n_turns, cuda_stream, nullptr);
+}
+
+extern "C" int xt_track_host(const xt_lattice *lat, const xt_particles *hp, int64_t n_part, int64_t n_turns,
+                             void *cuda_stream, const xt_track_opts *opts) {
+  int rc = xt::check_particles("xt_track_host", lat, hp, n_part);
+  if (rc != XT_OK) return rc;
+  if (n_turns < 0) {
+    xt::set_error("xt_track_host: negative n_turns");
+    return XT_ERR_INVALID_ARG;
+  }
+  if (n_part == 0 || n_turns == 0) return XT_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const size_t arr = (static_cast<size_t>(n_part) * 8 + 255) & ~static_cast<size_t>(255);
+  const int n_arr = 13;
+  unsigned char *buf = nullptr;
+  XT_CUDA(cudaMallocAsync(reinterpret_cast<void **>(&buf), arr * n_arr, st));
+  void *host[13] = {hp->x,   hp->px,  hp->y, hp->py,      hp->zeta,  hp->delta,     hp->ptau,
+                    hp->rpp, hp->rvv, hp->s, hp->at_turn, hp->state, hp->at_element};
+  void *dev[13];
+  for (int k = 0; k < n_arr; ++k) dev[k] = buf + arr * k;
+  auto bail = [&](int code) {
+    cudaFreeAsync(buf, st);
+    return code;
+  };
+  for (int k = 0; k < n_arr; ++k) {
+    if (!host[k]) continue;  // at_element is optional
+    cudaError_t e = cudaMemcpyAsync(dev[k], host[k], static_cast<size_t>(n_part) * 8, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return bail(xt::cuda_fail(e, "cudaMemcpyAsync(H2D)"));
+  }
+  xt_particles dp{};
+  dp.x = static_cast<double *>(dev[0]);
+  dp.px = static_cast<double *>(dev[1]);
+  dp.y = static_cast<double *>(dev[2]);
+  dp.py = static_cast<double *>(dev[3]);
+  dp.zeta = static_cast<double *>(dev[4]);
+  dp.delta = static_cast<double *>(dev[5]);
+  dp.ptau = static_cast<double *>(dev[6]);
+  dp.rpp = static_cast<double *>(dev[7]);
+  dp.rvv = static_cast<double *>(dev[8]);
+  dp.s = static_cast<double *>(dev[9]);
+  dp.at_turn = static_cast<int64_t *>(dev[10]);
+  dp.state = static_cast<int64_t *>(dev[11]);
+  dp.at_element = hp->at_element ? static_cast<int64_t *>(dev[12]) : nullptr;
+  dp.particle_id = nullptr;
+  if ((rc = xt_track_ex(lat, &dp, n_part, n_turns, cuda_stream, opts)) != XT_OK) return bail(rc);
+  for (int k = 0; k < n_arr; ++k) {
+    if (!host[k]) continue;
+    cudaError_t e = cudaMemcpyAsync(host[k], dev[k], static_cast<size_t>(n_part) * 8, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return bail(xt::cuda_fail(e, "cudaMemcpyAsync(D2H)"));
+  }
+  XT_CUDA(cudaFreeAsync(buf, st));
+  XT_CUDA(cudaStreamSynchronize(st));
+  return XT_OK;
+}
+
+extern "C" int xt_particles_init_derived(const xt_lattice *lat, const xt_particles *p, int64_t n_part,
+                                         void *cuda_stream) {
+  if (!lat || !p || n_part < 0 || (n_part > 0 && (!p->delta || !p->ptau || !p->rpp || !p->rvv))) {
+    xt::set_error("xt_particles_init_derived: NULL argument or negative n_part");
+    return XT_ERR_INVALID_ARG;
+  }
+  return xt::launch_init_derived(lat, *p, n_part, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int xt_survival_histogram(const int64_t *at_turn, const int64_t *state, int64_t n_part,
+                                     int64_t bin_width, int64_t n_bins, int64_t *hist, void *cuda_stream) {
+  if (!hist || n_part < 0 || bin_width <= 0 || n_bins <= 0 || n_bins > 8192 ||
+      (n_part > 0 && (!at_turn || !state))) {
+    xt::set_error("xt_survival_histogram: invalid argument (need bin_width > 0, 0 < n_bins <= 8192)");
+    return XT_ERR_INVALID_ARG;
+  }
+  return xt::launch_histogram(at_turn, state, n_part, bin_width, n_bins, hist,
+                              static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int xt_fp64_fma_peak(double *flops_per_s, double *ms, void *cuda_stream) {
+  return xt::run_fma_peak(flops_per_s, ms, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int64_t xt_launch_count(void) { return xt::g_launches.load(std::memory_order_relaxed); }
+
+extern "C" const char *xt_last_error(void) { return xt::g_error.c_str(); }
+
+extern "C" const char *xt_build_info(void) {
+#ifdef XT_FMAD_OFF
+  return "libxt_b200 sm_100a fmad=false (validation build)";
+#else
+  return "libxt_b200 sm_100a fmad=true";
+#endif
+}

@@ -1,0 +1,133 @@
+// Internal declarations shared by the translation units of libxt_b200 (never installed,
+// never seen by the oracle).  Public contract: include/xt.h.
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstddef>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/xt.h"
+
+namespace xt {
+
+// ------------------------------------------------------------------ device lattice image
+// The image is a byte stream of 16-byte-aligned records, cut into chunks of at most
+// chunk_bytes; every chunk ends with a TAG_END record so that the kernel's element loop
+// needs no counter.  Record = 16-byte header {u32 tag; u32 elem; f64 p0} + 16-byte slots:
+//
+//   TAG_DRIFT    p0 = length                                                     16 B
+//   TAG_MULT     p0 unused; (c[n], s[n]) pairs, n = N .. 0 (Horner order)        16 + 16(N+1)
+//   TAG_CMULT    p0 = hxl;  {wf, 0};  pairs as above (c[0] = knl[0] - hxl)       32 + 16(N+1)
+//   TAG_CAVITY   p0 = lag_rad; {kz, vn}                                          32 B
+//   TAG_SROT     p0 unused; {cos_z, sin_z}                                       32 B
+//   TAG_SHIFT    p0 unused; {dx, dy}                                             32 B
+//   TAG_RECT     p0 unused; {min_x, max_x}; {min_y, max_y}                       48 B
+//   TAG_ELLIPSE  p0 = a2*b2; {b2, a2}                                            32 B
+//   TAG_END      end of chunk                                                    16 B
+//
+// tag = type | (order << 8); elem = index of the element in the user's packed buffer.
+enum : uint32_t {
+  TAG_END = 0,
+  TAG_DRIFT = 1,
+  TAG_MULT = 2,
+  TAG_CAVITY = 3,
+  TAG_SROT = 4,
+  TAG_SHIFT = 5,
+  TAG_RECT = 6,
+  TAG_ELLIPSE = 7,
+  TAG_CMULT = 8
+};
+
+struct alignas(16) RecHdr {
+  uint32_t tag;
+  uint32_t elem;
+  double p0;
+};
+static_assert(sizeof(RecHdr) == 16, "record header must be one 16-byte slot");
+
+struct alignas(16) ChunkDesc {
+  uint64_t offset;  // byte offset into the image (multiple of 16)
+  uint32_t nbytes;  // multiple of 16, <= chunk_bytes, includes the TAG_END record
+  uint32_t pad;
+};
+
+struct RefConsts {
+  double beta0;  // p0c / E0
+  double tib;    // 2 / beta0
+  double igam2;  // 1 / gamma0^2
+  double ib;     // 1 / beta0
+  double ib2;    // ib * ib
+};
+
+constexpr uint32_t kDefaultChunkBytes = 16384;
+
+}  // namespace xt
+
+struct xt_lattice {
+  xt_lattice_info info{};
+  xt::RefConsts k{};
+  int device = -1;
+  std::vector<double> s_table_host;
+  unsigned char *d_image = nullptr;
+  xt::ChunkDesc *d_chunks = nullptr;
+  double *d_s_table = nullptr;
+};
+
+namespace xt {
+
+// xt_api.cu
+void set_error(const std::string &msg);
+int cuda_fail(cudaError_t e, const char *what);
+void count_launch(int64_t n = 1);
+#define XT_CUDA(call)                                      \
+  do {                                                     \
+    cudaError_t e__ = (call);                              \
+    if (e__ != cudaSuccess) return xt::cuda_fail(e__, #call); \
+  } while (0)
+
+// xt_lattice.cu: host packer (step P).  Builds the image bytes, chunk table, s table.
+struct HostImage {
+  std::vector<unsigned char> image;
+  std::vector<ChunkDesc> chunks;
+  std::vector<double> s_table;
+  xt_lattice_info info{};
+  RefConsts k{};
+};
+int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImage &out);
+
+// xt_track.cu
+int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part,
+                 const int64_t *d_n_active, int64_t n_turns, int block, cudaStream_t st);
+int launch_init_derived(const xt_lattice *lat, const xt_particles &p, int64_t n, cudaStream_t st);
+
+// xt_compact.cu (step C) -- SoA working set with an origin index
+struct WorkSet {
+  xt_particles p{};            // 10 f64 + at_turn, state, at_element (particle_id unused)
+  int64_t *origin = nullptr;   // index in the caller's arrays
+};
+size_t compaction_workspace_bytes(int64_t n_part);
+// Carves two WorkSets + counters + tile scratch out of `ws` (256-byte aligned pieces).
+struct CompactPlan {
+  WorkSet w[2];
+  int64_t *n_active = nullptr;   // device counter
+  int64_t *tile_counts = nullptr;
+  int64_t n_tiles = 0;
+};
+void plan_compaction(void *ws, int64_t n_part, CompactPlan &plan);
+// dst <- alive entries of src (stable); lost entries of src are written to `user` at their
+// origin unless src_is_user.  n_src read from plan.n_active unless src_is_user (then n_part).
+int launch_partition(const CompactPlan &plan, const xt_particles &src, const int64_t *src_origin,
+                     bool src_is_user, int64_t n_part, const WorkSet &dst, const xt_particles &user,
+                     cudaStream_t st);
+int launch_scatter_back(const CompactPlan &plan, const WorkSet &src, int64_t n_part,
+                        const xt_particles &user, cudaStream_t st);
+int launch_histogram(const int64_t *at_turn, const int64_t *state, int64_t n, int64_t bin_width,
+                     int64_t n_bins, int64_t *hist, cudaStream_t st);
+
+// xt_peak.cu
+int run_fma_peak(double *flops_per_s, double *ms, cudaStream_t st);
+
+}  // namespace xt

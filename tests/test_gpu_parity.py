@@ -1,0 +1,420 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU
+oracle on identical seeded inputs.
+
+Tolerances (BASELINE.json north_star, reading A8): per coordinate
+|gpu - ref| <= max(rtol*|ref|, 1e-15) with rtol = 1e-12 after 1 turn and 1e-10 after
+100 turns (stable particles, reading A9); lost flags / at_turn / at_element exact except
+for particles within 1e-9 m of an aperture edge (A3); bit-exact in the --fmad=false
+validation build on cavity-stripped lattices (A10).
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from xt_inputs import configs as C
+from xt_inputs.packed import (Cavity, Drift, LimitEllipse, LimitRect, Marker, Multipole,
+                              SRotation, XYShift, pack_lattice)
+import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+FLOAT_KEYS = ("x", "px", "y", "py", "zeta", "delta", "ptau", "rpp", "rvv")
+INT_KEYS = ("at_turn", "state", "at_element")
+ATOL = 1e-15
+THREADS = O.host_threads()
+
+
+@pytest.fixture(scope="module")
+def X():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (run with -m gpu on the B200 box)")
+    import paper_2310_00317_b200 as X
+    return X
+
+
+_buf_cache = {}
+
+
+def packed(cfg, strip=False):
+    key = (cfg, strip)
+    if key not in _buf_cache:
+        els = C.lattice(cfg)
+        if strip:
+            els = C.strip_cavities(els)
+        _buf_cache[key] = C.pack(els)
+    return _buf_cache[key]
+
+
+def run_both(X, buf, coords, n_turns, kind="prod", margin=False, **opts):
+    """-> (gpu result dict of numpy, oracle result dict, min_margin or None)."""
+    ref = O.new_particles(buf, coords)
+    mm = np.full(len(ref["x"]), np.inf) if margin else None
+    O.track(buf, ref, n_turns, threads=THREADS, min_margin=mm)
+    lat = X.xt_lattice_create(buf, kind=kind)
+    p = X.new_particles(lat, coords)
+    if opts:
+        X.xt_track_ex(lat, p, n_turns, **opts)
+    else:
+        X.xt_track(lat, p, n_turns)
+    got = X.particles_to_host(p)
+    lat.close()
+    return got, ref, mm
+
+
+def assert_close(got, ref, rtol, sel=None, keys=FLOAT_KEYS):
+    for k in keys:
+        a, r = got[k], ref[k]
+        if sel is not None:
+            a, r = a[sel], r[sel]
+        ok = H.within(a, r, rtol, ATOL)
+        if not ok.all():
+            j = int(np.argmin(ok))
+            raise AssertionError("%s: %d/%d outside tolerance; first %d gpu=%r ref=%r" %
+                                 (k, int((~ok).sum()), len(ok), j, a[j], r[j]))
+
+
+def assert_bit_identical(got, ref, keys=FLOAT_KEYS + ("s",) + INT_KEYS):
+    for k in keys:
+        a, r = got[k], ref[k]
+        if a.dtype == np.float64:
+            same = (a.view(np.int64) == r.view(np.int64)) | (np.isnan(a) & np.isnan(r))
+        else:
+            same = a == r
+        if not same.all():
+            j = int(np.argmin(same))
+            raise AssertionError("%s: %d/%d differ bitwise; first %d gpu=%r ref=%r" %
+                                 (k, int((~same).sum()), len(same), j, a[j], r[j]))
+
+
+def assert_losses_match(got, ref, mm):
+    """Loss records are integers: exact, except within 1e-9 m of an aperture edge (A3)."""
+    clear = mm >= 1e-9
+    for k in INT_KEYS:
+        bad = (got[k] != ref[k]) & clear
+        assert not bad.any(), (k, int(bad.sum()), int(np.argmax(bad)))
+    lost = clear & (ref["state"] == 0)
+    assert np.array_equal(got["s"][lost], ref["s"][lost])
+    return clear
+
+
+# ----------------------------------------------------------------- init helper, lattice
+def test_init_derived_and_s_table(X):
+    buf = packed(3)
+    coords = C.subsample(C.particles_cfg3(n=5000), slice(None))
+    ref = O.new_particles(buf, coords)
+    lat = X.xt_lattice_create(buf)
+    p = X.particles_to_host(X.new_particles(lat, coords))
+    assert_close(p, ref, 4e-16, keys=("ptau", "rpp", "rvv"))
+    assert np.array_equal(X.xt_lattice_s_table(lat), O.s_table(buf))
+    b0, g0 = O.reference(buf)
+    assert lat.info["beta0"] == b0 and lat.info["gamma0"] == g0
+    lat.close()
+    latv = X.xt_lattice_create(buf, kind="nofma")
+    pv = X.particles_to_host(X.new_particles(latv, coords))
+    assert_bit_identical(pv, ref, keys=("ptau", "rpp", "rvv"))
+    latv.close()
+
+
+# ------------------------------------------------------------------------------ config 0
+def test_cfg0_one_turn(X):
+    got, ref, _ = run_both(X, packed(0), C.particles(0), 1)
+    assert_close(got, ref, 1e-12)
+    assert np.array_equal(got["at_turn"], ref["at_turn"]) and (got["state"] == 1).all()
+    assert (got["s"] == 0).all()
+
+
+def test_cfg0_100_turns(X):
+    got, ref, _ = run_both(X, packed(0), C.particles(0), 100)
+    assert_close(got, ref, 1e-10)
+    assert (got["at_turn"] == 100).all()
+
+
+# --------------------------------------------------------------- worked examples (golden)
+def test_worked_examples_every_element_type(X):
+    g = H.load_golden()
+    for line in g["lines"]:
+        els = [H.element_from_json(d) for d in line["elements"]]
+        buf = pack_lattice(els, H.P0C, H.MASS0, H.Q0)
+        start = [H.unhex(v) for v in line["start"]]
+        got, ref, _ = run_both(X, buf, H.coords_from_rows([start] * 33), 1)
+        assert_close(got, ref, 1e-12)
+        gotv, refv, _ = run_both(X, buf, H.coords_from_rows([start] * 33), 1, kind="nofma")
+        has_cav = any(isinstance(e, Cavity) for e in els)
+        if not has_cav:
+            assert_bit_identical(gotv, refv)
+        else:
+            assert_close(gotv, refv, 1e-14)
+
+
+# --------------------------------------------------------------------- bit-exact (A10)
+@pytest.mark.parametrize("cfg,n,turns", [(0, 1000, 100), (2, 3000, 3), (3, 3000, 2), (4, 3000, 2)])
+def test_bit_exact_nofma_cavity_stripped(X, cfg, n, turns):
+    full = C.particles(cfg, n=n) if cfg in (0, 2, 3) else C.particles(cfg)
+    if cfg == 4:
+        idx = np.linspace(0, len(full["x"]) - 1, n).astype(np.int64)
+        full = C.subsample(full, idx)
+    got, ref, _ = run_both(X, packed(cfg, strip=True), full, turns, kind="nofma")
+    assert_bit_identical(got, ref)
+
+
+def test_bit_exact_nofma_cfg1b_with_losses(X):
+    """Supplementary config[1b] (sigma_grid = 1e-3 m): the literal config[1] loses nothing."""
+    coords = C.subsample(C.particles_cfg1(sigma=1e-3), slice(0, None, 97))
+    got, ref, _ = run_both(X, packed(1, strip=True), coords, 600, kind="nofma")
+    assert (ref["state"] == 0).sum() > 1000 and (ref["state"] == 1).sum() > 1000
+    assert_bit_identical(got, ref)
+
+
+# ------------------------------------------------------------------------ configs 1, 1b
+def test_cfg1_literal_one_turn_and_100_turns(X):
+    coords = C.subsample(C.particles_cfg1(), slice(0, None, 50))        # 20 000 particles
+    got, ref, _ = run_both(X, packed(1), coords, 1)
+    assert_close(got, ref, 1e-12)
+    got, ref, mm = run_both(X, packed(1), coords, 100, margin=True)
+    assert (ref["state"] == 1).all()
+    assert_losses_match(got, ref, mm)
+    assert_close(got, ref, 1e-10)
+
+
+def test_cfg1b_losses_first_100_turns(X):
+    coords = C.subsample(C.particles_cfg1(sigma=1e-3), slice(0, None, 50))
+    got, ref, mm = run_both(X, packed(1), coords, 100, margin=True)
+    assert (ref["state"] == 0).sum() > 5000
+    clear = assert_losses_match(got, ref, mm)
+    # coordinates of lost particles are those AT the aperture; compare all clear particles
+    # that the FMA-contracted oracle build also reproduces (A9: numerically stable ones)
+    fma = O.new_particles(packed(1), coords, kind="fma")
+    O.track(packed(1), fma, 100, kind="fma", threads=THREADS)
+    stable = clear & (fma["state"] == ref["state"]) & (fma["at_turn"] == ref["at_turn"])
+    for k in ("x", "px", "y", "py"):
+        stable &= H.within(fma[k], ref[k], 1e-11, ATOL)
+    assert stable.sum() > 0.5 * len(stable)
+    assert_close(got, ref, 1e-10, sel=stable, keys=("x", "px", "y", "py", "zeta", "delta", "ptau"))
+
+
+# --------------------------------------------------------------------------- configs 2-4
+def test_cfg2_one_turn_all_particles(X):
+    got, ref, mm = run_both(X, packed(2), C.particles(2), 1, margin=True)
+    assert_losses_match(got, ref, mm)
+    assert_close(got, ref, 1e-12, sel=ref["state"] == 1)
+
+
+def _stable_mask(buf, coords, ref, mm, n_turns):
+    fma = O.new_particles(buf, coords, kind="fma")
+    O.track(buf, fma, n_turns, kind="fma", threads=THREADS)
+    stable = (ref["state"] == 1) & (fma["state"] == 1) & (mm >= 1e-9)
+    for k in ("x", "px", "y", "py", "zeta"):
+        stable &= H.within(fma[k], ref[k], 1e-11, ATOL)
+    return stable
+
+
+def test_cfg2_100_turns(X):
+    coords = C.subsample(C.particles(2), slice(0, None, 50))            # 2 000 particles
+    got, ref, mm = run_both(X, packed(2), coords, 100, margin=True)
+    assert_losses_match(got, ref, mm)
+    stable = _stable_mask(packed(2), coords, ref, mm, 100)
+    assert stable.sum() > 0.95 * len(stable), stable.sum()
+    assert_close(got, ref, 1e-10, sel=stable)
+
+
+def test_cfg3_one_turn_and_100_turns(X):
+    coords = C.particles(3, n=100_000)
+    got, ref, mm = run_both(X, packed(3), coords, 1, margin=True)
+    assert_losses_match(got, ref, mm)
+    assert_close(got, ref, 1e-12, sel=ref["state"] == 1)
+    sub = C.subsample(coords, slice(0, 1000))
+    got, ref, mm = run_both(X, packed(3), sub, 100, margin=True)
+    assert_losses_match(got, ref, mm)
+    stable = _stable_mask(packed(3), sub, ref, mm, 100)
+    assert stable.sum() > 0.9 * len(stable), stable.sum()
+    assert_close(got, ref, 1e-10, sel=stable)
+
+
+def test_cfg4_grid_losses_and_histogram(X):
+    full = C.particles(4)
+    idx = np.linspace(0, len(full["x"]) - 1, 6000).astype(np.int64)
+    coords = C.subsample(full, idx)
+    buf = packed(4)
+    got, ref, mm = run_both(X, buf, coords, 60, margin=True, compact_every=20)
+    assert 0.3 < (ref["state"] == 0).mean() < 0.95
+    assert_losses_match(got, ref, mm)
+    # survival histogram (step H) against numpy on the oracle's records, edge band removed
+    import torch
+    clear = mm >= 1e-9
+    p = {k: torch.from_numpy(np.ascontiguousarray(got[k][clear])).cuda() for k in ("at_turn", "state", "x")}
+    hist = X.xt_survival_histogram(p, 10, 6).cpu().numpy()
+    lost = ref["state"][clear] == 0
+    want = np.bincount(np.minimum(ref["at_turn"][clear][lost] // 10, 5), minlength=6)
+    assert np.array_equal(hist[:6], want) and hist[6] == (~lost).sum()
+
+
+# ----------------------------------------------------- structural invariants (P9) on GPU
+def test_compaction_and_launch_chunking_do_not_change_results(X):
+    coords = C.subsample(C.particles_cfg1(sigma=1e-3), slice(0, None, 211))
+    buf = packed(1)
+    lat = X.xt_lattice_create(buf)
+    base = X.new_particles(lat, coords)
+    X.xt_track_ex(lat, base, 300, compact_every=-1)
+    base = X.particles_to_host(base)
+    assert 0.2 < (base["state"] == 0).mean() < 0.9
+    variants = [dict(compact_every=37), dict(compact_every=100, turns_per_launch=7),
+                dict(compact_every=-1, turns_per_launch=1, block_size=32),
+                dict(compact_every=299, block_size=512), dict(block_size=64, turns_per_launch=150)]
+    for v in variants:
+        p = X.new_particles(lat, coords)
+        X.xt_track_ex(lat, p, 300, **v)
+        assert_bit_identical(X.particles_to_host(p), base)
+    # continuation: 300 = 120 + 180 (state carried only by the arrays)
+    p = X.new_particles(lat, coords)
+    X.xt_track(lat, p, 120)
+    X.xt_track_ex(lat, p, 180, compact_every=50)
+    assert_bit_identical(X.particles_to_host(p), base)
+    lat.close()
+
+
+def test_multi_chunk_compaction_cfg4(X):
+    full = C.particles(4)
+    idx = np.linspace(0, len(full["x"]) - 1, 3001).astype(np.int64)
+    coords = C.subsample(full, idx)
+    lat = X.xt_lattice_create(packed(4))
+    a = X.new_particles(lat, coords)
+    X.xt_track_ex(lat, a, 12, compact_every=-1)
+    b = X.new_particles(lat, coords)
+    X.xt_track_ex(lat, b, 12, compact_every=5, block_size=96)
+    assert_bit_identical(X.particles_to_host(b), X.particles_to_host(a))
+    lat.close()
+
+
+def test_permutation_invariance_and_frozen_lost(X):
+    coords = C.subsample(C.particles_cfg1(sigma=1e-3), slice(0, None, 503))
+    n = len(coords["x"])
+    perm = np.random.default_rng(5).permutation(n)
+    lat = X.xt_lattice_create(packed(1))
+    a = X.new_particles(lat, coords)
+    b = X.new_particles(lat, C.subsample(coords, perm))
+    X.xt_track(lat, a, 50)
+    X.xt_track(lat, b, 50)
+    ha, hb = X.particles_to_host(a), X.particles_to_host(b)
+    assert_bit_identical({k: v for k, v in hb.items()}, {k: v[perm] for k, v in ha.items()})
+    X.xt_track(lat, a, 50)
+    ha2 = X.particles_to_host(a)
+    lost = ha["state"] == 0
+    assert lost.any()
+    for k in FLOAT_KEYS + ("s",) + INT_KEYS:
+        assert np.array_equal(ha2[k][lost], ha[k][lost]), k
+    lat.close()
+
+
+# ------------------------------------------------------------------------- edge cases
+def test_edge_cases(X):
+    import torch
+    buf = packed(1)
+    lat = X.xt_lattice_create(buf)
+    # empty ensemble and zero turns are successful no-ops
+    empty = X.new_particles(lat, {k: np.zeros(0) for k in C.COORDS})
+    X.xt_track(lat, empty, 5)
+    one = X.new_particles(lat, H.coords_from_rows([[1e-4, 0, 1e-4, 0, 0, 0]]))
+    before = X.particles_to_host(one)
+    X.xt_track(lat, one, 0)
+    assert_bit_identical(X.particles_to_host(one), before)
+    # ragged sizes around the block size
+    for n in (1, 31, 33, 127, 129, 257):
+        coords = C.subsample(C.particles_cfg1(sigma=1e-3), slice(0, n * 3001, 3001))
+        got, ref, mm = run_both(X, buf, coords, 3, margin=True)
+        assert_losses_match(got, ref, mm)
+        assert_close(got, ref, 1e-12, sel=ref["state"] == 1)
+    # everything lost at the first aperture; NaN is lost (A4); at_element may be NULL
+    rows = [[0.5, 0, 0, 0, 0, 0], [float("nan"), 0, 0, 0, 0, 0], [0, 0, -0.02, 0, 0, 0]]
+    got, ref, _ = run_both(X, buf, H.coords_from_rows(rows), 4)
+    assert (got["state"] == 0).all() and (got["at_turn"] == 0).all()
+    assert np.array_equal(got["at_element"], ref["at_element"]) and np.array_equal(got["s"], ref["s"])
+    p = X.new_particles(lat, H.coords_from_rows(rows))
+    del p["at_element"]
+    X.xt_track(lat, p, 2)
+    assert (p["state"] == 0).all()
+    # on the edge survives, one ulp beyond is lost (P8 on the GPU)
+    edge = pack_lattice([LimitRect(-0.01, 0.01, -0.01, 0.01), LimitEllipse(0.02, 0.015), Marker()],
+                        H.P0C, H.MASS0, H.Q0)
+    rows = [[0.01, 0, 0.01, 0, 0, 0], [np.nextafter(0.01, 1), 0, 0, 0, 0, 0], [0, 0, -0.01, 0, 0, 0],
+            [0, 0, np.nextafter(-0.01, -1), 0, 0, 0]]
+    got, ref, _ = run_both(X, edge, H.coords_from_rows(rows), 2)
+    assert list(got["state"]) == [1, 0, 1, 0] == list(ref["state"])
+    assert_bit_identical(got, ref)
+    # errors: bad arguments come back as XtError, nothing is written
+    with pytest.raises(X.XtError):
+        X.xt_lattice_create(buf[:-8])
+    with pytest.raises(X.XtError):
+        X.xt_track_ex(lat, one, 1, block_size=48)
+    with pytest.raises(X.XtError):
+        X.xt_track(lat, one, -1)
+    lat.close()
+    # a marker-only / empty line is the identity apart from at_turn
+    ident = X.xt_lattice_create(pack_lattice([Marker(), Marker()], H.P0C, H.MASS0, H.Q0))
+    q = X.new_particles(ident, C.particles(0))
+    h0 = X.particles_to_host(q)
+    X.xt_track(ident, q, 7)
+    h1 = X.particles_to_host(q)
+    assert (h1["at_turn"] == 7).all()
+    assert_bit_identical(h1, h0, keys=FLOAT_KEYS)
+    ident.close()
+    torch.cuda.synchronize()
+
+
+def test_maximum_order_and_all_orders(X):
+    rng = np.random.default_rng(11)
+    els = []
+    for n in range(0, 21):
+        knl = tuple(rng.normal(0, 1.0, n + 1) * 10.0 ** np.arange(n + 1) * 1e-3)
+        ksl = tuple(rng.normal(0, 1.0, n + 1) * 10.0 ** np.arange(n + 1) * 1e-3)
+        els += [Multipole(knl=knl, ksl=ksl, hxl=(1e-3 if n % 3 == 0 else 0.0), length=0.7), Drift(0.3)]
+    buf = pack_lattice(els, H.P0C, H.MASS0, H.Q0)
+    coords = C.particles_cfg0(n=500, seed=77)
+    for k in ("x", "y"):
+        coords[k] = coords[k] * 20.0
+    got, ref, _ = run_both(X, buf, coords, 1)
+    assert_close(got, ref, 1e-12)
+    gotv, refv, _ = run_both(X, buf, coords, 2, kind="nofma")
+    assert_bit_identical(gotv, refv)
+
+
+# ------------------------------------------------------- host-buffer entry point (e2e)
+def test_track_host_equals_device_path(X):
+    import torch
+    coords = C.subsample(C.particles_cfg1(sigma=1e-3), slice(0, None, 401))
+    buf = packed(1)
+    lat = X.xt_lattice_create(buf)
+    d = X.new_particles(lat, coords)
+    host0 = X.particles_to_host(d)
+    X.xt_track(lat, d, 40)
+    host = {k: torch.from_numpy(v.copy()).pin_memory() for k, v in host0.items()}
+    X.xt_track_host(lat, host, 40)
+    assert_bit_identical({k: v.numpy() for k, v in host.items()}, X.particles_to_host(d))
+    lat.close()
+
+
+# ---------------------------------------- full-size launch configuration, sampled outputs
+def test_full_size_cfg3_sampled_against_oracle(X):
+    """BASELINE.json configs[3] at its full 10^7 particles, the launch bench.py times; the
+    oracle recomputes a strided sample one by one."""
+    import torch
+    coords = C.particles(3)
+    n = len(coords["x"])
+    buf = packed(3)
+    lat = X.xt_lattice_create(buf)
+    p = X.new_particles(lat, coords)
+    X.xt_track(lat, p, 1)
+    torch.cuda.synchronize()
+    idx = np.arange(0, n, n // 4000)
+    got = {k: v[torch.from_numpy(idx).cuda()].cpu().numpy() for k, v in p.items()}
+    alive = int((p["state"] == 1).sum().item())
+    assert alive > 0.99 * n
+    assert int(p["at_turn"].sum().item()) == alive
+    lat.close()
+    del p
+    sub = C.subsample(coords, idx)
+    ref = O.new_particles(buf, sub)
+    mm = np.full(len(idx), np.inf)
+    O.track(buf, ref, 1, threads=THREADS, min_margin=mm)
+    assert_losses_match(got, ref, mm)
+    assert_close(got, ref, 1e-12, sel=ref["state"] == 1)
