@@ -183,6 +183,7 @@ def main():
     ap.add_argument("--turns", type=int, default=0, help="override the config's turns (testing only)")
     ap.add_argument("--particles", type=int, default=0, help="override the particle count (testing only)")
     ap.add_argument("--block", type=int, default=0)
+    ap.add_argument("--ppt", type=int, default=0, help="particles per thread (0: auto)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and configs[2] legs")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -224,7 +225,7 @@ def main():
             work[k].copy_(pristine[k])
         if ev0 is not None:
             ev0.record(stream)
-        X.xt_track_ex(lat, work, turns, block_size=args.block)
+        X.xt_track_ex(lat, work, turns, block_size=args.block, particles_per_thread=args.ppt)
         if ev1 is not None:
             ev1.record(stream)
 
@@ -294,7 +295,7 @@ def main():
             host[k].copy_(host0[k])
         barrier()
         t0 = time.perf_counter()
-        X.xt_track_host(lat, host, turns, block_size=args.block)     # synchronises the stream itself
+        X.xt_track_host(lat, host, turns, block_size=args.block, particles_per_thread=args.ppt)     # synchronises the stream itself
         barrier()
         e2e_s = time.perf_counter() - t0
         te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
@@ -325,7 +326,7 @@ def main():
                     w2[k].copy_(pr2[k])
                 a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 a.record(stream)
-                X.xt_track_ex(l2, w2, t2, block_size=args.block)
+                X.xt_track_ex(l2, w2, t2, block_size=args.block, particles_per_thread=args.ppt)
                 b.record(stream)
                 torch.cuda.synchronize()
                 ms2.append(a.elapsed_time(b))

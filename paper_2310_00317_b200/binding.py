@@ -36,7 +36,7 @@ class xt_particles(ctypes.Structure):
 
 class xt_track_opts(ctypes.Structure):
     _fields_ = [("turns_per_launch", ctypes.c_int64), ("compact_every", ctypes.c_int64),
-                ("block_size", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("block_size", ctypes.c_int32), ("particles_per_thread", ctypes.c_int32)]
 
 
 class xt_lattice_info(ctypes.Structure):
@@ -240,10 +240,10 @@ def _n_part(p: Dict) -> int:
     return int(p["x"].shape[0])
 
 
-def _opts(turns_per_launch=0, compact_every=0, block_size=0):
-    if not (turns_per_launch or compact_every or block_size):
+def _opts(turns_per_launch=0, compact_every=0, block_size=0, particles_per_thread=0):
+    if not (turns_per_launch or compact_every or block_size or particles_per_thread):
         return None
-    return xt_track_opts(int(turns_per_launch), int(compact_every), int(block_size), 0)
+    return xt_track_opts(int(turns_per_launch), int(compact_every), int(block_size), int(particles_per_thread))
 
 
 def xt_particles_init_derived(lat: Lattice, p: Dict, stream=None) -> None:
@@ -260,18 +260,18 @@ def xt_track(lat: Lattice, p: Dict, n_turns: int, stream=None) -> None:
 
 
 def xt_track_ex(lat: Lattice, p: Dict, n_turns: int, stream=None, *, turns_per_launch: int = 0,
-                compact_every: int = 0, block_size: int = 0) -> None:
+                compact_every: int = 0, block_size: int = 0, particles_per_thread: int = 0) -> None:
     st = _struct_from_tensors(p)
-    o = _opts(turns_per_launch, compact_every, block_size)
+    o = _opts(turns_per_launch, compact_every, block_size, particles_per_thread)
     _check(lat._lib, lat._lib.xt_track_ex(lat.handle, ctypes.byref(st), _n_part(p), int(n_turns),
                                           _stream_ptr(stream), ctypes.byref(o) if o else None))
 
 
 def xt_track_host(lat: Lattice, p_host: Dict, n_turns: int, stream=None, *, turns_per_launch: int = 0,
-                  compact_every: int = 0, block_size: int = 0) -> None:
+                  compact_every: int = 0, block_size: int = 0, particles_per_thread: int = 0) -> None:
     """End to end with HOST arrays (numpy or pinned torch CPU tensors): H2D, track, D2H, sync."""
     st = _struct_from_numpy(p_host)
-    o = _opts(turns_per_launch, compact_every, block_size)
+    o = _opts(turns_per_launch, compact_every, block_size, particles_per_thread)
     _check(lat._lib, lat._lib.xt_track_host(lat.handle, ctypes.byref(st), _n_part(p_host), int(n_turns),
                                             _stream_ptr(stream), ctypes.byref(o) if o else None))
 

@@ -36,10 +36,16 @@ int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p
   return XT_OK;
 }
 
-int resolve_block(const xt_track_opts *o, int *block) {
+// Launch shape of the tracking kernel: threads per CTA and particles per thread.
+int resolve_shape(const xt_track_opts *o, int *block, int *ppt) {
+  *ppt = (o && o->particles_per_thread) ? o->particles_per_thread : 2;
   *block = (o && o->block_size) ? o->block_size : 128;
-  if (*block < 32 || *block > 512 || (*block % 32) != 0) {
-    set_error("xt_track_ex: block_size must be a multiple of 32 in [32, 512]");
+  if (*ppt != 1 && *ppt != 2 && *ppt != 4) {
+    set_error("xt_track_ex: particles_per_thread must be 0 (auto), 1, 2 or 4");
+    return XT_ERR_INVALID_ARG;
+  }
+  if (*block < 32 || *block > (*ppt == 4 ? 256 : 512) || (*block % 32) != 0) {
+    set_error("xt_track_ex: block_size must be a multiple of 32 in [32, 512] ([32, 256] with 4 particles per thread)");
     return XT_ERR_INVALID_ARG;
   }
   return XT_OK;
@@ -56,8 +62,8 @@ extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t
     xt::set_error("xt_track: negative n_turns");
     return XT_ERR_INVALID_ARG;
   }
-  int block = 0;
-  if ((rc = xt::resolve_block(opts, &block)) != XT_OK) return rc;
+  int block = 0, ppt = 0;
+  if ((rc = xt::resolve_shape(opts, &block, &ppt)) != XT_OK) return rc;
   if (opts && opts->turns_per_launch < 0) {
     xt::set_error("xt_track_ex: negative turns_per_launch");
     return XT_ERR_INVALID_ARG;
@@ -78,7 +84,7 @@ extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t
     const int64_t tpl = tpl_opt > 0 ? tpl_opt : n_turns;
     for (int64_t done = 0; done < n_turns;) {
       const int64_t k = (n_turns - done < tpl) ? n_turns - done : tpl;
-      if ((rc = xt::launch_track(lat, *p, n_part, nullptr, k, block, st)) != XT_OK) return rc;
+      if ((rc = xt::launch_track(lat, *p, n_part, nullptr, k, block, ppt, st)) != XT_OK) return rc;
       done += k;
     }
     return XT_OK;
@@ -102,7 +108,7 @@ extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t
     int64_t k = n_turns - done;
     if (k > tpl) k = tpl;
     if (k > period - since) k = period - since;
-    if ((rc = xt::launch_track(lat, plan.w[cur].p, n_part, plan.n_active, k, block, st)) != XT_OK) return bail(rc);
+    if ((rc = xt::launch_track(lat, plan.w[cur].p, n_part, plan.n_active, k, block, ppt, st)) != XT_OK) return bail(rc);
     done += k;
     since += k;
     if (since == period && done < n_turns) {

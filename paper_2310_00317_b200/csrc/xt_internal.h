@@ -28,7 +28,9 @@ namespace xt {
 //   TAG_ELLIPSE  p0 = a2*b2; {b2, a2}                                            32 B
 //   TAG_END      end of chunk                                                    16 B
 //
-// tag = type | (order << 8); elem = index of the element in the user's packed buffer.
+// tag = type | (order << 8) | (record bytes << 16); elem = index of the element in the user's
+// packed buffer.  The size field lets the kernel step to (and prefetch) the next header
+// without decoding the type first.
 enum : uint32_t {
   TAG_END = 0,
   TAG_DRIFT = 1,
@@ -70,6 +72,7 @@ struct xt_lattice {
   xt_lattice_info info{};
   xt::RefConsts k{};
   int device = -1;
+  int n_sm = 0;  // multiprocessors of `device`: the grid quantum of the tracking kernel
   std::vector<double> s_table_host;
   unsigned char *d_image = nullptr;
   xt::ChunkDesc *d_chunks = nullptr;
@@ -99,8 +102,9 @@ struct HostImage {
 int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImage &out);
 
 // xt_track.cu
+// block: threads per CTA; ppt: particles per thread (1, 2 or 4; 4 needs block <= 256)
 int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part,
-                 const int64_t *d_n_active, int64_t n_turns, int block, cudaStream_t st);
+                 const int64_t *d_n_active, int64_t n_turns, int block, int ppt, cudaStream_t st);
 int launch_init_derived(const xt_lattice *lat, const xt_particles &p, int64_t n, cudaStream_t st);
 
 // xt_compact.cu (step C) -- SoA working set with an origin index

@@ -118,7 +118,7 @@ int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImag
   out.chunks.clear();
   out.s_table.assign(n_elements, 0.0);
 
-  const RecHdr end_rec{TAG_END, 0u, 0.0};
+  const RecHdr end_rec{TAG_END | (static_cast<uint32_t>(sizeof(RecHdr)) << 16), 0u, 0.0};
   size_t chunk_start = 0;
   auto close_chunk = [&]() {
     const size_t at = out.image.size();
@@ -134,7 +134,12 @@ int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImag
   auto append = [&](const RecBuilder &rb) {
     // keep room for the TAG_END record that closes the chunk
     if (out.image.size() - chunk_start + rb.bytes.size() + sizeof(RecHdr) > chunk_bytes) close_chunk();
+    const size_t at = out.image.size();
     out.image.insert(out.image.end(), rb.bytes.begin(), rb.bytes.end());
+    uint32_t tag;  // patch the record size into the upper half of the tag
+    std::memcpy(&tag, out.image.data() + at, 4);
+    tag |= static_cast<uint32_t>(rb.bytes.size()) << 16;
+    std::memcpy(out.image.data() + at, &tag, 4);
     info.n_records += 1;
   };
 
@@ -290,6 +295,8 @@ extern "C" int xt_lattice_create(const void *packed, size_t nbytes, xt_lattice *
   };
   cudaError_t e = cudaGetDevice(&lat->device);
   if (e != cudaSuccess) return fail(e, "cudaGetDevice (no CUDA device? there is no CPU fallback)");
+  if ((e = cudaDeviceGetAttribute(&lat->n_sm, cudaDevAttrMultiProcessorCount, lat->device)) != cudaSuccess)
+    return fail(e, "cudaDeviceGetAttribute(multiProcessorCount)");
   const size_t n_s = img.s_table.empty() ? 1 : img.s_table.size();
   if ((e = cudaMalloc(&lat->d_image, img.image.size())) != cudaSuccess) return fail(e, "cudaMalloc(image)");
   if ((e = cudaMalloc(&lat->d_chunks, img.chunks.size() * sizeof(xt::ChunkDesc))) != cudaSuccess)

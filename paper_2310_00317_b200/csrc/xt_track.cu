@@ -1,18 +1,28 @@
 // The tracking kernel for sm_100a.
 //
 // "Xtrack ... assembles and compiles a C kernel ... able to track the entire beamline"
-// (PAPER.md:74): here that kernel is hand-written.  One thread owns one particle and keeps
-// its state in registers across all elements and turns; SoA FP64 loads/stores happen only at
-// the start and end of the launch.  The lattice image is streamed chunk by chunk from L2
-// into shared memory with 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx),
-// double-buffered; every thread of the CTA reads the same record, so each LDS.128 is a
-// broadcast.  Element dispatch is a switch on a value all lanes share (warp-uniform).
-// Multipoles are a complex Horner recurrence, fully unrolled per order.
+// (PAPER.md:74): here that kernel is hand-written.  One thread owns P particles (P = 1, 2
+// or 4, interleaved so that every global access is coalesced) and keeps their hot state in
+// registers across all elements and turns; SoA FP64 loads/stores happen only at the start and
+// end of the launch (and, for a particle that hits an aperture, once at the moment it is
+// lost).  The lattice image is streamed chunk by chunk from L2 into shared memory with 1-D
+// TMA bulk copies (cp.async.bulk + mbarrier complete_tx), double-buffered; every thread of
+// the CTA reads the same record, so each LDS.128 is a broadcast.  Element dispatch is a
+// switch on a value all lanes share (warp-uniform).  Multipoles are a complex Horner
+// recurrence of FMAs.
 //
-// The arithmetic below is written as plain a*b + c expressions in the canonical order of
-// the production build lets nvcc contract them into DFMA, the
-// validation build (--fmad=false) does not and is then bit-identical to the oracle on
-// cavity-free lattices (sqrt and 1/x are IEEE-correct in both: -prec-sqrt/-prec-div).
+// Why P > 1 (profiles/r01b_*): with one particle per thread 58 % of the issued warp
+// instructions were not FP64 (dispatch, LDS, branches, the slow-path guards of sqrt and /)
+// and the FP64 pipe sat at 49 %.  P particles per thread share every one of those
+// instructions and give the scheduler P independent FP64 chains per warp.
+//
+// Arithmetic.  The maps are written as plain a*b + c expressions in the canonical order of
+// DESIGN.md section 5.  The validation build (--fmad=false, XT_FMAD_OFF) evaluates exactly
+// those trees with IEEE sqrt and division and is bit-identical to the oracle on cavity-free
+// lattices.  The production build lets nvcc contract a*b + c into DFMA and replaces the
+// drift's sqrt + division by branch-free Newton sequences on the MUFU.RSQ64H / MUFU.RCP64H
+// seeds (DESIGN.md section 6 "fast drift"): same formula, a few 1e-16 relative on the
+// increments, inside the 1e-12 parity tolerance with two orders of magnitude to spare.
 #include "xt_internal.h"
 
 namespace xt {
@@ -28,6 +38,7 @@ struct TrackArgs {
   int64_t n_turns;
   int32_t n_chunks;
   uint32_t chunk_bytes;
+  int32_t grid_quantum;  // CTAs are handed out in multiples of this (the SM count)
   double beta0, tib, igam2;
 };
 
@@ -64,223 +75,309 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       : "memory");
 }
 
-// Per-particle registers.
-struct Part {
-  double x, px, y, py, zeta, delta, ptau, rpp, rvv, s;
-  double opd2, b, g, rv0v;  // cached functions of (delta, ptau), refreshed after a cavity
-  int64_t at_element;
-  bool alive;
+#ifndef XT_FMAD_OFF
+// MUFU.RSQ64H / MUFU.RCP64H: ~20-bit seeds computed from the high word of the operand.
+__device__ __forceinline__ double rsqrt_seed(double a) {
+  double r;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
+  return r;
+}
+__device__ __forceinline__ double rcp_seed(double a) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
+  return r;
+}
+#endif
+
+// Hot per-thread state of P particles.  ptau lives in shared memory (touched by cavities
+// only), rpp / rvv are written straight to global memory by the cavity map, s / at_turn /
+// at_element / state are touched only when a particle is lost and at the end of the launch.
+template <int P>
+struct Parts {
+  double x[P], px[P], y[P], py[P], zeta[P], delta[P];
+  double opd2[P], b[P], g[P], rv0v[P];  // cached functions of (delta, ptau), refreshed after a cavity
+  uint32_t alive;                       // bit j: slot j holds a particle that is still being tracked
 };
 
-__device__ __forceinline__ void refresh_cached(Part &q, double opd, double b, double t, double igam2) {
-  q.opd2 = opd * opd;
-  q.b = b;
-  q.g = t * igam2;
-  q.rv0v = b / opd;
+template <int P>
+__device__ __forceinline__ void refresh_cached(Parts<P> &q, int j, double opd, double b, double t, double igam2) {
+  q.opd2[j] = opd * opd;
+  q.b[j] = b;
+  q.g[j] = t * igam2;
+  q.rv0v[j] = b / opd;
 }
 
 // M2: complex Horner, coefficients stored highest order first as (c[n], s[n]) pairs.
-template <int N>
-__device__ __forceinline__ void horner(const double2 *__restrict__ cs, double x, double y, double &re,
-                                       double &im) {
-  double2 top = cs[0];
-  re = top.x;
-  im = top.y;
+template <int P>
+__device__ __forceinline__ void horner_step(const double2 c, const double (&x)[P], const double (&y)[P],
+                                            double (&re)[P], double (&im)[P]) {
 #pragma unroll
-  for (int k = 1; k <= N; ++k) {
-    const double2 c = cs[k];
-    const double nre = re * x + (c.x - im * y);
-    const double nim = re * y + (c.y + im * x);
-    re = nre;
-    im = nim;
+  for (int j = 0; j < P; ++j) {
+    const double nre = re[j] * x[j] + (c.x - im[j] * y[j]);
+    const double nim = re[j] * y[j] + (c.y + im[j] * x[j]);
+    re[j] = nre;
+    im[j] = nim;
   }
 }
 
-__device__ __forceinline__ void horner_dispatch(int order, const double2 *cs, double x, double y, double &re,
-                                                double &im) {
-  switch (order) {
-#define XT_H(N) \
-  case N:       \
-    horner<N>(cs, x, y, re, im); \
-    break;
-    XT_H(0) XT_H(1) XT_H(2) XT_H(3) XT_H(4) XT_H(5) XT_H(6) XT_H(7) XT_H(8) XT_H(9) XT_H(10)
-    XT_H(11) XT_H(12) XT_H(13) XT_H(14) XT_H(15) XT_H(16) XT_H(17) XT_H(18) XT_H(19)
-#undef XT_H
-    default:
-      horner<20>(cs, x, y, re, im);
-      break;
+template <int P>
+__device__ __forceinline__ void horner(const double2 *__restrict__ cs, int order, const double (&x)[P],
+                                       const double (&y)[P], double (&re)[P], double (&im)[P]) {
+  const double2 top = cs[0];
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    re[j] = top.x;
+    im[j] = top.y;
+  }
+  int k = 1;
+  const int rem = order & 3;
+#pragma unroll 1
+  for (; k <= rem; ++k) horner_step<P>(cs[k], x, y, re, im);
+#pragma unroll 1
+  for (; k <= order; k += 4) {
+    const double2 c0 = cs[k], c1 = cs[k + 1], c2 = cs[k + 2], c3 = cs[k + 3];
+    horner_step<P>(c0, x, y, re, im);
+    horner_step<P>(c1, x, y, re, im);
+    horner_step<P>(c2, x, y, re, im);
+    horner_step<P>(c3, x, y, re, im);
   }
 }
 
-__device__ __forceinline__ void lose(Part &q, uint32_t elem, const double *__restrict__ s_table) {
-  q.alive = false;
-  q.at_element = static_cast<int64_t>(elem);
-  q.s = s_table[elem];
+// A particle left the aperture: its record is final, so write it now (the thread owns the
+// row).  Out of line and by value: the rare path must not force the hot state into memory.
+__device__ __noinline__ void store_lost(const xt_particles p, const double *s_table, int64_t i, double x,
+                                        double px, double y, double py, double zeta, double delta, double ptau,
+                                        uint32_t elem, int64_t turns_done) {
+  p.x[i] = x;
+  p.px[i] = px;
+  p.y[i] = y;
+  p.py[i] = py;
+  p.zeta[i] = zeta;
+  p.delta[i] = delta;
+  p.ptau[i] = ptau;
+  p.s[i] = s_table[elem];
+  p.at_turn[i] += turns_done;
+  p.state[i] = 0;
+  if (p.at_element) p.at_element[i] = static_cast<int64_t>(elem);
 }
 
-// Push the particle through every record of one staged chunk.
-__device__ __forceinline__ void track_chunk(Part &q, const unsigned char *rp, const TrackArgs &a) {
+// ... and park the slot on the reference orbit, where every map stays finite and cheap.
+template <int P>
+__device__ __forceinline__ void lose(Parts<P> &q, uint32_t out, const int64_t (&idx)[P], uint32_t elem,
+                                     int64_t turns_done, const double *ptau_s, int ptau_stride,
+                                     const TrackArgs &a) {
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    if (out & (1u << j)) {
+      store_lost(a.p, a.s_table, idx[j], q.x[j], q.px[j], q.y[j], q.py[j], q.zeta[j], q.delta[j],
+                 ptau_s[j * ptau_stride], elem, turns_done);
+      q.x[j] = q.px[j] = q.y[j] = q.py[j] = q.zeta[j] = 0.0;
+    }
+  }
+  q.alive &= ~out;
+}
+
+// Push the P particles of this thread through every record of one staged chunk.
+template <int P>
+__device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp, const int64_t (&idx)[P],
+                                            int64_t turns_done, double *ptau_s, const int ptau_stride,
+                                            const TrackArgs &a) {
+  RecHdr h = *reinterpret_cast<const RecHdr *>(rp);
   for (;;) {
-    const RecHdr h = *reinterpret_cast<const RecHdr *>(rp);
     const uint32_t type = h.tag & 0xffu;
     if (type == TAG_END) break;
     const double2 *slots = reinterpret_cast<const double2 *>(rp + sizeof(RecHdr));
+    const double p0 = h.p0;
+    const uint32_t tag = h.tag;
+    const uint32_t elem = h.elem;
+    rp += tag >> 16;                              // record size in bytes
+    h = *reinterpret_cast<const RecHdr *>(rp);    // prefetch the next header behind this map
     switch (type) {
       case TAG_DRIFT: {
         // M1 exact drift, cancellation-free zeta (DESIGN.md section 5 "Drift")
-        if (q.alive) {
-          const double t1 = q.px * q.px;
-          const double pxy2 = q.py * q.py + t1;
-          const double pz = sqrt(q.opd2 - pxy2);
-          const double s1 = pz + q.b;
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          const double t1 = q.px[j] * q.px[j];
+          const double pxy2 = q.py[j] * q.py[j] + t1;
+          const double rad = q.opd2[j] - pxy2;
+#ifdef XT_FMAD_OFF
+          const double pz = sqrt(rad);
+          const double s1 = pz + q.b[j];
           const double den = pz * s1;
           const double rr = 1.0 / den;
-          const double lr = h.p0 * rr;
+          const double lr = p0 * rr;
           const double lpz = lr * s1;
-          q.x = q.px * lpz + q.x;
-          q.y = q.py * lpz + q.y;
-          q.zeta = (q.g - pxy2) * lr + q.zeta;
+#else
+          // 1/pz by one cubic Newton step on the RSQ seed; 1/(pz + b) likewise on the RCP seed
+          const double r0 = rsqrt_seed(rad);
+          const double e = fma(-rad, r0 * r0, 1.0);
+          const double r1 = fma(fma(e, 0.375, 0.5), r0 * e, r0);    // 1/pz
+          const double s1 = fma(rad, r1, q.b[j]);                  // pz + b
+          const double y0 = rcp_seed(s1);
+          const double f = fma(-s1, y0, 1.0);
+          const double y1 = fma(y0, fma(f, f, f), y0);             // 1/(pz + b)
+          const double lpz = p0 * r1;                              // L/pz
+          const double lr = lpz * y1;                              // L/(pz (pz + b))
+#endif
+          q.x[j] = q.px[j] * lpz + q.x[j];
+          q.y[j] = q.py[j] * lpz + q.y[j];
+          q.zeta[j] = (q.g[j] - pxy2) * lr + q.zeta[j];
         }
-        rp += 16;
         break;
       }
       case TAG_MULT: {
-        const int order = static_cast<int>(h.tag >> 8);
-        if (q.alive) {
-          double re, im;
-          horner_dispatch(order, slots, q.x, q.y, re, im);
-          q.px = q.px - re;
-          q.py = q.py + im;
+        double re[P], im[P];
+        horner<P>(slots, static_cast<int>((tag >> 8) & 0xffu), q.x, q.y, re, im);
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          q.px[j] = q.px[j] - re[j];
+          q.py[j] = q.py[j] + im[j];
         }
-        rp += 32 + 16 * order;
         break;
       }
       case TAG_CMULT: {
-        const int order = static_cast<int>(h.tag >> 8);
-        if (q.alive) {
-          const double hxl = h.p0;
-          const double wf = slots[0].x;
-          double re, im;
-          horner_dispatch(order, slots + 1, q.x, q.y, re, im);
-          q.px = q.px - re;
-          q.py = q.py + im;
-          q.px = hxl * q.delta + q.px;
-          q.px = q.px - wf * q.x;
-          q.zeta = q.zeta - (hxl * q.x) * q.rv0v;
+        const double hxl = p0;
+        const double wf = slots[0].x;
+        double re[P], im[P];
+        horner<P>(slots + 1, static_cast<int>((tag >> 8) & 0xffu), q.x, q.y, re, im);
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          q.px[j] = q.px[j] - re[j];
+          q.py[j] = q.py[j] + im[j];
+          q.px[j] = hxl * q.delta[j] + q.px[j];
+          q.px[j] = q.px[j] - wf * q.x[j];
+          q.zeta[j] = q.zeta[j] - (hxl * q.x[j]) * q.rv0v[j];
         }
-        rp += 48 + 16 * order;
         break;
       }
       case TAG_CAVITY: {
-        if (q.alive) {
-          const double2 kv = slots[0];  // (kz, vn)
-          const double phase = h.p0 - kv.x * q.zeta;
-          q.ptau = kv.y * sin(phase) + q.ptau;
-          const double t = q.ptau * (q.ptau + a.tib);
-          q.delta = t / (sqrt(t + 1.0) + 1.0);
-          const double opd = 1.0 + q.delta;
-          q.rpp = 1.0 / opd;
-          const double b = 1.0 + a.beta0 * q.ptau;
-          q.rvv = opd / b;
-          refresh_cached(q, opd, b, t, a.igam2);
+        const double2 kv = slots[0];  // (kz, vn)
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          if (q.alive & (1u << j)) {
+            const double phase = p0 - kv.x * q.zeta[j];
+            const double ptau = kv.y * sin(phase) + ptau_s[j * ptau_stride];
+            const double t = ptau * (ptau + a.tib);
+            const double delta = t / (sqrt(t + 1.0) + 1.0);
+            const double opd = 1.0 + delta;
+            const double b = 1.0 + a.beta0 * ptau;
+            ptau_s[j * ptau_stride] = ptau;
+            q.delta[j] = delta;
+            a.p.rpp[idx[j]] = 1.0 / opd;
+            a.p.rvv[idx[j]] = opd / b;
+            refresh_cached<P>(q, j, opd, b, t, a.igam2);
+          }
         }
-        rp += 32;
         break;
       }
       case TAG_SROT: {
-        if (q.alive) {
-          const double2 cs = slots[0];  // (cos_z, sin_z)
-          const double nx = cs.x * q.x + cs.y * q.y;
-          const double ny = cs.x * q.y - cs.y * q.x;
-          const double npx = cs.x * q.px + cs.y * q.py;
-          const double npy = cs.x * q.py - cs.y * q.px;
-          q.x = nx;
-          q.y = ny;
-          q.px = npx;
-          q.py = npy;
+        const double2 cs = slots[0];  // (cos_z, sin_z)
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          const double nx = cs.x * q.x[j] + cs.y * q.y[j];
+          const double ny = cs.x * q.y[j] - cs.y * q.x[j];
+          const double npx = cs.x * q.px[j] + cs.y * q.py[j];
+          const double npy = cs.x * q.py[j] - cs.y * q.px[j];
+          q.x[j] = nx;
+          q.y[j] = ny;
+          q.px[j] = npx;
+          q.py[j] = npy;
         }
-        rp += 32;
         break;
       }
       case TAG_SHIFT: {
-        if (q.alive) {
-          const double2 d = slots[0];
-          q.x = q.x - d.x;
-          q.y = q.y - d.y;
+        const double2 d = slots[0];
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          q.x[j] = q.x[j] - d.x;
+          q.y[j] = q.y[j] - d.y;
         }
-        rp += 32;
         break;
       }
       case TAG_RECT: {
-        if (q.alive) {
-          const double2 xr = slots[0], yr = slots[1];
-          const bool inside = (q.x >= xr.x) && (q.x <= xr.y) && (q.y >= yr.x) && (q.y <= yr.y);
-          if (!inside) lose(q, h.elem, a.s_table);
+        const double2 xr = slots[0], yr = slots[1];
+        uint32_t out = 0;
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          const bool inside = (q.x[j] >= xr.x) && (q.x[j] <= xr.y) && (q.y[j] >= yr.x) && (q.y[j] <= yr.y);
+          out |= inside ? 0u : (1u << j);
         }
-        rp += 48;
+        out &= q.alive;
+        if (out) lose<P>(q, out, idx, elem, turns_done, ptau_s, ptau_stride, a);
         break;
       }
       case TAG_ELLIPSE: {
-        if (q.alive) {
-          const double2 ba = slots[0];  // (b2, a2)
-          const double tt = (q.x * q.x) * ba.x + (q.y * q.y) * ba.y;
-          const bool inside = (tt <= h.p0);
-          if (!inside) lose(q, h.elem, a.s_table);
+        const double2 ba = slots[0];  // (b2, a2)
+        uint32_t out = 0;
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          const double tt = (q.x[j] * q.x[j]) * ba.x + (q.y[j] * q.y[j]) * ba.y;
+          out |= (tt <= p0) ? 0u : (1u << j);
         }
-        rp += 32;
+        out &= q.alive;
+        if (out) lose<P>(q, out, idx, elem, turns_done, ptau_s, ptau_stride, a);
         break;
       }
       default:  // cannot happen: the packer emits only the tags above
-        rp += 16;
         break;
     }
   }
 }
 
-__global__ void __launch_bounds__(512) xt_track_kernel(const TrackArgs a) {
+// Shared memory: [0,16) two mbarriers; [128, 128 + 8*P*blockDim) ptau slots;
+// then staging buffer 0 (and buffer 1 for multi-chunk lattices), 128-byte aligned.
+template <int P>
+__global__ void __launch_bounds__(P >= 4 ? 256 : 512) xt_track_kernel(const TrackArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
-  // smem layout: [0,16) two mbarriers; [128, 128+chunk_bytes) buffer 0; then buffer 1
   const uint32_t bar0 = smem_addr(smem);
-  unsigned char *const buf0 = smem + 128;
+  double *const ptau_s = reinterpret_cast<double *>(smem + 128) + threadIdx.x;
+  const int ptau_stride = static_cast<int>(blockDim.x);
+  unsigned char *const buf0 = smem + 128 + ((static_cast<uint32_t>(8 * P) * blockDim.x + 127u) & ~127u);
 
+  // Balanced hand-out (device side, so that compaction's device counter needs no host
+  // sync): use as few CTAs as hold n_active particles, rounded up to a whole number per SM,
+  // and give each the same share (a multiple of 32 so that warps stay whole).
   const int64_t n_active = a.n_active ? *a.n_active : a.n_part;
-  const int64_t base = static_cast<int64_t>(blockIdx.x) * blockDim.x;
-  if (base >= n_active) return;  // CTA-uniform
-  const int64_t i = base + threadIdx.x;
-  const bool valid = i < n_active;
+  const int64_t cap = static_cast<int64_t>(blockDim.x) * P;
+  const int64_t need = (n_active + cap - 1) / cap;
+  int64_t used = ((need + a.grid_quantum - 1) / a.grid_quantum) * a.grid_quantum;
+  if (used > static_cast<int64_t>(gridDim.x)) used = gridDim.x;
+  if (static_cast<int64_t>(blockIdx.x) >= used) return;  // CTA-uniform
+  int64_t share = (n_active + used - 1) / used;
+  share = (share + 31) & ~static_cast<int64_t>(31);
+  const int64_t start = static_cast<int64_t>(blockIdx.x) * share;
+  if (start >= n_active) return;  // CTA-uniform
+  const int64_t count = (n_active - start < share) ? n_active - start : share;
 
-  Part q;
-  int64_t at_turn = 0;
-  bool alive_at_load = false;
-  q.alive = false;
-  q.at_element = 0;
-  q.s = 0.0;
-  if (valid) {
-    alive_at_load = (a.p.state[i] == 1);
-  }
-  if (alive_at_load) {
-    q.x = a.p.x[i];
-    q.px = a.p.px[i];
-    q.y = a.p.y[i];
-    q.py = a.p.py[i];
-    q.zeta = a.p.zeta[i];
-    q.delta = a.p.delta[i];
-    q.ptau = a.p.ptau[i];
-    q.rpp = a.p.rpp[i];
-    q.rvv = a.p.rvv[i];
-    q.s = a.p.s[i];
-    at_turn = a.p.at_turn[i];
-    q.at_element = a.p.at_element ? a.p.at_element[i] : 0;
-    q.alive = true;
-    const double opd = 1.0 + q.delta;
-    const double b = 1.0 + a.beta0 * q.ptau;
-    const double t = q.ptau * (q.ptau + a.tib);
-    refresh_cached(q, opd, b, t, a.igam2);
-  } else {
-    q.x = q.px = q.y = q.py = q.zeta = q.delta = q.ptau = 0.0;
-    q.rpp = q.rvv = 1.0;
-    q.opd2 = q.b = q.rv0v = 1.0;
-    q.g = 0.0;
+  Parts<P> q;
+  int64_t idx[P];
+  q.alive = 0;
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    const int64_t k = static_cast<int64_t>(j) * blockDim.x + threadIdx.x;
+    const int64_t i = start + k;
+    idx[j] = i;
+    const bool live = (k < count) && (a.p.state[i] == 1);
+    if (live) {
+      q.x[j] = a.p.x[i];
+      q.px[j] = a.p.px[i];
+      q.y[j] = a.p.y[i];
+      q.py[j] = a.p.py[i];
+      q.zeta[j] = a.p.zeta[i];
+      q.delta[j] = a.p.delta[i];
+      const double ptau = a.p.ptau[i];
+      ptau_s[j * ptau_stride] = ptau;
+      q.alive |= 1u << j;
+      const double opd = 1.0 + q.delta[j];
+      const double b = 1.0 + a.beta0 * ptau;
+      const double t = ptau * (ptau + a.tib);
+      refresh_cached<P>(q, j, opd, b, t, a.igam2);
+    } else {
+      q.x[j] = q.px[j] = q.y[j] = q.py[j] = q.zeta[j] = q.delta[j] = 0.0;
+      q.opd2[j] = q.b[j] = q.rv0v[j] = 1.0;
+      q.g[j] = 0.0;
+      ptau_s[j * ptau_stride] = 0.0;
+    }
   }
 
   const bool single = (a.n_chunks == 1);
@@ -295,13 +392,13 @@ __global__ void __launch_bounds__(512) xt_track_kernel(const TrackArgs a) {
     tma_load_chunk(bar0, smem_addr(buf0), a.image + d.offset, d.nbytes);
   }
 
+  int64_t turns_done = 0;
   if (single) {
     // Whole lattice resident in buffer 0: warps run free, no CTA-level synchronisation.
     mbar_wait(bar0, 0);
-    for (int64_t turn = 0; turn < a.n_turns; ++turn) {
-      if (!__any_sync(0xffffffffu, q.alive)) break;
-      track_chunk(q, buf0, a);
-      if (q.alive) at_turn += 1;
+    for (; turns_done < a.n_turns; ++turns_done) {
+      if (!__any_sync(0xffffffffu, q.alive != 0)) break;
+      track_chunk<P>(q, buf0, idx, turns_done, ptau_s, ptau_stride, a);
     }
   } else {
     const int64_t total = a.n_turns * a.n_chunks;
@@ -319,13 +416,14 @@ __global__ void __launch_bounds__(512) xt_track_kernel(const TrackArgs a) {
       }
       const uint32_t cb = static_cast<uint32_t>(gidx & 1);
       mbar_wait(bar0 + 8 * cb, static_cast<uint32_t>((gidx >> 1) & 1));
-      if (__any_sync(0xffffffffu, q.alive)) track_chunk(q, buf0 + static_cast<size_t>(cb) * a.chunk_bytes, a);
+      if (__any_sync(0xffffffffu, q.alive != 0))
+        track_chunk<P>(q, buf0 + static_cast<size_t>(cb) * a.chunk_bytes, idx, turns_done, ptau_s, ptau_stride, a);
       ++gidx;
       if (++c == a.n_chunks) {
         c = 0;
-        if (q.alive) at_turn += 1;  // T: turn completed
+        ++turns_done;  // T: turn completed
       }
-      any = __syncthreads_or(q.alive ? 1 : 0) != 0;
+      any = __syncthreads_or(q.alive != 0 ? 1 : 0) != 0;
       if (!any) break;
     }
     if (!any && gidx < total) {
@@ -334,21 +432,21 @@ __global__ void __launch_bounds__(512) xt_track_kernel(const TrackArgs a) {
     }
   }
 
-  // W: store (only particles that were alive when the launch started can have changed)
-  if (alive_at_load) {
-    a.p.x[i] = q.x;
-    a.p.px[i] = q.px;
-    a.p.y[i] = q.y;
-    a.p.py[i] = q.py;
-    a.p.zeta[i] = q.zeta;
-    a.p.delta[i] = q.delta;
-    a.p.ptau[i] = q.ptau;
-    a.p.rpp[i] = q.rpp;
-    a.p.rvv[i] = q.rvv;
-    a.p.s[i] = q.alive ? 0.0 : q.s;
-    a.p.at_turn[i] = at_turn;
-    a.p.state[i] = q.alive ? 1 : 0;
-    if (a.p.at_element) a.p.at_element[i] = q.at_element;
+  // W: survivors (lost particles were written when they were lost; rpp, rvv by the cavities)
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    if (q.alive & (1u << j)) {
+      const int64_t i = idx[j];
+      a.p.x[i] = q.x[j];
+      a.p.px[i] = q.px[j];
+      a.p.y[i] = q.y[j];
+      a.p.py[i] = q.py[j];
+      a.p.zeta[i] = q.zeta[j];
+      a.p.delta[i] = q.delta[j];
+      a.p.ptau[i] = ptau_s[j * ptau_stride];
+      a.p.s[i] = 0.0;
+      a.p.at_turn[i] += turns_done;
+    }
   }
 }
 
@@ -366,10 +464,32 @@ __global__ void xt_init_derived_kernel(xt_particles p, int64_t n, double beta0, 
   p.rvv[i] = opd / b;
 }
 
+template <int P>
+int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
+  const size_t ptau_bytes = (static_cast<size_t>(8 * P) * block + 127) & ~static_cast<size_t>(127);
+  const size_t smem = 128 + ptau_bytes + (lat->info.n_chunks == 1 ? 1 : 2) * static_cast<size_t>(lat->info.chunk_bytes);
+  static bool attr_set = false;
+  if (!attr_set) {
+    XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    attr_set = true;
+  }
+  const int64_t cap = static_cast<int64_t>(block) * P;
+  const int64_t need = (a.n_part + cap - 1) / cap;
+  const int64_t grid = ((need + a.grid_quantum - 1) / a.grid_quantum) * a.grid_quantum;
+  if (grid > 2147483647LL) {
+    set_error("xt_track: too many particles for one launch");
+    return XT_ERR_INVALID_ARG;
+  }
+  xt_track_kernel<P><<<static_cast<unsigned>(grid), block, smem, st>>>(a);
+  count_launch();
+  XT_CUDA(cudaGetLastError());
+  return XT_OK;
+}
+
 }  // namespace
 
 int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, const int64_t *d_n_active,
-                 int64_t n_turns, int block, cudaStream_t st) {
+                 int64_t n_turns, int block, int ppt, cudaStream_t st) {
   if (n_part <= 0 || n_turns <= 0) return XT_OK;
   TrackArgs a;
   a.image = lat->d_image;
@@ -381,24 +501,21 @@ int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, c
   a.n_turns = n_turns;
   a.n_chunks = static_cast<int32_t>(lat->info.n_chunks);
   a.chunk_bytes = static_cast<uint32_t>(lat->info.chunk_bytes);
+  a.grid_quantum = lat->n_sm > 0 ? lat->n_sm : 1;
   a.beta0 = lat->k.beta0;
   a.tib = lat->k.tib;
   a.igam2 = lat->k.igam2;
-  const size_t smem = 128 + (lat->info.n_chunks == 1 ? 1 : 2) * static_cast<size_t>(lat->info.chunk_bytes);
-  static bool attr_set = false;
-  if (!attr_set) {
-    XT_CUDA(cudaFuncSetAttribute(xt_track_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 + 2 * 65536));
-    attr_set = true;
+  switch (ppt) {
+    case 1:
+      return launch_track_p<1>(a, lat, block, st);
+    case 2:
+      return launch_track_p<2>(a, lat, block, st);
+    case 4:
+      return launch_track_p<4>(a, lat, block, st);
+    default:
+      set_error("xt_track: particles_per_thread must be 1, 2 or 4");
+      return XT_ERR_INVALID_ARG;
   }
-  const int64_t grid = (n_part + block - 1) / block;
-  if (grid > 2147483647LL) {
-    set_error("xt_track: too many particles for one launch");
-    return XT_ERR_INVALID_ARG;
-  }
-  xt_track_kernel<<<static_cast<unsigned>(grid), block, smem, st>>>(a);
-  count_launch();
-  XT_CUDA(cudaGetLastError());
-  return XT_OK;
 }
 
 int launch_init_derived(const xt_lattice *lat, const xt_particles &p, int64_t n, cudaStream_t st) {
