@@ -44,8 +44,8 @@ int resolve_shape(const xt_track_opts *o, int *block, int *ppt) {
     set_error("xt_track_ex: particles_per_thread must be 0 (auto), 1, 2 or 4");
     return XT_ERR_INVALID_ARG;
   }
-  if (*block < 32 || *block > (*ppt == 4 ? 256 : 512) || (*block % 32) != 0) {
-    set_error("xt_track_ex: block_size must be a multiple of 32 in [32, 512] ([32, 256] with 4 particles per thread)");
+  if (*block < 32 || *block > 256 || (*block % 32) != 0) {
+    set_error("xt_track_ex: block_size must be a multiple of 32 in [32, 256]");
     return XT_ERR_INVALID_ARG;
   }
   return XT_OK;

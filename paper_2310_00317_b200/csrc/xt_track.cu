@@ -89,22 +89,37 @@ __device__ __forceinline__ double rcp_seed(double a) {
 }
 #endif
 
-// Hot per-thread state of P particles.  ptau lives in shared memory (touched by cavities
-// only), rpp / rvv are written straight to global memory by the cavity map, s / at_turn /
-// at_element / state are touched only when a particle is lost and at the end of the launch.
+// Hot per-thread state of P particles: what drifts and kicks touch at every element.
 template <int P>
 struct Parts {
-  double x[P], px[P], y[P], py[P], zeta[P], delta[P];
-  double opd2[P], b[P], g[P], rv0v[P];  // cached functions of (delta, ptau), refreshed after a cavity
-  uint32_t alive;                       // bit j: slot j holds a particle that is still being tracked
+  double x[P], px[P], y[P], py[P], zeta[P];
+  double opd2[P], b[P], g[P];  // cached functions of (delta, ptau), refreshed after a cavity
+  uint32_t alive;              // bit j: slot j holds a particle that is still being tracked
+};
+
+// Cold per-thread state, kept out of the register file: ptau (cavities only), delta and
+// rv0v = (1 + beta0 ptau)/(1 + delta) (curved multipoles only) live in shared memory, one
+// conflict-free column per thread; rpp / rvv are written straight to global memory by the
+// cavity map; s / at_turn / at_element / state are touched only when a particle is lost and
+// at the end of the launch.
+template <int P>
+struct Cold {
+  double *col;    // this thread's column: value m of slot j at col[(m * P + j) * stride]
+  int stride;     // blockDim.x
+  int64_t first;  // index of slot 0's particle; slot j is first + j * stride
+  __device__ __forceinline__ double &ptau(int j) const { return col[j * stride]; }
+  __device__ __forceinline__ double &delta(int j) const { return col[(P + j) * stride]; }
+  __device__ __forceinline__ double &rv0v(int j) const { return col[(2 * P + j) * stride]; }
+  __device__ __forceinline__ int64_t idx(int j) const { return first + static_cast<int64_t>(j) * stride; }
 };
 
 template <int P>
-__device__ __forceinline__ void refresh_cached(Parts<P> &q, int j, double opd, double b, double t, double igam2) {
+__device__ __forceinline__ void refresh_cached(Parts<P> &q, const Cold<P> &cold, int j, double opd, double b,
+                                               double t, double igam2) {
   q.opd2[j] = opd * opd;
   q.b[j] = b;
   q.g[j] = t * igam2;
-  q.rv0v[j] = b / opd;
+  cold.rv0v(j) = b / opd;
 }
 
 // M2: complex Horner, coefficients stored highest order first as (c[n], s[n]) pairs.
@@ -129,12 +144,13 @@ __device__ __forceinline__ void horner(const double2 *__restrict__ cs, int order
     re[j] = top.x;
     im[j] = top.y;
   }
-  int k = 1;
+  // order mod 4 leading steps, then whole groups of four
   const int rem = order & 3;
+  if (rem >= 1) horner_step<P>(cs[1], x, y, re, im);
+  if (rem >= 2) horner_step<P>(cs[2], x, y, re, im);
+  if (rem == 3) horner_step<P>(cs[3], x, y, re, im);
 #pragma unroll 1
-  for (; k <= rem; ++k) horner_step<P>(cs[k], x, y, re, im);
-#pragma unroll 1
-  for (; k <= order; k += 4) {
+  for (int k = rem + 1; k <= order; k += 4) {
     const double2 c0 = cs[k], c1 = cs[k + 1], c2 = cs[k + 2], c3 = cs[k + 3];
     horner_step<P>(c0, x, y, re, im);
     horner_step<P>(c1, x, y, re, im);
@@ -163,14 +179,13 @@ __device__ __noinline__ void store_lost(const xt_particles p, const double *s_ta
 
 // ... and park the slot on the reference orbit, where every map stays finite and cheap.
 template <int P>
-__device__ __forceinline__ void lose(Parts<P> &q, uint32_t out, const int64_t (&idx)[P], uint32_t elem,
-                                     int64_t turns_done, const double *ptau_s, int ptau_stride,
-                                     const TrackArgs &a) {
+__device__ __forceinline__ void lose(Parts<P> &q, uint32_t out, const Cold<P> &cold, uint32_t elem,
+                                     int64_t turns_done, const TrackArgs &a) {
 #pragma unroll
   for (int j = 0; j < P; ++j) {
     if (out & (1u << j)) {
-      store_lost(a.p, a.s_table, idx[j], q.x[j], q.px[j], q.y[j], q.py[j], q.zeta[j], q.delta[j],
-                 ptau_s[j * ptau_stride], elem, turns_done);
+      store_lost(a.p, a.s_table, cold.idx(j), q.x[j], q.px[j], q.y[j], q.py[j], q.zeta[j], cold.delta(j),
+                 cold.ptau(j), elem, turns_done);
       q.x[j] = q.px[j] = q.y[j] = q.py[j] = q.zeta[j] = 0.0;
     }
   }
@@ -179,9 +194,8 @@ __device__ __forceinline__ void lose(Parts<P> &q, uint32_t out, const int64_t (&
 
 // Push the P particles of this thread through every record of one staged chunk.
 template <int P>
-__device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp, const int64_t (&idx)[P],
-                                            int64_t turns_done, double *ptau_s, const int ptau_stride,
-                                            const TrackArgs &a) {
+__device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp, const Cold<P> &cold,
+                                            int64_t turns_done, const TrackArgs &a) {
   RecHdr h = *reinterpret_cast<const RecHdr *>(rp);
   for (;;) {
     const uint32_t type = h.tag & 0xffu;
@@ -238,15 +252,20 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
       case TAG_CMULT: {
         const double hxl = p0;
         const double wf = slots[0].x;
-        double re[P], im[P];
+        double re[P], im[P], delta[P], rv0v[P];
+#pragma unroll
+        for (int j = 0; j < P; ++j) {  // issued ahead of the Horner loop that hides their latency
+          delta[j] = cold.delta(j);
+          rv0v[j] = cold.rv0v(j);
+        }
         horner<P>(slots + 1, static_cast<int>((tag >> 8) & 0xffu), q.x, q.y, re, im);
 #pragma unroll
         for (int j = 0; j < P; ++j) {
           q.px[j] = q.px[j] - re[j];
           q.py[j] = q.py[j] + im[j];
-          q.px[j] = hxl * q.delta[j] + q.px[j];
+          q.px[j] = hxl * delta[j] + q.px[j];
           q.px[j] = q.px[j] - wf * q.x[j];
-          q.zeta[j] = q.zeta[j] - (hxl * q.x[j]) * q.rv0v[j];
+          q.zeta[j] = q.zeta[j] - (hxl * q.x[j]) * rv0v[j];
         }
         break;
       }
@@ -256,16 +275,16 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         for (int j = 0; j < P; ++j) {
           if (q.alive & (1u << j)) {
             const double phase = p0 - kv.x * q.zeta[j];
-            const double ptau = kv.y * sin(phase) + ptau_s[j * ptau_stride];
+            const double ptau = kv.y * sin(phase) + cold.ptau(j);
             const double t = ptau * (ptau + a.tib);
             const double delta = t / (sqrt(t + 1.0) + 1.0);
             const double opd = 1.0 + delta;
             const double b = 1.0 + a.beta0 * ptau;
-            ptau_s[j * ptau_stride] = ptau;
-            q.delta[j] = delta;
-            a.p.rpp[idx[j]] = 1.0 / opd;
-            a.p.rvv[idx[j]] = opd / b;
-            refresh_cached<P>(q, j, opd, b, t, a.igam2);
+            cold.ptau(j) = ptau;
+            cold.delta(j) = delta;
+            a.p.rpp[cold.idx(j)] = 1.0 / opd;
+            a.p.rvv[cold.idx(j)] = opd / b;
+            refresh_cached<P>(q, cold, j, opd, b, t, a.igam2);
           }
         }
         break;
@@ -303,7 +322,7 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
           out |= inside ? 0u : (1u << j);
         }
         out &= q.alive;
-        if (out) lose<P>(q, out, idx, elem, turns_done, ptau_s, ptau_stride, a);
+        if (out) lose<P>(q, out, cold, elem, turns_done, a);
         break;
       }
       case TAG_ELLIPSE: {
@@ -315,7 +334,7 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
           out |= (tt <= p0) ? 0u : (1u << j);
         }
         out &= q.alive;
-        if (out) lose<P>(q, out, idx, elem, turns_done, ptau_s, ptau_stride, a);
+        if (out) lose<P>(q, out, cold, elem, turns_done, a);
         break;
       }
       default:  // cannot happen: the packer emits only the tags above
@@ -324,15 +343,26 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
   }
 }
 
-// Shared memory: [0,16) two mbarriers; [128, 128 + 8*P*blockDim) ptau slots;
+// Register budget: 65536 / (kMaxBlock * min CTAs per SM).
+#ifndef XT_MINB4
+#define XT_MINB4 2  // P = 4: 128 registers
+#endif
+#ifndef XT_MINB2
+#define XT_MINB2 3  // P = 2: 80 registers
+#endif
+constexpr int kMaxBlock = 256;
+
+// Shared memory: [0,16) two mbarriers; [128, 128 + 24*P*blockDim) cold per-thread columns;
 // then staging buffer 0 (and buffer 1 for multi-chunk lattices), 128-byte aligned.
 template <int P>
-__global__ void __launch_bounds__(P >= 4 ? 256 : 512) xt_track_kernel(const TrackArgs a) {
+__global__ void __launch_bounds__(kMaxBlock, P == 4 ? XT_MINB4 : (P == 2 ? XT_MINB2 : 4))
+    xt_track_kernel(const TrackArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   const uint32_t bar0 = smem_addr(smem);
-  double *const ptau_s = reinterpret_cast<double *>(smem + 128) + threadIdx.x;
-  const int ptau_stride = static_cast<int>(blockDim.x);
-  unsigned char *const buf0 = smem + 128 + ((static_cast<uint32_t>(8 * P) * blockDim.x + 127u) & ~127u);
+  Cold<P> cold;
+  cold.col = reinterpret_cast<double *>(smem + 128) + threadIdx.x;
+  cold.stride = static_cast<int>(blockDim.x);
+  unsigned char *const buf0 = smem + 128 + ((static_cast<uint32_t>(24 * P) * blockDim.x + 127u) & ~127u);
 
   // Balanced hand-out (device side, so that compaction's device counter needs no host
   // sync): use as few CTAs as hold n_active particles, rounded up to a whole number per SM,
@@ -350,13 +380,12 @@ __global__ void __launch_bounds__(P >= 4 ? 256 : 512) xt_track_kernel(const Trac
   const int64_t count = (n_active - start < share) ? n_active - start : share;
 
   Parts<P> q;
-  int64_t idx[P];
+  cold.first = start + threadIdx.x;
   q.alive = 0;
 #pragma unroll
   for (int j = 0; j < P; ++j) {
     const int64_t k = static_cast<int64_t>(j) * blockDim.x + threadIdx.x;
     const int64_t i = start + k;
-    idx[j] = i;
     const bool live = (k < count) && (a.p.state[i] == 1);
     if (live) {
       q.x[j] = a.p.x[i];
@@ -364,19 +393,21 @@ __global__ void __launch_bounds__(P >= 4 ? 256 : 512) xt_track_kernel(const Trac
       q.y[j] = a.p.y[i];
       q.py[j] = a.p.py[i];
       q.zeta[j] = a.p.zeta[i];
-      q.delta[j] = a.p.delta[i];
+      const double delta = a.p.delta[i];
       const double ptau = a.p.ptau[i];
-      ptau_s[j * ptau_stride] = ptau;
+      cold.delta(j) = delta;
+      cold.ptau(j) = ptau;
       q.alive |= 1u << j;
-      const double opd = 1.0 + q.delta[j];
+      const double opd = 1.0 + delta;
       const double b = 1.0 + a.beta0 * ptau;
       const double t = ptau * (ptau + a.tib);
-      refresh_cached<P>(q, j, opd, b, t, a.igam2);
+      refresh_cached<P>(q, cold, j, opd, b, t, a.igam2);
     } else {
-      q.x[j] = q.px[j] = q.y[j] = q.py[j] = q.zeta[j] = q.delta[j] = 0.0;
-      q.opd2[j] = q.b[j] = q.rv0v[j] = 1.0;
+      q.x[j] = q.px[j] = q.y[j] = q.py[j] = q.zeta[j] = 0.0;
+      q.opd2[j] = q.b[j] = 1.0;
       q.g[j] = 0.0;
-      ptau_s[j * ptau_stride] = 0.0;
+      cold.ptau(j) = cold.delta(j) = 0.0;
+      cold.rv0v(j) = 1.0;
     }
   }
 
@@ -398,7 +429,7 @@ __global__ void __launch_bounds__(P >= 4 ? 256 : 512) xt_track_kernel(const Trac
     mbar_wait(bar0, 0);
     for (; turns_done < a.n_turns; ++turns_done) {
       if (!__any_sync(0xffffffffu, q.alive != 0)) break;
-      track_chunk<P>(q, buf0, idx, turns_done, ptau_s, ptau_stride, a);
+      track_chunk<P>(q, buf0, cold, turns_done, a);
     }
   } else {
     const int64_t total = a.n_turns * a.n_chunks;
@@ -417,7 +448,7 @@ __global__ void __launch_bounds__(P >= 4 ? 256 : 512) xt_track_kernel(const Trac
       const uint32_t cb = static_cast<uint32_t>(gidx & 1);
       mbar_wait(bar0 + 8 * cb, static_cast<uint32_t>((gidx >> 1) & 1));
       if (__any_sync(0xffffffffu, q.alive != 0))
-        track_chunk<P>(q, buf0 + static_cast<size_t>(cb) * a.chunk_bytes, idx, turns_done, ptau_s, ptau_stride, a);
+        track_chunk<P>(q, buf0 + static_cast<size_t>(cb) * a.chunk_bytes, cold, turns_done, a);
       ++gidx;
       if (++c == a.n_chunks) {
         c = 0;
@@ -436,14 +467,14 @@ __global__ void __launch_bounds__(P >= 4 ? 256 : 512) xt_track_kernel(const Trac
 #pragma unroll
   for (int j = 0; j < P; ++j) {
     if (q.alive & (1u << j)) {
-      const int64_t i = idx[j];
+      const int64_t i = cold.idx(j);
       a.p.x[i] = q.x[j];
       a.p.px[i] = q.px[j];
       a.p.y[i] = q.y[j];
       a.p.py[i] = q.py[j];
       a.p.zeta[i] = q.zeta[j];
-      a.p.delta[i] = q.delta[j];
-      a.p.ptau[i] = ptau_s[j * ptau_stride];
+      a.p.delta[i] = cold.delta(j);
+      a.p.ptau[i] = cold.ptau(j);
       a.p.s[i] = 0.0;
       a.p.at_turn[i] += turns_done;
     }
@@ -466,11 +497,14 @@ __global__ void xt_init_derived_kernel(xt_particles p, int64_t n, double beta0, 
 
 template <int P>
 int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
-  const size_t ptau_bytes = (static_cast<size_t>(8 * P) * block + 127) & ~static_cast<size_t>(127);
-  const size_t smem = 128 + ptau_bytes + (lat->info.n_chunks == 1 ? 1 : 2) * static_cast<size_t>(lat->info.chunk_bytes);
+  const size_t cold_bytes = (static_cast<size_t>(24 * P) * block + 127) & ~static_cast<size_t>(127);
+  const size_t smem = 128 + cold_bytes + (lat->info.n_chunks == 1 ? 1 : 2) * static_cast<size_t>(lat->info.chunk_bytes);
   static bool attr_set = false;
   if (!attr_set) {
     XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    // the kernel has no use for L1 (every hot read is a shared-memory broadcast)
+    XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                 cudaSharedmemCarveoutMaxShared));
     attr_set = true;
   }
   const int64_t cap = static_cast<int64_t>(block) * P;

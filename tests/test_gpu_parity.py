@@ -262,7 +262,7 @@ def test_compaction_and_launch_chunking_do_not_change_results(X):
     assert 0.2 < (base["state"] == 0).mean() < 0.9
     variants = [dict(compact_every=37), dict(compact_every=100, turns_per_launch=7),
                 dict(compact_every=-1, turns_per_launch=1, block_size=32),
-                dict(compact_every=299, block_size=512), dict(block_size=64, turns_per_launch=150)]
+                dict(compact_every=299, block_size=256), dict(block_size=64, turns_per_launch=150)]
     for v in variants:
         p = X.new_particles(lat, coords)
         X.xt_track_ex(lat, p, 300, **v)
