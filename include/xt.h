@@ -104,11 +104,23 @@ typedef struct {
   double circumference;     /* sum of drift lengths [m]                                       */
 } xt_lattice_info;
 
+/* Options of xt_lattice_create_ex.  Zero-initialise for the defaults.  Neither changes any
+ * result: the same maps run in the same order with the same arithmetic. */
+typedef struct {
+  int64_t chunk_bytes; /* 0: default (16384); else shared-memory bytes of one staging buffer,  */
+                       /*    a multiple of 128 in [1024, 65536], at least one record + 16      */
+  int32_t fuse;        /* 0 or 1: [Drift] Multipole [Drift] share one record and one dispatch; */
+                       /*    2: one record per element                                         */
+  int32_t reserved;
+} xt_lattice_opts;
+
 /* Step P: parse + validate the packed buffer, pre-scale the multipole
  * coefficients, fold curvature into the dipole term, lay out 16-byte-aligned records in
  * Horner order, cut them into TMA chunks and copy the image to the current CUDA device.
  * The caller may free `packed` as soon as the call returns.  *out untouched on failure. */
 int xt_lattice_create(const void *packed, size_t nbytes, xt_lattice **out);
+int xt_lattice_create_ex(const void *packed, size_t nbytes, const xt_lattice_opts *opts,
+                         xt_lattice **out);
 int xt_lattice_destroy(xt_lattice *lat);
 int xt_lattice_get_info(const xt_lattice *lat, xt_lattice_info *info);
 /* s position (entrance) of every element; `out` is a HOST array of `cap` doubles; returns
@@ -116,11 +128,11 @@ int xt_lattice_get_info(const xt_lattice *lat, xt_lattice_info *info);
 int64_t xt_lattice_s_table(const xt_lattice *lat, double *out, int64_t cap);
 
 /* Host-only form of step P for tests and tools (makes NO CUDA call): packs the image exactly
- * as xt_lattice_create would upload it.  Copies min(image size, cap) bytes to `image` (HOST;
+ * as xt_lattice_create_ex would upload it.  Copies min(image size, cap) bytes to `image` (HOST;
  * may be NULL when cap == 0), fills *info if non-NULL, returns the image size in bytes or a
  * negative xt_status. */
-int64_t xt_lattice_pack_host(const void *packed, size_t nbytes, void *image, size_t cap,
-                             xt_lattice_info *info);
+int64_t xt_lattice_pack_host(const void *packed, size_t nbytes, const xt_lattice_opts *opts,
+                             void *image, size_t cap, xt_lattice_info *info);
 
 /* Steps L, S, D, M1-M4, A, T, W (+ C when compaction is active): track every particle with
  * state == 1 for n_turns turns through the whole line.  DEVICE pointers.

@@ -39,6 +39,10 @@ class xt_track_opts(ctypes.Structure):
                 ("block_size", ctypes.c_int32), ("particles_per_thread", ctypes.c_int32)]
 
 
+class xt_lattice_opts(ctypes.Structure):
+    _fields_ = [("chunk_bytes", ctypes.c_int64), ("fuse", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
 class xt_lattice_info(ctypes.Structure):
     _fields_ = [("n_elements", ctypes.c_int64), ("n_records", ctypes.c_int64),
                 ("n_chunks", ctypes.c_int64), ("image_bytes", ctypes.c_int64),
@@ -57,10 +61,13 @@ class xt_lattice_info(ctypes.Structure):
 _VP, _I64, _SZ = ctypes.c_void_p, ctypes.c_int64, ctypes.c_size_t
 SIGNATURES = {
     "xt_lattice_create": (ctypes.c_int, [ctypes.c_char_p, _SZ, ctypes.POINTER(_VP)]),
+    "xt_lattice_create_ex": (ctypes.c_int, [ctypes.c_char_p, _SZ, ctypes.POINTER(xt_lattice_opts),
+                                            ctypes.POINTER(_VP)]),
     "xt_lattice_destroy": (ctypes.c_int, [_VP]),
     "xt_lattice_get_info": (ctypes.c_int, [_VP, ctypes.POINTER(xt_lattice_info)]),
     "xt_lattice_s_table": (_I64, [_VP, _VP, _I64]),
-    "xt_lattice_pack_host": (_I64, [ctypes.c_char_p, _SZ, _VP, _SZ, ctypes.POINTER(xt_lattice_info)]),
+    "xt_lattice_pack_host": (_I64, [ctypes.c_char_p, _SZ, ctypes.POINTER(xt_lattice_opts), _VP, _SZ,
+                                    ctypes.POINTER(xt_lattice_info)]),
     "xt_track": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _VP]),
     "xt_track_ex": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _VP,
                                    ctypes.POINTER(xt_track_opts)]),
@@ -133,10 +140,27 @@ class Lattice:
             pass
 
 
+def _lattice_opts(chunk_bytes: int = 0, fuse: Optional[bool] = None):
+    if not chunk_bytes and fuse is None:
+        return None
+    return xt_lattice_opts(int(chunk_bytes), 0 if fuse is None else (1 if fuse else 2), 0)
+
+
 def xt_lattice_create(packed: bytes, kind: str = "prod") -> Lattice:
     lib = load_library(kind)
     out = _VP()
     _check(lib, lib.xt_lattice_create(packed, len(packed), ctypes.byref(out)))
+    return Lattice(out.value, lib, kind)
+
+
+def xt_lattice_create_ex(packed: bytes, kind: str = "prod", *, chunk_bytes: int = 0,
+                         fuse: Optional[bool] = None) -> Lattice:
+    """As ``xt_lattice_create`` with a staging-buffer size and/or record fusion switched off
+    (``fuse=False``); neither changes any result."""
+    lib = load_library(kind)
+    out = _VP()
+    o = _lattice_opts(chunk_bytes, fuse)
+    _check(lib, lib.xt_lattice_create_ex(packed, len(packed), ctypes.byref(o) if o else None, ctypes.byref(out)))
     return Lattice(out.value, lib, kind)
 
 
@@ -157,15 +181,18 @@ def xt_lattice_s_table(lat: Lattice) -> np.ndarray:
     return out
 
 
-def xt_lattice_pack_host(packed: bytes, kind: str = "prod"):
+def xt_lattice_pack_host(packed: bytes, kind: str = "prod", *, chunk_bytes: int = 0,
+                         fuse: Optional[bool] = None):
     """(image bytes, info dict) of the device image; makes no CUDA call."""
     lib = load_library(kind)
     info = xt_lattice_info()
-    n = lib.xt_lattice_pack_host(packed, len(packed), None, 0, ctypes.byref(info))
+    o = _lattice_opts(chunk_bytes, fuse)
+    op = ctypes.byref(o) if o else None
+    n = lib.xt_lattice_pack_host(packed, len(packed), op, None, 0, ctypes.byref(info))
     if n < 0:
         _check(lib, int(n))
     buf = ctypes.create_string_buffer(int(n))
-    lib.xt_lattice_pack_host(packed, len(packed), buf, int(n), ctypes.byref(info))
+    lib.xt_lattice_pack_host(packed, len(packed), op, buf, int(n), ctypes.byref(info))
     return buf.raw, info.as_dict()
 
 

@@ -15,8 +15,19 @@ namespace xt {
 
 // ------------------------------------------------------------------ device lattice image
 // The image is a byte stream of 16-byte-aligned records, cut into chunks of at most
-// chunk_bytes; every chunk ends with a TAG_END record so that the kernel's element loop
-// needs no counter.  Record = 16-byte header {u32 tag; u32 elem; f64 p0} + 16-byte slots:
+// chunk_bytes (one TMA bulk copy each).  A chunk is a 16-byte preamble followed by records.
+// Preamble and every record start with a 16-byte header {u32 next; u32 elem; f64 p0}:
+// `next` is the tag of the record that FOLLOWS (TAG_END after the last record of the chunk),
+// so the kernel's dispatch never waits for the load of the record it is about to enter;
+// elem and p0 belong to the record itself (unused in the preamble).
+//
+//   tag = type | flags | (order << 8) | (record bytes << 16)
+//
+// A multipole record may carry the drift before it (TAG_PRE) and one or two drifts after it
+// (TAG_POST, TAG_POST + TAG_POST2): then one slot {l_pre, l_post} follows the header, and a
+// slot {l_post2, 0} after that with TAG_POST2.  The maps are applied in element order with
+// unchanged arithmetic; the dispatch is shared, and so is what two consecutive drifts would
+// both compute from the unchanged (px, py).  16-byte slots after that:
 //
 //   TAG_DRIFT    p0 = length                                                     16 B
 //   TAG_MULT     p0 unused; (c[n], s[n]) pairs, n = N .. 0 (Horner order)        16 + 16(N+1)
@@ -26,11 +37,9 @@ namespace xt {
 //   TAG_SHIFT    p0 unused; {dx, dy}                                             32 B
 //   TAG_RECT     p0 unused; {min_x, max_x}; {min_y, max_y}                       48 B
 //   TAG_ELLIPSE  p0 = a2*b2; {b2, a2}                                            32 B
-//   TAG_END      end of chunk                                                    16 B
 //
-// tag = type | (order << 8) | (record bytes << 16); elem = index of the element in the user's
-// packed buffer.  The size field lets the kernel step to (and prefetch) the next header
-// without decoding the type first.
+// elem = index of the element in the user's packed buffer (for a fused record: the
+// multipole's; only aperture records ever report it).
 enum : uint32_t {
   TAG_END = 0,
   TAG_DRIFT = 1,
@@ -40,11 +49,15 @@ enum : uint32_t {
   TAG_SHIFT = 5,
   TAG_RECT = 6,
   TAG_ELLIPSE = 7,
-  TAG_CMULT = 8
+  TAG_CMULT = 8,
+  TAG_TYPE_MASK = 0xf,
+  TAG_PRE = 0x10,   // a drift of length l_pre comes first
+  TAG_POST = 0x20,  // a drift of length l_post follows the kick
+  TAG_POST2 = 0x40  // ... and a second one of length l_post2 (only with TAG_POST)
 };
 
 struct alignas(16) RecHdr {
-  uint32_t tag;
+  uint32_t next;
   uint32_t elem;
   double p0;
 };
@@ -99,7 +112,11 @@ struct HostImage {
   xt_lattice_info info{};
   RefConsts k{};
 };
-int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImage &out);
+struct PackOpts {
+  uint32_t chunk_bytes = kDefaultChunkBytes;
+  bool fuse = true;
+};
+int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImage &out);
 
 // xt_track.cu
 // block: threads per CTA; ppt: particles per thread (1, 2 or 4; 4 needs block <= 256)

@@ -43,26 +43,27 @@ struct Reader {
   }
 };
 
-// One record under construction: header + 16-byte slots of two doubles.
-struct RecBuilder {
-  std::vector<unsigned char> bytes;
-  void header(uint32_t type, uint32_t order, uint32_t elem, double p0) {
-    RecHdr h;
-    h.tag = type | (order << 8);
-    h.elem = elem;
-    h.p0 = p0;
-    bytes.resize(sizeof(RecHdr));
-    std::memcpy(bytes.data(), &h, sizeof(RecHdr));
-  }
+// One record of the device image before serialisation.
+struct Rec {
+  uint32_t type = TAG_END;
+  uint32_t order = 0;
+  uint32_t flags = 0;   // TAG_PRE / TAG_POST
+  uint32_t elem = 0;
+  double p0 = 0.0;
+  double l_pre = 0.0, l_post = 0.0, l_post2 = 0.0;
+  std::vector<double> slots;  // pairs, in the order the kernel reads them
   void slot(double a, double b) {
-    const double v[2] = {a, b};
-    const size_t at = bytes.size();
-    bytes.resize(at + 16);
-    std::memcpy(bytes.data() + at, v, 16);
+    slots.push_back(a);
+    slots.push_back(b);
   }
+  uint32_t bytes() const {
+    return static_cast<uint32_t>(sizeof(RecHdr) + (flags ? 16 : 0) + ((flags & TAG_POST2) ? 16 : 0) +
+                                 slots.size() * sizeof(double));
+  }
+  uint32_t tag() const { return type | flags | (order << 8) | (bytes() << 16); }
 };
 
-double inv_scale_factorial(int n) {  // n! as an exactly representable double (n <= 22)
+double factorial(int n) {  // n! as an exactly representable double (n <= 22)
   double f = 1.0;
   for (int i = 2; i <= n; ++i) f *= static_cast<double>(i);
   return f;
@@ -70,9 +71,14 @@ double inv_scale_factorial(int n) {  // n! as an exactly representable double (n
 
 }  // namespace
 
-int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImage &out) {
+int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImage &out) {
   if (!packed) {
     set_error("xt_lattice_create: packed buffer is NULL");
+    return XT_ERR_INVALID_ARG;
+  }
+  const uint32_t chunk_bytes = opts.chunk_bytes;
+  if (chunk_bytes < 1024 || chunk_bytes > 65536 || (chunk_bytes % 128) != 0) {
+    set_error("xt_lattice_create_ex: chunk_bytes must be a multiple of 128 in [1024, 65536]");
     return XT_ERR_INVALID_ARG;
   }
   Reader r{static_cast<const unsigned char *>(packed), nbytes, 0};
@@ -118,46 +124,25 @@ int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImag
   out.chunks.clear();
   out.s_table.assign(n_elements, 0.0);
 
-  const RecHdr end_rec{TAG_END | (static_cast<uint32_t>(sizeof(RecHdr)) << 16), 0u, 0.0};
-  size_t chunk_start = 0;
-  auto close_chunk = [&]() {
-    const size_t at = out.image.size();
-    out.image.resize(at + sizeof(RecHdr));
-    std::memcpy(out.image.data() + at, &end_rec, sizeof(RecHdr));
-    ChunkDesc d;
-    d.offset = chunk_start;
-    d.nbytes = static_cast<uint32_t>(out.image.size() - chunk_start);
-    d.pad = 0;
-    out.chunks.push_back(d);
-    chunk_start = out.image.size();
-  };
-  auto append = [&](const RecBuilder &rb) {
-    // keep room for the TAG_END record that closes the chunk
-    if (out.image.size() - chunk_start + rb.bytes.size() + sizeof(RecHdr) > chunk_bytes) close_chunk();
-    const size_t at = out.image.size();
-    out.image.insert(out.image.end(), rb.bytes.begin(), rb.bytes.end());
-    uint32_t tag;  // patch the record size into the upper half of the tag
-    std::memcpy(&tag, out.image.data() + at, 4);
-    tag |= static_cast<uint32_t>(rb.bytes.size()) << 16;
-    std::memcpy(out.image.data() + at, &tag, 4);
-    info.n_records += 1;
-  };
-
+  // ---- pass 1: one record per element (markers are the identity map: no record)
+  std::vector<Rec> recs;
+  recs.reserve(n_elements);
   double s_pos = 0.0;
-  RecBuilder rb;
   for (uint32_t ie = 0; ie < n_elements; ++ie) {
     const uint32_t type = r.get<uint32_t>();
     const uint32_t aux = r.get<uint32_t>();
     if (!r.ok) break;
     out.s_table[ie] = s_pos;
     if (type <= XT_LIMITELLIPSE) info.n_by_type[type] += 1;
+    Rec rec;
+    rec.elem = ie;
     switch (type) {
       case XT_MARKER:
-        break;  // no record: a marker is the identity map
+        continue;
       case XT_DRIFT: {
         const double length = r.real();
-        rb.header(TAG_DRIFT, 0, ie, length);
-        append(rb);
+        rec.type = TAG_DRIFT;
+        rec.p0 = length;
         s_pos += length;
         break;
       }
@@ -175,22 +160,23 @@ int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImag
         if (!r.ok) break;
         double cn[XT_MAX_ORDER + 1], sn[XT_MAX_ORDER + 1];
         for (int n = 0; n <= order; ++n) {
-          const double f = inv_scale_factorial(n);
+          const double f = factorial(n);
           cn[n] = knl[n] / f;
           sn[n] = ksl[n] / f;
         }
+        rec.order = aux;
         if (hxl != 0.0) {
           // -k0l + hxl(1+delta) = -(k0l - hxl) + hxl*delta : fold the constant part into c[0]
           cn[0] = knl[0] - hxl;
           const double wf = (length != 0.0) ? (knl[0] * hxl) / length : 0.0;
-          rb.header(TAG_CMULT, aux, ie, hxl);
-          rb.slot(wf, 0.0);
+          rec.type = TAG_CMULT;
+          rec.p0 = hxl;
+          rec.slot(wf, 0.0);
           info.n_curved += 1;
         } else {
-          rb.header(TAG_MULT, aux, ie, 0.0);
+          rec.type = TAG_MULT;
         }
-        for (int n = order; n >= 0; --n) rb.slot(cn[n], sn[n]);  // Horner order: highest first
-        append(rb);
+        for (int n = order; n >= 0; --n) rec.slot(cn[n], sn[n]);  // Horner order: highest first
         info.sum_order += order;
         break;
       }
@@ -198,28 +184,23 @@ int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImag
         const double volt = r.real();
         const double freq = r.real();
         const double lag_deg = r.real();
-        const double lag_rad = lag_deg * (kPi / 180.0);
-        const double kz = (2.0 * kPi * freq) / (beta0 * kClight);
-        const double vn = (q0 * volt) / p0c;
-        rb.header(TAG_CAVITY, 0, ie, lag_rad);
-        rb.slot(kz, vn);
-        append(rb);
+        rec.type = TAG_CAVITY;
+        rec.p0 = lag_deg * (kPi / 180.0);                                    // lag_rad
+        rec.slot((2.0 * kPi * freq) / (beta0 * kClight), (q0 * volt) / p0c);  // kz, vn
         break;
       }
       case XT_SROTATION: {
         const double cz = r.real();
         const double sz = r.real();
-        rb.header(TAG_SROT, 0, ie, 0.0);
-        rb.slot(cz, sz);
-        append(rb);
+        rec.type = TAG_SROT;
+        rec.slot(cz, sz);
         break;
       }
       case XT_XYSHIFT: {
         const double dx = r.real();
         const double dy = r.real();
-        rb.header(TAG_SHIFT, 0, ie, 0.0);
-        rb.slot(dx, dy);
-        append(rb);
+        rec.type = TAG_SHIFT;
+        rec.slot(dx, dy);
         break;
       }
       case XT_LIMITRECT: {
@@ -227,10 +208,9 @@ int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImag
         const double max_x = r.real();
         const double min_y = r.real();
         const double max_y = r.real();
-        rb.header(TAG_RECT, 0, ie, 0.0);
-        rb.slot(min_x, max_x);
-        rb.slot(min_y, max_y);
-        append(rb);
+        rec.type = TAG_RECT;
+        rec.slot(min_x, max_x);
+        rec.slot(min_y, max_y);
         info.has_aperture = 1;
         break;
       }
@@ -239,9 +219,9 @@ int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImag
         const double b = r.real();
         const double a2 = a * a;
         const double b2 = b * b;
-        rb.header(TAG_ELLIPSE, 0, ie, a2 * b2);
-        rb.slot(b2, a2);
-        append(rb);
+        rec.type = TAG_ELLIPSE;
+        rec.p0 = a2 * b2;
+        rec.slot(b2, a2);
         info.has_aperture = 1;
         break;
       }
@@ -250,6 +230,7 @@ int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImag
         return XT_ERR_BAD_LATTICE;
     }
     if (!r.ok) break;
+    recs.push_back(std::move(rec));
   }
   if (!r.ok) {
     set_error("xt_lattice_create: truncated buffer or non-finite parameter");
@@ -259,23 +240,133 @@ int pack_image(const void *packed, size_t nbytes, uint32_t chunk_bytes, HostImag
     set_error("xt_lattice_create: trailing bytes after the last element record");
     return XT_ERR_BAD_LATTICE;
   }
-  close_chunk();  // also yields one END-only chunk for an empty / marker-only line
+  info.circumference = s_pos;
+
+  // ---- pass 2: fuse [Drift] Multipole [Drift] into one record.  The maps are applied in
+  // the same order with the same arithmetic; only the dispatch is shared (a thin lattice is
+  // mostly drift-kick-drift).
+  std::vector<Rec> fused;
+  fused.reserve(recs.size());
+  auto is_mult = [&](size_t k) { return k < recs.size() && (recs[k].type == TAG_MULT || recs[k].type == TAG_CMULT); };
+  auto is_drift = [&](size_t k) { return k < recs.size() && recs[k].type == TAG_DRIFT; };
+  for (size_t i = 0; i < recs.size();) {
+    const bool pre = is_drift(i) && is_mult(i + 1);
+    if (opts.fuse && (pre || is_mult(i))) {
+      Rec m = std::move(recs[pre ? i + 1 : i]);
+      if (pre) {
+        m.flags |= TAG_PRE;
+        m.l_pre = recs[i].p0;
+      }
+      i += pre ? 2 : 1;
+      if (is_drift(i)) {
+        m.flags |= TAG_POST;
+        m.l_post = recs[i++].p0;
+        // a second drift shares the first one's evaluation (px, py unchanged in between)
+        if (is_drift(i)) {
+          m.flags |= TAG_POST2;
+          m.l_post2 = recs[i++].p0;
+        }
+      }
+      fused.push_back(std::move(m));
+    } else {
+      fused.push_back(std::move(recs[i]));
+      i += 1;
+    }
+  }
+  info.n_records = static_cast<int64_t>(fused.size());
+
+  // ---- pass 3: serialise.  Chunk = 16-byte preamble {tag of the first record} + records;
+  // every record header carries the tag of the record that FOLLOWS it (TAG_END after the last
+  // one of the chunk), so the kernel knows where it is going before it gets there.
+  auto put_header = [&](size_t at, uint32_t next_tag, uint32_t elem, double p0) {
+    RecHdr h;
+    h.next = next_tag;
+    h.elem = elem;
+    h.p0 = p0;
+    std::memcpy(out.image.data() + at, &h, sizeof(RecHdr));
+  };
+  size_t i = 0;
+  do {
+    const size_t chunk_start = out.image.size();
+    out.image.resize(chunk_start + sizeof(RecHdr));
+    size_t prev_hdr = chunk_start;  // where the next record's tag goes
+    uint32_t prev_elem = 0;
+    double prev_p0 = 0.0;
+    while (i < fused.size()) {
+      const Rec &rec = fused[i];
+      const uint32_t nb = rec.bytes();
+      if (sizeof(RecHdr) + nb > chunk_bytes) {
+        set_error("xt_lattice_create_ex: chunk_bytes is smaller than one record");
+        return XT_ERR_INVALID_ARG;
+      }
+      if (out.image.size() - chunk_start + nb > chunk_bytes) break;
+      put_header(prev_hdr, rec.tag(), prev_elem, prev_p0);
+      const size_t at = out.image.size();
+      out.image.resize(at + nb);
+      size_t w = at + sizeof(RecHdr);
+      if (rec.flags) {
+        const double l[2] = {rec.l_pre, rec.l_post};
+        std::memcpy(out.image.data() + w, l, 16);
+        w += 16;
+      }
+      if (rec.flags & TAG_POST2) {
+        const double l[2] = {rec.l_post2, 0.0};
+        std::memcpy(out.image.data() + w, l, 16);
+        w += 16;
+      }
+      if (!rec.slots.empty()) std::memcpy(out.image.data() + w, rec.slots.data(), rec.slots.size() * sizeof(double));
+      prev_hdr = at;
+      prev_elem = rec.elem;
+      prev_p0 = rec.p0;
+      ++i;
+    }
+    put_header(prev_hdr, TAG_END, prev_elem, prev_p0);
+    ChunkDesc d;
+    d.offset = chunk_start;
+    d.nbytes = static_cast<uint32_t>(out.image.size() - chunk_start);
+    d.pad = 0;
+    out.chunks.push_back(d);
+  } while (i < fused.size());
   info.n_chunks = static_cast<int64_t>(out.chunks.size());
   info.image_bytes = static_cast<int64_t>(out.image.size());
-  info.circumference = s_pos;
   return XT_OK;
 }
 
 }  // namespace xt
 
 // ------------------------------------------------------------------------------ C ABI
+namespace xt {
+namespace {
+int resolve_pack_opts(const xt_lattice_opts *o, PackOpts &po) {
+  po.chunk_bytes = kDefaultChunkBytes;
+  po.fuse = true;
+  if (!o) return XT_OK;
+  if (o->chunk_bytes < 0 || o->fuse < 0 || o->fuse > 2) {
+    set_error("xt_lattice_create_ex: chunk_bytes must be >= 0 and fuse one of 0 (default), 1 (on), 2 (off)");
+    return XT_ERR_INVALID_ARG;
+  }
+  if (o->chunk_bytes > 0) po.chunk_bytes = static_cast<uint32_t>(o->chunk_bytes);
+  if (o->fuse == 2) po.fuse = false;
+  return XT_OK;
+}
+}  // namespace
+}  // namespace xt
+
 extern "C" int xt_lattice_create(const void *packed, size_t nbytes, xt_lattice **out) {
+  return xt_lattice_create_ex(packed, nbytes, nullptr, out);
+}
+
+extern "C" int xt_lattice_create_ex(const void *packed, size_t nbytes, const xt_lattice_opts *opts,
+                                    xt_lattice **out) {
   if (!out) {
     xt::set_error("xt_lattice_create: out is NULL");
     return XT_ERR_INVALID_ARG;
   }
+  xt::PackOpts po;
+  int rc = xt::resolve_pack_opts(opts, po);
+  if (rc != XT_OK) return rc;
   xt::HostImage img;
-  int rc = xt::pack_image(packed, nbytes, xt::kDefaultChunkBytes, img);
+  rc = xt::pack_image(packed, nbytes, po, img);
   if (rc != XT_OK) return rc;
 
   xt_lattice *lat = new (std::nothrow) xt_lattice;
@@ -343,14 +434,17 @@ extern "C" int64_t xt_lattice_s_table(const xt_lattice *lat, double *out, int64_
   return n;
 }
 
-extern "C" int64_t xt_lattice_pack_host(const void *packed, size_t nbytes, void *image, size_t cap,
-                                        xt_lattice_info *info) {
+extern "C" int64_t xt_lattice_pack_host(const void *packed, size_t nbytes, const xt_lattice_opts *opts,
+                                        void *image, size_t cap, xt_lattice_info *info) {
   if (cap > 0 && !image) {
     xt::set_error("xt_lattice_pack_host: image is NULL but cap > 0");
     return XT_ERR_INVALID_ARG;
   }
+  xt::PackOpts po;
+  int rc = xt::resolve_pack_opts(opts, po);
+  if (rc != XT_OK) return rc;
   xt::HostImage img;
-  const int rc = xt::pack_image(packed, nbytes, xt::kDefaultChunkBytes, img);
+  rc = xt::pack_image(packed, nbytes, po, img);
   if (rc != XT_OK) return rc;
   const size_t n = img.image.size() < cap ? img.image.size() : cap;
   if (n) std::memcpy(image, img.image.data(), n);

@@ -75,6 +75,20 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       : "memory");
 }
 
+// a*b + c and c - a*b.  The validation build rounds the product and the sum separately, as
+// the oracle does; the production build fuses them, explicitly, so that the arithmetic does
+// not depend on which contractions the compiler happens to pick in each instantiation
+// (results are bit-identical for every launch shape).  XT_MUL is a product that is never
+// fused into a neighbouring sum.
+#ifdef XT_FMAD_OFF
+#define XT_MADD(a, b, c) ((a) * (b) + (c))
+#define XT_NMADD(a, b, c) ((c) - (a) * (b))
+#else
+#define XT_MADD(a, b, c) fma((a), (b), (c))
+#define XT_NMADD(a, b, c) fma(-(a), (b), (c))
+#endif
+#define XT_MUL(a, b) __dmul_rn((a), (b))
+
 #ifndef XT_FMAD_OFF
 // MUFU.RSQ64H / MUFU.RCP64H: ~20-bit seeds computed from the high word of the operand.
 __device__ __forceinline__ double rsqrt_seed(double a) {
@@ -128,8 +142,8 @@ __device__ __forceinline__ void horner_step(const double2 c, const double (&x)[P
                                             double (&re)[P], double (&im)[P]) {
 #pragma unroll
   for (int j = 0; j < P; ++j) {
-    const double nre = re[j] * x[j] + (c.x - im[j] * y[j]);
-    const double nim = re[j] * y[j] + (c.y + im[j] * x[j]);
+    const double nre = XT_MADD(re[j], x[j], XT_NMADD(im[j], y[j], c.x));  // re*x + (c - im*y)
+    const double nim = XT_MADD(re[j], y[j], XT_MADD(im[j], x[j], c.y));   // re*y + (s + im*x)
     re[j] = nre;
     im[j] = nim;
   }
@@ -192,54 +206,102 @@ __device__ __forceinline__ void lose(Parts<P> &q, uint32_t out, const Cold<P> &c
   q.alive &= ~out;
 }
 
+// M1 exact drift, cancellation-free zeta (DESIGN.md section 5 "Drift"), in two halves.
+// drift_eval computes what depends on (px, py, delta, ptau) only; drift_apply advances
+// x, y, zeta by one length.  A drift changes none of the inputs of drift_eval, so
+// consecutive drifts share one evaluation: the values are the ones each drift would have
+// recomputed, bit for bit.
+template <int P>
+struct DriftCoef {
+  double u[P], v[P], gm[P];  // validation: 1/(pz (pz + b)), pz + b;  production: 1/pz, 1/(pz + b);  g - pxy2
+};
+
+template <int P>
+__device__ __forceinline__ void drift_eval(const Parts<P> &q, DriftCoef<P> &d) {
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    const double t1 = XT_MUL(q.px[j], q.px[j]);
+    const double pxy2 = XT_MADD(q.py[j], q.py[j], t1);
+    const double rad = q.opd2[j] - pxy2;
+#ifdef XT_FMAD_OFF
+    const double pz = sqrt(rad);
+    const double s1 = pz + q.b[j];
+    const double den = pz * s1;
+    d.u[j] = 1.0 / den;
+    d.v[j] = s1;
+#else
+    // 1/pz by one cubic Newton step on the RSQ seed; 1/(pz + b) likewise on the RCP seed
+    const double r0 = rsqrt_seed(rad);
+    const double e = fma(-rad, XT_MUL(r0, r0), 1.0);
+    const double r1 = fma(fma(e, 0.375, 0.5), XT_MUL(r0, e), r0);  // 1/pz
+    const double s1 = fma(rad, r1, q.b[j]);                        // pz + b
+    const double y0 = rcp_seed(s1);
+    const double f = fma(-s1, y0, 1.0);
+    d.u[j] = r1;
+    d.v[j] = fma(y0, fma(f, f, f), y0);                            // 1/(pz + b)
+#endif
+    d.gm[j] = q.g[j] - pxy2;
+  }
+}
+
+template <int P>
+__device__ __forceinline__ void drift_apply(Parts<P> &q, const DriftCoef<P> &d, const double length) {
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+#ifdef XT_FMAD_OFF
+    const double lr = length * d.u[j];   // L/(pz (pz + b))
+    const double lpz = lr * d.v[j];      // L/pz
+#else
+    const double lpz = XT_MUL(length, d.u[j]);
+    const double lr = XT_MUL(lpz, d.v[j]);
+#endif
+    q.x[j] = XT_MADD(q.px[j], lpz, q.x[j]);
+    q.y[j] = XT_MADD(q.py[j], lpz, q.y[j]);
+    q.zeta[j] = XT_MADD(d.gm[j], lr, q.zeta[j]);
+  }
+}
+
+template <int P>
+__device__ __forceinline__ void drift(Parts<P> &q, const double length) {
+  DriftCoef<P> d;
+  drift_eval<P>(q, d);
+  drift_apply<P>(q, d, length);
+}
+
+// The drifts a multipole record carries behind the kick (TAG_POST, TAG_POST2).
+template <int P>
+__device__ __forceinline__ void drifts_after(Parts<P> &q, uint32_t tag, const double l1, const double2 *slots2) {
+  if (tag & TAG_POST) {
+    DriftCoef<P> d;
+    drift_eval<P>(q, d);
+    drift_apply<P>(q, d, l1);
+    if (tag & TAG_POST2) drift_apply<P>(q, d, slots2->x);
+  }
+}
+
 // Push the P particles of this thread through every record of one staged chunk.
 template <int P>
 __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp, const Cold<P> &cold,
                                             int64_t turns_done, const TrackArgs &a) {
-  RecHdr h = *reinterpret_cast<const RecHdr *>(rp);
-  for (;;) {
-    const uint32_t type = h.tag & 0xffu;
-    if (type == TAG_END) break;
+  uint32_t tag = reinterpret_cast<const RecHdr *>(rp)->next;  // chunk preamble
+  rp += sizeof(RecHdr);
+  while ((tag & TAG_TYPE_MASK) != TAG_END) {
+    const RecHdr h = *reinterpret_cast<const RecHdr *>(rp);  // {tag of the NEXT record, elem, p0}
     const double2 *slots = reinterpret_cast<const double2 *>(rp + sizeof(RecHdr));
     const double p0 = h.p0;
-    const uint32_t tag = h.tag;
     const uint32_t elem = h.elem;
-    rp += tag >> 16;                              // record size in bytes
-    h = *reinterpret_cast<const RecHdr *>(rp);    // prefetch the next header behind this map
-    switch (type) {
+    rp += tag >> 16;  // record size in bytes
+    switch (tag & TAG_TYPE_MASK) {
       case TAG_DRIFT: {
-        // M1 exact drift, cancellation-free zeta (DESIGN.md section 5 "Drift")
-#pragma unroll
-        for (int j = 0; j < P; ++j) {
-          const double t1 = q.px[j] * q.px[j];
-          const double pxy2 = q.py[j] * q.py[j] + t1;
-          const double rad = q.opd2[j] - pxy2;
-#ifdef XT_FMAD_OFF
-          const double pz = sqrt(rad);
-          const double s1 = pz + q.b[j];
-          const double den = pz * s1;
-          const double rr = 1.0 / den;
-          const double lr = p0 * rr;
-          const double lpz = lr * s1;
-#else
-          // 1/pz by one cubic Newton step on the RSQ seed; 1/(pz + b) likewise on the RCP seed
-          const double r0 = rsqrt_seed(rad);
-          const double e = fma(-rad, r0 * r0, 1.0);
-          const double r1 = fma(fma(e, 0.375, 0.5), r0 * e, r0);    // 1/pz
-          const double s1 = fma(rad, r1, q.b[j]);                  // pz + b
-          const double y0 = rcp_seed(s1);
-          const double f = fma(-s1, y0, 1.0);
-          const double y1 = fma(y0, fma(f, f, f), y0);             // 1/(pz + b)
-          const double lpz = p0 * r1;                              // L/pz
-          const double lr = lpz * y1;                              // L/(pz (pz + b))
-#endif
-          q.x[j] = q.px[j] * lpz + q.x[j];
-          q.y[j] = q.py[j] * lpz + q.y[j];
-          q.zeta[j] = (q.g[j] - pxy2) * lr + q.zeta[j];
-        }
+        drift<P>(q, p0);
         break;
       }
       case TAG_MULT: {
+        double2 dl = make_double2(0.0, 0.0);
+        const double2 *l2 = slots + 1;
+        if (tag & (TAG_PRE | TAG_POST)) dl = *slots++;
+        if (tag & TAG_POST2) ++slots;
+        if (tag & TAG_PRE) drift<P>(q, dl.x);
         double re[P], im[P];
         horner<P>(slots, static_cast<int>((tag >> 8) & 0xffu), q.x, q.y, re, im);
 #pragma unroll
@@ -247,9 +309,15 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
           q.px[j] = q.px[j] - re[j];
           q.py[j] = q.py[j] + im[j];
         }
+        drifts_after<P>(q, tag, dl.y, l2);
         break;
       }
       case TAG_CMULT: {
+        double2 dl = make_double2(0.0, 0.0);
+        const double2 *l2 = slots + 1;
+        if (tag & (TAG_PRE | TAG_POST)) dl = *slots++;
+        if (tag & TAG_POST2) ++slots;
+        if (tag & TAG_PRE) drift<P>(q, dl.x);
         const double hxl = p0;
         const double wf = slots[0].x;
         double re[P], im[P], delta[P], rv0v[P];
@@ -263,10 +331,11 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         for (int j = 0; j < P; ++j) {
           q.px[j] = q.px[j] - re[j];
           q.py[j] = q.py[j] + im[j];
-          q.px[j] = hxl * delta[j] + q.px[j];
-          q.px[j] = q.px[j] - wf * q.x[j];
-          q.zeta[j] = q.zeta[j] - (hxl * q.x[j]) * rv0v[j];
+          q.px[j] = XT_MADD(hxl, delta[j], q.px[j]);
+          q.px[j] = XT_NMADD(wf, q.x[j], q.px[j]);
+          q.zeta[j] = XT_NMADD(XT_MUL(hxl, q.x[j]), rv0v[j], q.zeta[j]);
         }
+        drifts_after<P>(q, tag, dl.y, l2);
         break;
       }
       case TAG_CAVITY: {
@@ -274,12 +343,12 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
 #pragma unroll
         for (int j = 0; j < P; ++j) {
           if (q.alive & (1u << j)) {
-            const double phase = p0 - kv.x * q.zeta[j];
-            const double ptau = kv.y * sin(phase) + cold.ptau(j);
-            const double t = ptau * (ptau + a.tib);
+            const double phase = XT_NMADD(kv.x, q.zeta[j], p0);
+            const double ptau = XT_MADD(kv.y, sin(phase), cold.ptau(j));
+            const double t = XT_MUL(ptau, ptau + a.tib);
             const double delta = t / (sqrt(t + 1.0) + 1.0);
             const double opd = 1.0 + delta;
-            const double b = 1.0 + a.beta0 * ptau;
+            const double b = XT_MADD(a.beta0, ptau, 1.0);
             cold.ptau(j) = ptau;
             cold.delta(j) = delta;
             a.p.rpp[cold.idx(j)] = 1.0 / opd;
@@ -293,10 +362,10 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         const double2 cs = slots[0];  // (cos_z, sin_z)
 #pragma unroll
         for (int j = 0; j < P; ++j) {
-          const double nx = cs.x * q.x[j] + cs.y * q.y[j];
-          const double ny = cs.x * q.y[j] - cs.y * q.x[j];
-          const double npx = cs.x * q.px[j] + cs.y * q.py[j];
-          const double npy = cs.x * q.py[j] - cs.y * q.px[j];
+          const double nx = XT_MADD(cs.x, q.x[j], XT_MUL(cs.y, q.y[j]));
+          const double ny = XT_MADD(cs.x, q.y[j], -XT_MUL(cs.y, q.x[j]));
+          const double npx = XT_MADD(cs.x, q.px[j], XT_MUL(cs.y, q.py[j]));
+          const double npy = XT_MADD(cs.x, q.py[j], -XT_MUL(cs.y, q.px[j]));
           q.x[j] = nx;
           q.y[j] = ny;
           q.px[j] = npx;
@@ -330,7 +399,7 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         uint32_t out = 0;
 #pragma unroll
         for (int j = 0; j < P; ++j) {
-          const double tt = (q.x[j] * q.x[j]) * ba.x + (q.y[j] * q.y[j]) * ba.y;
+          const double tt = XT_MADD(XT_MUL(q.x[j], q.x[j]), ba.x, XT_MUL(XT_MUL(q.y[j], q.y[j]), ba.y));
           out |= (tt <= p0) ? 0u : (1u << j);
         }
         out &= q.alive;
@@ -340,6 +409,7 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
       default:  // cannot happen: the packer emits only the tags above
         break;
     }
+    tag = h.next;
   }
 }
 
@@ -399,8 +469,8 @@ __global__ void __launch_bounds__(kMaxBlock, P == 4 ? XT_MINB4 : (P == 2 ? XT_MI
       cold.ptau(j) = ptau;
       q.alive |= 1u << j;
       const double opd = 1.0 + delta;
-      const double b = 1.0 + a.beta0 * ptau;
-      const double t = ptau * (ptau + a.tib);
+      const double b = XT_MADD(a.beta0, ptau, 1.0);
+      const double t = XT_MUL(ptau, ptau + a.tib);
       refresh_cached<P>(q, cold, j, opd, b, t, a.igam2);
     } else {
       q.x[j] = q.px[j] = q.y[j] = q.py[j] = q.zeta[j] = 0.0;

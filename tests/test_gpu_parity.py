@@ -275,6 +275,32 @@ def test_compaction_and_launch_chunking_do_not_change_results(X):
     lat.close()
 
 
+def test_launch_shape_fusion_and_chunk_size_do_not_change_results(X):
+    """Particles per thread, CTA size, record fusion and the staging-buffer size only change
+    how the work is laid out: every variant must reproduce the default bit for bit."""
+    full = C.particles(4)
+    idx = np.linspace(0, len(full["x"]) - 1, 2777).astype(np.int64)     # ragged: not a multiple of 32
+    coords = C.subsample(full, idx)
+    buf = packed(4)
+    lat = X.xt_lattice_create(buf)
+    base = X.new_particles(lat, coords)
+    X.xt_track_ex(lat, base, 6, compact_every=-1)
+    base = X.particles_to_host(base)
+    assert 0.05 < (base["state"] == 0).mean() < 0.95
+    for ppt in (1, 2, 4):
+        for block in (32, 96, 256):
+            p = X.new_particles(lat, coords)
+            X.xt_track_ex(lat, p, 6, compact_every=-1, block_size=block, particles_per_thread=ppt)
+            assert_bit_identical(X.particles_to_host(p), base)
+    lat.close()
+    for kw in (dict(fuse=False), dict(chunk_bytes=1024), dict(chunk_bytes=65536), dict(chunk_bytes=4224, fuse=False)):
+        lat2 = X.xt_lattice_create_ex(buf, **kw)
+        p = X.new_particles(lat2, coords)
+        X.xt_track_ex(lat2, p, 6, compact_every=4, particles_per_thread=2)
+        assert_bit_identical(X.particles_to_host(p), base)
+        lat2.close()
+
+
 def test_multi_chunk_compaction_cfg4(X):
     full = C.particles(4)
     idx = np.linspace(0, len(full["x"]) - 1, 3001).astype(np.int64)
