@@ -23,13 +23,17 @@ namespace xt {
 //
 //   tag = type | flags | (order << 8) | (record bytes << 16)
 //
-// A multipole record may carry the drift before it (TAG_PRE) and one or two drifts after it
-// (TAG_POST, TAG_POST + TAG_POST2): then one slot {l_pre, l_post} follows the header, and a
-// slot {l_post2, 0} after that with TAG_POST2.  The maps are applied in element order with
-// unchanged arithmetic; the dispatch is shared, and so is what two consecutive drifts would
-// both compute from the unchanged (px, py).  16-byte slots after that:
+// Fused records.  A multipole record may carry its neighbours: the drift before it
+// (TAG_PRE), the XYShift + SRotation before and SRotation + XYShift after it (TAG_MISAL: a
+// misaligned magnet), and one or two drifts after it (TAG_POST, + TAG_POST2).
+// A drift record may carry a second drift (TAG_POST).  The maps are applied in element order
+// with unchanged arithmetic; the dispatch is shared, and so is what two consecutive drifts
+// would both compute from the unchanged (px, py).  Slots of a multipole record, in order:
+//   {l_pre, l_post} if PRE|POST; {l_post2, 0} if POST2; {dx, dy}, {cos, sin} if MISAL;
+//   {wf, 0} if TAG_CMULT; the N+1 coefficient pairs; {cos', sin'}, {dx', dy'} if MISAL.
+// Unfused records:
 //
-//   TAG_DRIFT    p0 = length                                                     16 B
+//   TAG_DRIFT    p0 = length; {l_2nd, 0} with TAG_POST                           16 B (32 B)
 //   TAG_MULT     p0 unused; (c[n], s[n]) pairs, n = N .. 0 (Horner order)        16 + 16(N+1)
 //   TAG_CMULT    p0 = hxl;  {wf, 0};  pairs as above (c[0] = knl[0] - hxl)       32 + 16(N+1)
 //   TAG_CAVITY   p0 = lag_rad; {kz, vn}                                          32 B
@@ -53,7 +57,8 @@ enum : uint32_t {
   TAG_TYPE_MASK = 0xf,
   TAG_PRE = 0x10,   // a drift of length l_pre comes first
   TAG_POST = 0x20,  // a drift of length l_post follows the kick
-  TAG_POST2 = 0x40  // ... and a second one of length l_post2 (only with TAG_POST)
+  TAG_POST2 = 0x40,  // ... and a second one of length l_post2 (only with TAG_POST)
+  TAG_MISAL = 0x80   // shift + rotation before the kick, rotation + shift after it
 };
 
 struct alignas(16) RecHdr {

@@ -47,19 +47,15 @@ struct Reader {
 struct Rec {
   uint32_t type = TAG_END;
   uint32_t order = 0;
-  uint32_t flags = 0;   // TAG_PRE / TAG_POST
+  uint32_t flags = 0;  // TAG_PRE / TAG_POST / TAG_POST2 / TAG_MISAL
   uint32_t elem = 0;
   double p0 = 0.0;
-  double l_pre = 0.0, l_post = 0.0, l_post2 = 0.0;
   std::vector<double> slots;  // pairs, in the order the kernel reads them
   void slot(double a, double b) {
     slots.push_back(a);
     slots.push_back(b);
   }
-  uint32_t bytes() const {
-    return static_cast<uint32_t>(sizeof(RecHdr) + (flags ? 16 : 0) + ((flags & TAG_POST2) ? 16 : 0) +
-                                 slots.size() * sizeof(double));
-  }
+  uint32_t bytes() const { return static_cast<uint32_t>(sizeof(RecHdr) + slots.size() * sizeof(double)); }
   uint32_t tag() const { return type | flags | (order << 8) | (bytes() << 16); }
 };
 
@@ -242,36 +238,62 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
   }
   info.circumference = s_pos;
 
-  // ---- pass 2: fuse [Drift] Multipole [Drift] into one record.  The maps are applied in
-  // the same order with the same arithmetic; only the dispatch is shared (a thin lattice is
-  // mostly drift-kick-drift).
+  // ---- pass 2: fuse.  A thin lattice is mostly drift - kick - drift, with
+  // misaligned magnets wrapped in XYShift / SRotation.  A fused record applies
+  // the same maps in the same order with the same arithmetic; what is shared is the dispatch
+  // and, between consecutive drifts, the evaluation of what depends on (px, py) only.
   std::vector<Rec> fused;
   fused.reserve(recs.size());
-  auto is_mult = [&](size_t k) { return k < recs.size() && (recs[k].type == TAG_MULT || recs[k].type == TAG_CMULT); };
-  auto is_drift = [&](size_t k) { return k < recs.size() && recs[k].type == TAG_DRIFT; };
+  auto is = [&](size_t k, uint32_t type) { return k < recs.size() && recs[k].type == type; };
+  auto is_mult = [&](size_t k) { return is(k, TAG_MULT) || is(k, TAG_CMULT); };
   for (size_t i = 0; i < recs.size();) {
-    const bool pre = is_drift(i) && is_mult(i + 1);
-    if (opts.fuse && (pre || is_mult(i))) {
-      Rec m = std::move(recs[pre ? i + 1 : i]);
-      if (pre) {
-        m.flags |= TAG_PRE;
-        m.l_pre = recs[i].p0;
-      }
-      i += pre ? 2 : 1;
-      if (is_drift(i)) {
-        m.flags |= TAG_POST;
-        m.l_post = recs[i++].p0;
-        // a second drift shares the first one's evaluation (px, py unchanged in between)
-        if (is_drift(i)) {
-          m.flags |= TAG_POST2;
-          m.l_post2 = recs[i++].p0;
-        }
-      }
-      fused.push_back(std::move(m));
-    } else {
-      fused.push_back(std::move(recs[i]));
-      i += 1;
+    if (!opts.fuse) {
+      fused.push_back(std::move(recs[i++]));
+      continue;
     }
+    if (is(i, TAG_DRIFT) && is(i + 1, TAG_DRIFT)) {  // two drifts in a row
+      Rec d = std::move(recs[i]);
+      d.flags |= TAG_POST;
+      d.slot(recs[i + 1].p0, 0.0);
+      fused.push_back(std::move(d));
+      i += 2;
+      continue;
+    }
+    size_t j = i;
+    const bool pre = is(j, TAG_DRIFT);
+    if (pre) ++j;
+    const bool misal = is(j, TAG_SHIFT) && is(j + 1, TAG_SROT) && is_mult(j + 2) && is(j + 3, TAG_SROT) &&
+                       is(j + 4, TAG_SHIFT);
+    if (!misal && !is_mult(j)) {  // not a magnet group
+      fused.push_back(std::move(recs[i++]));
+      continue;
+    }
+    const size_t m = misal ? j + 2 : j;
+    size_t after = misal ? j + 5 : j + 1;
+    Rec out_rec;
+    out_rec.type = recs[m].type;
+    out_rec.order = recs[m].order;
+    out_rec.elem = recs[m].elem;
+    out_rec.p0 = recs[m].p0;
+    const bool post = is(after, TAG_DRIFT);
+    const bool post2 = post && is(after + 1, TAG_DRIFT);
+    if (pre) out_rec.flags |= TAG_PRE;
+    if (post) out_rec.flags |= TAG_POST;
+    if (post2) out_rec.flags |= TAG_POST2;
+    if (misal) out_rec.flags |= TAG_MISAL;
+    if (pre || post) out_rec.slot(pre ? recs[i].p0 : 0.0, post ? recs[after].p0 : 0.0);
+    if (post2) out_rec.slot(recs[after + 1].p0, 0.0);
+    if (misal) {
+      out_rec.slots.insert(out_rec.slots.end(), recs[j].slots.begin(), recs[j].slots.end());          // {dx, dy}
+      out_rec.slots.insert(out_rec.slots.end(), recs[j + 1].slots.begin(), recs[j + 1].slots.end());  // {cos, sin}
+    }
+    out_rec.slots.insert(out_rec.slots.end(), recs[m].slots.begin(), recs[m].slots.end());  // [{wf, 0}] + pairs
+    if (misal) {
+      out_rec.slots.insert(out_rec.slots.end(), recs[j + 3].slots.begin(), recs[j + 3].slots.end());
+      out_rec.slots.insert(out_rec.slots.end(), recs[j + 4].slots.begin(), recs[j + 4].slots.end());
+    }
+    fused.push_back(std::move(out_rec));
+    i = after + (post ? 1 : 0) + (post2 ? 1 : 0);
   }
   info.n_records = static_cast<int64_t>(fused.size());
 
@@ -303,18 +325,8 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
       put_header(prev_hdr, rec.tag(), prev_elem, prev_p0);
       const size_t at = out.image.size();
       out.image.resize(at + nb);
-      size_t w = at + sizeof(RecHdr);
-      if (rec.flags) {
-        const double l[2] = {rec.l_pre, rec.l_post};
-        std::memcpy(out.image.data() + w, l, 16);
-        w += 16;
-      }
-      if (rec.flags & TAG_POST2) {
-        const double l[2] = {rec.l_post2, 0.0};
-        std::memcpy(out.image.data() + w, l, 16);
-        w += 16;
-      }
-      if (!rec.slots.empty()) std::memcpy(out.image.data() + w, rec.slots.data(), rec.slots.size() * sizeof(double));
+      if (!rec.slots.empty())
+        std::memcpy(out.image.data() + at + sizeof(RecHdr), rec.slots.data(), rec.slots.size() * sizeof(double));
       prev_hdr = at;
       prev_elem = rec.elem;
       prev_p0 = rec.p0;

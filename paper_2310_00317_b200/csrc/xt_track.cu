@@ -268,14 +268,28 @@ __device__ __forceinline__ void drift(Parts<P> &q, const double length) {
   drift_apply<P>(q, d, length);
 }
 
-// The drifts a multipole record carries behind the kick (TAG_POST, TAG_POST2).
+// M4: change of reference frame ("tilts, misalignments").
 template <int P>
-__device__ __forceinline__ void drifts_after(Parts<P> &q, uint32_t tag, const double l1, const double2 *slots2) {
-  if (tag & TAG_POST) {
-    DriftCoef<P> d;
-    drift_eval<P>(q, d);
-    drift_apply<P>(q, d, l1);
-    if (tag & TAG_POST2) drift_apply<P>(q, d, slots2->x);
+__device__ __forceinline__ void s_rotation(Parts<P> &q, const double2 cs) {  // cs = (cos_z, sin_z)
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    const double nx = XT_MADD(cs.x, q.x[j], XT_MUL(cs.y, q.y[j]));
+    const double ny = XT_MADD(cs.x, q.y[j], -XT_MUL(cs.y, q.x[j]));
+    const double npx = XT_MADD(cs.x, q.px[j], XT_MUL(cs.y, q.py[j]));
+    const double npy = XT_MADD(cs.x, q.py[j], -XT_MUL(cs.y, q.px[j]));
+    q.x[j] = nx;
+    q.y[j] = ny;
+    q.px[j] = npx;
+    q.py[j] = npy;
+  }
+}
+
+template <int P>
+__device__ __forceinline__ void xy_shift(Parts<P> &q, const double2 d) {  // d = (dx, dy)
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    q.x[j] = q.x[j] - d.x;
+    q.y[j] = q.y[j] - d.y;
   }
 }
 
@@ -293,49 +307,63 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
     rp += tag >> 16;  // record size in bytes
     switch (tag & TAG_TYPE_MASK) {
       case TAG_DRIFT: {
-        drift<P>(q, p0);
+        DriftCoef<P> d;
+        drift_eval<P>(q, d);
+        drift_apply<P>(q, d, p0);
+        if (tag & TAG_POST) drift_apply<P>(q, d, slots[0].x);  // a second drift, same (px, py)
         break;
       }
-      case TAG_MULT: {
-        double2 dl = make_double2(0.0, 0.0);
-        const double2 *l2 = slots + 1;
-        if (tag & (TAG_PRE | TAG_POST)) dl = *slots++;
-        if (tag & TAG_POST2) ++slots;
-        if (tag & TAG_PRE) drift<P>(q, dl.x);
-        double re[P], im[P];
-        horner<P>(slots, static_cast<int>((tag >> 8) & 0xffu), q.x, q.y, re, im);
-#pragma unroll
-        for (int j = 0; j < P; ++j) {
-          q.px[j] = q.px[j] - re[j];
-          q.py[j] = q.py[j] + im[j];
-        }
-        drifts_after<P>(q, tag, dl.y, l2);
-        break;
-      }
+      case TAG_MULT:
       case TAG_CMULT: {
+        // [drift] [shift, rotate] kick [rotate, shift] [drift [drift]]: one dispatch
         double2 dl = make_double2(0.0, 0.0);
-        const double2 *l2 = slots + 1;
+        double l_post2 = 0.0;
         if (tag & (TAG_PRE | TAG_POST)) dl = *slots++;
-        if (tag & TAG_POST2) ++slots;
+        if (tag & TAG_POST2) l_post2 = (slots++)->x;
         if (tag & TAG_PRE) drift<P>(q, dl.x);
-        const double hxl = p0;
-        const double wf = slots[0].x;
-        double re[P], im[P], delta[P], rv0v[P];
-#pragma unroll
-        for (int j = 0; j < P; ++j) {  // issued ahead of the Horner loop that hides their latency
-          delta[j] = cold.delta(j);
-          rv0v[j] = cold.rv0v(j);
+        if (tag & TAG_MISAL) {
+          xy_shift<P>(q, slots[0]);
+          s_rotation<P>(q, slots[1]);
+          slots += 2;
         }
-        horner<P>(slots + 1, static_cast<int>((tag >> 8) & 0xffu), q.x, q.y, re, im);
+        const bool curved = (tag & TAG_TYPE_MASK) == TAG_CMULT;
+        double wf = 0.0;
+        double re[P], im[P], delta[P], rv0v[P];
+        if (curved) {
+          wf = (slots++)->x;
+#pragma unroll
+          for (int j = 0; j < P; ++j) {  // issued ahead of the Horner loop that hides their latency
+            delta[j] = cold.delta(j);
+            rv0v[j] = cold.rv0v(j);
+          }
+        }
+        const int order = static_cast<int>((tag >> 8) & 0xffu);
+        horner<P>(slots, order, q.x, q.y, re, im);
+        slots += order + 1;
 #pragma unroll
         for (int j = 0; j < P; ++j) {
           q.px[j] = q.px[j] - re[j];
           q.py[j] = q.py[j] + im[j];
-          q.px[j] = XT_MADD(hxl, delta[j], q.px[j]);
-          q.px[j] = XT_NMADD(wf, q.x[j], q.px[j]);
-          q.zeta[j] = XT_NMADD(XT_MUL(hxl, q.x[j]), rv0v[j], q.zeta[j]);
         }
-        drifts_after<P>(q, tag, dl.y, l2);
+        if (curved) {
+          const double hxl = p0;
+#pragma unroll
+          for (int j = 0; j < P; ++j) {
+            q.px[j] = XT_MADD(hxl, delta[j], q.px[j]);
+            q.px[j] = XT_NMADD(wf, q.x[j], q.px[j]);
+            q.zeta[j] = XT_NMADD(XT_MUL(hxl, q.x[j]), rv0v[j], q.zeta[j]);
+          }
+        }
+        if (tag & TAG_MISAL) {
+          s_rotation<P>(q, slots[0]);
+          xy_shift<P>(q, slots[1]);
+        }
+        if (tag & TAG_POST) {
+          DriftCoef<P> d;
+          drift_eval<P>(q, d);
+          drift_apply<P>(q, d, dl.y);
+          if (tag & TAG_POST2) drift_apply<P>(q, d, l_post2);
+        }
         break;
       }
       case TAG_CAVITY: {
@@ -359,27 +387,11 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         break;
       }
       case TAG_SROT: {
-        const double2 cs = slots[0];  // (cos_z, sin_z)
-#pragma unroll
-        for (int j = 0; j < P; ++j) {
-          const double nx = XT_MADD(cs.x, q.x[j], XT_MUL(cs.y, q.y[j]));
-          const double ny = XT_MADD(cs.x, q.y[j], -XT_MUL(cs.y, q.x[j]));
-          const double npx = XT_MADD(cs.x, q.px[j], XT_MUL(cs.y, q.py[j]));
-          const double npy = XT_MADD(cs.x, q.py[j], -XT_MUL(cs.y, q.px[j]));
-          q.x[j] = nx;
-          q.y[j] = ny;
-          q.px[j] = npx;
-          q.py[j] = npy;
-        }
+        s_rotation<P>(q, slots[0]);
         break;
       }
       case TAG_SHIFT: {
-        const double2 d = slots[0];
-#pragma unroll
-        for (int j = 0; j < P; ++j) {
-          q.x[j] = q.x[j] - d.x;
-          q.y[j] = q.y[j] - d.y;
-        }
+        xy_shift<P>(q, slots[0]);
         break;
       }
       case TAG_RECT: {
