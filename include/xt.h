@@ -107,7 +107,7 @@ typedef struct {
 /* Options of xt_lattice_create_ex.  Zero-initialise for the defaults.  Neither changes any
  * result: the same maps run in the same order with the same arithmetic. */
 typedef struct {
-  int64_t chunk_bytes; /* 0: default (16384); else shared-memory bytes of one staging buffer,  */
+  int64_t chunk_bytes; /* 0: default (8192);  else shared-memory bytes of one staging buffer,  */
                        /*    a multiple of 128 in [1024, 65536], at least one record + 16      */
   int32_t fuse;        /* 0 or 1: [Drift] Multipole [Drift] share one record and one dispatch; */
                        /*    2: one record per element                                         */

@@ -82,7 +82,7 @@ struct RefConsts {
   double ib2;    // ib * ib
 };
 
-constexpr uint32_t kDefaultChunkBytes = 16384;
+constexpr uint32_t kDefaultChunkBytes = 8192;
 
 }  // namespace xt
 

@@ -107,36 +107,44 @@ __device__ __forceinline__ double rcp_seed(double a) {
 template <int P>
 struct Parts {
   double x[P], px[P], y[P], py[P], zeta[P];
-  double opd2[P], b[P], g[P];  // cached functions of (delta, ptau), refreshed after a cavity
-  uint32_t alive;              // bit j: slot j holds a particle that is still being tracked
+  uint32_t alive;  // bit j: slot j holds a particle that is still being tracked
 };
 
-// Cold per-thread state, kept out of the register file: ptau (cavities only), delta and
-// rv0v = (1 + beta0 ptau)/(1 + delta) (curved multipoles only) live in shared memory, one
-// conflict-free column per thread; rpp / rvv are written straight to global memory by the
+// Cold per-thread state, kept out of the register file (the Horner loop needs the
+// registers to interleave its P independent chains): functions of (delta, ptau), which only
+// a cavity changes.  ptau (cavities), delta and rv0v = (1 + beta0 ptau)/(1 + delta) (curved
+// multipoles), opd2 = (1 + delta)^2, b = 1 + beta0 ptau and g = ptau (ptau + 2/beta0)/gamma0^2
+// (drifts) live in shared memory, one row of 6P doubles per thread at compile-time offsets
+// from one base register; the row pitch is odd (in doubles) so that a warp's 64-bit
+// accesses are bank-conflict free.  rpp / rvv are written straight to global memory by the
 // cavity map; s / at_turn / at_element / state are touched only when a particle is lost and
 // at the end of the launch.
 template <int P>
 struct Cold {
-  double *col;    // this thread's column: value m of slot j at col[(m * P + j) * stride]
+  static constexpr int kPitch = (6 * P) | 1;  // doubles per thread row
+  double *row;    // this thread's row: P each of ptau, delta, rv0v, opd2, b, g
   int stride;     // blockDim.x
   int64_t first;  // index of slot 0's particle; slot j is first + j * stride
-  __device__ __forceinline__ double &ptau(int j) const { return col[j * stride]; }
-  __device__ __forceinline__ double &delta(int j) const { return col[(P + j) * stride]; }
-  __device__ __forceinline__ double &rv0v(int j) const { return col[(2 * P + j) * stride]; }
+  __device__ __forceinline__ double &ptau(int j) const { return row[j]; }
+  __device__ __forceinline__ double &delta(int j) const { return row[P + j]; }
+  __device__ __forceinline__ double &rv0v(int j) const { return row[2 * P + j]; }
+  __device__ __forceinline__ double &opd2(int j) const { return row[3 * P + j]; }
+  __device__ __forceinline__ double &b(int j) const { return row[4 * P + j]; }
+  __device__ __forceinline__ double &g(int j) const { return row[5 * P + j]; }
   __device__ __forceinline__ int64_t idx(int j) const { return first + static_cast<int64_t>(j) * stride; }
 };
 
 template <int P>
-__device__ __forceinline__ void refresh_cached(Parts<P> &q, const Cold<P> &cold, int j, double opd, double b,
-                                               double t, double igam2) {
-  q.opd2[j] = opd * opd;
-  q.b[j] = b;
-  q.g[j] = t * igam2;
+__device__ __forceinline__ void refresh_cached(const Cold<P> &cold, int j, double opd, double b, double t,
+                                               double igam2) {
+  cold.opd2(j) = opd * opd;
+  cold.b(j) = b;
+  cold.g(j) = t * igam2;
   cold.rv0v(j) = b / opd;
 }
 
 // M2: complex Horner, coefficients stored highest order first as (c[n], s[n]) pairs.
+// One step: (re + i im) <- (re + i im)(x + i y) + (c + i s).
 template <int P>
 __device__ __forceinline__ void horner_step(const double2 c, const double (&x)[P], const double (&y)[P],
                                             double (&re)[P], double (&im)[P]) {
@@ -149,27 +157,54 @@ __device__ __forceinline__ void horner_step(const double2 c, const double (&x)[P
   }
 }
 
+// The first step, straight from the leading pair (the same arithmetic as a step from
+// re = top.x, im = top.y, without the register copies).
+template <int P>
+__device__ __forceinline__ void horner_first(const double2 top, const double2 c, const double (&x)[P],
+                                             const double (&y)[P], double (&re)[P], double (&im)[P]) {
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    re[j] = XT_MADD(top.x, x[j], XT_NMADD(top.y, y[j], c.x));
+    im[j] = XT_MADD(top.x, y[j], XT_MADD(top.y, x[j], c.y));
+  }
+}
+
 template <int P>
 __device__ __forceinline__ void horner(const double2 *__restrict__ cs, int order, const double (&x)[P],
                                        const double (&y)[P], double (&re)[P], double (&im)[P]) {
+  // (order mod 4) leading steps, their coefficients loaded together, then groups of four
   const double2 top = cs[0];
-#pragma unroll
-  for (int j = 0; j < P; ++j) {
-    re[j] = top.x;
-    im[j] = top.y;
-  }
-  // order mod 4 leading steps, then whole groups of four
   const int rem = order & 3;
-  if (rem >= 1) horner_step<P>(cs[1], x, y, re, im);
-  if (rem >= 2) horner_step<P>(cs[2], x, y, re, im);
-  if (rem == 3) horner_step<P>(cs[3], x, y, re, im);
+  if (rem == 3) {
+    const double2 c1 = cs[1], c2 = cs[2], c3 = cs[3];
+    horner_first<P>(top, c1, x, y, re, im);
+    horner_step<P>(c2, x, y, re, im);
+    horner_step<P>(c3, x, y, re, im);
+  } else if (rem == 2) {
+    const double2 c1 = cs[1], c2 = cs[2];
+    horner_first<P>(top, c1, x, y, re, im);
+    horner_step<P>(c2, x, y, re, im);
+  } else if (rem == 1) {
+    horner_first<P>(top, cs[1], x, y, re, im);
+  } else {
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+      re[j] = top.x;
+      im[j] = top.y;
+    }
+  }
+  cs += rem + 1;
+  double2 c0 = cs[0];  // first pair of the next group: always one group ahead of its use
 #pragma unroll 1
   for (int k = rem + 1; k <= order; k += 4) {
-    const double2 c0 = cs[k], c1 = cs[k + 1], c2 = cs[k + 2], c3 = cs[k + 3];
+    const double2 c1 = cs[1], c2 = cs[2], c3 = cs[3];
+    const double2 n0 = cs[4];  // may lie just past the record: never used then
+    cs += 4;
     horner_step<P>(c0, x, y, re, im);
     horner_step<P>(c1, x, y, re, im);
     horner_step<P>(c2, x, y, re, im);
     horner_step<P>(c3, x, y, re, im);
+    c0 = n0;
   }
 }
 
@@ -217,15 +252,22 @@ struct DriftCoef {
 };
 
 template <int P>
-__device__ __forceinline__ void drift_eval(const Parts<P> &q, DriftCoef<P> &d) {
+__device__ __forceinline__ void drift_eval(const Parts<P> &q, const Cold<P> &cold, DriftCoef<P> &d) {
+  double opd2[P], b[P], g[P];
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    opd2[j] = cold.opd2(j);
+    b[j] = cold.b(j);
+    g[j] = cold.g(j);
+  }
 #pragma unroll
   for (int j = 0; j < P; ++j) {
     const double t1 = XT_MUL(q.px[j], q.px[j]);
     const double pxy2 = XT_MADD(q.py[j], q.py[j], t1);
-    const double rad = q.opd2[j] - pxy2;
+    const double rad = opd2[j] - pxy2;
 #ifdef XT_FMAD_OFF
     const double pz = sqrt(rad);
-    const double s1 = pz + q.b[j];
+    const double s1 = pz + b[j];
     const double den = pz * s1;
     d.u[j] = 1.0 / den;
     d.v[j] = s1;
@@ -234,13 +276,13 @@ __device__ __forceinline__ void drift_eval(const Parts<P> &q, DriftCoef<P> &d) {
     const double r0 = rsqrt_seed(rad);
     const double e = fma(-rad, XT_MUL(r0, r0), 1.0);
     const double r1 = fma(fma(e, 0.375, 0.5), XT_MUL(r0, e), r0);  // 1/pz
-    const double s1 = fma(rad, r1, q.b[j]);                        // pz + b
+    const double s1 = fma(rad, r1, b[j]);                          // pz + b
     const double y0 = rcp_seed(s1);
     const double f = fma(-s1, y0, 1.0);
     d.u[j] = r1;
     d.v[j] = fma(y0, fma(f, f, f), y0);                            // 1/(pz + b)
 #endif
-    d.gm[j] = q.g[j] - pxy2;
+    d.gm[j] = g[j] - pxy2;
   }
 }
 
@@ -262,9 +304,9 @@ __device__ __forceinline__ void drift_apply(Parts<P> &q, const DriftCoef<P> &d, 
 }
 
 template <int P>
-__device__ __forceinline__ void drift(Parts<P> &q, const double length) {
+__device__ __forceinline__ void drift(Parts<P> &q, const Cold<P> &cold, const double length) {
   DriftCoef<P> d;
-  drift_eval<P>(q, d);
+  drift_eval<P>(q, cold, d);
   drift_apply<P>(q, d, length);
 }
 
@@ -308,7 +350,7 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
     switch (tag & TAG_TYPE_MASK) {
       case TAG_DRIFT: {
         DriftCoef<P> d;
-        drift_eval<P>(q, d);
+        drift_eval<P>(q, cold, d);
         drift_apply<P>(q, d, p0);
         if (tag & TAG_POST) drift_apply<P>(q, d, slots[0].x);  // a second drift, same (px, py)
         break;
@@ -320,7 +362,7 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         double l_post2 = 0.0;
         if (tag & (TAG_PRE | TAG_POST)) dl = *slots++;
         if (tag & TAG_POST2) l_post2 = (slots++)->x;
-        if (tag & TAG_PRE) drift<P>(q, dl.x);
+        if (tag & TAG_PRE) drift<P>(q, cold, dl.x);
         if (tag & TAG_MISAL) {
           xy_shift<P>(q, slots[0]);
           s_rotation<P>(q, slots[1]);
@@ -328,15 +370,8 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         }
         const bool curved = (tag & TAG_TYPE_MASK) == TAG_CMULT;
         double wf = 0.0;
-        double re[P], im[P], delta[P], rv0v[P];
-        if (curved) {
-          wf = (slots++)->x;
-#pragma unroll
-          for (int j = 0; j < P; ++j) {  // issued ahead of the Horner loop that hides their latency
-            delta[j] = cold.delta(j);
-            rv0v[j] = cold.rv0v(j);
-          }
-        }
+        double re[P], im[P];
+        if (curved) wf = (slots++)->x;
         const int order = static_cast<int>((tag >> 8) & 0xffu);
         horner<P>(slots, order, q.x, q.y, re, im);
         slots += order + 1;
@@ -349,9 +384,9 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
           const double hxl = p0;
 #pragma unroll
           for (int j = 0; j < P; ++j) {
-            q.px[j] = XT_MADD(hxl, delta[j], q.px[j]);
+            q.px[j] = XT_MADD(hxl, cold.delta(j), q.px[j]);
             q.px[j] = XT_NMADD(wf, q.x[j], q.px[j]);
-            q.zeta[j] = XT_NMADD(XT_MUL(hxl, q.x[j]), rv0v[j], q.zeta[j]);
+            q.zeta[j] = XT_NMADD(XT_MUL(hxl, q.x[j]), cold.rv0v(j), q.zeta[j]);
           }
         }
         if (tag & TAG_MISAL) {
@@ -360,7 +395,7 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         }
         if (tag & TAG_POST) {
           DriftCoef<P> d;
-          drift_eval<P>(q, d);
+          drift_eval<P>(q, cold, d);
           drift_apply<P>(q, d, dl.y);
           if (tag & TAG_POST2) drift_apply<P>(q, d, l_post2);
         }
@@ -381,7 +416,7 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
             cold.delta(j) = delta;
             a.p.rpp[cold.idx(j)] = 1.0 / opd;
             a.p.rvv[cold.idx(j)] = opd / b;
-            refresh_cached<P>(q, cold, j, opd, b, t, a.igam2);
+            refresh_cached<P>(cold, j, opd, b, t, a.igam2);
           }
         }
         break;
@@ -434,17 +469,19 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
 #endif
 constexpr int kMaxBlock = 256;
 
-// Shared memory: [0,16) two mbarriers; [128, 128 + 24*P*blockDim) cold per-thread columns;
-// then staging buffer 0 (and buffer 1 for multi-chunk lattices), 128-byte aligned.
+// Shared memory: [0,16) two mbarriers; [128, 128 + 8*kPitch*blockDim) cold per-thread rows;
+// then staging buffer 0 (and buffer 1 for multi-chunk lattices), 128-byte aligned, and 64
+// spare bytes (the Horner loop prefetches one coefficient pair past the record it is in).
 template <int P>
 __global__ void __launch_bounds__(kMaxBlock, P == 4 ? XT_MINB4 : (P == 2 ? XT_MINB2 : 4))
     xt_track_kernel(const TrackArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   const uint32_t bar0 = smem_addr(smem);
   Cold<P> cold;
-  cold.col = reinterpret_cast<double *>(smem + 128) + threadIdx.x;
+  cold.row = reinterpret_cast<double *>(smem + 128) + static_cast<uint32_t>(Cold<P>::kPitch) * threadIdx.x;
   cold.stride = static_cast<int>(blockDim.x);
-  unsigned char *const buf0 = smem + 128 + ((static_cast<uint32_t>(24 * P) * blockDim.x + 127u) & ~127u);
+  unsigned char *const buf0 =
+      smem + 128 + ((static_cast<uint32_t>(8 * Cold<P>::kPitch) * blockDim.x + 127u) & ~127u);
 
   // Balanced hand-out (device side, so that compaction's device counter needs no host
   // sync): use as few CTAs as hold n_active particles, rounded up to a whole number per SM,
@@ -483,11 +520,11 @@ __global__ void __launch_bounds__(kMaxBlock, P == 4 ? XT_MINB4 : (P == 2 ? XT_MI
       const double opd = 1.0 + delta;
       const double b = XT_MADD(a.beta0, ptau, 1.0);
       const double t = XT_MUL(ptau, ptau + a.tib);
-      refresh_cached<P>(q, cold, j, opd, b, t, a.igam2);
+      refresh_cached<P>(cold, j, opd, b, t, a.igam2);
     } else {
       q.x[j] = q.px[j] = q.y[j] = q.py[j] = q.zeta[j] = 0.0;
-      q.opd2[j] = q.b[j] = 1.0;
-      q.g[j] = 0.0;
+      cold.opd2(j) = cold.b(j) = 1.0;
+      cold.g(j) = 0.0;
       cold.ptau(j) = cold.delta(j) = 0.0;
       cold.rv0v(j) = 1.0;
     }
@@ -579,8 +616,8 @@ __global__ void xt_init_derived_kernel(xt_particles p, int64_t n, double beta0, 
 
 template <int P>
 int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
-  const size_t cold_bytes = (static_cast<size_t>(24 * P) * block + 127) & ~static_cast<size_t>(127);
-  const size_t smem = 128 + cold_bytes + (lat->info.n_chunks == 1 ? 1 : 2) * static_cast<size_t>(lat->info.chunk_bytes);
+  const size_t cold_bytes = (static_cast<size_t>(8 * Cold<P>::kPitch) * block + 127) & ~static_cast<size_t>(127);
+  const size_t smem = 128 + 64 + cold_bytes + (lat->info.n_chunks == 1 ? 1 : 2) * static_cast<size_t>(lat->info.chunk_bytes);
   static bool attr_set = false;
   if (!attr_set) {
     XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
