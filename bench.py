@@ -47,16 +47,22 @@ WORKLOADS = {
 # canonical forms; FMA = 2, add/mul/sqrt/div = 1, compares = 0, sin = 1) ...
 FLOPS_MIN = dict(drift=17, mult_base=2, mult_per_order=8, curved_extra=7, cavity=19, srot=12,
                  shift=2, rect=0, ellipse=5)
-# ... and FP64 flops as executed by the sm_100a kernel (IEEE sqrt / div / sin expansions
-# counted; from the SASS of libxt_b200.so, profiles/sass_fp64_counts_r01.md)
-FLOPS_EXEC = dict(drift=43, mult_base=2, mult_per_order=8, curved_extra=7, cavity=110, srot=12,
-                  shift=2, rect=0, ellipse=5)
+# ... and FP64 flops as executed by the sm_100a kernel (counted in the SASS of
+# libxt_b200.so, profiles/r01_sass_fp64_counts.md): a drift is one evaluation of 1/pz and
+# 1/(pz + b) (13 FP64 instructions, 21 flops; consecutive drifts share it after fusion) plus
+# one application (5 instructions, 8 flops); sin and the cavity's sqrt / divisions expanded.
+FLOPS_EXEC = dict(drift_eval=21, drift_apply=8, mult_base=2, mult_per_order=8, curved_extra=7, cavity=110,
+                  srot=12, shift=2, rect=0, ellipse=5)
 
 
 def flops_per_particle_turn(info: dict, table: dict) -> float:
     t = info["n_by_type"]
     n_mult = t[2]
-    return (t[1] * table["drift"] + n_mult * table["mult_base"] + info["sum_order"] * table["mult_per_order"]
+    if "drift" in table:
+        drifts = t[1] * table["drift"]
+    else:
+        drifts = t[1] * table["drift_apply"] + info["n_drift_evals"] * table["drift_eval"]
+    return (drifts + n_mult * table["mult_base"] + info["sum_order"] * table["mult_per_order"]
             + info["n_curved"] * table["curved_extra"] + t[3] * table["cavity"] + t[4] * table["srot"]
             + t[5] * table["shift"] + t[6] * table["rect"] + t[7] * table["ellipse"])
 
@@ -269,7 +275,8 @@ def main():
             "config": {"workload": WORKLOADS[cfg], "n_particles_per_gpu": n_part, "n_elements": n_el,
                        "n_turns": turns, "l2": "inputs (%.2f GB SoA per GPU) larger than L2" %
                                               (n_part * 13 * 8 / 1e9),
-                       "alive_after_step": alive, "block_size": args.block or 128,
+                       "alive_after_step": alive, "block_size": args.block or "auto",
+                       "particles_per_thread": args.ppt or "auto", "records_per_turn": info["n_records"],
                        "lattice_image_bytes": info["image_bytes"], "tma_chunks_per_turn": info["n_chunks"]},
             "particle_turns_per_s": world * n_part * turns / (ms_per_step * 1e-3),
             "gpu_launches": int(launches),

@@ -102,6 +102,8 @@ typedef struct {
   int64_t has_aperture;     /* 1 if any LimitRect / LimitEllipse                              */
   double beta0, gamma0;     /* reference particle as derived by the packer                    */
   double circumference;     /* sum of drift lengths [m]                                       */
+  int64_t n_drift_evals;    /* sqrt evaluations per turn after fusion (consecutive drifts     */
+                            /* share one; equals the number of drifts when fuse is off)       */
 } xt_lattice_info;
 
 /* Options of xt_lattice_create_ex.  Zero-initialise for the defaults.  Neither changes any

@@ -37,9 +37,21 @@ int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p
 }
 
 // Launch shape of the tracking kernel: threads per CTA and particles per thread.
-int resolve_shape(const xt_track_opts *o, int *block, int *ppt) {
-  *ppt = (o && o->particles_per_thread) ? o->particles_per_thread : 2;
-  *block = (o && o->block_size) ? o->block_size : 128;
+// Auto rule (measured on B200, profiles/r01_shape_sweep.md): with at least ~1000 particles
+// per SM, 4 particles per thread in 128-thread CTAs (4 CTAs per SM at 128 registers) is
+// fastest; smaller ensembles need the warps more than the per-warp ILP, so 2 per thread,
+// then 1.  The kernel hands the particles out in equal shares over a whole number of CTAs
+// per SM, so the shape only has to make enough CTAs.
+int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part, int *block, int *ppt) {
+  const int64_t per_sm = n_part / (lat->n_sm > 0 ? lat->n_sm : 1);
+  int auto_ppt = 4, auto_block = 128;
+  if (per_sm < 1024) auto_ppt = 2;
+  if (per_sm < 256) {
+    auto_ppt = 1;
+    auto_block = 64;
+  }
+  *ppt = (o && o->particles_per_thread) ? o->particles_per_thread : auto_ppt;
+  *block = (o && o->block_size) ? o->block_size : auto_block;
   if (*ppt != 1 && *ppt != 2 && *ppt != 4) {
     set_error("xt_track_ex: particles_per_thread must be 0 (auto), 1, 2 or 4");
     return XT_ERR_INVALID_ARG;
@@ -63,7 +75,7 @@ extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t
     return XT_ERR_INVALID_ARG;
   }
   int block = 0, ppt = 0;
-  if ((rc = xt::resolve_shape(opts, &block, &ppt)) != XT_OK) return rc;
+  if ((rc = xt::resolve_shape(opts, lat, n_part, &block, &ppt)) != XT_OK) return rc;
   if (opts && opts->turns_per_launch < 0) {
     xt::set_error("xt_track_ex: negative turns_per_launch");
     return XT_ERR_INVALID_ARG;

@@ -296,6 +296,11 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
     i = after + (post ? 1 : 0) + (post2 ? 1 : 0);
   }
   info.n_records = static_cast<int64_t>(fused.size());
+  for (const Rec &rec : fused) {
+    if (rec.type == TAG_DRIFT) info.n_drift_evals += 1;
+    if (rec.type == TAG_MULT || rec.type == TAG_CMULT)
+      info.n_drift_evals += ((rec.flags & TAG_PRE) ? 1 : 0) + ((rec.flags & TAG_POST) ? 1 : 0);
+  }
 
   // ---- pass 3: serialise.  Chunk = 16-byte preamble {tag of the first record} + records;
   // every record header carries the tag of the record that FOLLOWS it (TAG_END after the last

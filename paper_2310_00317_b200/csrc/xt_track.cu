@@ -485,15 +485,14 @@ __global__ void __launch_bounds__(kMaxBlock, P == 4 ? XT_MINB4 : (P == 2 ? XT_MI
 
   // Balanced hand-out (device side, so that compaction's device counter needs no host
   // sync): use as few CTAs as hold n_active particles, rounded up to a whole number per SM,
-  // and give each the same share (a multiple of 32 so that warps stay whole).
+  // and give each the same share.
   const int64_t n_active = a.n_active ? *a.n_active : a.n_part;
   const int64_t cap = static_cast<int64_t>(blockDim.x) * P;
   const int64_t need = (n_active + cap - 1) / cap;
   int64_t used = ((need + a.grid_quantum - 1) / a.grid_quantum) * a.grid_quantum;
   if (used > static_cast<int64_t>(gridDim.x)) used = gridDim.x;
   if (static_cast<int64_t>(blockIdx.x) >= used) return;  // CTA-uniform
-  int64_t share = (n_active + used - 1) / used;
-  share = (share + 31) & ~static_cast<int64_t>(31);
+  const int64_t share = (n_active + used - 1) / used;
   const int64_t start = static_cast<int64_t>(blockIdx.x) * share;
   if (start >= n_active) return;  // CTA-uniform
   const int64_t count = (n_active - start < share) ? n_active - start : share;
