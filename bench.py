@@ -128,6 +128,23 @@ def make_inputs(cfg: int, rank: int):
     return buf, coords
 
 
+def reduce_max(value: float, world: int, device) -> float:
+    """MAX over ranks of a per-rank scalar (device time): the only collective of the job, outside
+    every timed region.  The data path itself has none (particles are independent)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_rank: float, world: int, ms_per_step: float) -> float:
+    """Weak scaling: every rank tracks its own ensemble of the config's size."""
+    return world * units_per_rank / (ms_per_step * 1e-3)
+
+
 def oracle_sample(cfg: int, buf: bytes, coords: dict, budget_s: float = 15.0):
     """The oracle, as it stands, single-threaded, on a bounded sample of the same workload."""
     from oracle import oracle as O
@@ -236,6 +253,8 @@ def main():
             ev1.record(stream)
 
     peak_flops, peak_ms = X.xt_fp64_fma_peak()
+    probe = {"dfma_three_distinct_registers": X.xt_fp64_fma_probe(1)[0] / 1e12,
+             "horner_4_particles_per_thread_no_lattice": X.xt_fp64_fma_probe(2)[0] / 1e12}
     for _ in range(args.warmup):
         step()
     barrier()
@@ -255,13 +274,10 @@ def main():
     total_ms = t_begin.elapsed_time(t_end)
     kernel_ms = float(np.mean([a.elapsed_time(b) for a, b in kev]))
     alive = int((work["state"] == 1).sum().item())
-    tm = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-    total_ms = float(tm.item())
+    total_ms = reduce_max(total_ms, world, "cuda")
     ms_per_step = total_ms / args.steps
     units_per_step = float(n_part) * n_el * turns            # per rank (nominal: lost ones included)
-    value = world * units_per_step / (ms_per_step * 1e-3)
+    value = whole_job_value(units_per_step, world, ms_per_step)
 
     line = None
     if rank == 0:
@@ -290,7 +306,11 @@ def main():
                                "nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2 TFLOP/s" % peak_ms,
                 "kernel": "xt_track_kernel", "kernel_ms": kernel_ms,
                 "flops_per_particle_turn": {"algorithmic": f_min, "executed": f_exec},
-                "traffic": None,
+                # DRAM bytes of one launch: the --set full capture (profiles/r01i_track_cfg3_summary.md:
+                # dram__bytes_read + dram__bytes_write = 77.1 B per particle) scaled to this launch
+                "traffic": 77.1 * n_part if cfg == 3 else None,
+                # the same DFMA count with the operand shapes of this arithmetic
+                "operand_pattern_ceilings_tflops": probe,
             },
         }
 
@@ -305,14 +325,12 @@ def main():
         X.xt_track_host(lat, host, turns, block_size=args.block, particles_per_thread=args.ppt)     # synchronises the stream itself
         barrier()
         e2e_s = time.perf_counter() - t0
-        te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e_max = reduce_max(e2e_s, world, "cuda")
         if rank == 0:
             nbytes = sum(v.numel() * 8 for v in host.values())
-            line["e2e"] = {"value": world * units_per_step / float(te.item()), "unit": UNIT,
+            line["e2e"] = {"value": world * units_per_step / e2e_max, "unit": UNIT,
                            "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
-                           "seconds": float(te.item()), "api": "xt_track_host (pinned host SoA)",
+                           "seconds": e2e_max, "api": "xt_track_host (pinned host SoA)",
                            "alive_after_step": int((host["state"] == 1).sum().item())}
         del host, host0
     del work, pristine

@@ -168,6 +168,11 @@ int xt_survival_histogram(const int64_t *at_turn, const int64_t *state, int64_t 
  * times it with CUDA events on `cuda_stream`, synchronises, and returns FLOP/s (2 per FMA)
  * in *flops_per_s and the kernel time in *ms (either may be NULL). */
 int xt_fp64_fma_peak(double *flops_per_s, double *ms, void *cuda_stream);
+/* The same measurement with the operand shapes of the tracking arithmetic:
+ * pattern 0 = xt_fp64_fma_peak (two of three operands shared by consecutive instructions);
+ * 1 = three distinct register operands per DFMA; 2 = the complex Horner recurrence of step M2
+ * for 4 particles per thread, coefficients broadcast from shared memory, no lattice. */
+int xt_fp64_fma_probe(int pattern, double *flops_per_s, double *ms, void *cuda_stream);
 
 /* Number of kernels the library has launched from this process so far (bench bookkeeping). */
 int64_t xt_launch_count(void);

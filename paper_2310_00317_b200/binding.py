@@ -77,6 +77,8 @@ SIGNATURES = {
     "xt_particles_init_derived": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _VP]),
     "xt_survival_histogram": (ctypes.c_int, [_VP, _VP, _I64, _I64, _I64, _VP, _VP]),
     "xt_fp64_fma_peak": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), _VP]),
+    "xt_fp64_fma_probe": (ctypes.c_int, [ctypes.c_int, ctypes.POINTER(ctypes.c_double),
+                                         ctypes.POINTER(ctypes.c_double), _VP]),
     "xt_launch_count": (_I64, []),
     "xt_last_error": (ctypes.c_char_p, []),
     "xt_build_info": (ctypes.c_char_p, []),
@@ -319,6 +321,14 @@ def xt_fp64_fma_peak(stream=None, kind: str = "prod"):
     lib = load_library(kind)
     f, ms = ctypes.c_double(), ctypes.c_double()
     _check(lib, lib.xt_fp64_fma_peak(ctypes.byref(f), ctypes.byref(ms), _stream_ptr(stream)))
+    return f.value, ms.value
+
+
+def xt_fp64_fma_probe(pattern: int, stream=None, kind: str = "prod"):
+    """(FLOP/s, kernel ms) of the DFMA probe with operand pattern 0, 1 or 2 (see include/xt.h)."""
+    lib = load_library(kind)
+    f, ms = ctypes.c_double(), ctypes.c_double()
+    _check(lib, lib.xt_fp64_fma_probe(int(pattern), ctypes.byref(f), ctypes.byref(ms), _stream_ptr(stream)))
     return f.value, ms.value
 
 

@@ -215,7 +215,11 @@ extern "C" int xt_survival_histogram(const int64_t *at_turn, const int64_t *stat
 }
 
 extern "C" int xt_fp64_fma_peak(double *flops_per_s, double *ms, void *cuda_stream) {
-  return xt::run_fma_peak(flops_per_s, ms, static_cast<cudaStream_t>(cuda_stream));
+  return xt::run_fma_peak(flops_per_s, ms, 0, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int xt_fp64_fma_probe(int pattern, double *flops_per_s, double *ms, void *cuda_stream) {
+  return xt::run_fma_peak(flops_per_s, ms, pattern, static_cast<cudaStream_t>(cuda_stream));
 }
 
 extern "C" int64_t xt_launch_count(void) { return xt::g_launches.load(std::memory_order_relaxed); }

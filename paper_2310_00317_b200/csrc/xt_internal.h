@@ -154,6 +154,6 @@ int launch_histogram(const int64_t *at_turn, const int64_t *state, int64_t n, in
                      int64_t n_bins, int64_t *hist, cudaStream_t st);
 
 // xt_peak.cu
-int run_fma_peak(double *flops_per_s, double *ms, cudaStream_t st);
+int run_fma_peak(double *flops_per_s, double *ms, int pattern, cudaStream_t st);
 
 }  // namespace xt

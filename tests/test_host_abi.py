@@ -1,0 +1,321 @@
+"""CPU tests of the boundary and the host logic (no GPU, no compute call):
+
+* both shared objects load and export every function ``include/xt.h`` declares;
+* step P (the lattice packer) through ``xt_lattice_pack_host``: the device image is walked
+  record by record with an independent decoder of the format documented in
+  ``csrc/xt_internal.h``; counts, sizes, chunking, fusion and error codes are checked;
+* argument validation of the compute entry points that needs no device;
+* the multi-rank plumbing of ``bench.py`` with world_size 2 on gloo.
+"""
+import ctypes
+import os
+import re
+import struct
+import sys
+
+import numpy as np
+import pytest
+
+import paper_2310_00317_b200 as X
+from paper_2310_00317_b200 import binding as B
+from xt_inputs import configs as C
+from xt_inputs.packed import (Cavity, Drift, LimitEllipse, LimitRect, Marker, Multipole, SRotation,
+                              XYShift, pack_lattice)
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+P0C, MASS0 = 450e9, 938272088.16
+
+T_END, T_DRIFT, T_MULT, T_CAV, T_SROT, T_SHIFT, T_RECT, T_ELL, T_CMULT = range(9)
+F_PRE, F_POST, F_POST2, F_MISAL = 0x10, 0x20, 0x40, 0x80
+
+
+def pack(els):
+    return pack_lattice(els, P0C, MASS0, 1.0)
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "xt.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(xt_[a-z0-9_]+)\s*\(", text)))
+
+
+# ------------------------------------------------------------------------------- ABI
+@pytest.mark.parametrize("kind", ["prod", "nofma"])
+def test_library_loads_and_exports_every_declared_symbol(kind):
+    lib = X.load_library(kind)
+    names = declared_functions()
+    assert len(names) >= 15 and "xt_track" in names and "xt_lattice_create_ex" in names
+    for name in names:
+        assert hasattr(lib, name), "%s is declared in include/xt.h but not exported" % name
+        assert name in B.SIGNATURES, "%s has no ctypes signature in the binding" % name
+    info = X.xt_build_info(kind)
+    assert "sm_100a" in info and ("fmad=false" in info) == (kind == "nofma")
+
+
+def test_struct_layouts_match_the_header():
+    # sizes the C compiler gives the public structs (LP64): 14 pointers; 2 x i64 + 2 x i32; ...
+    assert ctypes.sizeof(B.xt_particles) == 14 * 8
+    assert ctypes.sizeof(B.xt_track_opts) == 24
+    assert ctypes.sizeof(B.xt_lattice_opts) == 16
+    assert ctypes.sizeof(B.xt_lattice_info) == 8 * (5 + 8 + 3) + 8 * 3 + 8
+
+
+def test_compute_calls_validate_arguments_without_a_device():
+    lib = X.load_library("prod")
+    assert lib.xt_track(None, None, 0, 0, None) == -1                    # XT_ERR_INVALID_ARG
+    assert b"NULL" in lib.xt_last_error()
+    assert lib.xt_survival_histogram(None, None, 0, 0, 10, None, None) == -1
+    assert lib.xt_lattice_destroy(None) == 0
+    out = ctypes.c_void_p()
+    assert lib.xt_lattice_create(None, 0, ctypes.byref(out)) == -1 and not out.value
+    import torch
+    if not torch.cuda.is_available():                                    # no CPU fallback: fails loudly
+        buf = pack([Drift(1.0)])
+        rc = lib.xt_lattice_create(buf, len(buf), ctypes.byref(out))
+        assert rc == -3 and not out.value, "xt_lattice_create must fail with XT_ERR_CUDA without a device"
+        with pytest.raises(X.XtError):
+            X.xt_lattice_create(buf)
+
+
+# ------------------------------------------------------------------- image decoder
+def walk_image(img, chunk_bytes):
+    """-> list of chunks, each a list of records (type, flags, order, elem, p0, slots[doubles])."""
+    chunks, pos = [], 0
+    while pos < len(img):
+        start = pos
+        tag, _, _ = struct.unpack_from("<IId", img, pos)
+        pos += 16
+        recs = []
+        while tag & 0xF != T_END:
+            size = tag >> 16
+            nxt, elem, p0 = struct.unpack_from("<IId", img, pos)
+            assert size >= 16 and size % 16 == 0
+            slots = struct.unpack_from("<%dd" % ((size - 16) // 8), img, pos + 16)
+            recs.append((tag & 0xF, tag & 0xF0, (tag >> 8) & 0xFF, elem, p0, slots))
+            pos += size
+            tag = nxt
+        assert pos - start <= chunk_bytes
+        chunks.append(recs)
+    assert pos == len(img)
+    return chunks
+
+
+def maps_of(rec):
+    """Element maps a record stands for, in order, as (kind, parameters)."""
+    typ, flags, order, elem, p0, s = rec
+    out, k = [], 0
+    if typ == T_DRIFT:
+        out.append(("drift", p0))
+        if flags & F_POST:
+            out.append(("drift", s[0]))
+        return out
+    if typ in (T_MULT, T_CMULT):
+        l_pre = l_post = l_post2 = None
+        if flags & (F_PRE | F_POST):
+            l_pre, l_post = s[0], s[1]
+            k = 2
+        if flags & F_POST2:
+            l_post2 = s[k]
+            k += 2
+        if flags & F_PRE:
+            out.append(("drift", l_pre))
+        if flags & F_MISAL:
+            out += [("shift", s[k:k + 2]), ("srot", s[k + 2:k + 4])]
+            k += 4
+        wf = None
+        if typ == T_CMULT:
+            wf = s[k]
+            k += 2
+        coef = s[k:k + 2 * (order + 1)]
+        k += 2 * (order + 1)
+        out.append(("mult", (order, p0 if typ == T_CMULT else 0.0, wf, coef)))
+        if flags & F_MISAL:
+            out += [("srot", s[k:k + 2]), ("shift", s[k + 2:k + 4])]
+            k += 4
+        if flags & F_POST:
+            out.append(("drift", l_post))
+        if flags & F_POST2:
+            out.append(("drift", l_post2))
+        assert k == len(s)
+        return out
+    return [({T_CAV: "cavity", T_SROT: "srot", T_SHIFT: "shift", T_RECT: "rect", T_ELL: "ellipse"}[typ], s)]
+
+
+def all_maps(img, chunk_bytes):
+    return [m for ch in walk_image(img, chunk_bytes) for r in ch for m in maps_of(r)]
+
+
+def expected_maps(elements, beta0):
+    """What step P must encode, from the element list."""
+    out = []
+    for el in elements:
+        if isinstance(el, Marker):
+            continue
+        if isinstance(el, Drift):
+            out.append(("drift", el.length))
+        elif isinstance(el, Multipole):
+            n = el.order
+            knl = list(el.knl) + [0.0] * (n + 1 - len(el.knl))
+            ksl = list(el.ksl) + [0.0] * (n + 1 - len(el.ksl))
+            fact = [1.0]
+            for i in range(1, n + 1):
+                fact.append(fact[-1] * i)
+            c = [knl[i] / fact[i] for i in range(n + 1)]
+            s = [ksl[i] / fact[i] for i in range(n + 1)]
+            wf = None
+            if el.hxl != 0.0:
+                c[0] = knl[0] - el.hxl
+                wf = (knl[0] * el.hxl) / el.length if el.length != 0.0 else 0.0
+            coef = []
+            for i in range(n, -1, -1):                       # Horner order: highest first
+                coef += [c[i], s[i]]
+            out.append(("mult", (n, el.hxl, wf, tuple(coef))))
+        elif isinstance(el, Cavity):
+            out.append(("cavity", None))
+        elif isinstance(el, SRotation):
+            out.append(("srot", (el.cos_z, el.sin_z)))
+        elif isinstance(el, XYShift):
+            out.append(("shift", (el.dx, el.dy)))
+        elif isinstance(el, LimitRect):
+            out.append(("rect", (el.min_x, el.max_x, el.min_y, el.max_y)))
+        elif isinstance(el, LimitEllipse):
+            out.append(("ellipse", (el.b * el.b, el.a * el.a)))
+    return out
+
+
+def assert_same_maps(got, want):
+    assert len(got) == len(want)
+    for i, (g, w) in enumerate(zip(got, want)):
+        assert g[0] == w[0], (i, g[0], w[0])
+        if w[0] == "cavity":
+            continue
+        if w[0] == "mult":
+            assert g[1][0] == w[1][0] and g[1][1] == w[1][1], i
+            assert g[1][2] == w[1][2], (i, "weak-focusing coefficient")
+            assert tuple(g[1][3]) == w[1][3], (i, "Horner coefficients")
+        else:
+            gv = g[1] if isinstance(g[1], tuple) else (g[1],)
+            wv = w[1] if isinstance(w[1], tuple) else (w[1],)
+            assert tuple(gv)[:len(wv)] == tuple(wv), (i, g, w)
+
+
+ALL_TYPES = [Drift(1.5), XYShift(1e-4, -2e-4), SRotation.from_angle(1e-3),
+             Multipole(knl=(5e-3, 0.1, 0.5, 5.0), ksl=(0.0, 1e-3, -0.2, 1.0), hxl=5e-3, length=14.3),
+             SRotation.from_angle(-1e-3), XYShift(-1e-4, 2e-4), Drift(0.25), Drift(0.75), Marker(),
+             Cavity(1e6, 200e6, 180.0), Drift(1.0), LimitRect(-0.01, 0.01, -0.02, 0.02), Drift(2.0),
+             Multipole(knl=(0.0, 0.1)), LimitEllipse(0.02, 0.015), Multipole(knl=(0.0, 0.0, 0.5)), Drift(3.0),
+             Drift(0.5), Drift(0.125), Multipole(knl=(1e-3,), hxl=1e-3, length=0.0)]
+
+
+# ------------------------------------------------------------------------ step P
+@pytest.mark.parametrize("fuse", [True, False])
+def test_packer_encodes_every_map_in_order_with_prescaled_coefficients(fuse):
+    buf = pack(ALL_TYPES)
+    img, info = X.xt_lattice_pack_host(buf, fuse=fuse)
+    assert info["n_elements"] == len(ALL_TYPES) and info["image_bytes"] == len(img)
+    assert info["n_by_type"] == [1, 8, 4, 1, 2, 2, 1, 1]
+    assert info["sum_order"] == 3 + 1 + 2 + 0 and info["n_curved"] == 2 and info["has_aperture"] == 1
+    assert info["circumference"] == 1.5 + 0.25 + 0.75 + 1.0 + 2.0 + 3.0 + 0.5 + 0.125
+    e0 = np.sqrt(P0C * P0C + MASS0 * MASS0)
+    assert info["beta0"] == P0C / e0 and info["gamma0"] == e0 / MASS0
+    chunks = walk_image(img, info["chunk_bytes"])
+    assert len(chunks) == info["n_chunks"] == 1
+    assert sum(len(c) for c in chunks) == info["n_records"]
+    assert_same_maps(all_maps(img, info["chunk_bytes"]), expected_maps(ALL_TYPES, info["beta0"]))
+    if fuse:
+        # [D shift rot M rot shift D D], cavity, D, rect, [D M], ellipse, [M D D], [D M]
+        assert info["n_records"] == 8
+        first = chunks[0][0]
+        assert first[0] == T_CMULT and first[1] == (F_PRE | F_POST | F_POST2 | F_MISAL) and first[3] == 3
+        assert info["n_drift_evals"] == 2 + 1 + 1 + 1 + 1           # pre + post, D, [D M], [M D D], [D M]
+    else:
+        assert info["n_records"] == len(ALL_TYPES) - 1             # the marker has no record
+        assert info["n_drift_evals"] == 8
+        assert [r[3] for r in chunks[0]] == [i for i, e in enumerate(ALL_TYPES) if not isinstance(e, Marker)]
+
+
+def test_cavity_and_aperture_constants():
+    buf = pack([Cavity(2e6, 400e6, 90.0), LimitEllipse(0.02, 0.015)])
+    img, info = X.xt_lattice_pack_host(buf)
+    (cav, ell), = walk_image(img, info["chunk_bytes"])
+    beta0 = info["beta0"]
+    pi = 3.14159265358979323846
+    assert cav[4] == 90.0 * (pi / 180.0)                                      # lag_rad
+    assert cav[5][0] == (2.0 * pi * 400e6) / (beta0 * 299792458.0)            # kz
+    assert cav[5][1] == (1.0 * 2e6) / P0C                                     # vn
+    a2, b2 = 0.02 * 0.02, 0.015 * 0.015
+    assert ell[4] == a2 * b2 and ell[5][:2] == (b2, a2) and ell[3] == 1
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+def test_config_lattices_chunking_and_fusion(cfg):
+    els = C.lattice(cfg)
+    buf = C.pack(els)
+    img, info = X.xt_lattice_pack_host(buf)
+    want = expected_maps(els, info["beta0"])
+    assert_same_maps(all_maps(img, info["chunk_bytes"]), want)
+    n_drifts = sum(1 for m in want if m[0] == "drift")
+    assert info["n_by_type"][1] == n_drifts and info["n_drift_evals"] <= n_drifts
+    for kw in (dict(fuse=False), dict(chunk_bytes=1024), dict(chunk_bytes=65536, fuse=False)):
+        img2, info2 = X.xt_lattice_pack_host(buf, **kw)
+        assert info2["chunk_bytes"] == kw.get("chunk_bytes", 8192)
+        chunks = walk_image(img2, info2["chunk_bytes"])
+        assert len(chunks) == info2["n_chunks"] and sum(len(c) for c in chunks) == info2["n_records"]
+        assert_same_maps([m for ch in chunks for r in ch for m in maps_of(r)], want)
+        assert info2["circumference"] == info["circumference"]
+    if cfg >= 2:                                             # multi-chunk, mostly fused
+        assert info["n_chunks"] > 40 and info["n_records"] < 0.5 * info["n_elements"]
+        assert info["n_drift_evals"] < 0.65 * n_drifts
+
+
+def test_empty_and_marker_only_lattices():
+    for els in ([], [Marker(), Marker()]):
+        img, info = X.xt_lattice_pack_host(pack(els))
+        assert info["n_records"] == 0 and info["n_chunks"] == 1 and len(img) == 16
+        assert walk_image(img, info["chunk_bytes"]) == [[]]
+
+
+def test_bad_buffers_and_options_are_rejected():
+    lib = X.load_library("prod")
+    good = pack([Drift(1.0)])
+    bad = [good[:-1], b"XXXX" + good[4:], good + b"\0" * 8, pack([Multipole(knl=(0.0,) * 22)]),
+           pack([Drift(float("nan"))]), pack_lattice([Drift(1.0)], -1.0, MASS0, 1.0),
+           good[:48] + struct.pack("<IId", 99, 0, 1.0)]
+    for b in bad:
+        rc = lib.xt_lattice_pack_host(b, len(b), None, None, 0, None)
+        assert rc == -2, rc                                                   # XT_ERR_BAD_LATTICE
+        assert lib.xt_last_error()
+    for kw in (dict(chunk_bytes=1000), dict(chunk_bytes=512), dict(chunk_bytes=131072)):
+        with pytest.raises(X.XtError) as e:
+            X.xt_lattice_pack_host(good, **kw)
+        assert e.value.code == -1
+    big = pack([Multipole(knl=(0.0,) * 21, ksl=(0.0,) * 21)] * 3)              # 352-byte records
+    img, info = X.xt_lattice_pack_host(big, chunk_bytes=1024)
+    assert info["n_chunks"] == 2                                              # 16 + 2 x 352 fits, the third does not
+    assert X.xt_lattice_pack_host(good)[1]["n_records"] == 1
+
+
+# ------------------------------------------------- multi-rank plumbing (gloo, world_size 2)
+def _rank_main(rank, world, port, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+    import bench
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ms = bench.reduce_max(100.0 + 50.0 * rank, world, "cpu")                # slowest rank sets the time
+    buf, coords = bench.make_inputs(0, rank)
+    np.save(os.path.join(out_dir, "r%d.npy" % rank),
+            np.array([ms, bench.whole_job_value(1000.0, world, ms), coords["x"][0], len(coords["x"]), len(buf)]))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_bench_rank_plumbing_world_size_2(tmp_path):
+    import torch.multiprocessing as mp
+    port = 29500 + (os.getpid() % 400)
+    mp.spawn(_rank_main, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    r0, r1 = (np.load(os.path.join(str(tmp_path), "r%d.npy" % r)) for r in (0, 1))
+    assert r0[0] == r1[0] == 150.0                                           # MAX over ranks on both
+    assert r0[1] == r1[1] == 2 * 1000.0 / 0.150                              # whole-job aggregate
+    assert r0[2] != r1[2] and r0[3] == r1[3] == 1000                         # own ensemble, same size
+    assert r0[4] == r1[4]                                                    # same (replicated) lattice
