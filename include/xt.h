@@ -86,7 +86,7 @@ typedef struct {
   int64_t compact_every;    /* 0: auto (1000 turns if the lattice has apertures and n_turns   */
                             /*    exceeds it); < 0: never compact; > 0: period in turns       */
   int32_t block_size;       /* 0: auto; else threads per CTA, a multiple of 32 in [32, 256]   */
-  int32_t particles_per_thread; /* 0: auto; else 1, 2 or 4                                    */
+  int32_t particles_per_thread; /* 0: auto; else 1, 2, 3 or 4                                 */
 } xt_track_opts;
 
 /* Static description of a lattice image; counts are per turn. */

@@ -37,23 +37,24 @@ int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p
 }
 
 // Launch shape of the tracking kernel: threads per CTA and particles per thread.
-// Auto rule (measured on B200, profiles/r01_shape_sweep.md): with at least ~1000 particles
-// per SM, 4 particles per thread in 128-thread CTAs (4 CTAs per SM at 128 registers) is
-// fastest; smaller ensembles need the warps more than the per-warp ILP, so 2 per thread,
-// then 1.  The kernel hands the particles out in equal shares over a whole number of CTAs
-// per SM, so the shape only has to make enough CTAs.
+// Auto rule (measured on B200, profiles/r01_shape_sweep.md): 3 particles per thread in
+// 128-thread CTAs (4 CTAs per SM at <= 128 registers) is fastest both for 1e7 particles
+// (configs[3]) and for 676 per SM (configs[2]); 4 per thread loses more to register pressure
+// than it gains in shared dispatch, 2 per thread has too little ILP per warp.  Below ~100
+// particles per SM one per thread keeps more warps alive.  The kernel hands the particles
+// out in equal shares over a whole number of CTAs per SM, so the shape only has to make
+// enough CTAs.
 int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part, int *block, int *ppt) {
   const int64_t per_sm = n_part / (lat->n_sm > 0 ? lat->n_sm : 1);
-  int auto_ppt = 4, auto_block = 128;
-  if (per_sm < 1024) auto_ppt = 2;
-  if (per_sm < 256) {
+  int auto_ppt = 3, auto_block = 128;
+  if (per_sm < 96) {
     auto_ppt = 1;
-    auto_block = 64;
+    auto_block = 32;
   }
   *ppt = (o && o->particles_per_thread) ? o->particles_per_thread : auto_ppt;
   *block = (o && o->block_size) ? o->block_size : auto_block;
-  if (*ppt != 1 && *ppt != 2 && *ppt != 4) {
-    set_error("xt_track_ex: particles_per_thread must be 0 (auto), 1, 2 or 4");
+  if (*ppt < 1 || *ppt > 4) {
+    set_error("xt_track_ex: particles_per_thread must be 0 (auto), 1, 2, 3 or 4");
     return XT_ERR_INVALID_ARG;
   }
   if (*block < 32 || *block > 256 || (*block % 32) != 0) {

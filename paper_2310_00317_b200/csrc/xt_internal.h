@@ -29,13 +29,14 @@ namespace xt {
 // A drift record may carry a second drift (TAG_POST).  The maps are applied in element order
 // with unchanged arithmetic; the dispatch is shared, and so is what two consecutive drifts
 // would both compute from the unchanged (px, py).  Slots of a multipole record, in order:
-//   {l_pre, l_post} if PRE|POST; {l_post2, 0} if POST2; {dx, dy}, {cos, sin} if MISAL;
-//   {wf, 0} if TAG_CMULT; the N+1 coefficient pairs; {cos', sin'}, {dx', dy'} if MISAL.
+//   the N+1 coefficient pairs (the kernel prefetches the first slots behind every header);
+//   {wf, 0} if TAG_CMULT; {l_pre, l_post} if PRE|POST; {l_post2, 0} if POST2;
+//   {dx, dy}, {cos, sin}, {cos', sin'}, {dx', dy'} if MISAL.
 // Unfused records:
 //
 //   TAG_DRIFT    p0 = length; {l_2nd, 0} with TAG_POST                           16 B (32 B)
 //   TAG_MULT     p0 unused; (c[n], s[n]) pairs, n = N .. 0 (Horner order)        16 + 16(N+1)
-//   TAG_CMULT    p0 = hxl;  {wf, 0};  pairs as above (c[0] = knl[0] - hxl)       32 + 16(N+1)
+//   TAG_CMULT    p0 = hxl;  pairs as above (c[0] = knl[0] - hxl); {wf, 0}         32 + 16(N+1)
 //   TAG_CAVITY   p0 = lag_rad; {kz, vn}                                          32 B
 //   TAG_SROT     p0 unused; {cos_z, sin_z}                                       32 B
 //   TAG_SHIFT    p0 unused; {dx, dy}                                             32 B

@@ -164,15 +164,14 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
         if (hxl != 0.0) {
           // -k0l + hxl(1+delta) = -(k0l - hxl) + hxl*delta : fold the constant part into c[0]
           cn[0] = knl[0] - hxl;
-          const double wf = (length != 0.0) ? (knl[0] * hxl) / length : 0.0;
           rec.type = TAG_CMULT;
           rec.p0 = hxl;
-          rec.slot(wf, 0.0);
           info.n_curved += 1;
         } else {
           rec.type = TAG_MULT;
         }
         for (int n = order; n >= 0; --n) rec.slot(cn[n], sn[n]);  // Horner order: highest first
+        if (hxl != 0.0) rec.slot((length != 0.0) ? (knl[0] * hxl) / length : 0.0, 0.0);  // {wf, 0}
         info.sum_order += order;
         break;
       }
@@ -281,16 +280,14 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
     if (post) out_rec.flags |= TAG_POST;
     if (post2) out_rec.flags |= TAG_POST2;
     if (misal) out_rec.flags |= TAG_MISAL;
+    // coefficient pairs first (the kernel prefetches the slots right behind the header), then
+    // the extras: [{wf, 0}] [{l_pre, l_post}] [{l_post2, 0}] [{dx, dy} {cos, sin} {cos', sin'} {dx', dy'}]
+    out_rec.slots = recs[m].slots;  // pairs [+ {wf, 0}]
     if (pre || post) out_rec.slot(pre ? recs[i].p0 : 0.0, post ? recs[after].p0 : 0.0);
     if (post2) out_rec.slot(recs[after + 1].p0, 0.0);
     if (misal) {
-      out_rec.slots.insert(out_rec.slots.end(), recs[j].slots.begin(), recs[j].slots.end());          // {dx, dy}
-      out_rec.slots.insert(out_rec.slots.end(), recs[j + 1].slots.begin(), recs[j + 1].slots.end());  // {cos, sin}
-    }
-    out_rec.slots.insert(out_rec.slots.end(), recs[m].slots.begin(), recs[m].slots.end());  // [{wf, 0}] + pairs
-    if (misal) {
-      out_rec.slots.insert(out_rec.slots.end(), recs[j + 3].slots.begin(), recs[j + 3].slots.end());
-      out_rec.slots.insert(out_rec.slots.end(), recs[j + 4].slots.begin(), recs[j + 4].slots.end());
+      for (size_t k : {j, j + 1, j + 3, j + 4})
+        out_rec.slots.insert(out_rec.slots.end(), recs[k].slots.begin(), recs[k].slots.end());
     }
     fused.push_back(std::move(out_rec));
     i = after + (post ? 1 : 0) + (post2 ? 1 : 0);

@@ -103,6 +103,8 @@ __device__ __forceinline__ double rcp_seed(double a) {
 }
 #endif
 
+constexpr int kPrefetch = 4;  // 16-byte slots of a record loaded ahead of its dispatch
+
 // Hot per-thread state of P particles: what drifts and kicks touch at every element.
 template <int P>
 struct Parts {
@@ -169,23 +171,24 @@ __device__ __forceinline__ void horner_first(const double2 top, const double2 c,
   }
 }
 
+// pf = the first kPrefetch pairs, already in registers; the rest comes from cs (shared memory).
 template <int P>
-__device__ __forceinline__ void horner(const double2 *__restrict__ cs, int order, const double (&x)[P],
-                                       const double (&y)[P], double (&re)[P], double (&im)[P]) {
-  // (order mod 4) leading steps, their coefficients loaded together, then groups of four
-  const double2 top = cs[0];
+__device__ __forceinline__ void horner(const double2 *__restrict__ cs, const double2 (&pf)[kPrefetch], int order,
+                                       const double (&x)[P], const double (&y)[P], double (&re)[P],
+                                       double (&im)[P]) {
+  static_assert(kPrefetch == 4, "the leading steps below take exactly the four prefetched pairs");
+  // (order mod 4) leading steps, then groups of four
+  const double2 top = pf[0];
   const int rem = order & 3;
   if (rem == 3) {
-    const double2 c1 = cs[1], c2 = cs[2], c3 = cs[3];
-    horner_first<P>(top, c1, x, y, re, im);
-    horner_step<P>(c2, x, y, re, im);
-    horner_step<P>(c3, x, y, re, im);
+    horner_first<P>(top, pf[1], x, y, re, im);
+    horner_step<P>(pf[2], x, y, re, im);
+    horner_step<P>(pf[3], x, y, re, im);
   } else if (rem == 2) {
-    const double2 c1 = cs[1], c2 = cs[2];
-    horner_first<P>(top, c1, x, y, re, im);
-    horner_step<P>(c2, x, y, re, im);
+    horner_first<P>(top, pf[1], x, y, re, im);
+    horner_step<P>(pf[2], x, y, re, im);
   } else if (rem == 1) {
-    horner_first<P>(top, cs[1], x, y, re, im);
+    horner_first<P>(top, pf[1], x, y, re, im);
   } else {
 #pragma unroll
     for (int j = 0; j < P; ++j) {
@@ -335,6 +338,57 @@ __device__ __forceinline__ void xy_shift(Parts<P> &q, const double2 d) {  // d =
   }
 }
 
+// One multipole record: [drift] [shift, rotate] kick [rotate, shift] [drift [drift]] with one
+// dispatch.  F >= 0 fixes the flag set at compile time (no flag branches), F < 0 reads it
+// from the tag; CURVED likewise (1: TAG_CMULT, 0: TAG_MULT, < 0: from the tag).  pf holds the
+// first kPrefetch slots of the record, loaded before the dispatch.
+template <int P, int F, int CURVED>
+__device__ __forceinline__ void multipole_record(Parts<P> &q, const Cold<P> &cold, const double2 *slots,
+                                                 const double2 (&pf)[kPrefetch], const uint32_t tag,
+                                                 const double p0) {
+  const uint32_t f = F >= 0 ? static_cast<uint32_t>(F) : tag;
+  const bool curved = CURVED >= 0 ? (CURVED != 0) : ((tag & TAG_TYPE_MASK) == TAG_CMULT);
+  const int order = static_cast<int>((tag >> 8) & 0xffu);
+  const double2 *extra = slots + order + 1;  // behind the coefficient pairs
+  double wf = 0.0;
+  double2 dl = make_double2(0.0, 0.0);
+  double l_post2 = 0.0;
+  if (curved) wf = (extra++)->x;
+  if (f & (TAG_PRE | TAG_POST)) dl = *extra++;
+  if (f & TAG_POST2) l_post2 = (extra++)->x;
+  if (f & TAG_PRE) drift<P>(q, cold, dl.x);
+  if (f & TAG_MISAL) {
+    xy_shift<P>(q, extra[0]);
+    s_rotation<P>(q, extra[1]);
+  }
+  double re[P], im[P];
+  horner<P>(slots, pf, order, q.x, q.y, re, im);
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    q.px[j] = q.px[j] - re[j];
+    q.py[j] = q.py[j] + im[j];
+  }
+  if (curved) {
+    const double hxl = p0;
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+      q.px[j] = XT_MADD(hxl, cold.delta(j), q.px[j]);
+      q.px[j] = XT_NMADD(wf, q.x[j], q.px[j]);
+      q.zeta[j] = XT_NMADD(XT_MUL(hxl, q.x[j]), cold.rv0v(j), q.zeta[j]);
+    }
+  }
+  if (f & TAG_MISAL) {
+    s_rotation<P>(q, extra[2]);
+    xy_shift<P>(q, extra[3]);
+  }
+  if (f & TAG_POST) {
+    DriftCoef<P> d;
+    drift_eval<P>(q, cold, d);
+    drift_apply<P>(q, d, dl.y);
+    if (f & TAG_POST2) drift_apply<P>(q, d, l_post2);
+  }
+}
+
 // Push the P particles of this thread through every record of one staged chunk.
 template <int P>
 __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp, const Cold<P> &cold,
@@ -344,65 +398,36 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
   while ((tag & TAG_TYPE_MASK) != TAG_END) {
     const RecHdr h = *reinterpret_cast<const RecHdr *>(rp);  // {tag of the NEXT record, elem, p0}
     const double2 *slots = reinterpret_cast<const double2 *>(rp + sizeof(RecHdr));
+    // the first slots, loaded before the dispatch resolves (whatever the record is; at the end
+    // of a chunk this reads up to 64 spare bytes behind it)
+    const double2 pf[kPrefetch] = {slots[0], slots[1], slots[2], slots[3]};
     const double p0 = h.p0;
     const uint32_t elem = h.elem;
     rp += tag >> 16;  // record size in bytes
-    switch (tag & TAG_TYPE_MASK) {
-      case TAG_DRIFT: {
+    switch (tag & 0xffu) {  // type | flags
+      case TAG_DRIFT:
+      case TAG_DRIFT | TAG_POST: {
         DriftCoef<P> d;
         drift_eval<P>(q, cold, d);
         drift_apply<P>(q, d, p0);
-        if (tag & TAG_POST) drift_apply<P>(q, d, slots[0].x);  // a second drift, same (px, py)
+        if (tag & TAG_POST) drift_apply<P>(q, d, pf[0].x);  // a second drift, same (px, py)
         break;
       }
-      case TAG_MULT:
-      case TAG_CMULT: {
-        // [drift] [shift, rotate] kick [rotate, shift] [drift [drift]]: one dispatch
-        double2 dl = make_double2(0.0, 0.0);
-        double l_post2 = 0.0;
-        if (tag & (TAG_PRE | TAG_POST)) dl = *slots++;
-        if (tag & TAG_POST2) l_post2 = (slots++)->x;
-        if (tag & TAG_PRE) drift<P>(q, cold, dl.x);
-        if (tag & TAG_MISAL) {
-          xy_shift<P>(q, slots[0]);
-          s_rotation<P>(q, slots[1]);
-          slots += 2;
-        }
-        const bool curved = (tag & TAG_TYPE_MASK) == TAG_CMULT;
-        double wf = 0.0;
-        double re[P], im[P];
-        if (curved) wf = (slots++)->x;
-        const int order = static_cast<int>((tag >> 8) & 0xffu);
-        horner<P>(slots, order, q.x, q.y, re, im);
-        slots += order + 1;
-#pragma unroll
-        for (int j = 0; j < P; ++j) {
-          q.px[j] = q.px[j] - re[j];
-          q.py[j] = q.py[j] + im[j];
-        }
-        if (curved) {
-          const double hxl = p0;
-#pragma unroll
-          for (int j = 0; j < P; ++j) {
-            q.px[j] = XT_MADD(hxl, cold.delta(j), q.px[j]);
-            q.px[j] = XT_NMADD(wf, q.x[j], q.px[j]);
-            q.zeta[j] = XT_NMADD(XT_MUL(hxl, q.x[j]), cold.rv0v(j), q.zeta[j]);
-          }
-        }
-        if (tag & TAG_MISAL) {
-          s_rotation<P>(q, slots[0]);
-          xy_shift<P>(q, slots[1]);
-        }
-        if (tag & TAG_POST) {
-          DriftCoef<P> d;
-          drift_eval<P>(q, cold, d);
-          drift_apply<P>(q, d, dl.y);
-          if (tag & TAG_POST2) drift_apply<P>(q, d, l_post2);
-        }
-        break;
-      }
+#define XT_MULT_CASE(F)                                                        \
+  case TAG_MULT | (F):                                                         \
+    multipole_record<P, (F), 0>(q, cold, slots, pf, tag, p0);                  \
+    break;                                                                     \
+  case TAG_CMULT | (F):                                                        \
+    multipole_record<P, (F), 1>(q, cold, slots, pf, tag, p0);                  \
+    break;
+      // the flag sets a drift-kick-drift lattice is made of, specialised at compile time ...
+      XT_MULT_CASE(0)
+      XT_MULT_CASE(TAG_POST)
+      XT_MULT_CASE(TAG_POST | TAG_POST2)
+      XT_MULT_CASE(TAG_PRE | TAG_POST | TAG_POST2)
+#undef XT_MULT_CASE
       case TAG_CAVITY: {
-        const double2 kv = slots[0];  // (kz, vn)
+        const double2 kv = pf[0];  // (kz, vn)
 #pragma unroll
         for (int j = 0; j < P; ++j) {
           if (q.alive & (1u << j)) {
@@ -422,15 +447,15 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         break;
       }
       case TAG_SROT: {
-        s_rotation<P>(q, slots[0]);
+        s_rotation<P>(q, pf[0]);
         break;
       }
       case TAG_SHIFT: {
-        xy_shift<P>(q, slots[0]);
+        xy_shift<P>(q, pf[0]);
         break;
       }
       case TAG_RECT: {
-        const double2 xr = slots[0], yr = slots[1];
+        const double2 xr = pf[0], yr = pf[1];
         uint32_t out = 0;
 #pragma unroll
         for (int j = 0; j < P; ++j) {
@@ -442,7 +467,7 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         break;
       }
       case TAG_ELLIPSE: {
-        const double2 ba = slots[0];  // (b2, a2)
+        const double2 ba = pf[0];  // (b2, a2)
         uint32_t out = 0;
 #pragma unroll
         for (int j = 0; j < P; ++j) {
@@ -453,28 +478,33 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         if (out) lose<P>(q, out, cold, elem, turns_done, a);
         break;
       }
-      default:  // cannot happen: the packer emits only the tags above
+      default:  // ... and every other combination (misaligned magnets, lone leading drifts) at run time
+        if ((tag & TAG_TYPE_MASK) == TAG_MULT || (tag & TAG_TYPE_MASK) == TAG_CMULT)
+          multipole_record<P, -1, -1>(q, cold, slots, pf, tag, p0);
         break;
     }
     tag = h.next;
   }
 }
 
-// Register budget: 65536 / (kMaxBlock * min CTAs per SM).
-#ifndef XT_MINB4
-#define XT_MINB4 2  // P = 4: 128 registers
+// Register budget per thread (CTAs of 128 threads: 65536 / (128 * CTAs per SM)).
+#ifndef XT_REGS3
+#define XT_REGS3 128
 #endif
-#ifndef XT_MINB2
-#define XT_MINB2 3  // P = 2: 80 registers
+#ifndef XT_REGS4
+#define XT_REGS4 128
 #endif
 constexpr int kMaxBlock = 256;
+template <int P>
+struct RegBudget {
+  static constexpr int value = P == 1 ? 64 : (P == 2 ? 80 : (P == 3 ? XT_REGS3 : XT_REGS4));
+};
 
 // Shared memory: [0,16) two mbarriers; [128, 128 + 8*kPitch*blockDim) cold per-thread rows;
 // then staging buffer 0 (and buffer 1 for multi-chunk lattices), 128-byte aligned, and 64
 // spare bytes (the Horner loop prefetches one coefficient pair past the record it is in).
 template <int P>
-__global__ void __launch_bounds__(kMaxBlock, P == 4 ? XT_MINB4 : (P == 2 ? XT_MINB2 : 4))
-    xt_track_kernel(const TrackArgs a) {
+__global__ void __maxnreg__(RegBudget<P>::value) xt_track_kernel(const TrackArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   const uint32_t bar0 = smem_addr(smem);
   Cold<P> cold;
@@ -662,10 +692,12 @@ int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, c
       return launch_track_p<1>(a, lat, block, st);
     case 2:
       return launch_track_p<2>(a, lat, block, st);
+    case 3:
+      return launch_track_p<3>(a, lat, block, st);
     case 4:
       return launch_track_p<4>(a, lat, block, st);
     default:
-      set_error("xt_track: particles_per_thread must be 1, 2 or 4");
+      set_error("xt_track: particles_per_thread must be 1, 2, 3 or 4");
       return XT_ERR_INVALID_ARG;
   }
 }

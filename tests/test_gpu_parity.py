@@ -287,7 +287,7 @@ def test_launch_shape_fusion_and_chunk_size_do_not_change_results(X):
     X.xt_track_ex(lat, base, 6, compact_every=-1)
     base = X.particles_to_host(base)
     assert 0.05 < (base["state"] == 0).mean() < 0.95
-    for ppt in (1, 2, 4):
+    for ppt in (1, 2, 3, 4):
         for block in (32, 96, 256):
             p = X.new_particles(lat, coords)
             X.xt_track_ex(lat, p, 6, compact_every=-1, block_size=block, particles_per_thread=ppt)

@@ -110,10 +110,15 @@ def maps_of(rec):
             out.append(("drift", s[0]))
         return out
     if typ in (T_MULT, T_CMULT):
-        l_pre = l_post = l_post2 = None
+        coef = s[0:2 * (order + 1)]                      # coefficient pairs first, then the extras
+        k = 2 * (order + 1)
+        wf = l_pre = l_post = l_post2 = None
+        if typ == T_CMULT:
+            wf = s[k]
+            k += 2
         if flags & (F_PRE | F_POST):
-            l_pre, l_post = s[0], s[1]
-            k = 2
+            l_pre, l_post = s[k], s[k + 1]
+            k += 2
         if flags & F_POST2:
             l_post2 = s[k]
             k += 2
@@ -121,17 +126,10 @@ def maps_of(rec):
             out.append(("drift", l_pre))
         if flags & F_MISAL:
             out += [("shift", s[k:k + 2]), ("srot", s[k + 2:k + 4])]
-            k += 4
-        wf = None
-        if typ == T_CMULT:
-            wf = s[k]
-            k += 2
-        coef = s[k:k + 2 * (order + 1)]
-        k += 2 * (order + 1)
         out.append(("mult", (order, p0 if typ == T_CMULT else 0.0, wf, coef)))
         if flags & F_MISAL:
-            out += [("srot", s[k:k + 2]), ("shift", s[k + 2:k + 4])]
-            k += 4
+            out += [("srot", s[k + 4:k + 6]), ("shift", s[k + 6:k + 8])]
+            k += 8
         if flags & F_POST:
             out.append(("drift", l_post))
         if flags & F_POST2:
