@@ -32,6 +32,8 @@ namespace xt {
 //   the N+1 coefficient pairs (the kernel prefetches the first slots behind every header);
 //   {wf, 0} if TAG_CMULT; {l_pre, l_post} if PRE|POST; {l_post2, 0} if POST2;
 //   {dx, dy}, {cos, sin}, {cos', sin'}, {dx', dy'} if MISAL.
+// A multipole or drift record may also end with the LimitEllipse that follows it (TAG_APER):
+// its last two slots are then {b2, a2}, {a2*b2, element index of the aperture}.
 // Unfused records:
 //
 //   TAG_DRIFT    p0 = length; {l_2nd, 0} with TAG_POST                           16 B (32 B)
@@ -59,7 +61,8 @@ enum : uint32_t {
   TAG_PRE = 0x10,   // a drift of length l_pre comes first
   TAG_POST = 0x20,  // a drift of length l_post follows the kick
   TAG_POST2 = 0x40,  // ... and a second one of length l_post2 (only with TAG_POST)
-  TAG_MISAL = 0x80   // shift + rotation before the kick, rotation + shift after it
+  TAG_MISAL = 0x80,  // shift + rotation before the kick, rotation + shift after it
+  TAG_APER = 0x8000  // (top bit of the order byte) a LimitEllipse follows the record's last map
 };
 
 struct alignas(16) RecHdr {

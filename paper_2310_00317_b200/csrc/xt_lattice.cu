@@ -292,6 +292,25 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
     fused.push_back(std::move(out_rec));
     i = after + (post ? 1 : 0) + (post2 ? 1 : 0);
   }
+  // ... and an elliptical aperture rides at the end of the multipole / drift record before it
+  if (opts.fuse) {
+    std::vector<Rec> merged;
+    merged.reserve(fused.size());
+    for (Rec &rec : fused) {
+      const bool host = !merged.empty() && !(merged.back().flags & TAG_APER) &&
+                        (merged.back().type == TAG_MULT || merged.back().type == TAG_CMULT ||
+                         merged.back().type == TAG_DRIFT);
+      if (rec.type == TAG_ELLIPSE && host) {
+        Rec &m = merged.back();
+        m.flags |= TAG_APER;
+        m.slot(rec.slots[0], rec.slots[1]);                  // {b2, a2}
+        m.slot(rec.p0, static_cast<double>(rec.elem));       // {a2 b2, element index}
+      } else {
+        merged.push_back(std::move(rec));
+      }
+    }
+    fused.swap(merged);
+  }
   info.n_records = static_cast<int64_t>(fused.size());
   for (const Rec &rec : fused) {
     if (rec.type == TAG_DRIFT) info.n_drift_evals += 1;

@@ -348,7 +348,7 @@ __device__ __forceinline__ void multipole_record(Parts<P> &q, const Cold<P> &col
                                                  const double p0) {
   const uint32_t f = F >= 0 ? static_cast<uint32_t>(F) : tag;
   const bool curved = CURVED >= 0 ? (CURVED != 0) : ((tag & TAG_TYPE_MASK) == TAG_CMULT);
-  const int order = static_cast<int>((tag >> 8) & 0xffu);
+  const int order = static_cast<int>((tag >> 8) & 0x7fu);
   const double2 *extra = slots + order + 1;  // behind the coefficient pairs
   double wf = 0.0;
   double2 dl = make_double2(0.0, 0.0);
@@ -387,6 +387,20 @@ __device__ __forceinline__ void multipole_record(Parts<P> &q, const Cold<P> &col
     drift_apply<P>(q, d, dl.y);
     if (f & TAG_POST2) drift_apply<P>(q, d, l_post2);
   }
+}
+
+// A: elliptical aperture (x^2 b^2 + y^2 a^2 <= a^2 b^2, edge inclusive, NaN lost).
+template <int P>
+__device__ __forceinline__ void limit_ellipse(Parts<P> &q, const Cold<P> &cold, const double2 ba, const double a2b2,
+                                              uint32_t elem, int64_t turns_done, const TrackArgs &a) {
+  uint32_t out = 0;
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    const double tt = XT_MADD(XT_MUL(q.x[j], q.x[j]), ba.x, XT_MUL(XT_MUL(q.y[j], q.y[j]), ba.y));
+    out |= (tt <= a2b2) ? 0u : (1u << j);
+  }
+  out &= q.alive;
+  if (out) lose<P>(q, out, cold, elem, turns_done, a);
 }
 
 // Push the P particles of this thread through every record of one staged chunk.
@@ -467,21 +481,19 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         break;
       }
       case TAG_ELLIPSE: {
-        const double2 ba = pf[0];  // (b2, a2)
-        uint32_t out = 0;
-#pragma unroll
-        for (int j = 0; j < P; ++j) {
-          const double tt = XT_MADD(XT_MUL(q.x[j], q.x[j]), ba.x, XT_MUL(XT_MUL(q.y[j], q.y[j]), ba.y));
-          out |= (tt <= p0) ? 0u : (1u << j);
-        }
-        out &= q.alive;
-        if (out) lose<P>(q, out, cold, elem, turns_done, a);
+        limit_ellipse<P>(q, cold, pf[0], p0, elem, turns_done, a);  // pf[0] = (b2, a2), p0 = a2 b2
         break;
       }
       default:  // ... and every other combination (misaligned magnets, lone leading drifts) at run time
         if ((tag & TAG_TYPE_MASK) == TAG_MULT || (tag & TAG_TYPE_MASK) == TAG_CMULT)
           multipole_record<P, -1, -1>(q, cold, slots, pf, tag, p0);
         break;
+    }
+    if (tag & TAG_APER) {
+      // the record ends with an elliptical aperture: {b2, a2}, {a2 b2, element index} are its last slots
+      const double2 ba = *reinterpret_cast<const double2 *>(rp - 32);
+      const double2 ce = *reinterpret_cast<const double2 *>(rp - 16);
+      limit_ellipse<P>(q, cold, ba, ce.x, static_cast<uint32_t>(ce.y), turns_done, a);
     }
     tag = h.next;
   }

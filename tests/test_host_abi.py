@@ -26,7 +26,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 P0C, MASS0 = 450e9, 938272088.16
 
 T_END, T_DRIFT, T_MULT, T_CAV, T_SROT, T_SHIFT, T_RECT, T_ELL, T_CMULT = range(9)
-F_PRE, F_POST, F_POST2, F_MISAL = 0x10, 0x20, 0x40, 0x80
+F_PRE, F_POST, F_POST2, F_MISAL, F_APER = 0x10, 0x20, 0x40, 0x80, 0x8000
 
 
 def pack(els):
@@ -91,7 +91,7 @@ def walk_image(img, chunk_bytes):
             nxt, elem, p0 = struct.unpack_from("<IId", img, pos)
             assert size >= 16 and size % 16 == 0
             slots = struct.unpack_from("<%dd" % ((size - 16) // 8), img, pos + 16)
-            recs.append((tag & 0xF, tag & 0xF0, (tag >> 8) & 0xFF, elem, p0, slots))
+            recs.append((tag & 0xF, tag & 0x80F0, (tag >> 8) & 0x7F, elem, p0, slots))
             pos += size
             tag = nxt
         assert pos - start <= chunk_bytes
@@ -104,6 +104,10 @@ def maps_of(rec):
     """Element maps a record stands for, in order, as (kind, parameters)."""
     typ, flags, order, elem, p0, s = rec
     out, k = [], 0
+    if flags & F_APER:                                   # trailing LimitEllipse: {b2, a2}, {a2 b2, elem}
+        inner = maps_of((typ, flags & ~F_APER, order, elem, p0, s[:-4]))
+        assert s[-2] == s[-4] * s[-3] and s[-1] == int(s[-1]) > elem
+        return inner + [("ellipse", (s[-4], s[-3]))]
     if typ == T_DRIFT:
         out.append(("drift", p0))
         if flags & F_POST:
@@ -221,8 +225,9 @@ def test_packer_encodes_every_map_in_order_with_prescaled_coefficients(fuse):
     assert sum(len(c) for c in chunks) == info["n_records"]
     assert_same_maps(all_maps(img, info["chunk_bytes"]), expected_maps(ALL_TYPES, info["beta0"]))
     if fuse:
-        # [D shift rot M rot shift D D], cavity, D, rect, [D M], ellipse, [M D D], [D M]
-        assert info["n_records"] == 8
+        # [D shift rot M rot shift D D], cavity, D, rect, [D M + ellipse], [M D D], [D M]
+        assert info["n_records"] == 7
+        assert chunks[0][4][1] == (F_PRE | F_APER)
         first = chunks[0][0]
         assert first[0] == T_CMULT and first[1] == (F_PRE | F_POST | F_POST2 | F_MISAL) and first[3] == 3
         assert info["n_drift_evals"] == 2 + 1 + 1 + 1 + 1           # pre + post, D, [D M], [M D D], [D M]
