@@ -207,6 +207,7 @@ def main():
     ap.add_argument("--particles", type=int, default=0, help="override the particle count (testing only)")
     ap.add_argument("--block", type=int, default=0)
     ap.add_argument("--ppt", type=int, default=0, help="particles per thread (0: auto)")
+    ap.add_argument("--chunk", type=int, default=0, help="staging-buffer bytes (0: library default)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and configs[2] legs")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -235,7 +236,7 @@ def main():
     buf, coords = make_inputs(cfg, rank)
     if args.particles:
         coords = C.subsample(coords, slice(0, args.particles))
-    lat = X.xt_lattice_create(buf)
+    lat = X.xt_lattice_create_ex(buf, chunk_bytes=args.chunk) if args.chunk else X.xt_lattice_create(buf)
     info = lat.info
     n_el = info["n_elements"]
     n_part = len(coords["x"])

@@ -1,28 +1,29 @@
 // The tracking kernel for sm_100a.
 //
 // "Xtrack ... assembles and compiles a C kernel ... able to track the entire beamline"
-// (PAPER.md:74): here that kernel is hand-written.  One thread owns P particles (P = 1, 2
-// or 4, interleaved so that every global access is coalesced) and keeps their hot state in
-// registers across all elements and turns; SoA FP64 loads/stores happen only at the start and
-// end of the launch (and, for a particle that hits an aperture, once at the moment it is
-// lost).  The lattice image is streamed chunk by chunk from L2 into shared memory with 1-D
-// TMA bulk copies (cp.async.bulk + mbarrier complete_tx), double-buffered; every thread of
-// the CTA reads the same record, so each LDS.128 is a broadcast.  Element dispatch is a
-// switch on a value all lanes share (warp-uniform).  Multipoles are a complex Horner
-// recurrence of FMAs.
+// (PAPER.md:74): here that kernel is hand-written and interprets a packed record stream.
+// One thread owns P particles (P = 1..4, interleaved so that every global access is
+// coalesced) and keeps their hot state (x, px, y, py, zeta) in registers across all elements
+// and turns; SoA FP64 loads/stores happen only at the start and end of the launch (and, for a
+// particle that hits an aperture, once at the moment it is lost).  The lattice image is
+// streamed chunk by chunk from L2 into shared memory with 1-D TMA bulk copies
+// (cp.async.bulk + mbarrier complete_tx), double-buffered; every thread of the CTA reads the
+// same record, so each LDS.128 is a broadcast.  Dispatch is a switch on a value all lanes
+// share (warp-uniform); a record is usually a fused [drift] kick [drift drift] group
+// (xt_internal.h).  Multipoles are a complex Horner recurrence of FMAs.
 //
-// Why P > 1 (profiles/r01b_*): with one particle per thread 58 % of the issued warp
-// instructions were not FP64 (dispatch, LDS, branches, the slow-path guards of sqrt and /)
-// and the FP64 pipe sat at 49 %.  P particles per thread share every one of those
-// instructions and give the scheduler P independent FP64 chains per warp.
+// Why P > 1 (profiles/r01b_track_p1_summary.md): with one particle per thread 58 % of the
+// issued warp instructions were not FP64 (dispatch, LDS, branches, the slow-path guards of
+// sqrt and /) and the FP64 pipe sat at 49 %.  P particles per thread share every one of those
+// instructions and give each warp P independent FP64 chains.
 //
-// Arithmetic.  The maps are written as plain a*b + c expressions in the canonical order of
-// DESIGN.md section 5.  The validation build (--fmad=false, XT_FMAD_OFF) evaluates exactly
-// those trees with IEEE sqrt and division and is bit-identical to the oracle on cavity-free
-// lattices.  The production build lets nvcc contract a*b + c into DFMA and replaces the
-// drift's sqrt + division by branch-free Newton sequences on the MUFU.RSQ64H / MUFU.RCP64H
-// seeds (DESIGN.md section 6 "fast drift"): same formula, a few 1e-16 relative on the
-// increments, inside the 1e-12 parity tolerance with two orders of magnitude to spare.
+// Arithmetic.  The maps are written in the canonical order of DESIGN.md section 5 through
+// XT_MADD / XT_NMADD / XT_MUL.  The validation build (--fmad=false, XT_FMAD_OFF) evaluates
+// exactly those trees with IEEE sqrt and division and is bit-identical to the oracle on
+// cavity-free lattices.  The production build fuses every a*b + c into one DFMA (explicitly,
+// so that results do not depend on the launch shape) and replaces the drift's sqrt + division
+// by branch-free Newton sequences on the MUFU.RSQ64H / MUFU.RCP64H seeds (DESIGN.md section
+// 6.3): same formula, <= 2 ulp on the increments, far inside the 1e-12 parity tolerance.
 #include "xt_internal.h"
 
 namespace xt {
