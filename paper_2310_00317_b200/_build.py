@@ -22,6 +22,9 @@ LIBS: Dict[str, Dict] = {
     "prod": {"path": os.path.join(HERE, "libxt_b200.so"), "flags": []},
     "nofma": {"path": os.path.join(HERE, "libxt_b200_nofma.so"),
               "flags": ["--fmad=false", "-DXT_FMAD_OFF"]},
+    # optional, built on first use: production FMA fusion with IEEE sqrt and division in the drift
+    # (separates the two differences between the production and the validation arithmetic)
+    "ieee_drift": {"path": os.path.join(HERE, "libxt_b200_ieee_drift.so"), "flags": ["-DXT_CANONICAL_DRIFT"]},
 }
 
 COMMON = [

@@ -26,7 +26,8 @@ namespace xt {
 // Fused records.  A multipole record may carry its neighbours: the drift before it
 // (TAG_PRE), the XYShift + SRotation before and SRotation + XYShift after it (TAG_MISAL: a
 // misaligned magnet), and one or two drifts after it (TAG_POST, + TAG_POST2).
-// A drift record may carry a second drift (TAG_POST).  The maps are applied in element order
+// A drift record may carry a second drift (TAG_POST); an XYShift record the SRotation that
+// follows it and vice versa (TAG_POST: second slot).  The maps are applied in element order
 // with unchanged arithmetic; the dispatch is shared, and so is what two consecutive drifts
 // would both compute from the unchanged (px, py).  Slots of a multipole record, in order:
 //   the N+1 coefficient pairs (the kernel prefetches the first slots behind every header);

@@ -264,6 +264,15 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
     const bool misal = is(j, TAG_SHIFT) && is(j + 1, TAG_SROT) && is_mult(j + 2) && is(j + 3, TAG_SROT) &&
                        is(j + 4, TAG_SHIFT);
     if (!misal && !is_mult(j)) {  // not a magnet group
+      // half of a misalignment wrapper cut off from its magnet (by an aperture): still one dispatch
+      if ((is(i, TAG_SHIFT) && is(i + 1, TAG_SROT)) || (is(i, TAG_SROT) && is(i + 1, TAG_SHIFT))) {
+        Rec t = std::move(recs[i]);
+        t.flags |= TAG_POST;
+        t.slots.insert(t.slots.end(), recs[i + 1].slots.begin(), recs[i + 1].slots.end());
+        fused.push_back(std::move(t));
+        i += 2;
+        continue;
+      }
       fused.push_back(std::move(recs[i++]));
       continue;
     }

@@ -23,7 +23,8 @@
 // cavity-free lattices.  The production build fuses every a*b + c into one DFMA (explicitly,
 // so that results do not depend on the launch shape) and replaces the drift's sqrt + division
 // by branch-free Newton sequences on the MUFU.RSQ64H / MUFU.RCP64H seeds (DESIGN.md section
-// 6.3): same formula, <= 2 ulp on the increments, far inside the 1e-12 parity tolerance.
+// 6.3): same formula, <= 2 ulp on the increments; the measured distance to the oracle is set by
+// FMA fusion, not by this block (<= 0.5 of the 1e-12 bar either way).
 #include "xt_internal.h"
 
 namespace xt {
@@ -90,7 +91,13 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 #endif
 #define XT_MUL(a, b) __dmul_rn((a), (b))
 
-#ifndef XT_FMAD_OFF
+// XT_CANONICAL_DRIFT: IEEE sqrt and division in the canonical order of DESIGN.md section 5
+// (always in the validation build; -DXT_CANONICAL_DRIFT gives a production build with them).
+#if defined(XT_FMAD_OFF) && !defined(XT_CANONICAL_DRIFT)
+#define XT_CANONICAL_DRIFT
+#endif
+
+#ifndef XT_CANONICAL_DRIFT
 // MUFU.RSQ64H / MUFU.RCP64H: ~20-bit seeds computed from the high word of the operand.
 __device__ __forceinline__ double rsqrt_seed(double a) {
   double r;
@@ -269,10 +276,10 @@ __device__ __forceinline__ void drift_eval(const Parts<P> &q, const Cold<P> &col
     const double t1 = XT_MUL(q.px[j], q.px[j]);
     const double pxy2 = XT_MADD(q.py[j], q.py[j], t1);
     const double rad = opd2[j] - pxy2;
-#ifdef XT_FMAD_OFF
+#ifdef XT_CANONICAL_DRIFT
     const double pz = sqrt(rad);
     const double s1 = pz + b[j];
-    const double den = pz * s1;
+    const double den = XT_MUL(pz, s1);
     d.u[j] = 1.0 / den;
     d.v[j] = s1;
 #else
@@ -294,9 +301,9 @@ template <int P>
 __device__ __forceinline__ void drift_apply(Parts<P> &q, const DriftCoef<P> &d, const double length) {
 #pragma unroll
   for (int j = 0; j < P; ++j) {
-#ifdef XT_FMAD_OFF
-    const double lr = length * d.u[j];   // L/(pz (pz + b))
-    const double lpz = lr * d.v[j];      // L/pz
+#ifdef XT_CANONICAL_DRIFT
+    const double lr = XT_MUL(length, d.u[j]);   // L/(pz (pz + b))
+    const double lpz = XT_MUL(lr, d.v[j]);  // L/pz
 #else
     const double lpz = XT_MUL(length, d.u[j]);
     const double lr = XT_MUL(lpz, d.v[j]);
@@ -461,12 +468,16 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
         }
         break;
       }
-      case TAG_SROT: {
+      case TAG_SROT:
+      case TAG_SROT | TAG_POST: {
         s_rotation<P>(q, pf[0]);
+        if (tag & TAG_POST) xy_shift<P>(q, pf[1]);  // rotation, then shift: the way out of a misaligned magnet
         break;
       }
-      case TAG_SHIFT: {
+      case TAG_SHIFT:
+      case TAG_SHIFT | TAG_POST: {
         xy_shift<P>(q, pf[0]);
+        if (tag & TAG_POST) s_rotation<P>(q, pf[1]);  // shift, then rotation: the way in
         break;
       }
       case TAG_RECT: {

@@ -446,3 +446,43 @@ def test_full_size_cfg3_sampled_against_oracle(X):
     O.track(buf, ref, 1, threads=THREADS, min_margin=mm)
     assert_losses_match(got, ref, mm)
     assert_close(got, ref, 1e-12, sel=ref["state"] == 1)
+
+
+def test_full_size_cfg1_sampled_against_oracle(X):
+    """BASELINE.json configs[1] at its full 10^6 particles (single-chunk lattice: the warps run
+    free, no CTA-level synchronisation), 1 turn at 1e-12 and 20 turns at 1e-10; the oracle
+    recomputes a strided sample one by one."""
+    import torch
+    coords = C.particles(1)
+    n = len(coords["x"])
+    assert n == 1_000_000
+    buf = packed(1)
+    idx = np.arange(7, n, 250)
+    sub = C.subsample(coords, idx)
+    lat = X.xt_lattice_create(buf)
+    for turns, rtol in ((1, 1e-12), (20, 1e-10)):
+        p = X.new_particles(lat, coords)
+        X.xt_track(lat, p, turns)
+        torch.cuda.synchronize()
+        assert int((p["state"] == 1).sum().item()) == n          # the literal config[1] loses nothing
+        assert int(p["at_turn"].sum().item()) == n * turns
+        got = {k: v[torch.from_numpy(idx).cuda()].cpu().numpy() for k, v in p.items()}
+        ref = O.new_particles(buf, sub)
+        mm = np.full(len(idx), np.inf)
+        O.track(buf, ref, turns, threads=THREADS, min_margin=mm)
+        assert_losses_match(got, ref, mm)
+        assert_close(got, ref, rtol)
+        del p
+    lat.close()
+
+
+def test_fp64_probes_are_ordered(X):
+    """The roofline denominator and the two operand-pattern probes: shared
+    operands are fastest, three distinct registers slowest, the Horner recurrence in between."""
+    peak, _ = X.xt_fp64_fma_peak()
+    distinct, _ = X.xt_fp64_fma_probe(1)
+    horner, _ = X.xt_fp64_fma_probe(2)
+    assert 20e12 < peak < 40e12                     # B200: 148 SM x 64 lanes x 2 x ~1.9 GHz = 37 TFLOP/s nominal
+    assert 0.5 * peak < distinct < horner < peak
+    with pytest.raises(X.XtError):
+        X.xt_fp64_fma_probe(3)

@@ -140,6 +140,9 @@ def maps_of(rec):
             out.append(("drift", l_post2))
         assert k == len(s)
         return out
+    if typ in (T_SROT, T_SHIFT) and flags & F_POST:      # half a misalignment wrapper: two transforms
+        a, b = ("srot", "shift") if typ == T_SROT else ("shift", "srot")
+        return [(a, s[0:2]), (b, s[2:4])]
     return [({T_CAV: "cavity", T_SROT: "srot", T_SHIFT: "shift", T_RECT: "rect", T_ELL: "ellipse"}[typ], s)]
 
 
