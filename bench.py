@@ -307,9 +307,9 @@ def main():
                                "nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2 TFLOP/s" % peak_ms,
                 "kernel": "xt_track_kernel", "kernel_ms": kernel_ms,
                 "flops_per_particle_turn": {"algorithmic": f_min, "executed": f_exec},
-                # DRAM bytes of one launch: the --set full capture (profiles/r01i_track_cfg3_summary.md:
-                # dram__bytes_read + dram__bytes_write = 77.1 B per particle) scaled to this launch
-                "traffic": 77.1 * n_part if cfg == 3 else None,
+                # DRAM bytes of one launch: the --set full capture (profiles/r01m_track_cfg3_summary.md:
+                # dram__bytes_read + dram__bytes_write = 76.9 B per particle) scaled to this launch
+                "traffic": 76.9 * n_part if cfg == 3 else None,
                 # the same DFMA count with the operand shapes of this arithmetic
                 "operand_pattern_ceilings_tflops": probe,
             },

@@ -37,16 +37,17 @@ int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p
 }
 
 // Launch shape of the tracking kernel: threads per CTA and particles per thread.
-// Auto rule (measured on B200, profiles/r01_shape_sweep.md): 3 particles per thread in
-// 128-thread CTAs (4 CTAs per SM at <= 128 registers) is fastest both for 1e7 particles
-// (configs[3]) and for 676 per SM (configs[2]); 4 per thread loses more to register pressure
-// than it gains in shared dispatch, 2 per thread has too little ILP per warp.  Below ~100
-// particles per SM one per thread keeps more warps alive.  The kernel hands the particles
-// out in equal shares over a whole number of CTAs per SM, so the shape only has to make
-// enough CTAs.
+// Auto rule (measured on B200, profiles/r01_shape_sweep.md): 128-thread CTAs, 4 CTAs per SM
+// at <= 128 registers.  4 particles per thread when there are several waves of them
+// (configs[3]: 0.659 against 0.651 with 3), 3 per thread for smaller ensembles, where the
+// number of warps matters more (configs[2], 676 particles per SM: 0.49 against 0.38 with 4;
+// 2 per thread has too little ILP per warp: 0.47).  Below ~100 particles per SM one per
+// thread keeps more warps alive.  The kernel hands the particles out in equal shares over a
+// whole number of CTAs per SM, so the shape only has to make enough CTAs.
 int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part, int *block, int *ppt) {
   const int64_t per_sm = n_part / (lat->n_sm > 0 ? lat->n_sm : 1);
-  int auto_ppt = 3, auto_block = 128;
+  int auto_ppt = 4, auto_block = 128;
+  if (per_sm < 4096) auto_ppt = 3;
   if (per_sm < 96) {
     auto_ppt = 1;
     auto_block = 32;

@@ -111,7 +111,14 @@ __device__ __forceinline__ double rcp_seed(double a) {
 }
 #endif
 
-constexpr int kPrefetch = 4;  // 16-byte slots of a record loaded ahead of its dispatch
+constexpr int kPrefetch = 4;  // 16-byte slots of a record loaded ahead of its dispatch ...
+#ifndef XT_PF4
+#define XT_PF4 2
+#endif
+template <int P>
+struct Prefetched {  // ... of which this many really are (the rest is read where it is used)
+  static constexpr int value = P >= 4 ? XT_PF4 : kPrefetch;
+};
 
 // Hot per-thread state of P particles: what drifts and kicks touch at every element.
 template <int P>
@@ -184,17 +191,20 @@ template <int P>
 __device__ __forceinline__ void horner(const double2 *__restrict__ cs, const double2 (&pf)[kPrefetch], int order,
                                        const double (&x)[P], const double (&y)[P], double (&re)[P],
                                        double (&im)[P]) {
-  static_assert(kPrefetch == 4, "the leading steps below take exactly the four prefetched pairs");
+  static_assert(kPrefetch == 4, "the leading steps below take exactly the four leading pairs");
+  constexpr int kHave = Prefetched<P>::value;
   // (order mod 4) leading steps, then groups of four
   const double2 top = pf[0];
   const int rem = order & 3;
   if (rem == 3) {
+    const double2 c2 = kHave > 2 ? pf[2] : cs[2], c3 = kHave > 3 ? pf[3] : cs[3];
     horner_first<P>(top, pf[1], x, y, re, im);
-    horner_step<P>(pf[2], x, y, re, im);
-    horner_step<P>(pf[3], x, y, re, im);
+    horner_step<P>(c2, x, y, re, im);
+    horner_step<P>(c3, x, y, re, im);
   } else if (rem == 2) {
+    const double2 c2 = kHave > 2 ? pf[2] : cs[2];
     horner_first<P>(top, pf[1], x, y, re, im);
-    horner_step<P>(pf[2], x, y, re, im);
+    horner_step<P>(c2, x, y, re, im);
   } else if (rem == 1) {
     horner_first<P>(top, pf[1], x, y, re, im);
   } else {
@@ -422,7 +432,9 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
     const double2 *slots = reinterpret_cast<const double2 *>(rp + sizeof(RecHdr));
     // the first slots, loaded before the dispatch resolves (whatever the record is; at the end
     // of a chunk this reads up to 64 spare bytes behind it)
-    const double2 pf[kPrefetch] = {slots[0], slots[1], slots[2], slots[3]};
+    constexpr int kHave = Prefetched<P>::value;
+    const double2 zero2 = make_double2(0.0, 0.0);
+    const double2 pf[kPrefetch] = {slots[0], slots[1], kHave > 2 ? slots[2] : zero2, kHave > 3 ? slots[3] : zero2};
     const double p0 = h.p0;
     const uint32_t elem = h.elem;
     rp += tag >> 16;  // record size in bytes
