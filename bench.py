@@ -275,6 +275,7 @@ def main():
     total_ms = t_begin.elapsed_time(t_end)
     kernel_ms = float(np.mean([a.elapsed_time(b) for a, b in kev]))
     alive = int((work["state"] == 1).sum().item())
+    completed_turns = int(work["at_turn"].sum().item())     # alive particle-turns of one step (at_turn starts at 0)
     total_ms = reduce_max(total_ms, world, "cuda")
     ms_per_step = total_ms / args.steps
     units_per_step = float(n_part) * n_el * turns            # per rank (nominal: lost ones included)
@@ -296,6 +297,8 @@ def main():
                        "particles_per_thread": args.ppt or "auto", "records_per_turn": info["n_records"],
                        "lattice_image_bytes": info["image_bytes"], "tma_chunks_per_turn": info["n_chunks"]},
             "particle_turns_per_s": world * n_part * turns / (ms_per_step * 1e-3),
+            # visits of particles that were still alive (completed turns only): SURVEY.md 8(d)
+            "alive_particle_element_turns_per_s": world * float(completed_turns) * n_el / (ms_per_step * 1e-3),
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {
@@ -366,6 +369,7 @@ def main():
             l2.close()
         # ---- cpu_baseline: the oracle as it stands on a bounded sample of the same workload
         line["cpu_baseline"] = {k: v for k, v in oracle_sample(cfg, buf, coords).items() if k != "seconds"}
+        line["cpu_baseline"]["host_cores_on_this_box"] = os.cpu_count()
     if rank == 0:
         print(json.dumps(line))
     if world > 1:

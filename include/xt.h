@@ -35,7 +35,8 @@ typedef enum {
   XT_ERR_BAD_LATTICE = -2, /* bad magic/version/size, unknown type, truncated buffer,         */
                            /* order > XT_MAX_ORDER, non-finite parameter, p0c/mass0 <= 0      */
   XT_ERR_CUDA = -3,        /* CUDA runtime failure (message in xt_last_error)                 */
-  XT_ERR_NOMEM = -4        /* host or device allocation failed                                */
+  XT_ERR_NOMEM = -4,       /* host or device allocation failed                                */
+  XT_ERR_UNSTABLE = -5     /* xt_twiss4d: probe particle lost, singular map or no convergence  */
 } xt_status;
 
 #define XT_MAX_ORDER 20
@@ -173,6 +174,25 @@ int xt_fp64_fma_peak(double *flops_per_s, double *ms, void *cuda_stream);
  * 1 = three distinct register operands per DFMA; 2 = the complex Horner recurrence of step M2
  * for 4 particles per thread, coefficients broadcast from shared memory, no lattice. */
 int xt_fp64_fma_probe(int pattern, double *flops_per_s, double *ms, void *cuda_stream);
+
+/* Twiss from tracking, 4-D ("Twiss module"): the closed
+ * orbit at the start of the line for momentum deviation delta0 (zeta = 0) by Newton iteration on
+ * the one-turn map (step 1), the 4x4 one-turn Jacobian there by central differences of tracked
+ * particles (step 2; steps 1e-6 m / 1e-8 rad), and the uncoupled linear optics per plane (step 3:
+ * cos mu = (M11+M22)/2, beta = M12/sin mu, alpha = (M11-M22)/(2 sin mu)).  Every Newton step is one
+ * xt_track launch of nine particles through the whole line; only the 4x4 algebra is host code.
+ * guess4 (HOST, x px y py; may be NULL = origin).  Synchronises the stream.  XT_ERR_UNSTABLE if a
+ * probe particle is lost, M - 1 is singular, or 25 steps do not reach |dz| < 1e-13; an unstable
+ * plane (|cos mu| >= 1) is reported through stable = 0 and NaN optics, not as an error. */
+typedef struct {
+  double co[4];                 /* closed orbit x, px, y, py                                    */
+  double m[16];                 /* one-turn Jacobian at the closed orbit, row-major              */
+  double betx, alfx, mux, qx_frac; /* mu in rad in (-pi, pi], q = mu/2pi mod 1                    */
+  double bety, alfy, muy, qy_frac;
+  int32_t iterations, stable;
+} xt_twiss4d_result;
+int xt_twiss4d(const xt_lattice *lat, double delta0, const double *guess4, xt_twiss4d_result *out,
+               void *cuda_stream);
 
 /* Number of kernels the library has launched from this process so far (bench bookkeeping). */
 int64_t xt_launch_count(void);

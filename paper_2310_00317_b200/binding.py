@@ -43,6 +43,12 @@ class xt_lattice_opts(ctypes.Structure):
     _fields_ = [("chunk_bytes", ctypes.c_int64), ("fuse", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
+class xt_twiss4d_result(ctypes.Structure):
+    _fields_ = ([("co", ctypes.c_double * 4), ("m", ctypes.c_double * 16)] +
+                [(k, ctypes.c_double) for k in ("betx", "alfx", "mux", "qx_frac", "bety", "alfy", "muy", "qy_frac")] +
+                [("iterations", ctypes.c_int32), ("stable", ctypes.c_int32)])
+
+
 class xt_lattice_info(ctypes.Structure):
     _fields_ = [("n_elements", ctypes.c_int64), ("n_records", ctypes.c_int64),
                 ("n_chunks", ctypes.c_int64), ("image_bytes", ctypes.c_int64),
@@ -79,6 +85,8 @@ SIGNATURES = {
     "xt_fp64_fma_peak": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), _VP]),
     "xt_fp64_fma_probe": (ctypes.c_int, [ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                          ctypes.POINTER(ctypes.c_double), _VP]),
+    "xt_twiss4d": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
+                                  ctypes.POINTER(xt_twiss4d_result), _VP]),
     "xt_launch_count": (_I64, []),
     "xt_last_error": (ctypes.c_char_p, []),
     "xt_build_info": (ctypes.c_char_p, []),
@@ -330,6 +338,18 @@ def xt_fp64_fma_probe(pattern: int, stream=None, kind: str = "prod"):
     f, ms = ctypes.c_double(), ctypes.c_double()
     _check(lib, lib.xt_fp64_fma_probe(int(pattern), ctypes.byref(f), ctypes.byref(ms), _stream_ptr(stream)))
     return f.value, ms.value
+
+
+def xt_twiss4d(lat: Lattice, delta0: float = 0.0, guess4=None, stream=None) -> Dict:
+    """Closed orbit, one-turn matrix and uncoupled optics at the start of the line (see include/xt.h)."""
+    res = xt_twiss4d_result()
+    g = (ctypes.c_double * 4)(*[float(v) for v in guess4]) if guess4 is not None else None
+    _check(lat._lib, lat._lib.xt_twiss4d(lat.handle, float(delta0), g, ctypes.byref(res), _stream_ptr(stream)))
+    out = {k: getattr(res, k) for k in ("betx", "alfx", "mux", "qx_frac", "bety", "alfy", "muy", "qy_frac",
+                                        "iterations", "stable")}
+    out["co"] = np.array(list(res.co))
+    out["m"] = np.array(list(res.m)).reshape(4, 4)
+    return out
 
 
 def xt_launch_count(kind: str = "prod") -> int:

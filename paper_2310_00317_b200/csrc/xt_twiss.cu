@@ -1,0 +1,194 @@
+// Twiss from tracking, 4-D ("Twiss module"):
+//   1. "the closed orbit is found by a root finder" applied to the one-turn map,
+//   2. "the Jacobian matrix of the one-turn map is computed by central differences" of
+//      tracked particles,
+//   3. the linear optics follows from that matrix (here: the uncoupled reading per plane,
+//      cos mu = (M11 + M22)/2, beta = M12/sin mu, alpha = (M11 - M22)/(2 sin mu)).
+// The tracker is the inner loop of everything: each Newton step is ONE xt_track launch of
+// nine particles (the orbit and +-h along x, px, y, py) through the whole line; only the
+// 4 x 4 linear algebra runs on the host.
+#include <cmath>
+
+#include "xt_internal.h"
+
+namespace xt {
+namespace {
+
+constexpr int kProbe = 9;      // orbit + 2 x 4 displaced particles
+constexpr int kArr = 14;       // device arrays of the probe ensemble
+constexpr double kStep[4] = {1e-6, 1e-8, 1e-6, 1e-8};  // central-difference steps: x, px, y, py
+
+struct Probe {
+  double *d[10] = {};    // x px y py zeta delta ptau rpp rvv s
+  int64_t *i[4] = {};    // at_turn state particle_id at_element
+  void *block = nullptr;
+};
+
+int solve4(double a[4][5]) {  // Gaussian elimination with partial pivoting on [A | b]
+  for (int c = 0; c < 4; ++c) {
+    int piv = c;
+    for (int r = c + 1; r < 4; ++r)
+      if (std::fabs(a[r][c]) > std::fabs(a[piv][c])) piv = r;
+    if (a[piv][c] == 0.0) return -1;
+    if (piv != c)
+      for (int k = 0; k < 5; ++k) std::swap(a[piv][k], a[c][k]);
+    for (int r = c + 1; r < 4; ++r) {
+      const double f = a[r][c] / a[c][c];
+      for (int k = c; k < 5; ++k) a[r][k] -= f * a[c][k];
+    }
+  }
+  for (int r = 3; r >= 0; --r) {
+    double s = a[r][4];
+    for (int k = r + 1; k < 4; ++k) s -= a[r][k] * a[k][4];
+    a[r][4] = s / a[r][r];
+  }
+  return 0;
+}
+
+// One launch: track the orbit z and its eight neighbours for one turn.
+// out[0] = image of z, jac = central-difference Jacobian (row-major).  Returns XT_ERR_UNSTABLE
+// if any of the nine particles is lost or non-finite.
+int one_turn_and_jacobian(const xt_lattice *lat, const Probe &pr, const double z[4], double delta0, double out[4],
+                          double jac[16], cudaStream_t st) {
+  double h_x[4][kProbe];
+  for (int c = 0; c < 4; ++c)
+    for (int k = 0; k < kProbe; ++k) h_x[c][k] = z[c];
+  for (int c = 0; c < 4; ++c) {
+    h_x[c][1 + 2 * c] += kStep[c];
+    h_x[c][2 + 2 * c] -= kStep[c];
+  }
+  double zeros[kProbe] = {}, deltas[kProbe];
+  int64_t ones[kProbe], izeros[kProbe] = {};
+  for (int k = 0; k < kProbe; ++k) {
+    deltas[k] = delta0;
+    ones[k] = 1;
+  }
+  const size_t nb = kProbe * 8;
+  for (int c = 0; c < 4; ++c) XT_CUDA(cudaMemcpyAsync(pr.d[c], h_x[c], nb, cudaMemcpyHostToDevice, st));
+  XT_CUDA(cudaMemcpyAsync(pr.d[4], zeros, nb, cudaMemcpyHostToDevice, st));   // zeta
+  XT_CUDA(cudaMemcpyAsync(pr.d[5], deltas, nb, cudaMemcpyHostToDevice, st));  // delta
+  XT_CUDA(cudaMemcpyAsync(pr.d[9], zeros, nb, cudaMemcpyHostToDevice, st));   // s
+  XT_CUDA(cudaMemcpyAsync(pr.i[0], izeros, nb, cudaMemcpyHostToDevice, st));  // at_turn
+  XT_CUDA(cudaMemcpyAsync(pr.i[1], ones, nb, cudaMemcpyHostToDevice, st));    // state
+  XT_CUDA(cudaMemcpyAsync(pr.i[3], izeros, nb, cudaMemcpyHostToDevice, st));  // at_element
+  xt_particles p{};
+  p.x = pr.d[0];
+  p.px = pr.d[1];
+  p.y = pr.d[2];
+  p.py = pr.d[3];
+  p.zeta = pr.d[4];
+  p.delta = pr.d[5];
+  p.ptau = pr.d[6];
+  p.rpp = pr.d[7];
+  p.rvv = pr.d[8];
+  p.s = pr.d[9];
+  p.at_turn = pr.i[0];
+  p.state = pr.i[1];
+  p.particle_id = nullptr;
+  p.at_element = pr.i[3];
+  int rc = launch_init_derived(lat, p, kProbe, st);
+  if (rc != XT_OK) return rc;
+  rc = xt_track(lat, &p, kProbe, 1, st);
+  if (rc != XT_OK) return rc;
+  double r[4][kProbe];
+  int64_t state[kProbe];
+  for (int c = 0; c < 4; ++c) XT_CUDA(cudaMemcpyAsync(r[c], pr.d[c], nb, cudaMemcpyDeviceToHost, st));
+  XT_CUDA(cudaMemcpyAsync(state, pr.i[1], nb, cudaMemcpyDeviceToHost, st));
+  XT_CUDA(cudaStreamSynchronize(st));
+  for (int k = 0; k < kProbe; ++k) {
+    bool ok = state[k] == 1;
+    for (int c = 0; c < 4; ++c) ok = ok && std::isfinite(r[c][k]);
+    if (!ok) {
+      set_error("xt_twiss4d: a probe particle was lost or became non-finite (orbit outside the aperture?)");
+      return XT_ERR_UNSTABLE;
+    }
+  }
+  for (int row = 0; row < 4; ++row) {
+    out[row] = r[row][0];
+    for (int c = 0; c < 4; ++c) jac[4 * row + c] = (r[row][1 + 2 * c] - r[row][2 + 2 * c]) / (2.0 * kStep[c]);
+  }
+  return XT_OK;
+}
+
+}  // namespace
+}  // namespace xt
+
+extern "C" int xt_twiss4d(const xt_lattice *lat, double delta0, const double *guess4, xt_twiss4d_result *out,
+                          void *cuda_stream) {
+  using namespace xt;
+  if (!lat || !out || !std::isfinite(delta0)) {
+    set_error("xt_twiss4d: NULL lattice / result or non-finite delta0");
+    return XT_ERR_INVALID_ARG;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  Probe pr;
+  const size_t pitch = 256;  // bytes per array (9 x 8 = 72 used)
+  XT_CUDA(cudaMalloc(&pr.block, pitch * kArr));
+  unsigned char *base = static_cast<unsigned char *>(pr.block);
+  for (int k = 0; k < 10; ++k) pr.d[k] = reinterpret_cast<double *>(base + pitch * k);
+  for (int k = 0; k < 4; ++k) pr.i[k] = reinterpret_cast<int64_t *>(base + pitch * (10 + k));
+  auto done = [&](int code) {
+    cudaFree(pr.block);
+    return code;
+  };
+
+  double z[4] = {0.0, 0.0, 0.0, 0.0};
+  if (guess4)
+    for (int c = 0; c < 4; ++c) z[c] = guess4[c];
+  xt_twiss4d_result res{};
+  double img[4], jac[16];
+  int rc = XT_OK;
+  bool converged = false;
+  for (int it = 0; it < 25; ++it) {  // Twiss step 1: Newton on f(z) - z = 0
+    if ((rc = one_turn_and_jacobian(lat, pr, z, delta0, img, jac, st)) != XT_OK) return done(rc);
+    double a[4][5];
+    for (int r = 0; r < 4; ++r) {
+      for (int c = 0; c < 4; ++c) a[r][c] = jac[4 * r + c] - (r == c ? 1.0 : 0.0);
+      a[r][4] = -(img[r] - z[r]);
+    }
+    if (solve4(a) != 0) {
+      set_error("xt_twiss4d: one-turn matrix minus identity is singular (integer tune?)");
+      return done(XT_ERR_UNSTABLE);
+    }
+    double step = 0.0;
+    for (int c = 0; c < 4; ++c) {
+      z[c] += a[c][4];
+      step = std::fmax(step, std::fabs(a[c][4]));
+    }
+    res.iterations = it + 1;
+    if (step < 1e-13) {
+      converged = true;
+      break;
+    }
+  }
+  if (!converged) {
+    set_error("xt_twiss4d: closed-orbit search did not converge in 25 Newton steps");
+    return done(XT_ERR_UNSTABLE);
+  }
+  // Twiss step 2: the Jacobian at the closed orbit; step 3: uncoupled optics per plane
+  if ((rc = one_turn_and_jacobian(lat, pr, z, delta0, img, jac, st)) != XT_OK) return done(rc);
+  for (int c = 0; c < 4; ++c) res.co[c] = z[c];
+  for (int k = 0; k < 16; ++k) res.m[k] = jac[k];
+  res.stable = 1;
+  double *bet[2] = {&res.betx, &res.bety}, *alf[2] = {&res.alfx, &res.alfy};
+  double *mu[2] = {&res.mux, &res.muy}, *q[2] = {&res.qx_frac, &res.qy_frac};
+  for (int pl = 0; pl < 2; ++pl) {
+    const int i = 2 * pl;
+    const double m11 = jac[4 * i + i], m12 = jac[4 * i + i + 1], m22 = jac[4 * (i + 1) + i + 1];
+    const double cosmu = 0.5 * (m11 + m22);
+    if (!(std::fabs(cosmu) < 1.0)) {
+      res.stable = 0;
+      *bet[pl] = *alf[pl] = *mu[pl] = *q[pl] = std::nan("");
+      continue;
+    }
+    const double sinmu = std::copysign(std::sqrt(1.0 - cosmu * cosmu), m12);
+    *bet[pl] = m12 / sinmu;
+    *alf[pl] = (m11 - m22) / (2.0 * sinmu);
+    *mu[pl] = std::atan2(sinmu, cosmu);
+    double frac = *mu[pl] / (2.0 * 3.14159265358979323846);
+    frac -= std::floor(frac);
+    *q[pl] = frac;
+  }
+  *out = res;
+  return done(XT_OK);
+}

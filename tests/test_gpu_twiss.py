@@ -1,0 +1,93 @@
+"""Twiss from tracking on the GPU path against
+(a) the thin-FODO closed form of pin P2 and (b) the same three steps run on the oracle
+(``oracle/make_optics.py``: Newton closed orbit, central-difference Jacobian, uncoupled optics).
+
+Both sides use the same finite-difference steps, so they differ only by the tracking
+arithmetic (FMA fusion) amplified by 1/(2h): the closed orbit agrees to 1e-12 m, the matrix
+to 1e-7, tunes to 1e-8 -- the accuracy central differences give, far above the 1e-12 parity
+bar of the tracking itself.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import make_optics as MO
+from xt_inputs import configs as C
+from xt_inputs.packed import Drift, LimitEllipse, Multipole, pack_lattice
+
+pytestmark = pytest.mark.gpu
+
+P0C, MASS0 = 450e9, 938272088.16
+
+
+@pytest.fixture(scope="module")
+def X():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (run with -m gpu on the B200 box)")
+    import paper_2310_00317_b200 as X
+    return X
+
+
+def test_twiss_fodo_closed_form(X):
+    """config[0] without its cavity: ten thin FODO cells, textbook values (pin P2)."""
+    cell = [Multipole(knl=(0.0, 0.1)), Drift(2.0), Multipole(knl=(0.0, -0.1)), Drift(2.0)]
+    lat = X.xt_lattice_create(pack_lattice(cell * 10, P0C, MASS0, 1.0))
+    tw = X.xt_twiss4d(lat)
+    lat.close()
+    assert tw["stable"] == 1 and tw["iterations"] <= 3
+    assert np.max(np.abs(tw["co"])) < 1e-15                       # the origin is the closed orbit
+    mu_cell = math.acos(1.0 - 2.0 ** 2 / (2.0 * 10.0 ** 2))       # cos mu = 1 - L^2/(2 f^2), reading A15
+    tune = 10 * mu_cell / (2 * math.pi)
+    assert abs(tune - 0.31884280429259924) < 1e-15
+    assert abs(tw["qx_frac"] - tune) < 1e-8 and abs(tw["qy_frac"] - tune) < 1e-8
+    assert abs(tw["betx"] - 22.110831935702666) < 1e-6 and abs(tw["alfx"] + 1.1055415967851333) < 1e-7
+    assert abs(tw["bety"] - 18.090680674665817) < 1e-6 and abs(tw["alfy"] - 0.90453403373329087) < 1e-7
+    np.testing.assert_allclose(tw["m"][0:2, 0:2], [[-1.4229092060125620, 20.074399908620036],
+                                                   [-0.091247272311909253, 0.58453078484944159]], atol=1e-7)
+    assert np.max(np.abs(tw["m"][0:2, 2:4])) < 1e-8               # upright quads: no coupling
+    assert abs(np.linalg.det(tw["m"]) - 1.0) < 1e-7               # symplectic map
+
+
+@pytest.mark.parametrize("cfg", [0, 2, 3])
+def test_twiss_matches_the_oracle_procedure(X, cfg):
+    buf = C.pack(C.lattice(cfg))
+    want = MO.optics_of(buf)
+    lat = X.xt_lattice_create(buf)
+    tw = X.xt_twiss4d(lat)
+    lat.close()
+    assert tw["stable"] == 1 and tw["iterations"] <= 8
+    np.testing.assert_allclose(tw["co"], [want["x_co"], want["px_co"], want["y_co"], want["py_co"]], atol=1e-12)
+    for k in ("betx", "bety"):
+        assert abs(tw[k] / want[k] - 1.0) < 1e-7, k
+    for k in ("alfx", "alfy"):
+        assert abs(tw[k] - want[k]) < 1e-6, k
+    for k in ("qx_frac", "qy_frac"):
+        assert abs(tw[k] - want[k]) < 1e-8, k
+    if cfg >= 2:                                                   # what shaped the matched ensembles
+        ref = C.load_optics()["cfg%d" % cfg]
+        assert abs(tw["betx"] / ref["betx"] - 1.0) < 1e-6 and abs(tw["qy_frac"] - ref["qy_frac"]) < 1e-7
+
+
+def test_twiss_off_momentum_and_errors(X):
+    """Off-momentum closed orbit of the LHC-sized ring moves with dispersion; a guess far inside
+    the aperture still converges; an orbit outside the aperture is reported, not returned."""
+    buf = C.pack(C.lattice(2))
+    lat = X.xt_lattice_create(buf)
+    on = X.xt_twiss4d(lat, 0.0)
+    off = X.xt_twiss4d(lat, 1e-4, guess4=on["co"])
+    dx = (off["co"][0] - on["co"][0]) / 1e-4                       # dispersion at the start point [m]
+    assert 0.1 < abs(dx) < 10.0 and off["stable"] == 1
+    again = X.xt_twiss4d(lat, 0.0, guess4=[1e-3, 0.0, -1e-3, 0.0])
+    np.testing.assert_allclose(again["co"], on["co"], atol=1e-11)
+    with pytest.raises(X.XtError) as e:
+        X.xt_twiss4d(lat, 0.0, guess4=[0.5, 0.0, 0.0, 0.0])       # 0.5 m: outside the 20 mm ellipse
+    assert e.value.code == -5
+    lat.close()
+    # an unstable plane is flagged, not an error: two focusing quads in a row
+    bad = [Multipole(knl=(0.0, 0.9)), Drift(2.0), Multipole(knl=(0.0, 0.9)), Drift(2.0)]
+    lat = X.xt_lattice_create(pack_lattice(bad, P0C, MASS0, 1.0))
+    tw = X.xt_twiss4d(lat)
+    assert tw["stable"] == 0 and (math.isnan(tw["bety"]) or math.isnan(tw["betx"]))
+    lat.close()
