@@ -33,6 +33,12 @@ int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p
     set_error(std::string(fn) + ": a required particle array is NULL (only particle_id, at_element may be)");
     return XT_ERR_INVALID_ARG;
   }
+  int dev = -1;
+  XT_CUDA(cudaGetDevice(&dev));
+  if (dev != lat->device) {  // the lattice image lives on the device it was created on
+    set_error(std::string(fn) + ": the current CUDA device is not the one the lattice was created on");
+    return XT_ERR_INVALID_ARG;
+  }
   return XT_OK;
 }
 

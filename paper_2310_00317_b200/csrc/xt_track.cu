@@ -683,14 +683,11 @@ template <int P>
 int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
   const size_t cold_bytes = (static_cast<size_t>(8 * Cold<P>::kPitch) * block + 127) & ~static_cast<size_t>(127);
   const size_t smem = 128 + 64 + cold_bytes + (lat->info.n_chunks == 1 ? 1 : 2) * static_cast<size_t>(lat->info.chunk_bytes);
-  static bool attr_set = false;
-  if (!attr_set) {
-    XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    // the kernel has no use for L1 (every hot read is a shared-memory broadcast)
-    XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                 cudaSharedmemCarveoutMaxShared));
-    attr_set = true;
-  }
+  // per device, so set on every launch (a few microseconds against launches of milliseconds to seconds)
+  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+  // the kernel has no use for L1 (every hot read is a shared-memory broadcast)
+  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                               cudaSharedmemCarveoutMaxShared));
   const int64_t cap = static_cast<int64_t>(block) * P;
   const int64_t need = (a.n_part + cap - 1) / cap;
   const int64_t grid = ((need + a.grid_quantum - 1) / a.grid_quantum) * a.grid_quantum;
