@@ -254,6 +254,14 @@ def main():
             ev1.record(stream)
 
     peak_flops, peak_ms = X.xt_fp64_fma_peak()
+    props = torch.cuda.get_device_properties(local)
+    n_sm = props.multi_processor_count
+    sm_max_hz = 1.965e9                                   # B200 max SM clock (MEASURED_PEAKS.json sm_max_mhz)
+    try:
+        mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        sm_max_hz = float(mp.get("sm_max_mhz", 1965.0)) * 1e6
+    except (OSError, ValueError):
+        pass
     probe = {"dfma_three_distinct_registers": X.xt_fp64_fma_probe(1)[0] / 1e12,
              "horner_4_particles_per_thread_no_lattice": X.xt_fp64_fma_probe(2)[0] / 1e12}
     for _ in range(args.warmup):
@@ -305,6 +313,9 @@ def main():
                 "bound": "alu", "unit": "TFLOP/s",
                 "achieved": f_min * pt_per_s / 1e12, "peak": peak_flops / 1e12,
                 "frac": f_min * pt_per_s / peak_flops,
+                # against the nominal figure from unit counts and clocks: SMs x 64 FP64 lanes x 2 x max SM clock
+                "peak_nominal": n_sm * 64 * 2 * sm_max_hz / 1e12,
+                "frac_nominal": f_min * pt_per_s / (n_sm * 64 * 2 * sm_max_hz),
                 "achieved_executed": f_exec * pt_per_s / 1e12, "frac_executed": f_exec * pt_per_s / peak_flops,
                 "peak_source": "xt_fp64_fma_peak: DFMA microbenchmark in this run (%.2f ms), burst; "
                                "nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2 TFLOP/s" % peak_ms,
