@@ -40,6 +40,7 @@ struct TrackArgs {
   int64_t n_turns;
   int32_t n_chunks;
   uint32_t chunk_bytes;
+  int32_t stage_chunks;  // consecutive chunks staged by one bulk copy (they are contiguous in the image)
   int32_t grid_quantum;  // CTAs are handed out in multiples of this (the SM count)
   double beta0, tib, igam2;
 };
@@ -422,9 +423,11 @@ __device__ __forceinline__ void limit_ellipse(Parts<P> &q, const Cold<P> &cold, 
 }
 
 // Push the P particles of this thread through every record of one staged chunk.
+// Returns the position just behind the chunk (where the next chunk of the image starts).
 template <int P>
-__device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp, const Cold<P> &cold,
-                                            int64_t turns_done, const TrackArgs &a) {
+__device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const unsigned char *rp,
+                                                            const Cold<P> &cold, int64_t turns_done,
+                                                            const TrackArgs &a) {
   uint32_t tag = reinterpret_cast<const RecHdr *>(rp)->next;  // chunk preamble
   rp += sizeof(RecHdr);
   while ((tag & TAG_TYPE_MASK) != TAG_END) {
@@ -521,6 +524,7 @@ __device__ __forceinline__ void track_chunk(Parts<P> &q, const unsigned char *rp
     }
     tag = h.next;
   }
+  return rp;
 }
 
 // Register budget per thread (CTAs of 128 threads: 65536 / (128 * CTAs per SM)).
@@ -602,39 +606,50 @@ __global__ void __maxnreg__(RegBudget<P>::value) xt_track_kernel(const TrackArgs
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  if (threadIdx.x == 0) {
-    const ChunkDesc d = a.chunks[0];
-    tma_load_chunk(bar0, smem_addr(buf0), a.image + d.offset, d.nbytes);
-  }
-
   int64_t turns_done = 0;
   if (single) {
     // Whole lattice resident in buffer 0: warps run free, no CTA-level synchronisation.
+    if (threadIdx.x == 0) {
+      const ChunkDesc d = a.chunks[0];
+      tma_load_chunk(bar0, smem_addr(buf0), a.image + d.offset, d.nbytes);
+    }
     mbar_wait(bar0, 0);
     for (; turns_done < a.n_turns; ++turns_done) {
       if (!__any_sync(0xffffffffu, q.alive != 0)) break;
       track_chunk<P>(q, buf0, cold, turns_done, a);
     }
   } else {
-    const int64_t total = a.n_turns * a.n_chunks;
-    int64_t gidx = 0;  // global chunk counter: buffer = gidx & 1, phase parity = (gidx >> 1) & 1
+    // A stage = stage_chunks consecutive chunks = one bulk copy into one buffer.
+    const int32_t m = a.stage_chunks;
+    const int32_t n_stages = (a.n_chunks + m - 1) / m;
+    const uint32_t stage_bytes = static_cast<uint32_t>(m) * a.chunk_bytes;
+    auto load_stage = [&](int32_t sidx, uint32_t nb) {  // thread 0 only
+      const int32_t first = sidx * m;
+      const int32_t last = (first + m < a.n_chunks ? first + m : a.n_chunks) - 1;
+      const ChunkDesc d0 = a.chunks[first], d1 = a.chunks[last];
+      const uint32_t bytes = static_cast<uint32_t>(d1.offset + d1.nbytes - d0.offset);
+      tma_load_chunk(bar0 + 8 * nb, smem_addr(buf0 + static_cast<size_t>(nb) * stage_bytes), a.image + d0.offset,
+                     bytes);
+    };
+    if (threadIdx.x == 0) load_stage(0, 0);
+    const int64_t total = a.n_turns * n_stages;
+    int64_t gidx = 0;  // global stage counter: buffer = gidx & 1, phase parity = (gidx >> 1) & 1
     int32_t c = 0;
     bool any = true;
     while (gidx < total) {
       if (threadIdx.x == 0 && gidx + 1 < total) {
         // buffer (gidx+1)&1 was released by the __syncthreads_or that ended iteration gidx-1
-        const int32_t cn = (c + 1 == a.n_chunks) ? 0 : c + 1;
-        const ChunkDesc d = a.chunks[cn];
-        const uint32_t nb = static_cast<uint32_t>((gidx + 1) & 1);
-        tma_load_chunk(bar0 + 8 * nb, smem_addr(buf0 + static_cast<size_t>(nb) * a.chunk_bytes),
-                       a.image + d.offset, d.nbytes);
+        load_stage((c + 1 == n_stages) ? 0 : c + 1, static_cast<uint32_t>((gidx + 1) & 1));
       }
       const uint32_t cb = static_cast<uint32_t>(gidx & 1);
       mbar_wait(bar0 + 8 * cb, static_cast<uint32_t>((gidx >> 1) & 1));
-      if (__any_sync(0xffffffffu, q.alive != 0))
-        track_chunk<P>(q, buf0 + static_cast<size_t>(cb) * a.chunk_bytes, cold, turns_done, a);
+      if (__any_sync(0xffffffffu, q.alive != 0)) {
+        const int32_t n_sub = (c * m + m < a.n_chunks ? m : a.n_chunks - c * m);
+        const unsigned char *rp = buf0 + static_cast<size_t>(cb) * stage_bytes;
+        for (int32_t k = 0; k < n_sub; ++k) rp = track_chunk<P>(q, rp, cold, turns_done, a);
+      }
       ++gidx;
-      if (++c == a.n_chunks) {
+      if (++c == n_stages) {
         c = 0;
         ++turns_done;  // T: turn completed
       }
@@ -682,7 +697,6 @@ __global__ void xt_init_derived_kernel(xt_particles p, int64_t n, double beta0, 
 template <int P>
 int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
   const size_t cold_bytes = (static_cast<size_t>(8 * Cold<P>::kPitch) * block + 127) & ~static_cast<size_t>(127);
-  const size_t smem = 128 + 64 + cold_bytes + (lat->info.n_chunks == 1 ? 1 : 2) * static_cast<size_t>(lat->info.chunk_bytes);
   // per device, so set on every launch (a few microseconds against launches of milliseconds to seconds)
   XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   // the kernel has no use for L1 (every hot read is a shared-memory broadcast)
@@ -695,7 +709,26 @@ int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStr
     set_error("xt_track: too many particles for one launch");
     return XT_ERR_INVALID_ARG;
   }
-  xt_track_kernel<P><<<static_cast<unsigned>(grid), block, smem, st>>>(a);
+  // Staging depth: as many chunks per bulk copy (fewer CTA-wide barriers per turn) as shared memory
+  // allows without taking a resident CTA away.
+  cudaFuncAttributes fa;
+  XT_CUDA(cudaFuncGetAttributes(&fa, xt_track_kernel<P>));
+  int64_t resident = 65536 / (static_cast<int64_t>(fa.numRegs > 0 ? fa.numRegs : 128) * block);
+  if (resident > grid / a.grid_quantum) resident = grid / a.grid_quantum;
+  if (resident < 1) resident = 1;
+  TrackArgs b = a;
+  b.stage_chunks = 1;
+  const size_t chunk = static_cast<size_t>(lat->info.chunk_bytes);
+  auto smem_for = [&](int m) { return 128 + 64 + cold_bytes + (lat->info.n_chunks == 1 ? 1 : 2) * m * chunk; };
+  for (int m = 4; m > 1; m >>= 1) {
+    if (lat->info.n_chunks >= 2 * m && smem_for(m) <= 96 * 1024 &&
+        static_cast<size_t>(resident) * (smem_for(m) + 1024) <= 227 * 1024) {
+      b.stage_chunks = m;
+      break;
+    }
+  }
+  const size_t smem = smem_for(b.stage_chunks);
+  xt_track_kernel<P><<<static_cast<unsigned>(grid), block, smem, st>>>(b);
   count_launch();
   XT_CUDA(cudaGetLastError());
   return XT_OK;

@@ -486,3 +486,21 @@ def test_fp64_probes_are_ordered(X):
     assert 0.5 * peak < distinct < horner < peak
     with pytest.raises(X.XtError):
         X.xt_fp64_fma_probe(3)
+
+
+def test_staging_depth_does_not_change_results(X):
+    """A launch with several CTAs per SM stages one lattice chunk per bulk copy, a small ensemble
+    several chunks at once: a particle must come out bit-identical whichever company it is tracked in."""
+    import torch
+    coords = C.particles(3, n=400_000)                         # ~2700 particles per SM: one chunk per stage
+    buf = packed(3)
+    lat = X.xt_lattice_create(buf)
+    p = X.new_particles(lat, coords)
+    X.xt_track(lat, p, 2)
+    idx = np.arange(5, 400_000, 997)
+    big = {k: v[torch.from_numpy(idx).cuda()].cpu().numpy() for k, v in p.items()}
+    del p
+    q = X.new_particles(lat, C.subsample(coords, idx))         # 402 particles: four chunks per stage
+    X.xt_track(lat, q, 2)
+    assert_bit_identical(X.particles_to_host(q), big)
+    lat.close()
