@@ -116,9 +116,12 @@ constexpr int kPrefetch = 4;  // 16-byte slots of a record loaded ahead of its d
 #ifndef XT_PF4
 #define XT_PF4 2
 #endif
+#ifndef XT_PF3
+#define XT_PF3 2
+#endif
 template <int P>
 struct Prefetched {  // ... of which this many really are (the rest is read where it is used)
-  static constexpr int value = P >= 4 ? XT_PF4 : kPrefetch;
+  static constexpr int value = P >= 4 ? XT_PF4 : (P == 3 ? XT_PF3 : kPrefetch);
 };
 
 // Hot per-thread state of P particles: what drifts and kicks touch at every element.
