@@ -504,3 +504,34 @@ def test_staging_depth_does_not_change_results(X):
     X.xt_track(lat, q, 2)
     assert_bit_identical(X.particles_to_host(q), big)
     lat.close()
+
+
+def test_particles_dead_on_entry_are_left_alone(X):
+    """state == 0 on entry (lost in an earlier call, or never alive): every array of such a particle
+    comes back bit for bit, whatever shares its thread or warp; the others track as if alone."""
+    coords = C.subsample(C.particles(4), np.linspace(0, 2_000_399, 700).astype(np.int64))
+    buf = packed(4)
+    lat = X.xt_lattice_create(buf)
+    ref = X.new_particles(lat, coords)
+    X.xt_track(lat, ref, 3)
+    ref = X.particles_to_host(ref)
+    p = X.new_particles(lat, coords)
+    dead = np.zeros(700, dtype=bool)
+    dead[::3] = True
+    dead[100:160] = True                                           # whole warps' worth in a row
+    import torch
+    mask = torch.from_numpy(dead).cuda()
+    p["state"][mask] = 0
+    p["at_turn"][mask] = 17
+    p["x"][mask] = float("nan")                                    # must never be read into a live lane's result
+    before = X.particles_to_host(p)
+    for ppt in (1, 3, 4):
+        q = {k: v.clone() for k, v in p.items()}
+        X.xt_track_ex(lat, q, 3, particles_per_thread=ppt, block_size=64)
+        got = X.particles_to_host(q)
+        for k in got:
+            a, b = got[k][dead], before[k][dead]
+            same = (a == b) | (np.isnan(a.astype(np.float64)) & np.isnan(b.astype(np.float64)))
+            assert same.all(), k
+        assert_bit_identical({k: v[~dead] for k, v in got.items()}, {k: v[~dead] for k, v in ref.items()})
+    lat.close()
