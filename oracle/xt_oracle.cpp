@@ -31,7 +31,8 @@
 // of the one-turn Jacobian; P4 reversibility; P5 worked examples W1/W2 (60-digit textbook
 // evaluation, tests/golden/); P6 Horner vs direct complex power sum; P7 Courant-Snyder
 // invariant; P8 aperture edges; P9 structural invariants; P10 energy identities;
-// small-amplitude synchrotron tune for the cavity.
+// small-amplitude synchrotron tune for the cavity; P13 thick quadrupole: second-order limit of
+// thin slices (+ cubic paraxial residual), closed-form matrix, symplecticity, reversibility.
 // =====================================================================================
 #include <cmath>
 #include <cstdint>
@@ -47,7 +48,7 @@ constexpr int MAX_ORDER = 20;
 
 enum ElemType : uint32_t {
   MARKER = 0, DRIFT = 1, MULTIPOLE = 2, CAVITY = 3,
-  SROTATION = 4, XYSHIFT = 5, LIMITRECT = 6, LIMITELLIPSE = 7
+  SROTATION = 4, XYSHIFT = 5, LIMITRECT = 6, LIMITELLIPSE = 7, QUADRUPOLE = 8
 };
 
 struct Element {
@@ -69,6 +70,8 @@ struct Element {
   double min_x = 0.0, max_x = 0.0, min_y = 0.0, max_y = 0.0;
   // LIMITELLIPSE
   double a = 0.0, b = 0.0, a2 = 0.0, b2 = 0.0, a2b2 = 0.0;
+  // QUADRUPOLE (thick): k1, length
+  double k1 = 0.0;
 };
 
 struct Lattice {
@@ -179,6 +182,11 @@ int parse(const void* packed, size_t nbytes, Lattice& L) {
         e.a2 = e.a * e.a;
         e.b2 = e.b * e.b;
         e.a2b2 = e.a2 * e.b2;
+        break;
+      case QUADRUPOLE:
+        if (!rd(e.k1) || !rd(e.length)) return -2;
+        if (e.k1 == 0.0 || !(e.length > 0.0)) return -2;   // a zero-strength thick quadrupole is a Drift
+        s = s + e.length;
         break;
       default: return -2;
     }
@@ -326,6 +334,42 @@ int xo_track(const void* packed, size_t nbytes, const xo_particles* P, int64_t n
               px = px - e.wf * x;
               zeta = zeta - (e.hxl * x) * k.rv0v;
             }
+            break;
+          }
+
+          case QUADRUPOLE: {
+            // Thick quadrupole ("'Thick' maps for ... quadrupole magnets"; reading A18):
+            // exact flow of H = (px^2 + py^2)/(2(1+delta)) + (k1/2)(x^2 - y^2) over the length L.
+            // With w = sqrt(|k1|/(1+delta)) the focusing plane (u, pu) turns by the angle w L,
+            //   u' = u cos + pu sin/((1+delta) w),   pu' = pu cos - (1+delta) w u sin,
+            // the other one (v, pv) follows cosh / sinh, and the path length is
+            //   zeta' = zeta + L (1 - beta0/beta) - (beta0/beta)/(2 (1+delta)^2) int_0^L (px^2 + py^2) ds,
+            // the first term written cancellation-free as L g/((1+delta)((1+delta) + b)).
+            const double opd = 1.0 + delta;
+            const double rk = e.k1 / opd;
+            const double w = std::sqrt(std::fabs(rk));
+            const double wl = w * e.length;
+            const double cs = std::cos(wl), sn = std::sin(wl);
+            const double ch = std::cosh(wl), sh = std::sinh(wl);
+            const double ow = opd * w;
+            const double iw = 1.0 / ow;
+            const bool focus_x = rk > 0.0;
+            const double u = focus_x ? x : y, pu = focus_x ? px : py;
+            const double v = focus_x ? y : x, pv = focus_x ? py : px;
+            const double au = ow * u;
+            const double av = ow * v;
+            const double u1 = u * cs + (pu * iw) * sn;
+            const double pu1 = pu * cs - au * sn;
+            const double v1 = v * ch + (pv * iw) * sh;
+            const double pv1 = pv * ch + av * sh;
+            const double hl = 0.5 * e.length;
+            const double h2w = 0.5 / w;
+            const double pu2 = pu * pu, au2 = au * au, pv2 = pv * pv, av2 = av * av;
+            const double i_f = ((pu2 + au2) * hl + ((pu2 - au2) * (sn * cs)) * h2w) - ((au * pu) * (sn * sn)) / w;
+            const double i_d = ((pv2 - av2) * hl + ((pv2 + av2) * (sh * ch)) * h2w) + ((av * pv) * (sh * sh)) / w;
+            zeta = (zeta + e.length * (k.g / (opd * (opd + k.b)))) - (k.rv0v / (2.0 * k.opd2)) * (i_f + i_d);
+            if (focus_x) { x = u1; px = pu1; y = v1; py = pv1; }
+            else         { y = u1; py = pu1; x = v1; px = pv1; }
             break;
           }
 

@@ -439,3 +439,91 @@ def test_P12_weak_focusing_ring_dispersion_and_path_length():
         b0_over_b = (1 + mp.mpf(beta0) * pt) / (1 + d)
         dz = N * (mp.mpf(L) * (1 - b0_over_b) - d * mp.mpf(length) * b0_over_b)
         assert abs(mp.mpf(float(p["zeta"][0])) - dz) <= 1e-13 * max(abs(dz), mp.mpf(1e-9))
+
+
+# ----------------------------- P13 thick quadrupole (reading A18)
+from xt_inputs.packed import Quadrupole  # noqa: E402
+
+
+def _thin_sliced(k1, length, n):
+    """n symmetric drift-kick-drift slices built from the maps pinned above (P1, P2, P6)."""
+    h, kl = length / (2 * n), k1 * length / n
+    return [Drift(h), Multipole(knl=(0.0, kl)), Drift(h)] * n
+
+
+@pytest.mark.parametrize("k1", [0.35, -0.2])
+def test_P13_thick_quadrupole_is_the_limit_of_thin_slices(k1):
+    """The thick map is an exact flow; n symmetric thin slices converge to it as 1/n^2.  Pins x, px, y,
+    py and the path length zeta, the delta dependence and both signs of k1.  The slices use the exact
+    drift, the thick map the paraxial kinetic term (px^2 + py^2)/(2(1+delta)) (reading A18): what is left
+    after Richardson extrapolation is that difference, relative p^2/2, and must scale as amplitude^3."""
+    length = 3.1
+    base = np.array([[1e-3, 2e-4, -5e-4, 1e-4, 0.01, 3e-4], [-2e-3, -1e-4, 1e-3, 3e-4, -0.02, -8e-4],
+                     [5e-4, 0.0, 0.0, -2e-4, 0.0, 0.0]])
+
+    def run(els, start):
+        buf = pack(els)
+        p = O.new_particles(buf, start)
+        O.track(buf, p, 1)
+        return np.stack([p[k] for k in ("x", "px", "y", "py", "zeta")], axis=1)
+
+    residual = {}
+    for amp in (1.0, 0.1):
+        rows = base.copy()
+        rows[:, :4] *= amp
+        start = H.coords_from_rows(rows.tolist())
+        thick = run([Quadrupole(k1, length)], start)
+        s1, s2 = run(_thin_sliced(k1, length, 512), start), run(_thin_sliced(k1, length, 1024), start)
+        residual[amp] = ((4.0 * s2 - s1) / 3.0 - thick)[:, :4]
+        if amp == 0.1:                                          # paraxial difference below the slicing error
+            e1, e2 = np.abs(s1 - thick)[:, :4], np.abs(s2 - thick)[:, :4]
+            big = e1 > 50.0 * np.abs(residual[amp])             # slicing error well above the paraxial residual
+            assert big.sum() >= 6
+            assert np.all((e1[big] / e2[big] > 3.7) & (e1[big] / e2[big] < 4.4))      # second order in 1/n
+            scale = amp * np.array([1e-3, 1e-4, 1e-3, 1e-4])
+            assert np.max(np.abs(residual[amp]) / scale) < 2e-7   # p^2/2 with the momenta reached inside (<= 3e-4)
+            slip = thick[:, 4] - rows[:, 4]
+            slip_thin = ((4.0 * s2 - s1) / 3.0)[:, 4] - rows[:, 4]
+            assert np.all(np.abs(slip) > 1e-11)                                       # the path length moved
+            assert np.max(np.abs(slip_thin - slip) / np.abs(slip)) < 1e-6
+            assert np.all(np.abs(thick[:, 0] - rows[:, 0]) > 1e-6)                    # the element did something
+    ratio = residual[1.0] / residual[0.1]
+    strong = np.abs(residual[1.0]) > 1e-12
+    assert strong.sum() >= 6 and np.all(np.abs(ratio[strong] / 1e3 - 1.0) < 0.05)     # cubic in the amplitude
+
+
+def test_P13_thick_quadrupole_matrix_symplectic_reversible():
+    k1, length = 0.35, 3.1
+    buf = pack([Quadrupole(k1, length)])
+    J = H.jacobian6(O.track, buf, np.zeros(6))
+    w = math.sqrt(k1)
+    phi = w * length
+    np.testing.assert_allclose(J[0:2, 0:2], [[math.cos(phi), math.sin(phi) / w],
+                                             [-w * math.sin(phi), math.cos(phi)]], atol=1e-8)
+    np.testing.assert_allclose(J[2:4, 2:4], [[math.cosh(phi), math.sinh(phi) / w],
+                                             [w * math.sinh(phi), math.cosh(phi)]], atol=1e-8)
+    line = [Drift(0.7), Quadrupole(k1, length), Drift(0.4), Quadrupole(-0.5 * k1, 1.3), Cavity(1e6, 200e6, 180.0),
+            Drift(0.2)]
+    for z0 in (np.zeros(6), np.array([1e-3, 2e-4, -5e-4, 1e-4, 0.01, 3e-4])):
+        _check_symplectic(pack(line), z0)
+    rng = np.random.default_rng(8)
+    n = 32
+    co = dict(x=rng.normal(0, 1e-3, n), px=rng.normal(0, 1e-4, n), y=rng.normal(0, 1e-3, n),
+              py=rng.normal(0, 1e-4, n), zeta=rng.normal(0, 0.02, n), delta=rng.normal(0, 3e-4, n))
+    fwd, bwd = pack(line), pack(H.reversed_lattice(line))
+    p = O.new_particles(fwd, co)
+    p0 = O.copy_particles(p)
+    O.track(fwd, p, 2)
+    H.flip_R(p)
+    O.track(bwd, p, 2)
+    H.flip_R(p)
+    for k, scale in (("x", 1e-3), ("px", 1e-4), ("y", 1e-3), ("py", 1e-4), ("zeta", 0.02), ("delta", 3e-4)):
+        # cosh / sinh amplify rounding by e^(w L) ~ 6 per pass in the defocusing plane: 1e-11, not the 1e-13 of P4
+        assert np.max(np.abs(p[k] - p0[k])) < 1e-11 * scale, k
+
+
+def test_P13_thick_quadrupole_rejects_degenerate_parameters():
+    for bad in (Quadrupole(0.0, 1.0), Quadrupole(0.1, 0.0), Quadrupole(0.1, -1.0), Quadrupole(math.nan, 1.0)):
+        with pytest.raises(ValueError):
+            O.reference(pack([bad]))
+    assert abs(O.s_table(pack([Quadrupole(0.1, 2.5), Drift(1.0), Marker()]))[2] - 3.5) < 1e-15

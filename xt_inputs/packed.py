@@ -17,6 +17,7 @@ accelerator element".  Here that sequence is flattened into one little-endian,
     type 5 XYSHIFT       aux=0  dx, dy
     type 6 LIMITRECT     aux=0  min_x, max_x, min_y, max_y
     type 7 LIMITELLIPSE  aux=0  a, b
+    type 8 QUADRUPOLE    aux=0  k1 [1/m^2], length [m]   (thick; k1 != 0, length > 0)
 
 This module is pure serialisation (struct packing).  It performs no tracking
 arithmetic: the same bytes are handed to the oracle and to ``xt_lattice_create``;
@@ -35,7 +36,7 @@ HEADER_BYTES = 48
 
 ELEMENT_TYPE_IDS = {
     "Marker": 0, "Drift": 1, "Multipole": 2, "Cavity": 3,
-    "SRotation": 4, "XYShift": 5, "LimitRect": 6, "LimitEllipse": 7,
+    "SRotation": 4, "XYShift": 5, "LimitRect": 6, "LimitEllipse": 7, "Quadrupole": 8,
 }
 
 
@@ -99,6 +100,13 @@ class LimitEllipse:
     b: float
 
 
+@dataclass(frozen=True)
+class Quadrupole:
+    """Thick quadrupole: gradient k1 = (dBy/dx)/(P0/q0), magnetic length."""
+    k1: float
+    length: float
+
+
 def _record(el) -> bytes:
     if isinstance(el, Marker):
         return struct.pack("<II", 0, 0)
@@ -119,6 +127,8 @@ def _record(el) -> bytes:
         return struct.pack("<II4d", 6, 0, el.min_x, el.max_x, el.min_y, el.max_y)
     if isinstance(el, LimitEllipse):
         return struct.pack("<II2d", 7, 0, el.a, el.b)
+    if isinstance(el, Quadrupole):
+        return struct.pack("<II2d", 8, 0, el.k1, el.length)
     raise TypeError("unknown element %r" % (el,))
 
 
@@ -166,6 +176,9 @@ def unpack_lattice(buf: bytes):
         elif t == 7:
             a, b = struct.unpack_from("<2d", buf, off); off += 16
             out.append(LimitEllipse(a, b))
+        elif t == 8:
+            k1, length = struct.unpack_from("<2d", buf, off); off += 16
+            out.append(Quadrupole(k1, length))
         else:
             raise ValueError("unknown element type %d" % t)
     return out, p0c, mass0, q0
