@@ -51,7 +51,9 @@ enum {
   XT_SROTATION = 4,   /* cos_z, sin_z                                            (map M4)   */
   XT_XYSHIFT = 5,     /* dx, dy                                                  (map M4)   */
   XT_LIMITRECT = 6,   /* min_x, max_x, min_y, max_y (edges inclusive)            (step A)   */
-  XT_LIMITELLIPSE = 7 /* a, b (edge inclusive)                                   (step A)   */
+  XT_LIMITELLIPSE = 7,/* a, b (edge inclusive)                                   (step A)   */
+  XT_QUADRUPOLE = 8   /* k1 [1/m^2], length [m]: thick quadrupole, k1 != 0, length > 0           */
+                      /* (reading A18)             */
 };
 
 /* Packed lattice buffer (HOST memory, little-endian, 8-byte aligned records):
@@ -70,7 +72,7 @@ typedef struct xt_lattice xt_lattice; /* opaque; immutable after create; owns it
  * are loaded and stored verbatim so that n calls of k turns equal one call of n*k turns
  * bit for bit.  state: 1 alive, 0 lost on an aperture.  For a lost particle the coordinates
  * are those AT the aperture that stopped it, at_element is that element's index in the
- * packed buffer, s the sum of drift lengths before it, at_turn the number of COMPLETED
+ * packed buffer, s the sum of drift and thick-element lengths before it, at_turn the number of COMPLETED
  * turns.  For survivors s = 0 and at_turn has advanced by n_turns.
  * particle_id and at_element may be NULL.  particle_id is never written. */
 typedef struct {
@@ -102,9 +104,10 @@ typedef struct {
   int64_t n_curved;         /* multipoles with hxl != 0                                       */
   int64_t has_aperture;     /* 1 if any LimitRect / LimitEllipse                              */
   double beta0, gamma0;     /* reference particle as derived by the packer                    */
-  double circumference;     /* sum of drift lengths [m]                                       */
+  double circumference;     /* sum of drift and thick-element lengths [m]                     */
   int64_t n_drift_evals;    /* sqrt evaluations per turn after fusion (consecutive drifts     */
                             /* share one; equals the number of drifts when fuse is off)       */
+  int64_t n_thick;          /* thick elements (XT_QUADRUPOLE); not counted in n_by_type       */
 } xt_lattice_info;
 
 /* Options of xt_lattice_create_ex.  Zero-initialise for the defaults.  Neither changes any

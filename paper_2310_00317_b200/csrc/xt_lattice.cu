@@ -220,6 +220,21 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
         info.has_aperture = 1;
         break;
       }
+      case XT_QUADRUPOLE: {
+        const double k1 = r.real();
+        const double length = r.real();
+        if (!r.ok) break;
+        if (k1 == 0.0 || !(length > 0.0)) {
+          set_error("xt_lattice_create: thick quadrupole needs k1 != 0 and length > 0 (a zero-strength one is a Drift)");
+          return XT_ERR_BAD_LATTICE;
+        }
+        rec.type = TAG_QUAD;
+        rec.p0 = k1;
+        rec.slot(length, 0.0);
+        info.n_thick += 1;
+        s_pos += length;
+        break;
+      }
       default:
         set_error("xt_lattice_create: unknown element type id");
         return XT_ERR_BAD_LATTICE;

@@ -411,6 +411,58 @@ __device__ __forceinline__ void multipole_record(Parts<P> &q, const Cold<P> &col
   }
 }
 
+// Thick quadrupole (reading A18): the exact flow of
+// H = (px^2 + py^2)/(2(1+delta)) + (k1/2)(x^2 - y^2) over the length.  With w = sqrt(|k1|/(1+delta))
+// the focusing plane turns by w L (cos, sin), the other follows cosh, sinh; the path length is
+// zeta += L g/((1+delta)((1+delta)+b)) - rv0v/(2(1+delta)^2) int (px^2 + py^2) ds (closed form below).
+// The sign of k1/(1+delta) is the sign of k1 for every physical particle: a warp-uniform branch.
+// Only compiled into the THICK instantiations of the kernel: lattices without thick elements run
+// the same code as before.
+template <int P>
+__device__ __noinline__ void thick_quadrupole(Parts<P> &q, const Cold<P> &cold, const double k1, const double length) {
+#pragma unroll 1
+  for (int j = 0; j < P; ++j) {
+    const double opd = 1.0 + cold.delta(j);
+    const double rk = k1 / opd;
+    const double w = sqrt(fabs(rk));
+    const double wl = XT_MUL(w, length);
+    double sn, cs;
+    sincos(wl, &sn, &cs);
+    const double ch = cosh(wl), sh = sinh(wl);
+    const double ow = XT_MUL(opd, w);
+    const double iw = 1.0 / ow;
+    const bool focus_x = rk > 0.0;
+    const double u = focus_x ? q.x[j] : q.y[j], pu = focus_x ? q.px[j] : q.py[j];
+    const double v = focus_x ? q.y[j] : q.x[j], pv = focus_x ? q.py[j] : q.px[j];
+    const double au = XT_MUL(ow, u);
+    const double av = XT_MUL(ow, v);
+    const double u1 = XT_MADD(u, cs, XT_MUL(XT_MUL(pu, iw), sn));
+    const double pu1 = XT_NMADD(au, sn, XT_MUL(pu, cs));
+    const double v1 = XT_MADD(v, ch, XT_MUL(XT_MUL(pv, iw), sh));
+    const double pv1 = XT_MADD(pv, ch, XT_MUL(av, sh));
+    const double hl = XT_MUL(0.5, length);
+    const double h2w = 0.5 / w;
+    const double pu2 = XT_MUL(pu, pu), au2 = XT_MUL(au, au), pv2 = XT_MUL(pv, pv), av2 = XT_MUL(av, av);
+    const double i_f = XT_MADD(pu2 + au2, hl, XT_MUL(XT_MUL(pu2 - au2, XT_MUL(sn, cs)), h2w)) -
+                       XT_MUL(XT_MUL(au, pu), XT_MUL(sn, sn)) / w;
+    const double i_d = XT_MADD(pv2 - av2, hl, XT_MUL(XT_MUL(pv2 + av2, XT_MUL(sh, ch)), h2w)) +
+                       XT_MUL(XT_MUL(av, pv), XT_MUL(sh, sh)) / w;
+    const double slip = XT_MUL(length, cold.g(j) / XT_MUL(opd, opd + cold.b(j)));
+    q.zeta[j] = (q.zeta[j] + slip) - XT_MUL(cold.rv0v(j) / XT_MUL(2.0, cold.opd2(j)), i_f + i_d);
+    if (focus_x) {
+      q.x[j] = u1;
+      q.px[j] = pu1;
+      q.y[j] = v1;
+      q.py[j] = pv1;
+    } else {
+      q.y[j] = u1;
+      q.py[j] = pu1;
+      q.x[j] = v1;
+      q.px[j] = pv1;
+    }
+  }
+}
+
 // A: elliptical aperture (x^2 b^2 + y^2 a^2 <= a^2 b^2, edge inclusive, NaN lost).
 template <int P>
 __device__ __forceinline__ void limit_ellipse(Parts<P> &q, const Cold<P> &cold, const double2 ba, const double a2b2,
@@ -427,7 +479,7 @@ __device__ __forceinline__ void limit_ellipse(Parts<P> &q, const Cold<P> &cold, 
 
 // Push the P particles of this thread through every record of one staged chunk.
 // Returns the position just behind the chunk (where the next chunk of the image starts).
-template <int P>
+template <int P, bool THICK>
 __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const unsigned char *rp,
                                                             const Cold<P> &cold, int64_t turns_done,
                                                             const TrackArgs &a) {
@@ -514,6 +566,10 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
         limit_ellipse<P>(q, cold, pf[0], p0, elem, turns_done, a);  // pf[0] = (b2, a2), p0 = a2 b2
         break;
       }
+      case TAG_QUAD: {
+        if (THICK) thick_quadrupole<P>(q, cold, p0, pf[0].x);  // p0 = k1, pf[0].x = length
+        break;
+      }
       default:  // ... and every other combination (misaligned magnets, lone leading drifts) at run time
         if ((tag & TAG_TYPE_MASK) == TAG_MULT || (tag & TAG_TYPE_MASK) == TAG_CMULT)
           multipole_record<P, -1, -1>(q, cold, slots, pf, tag, p0);
@@ -546,7 +602,7 @@ struct RegBudget {
 // Shared memory: [0,16) two mbarriers; [128, 128 + 8*kPitch*blockDim) cold per-thread rows;
 // then staging buffer 0 (and buffer 1 for multi-chunk lattices), 128-byte aligned, and 64
 // spare bytes (the Horner loop prefetches one coefficient pair past the record it is in).
-template <int P>
+template <int P, bool THICK>
 __global__ void __maxnreg__(RegBudget<P>::value) xt_track_kernel(const TrackArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   const uint32_t bar0 = smem_addr(smem);
@@ -619,7 +675,7 @@ __global__ void __maxnreg__(RegBudget<P>::value) xt_track_kernel(const TrackArgs
     mbar_wait(bar0, 0);
     for (; turns_done < a.n_turns; ++turns_done) {
       if (!__any_sync(0xffffffffu, q.alive != 0)) break;
-      track_chunk<P>(q, buf0, cold, turns_done, a);
+      track_chunk<P, THICK>(q, buf0, cold, turns_done, a);
     }
   } else {
     // A stage = stage_chunks consecutive chunks = one bulk copy into one buffer.
@@ -649,7 +705,7 @@ __global__ void __maxnreg__(RegBudget<P>::value) xt_track_kernel(const TrackArgs
       if (__any_sync(0xffffffffu, q.alive != 0)) {
         const int32_t n_sub = (c * m + m < a.n_chunks ? m : a.n_chunks - c * m);
         const unsigned char *rp = buf0 + static_cast<size_t>(cb) * stage_bytes;
-        for (int32_t k = 0; k < n_sub; ++k) rp = track_chunk<P>(q, rp, cold, turns_done, a);
+        for (int32_t k = 0; k < n_sub; ++k) rp = track_chunk<P, THICK>(q, rp, cold, turns_done, a);
       }
       ++gidx;
       if (++c == n_stages) {
@@ -697,13 +753,13 @@ __global__ void xt_init_derived_kernel(xt_particles p, int64_t n, double beta0, 
   p.rvv[i] = opd / b;
 }
 
-template <int P>
-int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
+template <int P, bool THICK>
+int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
   const size_t cold_bytes = (static_cast<size_t>(8 * Cold<P>::kPitch) * block + 127) & ~static_cast<size_t>(127);
   // per device, so set on every launch (a few microseconds against launches of milliseconds to seconds)
-  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P, THICK>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
   // the kernel has no use for L1 (every hot read is a shared-memory broadcast)
-  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P>, cudaFuncAttributePreferredSharedMemoryCarveout,
+  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P, THICK>, cudaFuncAttributePreferredSharedMemoryCarveout,
                                cudaSharedmemCarveoutMaxShared));
   const int64_t cap = static_cast<int64_t>(block) * P;
   const int64_t need = (a.n_part + cap - 1) / cap;
@@ -715,7 +771,7 @@ int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStr
   // Staging depth: as many chunks per bulk copy (fewer CTA-wide barriers per turn) as shared memory
   // allows without taking a resident CTA away.
   cudaFuncAttributes fa;
-  XT_CUDA(cudaFuncGetAttributes(&fa, xt_track_kernel<P>));
+  XT_CUDA(cudaFuncGetAttributes(&fa, xt_track_kernel<P, THICK>));
   int64_t resident = 65536 / (static_cast<int64_t>(fa.numRegs > 0 ? fa.numRegs : 128) * block);
   if (resident > grid / a.grid_quantum) resident = grid / a.grid_quantum;
   if (resident < 1) resident = 1;
@@ -731,10 +787,16 @@ int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStr
     }
   }
   const size_t smem = smem_for(b.stage_chunks);
-  xt_track_kernel<P><<<static_cast<unsigned>(grid), block, smem, st>>>(b);
+  xt_track_kernel<P, THICK><<<static_cast<unsigned>(grid), block, smem, st>>>(b);
   count_launch();
   XT_CUDA(cudaGetLastError());
   return XT_OK;
+}
+
+// Lattices with thick elements take the instantiation that has their maps compiled in.
+template <int P>
+int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
+  return lat->info.n_thick > 0 ? launch_track_pt<P, true>(a, lat, block, st) : launch_track_pt<P, false>(a, lat, block, st);
 }
 
 }  // namespace

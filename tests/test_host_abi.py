@@ -57,7 +57,7 @@ def test_struct_layouts_match_the_header():
     assert ctypes.sizeof(B.xt_particles) == 14 * 8
     assert ctypes.sizeof(B.xt_track_opts) == 24
     assert ctypes.sizeof(B.xt_lattice_opts) == 16
-    assert ctypes.sizeof(B.xt_lattice_info) == 8 * (5 + 8 + 3) + 8 * 3 + 8
+    assert ctypes.sizeof(B.xt_lattice_info) == 8 * (5 + 8 + 3) + 8 * 3 + 8 + 8
 
 
 def test_compute_calls_validate_arguments_without_a_device():
@@ -325,3 +325,18 @@ def test_bench_rank_plumbing_world_size_2(tmp_path):
     assert r0[1] == r1[1] == 2 * 1000.0 / 0.150                              # whole-job aggregate
     assert r0[2] != r1[2] and r0[3] == r1[3] == 1000                         # own ensemble, same size
     assert r0[4] == r1[4]                                                    # same (replicated) lattice
+
+
+def test_thick_quadrupole_is_packed_unfused():
+    from xt_inputs.packed import Quadrupole
+    els = [Drift(1.0), Quadrupole(0.3, 2.5), Drift(0.5), Multipole(knl=(0.0, 0.1)), Quadrupole(-0.2, 1.0)]
+    img, info = X.xt_lattice_pack_host(pack(els))
+    assert info["n_thick"] == 2 and info["n_by_type"][1] == 2 and info["circumference"] == 5.0
+    (recs,) = walk_image(img, info["chunk_bytes"])
+    kinds = [(r[0], r[1]) for r in recs]
+    assert kinds == [(T_DRIFT, 0), (9, 0), (T_MULT, F_PRE), (9, 0)]            # 9 = TAG_QUAD, never fused
+    assert recs[1][4] == 0.3 and recs[1][5][0] == 2.5 and recs[1][3] == 1
+    lib = X.load_library("prod")
+    for bad in (Quadrupole(0.0, 1.0), Quadrupole(0.1, 0.0)):
+        b = pack([bad])
+        assert lib.xt_lattice_pack_host(b, len(b), None, None, 0, None) == -2
