@@ -535,3 +535,75 @@ def test_particles_dead_on_entry_are_left_alone(X):
             assert same.all(), k
         assert_bit_identical({k: v[~dead] for k, v in got.items()}, {k: v[~dead] for k, v in ref.items()})
     lat.close()
+
+
+def _random_line(rng, n_el):
+    """A random sequence of every cavity-free thin element, biased towards the patterns the packer
+    fuses (drift runs, shift/rotation wrappers, apertures behind magnets and drifts) and their
+    broken variants."""
+    els = []
+    while len(els) < n_el:
+        r = rng.random()
+        if r < 0.30:
+            els.append(Drift(float(rng.uniform(0.1, 3.0))))
+        elif r < 0.55:
+            order = int(rng.choice([0, 1, 2, 3, 4, 7, 8, 15, 20]))
+            knl = rng.normal(0, 1, order + 1) * 0.02 / (np.arange(order + 1) + 1.0) * 10.0 ** np.arange(order + 1)
+            ksl = rng.normal(0, 1, order + 1) * 0.02 / (np.arange(order + 1) + 1.0) * 10.0 ** np.arange(order + 1)
+            if rng.random() < 0.3:
+                ksl[:] = 0.0
+            hxl = float(rng.choice([0.0, 0.0, 2e-3, -1e-3]))
+            length = float(rng.choice([0.0, 1.7]))
+            knl, ksl = knl * 2e-3, ksl * 2e-3
+            knl[0] = knl[0] * 0.1 + hxl                   # a bend bends by its curvature, plus a small error
+            ksl[0] *= 0.1
+            els.append(Multipole(knl=tuple(knl), ksl=tuple(ksl), hxl=hxl, length=length))
+        elif r < 0.63:
+            els.append(XYShift(float(rng.normal(0, 1e-4)), float(rng.normal(0, 1e-4))))
+        elif r < 0.71:
+            els.append(SRotation.from_angle(float(rng.normal(0, 2e-3))))
+        elif r < 0.79:                                   # a whole misaligned magnet
+            th, dx, dy = rng.normal(0, 1e-3), rng.normal(0, 1e-4), rng.normal(0, 1e-4)
+            els += [XYShift(float(dx), float(dy)), SRotation.from_angle(float(th)),
+                    Multipole(knl=(0.0, float(rng.normal(0, 0.05)))), SRotation.from_angle(float(-th)),
+                    XYShift(float(-dx), float(-dy))]
+        elif r < 0.88:
+            els.append(LimitEllipse(float(rng.uniform(0.003, 0.03)), float(rng.uniform(0.003, 0.03))))
+        elif r < 0.95:
+            a = float(rng.uniform(0.003, 0.03))
+            els.append(LimitRect(-a, a, -0.8 * a, 1.2 * a))
+        else:
+            els.append(Marker())
+    return els
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_lattices_bit_exact_nofma(X, seed):
+    """Fuzz of step P and the dispatch: random lines through the --fmad=false build must reproduce the
+    oracle bit for bit (coordinates, loss records, s), for random chunk sizes, fusion on and off and
+    random launch shapes; the production build must agree within the 1-turn tolerance."""
+    rng = np.random.default_rng(1000 + seed)
+    els = _random_line(rng, int(rng.integers(30, 140)))
+    buf = pack_lattice(els, H.P0C, H.MASS0, H.Q0)
+    n = int(rng.integers(40, 700))
+    amp = float(rng.choice([0.2, 0.5, 1.0]))
+    co = dict(x=rng.normal(0, 1.5e-3 * amp, n), px=rng.normal(0, 1e-4 * amp, n), y=rng.normal(0, 1.5e-3 * amp, n),
+              py=rng.normal(0, 1e-4 * amp, n), zeta=rng.normal(0, 0.05, n), delta=rng.normal(0, 5e-4, n))
+    turns = int(rng.integers(1, 4))
+    ref = O.new_particles(buf, co)
+    mm = np.full(n, np.inf)
+    O.track(buf, ref, turns, min_margin=mm)
+    for kind in ("nofma", "prod"):
+        for trial in range(3):
+            kw = dict(chunk_bytes=int(rng.choice([1024, 1152, 2048, 8192, 65536])), fuse=bool(rng.random() < 0.7))
+            lat = X.xt_lattice_create_ex(buf, kind=kind, **kw)
+            p = X.new_particles(lat, co)
+            X.xt_track_ex(lat, p, turns, particles_per_thread=int(rng.choice([0, 1, 2, 3, 4])),
+                          block_size=int(rng.choice([0, 32, 64, 128, 256])), compact_every=int(rng.choice([-1, 1, 2])))
+            got = X.particles_to_host(p)
+            lat.close()
+            if kind == "nofma":
+                assert_bit_identical(got, ref)
+            else:
+                clear = assert_losses_match(got, ref, mm)
+                assert_close(got, ref, 1e-12, sel=clear & (ref["state"] == 1))
