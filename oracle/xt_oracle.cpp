@@ -33,6 +33,8 @@
 // invariant; P8 aperture edges; P9 structural invariants; P10 energy identities;
 // small-amplitude synchrotron tune for the cavity; P13 thick quadrupole: second-order limit of
 // thin slices (+ cubic paraxial residual), closed-form matrix, symplecticity, reversibility.
+// P14 thick sector bend ('expanded'): second-order limit of thin curved-dipole slices, textbook
+// matrix and dispersion, symplecticity, reversibility.
 // =====================================================================================
 #include <cmath>
 #include <cstdint>
@@ -48,7 +50,7 @@ constexpr int MAX_ORDER = 20;
 
 enum ElemType : uint32_t {
   MARKER = 0, DRIFT = 1, MULTIPOLE = 2, CAVITY = 3,
-  SROTATION = 4, XYSHIFT = 5, LIMITRECT = 6, LIMITELLIPSE = 7, QUADRUPOLE = 8
+  SROTATION = 4, XYSHIFT = 5, LIMITRECT = 6, LIMITELLIPSE = 7, QUADRUPOLE = 8, BEND = 9
 };
 
 struct Element {
@@ -72,6 +74,8 @@ struct Element {
   double a = 0.0, b = 0.0, a2 = 0.0, b2 = 0.0, a2b2 = 0.0;
   // QUADRUPOLE (thick): k1, length
   double k1 = 0.0;
+  // BEND (thick sector bend): k0, h, length
+  double k0 = 0.0, h = 0.0;
 };
 
 struct Lattice {
@@ -186,6 +190,11 @@ int parse(const void* packed, size_t nbytes, Lattice& L) {
       case QUADRUPOLE:
         if (!rd(e.k1) || !rd(e.length)) return -2;
         if (e.k1 == 0.0 || !(e.length > 0.0)) return -2;   // a zero-strength thick quadrupole is a Drift
+        s = s + e.length;
+        break;
+      case BEND:
+        if (!rd(e.k0) || !rd(e.h) || !rd(e.length)) return -2;
+        if (!(e.k0 * e.h > 0.0) || !(e.length > 0.0)) return -2;   // focusing strength k0 h must be > 0
         s = s + e.length;
         break;
       default: return -2;
@@ -370,6 +379,39 @@ int xo_track(const void* packed, size_t nbytes, const xo_particles* P, int64_t n
             zeta = (zeta + e.length * (k.g / (opd * (opd + k.b)))) - (k.rv0v / (2.0 * k.opd2)) * (i_f + i_d);
             if (focus_x) { x = u1; px = pu1; y = v1; py = pv1; }
             else         { y = u1; py = pu1; x = v1; px = pv1; }
+            break;
+          }
+
+          case BEND: {
+            // Thick sector bend, 'expanded' model ("the bend can be 'full' or 'expanded'";
+            // reading A19): exact flow of
+            //   H = (px^2 + py^2)/(2(1+delta)) - h x (1+delta) + k0 x + (k0 h/2) x^2
+            // (the thin curved multipole of this file, smeared over the arc length L).  With
+            // K = k0 h, w = sqrt(K/(1+delta)) and the equilibrium offset xe = (h (1+delta) - k0)/K:
+            //   x' - xe = (x - xe) cos + px sin/((1+delta) w),  px' = px cos - (1+delta) w (x - xe) sin,
+            //   y' = y + L py/(1+delta),
+            //   zeta' = zeta + L (1 - beta0/beta) - (beta0/beta) h int x ds
+            //           - (beta0/beta)/(2 (1+delta)^2) (int px^2 ds + L py^2).
+            const double opd = 1.0 + delta;
+            const double kk = e.k0 * e.h;
+            const double w = std::sqrt(kk / opd);
+            const double wl = w * e.length;
+            const double cs = std::cos(wl), sn = std::sin(wl);
+            const double c1 = 1.0 - cs;
+            const double ow = opd * w;
+            const double fw = (e.h * opd - e.k0) / w;            // (1+delta) w xe: the offset enters only through it
+            const double a = ow * x - fw;                         // (1+delta) w (x - xe)
+            const double pw = px / ow;
+            const double x1 = (x * cs + pw * sn) + (fw * c1) / ow;
+            const double px1 = px * cs - a * sn;
+            const double y1 = (e.length * py) / opd + y;
+            const double ix = ((x * sn) / w + (pw * c1) / w) + (fw / ow) * (e.length - sn / w);   // int x ds
+            const double px2 = px * px, a2 = a * a;
+            const double ip = ((px2 + a2) * (0.5 * e.length) + ((px2 - a2) * (sn * cs)) * (0.5 / w)) -
+                              ((a * px) * (sn * sn)) / w;                                     // int px^2 ds
+            zeta = ((zeta + e.length * (k.g / (opd * (opd + k.b)))) - (k.rv0v * e.h) * ix) -
+                   (k.rv0v / (2.0 * k.opd2)) * (ip + e.length * (py * py));
+            x = x1; px = px1; y = y1;
             break;
           }
 

@@ -527,3 +527,95 @@ def test_P13_thick_quadrupole_rejects_degenerate_parameters():
         with pytest.raises(ValueError):
             O.reference(pack([bad]))
     assert abs(O.s_table(pack([Quadrupole(0.1, 2.5), Drift(1.0), Marker()]))[2] - 3.5) < 1e-15
+
+
+# ----------------------------- P14 thick sector bend (reading A19)
+from xt_inputs.packed import Bend  # noqa: E402
+
+
+def _thin_sliced_bend(k0, h, length, n):
+    """n symmetric slices [drift, thin curved dipole, drift] of the maps pinned above (P1, P5 W2, P12)."""
+    d = length / (2 * n)
+    return [Drift(d), Multipole(knl=(k0 * length / n,), hxl=h * length / n, length=length / n), Drift(d)] * n
+
+
+@pytest.mark.parametrize("k0,h,length,n", [(2.5e-3, 2.5e-3, 14.3, 4), (2.5005e-3, 2.5e-3, 14.3, 4),
+                                           (-2.2004e-3, -2.2e-3, 14.3, 4), (0.05, 0.05, 8.0, 64)])
+def test_P14_thick_bend_is_the_limit_of_thin_slices(k0, h, length, n):
+    """The 'expanded' sector bend is the exact flow of the Hamiltonian whose kick the thin curved
+    multipole applies; n symmetric slices converge to it as 1/n^2 (x, px, y, zeta: curvature, weak
+    focusing, dispersion and all three path-length terms).  What Richardson extrapolation leaves is
+    the exact-drift vs paraxial difference: cubic in the amplitude."""
+    length = 14.3
+    base = np.array([[1e-3, 2e-4, -5e-4, 1e-4, 0.01, 3e-4], [-2e-3, -1e-4, 1e-3, 3e-4, -0.02, -8e-4],
+                     [5e-4, 0.0, 0.0, -2e-4, 0.0, 0.0]])
+
+    def run(els, start):
+        buf = pack(els)
+        p = O.new_particles(buf, start)
+        O.track(buf, p, 1)
+        return np.stack([p[k] for k in ("x", "px", "y", "py", "zeta")], axis=1)
+
+    residual = {}
+    for amp in (1.0, 0.1):
+        rows = base.copy()
+        rows[:, :4] *= amp
+        rows[:, 5] *= amp                                           # dispersion moves x by delta/h: scale it too
+        start = H.coords_from_rows(rows.tolist())
+        thick = run([Bend(k0, h, length)], start)
+        s1, s2 = run(_thin_sliced_bend(k0, h, length, n), start), run(_thin_sliced_bend(k0, h, length, 2 * n), start)
+        rich = (4.0 * s2 - s1) / 3.0
+        residual[amp] = (rich - thick)[:, :3]
+        if amp == 0.1:
+            e1, e2 = np.abs(s1 - thick)[:, [0, 1, 2, 4]], np.abs(s2 - thick)[:, [0, 1, 2, 4]]
+            big = e1 > 50.0 * np.abs(rich - thick)[:, [0, 1, 2, 4]] + 1e-16   # above the paraxial residual (y: pure drift)
+            assert big.sum() >= 5
+            assert np.all((e1[big] / e2[big] > 3.6) & (e1[big] / e2[big] < 4.4))      # second order in 1/n
+            scale = amp * np.array([1e-3, 1e-4, 1e-3])
+            assert np.max(np.abs(residual[amp]) / scale) < 1e-7
+            slip, slip_thin = thick[:, 4] - rows[:, 4], rich[:, 4] - rows[:, 4]
+            assert np.all(np.abs(slip) > 1e-9)                                         # h x L dominates the slip
+            assert np.max(np.abs(slip_thin - slip) / np.abs(slip)) < 1e-6
+            assert np.array_equal(thick[:, 3], rows[:, 3])                             # py untouched
+    strong = np.abs(residual[1.0]) > 1e-11
+    assert strong.sum() >= 3
+    ratio = residual[1.0][strong] / residual[0.1][strong]
+    # third order in (amplitude, delta): a linear error of the map would give 10, a quadratic one 100
+    assert np.all((ratio > 400.0) & (ratio < 2500.0)), ratio
+
+
+def test_P14_thick_bend_matrix_dispersion_symplectic_reversible():
+    h, length = 2.5e-3, 14.3
+    buf = pack([Bend(h, h, length)])
+    J = H.jacobian6(O.track, buf, np.zeros(6))
+    phi = h * length
+    # textbook sector-bend matrix (x, px) and dispersion column; drift in y
+    np.testing.assert_allclose(J[0:2, 0:2], [[math.cos(phi), math.sin(phi) / h], [-h * math.sin(phi), math.cos(phi)]],
+                               atol=1e-8)
+    np.testing.assert_allclose(J[2:4, 2:4], [[1.0, length], [0.0, 1.0]], atol=1e-8)
+    beta0, _ = O.reference(buf)
+    # d x / d delta = (1 - cos phi)/h, d px / d delta = sin phi; delta = pzeta * (beta0 ... ) at the origin: d delta/d pzeta = beta0/beta = 1
+    assert abs(J[0, 5] - (1.0 - math.cos(phi)) / h) < 1e-6 and abs(J[1, 5] - math.sin(phi)) < 1e-7
+    line = [Drift(0.7), Bend(h, h, length), Drift(0.4), Bend(1.0002 * h, h, 3.0), Cavity(1e6, 200e6, 180.0), Drift(0.2)]
+    for z0 in (np.zeros(6), np.array([1e-3, 2e-4, -5e-4, 1e-4, 0.01, 3e-4])):
+        _check_symplectic(pack(line), z0)
+    rng = np.random.default_rng(9)
+    n = 32
+    co = dict(x=rng.normal(0, 1e-3, n), px=rng.normal(0, 1e-4, n), y=rng.normal(0, 1e-3, n),
+              py=rng.normal(0, 1e-4, n), zeta=rng.normal(0, 0.02, n), delta=rng.normal(0, 3e-4, n))
+    fwd, bwd = pack(line), pack(H.reversed_lattice(line))
+    p = O.new_particles(fwd, co)
+    p0 = O.copy_particles(p)
+    O.track(fwd, p, 2)
+    H.flip_R(p)
+    O.track(bwd, p, 2)
+    H.flip_R(p)
+    for k, scale in (("x", 1e-3), ("px", 1e-4), ("y", 1e-3), ("py", 1e-4), ("zeta", 0.02), ("delta", 3e-4)):
+        assert np.max(np.abs(p[k] - p0[k])) < 1e-12 * scale, k
+
+
+def test_P14_thick_bend_rejects_degenerate_parameters():
+    for bad in (Bend(0.0, 1e-3, 1.0), Bend(1e-3, 0.0, 1.0), Bend(1e-3, -1e-3, 1.0), Bend(1e-3, 1e-3, 0.0)):
+        with pytest.raises(ValueError):
+            O.reference(pack([bad]))
+    assert abs(O.s_table(pack([Bend(1e-3, 1e-3, 2.5), Drift(1.0), Marker()]))[2] - 3.5) < 1e-15

@@ -18,6 +18,8 @@ accelerator element".  Here that sequence is flattened into one little-endian,
     type 6 LIMITRECT     aux=0  min_x, max_x, min_y, max_y
     type 7 LIMITELLIPSE  aux=0  a, b
     type 8 QUADRUPOLE    aux=0  k1 [1/m^2], length [m]   (thick; k1 != 0, length > 0)
+    type 9 BEND          aux=0  k0 [1/m], h [1/m], length [m]   (thick sector bend, 'expanded' map,
+                                PAPER.md:72; k0*h > 0, length > 0; a pure sector bend has k0 = h)
 
 This module is pure serialisation (struct packing).  It performs no tracking
 arithmetic: the same bytes are handed to the oracle and to ``xt_lattice_create``;
@@ -36,7 +38,7 @@ HEADER_BYTES = 48
 
 ELEMENT_TYPE_IDS = {
     "Marker": 0, "Drift": 1, "Multipole": 2, "Cavity": 3,
-    "SRotation": 4, "XYShift": 5, "LimitRect": 6, "LimitEllipse": 7, "Quadrupole": 8,
+    "SRotation": 4, "XYShift": 5, "LimitRect": 6, "LimitEllipse": 7, "Quadrupole": 8, "Bend": 9,
 }
 
 
@@ -107,6 +109,15 @@ class Quadrupole:
     length: float
 
 
+@dataclass(frozen=True)
+class Bend:
+    """Thick sector bend ('expanded' model): dipole strength k0 = By/(P0/q0), curvature h
+    of the reference orbit, arc length."""
+    k0: float
+    h: float
+    length: float
+
+
 def _record(el) -> bytes:
     if isinstance(el, Marker):
         return struct.pack("<II", 0, 0)
@@ -129,6 +140,8 @@ def _record(el) -> bytes:
         return struct.pack("<II2d", 7, 0, el.a, el.b)
     if isinstance(el, Quadrupole):
         return struct.pack("<II2d", 8, 0, el.k1, el.length)
+    if isinstance(el, Bend):
+        return struct.pack("<II3d", 9, 0, el.k0, el.h, el.length)
     raise TypeError("unknown element %r" % (el,))
 
 
@@ -179,6 +192,9 @@ def unpack_lattice(buf: bytes):
         elif t == 8:
             k1, length = struct.unpack_from("<2d", buf, off); off += 16
             out.append(Quadrupole(k1, length))
+        elif t == 9:
+            k0, h, length = struct.unpack_from("<3d", buf, off); off += 24
+            out.append(Bend(k0, h, length))
         else:
             raise ValueError("unknown element type %d" % t)
     return out, p0c, mass0, q0
