@@ -52,8 +52,10 @@ enum {
   XT_XYSHIFT = 5,     /* dx, dy                                                  (map M4)   */
   XT_LIMITRECT = 6,   /* min_x, max_x, min_y, max_y (edges inclusive)            (step A)   */
   XT_LIMITELLIPSE = 7,/* a, b (edge inclusive)                                   (step A)   */
-  XT_QUADRUPOLE = 8   /* k1 [1/m^2], length [m]: thick quadrupole, k1 != 0, length > 0           */
+  XT_QUADRUPOLE = 8,  /* k1 [1/m^2], length [m]: thick quadrupole, k1 != 0, length > 0           */
                       /* (reading A18)             */
+  XT_BEND = 9         /* k0 [1/m], h [1/m], length [m]: thick sector bend, 'expanded' model,     */
+                      /* k0*h > 0, length > 0 (reading A19)               */
 };
 
 /* Packed lattice buffer (HOST memory, little-endian, 8-byte aligned records):
@@ -107,7 +109,7 @@ typedef struct {
   double circumference;     /* sum of drift and thick-element lengths [m]                     */
   int64_t n_drift_evals;    /* sqrt evaluations per turn after fusion (consecutive drifts     */
                             /* share one; equals the number of drifts when fuse is off)       */
-  int64_t n_thick;          /* thick elements (XT_QUADRUPOLE); not counted in n_by_type       */
+  int64_t n_thick;          /* thick elements (XT_QUADRUPOLE, XT_BEND); not in n_by_type      */
 } xt_lattice_info;
 
 /* Options of xt_lattice_create_ex.  Zero-initialise for the defaults.  Neither changes any

@@ -46,6 +46,7 @@ namespace xt {
 //   TAG_RECT     p0 unused; {min_x, max_x}; {min_y, max_y}                       48 B
 //   TAG_ELLIPSE  p0 = a2*b2; {b2, a2}                                            32 B
 //   TAG_QUAD     p0 = k1; {length, 0}   (thick quadrupole; never fused)          32 B
+//   TAG_BEND     p0 = k0; {h, length}   (thick sector bend; never fused)         32 B
 //
 // elem = index of the element in the user's packed buffer (for a fused record: the
 // multipole's; only aperture records ever report it).
@@ -60,6 +61,7 @@ enum : uint32_t {
   TAG_ELLIPSE = 7,
   TAG_CMULT = 8,
   TAG_QUAD = 9,
+  TAG_BEND = 10,
   TAG_TYPE_MASK = 0xf,
   TAG_PRE = 0x10,   // a drift of length l_pre comes first
   TAG_POST = 0x20,  // a drift of length l_post follows the kick

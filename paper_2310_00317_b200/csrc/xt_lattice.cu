@@ -235,6 +235,22 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
         s_pos += length;
         break;
       }
+      case XT_BEND: {
+        const double k0 = r.real();
+        const double h = r.real();
+        const double length = r.real();
+        if (!r.ok) break;
+        if (!(k0 * h > 0.0) || !(length > 0.0)) {
+          set_error("xt_lattice_create: thick bend needs k0*h > 0 and length > 0");
+          return XT_ERR_BAD_LATTICE;
+        }
+        rec.type = TAG_BEND;
+        rec.p0 = k0;
+        rec.slot(h, length);
+        info.n_thick += 1;
+        s_pos += length;
+        break;
+      }
       default:
         set_error("xt_lattice_create: unknown element type id");
         return XT_ERR_BAD_LATTICE;

@@ -122,6 +122,11 @@ struct QuadCase {
   static constexpr uint32_t value = (P == 4 && !THICK) ? 0x1ffu : static_cast<uint32_t>(TAG_QUAD);
 };
 
+template <bool THICK>
+struct BendCase {  // thin kernels keep the dispatch tree they were measured with: the label is parked there
+  static constexpr uint32_t value = THICK ? static_cast<uint32_t>(TAG_BEND) : 0x2ffu;
+};
+
 constexpr int kPrefetch = 4;  // 16-byte slots of a record loaded ahead of its dispatch ...
 #ifndef XT_PF4
 #define XT_PF4 2
@@ -473,6 +478,41 @@ __device__ __noinline__ void thick_quadrupole(Parts<P> &q, const Cold<P> &cold, 
   }
 }
 
+// Thick sector bend, 'expanded' model (reading A19):
+// the exact flow of H = (px^2 + py^2)/(2(1+delta)) - h x (1+delta) + k0 x + (k0 h/2) x^2, i.e. the
+// thin curved multipole of step M2 smeared over the arc length.  Same arithmetic as the oracle's.
+template <int P>
+__device__ __noinline__ void thick_bend(Parts<P> &q, const Cold<P> &cold, const double k0, const double h,
+                                        const double length) {
+#pragma unroll 1
+  for (int j = 0; j < P; ++j) {
+    const double opd = 1.0 + cold.delta(j);
+    const double w = sqrt(XT_MUL(k0, h) / opd);
+    const double wl = XT_MUL(w, length);
+    double sn, cs;
+    sincos(wl, &sn, &cs);
+    const double c1 = 1.0 - cs;
+    const double ow = XT_MUL(opd, w);
+    const double fw = XT_NMADD(1.0, k0, XT_MUL(h, opd)) / w;  // (h (1+delta) - k0)/w
+    const double x = q.x[j], px = q.px[j], py = q.py[j];
+    const double a = XT_MADD(ow, x, -fw);
+    const double pw = px / ow;
+    const double x1 = XT_MADD(x, cs, XT_MUL(pw, sn)) + XT_MUL(fw, c1) / ow;
+    const double px1 = XT_NMADD(a, sn, XT_MUL(px, cs));
+    const double ix = (XT_MUL(x, sn) / w + XT_MUL(pw, c1) / w) + XT_MUL(fw / ow, length - sn / w);
+    const double px2 = XT_MUL(px, px), a2 = XT_MUL(a, a);
+    const double ip = XT_MADD(px2 + a2, XT_MUL(0.5, length), XT_MUL(XT_MUL(px2 - a2, XT_MUL(sn, cs)), 0.5 / w)) -
+                      XT_MUL(XT_MUL(a, px), XT_MUL(sn, sn)) / w;
+    const double rv = cold.rv0v(j);
+    const double slip = XT_MUL(length, cold.g(j) / XT_MUL(opd, opd + cold.b(j)));
+    q.zeta[j] = ((q.zeta[j] + slip) - XT_MUL(XT_MUL(rv, h), ix)) -
+                XT_MUL(rv / XT_MUL(2.0, cold.opd2(j)), ip + XT_MUL(length, XT_MUL(py, py)));
+    q.y[j] = XT_MUL(length, py) / opd + q.y[j];
+    q.x[j] = x1;
+    q.px[j] = px1;
+  }
+}
+
 // A: elliptical aperture (x^2 b^2 + y^2 a^2 <= a^2 b^2, edge inclusive, NaN lost).
 template <int P>
 __device__ __forceinline__ void limit_ellipse(Parts<P> &q, const Cold<P> &cold, const double2 ba, const double a2b2,
@@ -578,6 +618,10 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
       }
       case QuadCase<P, THICK>::value: {  // thick quadrupole (see QuadCase)
         if (THICK) thick_quadrupole<P>(q, cold, p0, pf[0].x);  // p0 = k1, pf[0].x = length
+        break;
+      }
+      case BendCase<THICK>::value: {  // thick sector bend: p0 = k0, pf[0] = (h, length)
+        if (THICK) thick_bend<P>(q, cold, p0, pf[0].x, pf[0].y);
         break;
       }
       default:  // ... and every other combination (misaligned magnets, lone leading drifts) at run time

@@ -1,0 +1,90 @@
+"""Thick sector bend ('expanded' model, reading A19) on the GPU path against the oracle: a
+ring of thick bends and thick quadrupoles with a cavity and apertures; 1 turn at 1e-12, 100 turns at
+1e-10, losses exact, every launch shape bit-identical."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from xt_inputs.packed import Bend, Cavity, Drift, LimitEllipse, Multipole, Quadrupole, pack_lattice
+
+pytestmark = pytest.mark.gpu
+P0C, MASS0 = 450e9, 938272088.16
+KEYS = ("x", "px", "y", "py", "zeta", "delta", "ptau")
+
+
+@pytest.fixture(scope="module")
+def X():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (run with -m gpu on the B200 box)")
+    import paper_2310_00317_b200 as X
+    return X
+
+
+def ring(n_cells=16, aperture=0.04):
+    h = 2.0 * np.pi / (2 * n_cells * 6.0)                      # 2 bends of 6 m per cell close the ring
+    cell = [Quadrupole(+0.35, 0.6), Drift(0.5), Bend(h, h, 6.0), Drift(0.5), Multipole(knl=(0.0, 0.0, 0.3)),
+            Quadrupole(-0.35, 0.6), Drift(0.5), Bend(h * 1.0001, h, 6.0), Drift(0.5), LimitEllipse(aperture, aperture)]
+    return cell * n_cells + [Cavity(1e6, 200e6, 180.0)]
+
+
+def ensemble(n, scale=1.0, seed=31):
+    rng = np.random.default_rng(seed)
+    return dict(x=rng.normal(0, 3e-4 * scale, n), px=rng.normal(0, 2e-5 * scale, n),
+                y=rng.normal(0, 3e-4 * scale, n), py=rng.normal(0, 2e-5 * scale, n),
+                zeta=rng.normal(0, 0.05, n), delta=rng.normal(0, 3e-4, n))
+
+
+def close(got, ref, rtol, sel):
+    for k in KEYS:
+        a, r = got[k][sel], ref[k][sel]
+        ok = np.abs(a - r) <= np.maximum(rtol * np.abs(r), rtol * 1e-3)
+        assert ok.all(), (k, int((~ok).sum()), float(np.max(np.abs(a - r))))
+
+
+def test_thick_bend_ring_parity(X):
+    buf = pack_lattice(ring(), P0C, MASS0, 1.0)
+    co = ensemble(4000)
+    lat = X.xt_lattice_create(buf)
+    assert lat.info["n_thick"] == 64
+    np.testing.assert_allclose(X.xt_lattice_s_table(lat), O.s_table(buf), rtol=0, atol=1e-12)
+    for turns, rtol in ((1, 1e-12), (100, 1e-10)):
+        ref = O.new_particles(buf, co)
+        O.track(buf, ref, turns, threads=O.host_threads())
+        p = X.new_particles(lat, co)
+        X.xt_track(lat, p, turns)
+        got = X.particles_to_host(p)
+        assert (ref["state"] == 1).mean() > 0.99 and np.array_equal(got["state"], ref["state"])
+        assert np.array_equal(got["at_turn"], ref["at_turn"])
+        close(got, ref, rtol, ref["state"] == 1)
+    lat.close()
+
+
+def test_thick_bend_losses_and_shapes(X):
+    buf = pack_lattice(ring(aperture=0.003), P0C, MASS0, 1.0)
+    co = ensemble(2500, scale=4.0)
+    ref = O.new_particles(buf, co)
+    mm = np.full(2500, np.inf)
+    O.track(buf, ref, 10, threads=O.host_threads(), min_margin=mm)
+    assert 0.05 < (ref["state"] == 0).mean() < 0.95
+    lat = X.xt_lattice_create(buf)
+    base = None
+    for ppt, block in ((0, 0), (1, 64), (2, 32), (3, 96), (4, 128)):
+        p = X.new_particles(lat, co)
+        X.xt_track_ex(lat, p, 10, particles_per_thread=ppt, block_size=block, compact_every=3 if ppt == 2 else -1)
+        got = X.particles_to_host(p)
+        if base is None:
+            base = got
+            clear = mm >= 1e-9
+            for k in ("state", "at_turn", "at_element"):
+                assert np.array_equal(got[k][clear], ref[k][clear]), k
+            close(got, ref, 1e-11, clear & (ref["state"] == 1))
+        else:
+            for k in got:
+                a, b = got[k], base[k]
+                assert ((a == b) | (np.isnan(a.astype(np.float64)) & np.isnan(b.astype(np.float64)))).all(), (ppt, k)
+    lat.close()
+    for bad in (Bend(0.0, 1e-3, 1.0), Bend(1e-3, -1e-3, 1.0), Bend(1e-3, 1e-3, 0.0)):
+        with pytest.raises(X.XtError) as e:
+            X.xt_lattice_create(pack_lattice([bad], P0C, MASS0, 1.0))
+        assert e.value.code == -2

@@ -340,3 +340,18 @@ def test_thick_quadrupole_is_packed_unfused():
     for bad in (Quadrupole(0.0, 1.0), Quadrupole(0.1, 0.0)):
         b = pack([bad])
         assert lib.xt_lattice_pack_host(b, len(b), None, None, 0, None) == -2
+
+
+def test_thick_bend_is_packed_unfused():
+    from xt_inputs.packed import Bend, Quadrupole
+    els = [Drift(1.0), Bend(2e-3, 2.1e-3, 3.0), Drift(0.5), Quadrupole(0.3, 1.5), Bend(1e-3, 1e-3, 2.0), Drift(1.0)]
+    img, info = X.xt_lattice_pack_host(pack(els))
+    assert info["n_thick"] == 3 and info["circumference"] == 9.0                # bends advance s by the arc length
+    (recs,) = walk_image(img, info["chunk_bytes"])
+    assert [(r[0], r[1]) for r in recs] == [(T_DRIFT, 0), (10, 0), (T_DRIFT, 0), (9, 0), (10, 0), (T_DRIFT, 0)]
+    assert recs[1][4] == 2e-3 and tuple(recs[1][5][:2]) == (2.1e-3, 3.0) and recs[1][3] == 1   # p0 = k0, slot {h, length}
+    assert recs[4][4] == 1e-3 and tuple(recs[4][5][:2]) == (1e-3, 2.0) and recs[4][3] == 4
+    lib = X.load_library("prod")
+    for bad in (Bend(0.0, 1e-3, 1.0), Bend(1e-3, 0.0, 1.0), Bend(1e-3, -1e-3, 1.0), Bend(1e-3, 1e-3, 0.0)):
+        b = pack([bad])
+        assert lib.xt_lattice_pack_host(b, len(b), None, None, 0, None) == -2
