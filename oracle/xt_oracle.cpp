@@ -34,7 +34,9 @@
 // small-amplitude synchrotron tune for the cavity; P13 thick quadrupole: second-order limit of
 // thin slices (+ cubic paraxial residual), closed-form matrix, symplecticity, reversibility.
 // P14 thick sector bend ('expanded'): second-order limit of thin curved-dipole slices, textbook
-// matrix and dispersion, symplecticity, reversibility.
+// matrix and dispersion, symplecticity, reversibility; P15 LimitPolygon (even-odd rule): half-plane
+// test on convex polygons, union of rectangles, LimitRect on four corners
+// (tests/test_oracle_refine_pins.py; P16 there pins oracle/refine.py, which tracks with this file).
 // =====================================================================================
 #include <cmath>
 #include <cstdint>
@@ -50,7 +52,8 @@ constexpr int MAX_ORDER = 20;
 
 enum ElemType : uint32_t {
   MARKER = 0, DRIFT = 1, MULTIPOLE = 2, CAVITY = 3,
-  SROTATION = 4, XYSHIFT = 5, LIMITRECT = 6, LIMITELLIPSE = 7, QUADRUPOLE = 8, BEND = 9
+  SROTATION = 4, XYSHIFT = 5, LIMITRECT = 6, LIMITELLIPSE = 7, QUADRUPOLE = 8, BEND = 9,
+  LIMITPOLYGON = 10
 };
 
 struct Element {
@@ -76,6 +79,8 @@ struct Element {
   double k1 = 0.0;
   // BEND (thick sector bend): k0, h, length
   double k0 = 0.0, h = 0.0;
+  // LIMITPOLYGON: vertices (vx[i], vy[i]), closed
+  std::vector<double> vx, vy;
 };
 
 struct Lattice {
@@ -196,6 +201,13 @@ int parse(const void* packed, size_t nbytes, Lattice& L) {
         if (!rd(e.k0) || !rd(e.h) || !rd(e.length)) return -2;
         if (!(e.k0 * e.h > 0.0) || !(e.length > 0.0)) return -2;   // focusing strength k0 h must be > 0
         s = s + e.length;
+        break;
+      case LIMITPOLYGON:
+        if (aux < 3 || aux > 256) return -2;
+        e.vx.resize(aux);
+        e.vy.resize(aux);
+        for (uint32_t n = 0; n < aux; ++n) if (!rd(e.vx[n])) return -2;
+        for (uint32_t n = 0; n < aux; ++n) if (!rd(e.vy[n])) return -2;
         break;
       default: return -2;
     }
@@ -462,6 +474,34 @@ int xo_track(const void* packed, size_t nbytes, const xo_particles* P, int64_t n
             const double tt = (x * x) * e.b2 + (y * y) * e.a2;
             const bool inside = (tt <= e.a2b2);
             double m = std::fabs(std::sqrt((x * x) / e.a2 + (y * y) / e.b2) - 1.0) * std::fmin(e.a, e.b);
+            if (m < margin) margin = m;
+            if (!inside) { state = 0; at_element = ie; s = e.s_pos; }
+            break;
+          }
+
+          case LIMITPOLYGON: {
+            // PAPER.md:178 "polygonal" aperture (reading A20): even-odd rule.  The half line from the
+            // particle towards +x crosses edge (j -> i) iff the edge's ends lie on different sides of the
+            // horizontal through the particle and the crossing point is to the right of it; an odd
+            // number of crossings means inside.  NaN coordinates cross nothing: lost (reading A4).
+            const size_t nv = e.vx.size();
+            bool inside = false;
+            double m = INFINITY;
+            for (size_t i = 0, j = nv - 1; i < nv; j = i, ++i) {
+              const double xi = e.vx[i], yi = e.vy[i], xj = e.vx[j], yj = e.vy[j];
+              if ((yi > y) != (yj > y)) {
+                const double xc = ((xj - xi) * (y - yi)) / (yj - yi) + xi;
+                if (x < xc) inside = !inside;
+              }
+              // distance to the edge (margin bookkeeping only)
+              const double ex = xj - xi, ey = yj - yi;
+              const double l2 = ex * ex + ey * ey;
+              double t = l2 > 0.0 ? ((x - xi) * ex + (y - yi) * ey) / l2 : 0.0;
+              t = std::fmin(1.0, std::fmax(0.0, t));
+              const double qx = x - (xi + t * ex), qy = y - (yi + t * ey);
+              const double d = std::sqrt(qx * qx + qy * qy);
+              if (d < m) m = d;
+            }
             if (m < margin) margin = m;
             if (!inside) { state = 0; at_element = ie; s = e.s_pos; }
             break;

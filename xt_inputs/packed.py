@@ -20,6 +20,8 @@ accelerator element".  Here that sequence is flattened into one little-endian,
     type 8 QUADRUPOLE    aux=0  k1 [1/m^2], length [m]   (thick; k1 != 0, length > 0)
     type 9 BEND          aux=0  k0 [1/m], h [1/m], length [m]   (thick sector bend, 'expanded' map,
                                 PAPER.md:72; k0*h > 0, length > 0; a pure sector bend has k0 = h)
+    type 10 LIMITPOLYGON aux=n  x[0..n), y[0..n)   (closed polygon, 3 <= n <= 256 vertices; PAPER.md:178
+                                "polygonal interpolation")
 
 This module is pure serialisation (struct packing).  It performs no tracking
 arithmetic: the same bytes are handed to the oracle and to ``xt_lattice_create``;
@@ -38,7 +40,7 @@ HEADER_BYTES = 48
 
 ELEMENT_TYPE_IDS = {
     "Marker": 0, "Drift": 1, "Multipole": 2, "Cavity": 3,
-    "SRotation": 4, "XYShift": 5, "LimitRect": 6, "LimitEllipse": 7, "Quadrupole": 8, "Bend": 9,
+    "SRotation": 4, "XYShift": 5, "LimitRect": 6, "LimitEllipse": 7, "Quadrupole": 8, "Bend": 9, "LimitPolygon": 10,
 }
 
 
@@ -118,6 +120,14 @@ class Bend:
     length: float
 
 
+@dataclass(frozen=True)
+class LimitPolygon:
+    """Aperture given by a closed polygon (the "locally refined aperture model obtained by
+    polygonal interpolation"); vertices in order, the last one joins the first."""
+    x: Tuple[float, ...]
+    y: Tuple[float, ...]
+
+
 def _record(el) -> bytes:
     if isinstance(el, Marker):
         return struct.pack("<II", 0, 0)
@@ -142,6 +152,9 @@ def _record(el) -> bytes:
         return struct.pack("<II2d", 8, 0, el.k1, el.length)
     if isinstance(el, Bend):
         return struct.pack("<II3d", 9, 0, el.k0, el.h, el.length)
+    if isinstance(el, LimitPolygon):
+        assert len(el.x) == len(el.y)
+        return struct.pack("<II%dd" % (2 * len(el.x)), 10, len(el.x), *el.x, *el.y)
     raise TypeError("unknown element %r" % (el,))
 
 
@@ -195,6 +208,9 @@ def unpack_lattice(buf: bytes):
         elif t == 9:
             k0, h, length = struct.unpack_from("<3d", buf, off); off += 24
             out.append(Bend(k0, h, length))
+        elif t == 10:
+            vals = struct.unpack_from("<%dd" % (2 * aux), buf, off); off += 16 * aux
+            out.append(LimitPolygon(tuple(vals[:aux]), tuple(vals[aux:])))
         else:
             raise ValueError("unknown element type %d" % t)
     return out, p0c, mass0, q0
