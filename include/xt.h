@@ -54,8 +54,10 @@ enum {
   XT_LIMITELLIPSE = 7,/* a, b (edge inclusive)                                   (step A)   */
   XT_QUADRUPOLE = 8,  /* k1 [1/m^2], length [m]: thick quadrupole, k1 != 0, length > 0           */
                       /* (reading A18)             */
-  XT_BEND = 9         /* k0 [1/m], h [1/m], length [m]: thick sector bend, 'expanded' model,     */
+  XT_BEND = 9,        /* k0 [1/m], h [1/m], length [m]: thick sector bend, 'expanded' model,     */
                       /* k0*h > 0, length > 0 (reading A19)               */
+  XT_LIMITPOLYGON = 10/* aux = n vertices (3..256); x[0..n), y[0..n): closed polygon, even-odd    */
+                      /* rule, NaN lost ("polygonal"; reading A20)         */
 };
 
 /* Packed lattice buffer (HOST memory, little-endian, 8-byte aligned records):
@@ -198,6 +200,22 @@ typedef struct {
 } xt_twiss4d_result;
 int xt_twiss4d(const xt_lattice *lat, double delta0, const double *guess4, xt_twiss4d_result *out,
                void *cuda_stream);
+
+/* Loss-location refinement ("particle backtracking and a locally
+ * refined aperture model obtained by polygonal interpolation", Fig. 4; reading A20 and
+ * section 16).  For every particle of `p` (DEVICE, as left by xt_track on `lat`) with state == 0 whose
+ * at_element is a LimitRect / LimitEllipse with length between it and the previous such aperture (or
+ * the start of the line): the particle is tracked back to that upstream aperture and forward again in
+ * steps of at most `ds` [m] through polygons of `n_poly` vertices (3..256) interpolated between the
+ * two apertures, shifts and tilts included; x, px, y, py, zeta, delta, ptau, rpp, rvv and s are
+ * overwritten with the values at the first polygon it fails (s = position of that polygon); state,
+ * at_turn and at_element are kept.  A particle that fails none keeps its record.  All tracking runs in
+ * the xt_track kernels on small lattices built on the host from the packed buffer the lattice was
+ * created from; one pair of launches per flagging aperture.  p->at_element must not be NULL.  Call it
+ * once per tracked ensemble: a refined record no longer sits at its at_element.
+ * *n_refined (HOST, may be NULL) = number of records moved.  Synchronises the stream. */
+int xt_refine_loss_location(const xt_lattice *lat, const xt_particles *p, int64_t n_part, double ds,
+                            int32_t n_poly, int64_t *n_refined, void *cuda_stream);
 
 /* Number of kernels the library has launched from this process so far (bench bookkeeping). */
 int64_t xt_launch_count(void);

@@ -87,6 +87,8 @@ SIGNATURES = {
                                          ctypes.POINTER(ctypes.c_double), _VP]),
     "xt_twiss4d": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
                                   ctypes.POINTER(xt_twiss4d_result), _VP]),
+    "xt_refine_loss_location": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, ctypes.c_double,
+                                               ctypes.c_int32, ctypes.POINTER(ctypes.c_int64), _VP]),
     "xt_launch_count": (_I64, []),
     "xt_last_error": (ctypes.c_char_p, []),
     "xt_build_info": (ctypes.c_char_p, []),
@@ -350,6 +352,15 @@ def xt_twiss4d(lat: Lattice, delta0: float = 0.0, guess4=None, stream=None) -> D
     out["co"] = np.array(list(res.co))
     out["m"] = np.array(list(res.m)).reshape(4, 4)
     return out
+
+
+def xt_refine_loss_location(lat: Lattice, p: Dict, ds: float, n_poly: int = 64, stream=None) -> int:
+    """Refine in place the loss records of the device SoA ``p`` (see include/xt.h); returns how many moved."""
+    st = _struct_from_tensors(p)
+    moved = ctypes.c_int64(0)
+    _check(lat._lib, lat._lib.xt_refine_loss_location(lat.handle, ctypes.byref(st), _n_part(p), float(ds),
+                                                      int(n_poly), ctypes.byref(moved), _stream_ptr(stream)))
+    return int(moved.value)
 
 
 def xt_launch_count(kind: str = "prod") -> int:

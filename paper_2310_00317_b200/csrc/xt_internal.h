@@ -47,6 +47,7 @@ namespace xt {
 //   TAG_ELLIPSE  p0 = a2*b2; {b2, a2}                                            32 B
 //   TAG_QUAD     p0 = k1; {length, 0}   (thick quadrupole; never fused)          32 B
 //   TAG_BEND     p0 = k0; {h, length}   (thick sector bend; never fused)         32 B
+//   TAG_POLY     p0 unused; n vertices {x_k, y_k} (polygon aperture; never fused)  16 + 16 n
 //
 // elem = index of the element in the user's packed buffer (for a fused record: the
 // multipole's; only aperture records ever report it).
@@ -62,6 +63,7 @@ enum : uint32_t {
   TAG_CMULT = 8,
   TAG_QUAD = 9,
   TAG_BEND = 10,
+  TAG_POLY = 11,
   TAG_TYPE_MASK = 0xf,
   TAG_PRE = 0x10,   // a drift of length l_pre comes first
   TAG_POST = 0x20,  // a drift of length l_post follows the kick
@@ -101,6 +103,8 @@ struct xt_lattice {
   int device = -1;
   int n_sm = 0;  // multiprocessors of `device`: the grid quantum of the tracking kernel
   std::vector<double> s_table_host;
+  std::vector<unsigned char> packed_host;  // the buffer the lattice was created from (xt_refine.cu re-reads it)
+  bool extended = false;                   // thick maps or polygon apertures: the THICK kernels
   unsigned char *d_image = nullptr;
   xt::ChunkDesc *d_chunks = nullptr;
   double *d_s_table = nullptr;
@@ -125,6 +129,7 @@ struct HostImage {
   std::vector<double> s_table;
   xt_lattice_info info{};
   RefConsts k{};
+  bool extended = false;
 };
 struct PackOpts {
   uint32_t chunk_bytes = kDefaultChunkBytes;

@@ -111,6 +111,7 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
 
   xt_lattice_info &info = out.info;
   info = xt_lattice_info{};
+  out.extended = false;
   info.n_elements = n_elements;
   info.beta0 = beta0;
   info.gamma0 = gamma0;
@@ -228,6 +229,7 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
           set_error("xt_lattice_create: thick quadrupole needs k1 != 0 and length > 0 (a zero-strength one is a Drift)");
           return XT_ERR_BAD_LATTICE;
         }
+        out.extended = true;
         rec.type = TAG_QUAD;
         rec.p0 = k1;
         rec.slot(length, 0.0);
@@ -244,11 +246,25 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
           set_error("xt_lattice_create: thick bend needs k0*h > 0 and length > 0");
           return XT_ERR_BAD_LATTICE;
         }
+        out.extended = true;
         rec.type = TAG_BEND;
         rec.p0 = k0;
         rec.slot(h, length);
         info.n_thick += 1;
         s_pos += length;
+        break;
+      }
+      case XT_LIMITPOLYGON: {
+        if (aux < 3 || aux > 256) {
+          set_error("xt_lattice_create: a polygon aperture needs 3 to 256 vertices");
+          return XT_ERR_BAD_LATTICE;
+        }
+        std::vector<double> vx(aux);
+        for (uint32_t k = 0; k < aux; ++k) vx[k] = r.real();
+        for (uint32_t k = 0; k < aux; ++k) rec.slot(vx[k], r.real());
+        rec.type = TAG_POLY;
+        info.has_aperture = 1;
+        out.extended = true;
         break;
       }
       default:
@@ -450,6 +466,8 @@ extern "C" int xt_lattice_create_ex(const void *packed, size_t nbytes, const xt_
   lat->info = img.info;
   lat->k = img.k;
   lat->s_table_host = img.s_table;
+  lat->extended = img.extended;
+  lat->packed_host.assign(static_cast<const unsigned char *>(packed), static_cast<const unsigned char *>(packed) + nbytes);
 
   auto fail = [&](cudaError_t e, const char *what) {
     int code = xt::cuda_fail(e, what);

@@ -127,6 +127,11 @@ struct BendCase {  // thin kernels keep the dispatch tree they were measured wit
   static constexpr uint32_t value = THICK ? static_cast<uint32_t>(TAG_BEND) : 0x2ffu;
 };
 
+template <bool THICK>
+struct PolyCase {
+  static constexpr uint32_t value = THICK ? static_cast<uint32_t>(TAG_POLY) : 0x3ffu;
+};
+
 constexpr int kPrefetch = 4;  // 16-byte slots of a record loaded ahead of its dispatch ...
 #ifndef XT_PF4
 #define XT_PF4 2
@@ -527,6 +532,31 @@ __device__ __forceinline__ void limit_ellipse(Parts<P> &q, const Cold<P> &cold, 
   if (out) lose<P>(q, out, cold, elem, turns_done, a);
 }
 
+// A: polygon aperture (even-odd rule; reading A20): the half line from the particle towards +x
+// crosses edge (v[i-1] -> v[i]) iff its ends lie on different sides of the horizontal through the particle
+// and the crossing point is to the right of it.  NaN crosses nothing: lost.  THICK kernels only.
+template <int P>
+__device__ __noinline__ void limit_polygon(Parts<P> &q, const Cold<P> &cold, const double2 *v, int n, uint32_t elem,
+                                           int64_t turns_done, const TrackArgs &a) {
+  uint32_t in = 0;
+  double2 vj = v[n - 1];
+#pragma unroll 1
+  for (int i = 0; i < n; ++i) {
+    const double2 vi = v[i];
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+      const double y = q.y[j];
+      if ((vi.y > y) != (vj.y > y)) {
+        const double xc = XT_MUL(vj.x - vi.x, y - vi.y) / (vj.y - vi.y) + vi.x;
+        if (q.x[j] < xc) in ^= (1u << j);
+      }
+    }
+    vj = vi;
+  }
+  const uint32_t out = ~in & q.alive;
+  if (out) lose<P>(q, out, cold, elem, turns_done, a);
+}
+
 // Push the P particles of this thread through every record of one staged chunk.
 // Returns the position just behind the chunk (where the next chunk of the image starts).
 template <int P, bool THICK>
@@ -622,6 +652,10 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
       }
       case BendCase<THICK>::value: {  // thick sector bend: p0 = k0, pf[0] = (h, length)
         if (THICK) thick_bend<P>(q, cold, p0, pf[0].x, pf[0].y);
+        break;
+      }
+      case PolyCase<THICK>::value: {  // polygon aperture: (record bytes - header) / 16 vertices
+        if (THICK) limit_polygon<P>(q, cold, slots, static_cast<int>(((tag >> 16) - sizeof(RecHdr)) / 16), elem, turns_done, a);
         break;
       }
       default:  // ... and every other combination (misaligned magnets, lone leading drifts) at run time
@@ -852,7 +886,7 @@ int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaSt
 // Lattices with thick elements take the instantiation that has their maps compiled in.
 template <int P>
 int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
-  return lat->info.n_thick > 0 ? launch_track_pt<P, true>(a, lat, block, st) : launch_track_pt<P, false>(a, lat, block, st);
+  return lat->extended ? launch_track_pt<P, true>(a, lat, block, st) : launch_track_pt<P, false>(a, lat, block, st);
 }
 
 }  // namespace

@@ -355,3 +355,21 @@ def test_thick_bend_is_packed_unfused():
     for bad in (Bend(0.0, 1e-3, 1.0), Bend(1e-3, 0.0, 1.0), Bend(1e-3, -1e-3, 1.0), Bend(1e-3, 1e-3, 0.0)):
         b = pack([bad])
         assert lib.xt_lattice_pack_host(b, len(b), None, None, 0, None) == -2
+
+
+def test_polygon_aperture_is_packed_unfused_and_refine_rejects_bad_arguments():
+    from xt_inputs.packed import LimitPolygon
+    tri = LimitPolygon((0.0, 1.0, 0.0), (0.0, 0.0, 2.0))
+    els = [Drift(1.0), Multipole(knl=(0.0, 0.1)), tri, Drift(0.5), LimitEllipse(0.01, 0.02)]
+    img, info = X.xt_lattice_pack_host(pack(els))
+    assert info["has_aperture"] == 1 and info["n_thick"] == 0
+    (recs,) = walk_image(img, info["chunk_bytes"])
+    assert [r[0] for r in recs][:2] == [T_MULT, 11]                             # 11 = TAG_POLY; never fused into the kick
+    assert recs[1][3] == 2 and list(recs[1][5][:6]) == [0.0, 0.0, 1.0, 0.0, 0.0, 2.0]
+    lib = X.load_library("prod")
+    for bad in (LimitPolygon((0.0, 1.0), (0.0, 1.0)), LimitPolygon(tuple(range(257)), tuple(range(257)))):
+        b = pack([bad])
+        assert lib.xt_lattice_pack_host(b, len(b), None, None, 0, None) == -2
+    big = pack([LimitPolygon(tuple(float(i) for i in range(256)), tuple(float(i * i) for i in range(256)))])
+    assert lib.xt_lattice_pack_host(big, len(big), None, None, 0, None) > 4096
+    assert lib.xt_refine_loss_location(None, None, 0, 0.1, 16, None, None) == -1  # NULL lattice: no CUDA call
