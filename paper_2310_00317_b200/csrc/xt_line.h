@@ -1,0 +1,70 @@
+// The user's packed lattice buffer (include/xt.h) re-read as a list of elements: what the host-side
+// features beyond the hot path (xt_refine.cu, xt_knobs.cu) work from.  The buffer was validated by
+// xt_lattice_create, which keeps a copy (xt_lattice::packed_host).
+#pragma once
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+#include "../../include/xt.h"
+
+namespace xt {
+
+struct Elem {
+  uint32_t type = 0, aux = 0;
+  std::vector<double> v;  // parameters as stored in the packed buffer
+  double length() const {
+    if (type == XT_DRIFT) return v[0];
+    if (type == XT_QUADRUPOLE) return v[1];
+    if (type == XT_BEND) return v[2];
+    return 0.0;
+  }
+  bool is_aperture() const { return type == XT_LIMITRECT || type == XT_LIMITELLIPSE; }
+  bool is_any_aperture() const { return is_aperture() || type == XT_LIMITPOLYGON; }
+};
+
+// number of doubles behind the 8-byte element header (include/xt.h, element table)
+inline int n_params(uint32_t type, uint32_t aux) {
+  switch (type) {
+    case XT_MARKER: return 0;
+    case XT_DRIFT: return 1;
+    case XT_MULTIPOLE: return 2 + 2 * (static_cast<int>(aux) + 1);
+    case XT_CAVITY: return 3;
+    case XT_SROTATION: case XT_XYSHIFT: case XT_LIMITELLIPSE: case XT_QUADRUPOLE: return 2;
+    case XT_LIMITRECT: return 4;
+    case XT_BEND: return 3;
+    case XT_LIMITPOLYGON: return 2 * static_cast<int>(aux);
+    default: return -1;
+  }
+}
+
+struct Line {
+  double p0c = 0, mass0 = 0, q0 = 0;
+  std::vector<Elem> el;
+};
+
+inline bool read_line(const std::vector<unsigned char> &buf, Line &line) {
+  if (buf.size() < 48) return false;
+  uint32_t n_el;
+  std::memcpy(&n_el, buf.data() + 12, 4);
+  std::memcpy(&line.p0c, buf.data() + 16, 8);
+  std::memcpy(&line.mass0, buf.data() + 24, 8);
+  std::memcpy(&line.q0, buf.data() + 32, 8);
+  size_t off = 48;
+  line.el.resize(n_el);
+  for (uint32_t i = 0; i < n_el; ++i) {
+    Elem &e = line.el[i];
+    if (off + 8 > buf.size()) return false;
+    std::memcpy(&e.type, buf.data() + off, 4);
+    std::memcpy(&e.aux, buf.data() + off + 4, 4);
+    off += 8;
+    const int n = n_params(e.type, e.aux);
+    if (n < 0 || off + 8 * static_cast<size_t>(n) > buf.size()) return false;
+    e.v.resize(n);
+    if (n) std::memcpy(e.v.data(), buf.data() + off, 8 * static_cast<size_t>(n));
+    off += 8 * static_cast<size_t>(n);
+  }
+  return true;
+}
+
+}  // namespace xt
