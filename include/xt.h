@@ -217,6 +217,29 @@ int xt_twiss4d(const xt_lattice *lat, double delta0, const double *guess4, xt_tw
 int xt_refine_loss_location(const xt_lattice *lat, const xt_particles *p, int64_t n_part, double ds,
                             int32_t n_poly, int64_t *n_refined, void *cuda_stream);
 
+/* Time functions ("time dependent knobs that are updated automatically
+ * during the simulation", Fig. 1; PAPER.md:80 one parameter controlling groups of elements; DESIGN.md reading
+ * A21 and section 17).  Time advances in turns.  `table` (HOST, row-major [n_knobs][n_steps]) holds the knob
+ * values f_k[step]; a link adds gain * f_knob[step] to knl[order] (skew = 0) or ksl[order] (skew = 1) of the
+ * XT_MULTIPOLE with index `element` in the packed buffer: value = base, then value = value + gain * f for the
+ * links of that coefficient in the order given (product rounded, then the sum); what the packer derives from
+ * the coefficient follows (knl/n!, the curvature fold, the weak-focusing term).  The call copies table and
+ * links to the device and replaces any earlier set; n_links == 0 removes it.  XT_ERR_BAD_LATTICE if a link
+ * does not name a multipole coefficient that exists or a knob of the table. */
+typedef struct {
+  int64_t element;
+  int32_t order, skew, knob, reserved;
+  double gain;
+} xt_knob_link;
+int xt_lattice_set_knobs(xt_lattice *lat, const double *table, int32_t n_knobs, int64_t n_steps,
+                         const xt_knob_link *links, int64_t n_links);
+/* xt_track for n_turns turns with the knobs applied: before turn j (0-based) a small kernel rewrites the linked
+ * coefficients in the device image for step = clamp(step0 + j, 0, n_steps - 1), then the tracking kernel runs
+ * that turn (one launch per turn, stream-ordered, no host synchronisation); afterwards the image is back at
+ * its base values.  While it runs the lattice must not be used by another stream.  No loss compaction. */
+int xt_track_knobs(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
+                   int64_t step0, void *cuda_stream);
+
 /* Number of kernels the library has launched from this process so far (bench bookkeeping). */
 int64_t xt_launch_count(void);
 

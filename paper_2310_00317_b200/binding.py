@@ -43,6 +43,11 @@ class xt_lattice_opts(ctypes.Structure):
     _fields_ = [("chunk_bytes", ctypes.c_int64), ("fuse", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
+class xt_knob_link(ctypes.Structure):
+    _fields_ = [("element", ctypes.c_int64), ("order", ctypes.c_int32), ("skew", ctypes.c_int32),
+                ("knob", ctypes.c_int32), ("reserved", ctypes.c_int32), ("gain", ctypes.c_double)]
+
+
 class xt_twiss4d_result(ctypes.Structure):
     _fields_ = ([("co", ctypes.c_double * 4), ("m", ctypes.c_double * 16)] +
                 [(k, ctypes.c_double) for k in ("betx", "alfx", "mux", "qx_frac", "bety", "alfy", "muy", "qy_frac")] +
@@ -89,6 +94,9 @@ SIGNATURES = {
                                   ctypes.POINTER(xt_twiss4d_result), _VP]),
     "xt_refine_loss_location": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, ctypes.c_double,
                                                ctypes.c_int32, ctypes.POINTER(ctypes.c_int64), _VP]),
+    "xt_lattice_set_knobs": (ctypes.c_int, [_VP, ctypes.POINTER(ctypes.c_double), ctypes.c_int32, _I64,
+                                            ctypes.POINTER(xt_knob_link), _I64]),
+    "xt_track_knobs": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _I64, _VP]),
     "xt_launch_count": (_I64, []),
     "xt_last_error": (ctypes.c_char_p, []),
     "xt_build_info": (ctypes.c_char_p, []),
@@ -361,6 +369,24 @@ def xt_refine_loss_location(lat: Lattice, p: Dict, ds: float, n_poly: int = 64, 
     _check(lat._lib, lat._lib.xt_refine_loss_location(lat.handle, ctypes.byref(st), _n_part(p), float(ds),
                                                       int(n_poly), ctypes.byref(moved), _stream_ptr(stream)))
     return int(moved.value)
+
+
+def xt_lattice_set_knobs(lat: Lattice, table, links) -> None:
+    """``table``: [n_knobs][n_steps] knob values; ``links``: (element, order, skew, knob, gain) tuples (include/xt.h)."""
+    t = np.ascontiguousarray(table, dtype=np.float64)
+    if t.ndim != 2:
+        raise ValueError("table must be 2-D [n_knobs][n_steps]")
+    arr = (xt_knob_link * max(1, len(links)))()
+    for i, (element, order, skew, knob, gain) in enumerate(links):
+        arr[i] = xt_knob_link(int(element), int(order), int(skew), int(knob), 0, float(gain))
+    _check(lat._lib, lat._lib.xt_lattice_set_knobs(lat.handle, t.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
+                                                   t.shape[0], t.shape[1], arr, len(links)))
+
+
+def xt_track_knobs(lat: Lattice, p: Dict, n_turns: int, step0: int = 0, stream=None) -> None:
+    st = _struct_from_tensors(p)
+    _check(lat._lib, lat._lib.xt_track_knobs(lat.handle, ctypes.byref(st), _n_part(p), int(n_turns), int(step0),
+                                             _stream_ptr(stream)))
 
 
 def xt_launch_count(kind: str = "prod") -> int:

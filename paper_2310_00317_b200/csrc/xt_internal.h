@@ -105,6 +105,12 @@ struct xt_lattice {
   std::vector<double> s_table_host;
   std::vector<unsigned char> packed_host;  // the buffer the lattice was created from (xt_refine.cu re-reads it)
   bool extended = false;                   // thick maps or polygon apertures: the THICK kernels
+  std::vector<uint64_t> mult_slot0;        // per element: image offset of a multipole's first coefficient pair
+  // time functions (xt_knobs.cu); all device memory, owned
+  double *d_knob_table = nullptr;
+  void *d_knob_targets = nullptr;
+  void *d_knob_links = nullptr;
+  int64_t n_knob_targets = 0, n_knob_steps = 0;
   unsigned char *d_image = nullptr;
   xt::ChunkDesc *d_chunks = nullptr;
   double *d_s_table = nullptr;
@@ -130,6 +136,7 @@ struct HostImage {
   xt_lattice_info info{};
   RefConsts k{};
   bool extended = false;
+  std::vector<uint64_t> mult_slot0;  // per element: offset of a multipole's first coefficient pair (else ~0)
 };
 struct PackOpts {
   uint32_t chunk_bytes = kDefaultChunkBytes;

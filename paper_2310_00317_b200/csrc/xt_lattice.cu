@@ -120,6 +120,7 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
   out.image.clear();
   out.chunks.clear();
   out.s_table.assign(n_elements, 0.0);
+  out.mult_slot0.assign(n_elements, ~0ull);
 
   // ---- pass 1: one record per element (markers are the identity map: no record)
   std::vector<Rec> recs;
@@ -404,6 +405,7 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
       out.image.resize(at + nb);
       if (!rec.slots.empty())
         std::memcpy(out.image.data() + at + sizeof(RecHdr), rec.slots.data(), rec.slots.size() * sizeof(double));
+      if (rec.type == TAG_MULT || rec.type == TAG_CMULT) out.mult_slot0[rec.elem] = at + sizeof(RecHdr);
       prev_hdr = at;
       prev_elem = rec.elem;
       prev_p0 = rec.p0;
@@ -467,6 +469,7 @@ extern "C" int xt_lattice_create_ex(const void *packed, size_t nbytes, const xt_
   lat->k = img.k;
   lat->s_table_host = img.s_table;
   lat->extended = img.extended;
+  lat->mult_slot0 = img.mult_slot0;
   lat->packed_host.assign(static_cast<const unsigned char *>(packed), static_cast<const unsigned char *>(packed) + nbytes);
 
   auto fail = [&](cudaError_t e, const char *what) {
@@ -502,6 +505,9 @@ extern "C" int xt_lattice_destroy(xt_lattice *lat) {
   if (lat->d_image) cudaFree(lat->d_image);
   if (lat->d_chunks) cudaFree(lat->d_chunks);
   if (lat->d_s_table) cudaFree(lat->d_s_table);
+  if (lat->d_knob_table) cudaFree(lat->d_knob_table);
+  if (lat->d_knob_targets) cudaFree(lat->d_knob_targets);
+  if (lat->d_knob_links) cudaFree(lat->d_knob_links);
   delete lat;
   return XT_OK;
 }

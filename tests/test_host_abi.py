@@ -373,3 +373,5 @@ def test_polygon_aperture_is_packed_unfused_and_refine_rejects_bad_arguments():
     big = pack([LimitPolygon(tuple(float(i) for i in range(256)), tuple(float(i * i) for i in range(256)))])
     assert lib.xt_lattice_pack_host(big, len(big), None, None, 0, None) > 4096
     assert lib.xt_refine_loss_location(None, None, 0, 0.1, 16, None, None) == -1  # NULL lattice: no CUDA call
+    assert lib.xt_lattice_set_knobs(None, None, 1, 1, None, 0) == -1 and lib.xt_track_knobs(None, None, 0, 1, 0, None) == -1
+    assert ctypes.sizeof(X.binding.xt_knob_link) == 32
