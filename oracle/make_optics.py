@@ -25,23 +25,23 @@ from oracle import oracle as O  # noqa: E402
 from xt_inputs import configs as C  # noqa: E402
 
 
-def one_turn(buf, z4):
+def one_turn(buf, z4, delta=0.0):
     co = dict(x=np.array([z4[0]]), px=np.array([z4[1]]), y=np.array([z4[2]]), py=np.array([z4[3]]),
-              zeta=np.zeros(1), delta=np.zeros(1))
+              zeta=np.zeros(1), delta=np.full(1, delta))
     p = O.new_particles(buf, co)
     O.track(buf, p, 1)
     assert p["state"][0] == 1
     return np.array([p["x"][0], p["px"][0], p["y"][0], p["py"][0]])
 
 
-def jac4(buf, z4, h=(1e-6, 1e-8, 1e-6, 1e-8)):
+def jac4(buf, z4, h=(1e-6, 1e-8, 1e-6, 1e-8), delta=0.0):
     n = 8
     pts = np.tile(np.asarray(z4, dtype=np.float64), (n, 1))
     for i in range(4):
         pts[2 * i, i] += h[i]
         pts[2 * i + 1, i] -= h[i]
     co = dict(x=pts[:, 0].copy(), px=pts[:, 1].copy(), y=pts[:, 2].copy(), py=pts[:, 3].copy(),
-              zeta=np.zeros(n), delta=np.zeros(n))
+              zeta=np.zeros(n), delta=np.full(n, delta))
     p = O.new_particles(buf, co)
     O.track(buf, p, 1)
     assert np.all(p["state"] == 1)
@@ -52,16 +52,16 @@ def jac4(buf, z4, h=(1e-6, 1e-8, 1e-6, 1e-8)):
     return J
 
 
-def optics_of(buf):
-    z = np.zeros(4)
+def optics_of(buf, delta=0.0, guess=None):
+    z = np.zeros(4) if guess is None else np.asarray(guess, dtype=np.float64).copy()
     for _ in range(12):                                   # Twiss step 1: closed orbit
-        J = jac4(buf, z)
-        r = one_turn(buf, z) - z
+        J = jac4(buf, z, delta=delta)
+        r = one_turn(buf, z, delta) - z
         dz = np.linalg.solve(J - np.eye(4), -r)
         z = z + dz
         if np.max(np.abs(dz)) < 1e-13:
             break
-    J = jac4(buf, z)                                      # Twiss step 2
+    J = jac4(buf, z, delta=delta)                         # Twiss step 2
     out = {"x_co": z[0], "px_co": z[1], "y_co": z[2], "py_co": z[3]}
     for name, i in (("x", 0), ("y", 2)):                  # Twiss step 3 (uncoupled)
         m = J[i:i + 2, i:i + 2]
@@ -72,6 +72,23 @@ def optics_of(buf):
         out["alf" + name] = (m[0, 0] - m[1, 1]) / (2.0 * sinmu)
         mu = math.atan2(sinmu, cosmu)
         out["q" + name + "_frac"] = (mu / (2 * math.pi)) % 1.0
+    return out
+
+
+def chromatic_optics_of(buf, ddelta=1e-4, delta=0.0):
+    """Dispersion and chromaticity at the start of the line (the optics "as a function of the
+    momentum"): central differences in delta of the closed orbit and of the tunes, each from the three steps
+    above at delta -+ ddelta."""
+    on = optics_of(buf, delta)
+    z0 = [on["x_co"], on["px_co"], on["y_co"], on["py_co"]]
+    hi, lo = optics_of(buf, delta + ddelta, z0), optics_of(buf, delta - ddelta, z0)
+    out = dict(on)
+    for name, key in (("dx", "x_co"), ("dpx", "px_co"), ("dy", "y_co"), ("dpy", "py_co")):
+        out[name] = (hi[key] - lo[key]) / (2.0 * ddelta)
+    for name, key in (("dqx", "qx_frac"), ("dqy", "qy_frac")):
+        d = hi[key] - lo[key]
+        d -= round(d)                                      # fractional tunes: the difference is taken on the circle
+        out[name] = d / (2.0 * ddelta)
     return out
 
 

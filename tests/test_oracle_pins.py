@@ -619,3 +619,39 @@ def test_P14_thick_bend_rejects_degenerate_parameters():
         with pytest.raises(ValueError):
             O.reference(pack([bad]))
     assert abs(O.s_table(pack([Bend(1e-3, 1e-3, 2.5), Drift(1.0), Marker()]))[2] - 3.5) < 1e-15
+
+
+# ----------------------------- P18 dispersion and chromaticity from tracking
+def test_P18_fodo_chromaticity_and_textbook_dispersion():
+    """oracle/make_optics.chromatic_optics_of against (a) the natural chromaticity of the thin-lens FODO
+    cell, d mu/d delta = -2 tan(mu/2) (every focal length scales as 1 + delta), and (b) the periodic
+    dispersion of a ring of thin quadrupoles and thin sector dipoles from 3x3 (x, px, delta) matrices."""
+    from oracle import make_optics as MO
+    n_cells, L, kq = 10, 2.0, 0.1
+    cell = [Multipole(knl=(0.0, kq)), Drift(L), Multipole(knl=(0.0, -kq)), Drift(L)]
+    got = MO.chromatic_optics_of(pack(cell * n_cells))
+    mu = math.acos(1.0 - (L * kq) ** 2 / 2.0)
+    want = -n_cells * math.tan(mu / 2.0) / math.pi
+    assert abs(got["dqx"] - want) < 2e-6 * abs(want) and abs(got["dqy"] - want) < 2e-6 * abs(want)
+    assert max(abs(got[k]) for k in ("dx", "dpx", "dy", "dpy")) < 1e-9                # no bends: no dispersion
+
+    n_cells, L, kq, ell = 8, 3.0, 0.25, 1.5
+    th = 2.0 * math.pi / (2 * n_cells)                                               # two dipoles per cell close the ring
+    bend = Multipole(knl=(th,), hxl=th, length=ell)
+    cell = [Multipole(knl=(0.0, kq)), Drift(L), bend, Drift(L), Multipole(knl=(0.0, -kq)), Drift(L), bend, Drift(L)]
+    got = MO.chromatic_optics_of(pack(cell * n_cells))
+
+    def quad(k):
+        return np.array([[1.0, 0.0, 0.0], [-k, 1.0, 0.0], [0.0, 0.0, 1.0]])
+    drift = np.array([[1.0, L, 0.0], [0.0, 1.0, 0.0], [0.0, 0.0, 1.0]])
+    dip = np.array([[1.0, 0.0, 0.0], [-th * th / ell, 1.0, th], [0.0, 0.0, 1.0]])    # px' = px + th delta - (k0 h l) x
+    m = np.eye(3)
+    for e in (quad(kq), drift, dip, drift, quad(-kq), drift, dip, drift):
+        m = e @ m
+    d = np.linalg.solve(np.eye(2) - m[:2, :2], m[:2, 2])
+    assert abs(d[0]) > 1.0
+    assert abs(got["dx"] - d[0]) < 1e-6 * abs(d[0]) and abs(got["dpx"] - d[1]) < 1e-6 * max(abs(d[1]), 0.1)
+    assert abs(got["dy"]) < 1e-9 and abs(got["x_co"]) < 1e-12
+    cosmu = 0.5 * (m[0, 0] + m[1, 1])
+    q_cell = math.acos(cosmu) / (2 * math.pi)
+    assert abs(got["qx_frac"] - (n_cells * q_cell) % 1.0) < 1e-8
