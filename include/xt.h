@@ -240,6 +240,19 @@ int xt_lattice_set_knobs(xt_lattice *lat, const double *table, int32_t n_knobs, 
 int xt_track_knobs(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
                    int64_t step0, void *cuda_stream);
 
+/* Dispersion and chromaticity at the start of the line ("tunes, beta, alpha,
+ * dispersion"): xt_twiss4d at delta0 and at delta0 -+ ddelta (ddelta > 0, e.g. 1e-4; the
+ * off-momentum searches start from the on-momentum orbit); dispersion = central difference of the closed
+ * orbit, chromaticity = central difference of the fractional tunes taken on the circle.  Errors as
+ * xt_twiss4d; NaN chromaticity in a plane that is unstable at any of the three momenta. */
+typedef struct {
+  xt_twiss4d_result on;    /* at delta0                                                       */
+  double dx, dpx, dy, dpy; /* d(closed orbit)/d(delta)                                        */
+  double dqx, dqy;         /* d(tune)/d(delta)                                                */
+} xt_twiss4d_chrom_result;
+int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
+                     xt_twiss4d_chrom_result *out, void *cuda_stream);
+
 /* Number of kernels the library has launched from this process so far (bench bookkeeping). */
 int64_t xt_launch_count(void);
 

@@ -54,6 +54,11 @@ class xt_twiss4d_result(ctypes.Structure):
                 [("iterations", ctypes.c_int32), ("stable", ctypes.c_int32)])
 
 
+class xt_twiss4d_chrom_result(ctypes.Structure):
+    _fields_ = ([("on", xt_twiss4d_result)] +
+                [(k, ctypes.c_double) for k in ("dx", "dpx", "dy", "dpy", "dqx", "dqy")])
+
+
 class xt_lattice_info(ctypes.Structure):
     _fields_ = [("n_elements", ctypes.c_int64), ("n_records", ctypes.c_int64),
                 ("n_chunks", ctypes.c_int64), ("image_bytes", ctypes.c_int64),
@@ -94,6 +99,8 @@ SIGNATURES = {
                                   ctypes.POINTER(xt_twiss4d_result), _VP]),
     "xt_refine_loss_location": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, ctypes.c_double,
                                                ctypes.c_int32, ctypes.POINTER(ctypes.c_int64), _VP]),
+    "xt_twiss4d_chrom": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
+                                        ctypes.POINTER(xt_twiss4d_chrom_result), _VP]),
     "xt_lattice_set_knobs": (ctypes.c_int, [_VP, ctypes.POINTER(ctypes.c_double), ctypes.c_int32, _I64,
                                             ctypes.POINTER(xt_knob_link), _I64]),
     "xt_track_knobs": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _I64, _VP]),
@@ -369,6 +376,26 @@ def xt_refine_loss_location(lat: Lattice, p: Dict, ds: float, n_poly: int = 64, 
     _check(lat._lib, lat._lib.xt_refine_loss_location(lat.handle, ctypes.byref(st), _n_part(p), float(ds),
                                                       int(n_poly), ctypes.byref(moved), _stream_ptr(stream)))
     return int(moved.value)
+
+
+def _twiss_dict(res) -> Dict:
+    out = {k: getattr(res, k) for k in ("betx", "alfx", "mux", "qx_frac", "bety", "alfy", "muy", "qy_frac",
+                                        "iterations", "stable")}
+    out["co"] = np.array(list(res.co))
+    out["m"] = np.array(list(res.m)).reshape(4, 4)
+    return out
+
+
+def xt_twiss4d_chrom(lat: Lattice, delta0: float = 0.0, ddelta: float = 1e-4, guess4=None, stream=None) -> Dict:
+    """xt_twiss4d plus dispersion (dx, dpx, dy, dpy) and chromaticity (dqx, dqy); see include/xt.h."""
+    res = xt_twiss4d_chrom_result()
+    g = (ctypes.c_double * 4)(*[float(v) for v in guess4]) if guess4 is not None else None
+    _check(lat._lib, lat._lib.xt_twiss4d_chrom(lat.handle, float(delta0), float(ddelta), g, ctypes.byref(res),
+                                               _stream_ptr(stream)))
+    out = _twiss_dict(res.on)
+    for k in ("dx", "dpx", "dy", "dpy", "dqx", "dqy"):
+        out[k] = getattr(res, k)
+    return out
 
 
 def xt_lattice_set_knobs(lat: Lattice, table, links) -> None:

@@ -192,3 +192,29 @@ extern "C" int xt_twiss4d(const xt_lattice *lat, double delta0, const double *gu
   *out = res;
   return done(XT_OK);
 }
+
+extern "C" int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
+                                xt_twiss4d_chrom_result *out, void *cuda_stream) {
+  using namespace xt;
+  if (!out || !(ddelta > 0.0) || !std::isfinite(ddelta)) {
+    set_error("xt_twiss4d_chrom: NULL result or ddelta not > 0");
+    return XT_ERR_INVALID_ARG;
+  }
+  xt_twiss4d_chrom_result res{};
+  xt_twiss4d_result hi{}, lo{};
+  int rc = xt_twiss4d(lat, delta0, guess4, &res.on, cuda_stream);
+  if (rc == XT_OK) rc = xt_twiss4d(lat, delta0 + ddelta, res.on.co, &hi, cuda_stream);
+  if (rc == XT_OK) rc = xt_twiss4d(lat, delta0 - ddelta, res.on.co, &lo, cuda_stream);
+  if (rc != XT_OK) return rc;
+  double *d[4] = {&res.dx, &res.dpx, &res.dy, &res.dpy};
+  for (int c = 0; c < 4; ++c) *d[c] = (hi.co[c] - lo.co[c]) / (2.0 * ddelta);
+  auto slope = [&](double a, double b) {
+    double diff = a - b;
+    diff -= std::nearbyint(diff);  // fractional tunes live on a circle
+    return diff / (2.0 * ddelta);  // NaN in, NaN out
+  };
+  res.dqx = slope(hi.qx_frac, lo.qx_frac);
+  res.dqy = slope(hi.qy_frac, lo.qy_frac);
+  *out = res;
+  return XT_OK;
+}

@@ -91,3 +91,47 @@ def test_twiss_off_momentum_and_errors(X):
     tw = X.xt_twiss4d(lat)
     assert tw["stable"] == 0 and (math.isnan(tw["bety"]) or math.isnan(tw["betx"]))
     lat.close()
+
+
+def test_dispersion_and_chromaticity(X):
+    """xt_twiss4d_chrom against closed forms (pin P18: thin-FODO natural chromaticity; periodic dispersion of a
+    ring of thin quadrupoles and thin sector dipoles from 3x3 matrices) and against the oracle procedure
+    on the LHC-sized ring."""
+    n_cells, L, kq = 10, 2.0, 0.1
+    cell = [Multipole(knl=(0.0, kq)), Drift(L), Multipole(knl=(0.0, -kq)), Drift(L)]
+    lat = X.xt_lattice_create(pack_lattice(cell * n_cells, P0C, MASS0, 1.0))
+    tw = X.xt_twiss4d_chrom(lat)
+    lat.close()
+    mu = math.acos(1.0 - (L * kq) ** 2 / 2.0)
+    want = -n_cells * math.tan(mu / 2.0) / math.pi
+    assert abs(tw["dqx"] - want) < 1e-5 * abs(want) and abs(tw["dqy"] - want) < 1e-5 * abs(want)
+    assert max(abs(tw[k]) for k in ("dx", "dpx", "dy", "dpy")) < 1e-9
+
+    n_cells, L, kq, ell = 8, 3.0, 0.25, 1.5
+    th = 2.0 * math.pi / (2 * n_cells)
+    bend = Multipole(knl=(th,), hxl=th, length=ell)
+    cell = [Multipole(knl=(0.0, kq)), Drift(L), bend, Drift(L), Multipole(knl=(0.0, -kq)), Drift(L), bend, Drift(L)]
+    lat = X.xt_lattice_create(pack_lattice(cell * n_cells, P0C, MASS0, 1.0))
+    tw = X.xt_twiss4d_chrom(lat, 0.0, 1e-4)
+    lat.close()
+    quad = lambda k: np.array([[1.0, 0.0, 0.0], [-k, 1.0, 0.0], [0.0, 0.0, 1.0]])
+    drift = np.array([[1.0, L, 0.0], [0.0, 1.0, 0.0], [0.0, 0.0, 1.0]])
+    dip = np.array([[1.0, 0.0, 0.0], [-th * th / ell, 1.0, th], [0.0, 0.0, 1.0]])
+    m = np.eye(3)
+    for e in (quad(kq), drift, dip, drift, quad(-kq), drift, dip, drift):
+        m = e @ m
+    d = np.linalg.solve(np.eye(2) - m[:2, :2], m[:2, 2])
+    assert abs(tw["dx"] - d[0]) < 1e-6 * abs(d[0]) and abs(tw["dpx"] - d[1]) < 1e-6 * max(abs(d[1]), 0.1)
+    assert abs(tw["dy"]) < 1e-9
+
+    buf = C.pack(C.lattice(2))
+    want = MO.chromatic_optics_of(buf, 1e-4)
+    lat = X.xt_lattice_create(buf)
+    tw = X.xt_twiss4d_chrom(lat, 0.0, 1e-4)
+    assert abs(tw["dx"] - want["dx"]) < 1e-6 * max(abs(want["dx"]), 1.0) and abs(tw["dpx"] - want["dpx"]) < 1e-7
+    assert abs(tw["dy"] - want["dy"]) < 1e-6 and abs(tw["dqx"] - want["dqx"]) < 2e-4 * max(abs(want["dqx"]), 1.0)
+    assert abs(tw["dqy"] - want["dqy"]) < 2e-4 * max(abs(want["dqy"]), 1.0) and abs(tw["betx"] / want["betx"] - 1) < 1e-7
+    with pytest.raises(X.XtError) as e:
+        X.xt_twiss4d_chrom(lat, 0.0, 0.0)
+    assert e.value.code == -1
+    lat.close()
