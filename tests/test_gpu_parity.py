@@ -607,3 +607,56 @@ def test_random_lattices_bit_exact_nofma(X, seed):
             else:
                 clear = assert_losses_match(got, ref, mm)
                 assert_close(got, ref, 1e-12, sel=clear & (ref["state"] == 1))
+
+
+def _random_polygon(rng):
+    n = int(rng.choice([3, 4, 5, 8, 17, 60]))
+    ang = 2 * np.pi * (np.arange(n) + rng.uniform(-0.3, 0.3, n) * (rng.random() < 0.5)) / n   # around the beam
+    r = rng.uniform(0.006, 0.03) * (1.0 - 0.4 * rng.random(n) * (rng.random() < 0.5))     # convex-ish or star-shaped
+    cx, cy = rng.normal(0, 5e-4, 2)
+    from xt_inputs.packed import LimitPolygon
+    return LimitPolygon(tuple(cx + r * np.cos(ang)), tuple(cy + r * np.sin(ang)))
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_random_lattices_with_extended_elements(X, seed):
+    """The fuzz above with the elements of the widened set mixed in: polygon apertures (even seeds: still
+    bit-exact in the --fmad=false build) and, on odd seeds, thick quadrupoles and sector bends (sincos / cosh
+    differ from glibc by an ulp or two: 1-turn tolerance in both builds)."""
+    from xt_inputs.packed import Bend, Quadrupole
+    rng = np.random.default_rng(5000 + seed)
+    els = _random_line(rng, int(rng.integers(30, 120)))
+    thick = seed % 2 == 1
+    for _ in range(int(rng.integers(3, 9))):
+        at = int(rng.integers(0, len(els) + 1))
+        r = rng.random()
+        if not thick or r < 0.4:
+            els.insert(at, _random_polygon(rng))
+        elif r < 0.7:
+            els.insert(at, Quadrupole(float(rng.choice([-1.0, 1.0]) * rng.uniform(0.01, 0.3)), float(rng.uniform(0.2, 3.0))))
+        else:
+            h = float(rng.choice([-1.0, 1.0]) * rng.uniform(1e-3, 2e-2))
+            els.insert(at, Bend(h * (1.0 + float(rng.normal(0, 1e-4))), h, float(rng.uniform(0.5, 6.0))))
+    buf = pack_lattice(els, H.P0C, H.MASS0, H.Q0)
+    n = int(rng.integers(40, 700))
+    amp = float(rng.choice([0.2, 0.5, 1.0]))
+    co = dict(x=rng.normal(0, 1.5e-3 * amp, n), px=rng.normal(0, 1e-4 * amp, n), y=rng.normal(0, 1.5e-3 * amp, n),
+              py=rng.normal(0, 1e-4 * amp, n), zeta=rng.normal(0, 0.05, n), delta=rng.normal(0, 5e-4, n))
+    turns = int(rng.integers(1, 4))
+    ref = O.new_particles(buf, co)
+    mm = np.full(n, np.inf)
+    O.track(buf, ref, turns, min_margin=mm)
+    for kind in ("nofma", "prod"):
+        for trial in range(3):
+            kw = dict(chunk_bytes=int(rng.choice([2048, 8192, 65536])), fuse=bool(rng.random() < 0.7))
+            lat = X.xt_lattice_create_ex(buf, kind=kind, **kw)
+            p = X.new_particles(lat, co)
+            X.xt_track_ex(lat, p, turns, particles_per_thread=int(rng.choice([0, 1, 2, 3, 4])),
+                          block_size=int(rng.choice([0, 32, 64, 128, 256])), compact_every=int(rng.choice([-1, 1, 2])))
+            got = X.particles_to_host(p)
+            lat.close()
+            if kind == "nofma" and not thick:
+                assert_bit_identical(got, ref)
+            else:
+                clear = assert_losses_match(got, ref, mm)
+                assert_close(got, ref, 1e-12, sel=clear & (ref["state"] == 1))
