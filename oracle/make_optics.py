@@ -92,6 +92,57 @@ def chromatic_optics_of(buf, ddelta=1e-4, delta=0.0):
     return out
 
 
+def optics_along(elements, p0c, mass0, q0, rows, ddelta=1e-4, delta=0.0):
+    """Twiss along the line (the optics is propagated from the start "to all other elements
+    by tracking"; beta functions along the ring).  For every requested row i (the ENTRANCE of
+    element i; i = len(elements) is the end of the line): the closed orbit, the 4x4 Jacobian J_i of the map
+    from the start to row i by central differences around the closed orbit (same steps as ``jac4``), then per
+    plane with m = the plane's 2x2 block of J_i and (beta0, alpha0, gamma0) at the start:
+        beta_i  = m11^2 beta0 - 2 m11 m12 alpha0 + m12^2 gamma0
+        alpha_i = -m11 m21 beta0 + (m11 m22 + m12 m21) alpha0 - m12 m22 gamma0
+        mu_i    = atan2(m12, m11 beta0 - m12 alpha0)   (mod 2 pi; the caller unwraps)
+    and the dispersion as the central difference of the closed orbits at delta -+ ddelta tracked to row i.
+    Each row is tracked through its own prefix line elements[:i] -- slow and obviously element i's entrance."""
+    from xt_inputs import packed as PK
+    buf = PK.pack_lattice(elements, p0c, mass0, q0)
+    on = optics_of(buf, delta)
+    z0 = np.array([on["x_co"], on["px_co"], on["y_co"], on["py_co"]])
+    hi, lo = optics_of(buf, delta + ddelta, z0), optics_of(buf, delta - ddelta, z0)
+    zh = np.array([hi["x_co"], hi["px_co"], hi["y_co"], hi["py_co"]])
+    zl = np.array([lo["x_co"], lo["px_co"], lo["y_co"], lo["py_co"]])
+    h = (1e-6, 1e-8, 1e-6, 1e-8)
+    pts = np.tile(z0, (11, 1))
+    for i in range(4):
+        pts[1 + 2 * i, i] += h[i]
+        pts[2 + 2 * i, i] -= h[i]
+    pts[9], pts[10] = zh, zl
+    deltas = np.full(11, delta)
+    deltas[9], deltas[10] = delta + ddelta, delta - ddelta
+    out = []
+    for row in rows:
+        prefix = PK.pack_lattice(list(elements[:row]) or [PK.Marker()], p0c, mass0, q0)
+        p = O.new_particles(prefix, dict(x=pts[:, 0].copy(), px=pts[:, 1].copy(), y=pts[:, 2].copy(),
+                                         py=pts[:, 3].copy(), zeta=np.zeros(11), delta=deltas.copy()))
+        O.track(prefix, p, 1)
+        assert np.all(p["state"] == 1)
+        z = np.stack([p["x"], p["px"], p["y"], p["py"]], axis=1)
+        J = np.zeros((4, 4))
+        for i in range(4):
+            J[:, i] = (z[1 + 2 * i] - z[2 + 2 * i]) / (2 * h[i])
+        r = {"x": z[0, 0], "px": z[0, 1], "y": z[0, 2], "py": z[0, 3]}
+        for name, i in (("x", 0), ("y", 2)):
+            m = J[i:i + 2, i:i + 2]
+            b0, a0 = on["bet" + name], on["alf" + name]
+            g0 = (1.0 + a0 * a0) / b0
+            r["bet" + name] = m[0, 0] ** 2 * b0 - 2.0 * m[0, 0] * m[0, 1] * a0 + m[0, 1] ** 2 * g0
+            r["alf" + name] = -m[0, 0] * m[1, 0] * b0 + (m[0, 0] * m[1, 1] + m[0, 1] * m[1, 0]) * a0 - m[0, 1] * m[1, 1] * g0
+            r["mu" + name] = math.atan2(m[0, 1], m[0, 0] * b0 - m[0, 1] * a0) % (2 * math.pi)
+        d = (z[9] - z[10]) / (2.0 * ddelta)
+        r["dx"], r["dpx"], r["dy"], r["dpy"] = d
+        out.append(r)
+    return on, out
+
+
 def main():
     res = {"_about": "written by oracle/make_optics.py (oracle one-turn Jacobian at the 4-D closed "
                      "orbit, PAPER.md:96-98); input shaping only"}

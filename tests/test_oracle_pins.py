@@ -655,3 +655,53 @@ def test_P18_fodo_chromaticity_and_textbook_dispersion():
     cosmu = 0.5 * (m[0, 0] + m[1, 1])
     q_cell = math.acos(cosmu) / (2 * math.pi)
     assert abs(got["qx_frac"] - (n_cells * q_cell) % 1.0) < 1e-8
+
+
+# ----------------------------- P19 optics along the line
+def test_P19_optics_along_a_fodo_ring_and_a_ring_with_dipoles():
+    """oracle/make_optics.optics_along against the thin-FODO textbook: beta = 2L(1 +- sin(mu/2))/sin(mu) in the
+    quadrupoles (L = half cell), alpha = -+ beta k/2 at their entrances, beta(s) = beta - 2 alpha s + gamma s^2
+    in a drift, the phase grows by mu per cell; and the dispersion propagated by 3x3 matrices (P18's ring)."""
+    from oracle import make_optics as MO
+    n_cells, L, kq = 10, 2.0, 0.1
+    cell = [Multipole(knl=(0.0, kq)), Drift(L / 2), Marker(), Drift(L / 2), Multipole(knl=(0.0, -kq)), Drift(L)]
+    els = cell * n_cells
+    on, rows = MO.optics_along(els, H.P0C, H.MASS0, H.Q0, list(range(len(els) + 1)))
+    mu = math.acos(1.0 - (L * kq) ** 2 / 2.0)
+    bmax, bmin = 2 * L * (1 + math.sin(mu / 2)) / math.sin(mu), 2 * L * (1 - math.sin(mu / 2)) / math.sin(mu)
+    for c in range(n_cells):
+        qf, mid, qd = rows[6 * c], rows[6 * c + 2], rows[6 * c + 4]
+        assert abs(qf["betx"] - bmax) < 1e-6 and abs(qf["bety"] - bmin) < 1e-6
+        assert abs(qd["betx"] - bmin) < 1e-6 and abs(qd["bety"] - bmax) < 1e-6
+        assert abs(qf["alfx"] + bmax * kq / 2) < 1e-7 and abs(qd["alfx"] - bmin * kq / 2) < 1e-7
+        assert abs(qf["alfy"] - bmin * kq / 2) < 1e-7 and abs(qd["alfy"] + bmax * kq / 2) < 1e-7
+        # behind the thin QF: alpha = +beta k/2; half a drift further
+        a1, g1 = bmax * kq / 2, (1 + (bmax * kq / 2) ** 2) / bmax
+        assert abs(mid["betx"] - (bmax - 2 * a1 * (L / 2) + g1 * (L / 2) ** 2)) < 1e-6
+        assert abs(mid["alfx"] - (a1 - g1 * (L / 2))) < 1e-7
+        assert abs((qf["mux"] - c * mu + 1e-9) % (2 * math.pi) - 1e-9) < 1e-7 and abs((qf["muy"] - c * mu + 1e-9) % (2 * math.pi) - 1e-9) < 1e-7
+        assert rows[6 * c + 2] is mid and abs(rows[6 * c + 3]["betx"] - mid["betx"]) < 1e-12     # a marker changes nothing
+    end = rows[-1]
+    assert abs(end["betx"] - on["betx"]) < 1e-6 and abs(end["alfx"] - on["alfx"]) < 1e-7        # periodic
+    assert abs((end["mux"] - n_cells * mu) % (2 * math.pi)) < 1e-7 or abs((end["mux"] - n_cells * mu) % (2 * math.pi) - 2 * math.pi) < 1e-7
+
+    n_cells, L, kq, ell = 8, 3.0, 0.25, 1.5
+    th = 2.0 * math.pi / (2 * n_cells)
+    bend = Multipole(knl=(th,), hxl=th, length=ell)
+    cell = [Multipole(knl=(0.0, kq)), Drift(L), bend, Drift(L), Multipole(knl=(0.0, -kq)), Drift(L), bend, Drift(L)]
+    els = cell * n_cells
+    on, rows = MO.optics_along(els, H.P0C, H.MASS0, H.Q0, list(range(9)) + [len(els)])
+    quad = lambda k: np.array([[1.0, 0.0, 0.0], [-k, 1.0, 0.0], [0.0, 0.0, 1.0]])
+    drift = np.array([[1.0, L, 0.0], [0.0, 1.0, 0.0], [0.0, 0.0, 1.0]])
+    dip = np.array([[1.0, 0.0, 0.0], [-th * th / ell, 1.0, th], [0.0, 0.0, 1.0]])
+    mats = [quad(kq), drift, dip, drift, quad(-kq), drift, dip, drift]
+    m = np.eye(3)
+    for e in mats:
+        m = e @ m
+    d = np.append(np.linalg.solve(np.eye(2) - m[:2, :2], m[:2, 2]), 1.0)
+    for i in range(9):
+        assert abs(rows[i]["dx"] - d[0]) < 1e-6 * max(abs(d[0]), 1.0) and abs(rows[i]["dpx"] - d[1]) < 1e-6, i
+        assert abs(rows[i]["x"]) < 1e-12 and abs(rows[i]["dy"]) < 1e-9
+        if i < 8:
+            d = mats[i] @ d
+    assert abs(rows[-1]["dx"] - rows[0]["dx"]) < 1e-6
