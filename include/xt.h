@@ -253,6 +253,25 @@ typedef struct {
 int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
                      xt_twiss4d_chrom_result *out, void *cuda_stream);
 
+/* Optics along the line (the optics found at the start is carried
+ * "to all other elements by tracking"; beta functions along the ring).  After the three closed-orbit
+ * searches of xt_twiss4d_chrom, ONE launch tracks eleven probe particles (the orbit, +-h along x, px, y, py,
+ * and the closed orbits at delta0 -+ ddelta) through the line with an internal monitor record in front of
+ * every element; from the rows the host forms, per element entrance, the closed orbit, the 4x4 Jacobian
+ * J_i from the start by central differences, per plane beta_i = m11^2 b0 - 2 m11 m12 a0 + m12^2 g0,
+ * alpha_i = -m11 m21 b0 + (m11 m22 + m12 m21) a0 - m12 m22 g0, mu_i = atan2(m12, m11 b0 - m12 a0) unwrapped
+ * along the line (mux of the last row / 2 pi is the tune WITH its integer part), and the dispersion as the
+ * central difference of the two off-momentum orbits.  rows: HOST array of cap >= n_elements + 1 entries;
+ * row i is the entrance of element i, row n_elements the end of the line.  start may be NULL.  Errors as
+ * xt_twiss4d (XT_ERR_UNSTABLE also if a probe is lost on the way or a plane is unstable). */
+typedef struct {
+  double s, x, px, y, py;
+  double betx, alfx, mux, bety, alfy, muy;
+  double dx, dpx, dy, dpy;
+} xt_twiss_row;
+int xt_twiss4d_line(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
+                    xt_twiss4d_chrom_result *start, xt_twiss_row *rows, int64_t cap, void *cuda_stream);
+
 /* Number of kernels the library has launched from this process so far (bench bookkeeping). */
 int64_t xt_launch_count(void);
 

@@ -59,6 +59,11 @@ class xt_twiss4d_chrom_result(ctypes.Structure):
                 [(k, ctypes.c_double) for k in ("dx", "dpx", "dy", "dpy", "dqx", "dqy")])
 
 
+class xt_twiss_row(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_double) for k in ("s", "x", "px", "y", "py", "betx", "alfx", "mux", "bety", "alfy",
+                                                "muy", "dx", "dpx", "dy", "dpy")]
+
+
 class xt_lattice_info(ctypes.Structure):
     _fields_ = [("n_elements", ctypes.c_int64), ("n_records", ctypes.c_int64),
                 ("n_chunks", ctypes.c_int64), ("image_bytes", ctypes.c_int64),
@@ -101,6 +106,9 @@ SIGNATURES = {
                                                ctypes.c_int32, ctypes.POINTER(ctypes.c_int64), _VP]),
     "xt_twiss4d_chrom": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
                                         ctypes.POINTER(xt_twiss4d_chrom_result), _VP]),
+    "xt_twiss4d_line": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
+                                       ctypes.POINTER(xt_twiss4d_chrom_result), ctypes.POINTER(xt_twiss_row), _I64,
+                                       _VP]),
     "xt_lattice_set_knobs": (ctypes.c_int, [_VP, ctypes.POINTER(ctypes.c_double), ctypes.c_int32, _I64,
                                             ctypes.POINTER(xt_knob_link), _I64]),
     "xt_track_knobs": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _I64, _VP]),
@@ -396,6 +404,21 @@ def xt_twiss4d_chrom(lat: Lattice, delta0: float = 0.0, ddelta: float = 1e-4, gu
     for k in ("dx", "dpx", "dy", "dpy", "dqx", "dqy"):
         out[k] = getattr(res, k)
     return out
+
+
+def xt_twiss4d_line(lat: Lattice, delta0: float = 0.0, ddelta: float = 1e-4, guess4=None, stream=None):
+    """Optics along the line: (start dict as xt_twiss4d_chrom, rows dict of arrays of n_elements + 1); include/xt.h."""
+    n = int(lat.info["n_elements"]) + 1
+    rows = (xt_twiss_row * n)()
+    res = xt_twiss4d_chrom_result()
+    g = (ctypes.c_double * 4)(*[float(v) for v in guess4]) if guess4 is not None else None
+    _check(lat._lib, lat._lib.xt_twiss4d_line(lat.handle, float(delta0), float(ddelta), g, ctypes.byref(res), rows, n,
+                                              _stream_ptr(stream)))
+    start = _twiss_dict(res.on)
+    for k in ("dx", "dpx", "dy", "dpy", "dqx", "dqy"):
+        start[k] = getattr(res, k)
+    arr = np.frombuffer(rows, dtype=np.float64).reshape(n, 15).copy()
+    return start, {k: arr[:, i] for i, (k, _) in enumerate(xt_twiss_row._fields_)}
 
 
 def xt_lattice_set_knobs(lat: Lattice, table, links) -> None:

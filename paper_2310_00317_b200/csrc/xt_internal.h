@@ -64,6 +64,7 @@ enum : uint32_t {
   TAG_QUAD = 9,
   TAG_BEND = 10,
   TAG_POLY = 11,
+  TAG_MON = 12,  // internal: store the coordinates of every alive particle into row p0 of the monitor buffer
   TAG_TYPE_MASK = 0xf,
   TAG_PRE = 0x10,   // a drift of length l_pre comes first
   TAG_POST = 0x20,  // a drift of length l_post follows the kick
@@ -141,10 +142,16 @@ struct HostImage {
 struct PackOpts {
   uint32_t chunk_bytes = kDefaultChunkBytes;
   bool fuse = true;
+  bool allow_monitor = false;  // accept the internal element type kMonitorType (xt_twiss4d_line builds such lines)
 };
+constexpr uint32_t kMonitorType = 11;  // packed-buffer type id, internal: {row} -> TAG_MON record
+int create_lattice(const void *packed, size_t nbytes, const PackOpts &po, xt_lattice **out);
 int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImage &out);
 
 // xt_track.cu
+// Where TAG_MON records store: rows of n_part x 6 doubles (x, px, y, py, zeta, delta).  One buffer per
+// process and library at a time (a __constant__ pointer), set stream-ordered before the launch that uses it.
+int set_monitor_base(double *d_rows, cudaStream_t st);
 // block: threads per CTA; ppt: particles per thread (1, 2 or 4; 4 needs block <= 256)
 int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part,
                  const int64_t *d_n_active, int64_t n_turns, int block, int ppt, cudaStream_t st);

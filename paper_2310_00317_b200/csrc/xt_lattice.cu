@@ -268,6 +268,16 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
         out.extended = true;
         break;
       }
+      case kMonitorType: {
+        if (!opts.allow_monitor) {
+          set_error("xt_lattice_create: unknown element type id");
+          return XT_ERR_BAD_LATTICE;
+        }
+        rec.type = TAG_MON;
+        rec.p0 = r.real();  // row
+        out.extended = true;
+        break;
+      }
       default:
         set_error("xt_lattice_create: unknown element type id");
         return XT_ERR_BAD_LATTICE;
@@ -454,10 +464,14 @@ extern "C" int xt_lattice_create_ex(const void *packed, size_t nbytes, const xt_
     return XT_ERR_INVALID_ARG;
   }
   xt::PackOpts po;
-  int rc = xt::resolve_pack_opts(opts, po);
+  const int rc = xt::resolve_pack_opts(opts, po);
   if (rc != XT_OK) return rc;
+  return xt::create_lattice(packed, nbytes, po, out);
+}
+
+int xt::create_lattice(const void *packed, size_t nbytes, const PackOpts &po, xt_lattice **out) {
   xt::HostImage img;
-  rc = xt::pack_image(packed, nbytes, po, img);
+  int rc = xt::pack_image(packed, nbytes, po, img);
   if (rc != XT_OK) return rc;
 
   xt_lattice *lat = new (std::nothrow) xt_lattice;

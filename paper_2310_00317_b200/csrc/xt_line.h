@@ -67,4 +67,33 @@ inline bool read_line(const std::vector<unsigned char> &buf, Line &line) {
   return true;
 }
 
+// A packed lattice buffer (include/xt.h) under construction.
+struct Writer {
+  std::vector<unsigned char> b;
+  uint32_t n = 0;
+  explicit Writer(const Line &l) : b(48, 0) {
+    std::memcpy(b.data(), "XTLAT001", 8);
+    const uint32_t version = 1;
+    std::memcpy(b.data() + 8, &version, 4);
+    std::memcpy(b.data() + 16, &l.p0c, 8);
+    std::memcpy(b.data() + 24, &l.mass0, 8);
+    std::memcpy(b.data() + 32, &l.q0, 8);
+  }
+  void put(uint32_t type, uint32_t aux, const double *v, size_t nv) {
+    const size_t at = b.size();
+    b.resize(at + 8 + 8 * nv);
+    std::memcpy(b.data() + at, &type, 4);
+    std::memcpy(b.data() + at + 4, &aux, 4);
+    if (nv) std::memcpy(b.data() + at + 8, v, 8 * nv);
+    ++n;
+  }
+  void put(const Elem &e) { put(e.type, e.aux, e.v.data(), e.v.size()); }
+  const std::vector<unsigned char> &finish() {
+    const uint64_t total = b.size();
+    std::memcpy(b.data() + 12, &n, 4);
+    std::memcpy(b.data() + 40, &total, 8);
+    return b;
+  }
+};
+
 }  // namespace xt

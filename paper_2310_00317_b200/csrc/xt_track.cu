@@ -128,6 +128,11 @@ struct BendCase {  // thin kernels keep the dispatch tree they were measured wit
 };
 
 template <bool THICK>
+struct MonCase {
+  static constexpr uint32_t value = THICK ? static_cast<uint32_t>(TAG_MON) : 0x4ffu;
+};
+
+template <bool THICK>
 struct PolyCase {
   static constexpr uint32_t value = THICK ? static_cast<uint32_t>(TAG_POLY) : 0x3ffu;
 };
@@ -557,6 +562,27 @@ __device__ __noinline__ void limit_polygon(Parts<P> &q, const Cold<P> &cold, con
   if (out) lose<P>(q, out, cold, elem, turns_done, a);
 }
 
+// Internal monitor record (xt_twiss4d_line): row p0 of the monitor buffer receives the coordinates of every
+// alive particle of this thread.  THICK kernels only.
+__constant__ double *g_monitor_rows;
+
+template <int P>
+__device__ __noinline__ void monitor_store(const Parts<P> &q, const Cold<P> &cold, double row, int64_t n_part) {
+  double *base = g_monitor_rows + static_cast<int64_t>(row) * n_part * 6;
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    if (q.alive & (1u << j)) {
+      double *o = base + cold.idx(j) * 6;
+      o[0] = q.x[j];
+      o[1] = q.px[j];
+      o[2] = q.y[j];
+      o[3] = q.py[j];
+      o[4] = q.zeta[j];
+      o[5] = cold.delta(j);
+    }
+  }
+}
+
 // Push the P particles of this thread through every record of one staged chunk.
 // Returns the position just behind the chunk (where the next chunk of the image starts).
 template <int P, bool THICK>
@@ -652,6 +678,10 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
       }
       case BendCase<THICK>::value: {  // thick sector bend: p0 = k0, pf[0] = (h, length)
         if (THICK) thick_bend<P>(q, cold, p0, pf[0].x, pf[0].y);
+        break;
+      }
+      case MonCase<THICK>::value: {
+        if (THICK) monitor_store<P>(q, cold, p0, a.n_part);
         break;
       }
       case PolyCase<THICK>::value: {  // polygon aperture: (record bytes - header) / 16 vertices
@@ -890,6 +920,11 @@ int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStr
 }
 
 }  // namespace
+
+int set_monitor_base(double *d_rows, cudaStream_t st) {
+  XT_CUDA(cudaMemcpyToSymbolAsync(g_monitor_rows, &d_rows, sizeof(double *), 0, cudaMemcpyHostToDevice, st));
+  return XT_OK;
+}
 
 int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, const int64_t *d_n_active,
                  int64_t n_turns, int block, int ppt, cudaStream_t st) {

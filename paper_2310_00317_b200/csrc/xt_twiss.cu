@@ -9,7 +9,10 @@
 // 4 x 4 linear algebra runs on the host.
 #include <cmath>
 
+#include <vector>
+
 #include "xt_internal.h"
+#include "xt_line.h"
 
 namespace xt {
 namespace {
@@ -217,4 +220,137 @@ extern "C" int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double dde
   res.dqy = slope(hi.qy_frac, lo.qy_frac);
   *out = res;
   return XT_OK;
+}
+
+extern "C" int xt_twiss4d_line(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
+                               xt_twiss4d_chrom_result *start, xt_twiss_row *rows, int64_t cap, void *cuda_stream) {
+  using namespace xt;
+  if (!lat || !rows || !(ddelta > 0.0) || !std::isfinite(ddelta) || !std::isfinite(delta0)) {
+    set_error("xt_twiss4d_line: NULL lattice / rows, or ddelta not > 0");
+    return XT_ERR_INVALID_ARG;
+  }
+  Line line;
+  if (!read_line(lat->packed_host, line)) {
+    set_error("xt_twiss4d_line: the lattice holds no readable packed buffer");
+    return XT_ERR_INVALID_ARG;
+  }
+  const int64_t n_el = static_cast<int64_t>(line.el.size());
+  if (cap < n_el + 1) {
+    set_error("xt_twiss4d_line: rows must hold n_elements + 1 entries");
+    return XT_ERR_INVALID_ARG;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  // the optics at the start and the off-momentum closed orbits
+  xt_twiss4d_chrom_result on{};
+  xt_twiss4d_result hi{}, lo{};
+  int rc = xt_twiss4d_chrom(lat, delta0, ddelta, guess4, &on, cuda_stream);
+  if (rc == XT_OK) rc = xt_twiss4d(lat, delta0 + ddelta, on.on.co, &hi, cuda_stream);
+  if (rc == XT_OK) rc = xt_twiss4d(lat, delta0 - ddelta, on.on.co, &lo, cuda_stream);
+  if (rc != XT_OK) return rc;
+  if (!on.on.stable) {
+    set_error("xt_twiss4d_line: a plane is unstable at the start of the line");
+    return XT_ERR_UNSTABLE;
+  }
+  // the monitored line: a monitor record in front of every element and one behind the last
+  Writer w(line);
+  for (int64_t i = 0; i <= n_el; ++i) {
+    const double row = static_cast<double>(i);
+    w.put(kMonitorType, 0, &row, 1);
+    if (i < n_el) w.put(line.el[i]);
+  }
+  const std::vector<unsigned char> &buf = w.finish();
+  PackOpts po;
+  po.allow_monitor = true;
+  xt_lattice *mon = nullptr;
+  if ((rc = create_lattice(buf.data(), buf.size(), po, &mon)) != XT_OK) return rc;
+
+  constexpr int kN = 11;
+  const size_t n_rows = static_cast<size_t>(n_el + 1);
+  double *d_rows = nullptr, *d_f64 = nullptr;
+  int64_t *d_i64 = nullptr;
+  std::vector<double> h_rows(n_rows * kN * 6);
+  auto done = [&](int code) {
+    if (d_rows) cudaFree(d_rows);
+    if (d_f64) cudaFree(d_f64);
+    if (d_i64) cudaFree(d_i64);
+    xt_lattice_destroy(mon);
+    return code;
+  };
+#define XT_TRYL(call)                               \
+  do {                                              \
+    cudaError_t e__ = (call);                       \
+    if (e__ != cudaSuccess) return done(xt::cuda_fail(e__, #call)); \
+  } while (0)
+  XT_TRYL(cudaMalloc(&d_rows, h_rows.size() * sizeof(double)));
+  XT_TRYL(cudaMalloc(&d_f64, 10 * 16 * sizeof(double)));
+  XT_TRYL(cudaMalloc(&d_i64, 3 * 16 * sizeof(int64_t)));
+  XT_TRYL(cudaMemsetAsync(d_rows, 0xff, h_rows.size() * sizeof(double), st));  // NaN: a row a lost probe never wrote
+  double h[10][16] = {};
+  for (int k = 0; k < kN; ++k) {
+    const double *z = k == 9 ? hi.co : k == 10 ? lo.co : on.on.co;
+    for (int c = 0; c < 4; ++c) h[c][k] = z[c];
+    h[5][k] = k == 9 ? delta0 + ddelta : k == 10 ? delta0 - ddelta : delta0;
+  }
+  for (int c = 0; c < 4; ++c) {
+    h[c][1 + 2 * c] += kStep[c];
+    h[c][2 + 2 * c] -= kStep[c];
+  }
+  int64_t hi64[3][16] = {};
+  for (int k = 0; k < kN; ++k) hi64[1][k] = 1;  // state
+  XT_TRYL(cudaMemcpyAsync(d_f64, h, sizeof(h), cudaMemcpyHostToDevice, st));
+  XT_TRYL(cudaMemcpyAsync(d_i64, hi64, sizeof(hi64), cudaMemcpyHostToDevice, st));
+  xt_particles p{};
+  double **d[10] = {&p.x, &p.px, &p.y, &p.py, &p.zeta, &p.delta, &p.ptau, &p.rpp, &p.rvv, &p.s};
+  for (int k = 0; k < 10; ++k) *d[k] = d_f64 + 16 * k;
+  p.at_turn = d_i64;
+  p.state = d_i64 + 16;
+  p.at_element = d_i64 + 32;
+  if ((rc = launch_init_derived(mon, p, kN, st)) != XT_OK) return done(rc);
+  if ((rc = set_monitor_base(d_rows, st)) != XT_OK) return done(rc);
+  if ((rc = xt_track(mon, &p, kN, 1, st)) != XT_OK) return done(rc);
+  XT_TRYL(cudaMemcpyAsync(h_rows.data(), d_rows, h_rows.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
+  XT_TRYL(cudaStreamSynchronize(st));
+#undef XT_TRYL
+
+  const double two_pi = 2.0 * 3.14159265358979323846;
+  const double b0[2] = {on.on.betx, on.on.bety}, a0[2] = {on.on.alfx, on.on.alfy};
+  double mu_prev[2] = {0.0, 0.0}, raw_prev[2] = {0.0, 0.0};
+  for (size_t i = 0; i < n_rows; ++i) {
+    const double *r = h_rows.data() + i * kN * 6;
+    for (int k = 0; k < kN * 6; ++k)
+      if (!std::isfinite(r[k])) {
+        set_error("xt_twiss4d_line: a probe particle was lost before element " + std::to_string(i));
+        return done(XT_ERR_UNSTABLE);
+      }
+    xt_twiss_row &o = rows[i];
+    o.s = i < static_cast<size_t>(n_el) ? lat->s_table_host[i] : lat->info.circumference;
+    o.x = r[0];
+    o.px = r[1];
+    o.y = r[2];
+    o.py = r[3];
+    double jac[4][4];
+    for (int row = 0; row < 4; ++row)
+      for (int c = 0; c < 4; ++c)
+        jac[row][c] = (r[(1 + 2 * c) * 6 + row] - r[(2 + 2 * c) * 6 + row]) / (2.0 * kStep[c]);
+    double *bet[2] = {&o.betx, &o.bety}, *alf[2] = {&o.alfx, &o.alfy}, *mu[2] = {&o.mux, &o.muy};
+    for (int pl = 0; pl < 2; ++pl) {
+      const int q = 2 * pl;
+      const double m11 = jac[q][q], m12 = jac[q][q + 1], m21 = jac[q + 1][q], m22 = jac[q + 1][q + 1];
+      const double g0 = (1.0 + a0[pl] * a0[pl]) / b0[pl];
+      *bet[pl] = m11 * m11 * b0[pl] - 2.0 * m11 * m12 * a0[pl] + m12 * m12 * g0;
+      *alf[pl] = -m11 * m21 * b0[pl] + (m11 * m22 + m12 * m21) * a0[pl] - m12 * m22 * g0;
+      double raw = std::atan2(m12, m11 * b0[pl] - m12 * a0[pl]);
+      if (raw < 0.0) raw += two_pi;
+      double step = raw - raw_prev[pl];             // the phase never runs backwards: unwrap
+      if (step < -1e-6) step += two_pi;
+      if (i == 0) step = 0.0;
+      mu_prev[pl] += step;
+      raw_prev[pl] = raw;
+      *mu[pl] = mu_prev[pl];
+    }
+    double *dd[4] = {&o.dx, &o.dpx, &o.dy, &o.dpy};
+    for (int c = 0; c < 4; ++c) *dd[c] = (r[9 * 6 + c] - r[10 * 6 + c]) / (2.0 * ddelta);
+  }
+  if (start) *start = on;
+  return done(XT_OK);
 }

@@ -135,3 +135,56 @@ def test_dispersion_and_chromaticity(X):
         X.xt_twiss4d_chrom(lat, 0.0, 0.0)
     assert e.value.code == -1
     lat.close()
+
+
+def test_optics_along_the_line(X):
+    """xt_twiss4d_line (one launch through internal monitor records) against the thin-FODO closed forms of pin
+    P19, against the oracle's prefix-tracking procedure on every row of configs[0] and on sampled rows of the
+    LHC-sized configs[2]; the last row closes on the first and carries the whole tune."""
+    from xt_inputs.packed import Marker
+    n_cells, L, kq = 10, 2.0, 0.1
+    cell = [Multipole(knl=(0.0, kq)), Drift(L / 2), Marker(), Drift(L / 2), Multipole(knl=(0.0, -kq)), Drift(L)]
+    lat = X.xt_lattice_create(pack_lattice(cell * n_cells, P0C, MASS0, 1.0))
+    start, rows = X.xt_twiss4d_line(lat)
+    lat.close()
+    mu = math.acos(1.0 - (L * kq) ** 2 / 2.0)
+    bmax, bmin = 2 * L * (1 + math.sin(mu / 2)) / math.sin(mu), 2 * L * (1 - math.sin(mu / 2)) / math.sin(mu)
+    qf, qd = np.arange(n_cells) * 6, np.arange(n_cells) * 6 + 4
+    np.testing.assert_allclose(rows["betx"][qf], bmax, rtol=1e-6)
+    np.testing.assert_allclose(rows["bety"][qf], bmin, rtol=1e-6)
+    np.testing.assert_allclose(rows["betx"][qd], bmin, rtol=1e-6)
+    np.testing.assert_allclose(rows["alfx"][qf], -bmax * kq / 2, atol=1e-6)
+    np.testing.assert_allclose(rows["alfy"][qd], -bmax * kq / 2, atol=1e-6)
+    np.testing.assert_allclose(rows["mux"][qf], np.arange(n_cells) * mu, atol=1e-6)
+    np.testing.assert_allclose(rows["muy"][-1], n_cells * mu, atol=1e-6)
+    np.testing.assert_allclose(rows["s"][qd], np.arange(n_cells) * 2 * L + L, atol=1e-12)
+    assert np.array_equal(rows["betx"][qf + 2], rows["betx"][qf + 3])           # a marker's row = the next element's
+    assert abs(rows["mux"][-1] / (2 * math.pi) % 1.0 - start["qx_frac"]) < 1e-7
+
+    for cfg, pick in ((0, None), (2, 24)):
+        els = C.lattice(cfg)
+        n = len(els)
+        sel = list(range(n + 1)) if pick is None else sorted(set(np.random.default_rng(3).integers(0, n + 1, pick)) | {0, n})
+        want_on, want = MO.optics_along(els, C.P0C, C.MASS0, 1.0, sel)
+        lat = X.xt_lattice_create(C.pack(els))
+        start, rows = X.xt_twiss4d_line(lat)
+        lat.close()
+        assert abs(start["betx"] / want_on["betx"] - 1) < 1e-7
+        for i, w in zip(sel, want):
+            for k in ("x", "y"):
+                assert abs(rows[k][i] - w[k]) < 1e-11, (cfg, i, k)
+            for k in ("betx", "bety"):
+                assert abs(rows[k][i] / w[k] - 1.0) < 2e-6, (cfg, i, k)
+            for k in ("alfx", "alfy"):
+                assert abs(rows[k][i] - w[k]) < 2e-6 * max(1.0, abs(w[k])), (cfg, i, k)
+            for k in ("mux", "muy"):
+                d = (rows[k][i] - w[k]) % (2 * math.pi)
+                assert min(d, 2 * math.pi - d) < 1e-6, (cfg, i, k)
+            for k in ("dx", "dy"):
+                assert abs(rows[k][i] - w[k]) < 2e-6 * max(1.0, abs(w[k])), (cfg, i, k)
+        assert np.all(np.diff(rows["mux"]) > -1e-9) and np.all(np.diff(rows["s"]) >= 0)
+        assert abs(rows["betx"][-1] / rows["betx"][0] - 1) < 1e-5 and abs(rows["dx"][-1] - rows["dx"][0]) < 1e-5
+        assert abs((rows["mux"][-1] / (2 * math.pi)) % 1.0 - start["qx_frac"]) < 1e-6
+        if cfg == 2:
+            assert rows["mux"][-1] / (2 * math.pi) > 10.0                       # integer part of the tune included
+            print("configs[2] tunes with integer part:", rows["mux"][-1] / (2 * math.pi), rows["muy"][-1] / (2 * math.pi))

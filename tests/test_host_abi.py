@@ -375,3 +375,12 @@ def test_polygon_aperture_is_packed_unfused_and_refine_rejects_bad_arguments():
     assert lib.xt_refine_loss_location(None, None, 0, 0.1, 16, None, None) == -1  # NULL lattice: no CUDA call
     assert lib.xt_lattice_set_knobs(None, None, 1, 1, None, 0) == -1 and lib.xt_track_knobs(None, None, 0, 1, 0, None) == -1
     assert ctypes.sizeof(X.binding.xt_knob_link) == 32
+
+
+def test_internal_monitor_type_is_not_a_public_element():
+    body = struct.pack("<IId", 11, 0, 0.0)
+    buf = struct.pack("<8sIIdddQ", b"XTLAT001", 1, 1, 450e9, 938272088.16, 1.0, 48 + len(body)) + body
+    lib = X.load_library("prod")
+    assert lib.xt_lattice_pack_host(buf, len(buf), None, None, 0, None) == -2
+    assert lib.xt_twiss4d_line(None, 0.0, 1e-4, None, None, None, 0, None) == -1
+    assert ctypes.sizeof(B.xt_twiss_row) == 15 * 8
