@@ -62,16 +62,53 @@ def optics_of(buf, delta=0.0, guess=None):
         if np.max(np.abs(dz)) < 1e-13:
             break
     J = jac4(buf, z, delta=delta)                         # Twiss step 2
-    out = {"x_co": z[0], "px_co": z[1], "y_co": z[2], "py_co": z[3]}
+    out = {"x_co": z[0], "px_co": z[1], "y_co": z[2], "py_co": z[3], "m": J}
     for name, i in (("x", 0), ("y", 2)):                  # Twiss step 3 (uncoupled)
         m = J[i:i + 2, i:i + 2]
         cosmu = 0.5 * (m[0, 0] + m[1, 1])
-        assert abs(cosmu) < 1.0, "unstable plane %s: cos mu = %g" % (name, cosmu)
+        if not abs(cosmu) < 1.0:                          # no uncoupled reading of this plane (coupled or unstable)
+            out["bet" + name] = out["alf" + name] = out["q" + name + "_frac"] = float("nan")
+            continue
         sinmu = math.copysign(math.sqrt(1.0 - cosmu * cosmu), m[0, 1])
         out["bet" + name] = m[0, 1] / sinmu
         out["alf" + name] = (m[0, 0] - m[1, 1]) / (2.0 * sinmu)
         mu = math.atan2(sinmu, cosmu)
         out["q" + name + "_frac"] = (mu / (2 * math.pi)) % 1.0
+    return out
+
+
+S4 = np.array([[0.0, 1.0, 0.0, 0.0], [-1.0, 0.0, 0.0, 0.0], [0.0, 0.0, 0.0, 1.0], [0.0, 0.0, -1.0, 0.0]])
+
+
+def normal_form4(J):
+    """Twiss step 3 in full ("Linear Normal Form of the map from the eigenvalues and eigenvectors
+    of the Jacobian matrix"; step 5 "Mais-Ripken"): the two normal modes of the 4x4 one-turn matrix.
+    numpy.linalg.eig gives eigenvalues exp(+-i mu_k) and eigenvectors; of each conjugate pair the one with
+    v^H S v = +2i after scaling (positive symplectic norm) is kept -- in one uncoupled plane that is
+    v = (sqrt(beta), (i - alpha)/sqrt(beta)) with eigenvalue exp(+i mu); mode 1 is the one with the larger
+    horizontal part.  Mais-Ripken functions of mode k in plane u: beta_uk = |v_u|^2,
+    alpha_uk = -Re(conj(v_u) v_pu).  Returns None if an eigenvalue is off the unit circle."""
+    lam, vec = np.linalg.eig(np.asarray(J, dtype=np.float64))
+    modes = []
+    for k in range(4):
+        if abs(abs(lam[k]) - 1.0) > 1e-6 or abs(lam[k].imag) < 1e-12:
+            return None
+        v = vec[:, k]
+        norm = (np.conj(v) @ S4 @ v).imag / 2.0
+        if norm > 0.0:
+            modes.append((lam[k], v / math.sqrt(norm)))
+    if len(modes) != 2:
+        return None
+    modes.sort(key=lambda m: -abs(m[1][0]) ** 2)
+    out = {}
+    for k, (lmb, v) in enumerate(modes, start=1):
+        ref = v[0] if k == 1 else v[2]                     # phase origin: the mode's own plane is real positive
+        v = v * (abs(ref) / ref)
+        out["q%d_frac" % k] = (math.atan2(lmb.imag, lmb.real) / (2 * math.pi)) % 1.0
+        out["v%d" % k] = v
+        for name, i in (("x", 0), ("y", 2)):
+            out["bet%s%d" % (name, k)] = abs(v[i]) ** 2
+            out["alf%s%d" % (name, k)] = -(np.conj(v[i]) * v[i + 1]).real
     return out
 
 
@@ -118,6 +155,9 @@ def optics_along(elements, p0c, mass0, q0, rows, ddelta=1e-4, delta=0.0):
     pts[9], pts[10] = zh, zl
     deltas = np.full(11, delta)
     deltas[9], deltas[10] = delta + ddelta, delta - ddelta
+    nf = normal_form4(on["m"])
+    if nf is not None:
+        on.update({k: v for k, v in nf.items()})
     out = []
     for row in rows:
         prefix = PK.pack_lattice(list(elements[:row]) or [PK.Marker()], p0c, mass0, q0)
@@ -139,6 +179,12 @@ def optics_along(elements, p0c, mass0, q0, rows, ddelta=1e-4, delta=0.0):
             r["mu" + name] = math.atan2(m[0, 1], m[0, 0] * b0 - m[0, 1] * a0) % (2 * math.pi)
         d = (z[9] - z[10]) / (2.0 * ddelta)
         r["dx"], r["dpx"], r["dy"], r["dpy"] = d
+        if nf is not None:                                 # steps 4-5: the eigenvectors carried by the tracked Jacobian
+            for k in (1, 2):
+                v = J @ nf["v%d" % k]
+                r["betx%d" % k], r["bety%d" % k] = abs(v[0]) ** 2, abs(v[2]) ** 2
+                own = v[0] if k == 1 else v[2]
+                r["mu%d" % k] = math.atan2(own.imag, own.real) % (2 * math.pi)
         out.append(r)
     return on, out
 
@@ -148,7 +194,7 @@ def main():
                      "orbit, PAPER.md:96-98); input shaping only"}
     for cfg in (2, 3, 4):
         buf = C.pack(C.lattice(cfg))
-        res["cfg%d" % cfg] = optics_of(buf)
+        res["cfg%d" % cfg] = {k: float(v) for k, v in optics_of(buf).items() if k != "m"}
         print(cfg, res["cfg%d" % cfg])
     path = os.path.join(os.path.dirname(os.path.abspath(C.__file__)), "optics.json")
     with open(path, "w") as fh:

@@ -705,3 +705,57 @@ def test_P19_optics_along_a_fodo_ring_and_a_ring_with_dipoles():
         if i < 8:
             d = mats[i] @ d
     assert abs(rows[-1]["dx"] - rows[0]["dx"]) < 1e-6
+
+
+# ----------------------------- P20 linear normal form with coupling
+def test_P20_normal_form_uncoupled_rotated_and_closest_tune_approach():
+    """oracle/make_optics.normal_form4 against (a) Courant-Snyder in an uncoupled ring: mode 1 is the
+    horizontal plane, beta_y1 = beta_x2 = 0; (b) the same ring seen from a frame rotated by theta about s:
+    tunes unchanged, Mais-Ripken beta_x1 = cos^2 beta_x, beta_y1 = sin^2 beta_x, beta_x2 = sin^2 beta_y,
+    beta_y2 = cos^2 beta_y; (c) a thin skew quadrupole in a ring with equal tunes splits them by
+    |ks| sqrt(beta_x beta_y) / (2 pi) (closest tune approach, first order in ks)."""
+    from oracle import make_optics as MO
+    n_cells, L, kq = 10, 2.0, 0.1
+    cell = [Multipole(knl=(0.0, kq)), Drift(L), Multipole(knl=(0.0, -0.95 * kq)), Drift(L)]    # unequal strengths: Qx != Qy
+    els = cell * n_cells
+    on = MO.optics_of(pack(els))
+    nf = MO.normal_form4(on["m"])
+    assert abs(nf["betx1"] / on["betx"] - 1) < 1e-7 and abs(nf["bety2"] / on["bety"] - 1) < 1e-7
+    assert abs(nf["alfx1"] - on["alfx"]) < 1e-7 and abs(nf["alfy2"] - on["alfy"]) < 1e-7
+    assert nf["bety1"] < 1e-12 and nf["betx2"] < 1e-12
+    assert abs(nf["q1_frac"] - on["qx_frac"]) < 1e-9 and abs(nf["q2_frac"] - on["qy_frac"]) < 1e-9
+    assert abs(on["qx_frac"] - on["qy_frac"]) > 0.01
+
+    th = 0.3
+    rot = [SRotation.from_angle(-th)] + els + [SRotation.from_angle(th)]
+    nfr = MO.normal_form4(MO.optics_of(pack(rot))["m"])
+    c2, s2 = math.cos(th) ** 2, math.sin(th) ** 2
+    assert abs(nfr["q1_frac"] - nf["q1_frac"]) < 1e-9 and abs(nfr["q2_frac"] - nf["q2_frac"]) < 1e-9
+    assert abs(nfr["betx1"] - c2 * on["betx"]) < 1e-6 and abs(nfr["bety1"] - s2 * on["betx"]) < 1e-6
+    assert abs(nfr["betx2"] - s2 * on["bety"]) < 1e-6 and abs(nfr["bety2"] - c2 * on["bety"]) < 1e-6
+    assert abs(nfr["alfx1"] - c2 * on["alfx"]) < 1e-6 and abs(nfr["alfy2"] - c2 * on["alfy"]) < 1e-6
+
+    # equal tunes: start in the middle of a drift of the symmetric cell, where beta_x = beta_y needs no care
+    ks = 2e-5
+    sym = [Multipole(knl=(0.0, kq)), Drift(L), Multipole(knl=(0.0, -kq)), Drift(L)] * n_cells
+    on = MO.optics_of(pack(sym))
+    assert abs(on["qx_frac"] - on["qy_frac"]) < 1e-9
+    skew = [Multipole(knl=(0.0, 0.0), ksl=(0.0, ks))] + sym
+    nfs = MO.normal_form4(MO.optics_of(pack(skew))["m"])
+    split = abs(nfs["q1_frac"] - nfs["q2_frac"])
+    want = ks * math.sqrt(on["betx"] * on["bety"]) / (2 * math.pi)
+    assert abs(split / want - 1.0) < 2e-3, (split, want)
+    assert abs(nfs["betx1"] / nfs["betx2"] - 1.0) < 0.05                     # fully mixed modes on the resonance
+    # steps 4-5: carried along the line, the modes of an uncoupled ring are its planes
+    on, rows = MO.optics_along(els, H.P0C, H.MASS0, H.Q0, list(range(0, len(els) + 1, 3)))
+    for r in rows:
+        assert abs(r["betx1"] / r["betx"] - 1) < 1e-7 and abs(r["bety2"] / r["bety"] - 1) < 1e-7
+        assert r["bety1"] < 1e-10 and r["betx2"] < 1e-10
+        for a, b in ((r["mu1"], r["mux"]), (r["mu2"], r["muy"])):
+            d = (a - b) % (2 * math.pi)
+            assert min(d, 2 * math.pi - d) < 1e-7
+    # ... and in the rotated frame the mode functions keep their cos^2 / sin^2 shares at every element
+    on_r, rows_r = MO.optics_along(rot, H.P0C, H.MASS0, H.Q0, [1 + i for i in range(0, len(els) + 1, 3)])
+    for r, rr in zip(rows, rows_r):
+        assert abs(rr["betx1"] - c2 * r["betx"]) < 1e-5 and abs(rr["bety1"] - s2 * r["betx"]) < 1e-5
+        assert abs(rr["bety2"] - c2 * r["bety"]) < 1e-5 and abs(rr["betx2"] - s2 * r["bety"]) < 1e-5
