@@ -754,8 +754,11 @@ def test_P20_normal_form_uncoupled_rotated_and_closest_tune_approach():
         for a, b in ((r["mu1"], r["mux"]), (r["mu2"], r["muy"])):
             d = (a - b) % (2 * math.pi)
             assert min(d, 2 * math.pi - d) < 1e-7
-    # ... and in the rotated frame the mode functions keep their cos^2 / sin^2 shares at every element
-    on_r, rows_r = MO.optics_along(rot, H.P0C, H.MASS0, H.Q0, [1 + i for i in range(0, len(els) + 1, 3)])
-    for r, rr in zip(rows, rows_r):
-        assert abs(rr["betx1"] - c2 * r["betx"]) < 1e-5 and abs(rr["bety1"] - s2 * r["betx"]) < 1e-5
-        assert abs(rr["bety2"] - c2 * r["bety"]) < 1e-5 and abs(rr["betx2"] - s2 * r["bety"]) < 1e-5
+    # ... seen from the rotated frame: inside the two rotations the coordinates are the ring's own again (the
+    # modes are its planes), at the start and at the end they carry the cos^2 / sin^2 shares
+    on_r, rows_r = MO.optics_along(rot, H.P0C, H.MASS0, H.Q0, [0] + [1 + i for i in range(0, len(els) + 1, 3)] + [len(rot)])
+    for r, rr in zip(rows, rows_r[1:-1]):
+        assert abs(rr["betx1"] - r["betx"]) < 1e-5 and rr["bety1"] < 1e-9 and abs(rr["bety2"] - r["bety"]) < 1e-5
+    for rr in (rows_r[0], rows_r[-1]):
+        assert abs(rr["betx1"] - c2 * rows[0]["betx"]) < 1e-5 and abs(rr["bety1"] - s2 * rows[0]["betx"]) < 1e-5
+        assert abs(rr["bety2"] - c2 * rows[0]["bety"]) < 1e-5 and abs(rr["betx2"] - s2 * rows[0]["bety"]) < 1e-5
