@@ -253,6 +253,26 @@ typedef struct {
 int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
                      xt_twiss4d_chrom_result *out, void *cuda_stream);
 
+/* Linear normal form of a 4x4 one-turn matrix with coupling (PAPER.md:98 step 3 "from the eigenvalues and
+ * eigenvectors of the Jacobian matrix", step 5 "Mais-Ripken").  Pure HOST arithmetic,
+ * no CUDA call.  m: row-major, e.g. xt_twiss4d_result.m.  The characteristic polynomial of a symplectic
+ * matrix is reciprocal: with u = lambda + 1/lambda it is u^2 - tr(M) u + (tr(M)^2 - tr(M^2))/2 - 2 = 0, so
+ * cos mu_k = u_k/2; the eigenvector of exp(i mu_k) is (M - conj(lambda_k)) (M^2 - u_other M + 1) w; of each
+ * conjugate pair the one with v^H S v = +2i is kept (in one uncoupled plane: (sqrt(beta),
+ * (i - alpha)/sqrt(beta)), eigenvalue exp(+i mu)); mode 1 is the one with the larger horizontal part, its x
+ * component real positive (mode 2: y).  beta_uk = |v_u|^2, alpha_uk = -Re(conj(v_u) v_pu).
+ * stable = 0 (and NaN) if an eigenvalue leaves the unit circle; degenerate = 1 (and NaN) if the two modes have
+ * the same tune (|cos mu_1 - cos mu_2| < 1.6e-4, what a central-difference Jacobian resolves): the eigenvectors
+ * are then not defined (use the per-plane optics). */
+typedef struct {
+  double q1_frac, q2_frac;
+  double betx1, alfx1, bety1, alfy1;
+  double betx2, alfx2, bety2, alfy2;
+  double v1[8], v2[8]; /* eigenvectors (x, px, y, py), re/im interleaved */
+  int32_t stable, degenerate;
+} xt_twiss4d_modes;
+int xt_twiss4d_normal_form(const double *m, xt_twiss4d_modes *out);
+
 /* Optics along the line (the optics found at the start is carried
  * "to all other elements by tracking"; beta functions along the ring).  After the three closed-orbit
  * searches of xt_twiss4d_chrom, ONE launch tracks eleven probe particles (the orbit, +-h along x, px, y, py,
@@ -268,6 +288,9 @@ typedef struct {
   double s, x, px, y, py;
   double betx, alfx, mux, bety, alfy, muy;
   double dx, dpx, dy, dpy;
+  double betx1, bety1, betx2, bety2; /* Mais-Ripken beta functions of the two normal modes (xt_twiss4d_normal_form) */
+  double mu1, mu2;                   /* their phase advances from the start, unwrapped; NaN like the four above  */
+                                     /* when the one-turn matrix has no two distinct stable modes                */
 } xt_twiss_row;
 int xt_twiss4d_line(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
                     xt_twiss4d_chrom_result *start, xt_twiss_row *rows, int64_t cap, void *cuda_stream);

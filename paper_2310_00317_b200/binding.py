@@ -61,7 +61,15 @@ class xt_twiss4d_chrom_result(ctypes.Structure):
 
 class xt_twiss_row(ctypes.Structure):
     _fields_ = [(k, ctypes.c_double) for k in ("s", "x", "px", "y", "py", "betx", "alfx", "mux", "bety", "alfy",
-                                                "muy", "dx", "dpx", "dy", "dpy")]
+                                                "muy", "dx", "dpx", "dy", "dpy", "betx1", "bety1", "betx2", "bety2",
+                                                "mu1", "mu2")]
+
+
+class xt_twiss4d_modes(ctypes.Structure):
+    _fields_ = ([(k, ctypes.c_double) for k in ("q1_frac", "q2_frac", "betx1", "alfx1", "bety1", "alfy1", "betx2",
+                                                 "alfx2", "bety2", "alfy2")] +
+                [("v1", ctypes.c_double * 8), ("v2", ctypes.c_double * 8), ("stable", ctypes.c_int32),
+                 ("degenerate", ctypes.c_int32)])
 
 
 class xt_lattice_info(ctypes.Structure):
@@ -106,6 +114,7 @@ SIGNATURES = {
                                                ctypes.c_int32, ctypes.POINTER(ctypes.c_int64), _VP]),
     "xt_twiss4d_chrom": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
                                         ctypes.POINTER(xt_twiss4d_chrom_result), _VP]),
+    "xt_twiss4d_normal_form": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(xt_twiss4d_modes)]),
     "xt_twiss4d_line": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
                                        ctypes.POINTER(xt_twiss4d_chrom_result), ctypes.POINTER(xt_twiss_row), _I64,
                                        _VP]),
@@ -406,6 +415,19 @@ def xt_twiss4d_chrom(lat: Lattice, delta0: float = 0.0, ddelta: float = 1e-4, gu
     return out
 
 
+def xt_twiss4d_normal_form(m, kind: str = "prod") -> Dict:
+    """Normal modes of a 4x4 one-turn matrix (host arithmetic only; include/xt.h)."""
+    lib = load_library(kind)
+    a = np.ascontiguousarray(m, dtype=np.float64).reshape(16)
+    res = xt_twiss4d_modes()
+    _check(lib, lib.xt_twiss4d_normal_form(a.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), ctypes.byref(res)))
+    out = {k: getattr(res, k) for k, _ in xt_twiss4d_modes._fields_ if k not in ("v1", "v2")}
+    for k in ("v1", "v2"):
+        raw = np.array(list(getattr(res, k)))
+        out[k] = raw[0::2] + 1j * raw[1::2]
+    return out
+
+
 def xt_twiss4d_line(lat: Lattice, delta0: float = 0.0, ddelta: float = 1e-4, guess4=None, stream=None):
     """Optics along the line: (start dict as xt_twiss4d_chrom, rows dict of arrays of n_elements + 1); include/xt.h."""
     n = int(lat.info["n_elements"]) + 1
@@ -417,7 +439,7 @@ def xt_twiss4d_line(lat: Lattice, delta0: float = 0.0, ddelta: float = 1e-4, gue
     start = _twiss_dict(res.on)
     for k in ("dx", "dpx", "dy", "dpy", "dqx", "dqy"):
         start[k] = getattr(res, k)
-    arr = np.frombuffer(rows, dtype=np.float64).reshape(n, 15).copy()
+    arr = np.frombuffer(rows, dtype=np.float64).reshape(n, len(xt_twiss_row._fields_)).copy()
     return start, {k: arr[:, i] for i, (k, _) in enumerate(xt_twiss_row._fields_)}
 
 

@@ -9,6 +9,7 @@
 // 4 x 4 linear algebra runs on the host.
 #include <cmath>
 
+#include <complex>
 #include <vector>
 
 #include "xt_internal.h"
@@ -222,6 +223,101 @@ extern "C" int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double dde
   return XT_OK;
 }
 
+extern "C" int xt_twiss4d_normal_form(const double *m, xt_twiss4d_modes *out) {
+  using namespace xt;
+  using cplx = std::complex<double>;
+  if (!m || !out) {
+    set_error("xt_twiss4d_normal_form: NULL argument");
+    return XT_ERR_INVALID_ARG;
+  }
+  xt_twiss4d_modes res;
+  const double nan = std::nan("");
+  double *all[] = {&res.q1_frac, &res.q2_frac, &res.betx1, &res.alfx1, &res.bety1, &res.alfy1,
+                   &res.betx2, &res.alfx2, &res.bety2, &res.alfy2};
+  for (double *p : all) *p = nan;
+  for (int k = 0; k < 8; ++k) res.v1[k] = res.v2[k] = nan;
+  res.stable = 0;
+  res.degenerate = 0;
+  *out = res;
+  double m2[16];
+  for (int r = 0; r < 4; ++r)
+    for (int c = 0; c < 4; ++c) {
+      double s = 0.0;
+      for (int k = 0; k < 4; ++k) s += m[4 * r + k] * m[4 * k + c];
+      m2[4 * r + c] = s;
+    }
+  const double a = m[0] + m[5] + m[10] + m[15], t2 = m2[0] + m2[5] + m2[10] + m2[15];
+  const double b = 0.5 * (a * a - t2);
+  double disc = a * a - 4.0 * (b - 2.0);
+  if (!std::isfinite(disc)) return XT_OK;
+  if (std::fabs(disc) < 1e-7) {  // |cos mu_1 - cos mu_2| < 1.6e-4: below what a central-difference Jacobian resolves
+    out->stable = (std::fabs(0.5 * a) < 4.0) ? 1 : 0;
+    out->degenerate = 1;
+    return XT_OK;
+  }
+  if (disc < 0.0) return XT_OK;  // complex u: a coupling (sum) resonance, unstable
+  const double rt = std::sqrt(disc);
+  const double u[2] = {0.5 * (a + rt), 0.5 * (a - rt)};
+  if (!(std::fabs(u[0]) < 2.0) || !(std::fabs(u[1]) < 2.0)) return XT_OK;
+  cplx v[2][4];
+  double q[2];
+  for (int k = 0; k < 2; ++k) {
+    // A = (M^2 - u_other M + 1) w, w the unit vector that gives the longest A
+    double best[4] = {0, 0, 0, 0}, best_n = -1.0;
+    for (int j = 0; j < 4; ++j) {
+      double col[4], n2 = 0.0;
+      for (int r = 0; r < 4; ++r) {
+        col[r] = m2[4 * r + j] - u[1 - k] * m[4 * r + j] + (r == j ? 1.0 : 0.0);
+        n2 += col[r] * col[r];
+      }
+      if (n2 > best_n) {
+        best_n = n2;
+        for (int r = 0; r < 4; ++r) best[r] = col[r];
+      }
+    }
+    const double c = 0.5 * u[k], sn = std::sqrt(1.0 - c * c);
+    cplx lam(c, sn);
+    for (int r = 0; r < 4; ++r) {
+      double ma = 0.0;
+      for (int j = 0; j < 4; ++j) ma += m[4 * r + j] * best[j];
+      v[k][r] = ma - std::conj(lam) * best[r];
+    }
+    // v^H S v = 2i * norm
+    double norm = 0.5 * (std::conj(v[k][0]) * v[k][1] - std::conj(v[k][1]) * v[k][0] + std::conj(v[k][2]) * v[k][3] -
+                         std::conj(v[k][3]) * v[k][2]).imag();
+    if (norm < 0.0) {
+      for (int r = 0; r < 4; ++r) v[k][r] = std::conj(v[k][r]);
+      lam = std::conj(lam);
+      norm = -norm;
+    }
+    if (!(norm > 0.0)) return XT_OK;
+    for (int r = 0; r < 4; ++r) v[k][r] /= std::sqrt(norm);
+    double f = std::atan2(lam.imag(), lam.real()) / (2.0 * 3.14159265358979323846);
+    q[k] = f - std::floor(f);
+  }
+  const int first = std::norm(v[0][0]) >= std::norm(v[1][0]) ? 0 : 1;
+  for (int k = 0; k < 2; ++k) {
+    const int src = k == 0 ? first : 1 - first;
+    const cplx ref = v[src][k == 0 ? 0 : 2];
+    const cplx ph = std::abs(ref) > 0.0 ? std::abs(ref) / ref : cplx(1.0, 0.0);
+    cplx w[4];
+    for (int r = 0; r < 4; ++r) w[r] = v[src][r] * ph;
+    double *vec = k == 0 ? res.v1 : res.v2;
+    for (int r = 0; r < 4; ++r) {
+      vec[2 * r] = w[r].real();
+      vec[2 * r + 1] = w[r].imag();
+    }
+    (k == 0 ? res.q1_frac : res.q2_frac) = q[src];
+    (k == 0 ? res.betx1 : res.betx2) = std::norm(w[0]);
+    (k == 0 ? res.alfx1 : res.alfx2) = -(std::conj(w[0]) * w[1]).real();
+    (k == 0 ? res.bety1 : res.bety2) = std::norm(w[2]);
+    (k == 0 ? res.alfy1 : res.alfy2) = -(std::conj(w[2]) * w[3]).real();
+  }
+  res.stable = 1;
+  *out = res;
+  return XT_OK;
+}
+
 extern "C" int xt_twiss4d_line(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
                                xt_twiss4d_chrom_result *start, xt_twiss_row *rows, int64_t cap, void *cuda_stream) {
   using namespace xt;
@@ -312,6 +408,10 @@ extern "C" int xt_twiss4d_line(const xt_lattice *lat, double delta0, double ddel
   XT_TRYL(cudaStreamSynchronize(st));
 #undef XT_TRYL
 
+  xt_twiss4d_modes modes{};
+  xt_twiss4d_normal_form(on.on.m, &modes);
+  const bool have_modes = modes.stable && !modes.degenerate;
+  double mode_mu[2] = {0.0, 0.0}, mode_raw[2] = {0.0, 0.0};
   const double two_pi = 2.0 * 3.14159265358979323846;
   const double b0[2] = {on.on.betx, on.on.bety}, a0[2] = {on.on.alfx, on.on.alfy};
   double mu_prev[2] = {0.0, 0.0}, raw_prev[2] = {0.0, 0.0};
@@ -347,6 +447,28 @@ extern "C" int xt_twiss4d_line(const xt_lattice *lat, double delta0, double ddel
       mu_prev[pl] += step;
       raw_prev[pl] = raw;
       *mu[pl] = mu_prev[pl];
+    }
+    o.betx1 = o.bety1 = o.betx2 = o.bety2 = o.mu1 = o.mu2 = std::nan("");
+    if (have_modes) {  // steps 4-5: the eigenvectors carried by the tracked Jacobian
+      for (int k = 0; k < 2; ++k) {
+        const double *vec = k == 0 ? modes.v1 : modes.v2;
+        std::complex<double> w[4];
+        for (int row = 0; row < 4; ++row) {
+          w[row] = 0.0;
+          for (int c = 0; c < 4; ++c) w[row] += jac[row][c] * std::complex<double>(vec[2 * c], vec[2 * c + 1]);
+        }
+        (k == 0 ? o.betx1 : o.betx2) = std::norm(w[0]);
+        (k == 0 ? o.bety1 : o.bety2) = std::norm(w[2]);
+        const std::complex<double> own = w[k == 0 ? 0 : 2];
+        double raw = std::atan2(own.imag(), own.real());
+        if (raw < 0.0) raw += two_pi;
+        double step = raw - mode_raw[k];
+        if (step < -1e-6) step += two_pi;
+        if (i == 0) step = 0.0;
+        mode_mu[k] += step;
+        mode_raw[k] = raw;
+        (k == 0 ? o.mu1 : o.mu2) = mode_mu[k];
+      }
     }
     double *dd[4] = {&o.dx, &o.dpx, &o.dy, &o.dpy};
     for (int c = 0; c < 4; ++c) *dd[c] = (r[9 * 6 + c] - r[10 * 6 + c]) / (2.0 * ddelta);

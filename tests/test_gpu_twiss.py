@@ -182,9 +182,54 @@ def test_optics_along_the_line(X):
                 assert min(d, 2 * math.pi - d) < 1e-6, (cfg, i, k)
             for k in ("dx", "dy"):
                 assert abs(rows[k][i] - w[k]) < 2e-6 * max(1.0, abs(w[k])), (cfg, i, k)
+            if cfg == 2:                                                         # normal modes (coupling from the tilted magnets?)
+                for k in ("betx1", "bety1", "betx2", "bety2"):
+                    assert abs(rows[k][i] - w[k]) < 3e-5 * max(w["betx1"], w["bety2"], 1.0), (cfg, i, k, rows[k][i], w[k])
+                for k in ("mu1", "mu2"):
+                    d = (rows[k][i] - w[k]) % (2 * math.pi)
+                    assert min(d, 2 * math.pi - d) < 1e-5, (cfg, i, k)
+            else:                                                                # symmetric FODO: equal tunes, no modes
+                assert np.isnan(rows["betx1"][i]) and np.isnan(rows["mu2"][i])
         assert np.all(np.diff(rows["mux"]) > -1e-9) and np.all(np.diff(rows["s"]) >= 0)
         assert abs(rows["betx"][-1] / rows["betx"][0] - 1) < 1e-5 and abs(rows["dx"][-1] - rows["dx"][0]) < 1e-5
         assert abs((rows["mux"][-1] / (2 * math.pi)) % 1.0 - start["qx_frac"]) < 1e-6
         if cfg == 2:
+            assert abs(rows["mu1"][-1] / (2 * math.pi) % 1.0 - want_on["q1_frac"]) < 1e-6
             assert rows["mux"][-1] / (2 * math.pi) > 10.0                       # integer part of the tune included
             print("configs[2] tunes with integer part:", rows["mux"][-1] / (2 * math.pi), rows["muy"][-1] / (2 * math.pi))
+
+
+def test_coupled_optics_along_the_line(X):
+    """A FODO ring with unequal tunes seen from a frame rotated about s (pin P20): the normal-mode functions from
+    the GPU path carry the cos^2 / sin^2 shares at the start and are the ring's own planes inside; with a skew
+    quadrupole they follow the oracle procedure at every element."""
+    from xt_inputs.packed import SRotation
+    kq, L, th = 0.1, 2.0, 0.3
+    ring = [Multipole(knl=(0.0, kq)), Drift(L), Multipole(knl=(0.0, -0.95 * kq)), Drift(L)] * 10
+    lat = X.xt_lattice_create(pack_lattice(ring, P0C, MASS0, 1.0))
+    flat, _ = X.xt_twiss4d_line(lat)
+    lat.close()
+    rot = [SRotation.from_angle(-th)] + ring + [SRotation.from_angle(th)]
+    lat = X.xt_lattice_create(pack_lattice(rot, P0C, MASS0, 1.0))
+    start, rows = X.xt_twiss4d_line(lat)
+    modes = X.xt_twiss4d_normal_form(start["m"])
+    lat.close()
+    c2, s2 = math.cos(th) ** 2, math.sin(th) ** 2
+    assert abs(modes["q1_frac"] - flat["qx_frac"]) < 1e-8 and abs(modes["q2_frac"] - flat["qy_frac"]) < 1e-8
+    for i in (0, len(rot)):
+        assert abs(rows["betx1"][i] - c2 * flat["betx"]) < 1e-5 and abs(rows["bety1"][i] - s2 * flat["betx"]) < 1e-5
+        assert abs(rows["bety2"][i] - c2 * flat["bety"]) < 1e-5 and abs(rows["betx2"][i] - s2 * flat["bety"]) < 1e-5
+    assert np.max(rows["bety1"][1:-1]) < 1e-9 and np.max(rows["betx2"][1:-1]) < 1e-9
+    assert abs(rows["mu1"][-1] / (2 * math.pi) % 1.0 - flat["qx_frac"]) < 1e-7
+    skew = [Multipole(knl=(0.0, 0.0), ksl=(0.0, 0.004))] + ring
+    want_on, want = MO.optics_along(skew, P0C, MASS0, 1.0, list(range(len(skew) + 1)))
+    lat = X.xt_lattice_create(pack_lattice(skew, P0C, MASS0, 1.0))
+    start, rows = X.xt_twiss4d_line(lat)
+    lat.close()
+    assert want_on["bety1"] > 1e-3                                               # really coupled
+    for i, w in enumerate(want):
+        for k in ("betx1", "bety1", "betx2", "bety2"):
+            assert abs(rows[k][i] - w[k]) < 1e-6 * max(w["betx1"], w["bety2"]), (i, k)
+        for k in ("mu1", "mu2"):
+            d = (rows[k][i] - w[k]) % (2 * math.pi)
+            assert min(d, 2 * math.pi - d) < 1e-6, (i, k)

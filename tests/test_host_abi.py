@@ -383,4 +383,39 @@ def test_internal_monitor_type_is_not_a_public_element():
     lib = X.load_library("prod")
     assert lib.xt_lattice_pack_host(buf, len(buf), None, None, 0, None) == -2
     assert lib.xt_twiss4d_line(None, 0.0, 1e-4, None, None, None, 0, None) == -1
-    assert ctypes.sizeof(B.xt_twiss_row) == 15 * 8
+    assert ctypes.sizeof(B.xt_twiss_row) == 21 * 8
+
+
+def test_normal_form_matches_the_oracle_eigen_decomposition():
+    """xt_twiss4d_normal_form is host arithmetic (reciprocal characteristic polynomial, projector eigenvectors):
+    checked here, without a GPU, against oracle/make_optics.normal_form4 (numpy.linalg.eig) on one-turn matrices
+    the oracle tracker produced: uncoupled, seen from a rotated frame, with a skew quadrupole, the LHC-sized ring."""
+    from oracle import make_optics as MO
+    from xt_inputs.packed import SRotation
+    kq, L = 0.1, 2.0
+    ring = [Multipole(knl=(0.0, kq)), Drift(L), Multipole(knl=(0.0, -0.95 * kq)), Drift(L)] * 10
+    cases = [ring, [SRotation.from_angle(-0.3)] + ring + [SRotation.from_angle(0.3)],
+             [Multipole(knl=(0.0, 0.0), ksl=(0.0, 0.004))] + ring, C.lattice(2)]
+    for els in cases:
+        m = MO.optics_of(pack(els))["m"]
+        want, got = MO.normal_form4(m), X.xt_twiss4d_normal_form(m)
+        assert got["stable"] == 1 and got["degenerate"] == 0
+        # the two methods agree to rounding on a symplectic matrix; the central-difference matrix of the big
+        # nonlinear ring is symplectic to 1e-5 only, and the methods split that error differently
+        big = len(els) > 1000
+        scale = max(want["betx1"], want["bety2"])
+        for k in ("q1_frac", "q2_frac"):
+            assert abs(got[k] - want[k]) < (5e-7 if big else 1e-12), k
+        for k in ("betx1", "bety1", "betx2", "bety2", "alfx1", "alfy1", "alfx2", "alfy2"):
+            assert abs(got[k] - want[k]) < (2e-5 if big else 1e-11) * scale, (k, got[k], want[k])
+        for k in ("v1", "v2"):
+            assert np.max(np.abs(got[k] - want[k])) < (2e-5 if big else 1e-11) * np.max(np.abs(want[k])), k
+    # equal tunes (the symmetric FODO ring of configs[0]): flagged, not guessed; an unstable matrix: flagged
+    sym = [Multipole(knl=(0.0, kq)), Drift(L), Multipole(knl=(0.0, -kq)), Drift(L)] * 10
+    got = X.xt_twiss4d_normal_form(MO.optics_of(pack(sym))["m"])
+    assert got["degenerate"] == 1 and got["stable"] == 1 and np.isnan(got["betx1"])
+    bad = np.eye(4)
+    bad[0, 0], bad[1, 1] = 2.0, 0.5
+    got = X.xt_twiss4d_normal_form(bad)
+    assert got["stable"] == 0 and np.isnan(got["q1_frac"])
+    assert X.load_library("prod").xt_twiss4d_normal_form(None, None) == -1
