@@ -36,7 +36,9 @@
 // P14 thick sector bend ('expanded'): second-order limit of thin curved-dipole slices, textbook
 // matrix and dispersion, symplecticity, reversibility; P15 LimitPolygon (even-odd rule): half-plane
 // test on convex polygons, union of rectangles, LimitRect on four corners
-// (tests/test_oracle_refine_pins.py; P16 there pins oracle/refine.py, which tracks with this file).
+// (tests/test_oracle_refine_pins.py; P16 there pins oracle/refine.py, which tracks with this file);
+// P21 mean synchrotron radiation in a thin multipole: U0 of an isomagnetic ring, scaling laws, vertical
+// damping rate U0/2E, proton limit (tests/test_oracle_radiation_pins.py).
 // =====================================================================================
 #include <cmath>
 #include <cstdint>
@@ -53,7 +55,7 @@ constexpr int MAX_ORDER = 20;
 enum ElemType : uint32_t {
   MARKER = 0, DRIFT = 1, MULTIPOLE = 2, CAVITY = 3,
   SROTATION = 4, XYSHIFT = 5, LIMITRECT = 6, LIMITELLIPSE = 7, QUADRUPOLE = 8, BEND = 9,
-  LIMITPOLYGON = 10
+  LIMITPOLYGON = 10, RADMULTIPOLE = 12   // 11 is internal to the CUDA library
 };
 
 struct Element {
@@ -81,6 +83,8 @@ struct Element {
   double k0 = 0.0, h = 0.0;
   // LIMITPOLYGON: vertices (vx[i], vy[i]), closed
   std::vector<double> vx, vy;
+  // RADMULTIPOLE: as MULTIPOLE with c[0] NOT folded, plus krad = (2/3) r0 (beta0 gamma0)^3
+  double krad = 0.0;
 };
 
 struct Lattice {
@@ -202,6 +206,24 @@ int parse(const void* packed, size_t nbytes, Lattice& L) {
         if (!(e.k0 * e.h > 0.0) || !(e.length > 0.0)) return -2;   // focusing strength k0 h must be > 0
         s = s + e.length;
         break;
+      case RADMULTIPOLE: {
+        // Thin multipole that radiates ("mean" model; reading A22): parameters as MULTIPOLE,
+        // length > 0 (the curvature of the trajectory is kick / length).
+        if (aux > static_cast<uint32_t>(MAX_ORDER)) return -2;
+        e.order = static_cast<int>(aux);
+        if (!rd(e.hxl) || !rd(e.length)) return -2;
+        if (!(e.length > 0.0)) return -2;
+        e.c.resize(e.order + 1);
+        e.sn.resize(e.order + 1);
+        for (int n = 0; n <= e.order; ++n) { double v; if (!rd(v)) return -2; e.c[n] = v / factorial(n); }
+        for (int n = 0; n <= e.order; ++n) { double v; if (!rd(v)) return -2; e.sn[n] = v / factorial(n); }
+        e.wf = (e.c[0] * e.hxl) / e.length;
+        // classical radius r0 = q0^2 e^2/(4 pi eps0 m c^2), e^2/(4 pi eps0) = 1.4399645478e-9 eV m (CODATA 2018)
+        const double r0 = ((L.q0 * L.q0) * 1.4399645478e-9) / L.mass0;
+        const double bg0 = L.p0c / L.mass0;
+        e.krad = ((2.0 / 3.0) * r0) * ((bg0 * bg0) * bg0);
+        break;
+      }
       case LIMITPOLYGON:
         if (aux < 3 || aux > 256) return -2;
         e.vx.resize(aux);
@@ -354,6 +376,55 @@ int xo_track(const void* packed, size_t nbytes, const xo_particles* P, int64_t n
               px = e.hxl * delta + px;
               px = px - e.wf * x;
               zeta = zeta - (e.hxl * x) * k.rv0v;
+            }
+            break;
+          }
+
+          case RADMULTIPOLE: {
+            // "Mean" synchrotron radiation ("the energy loss from the radiation is applied
+            // particle by particle without accounting for quantum fluctuations"; "only for the thin lattice
+            // modelling").  Reading A22.  The field of the slice bends the trajectory with
+            // curvature kappa = |kick| P0/(P lpath), lpath = length (1 + h x); the classical power
+            // (2/3) r0 m c^3 beta^4 gamma^4 kappa^2 over the time lpath/(beta c) takes the fraction
+            //   r = (2/3) r0 (beta gamma)^3 kappa^2 lpath = krad (1+delta) kick^2 / lpath
+            // of the particle's energy (beta gamma = beta0 gamma0 (1+delta)).  Half of it is taken before the
+            // kick and half after; each time the energy drops, E' = E (1 - r/2), the momentum follows from
+            // the energy (as behind a cavity) and px, py shrink with it: the photon leaves along the motion.
+            const int N = e.order;
+            double re = e.c[N];
+            double im = e.sn[N];
+            for (int n = N - 1; n >= 0; --n) {
+              const double nre = re * x + (e.c[n] - im * y);
+              const double nim = re * y + (e.sn[n] + im * x);
+              re = nre;
+              im = nim;
+            }
+            const double dpxf = -re - e.wf * x;          // the field's kick (weak focusing included)
+            const double dpyf = im;
+            const double kick2 = dpxf * dpxf + dpyf * dpyf;
+            const double lpath = e.length + e.hxl * x;
+            for (int half = 0; half < 2; ++half) {
+              const double opd = 1.0 + delta;
+              const double rh = ((0.5 * e.krad) * (opd * kick2)) / lpath;
+              ptau = ptau - rh * (ptau + 1.0 / L.beta0);
+              const double t = ptau * (ptau + L.tib);
+              delta = t / (std::sqrt(t + 1.0) + 1.0);
+              const double opd1 = 1.0 + delta;
+              const double f = opd1 / opd;
+              px = px * f;
+              py = py * f;
+              rpp = 1.0 / opd1;
+              const double b = 1.0 + L.beta0 * ptau;
+              rvv = opd1 / b;
+              k.opd2 = opd1 * opd1;
+              k.b = b;
+              k.g = t * L.igam2;
+              k.rv0v = b / opd1;
+              if (half == 0) {                             // the thin kick itself, geometric term included
+                px = (px + dpxf) + e.hxl * opd1;
+                py = py + dpyf;
+                zeta = zeta - (e.hxl * x) * k.rv0v;
+              }
             }
             break;
           }

@@ -197,15 +197,12 @@ extern "C" int xt_twiss4d(const xt_lattice *lat, double delta0, const double *gu
   return done(XT_OK);
 }
 
-extern "C" int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
-                                xt_twiss4d_chrom_result *out, void *cuda_stream) {
-  using namespace xt;
-  if (!out || !(ddelta > 0.0) || !std::isfinite(ddelta)) {
-    set_error("xt_twiss4d_chrom: NULL result or ddelta not > 0");
-    return XT_ERR_INVALID_ARG;
-  }
-  xt_twiss4d_chrom_result res{};
-  xt_twiss4d_result hi{}, lo{};
+namespace xt {
+namespace {
+// The optics at delta0 and the closed orbits / tunes at delta0 -+ ddelta; dispersion and chromaticity from them.
+int chromatic_twiss(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
+                    xt_twiss4d_chrom_result &res, xt_twiss4d_result &hi, xt_twiss4d_result &lo, void *cuda_stream) {
+  res = xt_twiss4d_chrom_result{};
   int rc = xt_twiss4d(lat, delta0, guess4, &res.on, cuda_stream);
   if (rc == XT_OK) rc = xt_twiss4d(lat, delta0 + ddelta, res.on.co, &hi, cuda_stream);
   if (rc == XT_OK) rc = xt_twiss4d(lat, delta0 - ddelta, res.on.co, &lo, cuda_stream);
@@ -219,6 +216,22 @@ extern "C" int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double dde
   };
   res.dqx = slope(hi.qx_frac, lo.qx_frac);
   res.dqy = slope(hi.qy_frac, lo.qy_frac);
+  return XT_OK;
+}
+}  // namespace
+}  // namespace xt
+
+extern "C" int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
+                                xt_twiss4d_chrom_result *out, void *cuda_stream) {
+  using namespace xt;
+  if (!out || !(ddelta > 0.0) || !std::isfinite(ddelta)) {
+    set_error("xt_twiss4d_chrom: NULL result or ddelta not > 0");
+    return XT_ERR_INVALID_ARG;
+  }
+  xt_twiss4d_chrom_result res{};
+  xt_twiss4d_result hi{}, lo{};
+  const int rc = chromatic_twiss(lat, delta0, ddelta, guess4, res, hi, lo, cuda_stream);
+  if (rc != XT_OK) return rc;
   *out = res;
   return XT_OK;
 }
@@ -339,9 +352,7 @@ extern "C" int xt_twiss4d_line(const xt_lattice *lat, double delta0, double ddel
   // the optics at the start and the off-momentum closed orbits
   xt_twiss4d_chrom_result on{};
   xt_twiss4d_result hi{}, lo{};
-  int rc = xt_twiss4d_chrom(lat, delta0, ddelta, guess4, &on, cuda_stream);
-  if (rc == XT_OK) rc = xt_twiss4d(lat, delta0 + ddelta, on.on.co, &hi, cuda_stream);
-  if (rc == XT_OK) rc = xt_twiss4d(lat, delta0 - ddelta, on.on.co, &lo, cuda_stream);
+  int rc = chromatic_twiss(lat, delta0, ddelta, guess4, on, hi, lo, cuda_stream);
   if (rc != XT_OK) return rc;
   if (!on.on.stable) {
     set_error("xt_twiss4d_line: a plane is unstable at the start of the line");

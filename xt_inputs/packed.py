@@ -22,6 +22,8 @@ accelerator element".  Here that sequence is flattened into one little-endian,
                                 PAPER.md:72; k0*h > 0, length > 0; a pure sector bend has k0 = h)
     type 10 LIMITPOLYGON aux=n  x[0..n), y[0..n)   (closed polygon, 3 <= n <= 256 vertices; PAPER.md:178
                                 "polygonal interpolation")
+    type 12 RADMULTIPOLE aux=N  hxl, length, knl[0..N], ksl[0..N]   (thin multipole with "mean" synchrotron
+                                radiation; length > 0)        [type 11 is internal to the library]
 
 This module is pure serialisation (struct packing).  It performs no tracking
 arithmetic: the same bytes are handed to the oracle and to ``xt_lattice_create``;
@@ -40,7 +42,7 @@ HEADER_BYTES = 48
 
 ELEMENT_TYPE_IDS = {
     "Marker": 0, "Drift": 1, "Multipole": 2, "Cavity": 3,
-    "SRotation": 4, "XYShift": 5, "LimitRect": 6, "LimitEllipse": 7, "Quadrupole": 8, "Bend": 9, "LimitPolygon": 10,
+    "SRotation": 4, "XYShift": 5, "LimitRect": 6, "LimitEllipse": 7, "Quadrupole": 8, "Bend": 9, "LimitPolygon": 10, "RadMultipole": 12,
 }
 
 
@@ -128,16 +130,30 @@ class LimitPolygon:
     y: Tuple[float, ...]
 
 
+@dataclass(frozen=True)
+class RadMultipole:
+    """Thin multipole slice that radiates ("mean" model); same parameters as Multipole, length > 0."""
+    knl: Tuple[float, ...]
+    ksl: Tuple[float, ...] = ()
+    hxl: float = 0.0
+    length: float = 1.0
+
+    @property
+    def order(self) -> int:
+        return max(len(self.knl), len(self.ksl), 1) - 1
+
+
 def _record(el) -> bytes:
     if isinstance(el, Marker):
         return struct.pack("<II", 0, 0)
     if isinstance(el, Drift):
         return struct.pack("<IId", 1, 0, el.length)
-    if isinstance(el, Multipole):
+    if isinstance(el, (Multipole, RadMultipole)):
         n = el.order
         knl = list(el.knl) + [0.0] * (n + 1 - len(el.knl))
         ksl = list(el.ksl) + [0.0] * (n + 1 - len(el.ksl))
-        return struct.pack("<II%dd" % (2 + 2 * (n + 1)), 2, n, el.hxl, el.length, *knl, *ksl)
+        return struct.pack("<II%dd" % (2 + 2 * (n + 1)), 12 if isinstance(el, RadMultipole) else 2, n, el.hxl,
+                           el.length, *knl, *ksl)
     if isinstance(el, Cavity):
         return struct.pack("<II3d", 3, 0, el.voltage, el.frequency, el.lag)
     if isinstance(el, SRotation):
@@ -208,6 +224,11 @@ def unpack_lattice(buf: bytes):
         elif t == 9:
             k0, h, length = struct.unpack_from("<3d", buf, off); off += 24
             out.append(Bend(k0, h, length))
+        elif t == 12:
+            m = aux + 1
+            vals = struct.unpack_from("<%dd" % (2 + 2 * m), buf, off); off += 8 * (2 + 2 * m)
+            out.append(RadMultipole(knl=tuple(vals[2:2 + m]), ksl=tuple(vals[2 + m:2 + 2 * m]),
+                                    hxl=vals[0], length=vals[1]))
         elif t == 10:
             vals = struct.unpack_from("<%dd" % (2 * aux), buf, off); off += 16 * aux
             out.append(LimitPolygon(tuple(vals[:aux]), tuple(vals[aux:])))
