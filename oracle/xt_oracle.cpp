@@ -83,7 +83,7 @@ struct Element {
   double k0 = 0.0, h = 0.0;
   // LIMITPOLYGON: vertices (vx[i], vy[i]), closed
   std::vector<double> vx, vy;
-  // RADMULTIPOLE: as MULTIPOLE with c[0] NOT folded, plus krad = (2/3) r0 (beta0 gamma0)^3
+  // RADMULTIPOLE: as MULTIPOLE (c[0] folded, wf from the raw knl[0]), plus krad = (2/3) r0 (beta0 gamma0)^3
   double krad = 0.0;
 };
 
@@ -218,6 +218,7 @@ int parse(const void* packed, size_t nbytes, Lattice& L) {
         for (int n = 0; n <= e.order; ++n) { double v; if (!rd(v)) return -2; e.c[n] = v / factorial(n); }
         for (int n = 0; n <= e.order; ++n) { double v; if (!rd(v)) return -2; e.sn[n] = v / factorial(n); }
         e.wf = (e.c[0] * e.hxl) / e.length;
+        e.c[0] = e.c[0] - e.hxl;      // curvature folded into the dipole coefficient, as in MULTIPOLE (cancellation-free)
         // classical radius r0 = q0^2 e^2/(4 pi eps0 m c^2), e^2/(4 pi eps0) = 1.4399645478e-9 eV m (CODATA 2018)
         const double r0 = ((L.q0 * L.q0) * 1.4399645478e-9) / L.mass0;
         const double bg0 = L.p0c / L.mass0;
@@ -399,7 +400,7 @@ int xo_track(const void* packed, size_t nbytes, const xo_particles* P, int64_t n
               re = nre;
               im = nim;
             }
-            const double dpxf = -re - e.wf * x;          // the field's kick (weak focusing included)
+            const double dpxf = (-re - e.hxl) - e.wf * x;  // the field's kick (re has the curvature folded in; weak focusing included)
             const double dpyf = im;
             const double kick2 = dpxf * dpxf + dpyf * dpyf;
             const double lpath = e.length + e.hxl * x;
@@ -420,9 +421,11 @@ int xo_track(const void* packed, size_t nbytes, const xo_particles* P, int64_t n
               k.b = b;
               k.g = t * L.igam2;
               k.rv0v = b / opd1;
-              if (half == 0) {                             // the thin kick itself, geometric term included
-                px = (px + dpxf) + e.hxl * opd1;
-                py = py + dpyf;
+              if (half == 0) {                             // the thin kick itself, in the arithmetic of MULTIPOLE
+                px = px - re;
+                py = py + im;
+                px = e.hxl * delta + px;
+                px = px - e.wf * x;
                 zeta = zeta - (e.hxl * x) * k.rv0v;
               }
             }
