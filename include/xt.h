@@ -56,8 +56,11 @@ enum {
                       /* (reading A18)             */
   XT_BEND = 9,        /* k0 [1/m], h [1/m], length [m]: thick sector bend, 'expanded' model,     */
                       /* k0*h > 0, length > 0 (reading A19)               */
-  XT_LIMITPOLYGON = 10/* aux = n vertices (3..256); x[0..n), y[0..n): closed polygon, even-odd    */
+  XT_LIMITPOLYGON = 10,/* aux = n vertices (3..256); x[0..n), y[0..n): closed polygon, even-odd   */
                       /* rule, NaN lost ("polygonal"; reading A20)         */
+                      /* 11 is reserved (internal)                                                */
+  XT_RADMULTIPOLE = 12/* parameters as XT_MULTIPOLE, length > 0: thin multipole with "mean"       */
+                      /* synchrotron radiation (reading A22)              */
 };
 
 /* Packed lattice buffer (HOST memory, little-endian, 8-byte aligned records):

@@ -268,6 +268,35 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
         out.extended = true;
         break;
       }
+      case XT_RADMULTIPOLE: {
+        if (aux > XT_MAX_ORDER) {
+          set_error("xt_lattice_create: multipole order exceeds XT_MAX_ORDER");
+          return XT_ERR_BAD_LATTICE;
+        }
+        const int order = static_cast<int>(aux);
+        const double hxl = r.real();
+        const double length = r.real();
+        double knl[XT_MAX_ORDER + 1], ksl[XT_MAX_ORDER + 1];
+        for (int n = 0; n <= order; ++n) knl[n] = r.real();
+        for (int n = 0; n <= order; ++n) ksl[n] = r.real();
+        if (!r.ok) break;
+        if (!(length > 0.0)) {
+          set_error("xt_lattice_create: a radiating multipole needs length > 0");
+          return XT_ERR_BAD_LATTICE;
+        }
+        rec.type = TAG_RMULT;
+        rec.order = aux;
+        rec.p0 = hxl;
+        for (int n = order; n >= 1; --n) rec.slot(knl[n] / factorial(n), ksl[n] / factorial(n));
+        rec.slot(knl[0] - hxl, ksl[0]);             // curvature folded into c[0] as in XT_MULTIPOLE (cancellation-free)
+        rec.slot((knl[0] * hxl) / length, length);  // {wf, length}
+        // (2/3) r0 (beta0 gamma0)^3, r0 = q0^2 e^2/(4 pi eps0 m c^2), e^2/(4 pi eps0) = 1.4399645478e-9 eV m
+        const double r0 = ((q0 * q0) * 1.4399645478e-9) / mass0;
+        const double bg0 = p0c / mass0;
+        rec.slot(((2.0 / 3.0) * r0) * ((bg0 * bg0) * bg0), 0.0);
+        out.extended = true;
+        break;
+      }
       case kMonitorType: {
         if (!opts.allow_monitor) {
           set_error("xt_lattice_create: unknown element type id");

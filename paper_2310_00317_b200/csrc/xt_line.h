@@ -28,7 +28,7 @@ inline int n_params(uint32_t type, uint32_t aux) {
   switch (type) {
     case XT_MARKER: return 0;
     case XT_DRIFT: return 1;
-    case XT_MULTIPOLE: return 2 + 2 * (static_cast<int>(aux) + 1);
+    case XT_MULTIPOLE: case XT_RADMULTIPOLE: return 2 + 2 * (static_cast<int>(aux) + 1);
     case XT_CAVITY: return 3;
     case XT_SROTATION: case XT_XYSHIFT: case XT_LIMITELLIPSE: case XT_QUADRUPOLE: return 2;
     case XT_LIMITRECT: return 4;

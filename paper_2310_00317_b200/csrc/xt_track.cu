@@ -128,6 +128,11 @@ struct BendCase {  // thin kernels keep the dispatch tree they were measured wit
 };
 
 template <bool THICK>
+struct RadCase {
+  static constexpr uint32_t value = THICK ? static_cast<uint32_t>(TAG_RMULT) : 0x5ffu;
+};
+
+template <bool THICK>
 struct MonCase {
   static constexpr uint32_t value = THICK ? static_cast<uint32_t>(TAG_MON) : 0x4ffu;
 };
@@ -562,6 +567,64 @@ __device__ __noinline__ void limit_polygon(Parts<P> &q, const Cold<P> &cold, con
   if (out) lose<P>(q, out, cold, elem, turns_done, a);
 }
 
+// Thin multipole with "mean" synchrotron radiation (reading A22, section 18): the
+// fraction r = krad (1+delta) kick^2 / lpath of the particle's energy is radiated, half before the kick and
+// half after; delta follows from the energy as behind a cavity, px and py shrink with the momentum.
+// slots: (c[n], s[n]) pairs n = N .. 0 with c[0] = knl[0] - hxl, {wf, length}, {krad, 0}.  THICK kernels only.
+template <int P>
+__device__ __noinline__ void rad_multipole(Parts<P> &q, const Cold<P> &cold, const double2 *slots, int order,
+                                           double hxl, const TrackArgs &a) {
+  const double2 wl = slots[order + 1], kr = slots[order + 2];
+  const double ib = 1.0 / a.beta0;
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    if (!(q.alive & (1u << j))) continue;
+    const double x = q.x[j], y = q.y[j];
+    double re = slots[0].x, im = slots[0].y;
+#pragma unroll 1
+    for (int n = 1; n <= order; ++n) {
+      const double2 c = slots[n];
+      const double nre = XT_MADD(re, x, XT_NMADD(im, y, c.x));
+      const double nim = XT_MADD(re, y, XT_MADD(im, x, c.y));
+      re = nre;
+      im = nim;
+    }
+    const double dpxf = XT_NMADD(wl.x, x, -re - hxl);  // the field's kick (re has the curvature folded in)
+    const double dpyf = im;
+    const double kick2 = XT_MADD(dpxf, dpxf, XT_MUL(dpyf, dpyf));
+    const double lpath = XT_MADD(hxl, x, wl.y);
+    double px = q.px[j], py = q.py[j], ptau = cold.ptau(j), delta = cold.delta(j);
+#pragma unroll 1
+    for (int half = 0; half < 2; ++half) {
+      const double opd = 1.0 + delta;
+      const double rh = XT_MUL(0.5 * kr.x, XT_MUL(opd, kick2)) / lpath;
+      ptau = XT_NMADD(rh, ptau + ib, ptau);
+      const double t = XT_MUL(ptau, ptau + a.tib);
+      delta = t / (sqrt(t + 1.0) + 1.0);
+      const double opd1 = 1.0 + delta;
+      const double f = opd1 / opd;
+      px = XT_MUL(px, f);
+      py = XT_MUL(py, f);
+      const double b = XT_MADD(a.beta0, ptau, 1.0);
+      refresh_cached<P>(cold, j, opd1, b, t, a.igam2);
+      if (half == 0) {  // the thin kick itself, in the arithmetic of the plain multipole
+        px = px - re;
+        py = py + im;
+        px = XT_MADD(hxl, delta, px);
+        px = XT_NMADD(wl.x, x, px);
+        q.zeta[j] = XT_NMADD(XT_MUL(hxl, x), cold.rv0v(j), q.zeta[j]);
+      } else {
+        a.p.rpp[cold.idx(j)] = 1.0 / opd1;
+        a.p.rvv[cold.idx(j)] = opd1 / b;
+      }
+    }
+    q.px[j] = px;
+    q.py[j] = py;
+    cold.ptau(j) = ptau;
+    cold.delta(j) = delta;
+  }
+}
+
 // Internal monitor record (xt_twiss4d_line): row p0 of the monitor buffer receives the coordinates of every
 // alive particle of this thread.  THICK kernels only.
 __constant__ double *g_monitor_rows;
@@ -678,6 +741,10 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
       }
       case BendCase<THICK>::value: {  // thick sector bend: p0 = k0, pf[0] = (h, length)
         if (THICK) thick_bend<P>(q, cold, p0, pf[0].x, pf[0].y);
+        break;
+      }
+      case RadCase<THICK>::value: {  // radiating multipole: p0 = hxl
+        if (THICK) rad_multipole<P>(q, cold, slots, static_cast<int>((tag >> 8) & 0x7fu), p0, a);
         break;
       }
       case MonCase<THICK>::value: {

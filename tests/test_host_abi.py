@@ -419,3 +419,20 @@ def test_normal_form_matches_the_oracle_eigen_decomposition():
     got = X.xt_twiss4d_normal_form(bad)
     assert got["stable"] == 0 and np.isnan(got["q1_frac"])
     assert X.load_library("prod").xt_twiss4d_normal_form(None, None) == -1
+
+
+def test_radiating_multipole_is_packed_unfused():
+    from xt_inputs.packed import RadMultipole
+    els = [Drift(1.0), RadMultipole(knl=(2e-3, 0.1, 6.0), ksl=(0.0, 0.01), hxl=1.5e-3, length=4.0), Drift(1.0)]
+    img, info = X.xt_lattice_pack_host(pack(els))
+    (recs,) = walk_image(img, info["chunk_bytes"])
+    assert [r[0] for r in recs] == [T_DRIFT, 13, T_DRIFT]                         # 13 = TAG_RMULT: no drift fused into it
+    slots = list(recs[1][5])
+    assert recs[1][4] == 1.5e-3 and slots[:6] == [3.0, 0.0, 0.1, 0.01, 2e-3 - 1.5e-3, 0.0]   # Horner order, c[0] folded
+    assert slots[6:8] == [(2e-3 * 1.5e-3) / 4.0, 4.0]
+    r0 = 1.4399645478e-9 / 938272088.16
+    assert abs(slots[8] / ((2.0 / 3.0) * r0 * (450e9 / 938272088.16) ** 3) - 1.0) < 1e-14
+    lib = X.load_library("prod")
+    for bad in (RadMultipole(knl=(1e-3,), length=0.0), RadMultipole(knl=(1e-3,), length=-2.0)):
+        b = pack([bad])
+        assert lib.xt_lattice_pack_host(b, len(b), None, None, 0, None) == -2
