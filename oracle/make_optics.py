@@ -77,6 +77,60 @@ def optics_of(buf, delta=0.0, guess=None):
     return out
 
 
+H6 = (1e-6, 1e-8, 1e-6, 1e-8, 1e-5, 1e-8)
+
+
+def track6(buf, pts):
+    """One turn of the rows (x, px, y, py, zeta, delta) of ``pts``."""
+    pts = np.atleast_2d(np.asarray(pts, dtype=np.float64))
+    p = O.new_particles(buf, dict(x=pts[:, 0].copy(), px=pts[:, 1].copy(), y=pts[:, 2].copy(), py=pts[:, 3].copy(),
+                                  zeta=pts[:, 4].copy(), delta=pts[:, 5].copy()))
+    O.track(buf, p, 1)
+    assert np.all(p["state"] == 1)
+    return np.stack([p["x"], p["px"], p["y"], p["py"], p["zeta"], p["delta"]], axis=1)
+
+
+def jac6(buf, z, h=H6):
+    pts = np.tile(np.asarray(z, dtype=np.float64), (12, 1))
+    for i in range(6):
+        pts[2 * i, i] += h[i]
+        pts[2 * i + 1, i] -= h[i]
+    out = track6(buf, pts)
+    J = np.zeros((6, 6))
+    for i in range(6):
+        J[:, i] = (out[2 * i] - out[2 * i + 1]) / (2 * h[i])
+    return J
+
+
+def optics6d_of(buf, guess=None):
+    """The paper's steps 1-3 in all six dimensions (a ring with an RF cavity): closed orbit
+    by Newton on (x, px, y, py, zeta, delta), the 6x6 Jacobian there by central differences, and the three
+    tunes from its eigenvalues exp(+-i mu_k): the synchrotron tune qs is the smallest angle (reported in
+    (0, 1/2)); of the other two, q1 is the one whose cos mu is closer to that of the horizontal 2x2 block;
+    their side of the half integer is read from the sign of that block's M12, as in ``optics_of``."""
+    z = np.zeros(6) if guess is None else np.asarray(guess, dtype=np.float64).copy()
+    for _ in range(20):
+        J = jac6(buf, z)
+        r = track6(buf, z)[0] - z
+        dz = np.linalg.solve(J - np.eye(6), -r)
+        z = z + dz
+        if np.max(np.abs(dz)) < 1e-12:
+            break
+    J = jac6(buf, z)
+    lam = np.linalg.eigvals(J)
+    assert np.all(np.abs(np.abs(lam) - 1.0) < 1e-5), "unstable"
+    ang = sorted(set(round(abs(math.atan2(l.imag, l.real)), 9) for l in lam))
+    assert len(ang) == 3
+    out = {"co": z, "m": J, "qs": ang[0] / (2 * math.pi)}
+    rest = ang[1:]
+    cx = 0.5 * (J[0, 0] + J[1, 1])
+    if abs(math.cos(rest[0]) - cx) > abs(math.cos(rest[1]) - cx):
+        rest = rest[::-1]
+    for name, a, i in (("q1_frac", rest[0], 0), ("q2_frac", rest[1], 2)):
+        out[name] = (math.copysign(a, J[i, i + 1]) / (2 * math.pi)) % 1.0
+    return out
+
+
 S4 = np.array([[0.0, 1.0, 0.0, 0.0], [-1.0, 0.0, 0.0, 0.0], [0.0, 0.0, 0.0, 1.0], [0.0, 0.0, -1.0, 0.0]])
 
 

@@ -762,3 +762,30 @@ def test_P20_normal_form_uncoupled_rotated_and_closest_tune_approach():
     for rr in (rows_r[0], rows_r[-1]):
         assert abs(rr["betx1"] - c2 * rows[0]["betx"]) < 1e-5 and abs(rr["bety1"] - s2 * rows[0]["betx"]) < 1e-5
         assert abs(rr["bety2"] - c2 * rows[0]["bety"]) < 1e-5 and abs(rr["betx2"] - s2 * rows[0]["bety"]) < 1e-5
+
+
+# ----------------------------- P22 six-dimensional closed orbit and tunes
+def test_P22_six_dimensional_closed_orbit_and_synchrotron_tune():
+    """oracle/make_optics.optics6d_of: (a) drifts + cavity (pin P11's ring): cos mu_s = 1 - A B / 2 in closed
+    form; (b) a cavity phased away from zero moves the fixed point to zeta = lag / kz; (c) a thin FODO ring with
+    a cavity and no bends: the transverse tunes are the FODO closed form, the synchrotron tune the same formula."""
+    from oracle import make_optics as MO
+    p0c, volt, freq, circ = 1.0e9, 1e5, 200e6, 40.0
+    buf = pack([Drift(circ / 4)] * 4 + [Cavity(volt, freq, 0.0)], p0c=p0c)
+    beta0, gamma0 = O.reference(buf)
+    kz = 2 * math.pi * freq / (beta0 * 299792458.0)
+    A, B = circ / gamma0 ** 2, (volt / p0c) * kz / beta0
+    # no transverse focusing at all: only the longitudinal 2x2 block of the 6x6 matrix is an oscillator
+    J = MO.jac6(buf, np.zeros(6))
+    mu_s = math.acos(1.0 - A * B / 2.0)
+    assert abs(0.5 * (J[4, 4] + J[5, 5]) - math.cos(mu_s)) < 1e-9
+    cell = [Multipole(knl=(0.0, 0.1)), Drift(2.0), Multipole(knl=(0.0, -0.095)), Drift(2.0)]
+    for lag in (0.0, 25.0):
+        buf = pack(cell * 10 + [Cavity(volt, freq, lag)], p0c=p0c)
+        got = MO.optics6d_of(buf)
+        np.testing.assert_allclose(got["co"][:4], 0.0, atol=1e-13)
+        assert abs(got["co"][4] - math.radians(lag) / kz) < 1e-10 and abs(got["co"][5]) < 1e-13
+        assert abs(got["qs"] - mu_s / (2 * math.pi)) < 1e-9
+        flat = MO.optics_of(pack(cell * 10, p0c=p0c))
+        assert abs(got["q1_frac"] - flat["qx_frac"]) < 1e-8 and abs(got["q2_frac"] - flat["qy_frac"]) < 1e-8
+    assert abs(flat["qx_frac"] - flat["qy_frac"]) > 0.01
