@@ -256,6 +256,24 @@ typedef struct {
 int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
                      xt_twiss4d_chrom_result *out, void *cuda_stream);
 
+/* Twiss steps 1-3 in six dimensions for a ring with an RF cavity ("6x6 Jacobian by
+ * central differences (13 particles through xt_track)"): Newton on (x, px, y, py, zeta, delta)
+ * with one launch of thirteen probes per step (steps 1e-6 m, 1e-8, 1e-6 m, 1e-8, 1e-5 m, 1e-8), the 6x6
+ * Jacobian at the fixed point, and the three tunes from its reciprocal characteristic polynomial: with
+ * u = lambda + 1/lambda the cubic u^3 - s1 u^2 + s2 u - s3 = 0 (s1 = e1, s2 = e2 - 3, s3 = e3 - 2 e1, e_k the
+ * elementary symmetric functions from the traces of M, M^2, M^3) has the roots 2 cos mu_k.  qs = the smallest
+ * angle / 2 pi, in (0, 1/2); q1 (q2) = the remaining one closer to the horizontal (vertical) 2x2 block, its side
+ * of the half integer from the sign of that block's M12.  guess6 (HOST, may be NULL = origin).
+ * XT_ERR_UNSTABLE: probe lost, no convergence in 25 steps, M - 1 singular (no cavity), or a root outside
+ * (-2, 2).  Synchronises the stream. */
+typedef struct {
+  double co[6];  /* x, px, y, py, zeta, delta */
+  double m[36];  /* row-major, in these variables */
+  double q1_frac, q2_frac, qs;
+  int32_t iterations, reserved;
+} xt_twiss6d_result;
+int xt_twiss6d(const xt_lattice *lat, const double *guess6, xt_twiss6d_result *out, void *cuda_stream);
+
 /* Linear normal form of a 4x4 one-turn matrix with coupling (PAPER.md:98 step 3 "from the eigenvalues and
  * eigenvectors of the Jacobian matrix", step 5 "Mais-Ripken").  Pure HOST arithmetic,
  * no CUDA call.  m: row-major, e.g. xt_twiss4d_result.m.  The characteristic polynomial of a symplectic

@@ -59,6 +59,12 @@ class xt_twiss4d_chrom_result(ctypes.Structure):
                 [(k, ctypes.c_double) for k in ("dx", "dpx", "dy", "dpy", "dqx", "dqy")])
 
 
+class xt_twiss6d_result(ctypes.Structure):
+    _fields_ = [("co", ctypes.c_double * 6), ("m", ctypes.c_double * 36), ("q1_frac", ctypes.c_double),
+                ("q2_frac", ctypes.c_double), ("qs", ctypes.c_double), ("iterations", ctypes.c_int32),
+                ("reserved", ctypes.c_int32)]
+
+
 class xt_twiss_row(ctypes.Structure):
     _fields_ = [(k, ctypes.c_double) for k in ("s", "x", "px", "y", "py", "betx", "alfx", "mux", "bety", "alfy",
                                                 "muy", "dx", "dpx", "dy", "dpy", "betx1", "bety1", "betx2", "bety2",
@@ -114,6 +120,7 @@ SIGNATURES = {
                                                ctypes.c_int32, ctypes.POINTER(ctypes.c_int64), _VP]),
     "xt_twiss4d_chrom": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
                                         ctypes.POINTER(xt_twiss4d_chrom_result), _VP]),
+    "xt_twiss6d": (ctypes.c_int, [_VP, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(xt_twiss6d_result), _VP]),
     "xt_twiss4d_normal_form": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(xt_twiss4d_modes)]),
     "xt_twiss4d_line": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
                                        ctypes.POINTER(xt_twiss4d_chrom_result), ctypes.POINTER(xt_twiss_row), _I64,
@@ -413,6 +420,15 @@ def xt_twiss4d_chrom(lat: Lattice, delta0: float = 0.0, ddelta: float = 1e-4, gu
     for k in ("dx", "dpx", "dy", "dpy", "dqx", "dqy"):
         out[k] = getattr(res, k)
     return out
+
+
+def xt_twiss6d(lat: Lattice, guess6=None, stream=None) -> Dict:
+    """Six-dimensional closed orbit, 6x6 one-turn matrix and the three tunes (include/xt.h)."""
+    res = xt_twiss6d_result()
+    g = (ctypes.c_double * 6)(*[float(v) for v in guess6]) if guess6 is not None else None
+    _check(lat._lib, lat._lib.xt_twiss6d(lat.handle, g, ctypes.byref(res), _stream_ptr(stream)))
+    return dict(co=np.array(list(res.co)), m=np.array(list(res.m)).reshape(6, 6), q1_frac=res.q1_frac,
+                q2_frac=res.q2_frac, qs=res.qs, iterations=res.iterations)
 
 
 def xt_twiss4d_normal_form(m, kind: str = "prod") -> Dict:

@@ -9,6 +9,7 @@
 // 4 x 4 linear algebra runs on the host.
 #include <cmath>
 
+#include <algorithm>
 #include <complex>
 #include <vector>
 
@@ -485,5 +486,194 @@ extern "C" int xt_twiss4d_line(const xt_lattice *lat, double delta0, double ddel
     for (int c = 0; c < 4; ++c) *dd[c] = (r[9 * 6 + c] - r[10 * 6 + c]) / (2.0 * ddelta);
   }
   if (start) *start = on;
+  return done(XT_OK);
+}
+
+namespace xt {
+namespace {
+constexpr int kProbe6 = 13;
+constexpr double kStep6[6] = {1e-6, 1e-8, 1e-6, 1e-8, 1e-5, 1e-8};
+
+// One launch: the orbit z and its twelve neighbours for one turn (x, px, y, py, zeta, delta).
+int one_turn_and_jacobian6(const xt_lattice *lat, double *d_f64, int64_t *d_i64, const double z[6], double out[6],
+                           double jac[36], cudaStream_t st) {
+  double h[10][16] = {};
+  for (int k = 0; k < kProbe6; ++k)
+    for (int c = 0; c < 6; ++c) h[c][k] = z[c];
+  for (int c = 0; c < 6; ++c) {
+    h[c][1 + 2 * c] += kStep6[c];
+    h[c][2 + 2 * c] -= kStep6[c];
+  }
+  int64_t hi64[3][16] = {};
+  for (int k = 0; k < kProbe6; ++k) hi64[1][k] = 1;
+  XT_CUDA(cudaMemcpyAsync(d_f64, h, sizeof(h), cudaMemcpyHostToDevice, st));
+  XT_CUDA(cudaMemcpyAsync(d_i64, hi64, sizeof(hi64), cudaMemcpyHostToDevice, st));
+  xt_particles p{};
+  double **d[10] = {&p.x, &p.px, &p.y, &p.py, &p.zeta, &p.delta, &p.ptau, &p.rpp, &p.rvv, &p.s};
+  for (int k = 0; k < 10; ++k) *d[k] = d_f64 + 16 * k;
+  p.at_turn = d_i64;
+  p.state = d_i64 + 16;
+  p.at_element = d_i64 + 32;
+  int rc = launch_init_derived(lat, p, kProbe6, st);
+  if (rc != XT_OK) return rc;
+  if ((rc = xt_track(lat, &p, kProbe6, 1, st)) != XT_OK) return rc;
+  double r[6][16];
+  int64_t state[16];
+  XT_CUDA(cudaMemcpyAsync(r, d_f64, sizeof(r), cudaMemcpyDeviceToHost, st));
+  XT_CUDA(cudaMemcpyAsync(state, d_i64 + 16, sizeof(state), cudaMemcpyDeviceToHost, st));
+  XT_CUDA(cudaStreamSynchronize(st));
+  for (int k = 0; k < kProbe6; ++k) {
+    bool ok = state[k] == 1;
+    for (int c = 0; c < 6; ++c) ok = ok && std::isfinite(r[c][k]);
+    if (!ok) {
+      set_error("xt_twiss6d: a probe particle was lost or became non-finite");
+      return XT_ERR_UNSTABLE;
+    }
+  }
+  for (int row = 0; row < 6; ++row) {
+    out[row] = r[row][0];
+    for (int c = 0; c < 6; ++c) jac[6 * row + c] = (r[row][1 + 2 * c] - r[row][2 + 2 * c]) / (2.0 * kStep6[c]);
+  }
+  return XT_OK;
+}
+
+int solve6(double a[6][7]) {  // Gaussian elimination with partial pivoting on [A | b]
+  for (int c = 0; c < 6; ++c) {
+    int piv = c;
+    for (int r = c + 1; r < 6; ++r)
+      if (std::fabs(a[r][c]) > std::fabs(a[piv][c])) piv = r;
+    if (std::fabs(a[piv][c]) < 1e-300) return -1;
+    if (piv != c)
+      for (int k = 0; k < 7; ++k) std::swap(a[piv][k], a[c][k]);
+    for (int r = c + 1; r < 6; ++r) {
+      const double f = a[r][c] / a[c][c];
+      for (int k = c; k < 7; ++k) a[r][k] -= f * a[c][k];
+    }
+  }
+  for (int r = 5; r >= 0; --r) {
+    double s = a[r][6];
+    for (int k = r + 1; k < 6; ++k) s -= a[r][k] * a[k][6];
+    a[r][6] = s / a[r][r];
+  }
+  return 0;
+}
+}  // namespace
+}  // namespace xt
+
+extern "C" int xt_twiss6d(const xt_lattice *lat, const double *guess6, xt_twiss6d_result *out, void *cuda_stream) {
+  using namespace xt;
+  if (!lat || !out) {
+    set_error("xt_twiss6d: NULL lattice or result");
+    return XT_ERR_INVALID_ARG;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  double *d_f64 = nullptr;
+  int64_t *d_i64 = nullptr;
+  XT_CUDA(cudaMalloc(&d_f64, 10 * 16 * sizeof(double)));
+  cudaError_t e = cudaMalloc(&d_i64, 3 * 16 * sizeof(int64_t));
+  if (e != cudaSuccess) {
+    cudaFree(d_f64);
+    return cuda_fail(e, "cudaMalloc(probe)");
+  }
+  auto done = [&](int code) {
+    cudaFree(d_f64);
+    cudaFree(d_i64);
+    return code;
+  };
+  xt_twiss6d_result res{};
+  double z[6] = {0, 0, 0, 0, 0, 0}, img[6], jac[36];
+  if (guess6)
+    for (int c = 0; c < 6; ++c) z[c] = guess6[c];
+  int rc;
+  bool converged = false;
+  for (int it = 0; it < 25; ++it) {
+    if ((rc = one_turn_and_jacobian6(lat, d_f64, d_i64, z, img, jac, st)) != XT_OK) return done(rc);
+    double a[6][7];
+    for (int r = 0; r < 6; ++r) {
+      for (int c = 0; c < 6; ++c) a[r][c] = jac[6 * r + c] - (r == c ? 1.0 : 0.0);
+      a[r][6] = -(img[r] - z[r]);
+    }
+    // without a cavity delta is invariant and zeta slips: the row of delta in M - 1 vanishes
+    double row5 = 0.0;
+    for (int c = 0; c < 6; ++c) row5 = std::fmax(row5, std::fabs(a[5][c]));
+    if (row5 < 1e-12 || solve6(a) != 0) {
+      set_error("xt_twiss6d: one-turn matrix minus identity is singular (no RF cavity, or an integer tune)");
+      return done(XT_ERR_UNSTABLE);
+    }
+    double step = 0.0;
+    for (int c = 0; c < 6; ++c) {
+      z[c] += a[c][6];
+      step = std::fmax(step, std::fabs(a[c][6]));
+    }
+    res.iterations = it + 1;
+    if (step < 1e-12) {
+      converged = true;
+      break;
+    }
+  }
+  if (!converged) {
+    set_error("xt_twiss6d: closed-orbit search did not converge in 25 Newton steps");
+    return done(XT_ERR_UNSTABLE);
+  }
+  if ((rc = one_turn_and_jacobian6(lat, d_f64, d_i64, z, img, jac, st)) != XT_OK) return done(rc);
+  for (int c = 0; c < 6; ++c) res.co[c] = z[c];
+  for (int k = 0; k < 36; ++k) res.m[k] = jac[k];
+  // traces of M, M^2, M^3 -> elementary symmetric functions -> the cubic in u = lambda + 1/lambda
+  double m2[36], m3[36];
+  auto mul = [](const double *x, const double *y, double *o) {
+    for (int r = 0; r < 6; ++r)
+      for (int c = 0; c < 6; ++c) {
+        double s = 0.0;
+        for (int k = 0; k < 6; ++k) s += x[6 * r + k] * y[6 * k + c];
+        o[6 * r + c] = s;
+      }
+  };
+  mul(jac, jac, m2);
+  mul(m2, jac, m3);
+  double t1 = 0, t2 = 0, t3 = 0;
+  for (int k = 0; k < 6; ++k) {
+    t1 += jac[7 * k];
+    t2 += m2[7 * k];
+    t3 += m3[7 * k];
+  }
+  const double e1 = t1, e2 = 0.5 * (e1 * t1 - t2), e3 = (e2 * t1 - e1 * t2 + t3) / 3.0;
+  const double s1 = e1, s2 = e2 - 3.0, s3 = e3 - 2.0 * e1;
+  // u = w + s1/3: w^3 + p w + q = 0, three real roots by the trigonometric form
+  const double pp = s2 - s1 * s1 / 3.0, qq = -2.0 * s1 * s1 * s1 / 27.0 + s1 * s2 / 3.0 - s3;
+  double u[3];
+  if (!(pp < 0.0)) {
+    set_error("xt_twiss6d: the one-turn matrix has no three distinct stable modes");
+    return done(XT_ERR_UNSTABLE);
+  }
+  const double amp = 2.0 * std::sqrt(-pp / 3.0);
+  double arg = 3.0 * qq / (pp * amp);
+  if (std::fabs(arg) > 1.0 + 1e-9) {
+    set_error("xt_twiss6d: complex eigenvalue pair off the unit circle (unstable)");
+    return done(XT_ERR_UNSTABLE);
+  }
+  arg = std::fmax(-1.0, std::fmin(1.0, arg));
+  const double th = std::acos(arg) / 3.0;
+  for (int k = 0; k < 3; ++k) u[k] = amp * std::cos(th - 2.0 * 3.14159265358979323846 * k / 3.0) + s1 / 3.0;
+  double ang[3];
+  for (int k = 0; k < 3; ++k) {
+    if (!(std::fabs(u[k]) < 2.0)) {
+      set_error("xt_twiss6d: an eigenvalue pair is off the unit circle (unstable)");
+      return done(XT_ERR_UNSTABLE);
+    }
+    ang[k] = std::acos(0.5 * u[k]);
+  }
+  std::sort(ang, ang + 3);
+  const double two_pi = 2.0 * 3.14159265358979323846;
+  res.qs = ang[0] / two_pi;
+  const double cx = 0.5 * (jac[0] + jac[7]);
+  double a1 = ang[1], a2 = ang[2];
+  if (std::fabs(std::cos(a1) - cx) > std::fabs(std::cos(a2) - cx)) std::swap(a1, a2);
+  auto frac = [&](double a, double m12) {
+    double f = std::copysign(a, m12) / two_pi;
+    return f - std::floor(f);
+  };
+  res.q1_frac = frac(a1, jac[1]);
+  res.q2_frac = frac(a2, jac[6 * 2 + 3]);
+  *out = res;
   return done(XT_OK);
 }

@@ -233,3 +233,45 @@ def test_coupled_optics_along_the_line(X):
         for k in ("mu1", "mu2"):
             d = (rows[k][i] - w[k]) % (2 * math.pi)
             assert min(d, 2 * math.pi - d) < 1e-6, (i, k)
+
+
+def test_six_dimensional_twiss(X):
+    """xt_twiss6d: the closed forms of pin P22 (synchrotron tune of a cavity in a ring without bends, fixed point at
+    zeta = lag/kz, FODO tunes) and the oracle procedure (make_optics.optics6d_of) on the LHC-sized configs[2] and
+    configs[3] with their eight cavities; a ring without a cavity is reported, not solved."""
+    from xt_inputs.packed import Cavity
+    from oracle import oracle as O
+    p0c, volt, freq = 1.0e9, 1e5, 200e6
+    cell = [Multipole(knl=(0.0, 0.1)), Drift(2.0), Multipole(knl=(0.0, -0.095)), Drift(2.0)]
+    for lag in (0.0, 25.0):
+        buf = pack_lattice(cell * 10 + [Cavity(volt, freq, lag)], p0c, MASS0, 1.0)
+        beta0, gamma0 = O.reference(buf)
+        kz = 2 * math.pi * freq / (beta0 * 299792458.0)
+        A, B = 40.0 / gamma0 ** 2, (volt / p0c) * kz / beta0
+        lat = X.xt_lattice_create(buf)
+        tw = X.xt_twiss6d(lat)
+        flat = X.xt_twiss4d(lat)
+        lat.close()
+        assert abs(tw["qs"] - math.acos(1.0 - A * B / 2.0) / (2 * math.pi)) < 1e-8
+        assert abs(tw["co"][4] - math.radians(lag) / kz) < 1e-9 and np.max(np.abs(tw["co"][[0, 1, 2, 3, 5]])) < 1e-12
+        assert abs(tw["q1_frac"] - flat["qx_frac"]) < 1e-7 and abs(tw["q2_frac"] - flat["qy_frac"]) < 1e-7
+    for cfg in (2, 3):
+        buf = C.pack(C.lattice(cfg))
+        want = MO.optics6d_of(buf)
+        lat = X.xt_lattice_create(buf)
+        tw = X.xt_twiss6d(lat)
+        lat.close()
+        np.testing.assert_allclose(tw["co"][:4], want["co"][:4], atol=1e-10)
+        assert abs(tw["co"][4] - want["co"][4]) < 1e-8 and abs(tw["co"][5] - want["co"][5]) < 1e-10
+        for k in ("q1_frac", "q2_frac"):
+            assert abs(tw[k] - want[k]) < 2e-6, (cfg, k, tw[k], want[k])
+        assert abs(tw["qs"] - want["qs"]) < 1e-7 and 0 < tw["qs"] < 0.1, (cfg, tw["qs"], want["qs"])
+        print("configs[%d]: q1 %.6f q2 %.6f qs %.6f, %d Newton steps" % (cfg, tw["q1_frac"], tw["q2_frac"], tw["qs"], tw["iterations"]))
+    # no cavity: singular; configs[0] (no bends, cavity at lag 180 deg: below transition that is the unstable phase,
+    # the longitudinal eigenvalues are real, 1 -+ 4e-5): reported
+    for buf in (pack_lattice(cell * 10, p0c, MASS0, 1.0), C.pack(C.lattice(0))):
+        lat = X.xt_lattice_create(buf)
+        with pytest.raises(X.XtError) as e:
+            X.xt_twiss6d(lat)
+        assert e.value.code == -5
+        lat.close()
