@@ -10,9 +10,9 @@ obtained by polygonal interpolation (an example is shown in Fig. 4)" -- Fig. 4 (
 tilted with respect to each other".
 
 The paper gives no further detail; reading A20 fixes the procedure, followed here
-step by step for every lost particle whose ``at_element`` is a LimitRect / LimitEllipse ``l``:
+step by step for every lost particle whose ``at_element`` is a LimitRect / LimitEllipse / LimitPolygon ``l``:
 
- 1. Upstream aperture ``u``: the nearest LimitRect / LimitEllipse before ``l`` in the line; if
+ 1. Upstream aperture ``u``: the nearest LimitRect / LimitEllipse / LimitPolygon before ``l`` in the line; if
     there is none, the start of the line (s = 0) with the cross-section of ``l`` itself.  If no
     length lies between the two, nothing is refined.
  2. Frames: XYShift / SRotation elements are changes of the reference system.  The
@@ -23,7 +23,8 @@ step by step for every lost particle whose ``at_element`` is a LimitRect / Limit
     (machine frame) at the machine-frame angles phi_k = 2 pi k / n_poly: V_k = C + r_k (cos phi_k,
     sin phi_k); with u = R (cos phi_k, sin phi_k) the local direction, r_k = 1/sqrt((ux/a)^2 +
     (uy/b)^2) for an ellipse and min(hx/|ux|, hy/|uy|) for a rectangle of half widths hx, hy
-    about its centre.
+    about its centre; for a polygon the centre is the mean of its vertices and r_k the smallest
+    positive distance at which the ray meets an edge.
  4. Backtracking: the maps are reversible (reading A11, pins P6, P13, P14): flip (px, py, zeta),
     track through the elements between u and l in reverse order (cavity lag, rotation angle and
     shifts negated; apertures dropped), flip again.  The result is the particle just after u.
@@ -47,7 +48,7 @@ import numpy as np
 from oracle import oracle as O
 from xt_inputs import packed as PK
 
-APERTURES = (PK.LimitRect, PK.LimitEllipse)
+APERTURES = (PK.LimitRect, PK.LimitEllipse, PK.LimitPolygon)
 STATE_KEYS = ("x", "px", "y", "py", "zeta", "delta", "ptau", "rpp", "rvv")
 
 
@@ -77,6 +78,8 @@ def aperture_polygon(el, frame, n_poly: int) -> Tuple[np.ndarray, np.ndarray]:
     if isinstance(el, PK.LimitRect):
         cx, cy = 0.5 * (el.min_x + el.max_x), 0.5 * (el.min_y + el.max_y)
         hx, hy = 0.5 * (el.max_x - el.min_x), 0.5 * (el.max_y - el.min_y)
+    elif isinstance(el, PK.LimitPolygon):
+        cx, cy = sum(el.x) / len(el.x), sum(el.y) / len(el.y)
     else:
         cx, cy = 0.0, 0.0
     # centre in the machine frame: m = R^T (local - t)
@@ -91,6 +94,22 @@ def aperture_polygon(el, frame, n_poly: int) -> Tuple[np.ndarray, np.ndarray]:
             rx = hx / abs(ux) if ux != 0.0 else math.inf
             ry = hy / abs(uy) if uy != 0.0 else math.inf
             r = min(rx, ry)
+        elif isinstance(el, PK.LimitPolygon):
+            # the ray c + r u meets the edge a + t (b - a), 0 <= t <= 1, where cross(u, e) != 0:
+            # r = cross(a - c, e) / cross(u, e),  t = cross(a - c, u) / cross(u, e)
+            r = math.inf
+            nv = len(el.x)
+            for i in range(nv):
+                ax, ay = el.x[i] - cx, el.y[i] - cy
+                ex, ey = el.x[(i + 1) % nv] - el.x[i], el.y[(i + 1) % nv] - el.y[i]
+                den = ux * ey - uy * ex
+                if den == 0.0:
+                    continue
+                rr = (ax * ey - ay * ex) / den
+                t = (ax * uy - ay * ux) / den
+                if rr > 0.0 and 0.0 <= t <= 1.0 and rr < r:
+                    r = rr
+            assert math.isfinite(r), "the polygon does not surround the mean of its vertices"
         else:
             r = 1.0 / math.sqrt((ux / el.a) * (ux / el.a) + (uy / el.b) * (uy / el.b))
         vx[k], vy[k] = mx + r * dx, my + r * dy
@@ -101,7 +120,7 @@ def reversed_elements(elements: Sequence) -> List:
     """Step 4 (reading A11): reverse order; cavity lag, rotation angle, shifts negated; apertures dropped."""
     out = []
     for el in reversed(elements):
-        if isinstance(el, APERTURES) or isinstance(el, PK.LimitPolygon):
+        if isinstance(el, APERTURES):
             continue
         if isinstance(el, PK.Cavity):
             out.append(PK.Cavity(el.voltage, el.frequency, -el.lag))
@@ -119,7 +138,7 @@ def sliced_elements(elements: Sequence, frames: Sequence, poly_u, poly_l, seg_le
     out, sloc_of = [], []
     sloc = 0.0
     for el, fr in zip(elements, frames):
-        if isinstance(el, APERTURES) or isinstance(el, PK.LimitPolygon):
+        if isinstance(el, APERTURES):
             continue
         length = element_length(el)
         if length > 0.0:

@@ -299,3 +299,38 @@ def test_P16_four_rays_cut_a_diamond_out_of_a_square_pipe():
     # with 8 rays the corners are vertices too: the first particle (on the x axis) leaves at x = h exactly
     p8, _, _, _ = lose_and_refine(els, rows[:1], ds, 8, 2)
     assert abs(p8["s"][0] - first_grid_point(h / vx[0], piece)) < 1e-9
+
+
+def test_P16_polygon_apertures_as_end_points():
+    """A rectangle given by its four corners and an ellipse given by 64 points on it are refined like the
+    LimitRect / LimitEllipse they describe (the rays meet the same boundary; the 64-gon is inscribed, so a loss
+    may be flagged one slice earlier at most), shifted and tilted brackets included."""
+    L, ds, n_poly = 12.0, 0.1, 64
+    th1, th2 = 0.3, -0.2
+    ang = 2 * np.pi * np.arange(64) / 64
+
+    def line(first, last):
+        return [XYShift(1e-3, -2e-3), SRotation.from_angle(th1), first, SRotation.from_angle(-th1), XYShift(-1e-3, 2e-3),
+                Drift(L / 3), Multipole(knl=(0.0, 0.01)), Drift(2 * L / 3), SRotation.from_angle(th2), XYShift(-2e-3, 1e-3),
+                last, XYShift(2e-3, -1e-3), SRotation.from_angle(-th2)]
+
+    rect, ell = LimitRect(-0.02, 0.015, -0.01, 0.012), LimitEllipse(0.012, 0.008)
+    rect_p = LimitPolygon((-0.02, 0.015, 0.015, -0.02), (-0.01, -0.01, 0.012, 0.012))
+    ell_p = LimitPolygon(tuple(0.012 * np.cos(ang)), tuple(0.008 * np.sin(ang)))
+    rows = rays(40, 4, 0.004)
+    ref, _, moved, mm = lose_and_refine(line(rect, ell), rows, ds, n_poly, 10)
+    # the mean of the four corners is the rectangle's midpoint: same centre, same rays, same boundary points
+    a, _, moved_a, mm_a = lose_and_refine(line(rect_p, ell), rows, ds, n_poly, 10)
+    clear = (mm > 1e-9) & (mm_a > 1e-9)
+    assert moved_a == moved and clear.sum() >= 38
+    np.testing.assert_allclose(a["s"][clear], ref["s"][clear], rtol=0, atol=1e-12)
+    np.testing.assert_allclose(a["x"][clear], ref["x"][clear], rtol=0, atol=1e-15)
+    # the flagging aperture as a 64-gon: particles between the polygon and the ellipse are lost on it but not on
+    # the ellipse, so compare the ones both lines lose there
+    p = particles(line(rect, ell_p), rows)
+    O.track(pack(line(rect, ell_p)), p, 1)
+    assert np.all(p["state"] == 0) and np.all(p["at_element"] == 10)
+    moved_b = R.refine_loss_location(line(rect, ell_p), H.P0C, H.MASS0, H.Q0, p, ds, n_poly)
+    assert moved_b == len(rows)
+    assert np.all(p["s"] <= ref["s"] + 1e-12) and np.all(ref["s"] - p["s"] <= ds + 1e-12)
+    assert (np.abs(p["s"] - ref["s"]) < 1e-12).mean() > 0.9
