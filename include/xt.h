@@ -207,7 +207,7 @@ int xt_twiss4d(const xt_lattice *lat, double delta0, const double *guess4, xt_tw
 /* Loss-location refinement ("particle backtracking and a locally
  * refined aperture model obtained by polygonal interpolation", Fig. 4; reading A20 and
  * section 16).  For every particle of `p` (DEVICE, as left by xt_track on `lat`) with state == 0 whose
- * at_element is a LimitRect / LimitEllipse with length between it and the previous such aperture (or
+ * at_element is a LimitRect / LimitEllipse / LimitPolygon with length between it and the previous aperture (or
  * the start of the line): the particle is tracked back to that upstream aperture and forward again in
  * steps of at most `ds` [m] through polygons of `n_poly` vertices (3..256) interpolated between the
  * two apertures, shifts and tilts included; x, px, y, py, zeta, delta, ptau, rpp, rvv and s are

@@ -19,8 +19,8 @@ struct Elem {
     if (type == XT_BEND) return v[2];
     return 0.0;
   }
-  bool is_aperture() const { return type == XT_LIMITRECT || type == XT_LIMITELLIPSE; }
-  bool is_any_aperture() const { return is_aperture() || type == XT_LIMITPOLYGON; }
+  bool is_aperture() const { return type == XT_LIMITRECT || type == XT_LIMITELLIPSE || type == XT_LIMITPOLYGON; }
+  bool is_any_aperture() const { return is_aperture(); }
 };
 
 // number of doubles behind the 8-byte element header (include/xt.h, element table)

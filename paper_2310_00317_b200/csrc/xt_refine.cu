@@ -51,8 +51,9 @@ std::vector<Frame> frames_of(const Line &line) {
   return out;
 }
 
-// One LimitRect / LimitEllipse sampled on n rays from its centre at machine-frame angles 2 pi k / n.
-void sample_aperture(const Elem &e, const Frame &f, int n, std::vector<double> &vx, std::vector<double> &vy) {
+// One LimitRect / LimitEllipse / LimitPolygon sampled on n rays from its centre at machine-frame angles
+// 2 pi k / n.  false: a polygon that does not surround the mean of its vertices.
+bool sample_aperture(const Elem &e, const Frame &f, int n, std::vector<double> &vx, std::vector<double> &vy) {
   const double pi = 3.14159265358979323846264338327950288;
   double cx = 0.0, cy = 0.0, hx = 0.0, hy = 0.0;
   if (e.type == XT_LIMITRECT) {
@@ -60,6 +61,15 @@ void sample_aperture(const Elem &e, const Frame &f, int n, std::vector<double> &
     cy = 0.5 * (e.v[2] + e.v[3]);
     hx = 0.5 * (e.v[1] - e.v[0]);
     hy = 0.5 * (e.v[3] - e.v[2]);
+  }
+  const int nv = e.type == XT_LIMITPOLYGON ? static_cast<int>(e.aux) : 0;
+  if (nv) {  // centre: the mean of the vertices (x[0..nv), y[0..nv))
+    for (int i = 0; i < nv; ++i) {
+      cx += e.v[i];
+      cy += e.v[nv + i];
+    }
+    cx /= nv;
+    cy /= nv;
   }
   const double lx = cx - f.tx, ly = cy - f.ty;  // centre in the machine frame: R^T (local - t)
   const double mx = f.c * lx - f.s * ly, my = f.s * lx + f.c * ly;
@@ -74,6 +84,19 @@ void sample_aperture(const Elem &e, const Frame &f, int n, std::vector<double> &
       const double rx = ux != 0.0 ? hx / std::fabs(ux) : INFINITY;
       const double ry = uy != 0.0 ? hy / std::fabs(uy) : INFINITY;
       r = std::fmin(rx, ry);
+    } else if (nv) {
+      // the ray c + r u meets the edge a + t (b - a): r = cross(a - c, e)/cross(u, e), t = cross(a - c, u)/cross(u, e)
+      r = INFINITY;
+      for (int i = 0; i < nv; ++i) {
+        const int j = (i + 1) % nv;
+        const double ax = e.v[i] - cx, ay = e.v[nv + i] - cy;
+        const double ex = e.v[j] - e.v[i], ey = e.v[nv + j] - e.v[nv + i];
+        const double den = ux * ey - uy * ex;
+        if (den == 0.0) continue;
+        const double rr = (ax * ey - ay * ex) / den, t = (ax * uy - ay * ux) / den;
+        if (rr > 0.0 && t >= 0.0 && t <= 1.0 && rr < r) r = rr;
+      }
+      if (!std::isfinite(r)) return false;
     } else {
       const double qa = ux / e.v[0], qb = uy / e.v[1];
       r = 1.0 / std::sqrt(qa * qa + qb * qb);
@@ -81,6 +104,7 @@ void sample_aperture(const Elem &e, const Frame &f, int n, std::vector<double> &
     vx[k] = mx + r * dx;
     vy[k] = my + r * dy;
   }
+  return true;
 }
 
 struct Work {  // compact ensemble of one group, device
@@ -244,12 +268,17 @@ extern "C" int xt_refine_loss_location(const xt_lattice *lat, const xt_particles
     const double s_u = u >= 0 ? s_tab[u] : 0.0;
     const double seg_len = s_tab[l] - s_u;
     if (!(seg_len > 0.0)) continue;
-    sample_aperture(line.el[l], frames[l], n_poly, lx, ly);
+    bool ok = sample_aperture(line.el[l], frames[l], n_poly, lx, ly);
     if (u >= 0) {
-      sample_aperture(line.el[u], frames[u], n_poly, ux, uy);
+      ok = ok && sample_aperture(line.el[u], frames[u], n_poly, ux, uy);
     } else {
       ux = lx;
       uy = ly;
+    }
+    if (!ok) {
+      release();
+      set_error("xt_refine_loss_location: a polygon aperture does not surround the mean of its vertices");
+      return XT_ERR_BAD_LATTICE;
     }
 
     // back: elements l-1 .. u+1, reversed (reading A11)

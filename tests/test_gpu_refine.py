@@ -204,3 +204,45 @@ def test_refinement_on_the_configs4_lattice_sampled(X):
         good = (np.isnan(a) & np.isnan(r)) | (np.abs(a - r) <= 1e-10 * np.maximum(np.abs(r), SCALE[k]))
         assert good.mean() > 0.99, (k, float(good.mean()), float(np.nanmax(np.abs(a - r))))
     assert np.isnan(ref["x"][ok]).mean() < 0.3                     # particles born beyond |p| = 1 are lost as NaN
+
+
+def test_refinement_between_polygon_apertures(X):
+    """LimitPolygon apertures as the flagging and the upstream aperture (a star and a 64-gon, one of them in a
+    shifted / tilted bracket), against the oracle."""
+    ang = 2 * np.pi * np.arange(64) / 64
+    els = [Drift(1.0), star(12, 0.0065, 0.005, 5e-4, -3e-4, 0.2), Drift(3.0), Multipole(knl=(0.0, 0.03, 1.0)), Quadrupole(0.04, 1.2),
+           Drift(2.5), XYShift(-1e-3, 5e-4), SRotation.from_angle(0.4),
+           LimitPolygon(tuple(0.008 * np.cos(ang)), tuple(0.005 * np.sin(ang))), SRotation.from_angle(-0.4), XYShift(1e-3, -5e-4),
+           Drift(4.0), LimitRect(-0.004, 0.004, -0.003, 0.003)]
+    buf = pack_lattice(els, P0C, MASS0, 1.0)
+    co = ensemble(4000, 2.5e-3, 3e-4, 21)
+    ref = O.new_particles(buf, co)
+    mm0 = np.full(4000, np.inf)
+    O.track(buf, ref, 1, threads=O.host_threads(), min_margin=mm0)
+    coarse = O.copy_particles(ref)
+    mm = np.full(4000, np.inf)
+    moved_ref = R.refine_loss_location(els, P0C, MASS0, 1.0, ref, 0.05, 48, min_margin=mm)
+    per_ap = [int(((coarse["state"] == 0) & (coarse["at_element"] == i)).sum()) for i in (1, 8, 12)]
+    assert min(per_ap) > 100 and moved_ref > 1000, (per_ap, moved_ref)
+    lat = X.xt_lattice_create(buf)
+    p = X.new_particles(lat, co)
+    X.xt_track(lat, p, 1)
+    moved = X.xt_refine_loss_location(lat, p, 0.05, 48)
+    got = X.particles_to_host(p)
+    lat.close()
+    clear = ~(mm0 < 1e-9) & ~(mm < 1e-9)
+    assert clear.sum() > 3950 and abs(moved - moved_ref) <= (~clear).sum()
+    assert np.array_equal(got["at_element"][clear], ref["at_element"][clear])
+    assert np.max(np.abs(got["s"][clear] - ref["s"][clear])) < 1e-9
+    for k in KEYS:
+        ok = np.abs(got[k] - ref[k]) <= 1e-12 * np.maximum(np.abs(ref[k]), SCALE[k])
+        assert ok[clear].all(), (k, int((~ok[clear]).sum()))
+    # a polygon that does not surround the mean of its vertices cannot be sampled from there: reported
+    bad = [Drift(1.0), LimitPolygon((0.0, 0.02, 0.02, 0.019, 0.019, 0.0), (0.0, 0.0, 0.02, 0.02, 0.001, 0.001))]
+    lat = X.xt_lattice_create(pack_lattice(bad, P0C, MASS0, 1.0))
+    p = X.new_particles(lat, ensemble(64, 5e-3, 1e-4, 2))
+    X.xt_track(lat, p, 1)
+    with pytest.raises(X.XtError) as e:
+        X.xt_refine_loss_location(lat, p, 0.1, 16)
+    assert e.value.code == -2
+    lat.close()
