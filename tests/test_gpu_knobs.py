@@ -5,6 +5,8 @@ base values afterwards."""
 import numpy as np
 import pytest
 
+import helpers as H
+
 from oracle import knobs as K
 from oracle import oracle as O
 from xt_inputs.packed import (Cavity, Drift, LimitEllipse, Multipole, SRotation, XYShift, pack_lattice)
@@ -12,7 +14,6 @@ from xt_inputs.packed import (Cavity, Drift, LimitEllipse, Multipole, SRotation,
 pytestmark = pytest.mark.gpu
 P0C, MASS0 = 450e9, 938272088.16
 KEYS = ("x", "px", "y", "py", "zeta", "delta", "ptau")
-SCALE = dict(x=1e-3, px=1e-4, y=1e-3, py=1e-4, zeta=1e-2, delta=1e-4, ptau=1e-4)
 
 
 @pytest.fixture(scope="module")
@@ -95,7 +96,7 @@ def test_knobs_match_the_oracle(X, kind, cavity, turns):
     else:
         rtol = 1e-12 if turns == 1 else 1e-10
         for k in KEYS:
-            ok = np.abs(got[k] - ref[k]) <= rtol * np.maximum(np.abs(ref[k]), SCALE[k])
+            ok = np.abs(got[k] - ref[k]) <= np.maximum(rtol * np.abs(ref[k]), H.parity_atol(ref[k][clear], rtol))
             assert ok[clear].mean() > (0.999 if turns > 1 else 1.0 - 1e-12), (k, float(ok[clear].mean()))
     # the image is back at base: a plain xt_track equals a fresh lattice, bit for bit; and the knobs can be dropped
     fresh = X.xt_lattice_create(buf, kind=kind)
@@ -136,5 +137,5 @@ def test_knob_argument_errors_and_step_clamping(X):
     K.track_with_knobs(els, P0C, MASS0, 1.0, ref, 5, [[1.0, 2.0, 2.0, 2.0, 2.0]], [(idx[0], 0, 0, 0, 2e-5)])
     got = X.particles_to_host(p)
     for k in KEYS:
-        assert np.all(np.abs(got[k] - ref[k]) <= 1e-11 * np.maximum(np.abs(ref[k]), SCALE[k])), k
+        assert np.all(np.abs(got[k] - ref[k]) <= np.maximum(1e-11 * np.abs(ref[k]), H.parity_atol(ref[k], 1e-11))), k
     lat.close()

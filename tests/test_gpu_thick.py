@@ -6,6 +6,8 @@ aperture, 1 turn at 1e-12 and 100 turns at 1e-10; every launch shape bit-identic
 import numpy as np
 import pytest
 
+import helpers as H
+
 from oracle import oracle as O
 from xt_inputs.packed import Cavity, Drift, LimitEllipse, Marker, Multipole, Quadrupole, pack_lattice
 
@@ -37,10 +39,7 @@ def ensemble(n, scale=1.0, seed=21):
 
 
 def close(got, ref, rtol, sel):
-    for k in KEYS:
-        a, r = got[k][sel], ref[k][sel]
-        ok = np.abs(a - r) <= np.maximum(rtol * np.abs(r), rtol * 1e-3)
-        assert ok.all(), (k, int((~ok).sum()), float(np.max(np.abs(a - r))))
+    H.assert_parity(got, ref, rtol, sel=sel, keys=KEYS)      # reading A8: per-coordinate floor
 
 
 def test_thick_quadrupole_ring_parity(X):

@@ -4,6 +4,8 @@ ring of thick bends and thick quadrupoles with a cavity and apertures; 1 turn at
 import numpy as np
 import pytest
 
+import helpers as H
+
 from oracle import oracle as O
 from xt_inputs.packed import Bend, Cavity, Drift, LimitEllipse, Multipole, Quadrupole, pack_lattice
 
@@ -36,10 +38,7 @@ def ensemble(n, scale=1.0, seed=31):
 
 
 def close(got, ref, rtol, sel):
-    for k in KEYS:
-        a, r = got[k][sel], ref[k][sel]
-        ok = np.abs(a - r) <= np.maximum(rtol * np.abs(r), rtol * 1e-3)
-        assert ok.all(), (k, int((~ok).sum()), float(np.max(np.abs(a - r))))
+    H.assert_parity(got, ref, rtol, sel=sel, keys=KEYS)      # reading A8: per-coordinate floor
 
 
 def test_thick_bend_ring_parity(X):
