@@ -90,13 +90,38 @@ typedef struct {
   int64_t *particle_id, *at_element;
 } xt_particles;
 
+/* Timing record of one xt_track_ex call (optional, HOST memory).  Asking for it makes the call
+ * synchronous: it brackets every tracking launch and every compaction pass (step C: count, scan, move)
+ * with CUDA events on the stream, synchronises at the end and fills the record.  Algorithmic bytes of a
+ * pass over n_in particles: 2 x n_in x 112 B (every one of the 13 arrays and the
+ * origin index is read once and written once, to the next working set or to its final place). */
+#define XT_STATS_MAX_PASSES 128
+typedef struct {
+  int64_t n_track_launches;   /* tracking launches of the call                                   */
+  int64_t n_passes;           /* compaction passes, the initial partition included (0: none ran) */
+  double track_ms;            /* sum of the tracking launches' device times                      */
+  double compact_ms;          /* sum of the passes' device times                                 */
+  double compact_bytes;       /* sum of their algorithmic bytes                                  */
+  double scatter_ms;          /* the final restore-order scatter                                 */
+  double scatter_bytes;       /* 2 x n_alive x 112                                               */
+  int64_t pass_n_in[XT_STATS_MAX_PASSES];   /* particles entering pass k (first passes only)     */
+  int64_t pass_n_out[XT_STATS_MAX_PASSES];  /* alive behind it                                   */
+  double pass_ms[XT_STATS_MAX_PASSES];
+} xt_track_stats;
+
 /* Options of xt_track_ex.  Zero-initialise for the defaults. */
 typedef struct {
   int64_t turns_per_launch; /* 0: auto (= compact_every when compaction is active, else all)  */
   int64_t compact_every;    /* 0: auto (1000 turns if the lattice has apertures and n_turns   */
                             /*    exceeds it); < 0: never compact; > 0: period in turns       */
   int32_t block_size;       /* 0: auto; else threads per CTA, a multiple of 32 in [32, 256]   */
-  int32_t particles_per_thread; /* 0: auto; else 1, 2, 3 or 4                                 */
+  int32_t particles_per_thread; /* 0: auto; else 1, 2, 3, 4 or 6                              */
+  void *workspace;          /* DEVICE scratch for compaction, caller-owned, or NULL: the      */
+  uint64_t workspace_bytes; /*    library then uses cudaMallocAsync / cudaFreeAsync on the    */
+                            /*    stream.  Needs xt_track_workspace_bytes(n_part) bytes,      */
+                            /*    256-byte aligned; too small: XT_ERR_INVALID_ARG.  With it   */
+                            /*    xt_track_ex allocates nothing.                              */
+  xt_track_stats *stats;    /* HOST, optional: see xt_track_stats (makes the call synchronous) */
 } xt_track_opts;
 
 /* Static description of a lattice image; counts are per turn. */
@@ -157,6 +182,10 @@ int xt_track(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64
 int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
                 void *cuda_stream, const xt_track_opts *opts);
 
+/* Bytes of device scratch step C needs for n_part particles (two working sets of 14 arrays, tile
+ * counts, two counters): what xt_track_opts.workspace must provide. */
+uint64_t xt_track_workspace_bytes(int64_t n_part);
+
 /* End-to-end variant: the SAME call with HOST arrays.  Copies the ensemble to the device
  * (stream-ordered allocation), tracks, copies everything back and synchronises the stream.
  * Pinned host memory makes the copies asynchronous; pageable memory also works. */
@@ -175,14 +204,22 @@ int xt_survival_histogram(const int64_t *at_turn, const int64_t *state, int64_t 
                           int64_t bin_width, int64_t n_bins, int64_t *hist, void *cuda_stream);
 
 /* FP64 FMA microbenchmark (roofline denominator, north_star: "measured by an FMA
- * microbenchmark in the same run"): runs a register-resident DFMA kernel on the whole chip,
- * times it with CUDA events on `cuda_stream`, synchronises, and returns FLOP/s (2 per FMA)
- * in *flops_per_s and the kernel time in *ms (either may be NULL). */
+ * microbenchmark in the same run"): runs register-resident DFMA kernels on the whole chip -- a sweep
+ * over operand forms (fma(acc, a, b) with a, b kernel parameters; one per-chain vector register plus
+ * one parameter as multiplicand or as addend), 4-16 independent chains per thread and launch shapes of
+ * 128-1024 threads x 1-4 CTAs per SM -- times each with CUDA events on `cuda_stream`, synchronises,
+ * and returns the MAXIMUM in FLOP/s (2 per FMA) in *flops_per_s and that kernel's time in *ms (either
+ * may be NULL).  On B200 the maximum is 2.00 cycles per warp DFMA per scheduler. */
 int xt_fp64_fma_peak(double *flops_per_s, double *ms, void *cuda_stream);
+/* One row of that sweep: shape `index` in [0, xt_fp64_fma_peak_sweep_size()); desc (HOST, 4 ints, may be
+ * NULL) receives {chains per thread, operand form 0/1/2, threads per CTA, CTAs per SM}.
+ * XT_ERR_INVALID_ARG for an index out of range. */
+int xt_fp64_fma_peak_sweep_size(void);
+int xt_fp64_fma_peak_sweep(int index, double *flops_per_s, double *ms, int *desc, void *cuda_stream);
 /* The same measurement with the operand shapes of the tracking arithmetic:
- * pattern 0 = xt_fp64_fma_peak (two of three operands shared by consecutive instructions);
- * 1 = three distinct register operands per DFMA; 2 = the complex Horner recurrence of step M2
- * for 4 particles per thread, coefficients broadcast from shared memory, no lattice. */
+ * pattern 0 = xt_fp64_fma_peak; 1 = three distinct vector-register operands per DFMA; 2 = the complex
+ * Horner recurrence of step M2 for 4 particles per thread, coefficients broadcast from shared memory,
+ * no lattice; 3 = the same recurrence with the coefficients in uniform registers (constant memory). */
 int xt_fp64_fma_probe(int pattern, double *flops_per_s, double *ms, void *cuda_stream);
 
 /* Twiss from tracking, 4-D ("Twiss module"): the closed

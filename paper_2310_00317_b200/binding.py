@@ -34,9 +34,23 @@ class xt_particles(ctypes.Structure):
     _fields_ = ([(k, ctypes.c_void_p) for k in F64_FIELDS] + [(k, ctypes.c_void_p) for k in I64_FIELDS])
 
 
+XT_STATS_MAX_PASSES = 128
+
+
+class xt_track_stats(ctypes.Structure):
+    _fields_ = [("n_track_launches", ctypes.c_int64), ("n_passes", ctypes.c_int64),
+                ("track_ms", ctypes.c_double), ("compact_ms", ctypes.c_double), ("compact_bytes", ctypes.c_double),
+                ("scatter_ms", ctypes.c_double), ("scatter_bytes", ctypes.c_double),
+                ("pass_n_in", ctypes.c_int64 * XT_STATS_MAX_PASSES),
+                ("pass_n_out", ctypes.c_int64 * XT_STATS_MAX_PASSES),
+                ("pass_ms", ctypes.c_double * XT_STATS_MAX_PASSES)]
+
+
 class xt_track_opts(ctypes.Structure):
     _fields_ = [("turns_per_launch", ctypes.c_int64), ("compact_every", ctypes.c_int64),
-                ("block_size", ctypes.c_int32), ("particles_per_thread", ctypes.c_int32)]
+                ("block_size", ctypes.c_int32), ("particles_per_thread", ctypes.c_int32),
+                ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_uint64),
+                ("stats", ctypes.POINTER(xt_track_stats))]
 
 
 class xt_lattice_opts(ctypes.Structure):
@@ -112,6 +126,10 @@ SIGNATURES = {
     "xt_particles_init_derived": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _VP]),
     "xt_survival_histogram": (ctypes.c_int, [_VP, _VP, _I64, _I64, _I64, _VP, _VP]),
     "xt_fp64_fma_peak": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), _VP]),
+    "xt_track_workspace_bytes": (ctypes.c_uint64, [_I64]),
+    "xt_fp64_fma_peak_sweep_size": (ctypes.c_int, []),
+    "xt_fp64_fma_peak_sweep": (ctypes.c_int, [ctypes.c_int, ctypes.POINTER(ctypes.c_double),
+                                              ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int), _VP]),
     "xt_fp64_fma_probe": (ctypes.c_int, [ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                          ctypes.POINTER(ctypes.c_double), _VP]),
     "xt_twiss4d": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
@@ -319,10 +337,30 @@ def _n_part(p: Dict) -> int:
     return int(p["x"].shape[0])
 
 
-def _opts(turns_per_launch=0, compact_every=0, block_size=0, particles_per_thread=0):
-    if not (turns_per_launch or compact_every or block_size or particles_per_thread):
+def _opts(turns_per_launch=0, compact_every=0, block_size=0, particles_per_thread=0, workspace=None, stats=None):
+    if not (turns_per_launch or compact_every or block_size or particles_per_thread) and workspace is None \
+            and stats is None:
         return None
-    return xt_track_opts(int(turns_per_launch), int(compact_every), int(block_size), int(particles_per_thread))
+    o = xt_track_opts(int(turns_per_launch), int(compact_every), int(block_size), int(particles_per_thread))
+    if workspace is not None:                      # a torch uint8 CUDA tensor, caller-owned
+        o.workspace = workspace.data_ptr()
+        o.workspace_bytes = workspace.numel() * workspace.element_size()
+    if stats is not None:
+        o.stats = ctypes.pointer(stats)
+    return o
+
+
+def xt_track_workspace_bytes(n_part: int, kind: str = "prod") -> int:
+    return int(load_library(kind).xt_track_workspace_bytes(int(n_part)))
+
+
+def _stats_dict(st: "xt_track_stats") -> Dict:
+    n = min(int(st.n_passes), XT_STATS_MAX_PASSES)
+    return {"n_track_launches": int(st.n_track_launches), "n_passes": int(st.n_passes),
+            "track_ms": st.track_ms, "compact_ms": st.compact_ms, "compact_bytes": st.compact_bytes,
+            "scatter_ms": st.scatter_ms, "scatter_bytes": st.scatter_bytes,
+            "pass_n_in": [int(v) for v in st.pass_n_in[:n]], "pass_n_out": [int(v) for v in st.pass_n_out[:n]],
+            "pass_ms": [float(v) for v in st.pass_ms[:n]]}
 
 
 def xt_particles_init_derived(lat: Lattice, p: Dict, stream=None) -> None:
@@ -339,11 +377,16 @@ def xt_track(lat: Lattice, p: Dict, n_turns: int, stream=None) -> None:
 
 
 def xt_track_ex(lat: Lattice, p: Dict, n_turns: int, stream=None, *, turns_per_launch: int = 0,
-                compact_every: int = 0, block_size: int = 0, particles_per_thread: int = 0) -> None:
+                compact_every: int = 0, block_size: int = 0, particles_per_thread: int = 0,
+                workspace=None, stats: bool = False):
+    """``workspace``: optional torch uint8 CUDA tensor of xt_track_workspace_bytes(n) bytes; ``stats=True``
+    returns the call's xt_track_stats as a dict (and makes the call synchronous)."""
     st = _struct_from_tensors(p)
-    o = _opts(turns_per_launch, compact_every, block_size, particles_per_thread)
+    rec = xt_track_stats() if stats else None
+    o = _opts(turns_per_launch, compact_every, block_size, particles_per_thread, workspace, rec)
     _check(lat._lib, lat._lib.xt_track_ex(lat.handle, ctypes.byref(st), _n_part(p), int(n_turns),
                                           _stream_ptr(stream), ctypes.byref(o) if o else None))
+    return _stats_dict(rec) if stats else None
 
 
 def xt_track_host(lat: Lattice, p_host: Dict, n_turns: int, stream=None, *, turns_per_launch: int = 0,
@@ -373,8 +416,20 @@ def xt_fp64_fma_peak(stream=None, kind: str = "prod"):
     return f.value, ms.value
 
 
+def xt_fp64_fma_peak_sweep(stream=None, kind: str = "prod"):
+    """Every row of the peak sweep: list of dicts {chains, form, block, ctas_per_sm, tflops, ms}."""
+    lib = load_library(kind)
+    rows = []
+    for i in range(lib.xt_fp64_fma_peak_sweep_size()):
+        f, ms, d = ctypes.c_double(), ctypes.c_double(), (ctypes.c_int * 4)()
+        _check(lib, lib.xt_fp64_fma_peak_sweep(i, ctypes.byref(f), ctypes.byref(ms), d, _stream_ptr(stream)))
+        rows.append({"chains": d[0], "form": d[1], "block": d[2], "ctas_per_sm": d[3],
+                     "tflops": f.value / 1e12, "ms": ms.value})
+    return rows
+
+
 def xt_fp64_fma_probe(pattern: int, stream=None, kind: str = "prod"):
-    """(FLOP/s, kernel ms) of the DFMA probe with operand pattern 0, 1 or 2 (see include/xt.h)."""
+    """(FLOP/s, kernel ms) of the DFMA probe with operand pattern 0, 1, 2 or 3 (see include/xt.h)."""
     lib = load_library(kind)
     f, ms = ctypes.c_double(), ctypes.c_double()
     _check(lib, lib.xt_fp64_fma_probe(int(pattern), ctypes.byref(f), ctypes.byref(ms), _stream_ptr(stream)))

@@ -3,6 +3,7 @@
 // the init helper, the survival histogram, the FMA microbenchmark and error reporting.
 #include <atomic>
 #include <string>
+#include <vector>
 
 #include "xt_internal.h"
 
@@ -71,6 +72,87 @@ int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part,
   return XT_OK;
 }
 
+
+// Optional timing of one xt_track_ex call (xt_track_stats): events around every tracking launch and every
+// compaction pass; the alive count behind each pass is logged by an 8-byte device copy.  All host work
+// happens in finish(), after one stream synchronisation.  Inactive (stats == nullptr) it does nothing.
+class StatsTimer {
+ public:
+  StatsTimer(xt_track_stats *stats, cudaStream_t st) : stats_(stats), st_(st) {}
+  ~StatsTimer() {
+    for (auto &e : ev_) {
+      cudaEventDestroy(e.a);
+      cudaEventDestroy(e.b);
+    }
+    if (d_log_) cudaFree(d_log_);
+  }
+  void begin() {
+    if (!stats_) return;
+    Span s{};
+    if (cudaEventCreate(&s.a) != cudaSuccess || cudaEventCreate(&s.b) != cudaSuccess) return;
+    cudaEventRecord(s.a, st_);
+    ev_.push_back(s);
+  }
+  void end_track() { end(0, nullptr); }
+  void end_pass(const int64_t *d_n_active) { end(1, d_n_active); }
+  void end_scatter() { end(2, nullptr); }
+  int finish(int64_t n_part) {
+    if (!stats_) return XT_OK;
+    XT_CUDA(cudaStreamSynchronize(st_));
+    xt_track_stats &o = *stats_;
+    o = xt_track_stats{};
+    std::vector<int64_t> log(n_pass_);
+    if (n_pass_) XT_CUDA(cudaMemcpy(log.data(), d_log_, sizeof(int64_t) * n_pass_, cudaMemcpyDeviceToHost));
+    int64_t n_in = n_part, pass = 0;
+    for (const Span &s : ev_) {
+      float ms = 0.f;
+      XT_CUDA(cudaEventElapsedTime(&ms, s.a, s.b));
+      if (s.kind == 0) {
+        o.n_track_launches++;
+        o.track_ms += ms;
+      } else if (s.kind == 1) {
+        const int64_t n_out = log[pass];
+        if (pass < XT_STATS_MAX_PASSES) {
+          o.pass_n_in[pass] = n_in;
+          o.pass_n_out[pass] = n_out;
+          o.pass_ms[pass] = ms;
+        }
+        o.compact_ms += ms;
+        o.compact_bytes += 2.0 * 112.0 * static_cast<double>(n_in);
+        n_in = n_out;
+        ++pass;
+      } else {
+        o.scatter_ms += ms;
+        o.scatter_bytes += 2.0 * 112.0 * static_cast<double>(n_in);
+      }
+    }
+    o.n_passes = pass;
+    return XT_OK;
+  }
+
+ private:
+  struct Span {
+    cudaEvent_t a, b;
+    int kind;
+  };
+  void end(int kind, const int64_t *d_n_active) {
+    if (!stats_ || ev_.empty()) return;
+    ev_.back().kind = kind;
+    cudaEventRecord(ev_.back().b, st_);
+    if (kind == 1 && d_n_active) {
+      if (!d_log_) cudaMalloc(reinterpret_cast<void **>(&d_log_), sizeof(int64_t) * kMaxLog);
+      if (d_log_ && n_pass_ < kMaxLog)
+        cudaMemcpyAsync(d_log_ + n_pass_++, d_n_active, sizeof(int64_t), cudaMemcpyDeviceToDevice, st_);
+    }
+  }
+  static constexpr int kMaxLog = 1 << 16;
+  xt_track_stats *stats_;
+  cudaStream_t st_;
+  std::vector<Span> ev_;
+  int64_t *d_log_ = nullptr;
+  int n_pass_ = 0;
+};
+
 }  // namespace
 }  // namespace xt
 
@@ -100,27 +182,37 @@ extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t
   }
   const int64_t tpl_opt = opts ? opts->turns_per_launch : 0;
 
+  xt::StatsTimer tm(opts ? opts->stats : nullptr, st);
   if (period == 0) {
     const int64_t tpl = tpl_opt > 0 ? tpl_opt : n_turns;
     for (int64_t done = 0; done < n_turns;) {
       const int64_t k = (n_turns - done < tpl) ? n_turns - done : tpl;
+      tm.begin();
       if ((rc = xt::launch_track(lat, *p, n_part, nullptr, k, block, ppt, st)) != XT_OK) return rc;
+      tm.end_track();
       done += k;
     }
-    return XT_OK;
+    return tm.finish(n_part);
   }
 
-  void *ws = nullptr;
+  void *ws = opts ? opts->workspace : nullptr;
   const size_t ws_bytes = xt::compaction_workspace_bytes(n_part);
-  XT_CUDA(cudaMallocAsync(&ws, ws_bytes, st));
+  const bool own_ws = (ws == nullptr);
+  if (!own_ws && (opts->workspace_bytes < ws_bytes || (reinterpret_cast<uintptr_t>(ws) & 255u))) {
+    xt::set_error("xt_track_ex: workspace too small (see xt_track_workspace_bytes) or not 256-byte aligned");
+    return XT_ERR_INVALID_ARG;
+  }
+  if (own_ws) XT_CUDA(cudaMallocAsync(&ws, ws_bytes, st));
   xt::CompactPlan plan;
   xt::plan_compaction(ws, n_part, plan);
   auto bail = [&](int code) {
-    cudaFreeAsync(ws, st);
+    if (own_ws) cudaFreeAsync(ws, st);
     return code;
   };
   // initial partition: alive particles of the caller's arrays -> working set 0
+  tm.begin();
   if ((rc = xt::launch_partition(plan, *p, nullptr, true, n_part, plan.w[0], *p, st)) != XT_OK) return bail(rc);
+  tm.end_pass(plan.n_active);
   int cur = 0;
   const int64_t tpl = (tpl_opt > 0 && tpl_opt < period) ? tpl_opt : period;
   int64_t since = 0;
@@ -128,20 +220,31 @@ extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t
     int64_t k = n_turns - done;
     if (k > tpl) k = tpl;
     if (k > period - since) k = period - since;
+    tm.begin();
     if ((rc = xt::launch_track(lat, plan.w[cur].p, n_part, plan.n_active, k, block, ppt, st)) != XT_OK) return bail(rc);
+    tm.end_track();
     done += k;
     since += k;
     if (since == period && done < n_turns) {
+      tm.begin();
       if ((rc = xt::launch_partition(plan, plan.w[cur].p, plan.w[cur].origin, false, n_part, plan.w[1 - cur], *p,
                                      st)) != XT_OK)
         return bail(rc);
+      tm.end_pass(plan.n_active);
       cur = 1 - cur;
       since = 0;
     }
   }
+  tm.begin();
   if ((rc = xt::launch_scatter_back(plan, plan.w[cur], n_part, *p, st)) != XT_OK) return bail(rc);
-  XT_CUDA(cudaFreeAsync(ws, st));
+  tm.end_scatter();
+  if ((rc = tm.finish(n_part)) != XT_OK) return bail(rc);
+  if (own_ws) XT_CUDA(cudaFreeAsync(ws, st));
   return XT_OK;
+}
+
+extern "C" uint64_t xt_track_workspace_bytes(int64_t n_part) {
+  return n_part > 0 ? static_cast<uint64_t>(xt::compaction_workspace_bytes(n_part)) : 0;
 }
 
 extern "C" int xt_track(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
@@ -224,6 +327,12 @@ extern "C" int xt_survival_histogram(const int64_t *at_turn, const int64_t *stat
 
 extern "C" int xt_fp64_fma_peak(double *flops_per_s, double *ms, void *cuda_stream) {
   return xt::run_fma_peak(flops_per_s, ms, 0, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int xt_fp64_fma_peak_sweep_size(void) { return xt::fma_peak_sweep_size(); }
+
+extern "C" int xt_fp64_fma_peak_sweep(int index, double *flops_per_s, double *ms, int *desc, void *cuda_stream) {
+  return xt::run_fma_peak_shape(index, flops_per_s, ms, desc, static_cast<cudaStream_t>(cuda_stream));
 }
 
 extern "C" int xt_fp64_fma_probe(int pattern, double *flops_per_s, double *ms, void *cuda_stream) {

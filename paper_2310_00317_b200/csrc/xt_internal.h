@@ -184,5 +184,7 @@ int launch_histogram(const int64_t *at_turn, const int64_t *state, int64_t n, in
 
 // xt_peak.cu
 int run_fma_peak(double *flops_per_s, double *ms, int pattern, cudaStream_t st);
+int fma_peak_sweep_size();
+int run_fma_peak_shape(int i, double *flops_per_s, double *ms, int *desc, cudaStream_t st);
 
 }  // namespace xt

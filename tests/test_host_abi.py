@@ -55,7 +55,8 @@ def test_library_loads_and_exports_every_declared_symbol(kind):
 def test_struct_layouts_match_the_header():
     # sizes the C compiler gives the public structs (LP64): 14 pointers; 2 x i64 + 2 x i32; ...
     assert ctypes.sizeof(B.xt_particles) == 14 * 8
-    assert ctypes.sizeof(B.xt_track_opts) == 24
+    assert ctypes.sizeof(B.xt_track_opts) == 48          # + workspace ptr, bytes, stats ptr
+    assert ctypes.sizeof(B.xt_track_stats) == 7 * 8 + 3 * 8 * B.XT_STATS_MAX_PASSES
     assert ctypes.sizeof(B.xt_lattice_opts) == 16
     assert ctypes.sizeof(B.xt_lattice_info) == 8 * (5 + 8 + 3) + 8 * 3 + 8 + 8
 
