@@ -229,7 +229,8 @@ def time_workload(X, torch, lat, coords, turns, steps, warmup, args, barrier, sa
             work[k].copy_(pristine[k])
         if ev0 is not None:
             ev0.record(stream)
-        X.xt_track_ex(lat, work, turns, block_size=args.block, particles_per_thread=args.ppt)
+        X.xt_track_ex(lat, work, turns, block_size=args.block, particles_per_thread=args.ppt,
+                      cold_in_registers=args.cold)
         if ev1 is not None:
             ev1.record(stream)
 
@@ -297,6 +298,7 @@ def main():
     ap.add_argument("--block", type=int, default=0)
     ap.add_argument("--ppt", type=int, default=0, help="particles per thread (0: auto)")
     ap.add_argument("--chunk", type=int, default=0, help="staging-buffer bytes (0: library default)")
+    ap.add_argument("--cold", type=int, default=0, help="cold state: 0 auto, 1 registers, -1 shared memory")
     ap.add_argument("--also-steps", type=int, default=5, help="timed steps of the configs[2] leg (mean)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and configs[2] legs")
     args = ap.parse_args()

@@ -115,13 +115,18 @@ typedef struct {
   int64_t compact_every;    /* 0: auto (1000 turns if the lattice has apertures and n_turns   */
                             /*    exceeds it); < 0: never compact; > 0: period in turns       */
   int32_t block_size;       /* 0: auto; else threads per CTA, a multiple of 32 in [32, 256]   */
-  int32_t particles_per_thread; /* 0: auto; else 1, 2, 3, 4 or 6                              */
+  int32_t particles_per_thread; /* 0: auto; else 1, 2, 3 or 4                                 */
   void *workspace;          /* DEVICE scratch for compaction, caller-owned, or NULL: the      */
   uint64_t workspace_bytes; /*    library then uses cudaMallocAsync / cudaFreeAsync on the    */
                             /*    stream.  Needs xt_track_workspace_bytes(n_part) bytes,      */
                             /*    256-byte aligned; too small: XT_ERR_INVALID_ARG.  With it   */
                             /*    xt_track_ex allocates nothing.                              */
   xt_track_stats *stats;    /* HOST, optional: see xt_track_stats (makes the call synchronous) */
+  int32_t cold_in_registers;/* 0: auto; 1: keep the per-particle functions of (delta, ptau) in   */
+                            /*    registers (2 or 3 particles per thread only); -1: in shared    */
+                            /*    memory.  Launch-shape option like the two above: results are   */
+                            /*    bit-identical for every shape.                                 */
+  int32_t reserved;         /* 0                                                               */
 } xt_track_opts;
 
 /* Static description of a lattice image; counts are per turn. */

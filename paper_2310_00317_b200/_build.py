@@ -42,30 +42,64 @@ def nvcc() -> str:
     return exe
 
 
-def _stale(path: str) -> bool:
-    if not os.path.exists(path):
+def _objdir(kind: str) -> str:
+    d = os.path.join(HERE, "build", kind)
+    os.makedirs(d, exist_ok=True)
+    return d
+
+
+def _stale(target: str, deps: List[str]) -> bool:
+    if not os.path.exists(target):
         return True
-    t = os.path.getmtime(path)
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS + [os.path.abspath(__file__)]
+    t = os.path.getmtime(target)
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def compile_command(kind: str, src: str, obj: str, extra: List[str] = ()) -> List[str]:
+    flags = [f for f in COMMON if f != "-shared"]
+    return [nvcc(), *flags, *LIBS[kind]["flags"], *extra, "-c", os.path.join(CSRC, src), "-o", obj]
+
+
 def command(kind: str, extra: List[str] = ()) -> List[str]:
+    """The one-line equivalent of the build (every source in one nvcc call), for the record."""
     lib = LIBS[kind]
     return [nvcc(), *COMMON, *lib["flags"], *extra,
             *[os.path.join(CSRC, s) for s in SOURCES], "-o", lib["path"]]
 
 
-def build(kinds=("prod", "nofma"), force: bool = False, verbose: bool = False) -> None:
+def build(kinds=("prod", "nofma"), force: bool = False, verbose: bool = False, extra: List[str] = ()) -> None:
+    """Each translation unit is compiled to an object file (in parallel, only when stale) and the objects
+    are linked into the shared library: no device code crosses translation units, so no device link."""
+    from concurrent.futures import ThreadPoolExecutor
+    jobs = []
     for kind in kinds:
-        if not force and not _stale(LIBS[kind]["path"]):
-            continue
-        cmd = command(kind, ["-Xptxas", "-v"] if verbose else [])
+        od = _objdir(kind)
+        for src in SOURCES:
+            obj = os.path.join(od, src.replace(".cu", ".o"))
+            deps = [os.path.join(CSRC, src)] + HEADERS + [os.path.abspath(__file__)]
+            if force or _stale(obj, deps):
+                jobs.append((kind, src, obj))
+
+    def run(job):
+        kind, src, obj = job
+        cmd = compile_command(kind, src, obj, list(extra) + (["-Xptxas", "-v"] if verbose else []))
         res = subprocess.run(cmd, capture_output=True, text=True)
-        if verbose:
-            print(res.stderr)
-        if res.returncode != 0:
-            raise RuntimeError("nvcc failed:\n%s\n%s" % (" ".join(cmd), res.stderr))
+        return job, cmd, res
+
+    with ThreadPoolExecutor(max_workers=max(1, min(len(jobs), os.cpu_count() or 4))) as ex:
+        for job, cmd, res in ex.map(run, jobs):
+            if verbose:
+                print(res.stderr)
+            if res.returncode != 0:
+                raise RuntimeError("nvcc failed:\n%s\n%s" % (" ".join(cmd), res.stderr))
+    for kind in kinds:
+        od = _objdir(kind)
+        objs = [os.path.join(od, s.replace(".cu", ".o")) for s in SOURCES]
+        if force or _stale(LIBS[kind]["path"], objs):
+            cmd = [nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", *objs, "-o", LIBS[kind]["path"]]
+            res = subprocess.run(cmd, capture_output=True, text=True)
+            if res.returncode != 0:
+                raise RuntimeError("link failed:\n%s\n%s" % (" ".join(cmd), res.stderr))
 
 
 if __name__ == "__main__":

@@ -50,7 +50,8 @@ class xt_track_opts(ctypes.Structure):
     _fields_ = [("turns_per_launch", ctypes.c_int64), ("compact_every", ctypes.c_int64),
                 ("block_size", ctypes.c_int32), ("particles_per_thread", ctypes.c_int32),
                 ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_uint64),
-                ("stats", ctypes.POINTER(xt_track_stats))]
+                ("stats", ctypes.POINTER(xt_track_stats)),
+                ("cold_in_registers", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
 class xt_lattice_opts(ctypes.Structure):
@@ -337,11 +338,13 @@ def _n_part(p: Dict) -> int:
     return int(p["x"].shape[0])
 
 
-def _opts(turns_per_launch=0, compact_every=0, block_size=0, particles_per_thread=0, workspace=None, stats=None):
-    if not (turns_per_launch or compact_every or block_size or particles_per_thread) and workspace is None \
-            and stats is None:
+def _opts(turns_per_launch=0, compact_every=0, block_size=0, particles_per_thread=0, workspace=None, stats=None,
+          cold_in_registers=0):
+    if not (turns_per_launch or compact_every or block_size or particles_per_thread or cold_in_registers) \
+            and workspace is None and stats is None:
         return None
     o = xt_track_opts(int(turns_per_launch), int(compact_every), int(block_size), int(particles_per_thread))
+    o.cold_in_registers = int(cold_in_registers)
     if workspace is not None:                      # a torch uint8 CUDA tensor, caller-owned
         o.workspace = workspace.data_ptr()
         o.workspace_bytes = workspace.numel() * workspace.element_size()
@@ -378,12 +381,12 @@ def xt_track(lat: Lattice, p: Dict, n_turns: int, stream=None) -> None:
 
 def xt_track_ex(lat: Lattice, p: Dict, n_turns: int, stream=None, *, turns_per_launch: int = 0,
                 compact_every: int = 0, block_size: int = 0, particles_per_thread: int = 0,
-                workspace=None, stats: bool = False):
+                workspace=None, stats: bool = False, cold_in_registers: int = 0):
     """``workspace``: optional torch uint8 CUDA tensor of xt_track_workspace_bytes(n) bytes; ``stats=True``
     returns the call's xt_track_stats as a dict (and makes the call synchronous)."""
     st = _struct_from_tensors(p)
     rec = xt_track_stats() if stats else None
-    o = _opts(turns_per_launch, compact_every, block_size, particles_per_thread, workspace, rec)
+    o = _opts(turns_per_launch, compact_every, block_size, particles_per_thread, workspace, rec, cold_in_registers)
     _check(lat._lib, lat._lib.xt_track_ex(lat.handle, ctypes.byref(st), _n_part(p), int(n_turns),
                                           _stream_ptr(stream), ctypes.byref(o) if o else None))
     return _stats_dict(rec) if stats else None

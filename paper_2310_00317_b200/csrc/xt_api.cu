@@ -43,15 +43,20 @@ int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p
   return XT_OK;
 }
 
-// Launch shape of the tracking kernel: threads per CTA and particles per thread.
-// Auto rule (measured on B200, profiles/r01_shape_sweep.md): 128-thread CTAs, 4 CTAs per SM
-// at <= 128 registers.  4 particles per thread when there are several waves of them
-// (configs[3]: 0.659 against 0.651 with 3), 3 per thread for smaller ensembles, where the
-// number of warps matters more (configs[2], 676 particles per SM: 0.49 against 0.38 with 4;
-// 2 per thread has too little ILP per warp: 0.47).  Below ~100 particles per SM one per
-// thread keeps more warps alive.  The kernel hands the particles out in equal shares over a
-// whole number of CTAs per SM, so the shape only has to make enough CTAs.
-int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part, int *block, int *ppt) {
+// Launch shape of the tracking kernel: threads per CTA, particles per thread, and where the cold
+// per-particle state lives.  Auto rule (measured on B200, profiles/r02_shape_sweep.md): 128-thread CTAs.
+// Several waves of particles (>= 4096 per SM, configs[3]): 4 per thread, cold state in shared memory,
+// 4 CTAs per SM at <= 128 registers.  Ensembles that fit the SMs in one wave of two CTAs
+// (<= 768 per SM, configs[2]: 676): 3 per thread with the cold state in registers -- the register file
+// is half empty there and every LDS taken out of a record shortens what a warp waits for.  In
+// between: 3 per thread, cold state in shared memory.  Below ~100 particles per SM one per thread keeps
+// more warps alive.  The kernel hands the particles out in equal shares over a whole number of CTAs
+// per SM, so the shape only has to make enough CTAs.
+struct Shape {
+  int block, ppt;
+  bool cold_in_regs;
+};
+int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part, Shape *sh) {
   const int64_t per_sm = n_part / (lat->n_sm > 0 ? lat->n_sm : 1);
   int auto_ppt = 4, auto_block = 128;
   if (per_sm < 4096) auto_ppt = 3;
@@ -59,19 +64,29 @@ int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part,
     auto_ppt = 1;
     auto_block = 32;
   }
-  *ppt = (o && o->particles_per_thread) ? o->particles_per_thread : auto_ppt;
-  *block = (o && o->block_size) ? o->block_size : auto_block;
-  if (*ppt < 1 || *ppt > 4) {
+  sh->ppt = (o && o->particles_per_thread) ? o->particles_per_thread : auto_ppt;
+  sh->block = (o && o->block_size) ? o->block_size : auto_block;
+  const int want_regs = o ? o->cold_in_registers : 0;
+  if (want_regs > 0)
+    sh->cold_in_regs = true;
+  else if (want_regs < 0)
+    sh->cold_in_regs = false;
+  else
+    sh->cold_in_regs = (sh->ppt == 3 && per_sm >= 96 && per_sm <= 768);
+  if (sh->ppt < 1 || sh->ppt > 4) {
     set_error("xt_track_ex: particles_per_thread must be 0 (auto), 1, 2, 3 or 4");
     return XT_ERR_INVALID_ARG;
   }
-  if (*block < 32 || *block > 256 || (*block % 32) != 0) {
+  if (sh->cold_in_regs && sh->ppt != 2 && sh->ppt != 3) {
+    set_error("xt_track_ex: cold_in_registers needs 2 or 3 particles per thread");
+    return XT_ERR_INVALID_ARG;
+  }
+  if (sh->block < 32 || sh->block > 256 || (sh->block % 32) != 0) {
     set_error("xt_track_ex: block_size must be a multiple of 32 in [32, 256]");
     return XT_ERR_INVALID_ARG;
   }
   return XT_OK;
 }
-
 
 // Optional timing of one xt_track_ex call (xt_track_stats): events around every tracking launch and every
 // compaction pass; the alive count behind each pass is logged by an 8-byte device copy.  All host work
@@ -164,8 +179,8 @@ extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t
     xt::set_error("xt_track: negative n_turns");
     return XT_ERR_INVALID_ARG;
   }
-  int block = 0, ppt = 0;
-  if ((rc = xt::resolve_shape(opts, lat, n_part, &block, &ppt)) != XT_OK) return rc;
+  xt::Shape sh{};
+  if ((rc = xt::resolve_shape(opts, lat, n_part, &sh)) != XT_OK) return rc;
   if (opts && opts->turns_per_launch < 0) {
     xt::set_error("xt_track_ex: negative turns_per_launch");
     return XT_ERR_INVALID_ARG;
@@ -188,7 +203,7 @@ extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t
     for (int64_t done = 0; done < n_turns;) {
       const int64_t k = (n_turns - done < tpl) ? n_turns - done : tpl;
       tm.begin();
-      if ((rc = xt::launch_track(lat, *p, n_part, nullptr, k, block, ppt, st)) != XT_OK) return rc;
+      if ((rc = xt::launch_track(lat, *p, n_part, nullptr, k, sh.block, sh.ppt, sh.cold_in_regs, st)) != XT_OK) return rc;
       tm.end_track();
       done += k;
     }
@@ -221,7 +236,7 @@ extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t
     if (k > tpl) k = tpl;
     if (k > period - since) k = period - since;
     tm.begin();
-    if ((rc = xt::launch_track(lat, plan.w[cur].p, n_part, plan.n_active, k, block, ppt, st)) != XT_OK) return bail(rc);
+    if ((rc = xt::launch_track(lat, plan.w[cur].p, n_part, plan.n_active, k, sh.block, sh.ppt, sh.cold_in_regs, st)) != XT_OK) return bail(rc);
     tm.end_track();
     done += k;
     since += k;

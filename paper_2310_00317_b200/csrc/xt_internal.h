@@ -108,6 +108,7 @@ struct xt_lattice {
   std::vector<unsigned char> packed_host;  // the buffer the lattice was created from (xt_refine.cu re-reads it)
   bool extended = false;                   // thick maps or polygon apertures: the THICK kernels
   std::vector<uint64_t> mult_slot0;        // per element: image offset of a multipole's first coefficient pair
+  std::vector<uint64_t> mult_wf_off;       // per element: image offset of a multipole's weak-focusing term
   // time functions (xt_knobs.cu); all device memory, owned
   double *d_knob_table = nullptr;
   void *d_knob_targets = nullptr;
@@ -116,6 +117,7 @@ struct xt_lattice {
   unsigned char *d_image = nullptr;
   xt::ChunkDesc *d_chunks = nullptr;
   double *d_s_table = nullptr;
+  double *d_monitor_rows = nullptr;  // not owned: where the TAG_MON records of an internal monitor line store
 };
 
 namespace xt {
@@ -138,7 +140,8 @@ struct HostImage {
   xt_lattice_info info{};
   RefConsts k{};
   bool extended = false;
-  std::vector<uint64_t> mult_slot0;  // per element: offset of a multipole's first coefficient pair (else ~0)
+  std::vector<uint64_t> mult_slot0;   // per element: offset of a multipole's first coefficient pair (else ~0)
+  std::vector<uint64_t> mult_wf_off;  // per element: offset of a multipole's weak-focusing term wf (else ~0)
 };
 struct PackOpts {
   uint32_t chunk_bytes = kDefaultChunkBytes;
@@ -150,12 +153,12 @@ int create_lattice(const void *packed, size_t nbytes, const PackOpts &po, xt_lat
 int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImage &out);
 
 // xt_track.cu
-// Where TAG_MON records store: rows of n_part x 6 doubles (x, px, y, py, zeta, delta).  One buffer per
-// process and library at a time (a __constant__ pointer), set stream-ordered before the launch that uses it.
-int set_monitor_base(double *d_rows, cudaStream_t st);
-// block: threads per CTA; ppt: particles per thread (1, 2 or 4; 4 needs block <= 256)
+// block: threads per CTA; ppt: particles per thread (1, 2, 3 or 4; 4 needs block <= 256); cold_in_regs: the
+// per-particle functions of (delta, ptau) in registers instead of shared memory (ppt 2 or 3 only).
+// TAG_MON records store into lat->d_monitor_rows (rows of n_part x 6 doubles: x, px, y, py, zeta, delta).
 int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part,
-                 const int64_t *d_n_active, int64_t n_turns, int block, int ppt, cudaStream_t st);
+                 const int64_t *d_n_active, int64_t n_turns, int block, int ppt, bool cold_in_regs,
+                 cudaStream_t st);
 int launch_init_derived(const xt_lattice *lat, const xt_particles &p, int64_t n, cudaStream_t st);
 
 // xt_compact.cu (step C) -- SoA working set with an origin index

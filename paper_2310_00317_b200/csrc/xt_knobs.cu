@@ -123,7 +123,7 @@ extern "C" int xt_lattice_set_knobs(xt_lattice *lat, const double *table, int32_
     const int n = std::get<1>(key), skew = std::get<2>(key), big_n = static_cast<int>(e.aux);
     const double hxl = e.v[0], length = e.v[1];
     KnobTarget t{};
-    // slots: (c[n], s[n]) pairs, n = N .. 0, then {wf, 0} if curved (xt_internal.h)
+    // slots: (c[n], s[n]) pairs, n = N .. 0, from mult_slot0; wf sits in the record's second slot (xt_internal.h)
     t.off = lat->mult_slot0[std::get<0>(key)] + 16ull * static_cast<uint64_t>(big_n - n) + (skew ? 8ull : 0ull);
     t.wf_off = ~0ull;
     t.base = e.v[2 + (skew ? big_n + 1 : 0) + n];
@@ -134,7 +134,7 @@ extern "C" int xt_lattice_set_knobs(xt_lattice *lat, const double *table, int32_
     if (n == 0 && !skew && hxl != 0.0) {
       t.hxl = hxl;
       if (length != 0.0) {
-        t.wf_off = lat->mult_slot0[std::get<0>(key)] + 16ull * static_cast<uint64_t>(big_n + 1);
+        t.wf_off = lat->mult_wf_off[std::get<0>(key)];
         t.length = length;
       }
     }

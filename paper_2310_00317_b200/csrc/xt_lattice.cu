@@ -121,6 +121,7 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
   out.chunks.clear();
   out.s_table.assign(n_elements, 0.0);
   out.mult_slot0.assign(n_elements, ~0ull);
+  out.mult_wf_off.assign(n_elements, ~0ull);
 
   // ---- pass 1: one record per element (markers are the identity map: no record)
   std::vector<Rec> recs;
@@ -172,8 +173,12 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
         } else {
           rec.type = TAG_MULT;
         }
-        for (int n = order; n >= 0; --n) rec.slot(cn[n], sn[n]);  // Horner order: highest first
-        if (hxl != 0.0) rec.slot((length != 0.0) ? (knl[0] * hxl) / length : 0.0, 0.0);  // {wf, 0}
+        // two fixed slots in front, {l_pre, l_post} and {l_post2, wf} (the lengths are filled in by the
+        // fusion pass), then the pairs in Horner order (highest first): every slot of the record sits
+        // at an offset the handlers know at compile time
+        rec.slot(0.0, 0.0);
+        rec.slot(0.0, (hxl != 0.0 && length != 0.0) ? (knl[0] * hxl) / length : 0.0);
+        for (int n = order; n >= 0; --n) rec.slot(cn[n], sn[n]);
         info.sum_order += order;
         break;
       }
@@ -376,15 +381,15 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
     if (post) out_rec.flags |= TAG_POST;
     if (post2) out_rec.flags |= TAG_POST2;
     if (misal) out_rec.flags |= TAG_MISAL;
-    // coefficient pairs first (the kernel prefetches the slots right behind the header), then
-    // the extras: [{wf, 0}] [{l_pre, l_post}] [{l_post2, 0}] [{dx, dy} {cos, sin} {cos', sin'} {dx', dy'}]
-    out_rec.slots = recs[m].slots;  // pairs [+ {wf, 0}]
-    if (pre || post) out_rec.slot(pre ? recs[i].p0 : 0.0, post ? recs[after].p0 : 0.0);
-    if (post2) out_rec.slot(recs[after + 1].p0, 0.0);
+    // slots: {l_pre, l_post} {l_post2, wf} [{dx, dy} {cos, sin} {cos', sin'} {dx', dy'}] pairs
+    const std::vector<double> &ms = recs[m].slots;
+    out_rec.slot(pre ? recs[i].p0 : 0.0, post ? recs[after].p0 : 0.0);
+    out_rec.slot(post2 ? recs[after + 1].p0 : 0.0, ms[3]);
     if (misal) {
       for (size_t k : {j, j + 1, j + 3, j + 4})
         out_rec.slots.insert(out_rec.slots.end(), recs[k].slots.begin(), recs[k].slots.end());
     }
+    out_rec.slots.insert(out_rec.slots.end(), ms.begin() + 4, ms.end());
     fused.push_back(std::move(out_rec));
     i = after + (post ? 1 : 0) + (post2 ? 1 : 0);
   }
@@ -444,7 +449,10 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
       out.image.resize(at + nb);
       if (!rec.slots.empty())
         std::memcpy(out.image.data() + at + sizeof(RecHdr), rec.slots.data(), rec.slots.size() * sizeof(double));
-      if (rec.type == TAG_MULT || rec.type == TAG_CMULT) out.mult_slot0[rec.elem] = at + sizeof(RecHdr);
+      if (rec.type == TAG_MULT || rec.type == TAG_CMULT) {
+        out.mult_wf_off[rec.elem] = at + sizeof(RecHdr) + 16 + 8;  // slot 1, second half
+        out.mult_slot0[rec.elem] = at + sizeof(RecHdr) + 16 * (2 + ((rec.flags & TAG_MISAL) ? 4 : 0));
+      }
       prev_hdr = at;
       prev_elem = rec.elem;
       prev_p0 = rec.p0;
@@ -513,6 +521,7 @@ int xt::create_lattice(const void *packed, size_t nbytes, const PackOpts &po, xt
   lat->s_table_host = img.s_table;
   lat->extended = img.extended;
   lat->mult_slot0 = img.mult_slot0;
+  lat->mult_wf_off = img.mult_wf_off;
   lat->packed_host.assign(static_cast<const unsigned char *>(packed), static_cast<const unsigned char *>(packed) + nbytes);
 
   auto fail = [&](cudaError_t e, const char *what) {

@@ -25,6 +25,8 @@
 // by branch-free Newton sequences on the MUFU.RSQ64H / MUFU.RCP64H seeds (DESIGN.md section
 // 6.3): same formula, <= 2 ulp on the increments; the measured distance to the oracle is set by
 // FMA fusion, not by this block (<= 0.5 of the 1e-12 bar either way).
+#include <atomic>
+
 #include "xt_internal.h"
 
 namespace xt {
@@ -35,6 +37,7 @@ struct TrackArgs {
   const ChunkDesc *chunks;
   const double *s_table;
   const int64_t *n_active;  // device counter (compaction path) or nullptr
+  double *monitor_rows;     // where TAG_MON records store (xt_twiss4d_line), else nullptr
   xt_particles p;
   int64_t n_part;
   int64_t n_turns;
@@ -112,36 +115,6 @@ __device__ __forceinline__ double rcp_seed(double a) {
 }
 #endif
 
-// Where the thick quadrupole sits in the dispatch.  Its record never occurs in a thin lattice, but
-// the presence of the case label reshapes the compare tree ptxas builds for the switch: measured,
-// the 3-particle kernel is 1.2 % faster with the label (configs[2]) and the 4-particle one 1 %
-// faster without it (configs[3]).  So the thin 4-particle kernel parks the label on a key that
-// cannot occur (the switch key is 8 bits wide, the compiler drops the case).
-template <int P, bool THICK>
-struct QuadCase {
-  static constexpr uint32_t value = (P == 4 && !THICK) ? 0x1ffu : static_cast<uint32_t>(TAG_QUAD);
-};
-
-template <bool THICK>
-struct BendCase {  // thin kernels keep the dispatch tree they were measured with: the label is parked there
-  static constexpr uint32_t value = THICK ? static_cast<uint32_t>(TAG_BEND) : 0x2ffu;
-};
-
-template <bool THICK>
-struct RadCase {
-  static constexpr uint32_t value = THICK ? static_cast<uint32_t>(TAG_RMULT) : 0x5ffu;
-};
-
-template <bool THICK>
-struct MonCase {
-  static constexpr uint32_t value = THICK ? static_cast<uint32_t>(TAG_MON) : 0x4ffu;
-};
-
-template <bool THICK>
-struct PolyCase {
-  static constexpr uint32_t value = THICK ? static_cast<uint32_t>(TAG_POLY) : 0x3ffu;
-};
-
 constexpr int kPrefetch = 4;  // 16-byte slots of a record loaded ahead of its dispatch ...
 #ifndef XT_PF4
 #define XT_PF4 2
@@ -149,9 +122,9 @@ constexpr int kPrefetch = 4;  // 16-byte slots of a record loaded ahead of its d
 #ifndef XT_PF3
 #define XT_PF3 2
 #endif
-template <int P>
+template <int P, bool REG>
 struct Prefetched {  // ... of which this many really are (the rest is read where it is used)
-  static constexpr int value = P >= 4 ? XT_PF4 : (P == 3 ? XT_PF3 : kPrefetch);
+  static constexpr int value = REG ? kPrefetch : (P >= 4 ? XT_PF4 : (P == 3 ? XT_PF3 : kPrefetch));
 };
 
 // Hot per-thread state of P particles: what drifts and kicks touch at every element.
@@ -161,33 +134,59 @@ struct Parts {
   uint32_t alive;  // bit j: slot j holds a particle that is still being tracked
 };
 
-// Cold per-thread state, kept out of the register file (the Horner loop needs the
-// registers to interleave its P independent chains): functions of (delta, ptau), which only
-// a cavity changes.  ptau (cavities), delta and rv0v = (1 + beta0 ptau)/(1 + delta) (curved
-// multipoles), opd2 = (1 + delta)^2, b = 1 + beta0 ptau and g = ptau (ptau + 2/beta0)/gamma0^2
-// (drifts) live in shared memory, one row of 6P doubles per thread at compile-time offsets
-// from one base register; the row pitch is odd (in doubles) so that a warp's 64-bit
-// accesses are bank-conflict free.  rpp / rvv are written straight to global memory by the
-// cavity map; s / at_turn / at_element / state are touched only when a particle is lost and
-// at the end of the launch.
+// Cold per-thread state: functions of (delta, ptau), which only a cavity changes.  ptau
+// (cavities), delta and rv0v = (1 + beta0 ptau)/(1 + delta) (curved multipoles), opd2 =
+// (1 + delta)^2, b = 1 + beta0 ptau and g = ptau (ptau + 2/beta0)/gamma0^2 (drifts).  rpp / rvv are
+// written straight to global memory by the cavity map; s / at_turn / at_element / state are
+// touched only when a particle is lost and at the end of the launch.
+//
+// Two homes.  REG = false (large ensembles, 4 CTAs per SM at <= 128 registers): the values live in
+// shared memory, one row of 6P doubles per thread at compile-time offsets from one base
+// register; the row pitch is odd (in doubles) so that a warp's 64-bit accesses are bank-conflict
+// free; the Horner loop keeps the registers for its P independent chains.  REG = true (small
+// ensembles that leave the register file half empty, configs[2]: 8 warps per SM): the values stay
+// in registers, which takes ~6 LDS and their latency out of every record.
+template <int P, bool REG>
+struct Cold;
+
 template <int P>
-struct Cold {
+struct Cold<P, false> {
   static constexpr int kPitch = (6 * P) | 1;  // doubles per thread row
+  static constexpr bool kInRegs = false;
   double *row;    // this thread's row: P each of ptau, delta, rv0v, opd2, b, g
   int stride;     // blockDim.x
   int64_t first;  // index of slot 0's particle; slot j is first + j * stride
-  __device__ __forceinline__ double &ptau(int j) const { return row[j]; }
-  __device__ __forceinline__ double &delta(int j) const { return row[P + j]; }
-  __device__ __forceinline__ double &rv0v(int j) const { return row[2 * P + j]; }
-  __device__ __forceinline__ double &opd2(int j) const { return row[3 * P + j]; }
-  __device__ __forceinline__ double &b(int j) const { return row[4 * P + j]; }
-  __device__ __forceinline__ double &g(int j) const { return row[5 * P + j]; }
+  __device__ __forceinline__ void attach(unsigned char *smem_rows) {
+    row = reinterpret_cast<double *>(smem_rows) + static_cast<uint32_t>(kPitch) * threadIdx.x;
+  }
+  __device__ __forceinline__ double &ptau(int j) { return row[j]; }
+  __device__ __forceinline__ double &delta(int j) { return row[P + j]; }
+  __device__ __forceinline__ double &rv0v(int j) { return row[2 * P + j]; }
+  __device__ __forceinline__ double &opd2(int j) { return row[3 * P + j]; }
+  __device__ __forceinline__ double &b(int j) { return row[4 * P + j]; }
+  __device__ __forceinline__ double &g(int j) { return row[5 * P + j]; }
   __device__ __forceinline__ int64_t idx(int j) const { return first + static_cast<int64_t>(j) * stride; }
 };
 
 template <int P>
-__device__ __forceinline__ void refresh_cached(const Cold<P> &cold, int j, double opd, double b, double t,
-                                               double igam2) {
+struct Cold<P, true> {
+  static constexpr int kPitch = 0;  // no shared-memory rows
+  static constexpr bool kInRegs = true;
+  double v_ptau[P], v_delta[P], v_rv0v[P], v_opd2[P], v_b[P], v_g[P];
+  int stride;
+  int64_t first;
+  __device__ __forceinline__ void attach(unsigned char *) {}
+  __device__ __forceinline__ double &ptau(int j) { return v_ptau[j]; }
+  __device__ __forceinline__ double &delta(int j) { return v_delta[j]; }
+  __device__ __forceinline__ double &rv0v(int j) { return v_rv0v[j]; }
+  __device__ __forceinline__ double &opd2(int j) { return v_opd2[j]; }
+  __device__ __forceinline__ double &b(int j) { return v_b[j]; }
+  __device__ __forceinline__ double &g(int j) { return v_g[j]; }
+  __device__ __forceinline__ int64_t idx(int j) const { return first + static_cast<int64_t>(j) * stride; }
+};
+
+template <class ColdT>
+__device__ __forceinline__ void refresh_cached(ColdT &cold, int j, double opd, double b, double t, double igam2) {
   cold.opd2(j) = opd * opd;
   cold.b(j) = b;
   cold.g(j) = t * igam2;
@@ -220,27 +219,35 @@ __device__ __forceinline__ void horner_first(const double2 top, const double2 c,
   }
 }
 
-// pf = the first kPrefetch pairs, already in registers; the rest comes from cs (shared memory).
+// Order known at compile time (the orders a lattice is full of: N = 15 in configs[2-4]): fully unrolled,
+// no remainder branches, no loop; every coefficient sits at an immediate offset from the record, so
+// the LDS.128 are free to move up.  c0, c1 = the two leading pairs (prefetched before the dispatch).
+template <int P, int N>
+__device__ __forceinline__ void horner_fixed(const double2 *__restrict__ cs, const double2 c0, const double2 c1,
+                                             const double (&x)[P], const double (&y)[P], double (&re)[P],
+                                             double (&im)[P]) {
+  static_assert(N >= 1, "order 0 has no recurrence");
+  horner_first<P>(c0, c1, x, y, re, im);
+#pragma unroll
+  for (int k = 2; k <= N; ++k) horner_step<P>(cs[k], x, y, re, im);
+}
+
+// Any order (run time): (order mod 4) leading steps, then groups of four with the next group's first
+// pair loaded one group ahead.
 template <int P>
-__device__ __forceinline__ void horner(const double2 *__restrict__ cs, const double2 (&pf)[kPrefetch], int order,
-                                       const double (&x)[P], const double (&y)[P], double (&re)[P],
-                                       double (&im)[P]) {
-  static_assert(kPrefetch == 4, "the leading steps below take exactly the four leading pairs");
-  constexpr int kHave = Prefetched<P>::value;
-  // (order mod 4) leading steps, then groups of four
-  const double2 top = pf[0];
+__device__ __forceinline__ void horner(const double2 *__restrict__ cs, int order, const double (&x)[P],
+                                       const double (&y)[P], double (&re)[P], double (&im)[P]) {
+  const double2 top = cs[0];
   const int rem = order & 3;
   if (rem == 3) {
-    const double2 c2 = kHave > 2 ? pf[2] : cs[2], c3 = kHave > 3 ? pf[3] : cs[3];
-    horner_first<P>(top, pf[1], x, y, re, im);
-    horner_step<P>(c2, x, y, re, im);
-    horner_step<P>(c3, x, y, re, im);
+    horner_first<P>(top, cs[1], x, y, re, im);
+    horner_step<P>(cs[2], x, y, re, im);
+    horner_step<P>(cs[3], x, y, re, im);
   } else if (rem == 2) {
-    const double2 c2 = kHave > 2 ? pf[2] : cs[2];
-    horner_first<P>(top, pf[1], x, y, re, im);
-    horner_step<P>(c2, x, y, re, im);
+    horner_first<P>(top, cs[1], x, y, re, im);
+    horner_step<P>(cs[2], x, y, re, im);
   } else if (rem == 1) {
-    horner_first<P>(top, pf[1], x, y, re, im);
+    horner_first<P>(top, cs[1], x, y, re, im);
   } else {
 #pragma unroll
     for (int j = 0; j < P; ++j) {
@@ -253,7 +260,7 @@ __device__ __forceinline__ void horner(const double2 *__restrict__ cs, const dou
 #pragma unroll 1
   for (int k = rem + 1; k <= order; k += 4) {
     const double2 c1 = cs[1], c2 = cs[2], c3 = cs[3];
-    const double2 n0 = cs[4];  // may lie just past the record: never used then
+    const double2 n0 = cs[4];  // may lie just past the record (inside the stage buffer's spare bytes): never used then
     cs += 4;
     horner_step<P>(c0, x, y, re, im);
     horner_step<P>(c1, x, y, re, im);
@@ -282,9 +289,9 @@ __device__ __noinline__ void store_lost(const xt_particles p, const double *s_ta
 }
 
 // ... and park the slot on the reference orbit, where every map stays finite and cheap.
-template <int P>
-__device__ __forceinline__ void lose(Parts<P> &q, uint32_t out, const Cold<P> &cold, uint32_t elem,
-                                     int64_t turns_done, const TrackArgs &a) {
+template <int P, class ColdT>
+__device__ __forceinline__ void lose(Parts<P> &q, uint32_t out, ColdT &cold, uint32_t elem, int64_t turns_done,
+                                     const TrackArgs &a) {
 #pragma unroll
   for (int j = 0; j < P; ++j) {
     if (out & (1u << j)) {
@@ -306,8 +313,8 @@ struct DriftCoef {
   double u[P], v[P], gm[P];  // validation: 1/(pz (pz + b)), pz + b;  production: 1/pz, 1/(pz + b);  g - pxy2
 };
 
-template <int P>
-__device__ __forceinline__ void drift_eval(const Parts<P> &q, const Cold<P> &cold, DriftCoef<P> &d) {
+template <int P, class ColdT>
+__device__ __forceinline__ void drift_eval(const Parts<P> &q, ColdT &cold, DriftCoef<P> &d) {
   double opd2[P], b[P], g[P];
 #pragma unroll
   for (int j = 0; j < P; ++j) {
@@ -358,8 +365,8 @@ __device__ __forceinline__ void drift_apply(Parts<P> &q, const DriftCoef<P> &d, 
   }
 }
 
-template <int P>
-__device__ __forceinline__ void drift(Parts<P> &q, const Cold<P> &cold, const double length) {
+template <int P, class ColdT>
+__device__ __forceinline__ void drift(Parts<P> &q, ColdT &cold, const double length) {
   DriftCoef<P> d;
   drift_eval<P>(q, cold, d);
   drift_apply<P>(q, d, length);
@@ -391,37 +398,43 @@ __device__ __forceinline__ void xy_shift(Parts<P> &q, const double2 d) {  // d =
 }
 
 // One multipole record: [drift] [shift, rotate] kick [rotate, shift] [drift [drift]] with one
-// dispatch.  F >= 0 fixes the flag set at compile time (no flag branches), F < 0 reads it
-// from the tag; CURVED likewise (1: TAG_CMULT, 0: TAG_MULT, < 0: from the tag).  pf holds the
-// first kPrefetch slots of the record, loaded before the dispatch.
-template <int P, int F, int CURVED>
-__device__ __forceinline__ void multipole_record(Parts<P> &q, const Cold<P> &cold, const double2 *slots,
+// dispatch.  Slots (xt_internal.h): {l_pre, l_post} {l_post2, wf} [4 misalignment slots] pairs.
+// F >= 0 fixes the flag set at compile time (no flag branches), F < 0 reads it from the tag;
+// CURVED likewise (1: TAG_CMULT, 0: TAG_MULT, < 0: from the tag); ORDER >= 1 fixes the order (fully
+// unrolled Horner, F must not contain TAG_MISAL), ORDER < 0 reads it from the tag.  pf holds the first
+// kPrefetch slots of the record, loaded before the dispatch: the two extras and, without
+// misalignment, the two leading pairs.
+template <int P, int F, int CURVED, int ORDER, class ColdT>
+__device__ __forceinline__ void multipole_record(Parts<P> &q, ColdT &cold, const double2 *slots,
                                                  const double2 (&pf)[kPrefetch], const uint32_t tag,
                                                  const double p0) {
   const uint32_t f = F >= 0 ? static_cast<uint32_t>(F) : tag;
   const bool curved = CURVED >= 0 ? (CURVED != 0) : ((tag & TAG_TYPE_MASK) == TAG_CMULT);
-  const int order = static_cast<int>((tag >> 8) & 0x7fu);
-  const double2 *extra = slots + order + 1;  // behind the coefficient pairs
-  double wf = 0.0;
-  double2 dl = make_double2(0.0, 0.0);
-  double l_post2 = 0.0;
-  if (curved) wf = (extra++)->x;
-  if (f & (TAG_PRE | TAG_POST)) dl = *extra++;
-  if (f & TAG_POST2) l_post2 = (extra++)->x;
+  const double2 dl = pf[0];                  // {l_pre, l_post}
+  const double2 l2wf = pf[1];                // {l_post2, wf}
+  const double2 *mis = slots + 2;            // misalignment slots, if any
   if (f & TAG_PRE) drift<P>(q, cold, dl.x);
   if (f & TAG_MISAL) {
-    xy_shift<P>(q, extra[0]);
-    s_rotation<P>(q, extra[1]);
+    xy_shift<P>(q, mis[0]);
+    s_rotation<P>(q, mis[1]);
   }
   double re[P], im[P];
-  horner<P>(slots, pf, order, q.x, q.y, re, im);
+  if (ORDER >= 1) {
+    constexpr int kHave = Prefetched<P, ColdT::kInRegs>::value;
+    const double2 *cs = slots + 2;
+    horner_fixed<P, (ORDER >= 1 ? ORDER : 1)>(cs, kHave > 2 ? pf[2] : cs[0], kHave > 3 ? pf[3] : cs[1], q.x, q.y, re,
+                                               im);
+  } else {
+    const int order = static_cast<int>((tag >> 8) & 0x7fu);
+    horner<P>(slots + ((f & TAG_MISAL) ? 6 : 2), order, q.x, q.y, re, im);
+  }
 #pragma unroll
   for (int j = 0; j < P; ++j) {
     q.px[j] = q.px[j] - re[j];
     q.py[j] = q.py[j] + im[j];
   }
   if (curved) {
-    const double hxl = p0;
+    const double hxl = p0, wf = l2wf.y;
 #pragma unroll
     for (int j = 0; j < P; ++j) {
       q.px[j] = XT_MADD(hxl, cold.delta(j), q.px[j]);
@@ -430,107 +443,135 @@ __device__ __forceinline__ void multipole_record(Parts<P> &q, const Cold<P> &col
     }
   }
   if (f & TAG_MISAL) {
-    s_rotation<P>(q, extra[2]);
-    xy_shift<P>(q, extra[3]);
+    s_rotation<P>(q, mis[2]);
+    xy_shift<P>(q, mis[3]);
   }
   if (f & TAG_POST) {
     DriftCoef<P> d;
     drift_eval<P>(q, cold, d);
     drift_apply<P>(q, d, dl.y);
-    if (f & TAG_POST2) drift_apply<P>(q, d, l_post2);
+    if (f & TAG_POST2) drift_apply<P>(q, d, l2wf.x);
   }
 }
+
+// ---------------------------------------------------------------------------------------------------
+// Maps of the extended kernels (thick elements, polygons, radiation, monitors).  They are out of line,
+// but take ONE particle by value and return its new coordinates by value: arguments and results travel
+// in registers, the callers index their P slots statically, and nothing of the hot state is ever
+// forced into local memory (round 1 passed Parts<P>& and indexed it in a rolled loop: 600-2200
+// LDL/STL per kernel).
+struct Hot {
+  double x, px, y, py, zeta;
+};
 
 // Thick quadrupole (reading A18): the exact flow of
 // H = (px^2 + py^2)/(2(1+delta)) + (k1/2)(x^2 - y^2) over the length.  With w = sqrt(|k1|/(1+delta))
 // the focusing plane turns by w L (cos, sin), the other follows cosh, sinh; the path length is
 // zeta += L g/((1+delta)((1+delta)+b)) - rv0v/(2(1+delta)^2) int (px^2 + py^2) ds (closed form below).
-// The sign of k1/(1+delta) is the sign of k1 for every physical particle: a warp-uniform branch.
-// Only compiled into the THICK instantiations of the kernel: lattices without thick elements run
-// the same code as before.
-template <int P>
-__device__ __noinline__ void thick_quadrupole(Parts<P> &q, const Cold<P> &cold, const double k1, const double length) {
-#pragma unroll 1
-  for (int j = 0; j < P; ++j) {
-    const double opd = 1.0 + cold.delta(j);
-    const double rk = k1 / opd;
-    const double w = sqrt(fabs(rk));
-    const double wl = XT_MUL(w, length);
-    double sn, cs;
-    sincos(wl, &sn, &cs);
-    const double ch = cosh(wl), sh = sinh(wl);
-    const double ow = XT_MUL(opd, w);
-    const double iw = 1.0 / ow;
-    const bool focus_x = rk > 0.0;
-    const double u = focus_x ? q.x[j] : q.y[j], pu = focus_x ? q.px[j] : q.py[j];
-    const double v = focus_x ? q.y[j] : q.x[j], pv = focus_x ? q.py[j] : q.px[j];
-    const double au = XT_MUL(ow, u);
-    const double av = XT_MUL(ow, v);
-    const double u1 = XT_MADD(u, cs, XT_MUL(XT_MUL(pu, iw), sn));
-    const double pu1 = XT_NMADD(au, sn, XT_MUL(pu, cs));
-    const double v1 = XT_MADD(v, ch, XT_MUL(XT_MUL(pv, iw), sh));
-    const double pv1 = XT_MADD(pv, ch, XT_MUL(av, sh));
-    const double hl = XT_MUL(0.5, length);
-    const double h2w = 0.5 / w;
-    const double pu2 = XT_MUL(pu, pu), au2 = XT_MUL(au, au), pv2 = XT_MUL(pv, pv), av2 = XT_MUL(av, av);
-    const double i_f = XT_MADD(pu2 + au2, hl, XT_MUL(XT_MUL(pu2 - au2, XT_MUL(sn, cs)), h2w)) -
-                       XT_MUL(XT_MUL(au, pu), XT_MUL(sn, sn)) / w;
-    const double i_d = XT_MADD(pv2 - av2, hl, XT_MUL(XT_MUL(pv2 + av2, XT_MUL(sh, ch)), h2w)) +
-                       XT_MUL(XT_MUL(av, pv), XT_MUL(sh, sh)) / w;
-    const double slip = XT_MUL(length, cold.g(j) / XT_MUL(opd, opd + cold.b(j)));
-    q.zeta[j] = (q.zeta[j] + slip) - XT_MUL(cold.rv0v(j) / XT_MUL(2.0, cold.opd2(j)), i_f + i_d);
-    if (focus_x) {
-      q.x[j] = u1;
-      q.px[j] = pu1;
-      q.y[j] = v1;
-      q.py[j] = pv1;
-    } else {
-      q.y[j] = u1;
-      q.py[j] = pu1;
-      q.x[j] = v1;
-      q.px[j] = pv1;
-    }
-  }
+__device__ __noinline__ Hot thick_quadrupole_one(Hot h, const double delta, const double opd2, const double b,
+                                                 const double g, const double rv0v, const double k1,
+                                                 const double length) {
+  const double opd = 1.0 + delta;
+  const double rk = k1 / opd;
+  const double w = sqrt(fabs(rk));
+  const double wl = XT_MUL(w, length);
+  double sn, cs;
+  sincos(wl, &sn, &cs);
+  const double ch = cosh(wl), sh = sinh(wl);
+  const double ow = XT_MUL(opd, w);
+  const double iw = 1.0 / ow;
+  const bool focus_x = rk > 0.0;
+  const double u = focus_x ? h.x : h.y, pu = focus_x ? h.px : h.py;
+  const double v = focus_x ? h.y : h.x, pv = focus_x ? h.py : h.px;
+  const double au = XT_MUL(ow, u);
+  const double av = XT_MUL(ow, v);
+  const double u1 = XT_MADD(u, cs, XT_MUL(XT_MUL(pu, iw), sn));
+  const double pu1 = XT_NMADD(au, sn, XT_MUL(pu, cs));
+  const double v1 = XT_MADD(v, ch, XT_MUL(XT_MUL(pv, iw), sh));
+  const double pv1 = XT_MADD(pv, ch, XT_MUL(av, sh));
+  const double hl = XT_MUL(0.5, length);
+  const double h2w = 0.5 / w;
+  const double pu2 = XT_MUL(pu, pu), au2 = XT_MUL(au, au), pv2 = XT_MUL(pv, pv), av2 = XT_MUL(av, av);
+  const double i_f = XT_MADD(pu2 + au2, hl, XT_MUL(XT_MUL(pu2 - au2, XT_MUL(sn, cs)), h2w)) -
+                     XT_MUL(XT_MUL(au, pu), XT_MUL(sn, sn)) / w;
+  const double i_d = XT_MADD(pv2 - av2, hl, XT_MUL(XT_MUL(pv2 + av2, XT_MUL(sh, ch)), h2w)) +
+                     XT_MUL(XT_MUL(av, pv), XT_MUL(sh, sh)) / w;
+  const double slip = XT_MUL(length, g / XT_MUL(opd, opd + b));
+  Hot o;
+  o.zeta = (h.zeta + slip) - XT_MUL(rv0v / XT_MUL(2.0, opd2), i_f + i_d);
+  o.x = focus_x ? u1 : v1;
+  o.px = focus_x ? pu1 : pv1;
+  o.y = focus_x ? v1 : u1;
+  o.py = focus_x ? pv1 : pu1;
+  return o;
 }
 
 // Thick sector bend, 'expanded' model (reading A19):
 // the exact flow of H = (px^2 + py^2)/(2(1+delta)) - h x (1+delta) + k0 x + (k0 h/2) x^2, i.e. the
 // thin curved multipole of step M2 smeared over the arc length.  Same arithmetic as the oracle's.
-template <int P>
-__device__ __noinline__ void thick_bend(Parts<P> &q, const Cold<P> &cold, const double k0, const double h,
-                                        const double length) {
-#pragma unroll 1
+__device__ __noinline__ Hot thick_bend_one(Hot p, const double delta, const double opd2, const double b,
+                                           const double g, const double rv, const double k0, const double h,
+                                           const double length) {
+  const double opd = 1.0 + delta;
+  const double w = sqrt(XT_MUL(k0, h) / opd);
+  const double wl = XT_MUL(w, length);
+  double sn, cs;
+  sincos(wl, &sn, &cs);
+  const double c1 = 1.0 - cs;
+  const double ow = XT_MUL(opd, w);
+  const double fw = XT_NMADD(1.0, k0, XT_MUL(h, opd)) / w;  // (h (1+delta) - k0)/w
+  const double x = p.x, px = p.px, py = p.py;
+  const double a = XT_MADD(ow, x, -fw);
+  const double pw = px / ow;
+  const double x1 = XT_MADD(x, cs, XT_MUL(pw, sn)) + XT_MUL(fw, c1) / ow;
+  const double px1 = XT_NMADD(a, sn, XT_MUL(px, cs));
+  const double ix = (XT_MUL(x, sn) / w + XT_MUL(pw, c1) / w) + XT_MUL(fw / ow, length - sn / w);
+  const double px2 = XT_MUL(px, px), a2 = XT_MUL(a, a);
+  const double ip = XT_MADD(px2 + a2, XT_MUL(0.5, length), XT_MUL(XT_MUL(px2 - a2, XT_MUL(sn, cs)), 0.5 / w)) -
+                    XT_MUL(XT_MUL(a, px), XT_MUL(sn, sn)) / w;
+  const double slip = XT_MUL(length, g / XT_MUL(opd, opd + b));
+  Hot o;
+  o.zeta = ((p.zeta + slip) - XT_MUL(XT_MUL(rv, h), ix)) -
+           XT_MUL(rv / XT_MUL(2.0, opd2), ip + XT_MUL(length, XT_MUL(py, py)));
+  o.y = XT_MUL(length, py) / opd + p.y;
+  o.py = py;
+  o.x = x1;
+  o.px = px1;
+  return o;
+}
+
+template <int P, class ColdT>
+__device__ __forceinline__ void thick_quadrupole(Parts<P> &q, ColdT &cold, const double k1, const double length) {
+#pragma unroll
   for (int j = 0; j < P; ++j) {
-    const double opd = 1.0 + cold.delta(j);
-    const double w = sqrt(XT_MUL(k0, h) / opd);
-    const double wl = XT_MUL(w, length);
-    double sn, cs;
-    sincos(wl, &sn, &cs);
-    const double c1 = 1.0 - cs;
-    const double ow = XT_MUL(opd, w);
-    const double fw = XT_NMADD(1.0, k0, XT_MUL(h, opd)) / w;  // (h (1+delta) - k0)/w
-    const double x = q.x[j], px = q.px[j], py = q.py[j];
-    const double a = XT_MADD(ow, x, -fw);
-    const double pw = px / ow;
-    const double x1 = XT_MADD(x, cs, XT_MUL(pw, sn)) + XT_MUL(fw, c1) / ow;
-    const double px1 = XT_NMADD(a, sn, XT_MUL(px, cs));
-    const double ix = (XT_MUL(x, sn) / w + XT_MUL(pw, c1) / w) + XT_MUL(fw / ow, length - sn / w);
-    const double px2 = XT_MUL(px, px), a2 = XT_MUL(a, a);
-    const double ip = XT_MADD(px2 + a2, XT_MUL(0.5, length), XT_MUL(XT_MUL(px2 - a2, XT_MUL(sn, cs)), 0.5 / w)) -
-                      XT_MUL(XT_MUL(a, px), XT_MUL(sn, sn)) / w;
-    const double rv = cold.rv0v(j);
-    const double slip = XT_MUL(length, cold.g(j) / XT_MUL(opd, opd + cold.b(j)));
-    q.zeta[j] = ((q.zeta[j] + slip) - XT_MUL(XT_MUL(rv, h), ix)) -
-                XT_MUL(rv / XT_MUL(2.0, cold.opd2(j)), ip + XT_MUL(length, XT_MUL(py, py)));
-    q.y[j] = XT_MUL(length, py) / opd + q.y[j];
-    q.x[j] = x1;
-    q.px[j] = px1;
+    const Hot o = thick_quadrupole_one(Hot{q.x[j], q.px[j], q.y[j], q.py[j], q.zeta[j]}, cold.delta(j), cold.opd2(j),
+                                       cold.b(j), cold.g(j), cold.rv0v(j), k1, length);
+    q.x[j] = o.x;
+    q.px[j] = o.px;
+    q.y[j] = o.y;
+    q.py[j] = o.py;
+    q.zeta[j] = o.zeta;
+  }
+}
+
+template <int P, class ColdT>
+__device__ __forceinline__ void thick_bend(Parts<P> &q, ColdT &cold, const double k0, const double h,
+                                           const double length) {
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    const Hot o = thick_bend_one(Hot{q.x[j], q.px[j], q.y[j], q.py[j], q.zeta[j]}, cold.delta(j), cold.opd2(j),
+                                 cold.b(j), cold.g(j), cold.rv0v(j), k0, h, length);
+    q.x[j] = o.x;
+    q.px[j] = o.px;
+    q.y[j] = o.y;
+    q.py[j] = o.py;
+    q.zeta[j] = o.zeta;
   }
 }
 
 // A: elliptical aperture (x^2 b^2 + y^2 a^2 <= a^2 b^2, edge inclusive, NaN lost).
-template <int P>
-__device__ __forceinline__ void limit_ellipse(Parts<P> &q, const Cold<P> &cold, const double2 ba, const double a2b2,
+template <int P, class ColdT>
+__device__ __forceinline__ void limit_ellipse(Parts<P> &q, ColdT &cold, const double2 ba, const double a2b2,
                                               uint32_t elem, int64_t turns_done, const TrackArgs &a) {
   uint32_t out = 0;
 #pragma unroll
@@ -545,9 +586,9 @@ __device__ __forceinline__ void limit_ellipse(Parts<P> &q, const Cold<P> &cold, 
 // A: polygon aperture (even-odd rule; reading A20): the half line from the particle towards +x
 // crosses edge (v[i-1] -> v[i]) iff its ends lie on different sides of the horizontal through the particle
 // and the crossing point is to the right of it.  NaN crosses nothing: lost.  THICK kernels only.
-template <int P>
-__device__ __noinline__ void limit_polygon(Parts<P> &q, const Cold<P> &cold, const double2 *v, int n, uint32_t elem,
-                                           int64_t turns_done, const TrackArgs &a) {
+template <int P, class ColdT>
+__device__ __forceinline__ void limit_polygon(Parts<P> &q, ColdT &cold, const double2 *v, int n, uint32_t elem,
+                                              int64_t turns_done, const TrackArgs &a) {
   uint32_t in = 0;
   double2 vj = v[n - 1];
 #pragma unroll 1
@@ -571,67 +612,86 @@ __device__ __noinline__ void limit_polygon(Parts<P> &q, const Cold<P> &cold, con
 // fraction r = krad (1+delta) kick^2 / lpath of the particle's energy is radiated, half before the kick and
 // half after; delta follows from the energy as behind a cavity, px and py shrink with the momentum.
 // slots: (c[n], s[n]) pairs n = N .. 0 with c[0] = knl[0] - hxl, {wf, length}, {krad, 0}.  THICK kernels only.
-template <int P>
-__device__ __noinline__ void rad_multipole(Parts<P> &q, const Cold<P> &cold, const double2 *slots, int order,
-                                           double hxl, const TrackArgs &a) {
+// One particle by value in, its new state by value out (see Hot above).
+struct RadOut {
+  double px, py, zeta, ptau, delta, opd, b, t;
+};
+
+__device__ __noinline__ RadOut rad_multipole_one(const double x, const double y, double px, double py, double zeta,
+                                                 double ptau, double delta, const double2 *slots, const int order,
+                                                 const double hxl, const double beta0, const double tib) {
   const double2 wl = slots[order + 1], kr = slots[order + 2];
-  const double ib = 1.0 / a.beta0;
+  const double ib = 1.0 / beta0;
+  double re = slots[0].x, im = slots[0].y;
+#pragma unroll 1
+  for (int n = 1; n <= order; ++n) {
+    const double2 c = slots[n];
+    const double nre = XT_MADD(re, x, XT_NMADD(im, y, c.x));
+    const double nim = XT_MADD(re, y, XT_MADD(im, x, c.y));
+    re = nre;
+    im = nim;
+  }
+  const double dpxf = XT_NMADD(wl.x, x, -re - hxl);  // the field's kick (re has the curvature folded in)
+  const double dpyf = im;
+  const double kick2 = XT_MADD(dpxf, dpxf, XT_MUL(dpyf, dpyf));
+  const double lpath = XT_MADD(hxl, x, wl.y);
+  RadOut o{};
+#pragma unroll 1
+  for (int half = 0; half < 2; ++half) {
+    const double opd = 1.0 + delta;
+    const double rh = XT_MUL(0.5 * kr.x, XT_MUL(opd, kick2)) / lpath;
+    ptau = XT_NMADD(rh, ptau + ib, ptau);
+    const double t = XT_MUL(ptau, ptau + tib);
+    delta = t / (sqrt(t + 1.0) + 1.0);
+    const double opd1 = 1.0 + delta;
+    const double f = opd1 / opd;
+    px = XT_MUL(px, f);
+    py = XT_MUL(py, f);
+    const double b = XT_MADD(beta0, ptau, 1.0);
+    o.opd = opd1;
+    o.b = b;
+    o.t = t;
+    if (half == 0) {  // the thin kick itself, in the arithmetic of the plain multipole
+      px = px - re;
+      py = py + im;
+      px = XT_MADD(hxl, delta, px);
+      px = XT_NMADD(wl.x, x, px);
+      zeta = XT_NMADD(XT_MUL(hxl, x), b / opd1, zeta);  // b/opd1 = the refreshed rv0v
+    }
+  }
+  o.px = px;
+  o.py = py;
+  o.zeta = zeta;
+  o.ptau = ptau;
+  o.delta = delta;
+  return o;
+}
+
+template <int P, class ColdT>
+__device__ __forceinline__ void rad_multipole(Parts<P> &q, ColdT &cold, const double2 *slots, int order, double hxl,
+                                              const TrackArgs &a) {
 #pragma unroll
   for (int j = 0; j < P; ++j) {
     if (!(q.alive & (1u << j))) continue;
-    const double x = q.x[j], y = q.y[j];
-    double re = slots[0].x, im = slots[0].y;
-#pragma unroll 1
-    for (int n = 1; n <= order; ++n) {
-      const double2 c = slots[n];
-      const double nre = XT_MADD(re, x, XT_NMADD(im, y, c.x));
-      const double nim = XT_MADD(re, y, XT_MADD(im, x, c.y));
-      re = nre;
-      im = nim;
-    }
-    const double dpxf = XT_NMADD(wl.x, x, -re - hxl);  // the field's kick (re has the curvature folded in)
-    const double dpyf = im;
-    const double kick2 = XT_MADD(dpxf, dpxf, XT_MUL(dpyf, dpyf));
-    const double lpath = XT_MADD(hxl, x, wl.y);
-    double px = q.px[j], py = q.py[j], ptau = cold.ptau(j), delta = cold.delta(j);
-#pragma unroll 1
-    for (int half = 0; half < 2; ++half) {
-      const double opd = 1.0 + delta;
-      const double rh = XT_MUL(0.5 * kr.x, XT_MUL(opd, kick2)) / lpath;
-      ptau = XT_NMADD(rh, ptau + ib, ptau);
-      const double t = XT_MUL(ptau, ptau + a.tib);
-      delta = t / (sqrt(t + 1.0) + 1.0);
-      const double opd1 = 1.0 + delta;
-      const double f = opd1 / opd;
-      px = XT_MUL(px, f);
-      py = XT_MUL(py, f);
-      const double b = XT_MADD(a.beta0, ptau, 1.0);
-      refresh_cached<P>(cold, j, opd1, b, t, a.igam2);
-      if (half == 0) {  // the thin kick itself, in the arithmetic of the plain multipole
-        px = px - re;
-        py = py + im;
-        px = XT_MADD(hxl, delta, px);
-        px = XT_NMADD(wl.x, x, px);
-        q.zeta[j] = XT_NMADD(XT_MUL(hxl, x), cold.rv0v(j), q.zeta[j]);
-      } else {
-        a.p.rpp[cold.idx(j)] = 1.0 / opd1;
-        a.p.rvv[cold.idx(j)] = opd1 / b;
-      }
-    }
-    q.px[j] = px;
-    q.py[j] = py;
-    cold.ptau(j) = ptau;
-    cold.delta(j) = delta;
+    const RadOut o = rad_multipole_one(q.x[j], q.y[j], q.px[j], q.py[j], q.zeta[j], cold.ptau(j), cold.delta(j), slots,
+                                       order, hxl, a.beta0, a.tib);
+    q.px[j] = o.px;
+    q.py[j] = o.py;
+    q.zeta[j] = o.zeta;
+    cold.ptau(j) = o.ptau;
+    cold.delta(j) = o.delta;
+    refresh_cached(cold, j, o.opd, o.b, o.t, a.igam2);
+    a.p.rpp[cold.idx(j)] = 1.0 / o.opd;
+    a.p.rvv[cold.idx(j)] = o.opd / o.b;
   }
 }
 
-// Internal monitor record (xt_twiss4d_line): row p0 of the monitor buffer receives the coordinates of every
-// alive particle of this thread.  THICK kernels only.
-__constant__ double *g_monitor_rows;
-
-template <int P>
-__device__ __noinline__ void monitor_store(const Parts<P> &q, const Cold<P> &cold, double row, int64_t n_part) {
-  double *base = g_monitor_rows + static_cast<int64_t>(row) * n_part * 6;
+// Internal monitor record (xt_twiss4d_line): row p0 of the monitor buffer (TrackArgs::monitor_rows, set per
+// call: no process-global state) receives the coordinates of every alive particle of this thread.
+// THICK kernels only.
+template <int P, class ColdT>
+__device__ __forceinline__ void monitor_store(const Parts<P> &q, ColdT &cold, double row, const TrackArgs &a) {
+  double *base = a.monitor_rows + static_cast<int64_t>(row) * a.n_part * 6;
 #pragma unroll
   for (int j = 0; j < P; ++j) {
     if (q.alive & (1u << j)) {
@@ -648,10 +708,16 @@ __device__ __noinline__ void monitor_store(const Parts<P> &q, const Cold<P> &col
 
 // Push the P particles of this thread through every record of one staged chunk.
 // Returns the position just behind the chunk (where the next chunk of the image starts).
-template <int P, bool THICK>
-__device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const unsigned char *rp,
-                                                            const Cold<P> &cold, int64_t turns_done,
-                                                            const TrackArgs &a) {
+//
+// Dispatch: a switch on type | flags | order of the (warp-uniform) tag.  The records a thin
+// drift-kick-drift lattice is made of -- order-15 multipoles (straight and curved) with the flag sets
+// none, POST, POST+POST2, PRE+POST+POST2 -- have handlers in which flags, curvature and order are
+// compile-time constants: no flag branches, no remainder branches, a fully unrolled Horner whose
+// coefficient loads all sit at immediate offsets.  Every other multipole takes the same code with
+// flags and order read at run time.
+template <int P, bool THICK, class ColdT>
+__device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const unsigned char *rp, ColdT &cold,
+                                                            int64_t turns_done, const TrackArgs &a) {
   uint32_t tag = reinterpret_cast<const RecHdr *>(rp)->next;  // chunk preamble
   rp += sizeof(RecHdr);
   while ((tag & TAG_TYPE_MASK) != TAG_END) {
@@ -659,13 +725,25 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
     const double2 *slots = reinterpret_cast<const double2 *>(rp + sizeof(RecHdr));
     // the first slots, loaded before the dispatch resolves (whatever the record is; at the end
     // of a chunk this reads up to 64 spare bytes behind it)
-    constexpr int kHave = Prefetched<P>::value;
+    constexpr int kHave = Prefetched<P, ColdT::kInRegs>::value;
     const double2 zero2 = make_double2(0.0, 0.0);
     const double2 pf[kPrefetch] = {slots[0], slots[1], kHave > 2 ? slots[2] : zero2, kHave > 3 ? slots[3] : zero2};
     const double p0 = h.p0;
     const uint32_t elem = h.elem;
     rp += tag >> 16;  // record size in bytes
-    switch (tag & 0xffu) {  // type | flags
+#ifndef XT_FIXED_ORDER
+#define XT_FIXED_ORDER 15  // the multipole order with fully unrolled handlers (0: none, order always read at run time)
+#endif
+#if XT_FIXED_ORDER > 0
+    constexpr uint32_t kKeyMask = 0x7fffu;  // type | flags | order << 8
+    constexpr uint32_t kOrd = static_cast<uint32_t>(XT_FIXED_ORDER);
+    constexpr int kOrdT = XT_FIXED_ORDER;
+#else
+    constexpr uint32_t kKeyMask = 0xffu;  // type | flags
+    constexpr uint32_t kOrd = 0u;
+    constexpr int kOrdT = -1;
+#endif
+    switch (tag & kKeyMask) {
       case TAG_DRIFT:
       case TAG_DRIFT | TAG_POST: {
         DriftCoef<P> d;
@@ -674,18 +752,17 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
         if (tag & TAG_POST) drift_apply<P>(q, d, pf[0].x);  // a second drift, same (px, py)
         break;
       }
-#define XT_MULT_CASE(F)                                                        \
-  case TAG_MULT | (F):                                                         \
-    multipole_record<P, (F), 0>(q, cold, slots, pf, tag, p0);                  \
+#define XT_MULT_CASE(F, N, NT)                                                 \
+  case TAG_MULT | (F) | ((N) << 8):                                            \
+    multipole_record<P, (F), 0, (NT)>(q, cold, slots, pf, tag, p0);            \
     break;                                                                     \
-  case TAG_CMULT | (F):                                                        \
-    multipole_record<P, (F), 1>(q, cold, slots, pf, tag, p0);                  \
+  case TAG_CMULT | (F) | ((N) << 8):                                           \
+    multipole_record<P, (F), 1, (NT)>(q, cold, slots, pf, tag, p0);            \
     break;
-      // the flag sets a drift-kick-drift lattice is made of, specialised at compile time ...
-      XT_MULT_CASE(0)
-      XT_MULT_CASE(TAG_POST)
-      XT_MULT_CASE(TAG_POST | TAG_POST2)
-      XT_MULT_CASE(TAG_PRE | TAG_POST | TAG_POST2)
+      XT_MULT_CASE(0u, kOrd, kOrdT)
+      XT_MULT_CASE(TAG_POST, kOrd, kOrdT)
+      XT_MULT_CASE(TAG_POST | TAG_POST2, kOrd, kOrdT)
+      XT_MULT_CASE(TAG_PRE | TAG_POST | TAG_POST2, kOrd, kOrdT)
 #undef XT_MULT_CASE
       case TAG_CAVITY: {
         const double2 kv = pf[0];  // (kz, vn)
@@ -702,7 +779,7 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
             cold.delta(j) = delta;
             a.p.rpp[cold.idx(j)] = 1.0 / opd;
             a.p.rvv[cold.idx(j)] = opd / b;
-            refresh_cached<P>(cold, j, opd, b, t, a.igam2);
+            refresh_cached(cold, j, opd, b, t, a.igam2);
           }
         }
         break;
@@ -735,32 +812,21 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
         limit_ellipse<P>(q, cold, pf[0], p0, elem, turns_done, a);  // pf[0] = (b2, a2), p0 = a2 b2
         break;
       }
-      case QuadCase<P, THICK>::value: {  // thick quadrupole (see QuadCase)
-        if (THICK) thick_quadrupole<P>(q, cold, p0, pf[0].x);  // p0 = k1, pf[0].x = length
+      default: {
+        const uint32_t type = tag & TAG_TYPE_MASK;
+        if (type == TAG_MULT || type == TAG_CMULT) {  // any other order / flag set (misaligned magnets): run time
+          multipole_record<P, -1, -1, -1>(q, cold, slots, pf, tag, p0);
+        } else if (THICK) {  // the extended maps: only lattices that contain them run these instantiations
+          const int order = static_cast<int>((tag >> 8) & 0x7fu);
+          if (type == TAG_QUAD) thick_quadrupole<P>(q, cold, p0, pf[0].x);                 // p0 = k1, {length, 0}
+          else if (type == TAG_BEND) thick_bend<P>(q, cold, p0, pf[0].x, pf[0].y);         // p0 = k0, {h, length}
+          else if (type == TAG_RMULT) rad_multipole<P>(q, cold, slots, order, p0, a);      // p0 = hxl
+          else if (type == TAG_MON) monitor_store<P>(q, cold, p0, a);                      // p0 = row
+          else if (type == TAG_POLY)  // (record bytes - header) / 16 vertices
+            limit_polygon<P>(q, cold, slots, static_cast<int>(((tag >> 16) - sizeof(RecHdr)) / 16), elem, turns_done, a);
+        }
         break;
       }
-      case BendCase<THICK>::value: {  // thick sector bend: p0 = k0, pf[0] = (h, length)
-        if (THICK) thick_bend<P>(q, cold, p0, pf[0].x, pf[0].y);
-        break;
-      }
-      case RadCase<THICK>::value: {  // radiating multipole: p0 = hxl
-        if (THICK) rad_multipole<P>(q, cold, slots, static_cast<int>((tag >> 8) & 0x7fu), p0, a);
-        break;
-      }
-      case MonCase<THICK>::value: {
-        if (THICK) monitor_store<P>(q, cold, p0, a.n_part);
-        break;
-      }
-      case PolyCase<THICK>::value: {  // polygon aperture: (record bytes - header) / 16 vertices
-        if (THICK) limit_polygon<P>(q, cold, slots, static_cast<int>(((tag >> 16) - sizeof(RecHdr)) / 16), elem, turns_done, a);
-        break;
-      }
-      default:  // ... and every other combination (misaligned magnets, lone leading drifts) at run time
-        if ((tag & TAG_TYPE_MASK) == TAG_MULT || (tag & TAG_TYPE_MASK) == TAG_CMULT)
-          multipole_record<P, -1, -1>(q, cold, slots, pf, tag, p0);
-        else if (THICK && (tag & 0xffu) == TAG_QUAD)  // instantiations whose QuadCase label is parked
-          thick_quadrupole<P>(q, cold, p0, pf[0].x);
-        break;
     }
     if (tag & TAG_APER) {
       // the record ends with an elliptical aperture: {b2, a2}, {a2 b2, element index} are its last slots
@@ -780,24 +846,32 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
 #ifndef XT_REGS4
 #define XT_REGS4 128
 #endif
+#ifndef XT_REGS3R
+#define XT_REGS3R 255
+#endif
 // (CTAs are at most 256 threads: xt_api.cu)
-template <int P>
+// The extended kernels call the out-of-line thick maps: their small shapes get room for the call's live
+// state (at 64 / 80 registers they spilled ~100 values around every call).
+template <int P, bool REG, bool THICK>
 struct RegBudget {
-  static constexpr int value = P == 1 ? 64 : (P == 2 ? 80 : (P == 3 ? XT_REGS3 : XT_REGS4));
+  static constexpr int value = REG ? (P == 3 ? XT_REGS3R : 255)
+                                   : (P == 1 ? (THICK ? 96 : 64) : (P == 2 ? (THICK ? 128 : 80) : (P == 3 ? XT_REGS3 : XT_REGS4)));
 };
 
-// Shared memory: [0,16) two mbarriers; [128, 128 + 8*kPitch*blockDim) cold per-thread rows;
-// then staging buffer 0 (and buffer 1 for multi-chunk lattices), 128-byte aligned, and 64
-// spare bytes (the Horner loop prefetches one coefficient pair past the record it is in).
-template <int P, bool THICK>
-__global__ void __maxnreg__(RegBudget<P>::value) xt_track_kernel(const TrackArgs a) {
+// Shared memory: [0,16) two mbarriers; [128, 128 + 8*kPitch*blockDim) cold per-thread rows (none when
+// the cold state lives in registers); then staging buffer 0 (and buffer 1 for multi-chunk lattices),
+// 128-byte aligned, and 64 spare bytes (the record prefetch and the run-time Horner loop read up to four
+// slots past the record they are in; the values are never used).
+template <int P, bool THICK, bool REG>
+__global__ void __maxnreg__((RegBudget<P, REG, THICK>::value)) xt_track_kernel(const TrackArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   const uint32_t bar0 = smem_addr(smem);
-  Cold<P> cold;
-  cold.row = reinterpret_cast<double *>(smem + 128) + static_cast<uint32_t>(Cold<P>::kPitch) * threadIdx.x;
+  using ColdT = Cold<P, REG>;
+  ColdT cold;
+  cold.attach(smem + 128);
   cold.stride = static_cast<int>(blockDim.x);
   unsigned char *const buf0 =
-      smem + 128 + ((static_cast<uint32_t>(8 * Cold<P>::kPitch) * blockDim.x + 127u) & ~127u);
+      smem + 128 + ((static_cast<uint32_t>(8 * ColdT::kPitch) * blockDim.x + 127u) & ~127u);
 
   // Balanced hand-out (device side, so that compaction's device counter needs no host
   // sync): use as few CTAs as hold n_active particles, rounded up to a whole number per SM,
@@ -835,7 +909,7 @@ __global__ void __maxnreg__(RegBudget<P>::value) xt_track_kernel(const TrackArgs
       const double opd = 1.0 + delta;
       const double b = XT_MADD(a.beta0, ptau, 1.0);
       const double t = XT_MUL(ptau, ptau + a.tib);
-      refresh_cached<P>(cold, j, opd, b, t, a.igam2);
+      refresh_cached(cold, j, opd, b, t, a.igam2);
     } else {
       q.x[j] = q.px[j] = q.y[j] = q.py[j] = q.zeta[j] = 0.0;
       cold.opd2(j) = cold.b(j) = 1.0;
@@ -852,60 +926,59 @@ __global__ void __maxnreg__(RegBudget<P>::value) xt_track_kernel(const TrackArgs
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
+  // A stage = stage_chunks consecutive chunks = one bulk copy into one buffer.  A lattice that fits one
+  // chunk is loaded once and stays resident in buffer 0: its warps run free, no CTA-level
+  // synchronisation; otherwise the stages alternate between the two buffers and a __syncthreads_or at
+  // the end of each releases the buffer and tells the CTA whether anyone is still alive.  One loop (and
+  // one copy of the record interpreter in the instruction cache) serves both.
+  const int32_t m = a.stage_chunks;
+  const int32_t n_stages = (a.n_chunks + m - 1) / m;
+  const uint32_t stage_bytes = static_cast<uint32_t>(m) * a.chunk_bytes;
+  auto load_stage = [&](int32_t sidx, uint32_t nb) {  // thread 0 only
+    const int32_t first = sidx * m;
+    const int32_t last = (first + m < a.n_chunks ? first + m : a.n_chunks) - 1;
+    const ChunkDesc d0 = a.chunks[first], d1 = a.chunks[last];
+    const uint32_t bytes = static_cast<uint32_t>(d1.offset + d1.nbytes - d0.offset);
+    tma_load_chunk(bar0 + 8 * nb, smem_addr(buf0 + static_cast<size_t>(nb) * stage_bytes), a.image + d0.offset,
+                   bytes);
+  };
+  if (threadIdx.x == 0) load_stage(0, 0);
+  if (single) mbar_wait(bar0, 0);
+  const int64_t total = a.n_turns * n_stages;
   int64_t turns_done = 0;
-  if (single) {
-    // Whole lattice resident in buffer 0: warps run free, no CTA-level synchronisation.
-    if (threadIdx.x == 0) {
-      const ChunkDesc d = a.chunks[0];
-      tma_load_chunk(bar0, smem_addr(buf0), a.image + d.offset, d.nbytes);
-    }
-    mbar_wait(bar0, 0);
-    for (; turns_done < a.n_turns; ++turns_done) {
-      if (!__any_sync(0xffffffffu, q.alive != 0)) break;
-      track_chunk<P, THICK>(q, buf0, cold, turns_done, a);
-    }
-  } else {
-    // A stage = stage_chunks consecutive chunks = one bulk copy into one buffer.
-    const int32_t m = a.stage_chunks;
-    const int32_t n_stages = (a.n_chunks + m - 1) / m;
-    const uint32_t stage_bytes = static_cast<uint32_t>(m) * a.chunk_bytes;
-    auto load_stage = [&](int32_t sidx, uint32_t nb) {  // thread 0 only
-      const int32_t first = sidx * m;
-      const int32_t last = (first + m < a.n_chunks ? first + m : a.n_chunks) - 1;
-      const ChunkDesc d0 = a.chunks[first], d1 = a.chunks[last];
-      const uint32_t bytes = static_cast<uint32_t>(d1.offset + d1.nbytes - d0.offset);
-      tma_load_chunk(bar0 + 8 * nb, smem_addr(buf0 + static_cast<size_t>(nb) * stage_bytes), a.image + d0.offset,
-                     bytes);
-    };
-    if (threadIdx.x == 0) load_stage(0, 0);
-    const int64_t total = a.n_turns * n_stages;
-    int64_t gidx = 0;  // global stage counter: buffer = gidx & 1, phase parity = (gidx >> 1) & 1
-    int32_t c = 0;
-    bool any = true;
-    while (gidx < total) {
+  int64_t gidx = 0;  // global stage counter: buffer = gidx & 1, phase parity = (gidx >> 1) & 1
+  int32_t c = 0;
+  bool any = true;
+  while (gidx < total) {
+    uint32_t cb = 0;
+    if (!single) {
       if (threadIdx.x == 0 && gidx + 1 < total) {
         // buffer (gidx+1)&1 was released by the __syncthreads_or that ended iteration gidx-1
         load_stage((c + 1 == n_stages) ? 0 : c + 1, static_cast<uint32_t>((gidx + 1) & 1));
       }
-      const uint32_t cb = static_cast<uint32_t>(gidx & 1);
+      cb = static_cast<uint32_t>(gidx & 1);
       mbar_wait(bar0 + 8 * cb, static_cast<uint32_t>((gidx >> 1) & 1));
-      if (__any_sync(0xffffffffu, q.alive != 0)) {
-        const int32_t n_sub = (c * m + m < a.n_chunks ? m : a.n_chunks - c * m);
-        const unsigned char *rp = buf0 + static_cast<size_t>(cb) * stage_bytes;
-        for (int32_t k = 0; k < n_sub; ++k) rp = track_chunk<P, THICK>(q, rp, cold, turns_done, a);
-      }
-      ++gidx;
-      if (++c == n_stages) {
-        c = 0;
-        ++turns_done;  // T: turn completed
-      }
+    }
+    const bool warp_alive = __any_sync(0xffffffffu, q.alive != 0);
+    if (single && !warp_alive) break;  // this warp is done; the others do not wait for it
+    if (warp_alive) {
+      const int32_t n_sub = (c * m + m < a.n_chunks ? m : a.n_chunks - c * m);
+      const unsigned char *rp = buf0 + static_cast<size_t>(cb) * stage_bytes;
+      for (int32_t k = 0; k < n_sub; ++k) rp = track_chunk<P, THICK>(q, rp, cold, turns_done, a);
+    }
+    ++gidx;
+    if (++c == n_stages) {
+      c = 0;
+      ++turns_done;  // T: turn completed
+    }
+    if (!single) {
       any = __syncthreads_or(q.alive != 0 ? 1 : 0) != 0;
       if (!any) break;
     }
-    if (!any && gidx < total) {
-      // every particle of the CTA is lost: drain the copy still in flight before exiting
-      mbar_wait(bar0 + 8 * static_cast<uint32_t>(gidx & 1), static_cast<uint32_t>((gidx >> 1) & 1));
-    }
+  }
+  if (!single && !any && gidx < total) {
+    // every particle of the CTA is lost: drain the copy still in flight before exiting
+    mbar_wait(bar0 + 8 * static_cast<uint32_t>(gidx & 1), static_cast<uint32_t>((gidx >> 1) & 1));
   }
 
   // W: survivors (lost particles were written when they were lost; rpp, rvv by the cavities)
@@ -940,14 +1013,35 @@ __global__ void xt_init_derived_kernel(xt_particles p, int64_t n, double beta0, 
   p.rvv[i] = opd / b;
 }
 
-template <int P, bool THICK>
-int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
-  const size_t cold_bytes = (static_cast<size_t>(8 * Cold<P>::kPitch) * block + 127) & ~static_cast<size_t>(127);
-  // per device, so set on every launch (a few microseconds against launches of milliseconds to seconds)
-  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P, THICK>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-  // the kernel has no use for L1 (every hot read is a shared-memory broadcast)
-  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P, THICK>, cudaFuncAttributePreferredSharedMemoryCarveout,
+// Per device and instantiation, once: opt in to large dynamic shared memory, prefer shared memory over
+// L1 (every hot read is a shared-memory broadcast) and read the register count the occupancy rule below
+// needs.  (Round 1 made these three driver calls on every launch; xt_track_knobs launches once per turn.)
+constexpr int kMaxDevices = 64;
+template <int P, bool THICK, bool REG>
+int kernel_registers(int device, int *regs) {
+  static std::atomic<int> cache[kMaxDevices];  // 0: not configured yet
+  const int slot = (device >= 0 && device < kMaxDevices) ? device : -1;
+  if (slot >= 0) {
+    const int v = cache[slot].load(std::memory_order_acquire);
+    if (v > 0) {
+      *regs = v;
+      return XT_OK;
+    }
+  }
+  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P, THICK, REG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P, THICK, REG>, cudaFuncAttributePreferredSharedMemoryCarveout,
                                cudaSharedmemCarveoutMaxShared));
+  cudaFuncAttributes fa;
+  XT_CUDA(cudaFuncGetAttributes(&fa, xt_track_kernel<P, THICK, REG>));
+  *regs = fa.numRegs > 0 ? fa.numRegs : 128;
+  if (slot >= 0) cache[slot].store(*regs, std::memory_order_release);
+  return XT_OK;
+}
+
+template <int P, bool THICK, bool REG>
+int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
+  const size_t cold_bytes =
+      (static_cast<size_t>(8 * Cold<P, REG>::kPitch) * block + 127) & ~static_cast<size_t>(127);
   const int64_t cap = static_cast<int64_t>(block) * P;
   const int64_t need = (a.n_part + cap - 1) / cap;
   const int64_t grid = ((need + a.grid_quantum - 1) / a.grid_quantum) * a.grid_quantum;
@@ -957,9 +1051,10 @@ int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaSt
   }
   // Staging depth: as many chunks per bulk copy (fewer CTA-wide barriers per turn) as shared memory
   // allows without taking a resident CTA away.
-  cudaFuncAttributes fa;
-  XT_CUDA(cudaFuncGetAttributes(&fa, xt_track_kernel<P, THICK>));
-  int64_t resident = 65536 / (static_cast<int64_t>(fa.numRegs > 0 ? fa.numRegs : 128) * block);
+  int regs = 128;
+  const int rc = kernel_registers<P, THICK, REG>(lat->device, &regs);
+  if (rc != XT_OK) return rc;
+  int64_t resident = 65536 / (static_cast<int64_t>(regs) * block);
   if (resident > grid / a.grid_quantum) resident = grid / a.grid_quantum;
   if (resident < 1) resident = 1;
   TrackArgs b = a;
@@ -974,33 +1069,32 @@ int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaSt
     }
   }
   const size_t smem = smem_for(b.stage_chunks);
-  xt_track_kernel<P, THICK><<<static_cast<unsigned>(grid), block, smem, st>>>(b);
+  xt_track_kernel<P, THICK, REG><<<static_cast<unsigned>(grid), block, smem, st>>>(b);
   count_launch();
   XT_CUDA(cudaGetLastError());
   return XT_OK;
 }
 
 // Lattices with thick elements take the instantiation that has their maps compiled in.
-template <int P>
+template <int P, bool REG>
 int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
-  return lat->extended ? launch_track_pt<P, true>(a, lat, block, st) : launch_track_pt<P, false>(a, lat, block, st);
+  return lat->extended ? launch_track_pt<P, true, REG>(a, lat, block, st)
+                       : launch_track_pt<P, false, REG>(a, lat, block, st);
 }
 
 }  // namespace
 
-int set_monitor_base(double *d_rows, cudaStream_t st) {
-  XT_CUDA(cudaMemcpyToSymbolAsync(g_monitor_rows, &d_rows, sizeof(double *), 0, cudaMemcpyHostToDevice, st));
-  return XT_OK;
-}
-
+// ppt: particles per thread (1, 2, 3, 4); cold_in_regs: the cold per-particle state in registers
+// instead of shared memory (instantiated for 2 and 3 particles per thread: the small-ensemble shapes).
 int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, const int64_t *d_n_active,
-                 int64_t n_turns, int block, int ppt, cudaStream_t st) {
+                 int64_t n_turns, int block, int ppt, bool cold_in_regs, cudaStream_t st) {
   if (n_part <= 0 || n_turns <= 0) return XT_OK;
   TrackArgs a;
   a.image = lat->d_image;
   a.chunks = lat->d_chunks;
   a.s_table = lat->d_s_table;
   a.n_active = d_n_active;
+  a.monitor_rows = lat->d_monitor_rows;
   a.p = p;
   a.n_part = n_part;
   a.n_turns = n_turns;
@@ -1010,15 +1104,21 @@ int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, c
   a.beta0 = lat->k.beta0;
   a.tib = lat->k.tib;
   a.igam2 = lat->k.igam2;
+  if (cold_in_regs) {
+    if (ppt == 2) return launch_track_p<2, true>(a, lat, block, st);
+    if (ppt == 3) return launch_track_p<3, true>(a, lat, block, st);
+    set_error("xt_track: cold_in_registers needs 2 or 3 particles per thread");
+    return XT_ERR_INVALID_ARG;
+  }
   switch (ppt) {
     case 1:
-      return launch_track_p<1>(a, lat, block, st);
+      return launch_track_p<1, false>(a, lat, block, st);
     case 2:
-      return launch_track_p<2>(a, lat, block, st);
+      return launch_track_p<2, false>(a, lat, block, st);
     case 3:
-      return launch_track_p<3>(a, lat, block, st);
+      return launch_track_p<3, false>(a, lat, block, st);
     case 4:
-      return launch_track_p<4>(a, lat, block, st);
+      return launch_track_p<4, false>(a, lat, block, st);
     default:
       set_error("xt_track: particles_per_thread must be 1, 2, 3 or 4");
       return XT_ERR_INVALID_ARG;

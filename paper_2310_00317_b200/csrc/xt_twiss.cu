@@ -414,7 +414,7 @@ extern "C" int xt_twiss4d_line(const xt_lattice *lat, double delta0, double ddel
   p.state = d_i64 + 16;
   p.at_element = d_i64 + 32;
   if ((rc = launch_init_derived(mon, p, kN, st)) != XT_OK) return done(rc);
-  if ((rc = set_monitor_base(d_rows, st)) != XT_OK) return done(rc);
+  mon->d_monitor_rows = d_rows;  // `mon` is private to this call
   if ((rc = xt_track(mon, &p, kN, 1, st)) != XT_OK) return done(rc);
   XT_TRYL(cudaMemcpyAsync(h_rows.data(), d_rows, h_rows.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
   XT_TRYL(cudaStreamSynchronize(st));

@@ -55,7 +55,7 @@ def test_library_loads_and_exports_every_declared_symbol(kind):
 def test_struct_layouts_match_the_header():
     # sizes the C compiler gives the public structs (LP64): 14 pointers; 2 x i64 + 2 x i32; ...
     assert ctypes.sizeof(B.xt_particles) == 14 * 8
-    assert ctypes.sizeof(B.xt_track_opts) == 48          # + workspace ptr, bytes, stats ptr
+    assert ctypes.sizeof(B.xt_track_opts) == 56          # + workspace ptr, bytes, stats ptr, cold_in_registers
     assert ctypes.sizeof(B.xt_track_stats) == 7 * 8 + 3 * 8 * B.XT_STATS_MAX_PASSES
     assert ctypes.sizeof(B.xt_lattice_opts) == 16
     assert ctypes.sizeof(B.xt_lattice_info) == 8 * (5 + 8 + 3) + 8 * 3 + 8 + 8
@@ -115,26 +115,29 @@ def maps_of(rec):
             out.append(("drift", s[0]))
         return out
     if typ in (T_MULT, T_CMULT):
-        coef = s[0:2 * (order + 1)]                      # coefficient pairs first, then the extras
-        k = 2 * (order + 1)
-        wf = l_pre = l_post = l_post2 = None
-        if typ == T_CMULT:
-            wf = s[k]
-            k += 2
-        if flags & (F_PRE | F_POST):
-            l_pre, l_post = s[k], s[k + 1]
-            k += 2
-        if flags & F_POST2:
-            l_post2 = s[k]
-            k += 2
+        # {l_pre, l_post} {l_post2, wf} [4 misalignment slots] then the coefficient pairs, highest order first
+        l_pre, l_post, l_post2, wf = s[0], s[1], s[2], s[3]
+        k = 4
+        if typ != T_CMULT:
+            assert wf == 0.0
+            wf = None
+        if not flags & F_PRE:
+            assert l_pre == 0.0
+        if not flags & F_POST:
+            assert l_post == 0.0
+        if not flags & F_POST2:
+            assert l_post2 == 0.0
         if flags & F_PRE:
             out.append(("drift", l_pre))
-        if flags & F_MISAL:
-            out += [("shift", s[k:k + 2]), ("srot", s[k + 2:k + 4])]
-        out.append(("mult", (order, p0 if typ == T_CMULT else 0.0, wf, coef)))
-        if flags & F_MISAL:
-            out += [("srot", s[k + 4:k + 6]), ("shift", s[k + 6:k + 8])]
+        mis = s[k:k + 8] if flags & F_MISAL else None
+        if mis:
+            out += [("shift", mis[0:2]), ("srot", mis[2:4])]
             k += 8
+        coef = s[k:k + 2 * (order + 1)]
+        k += 2 * (order + 1)
+        out.append(("mult", (order, p0 if typ == T_CMULT else 0.0, wf, coef)))
+        if mis:
+            out += [("srot", mis[4:6]), ("shift", mis[6:8])]
         if flags & F_POST:
             out.append(("drift", l_post))
         if flags & F_POST2:
@@ -296,9 +299,9 @@ def test_bad_buffers_and_options_are_rejected():
         with pytest.raises(X.XtError) as e:
             X.xt_lattice_pack_host(good, **kw)
         assert e.value.code == -1
-    big = pack([Multipole(knl=(0.0,) * 21, ksl=(0.0,) * 21)] * 3)              # 352-byte records
+    big = pack([Multipole(knl=(0.0,) * 21, ksl=(0.0,) * 21)] * 3)              # 384-byte records
     img, info = X.xt_lattice_pack_host(big, chunk_bytes=1024)
-    assert info["n_chunks"] == 2                                              # 16 + 2 x 352 fits, the third does not
+    assert info["n_chunks"] == 2                                              # 16 + 2 x 384 fits, the third does not
     assert X.xt_lattice_pack_host(good)[1]["n_records"] == 1
 
 
