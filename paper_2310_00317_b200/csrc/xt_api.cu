@@ -77,8 +77,8 @@ int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part,
     set_error("xt_track_ex: particles_per_thread must be 0 (auto), 1, 2, 3 or 4");
     return XT_ERR_INVALID_ARG;
   }
-  if (sh->cold_in_regs && sh->ppt != 2 && sh->ppt != 3) {
-    set_error("xt_track_ex: cold_in_registers needs 2 or 3 particles per thread");
+  if (sh->cold_in_regs && sh->ppt != 3) {
+    set_error("xt_track_ex: cold_in_registers needs 3 particles per thread");
     return XT_ERR_INVALID_ARG;
   }
   if (sh->block < 32 || sh->block > 256 || (sh->block % 32) != 0) {

@@ -413,6 +413,15 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
     fused.swap(merged);
   }
   info.n_records = static_cast<int64_t>(fused.size());
+  {  // which instantiation of the tracking kernel suits the lattice: is it full of order-15 multipoles?
+    int64_t n_mult = 0, n_15 = 0;
+    for (const Rec &rec : fused) {
+      if (rec.type != TAG_MULT && rec.type != TAG_CMULT) continue;
+      ++n_mult;
+      if (rec.order == 15) ++n_15;
+    }
+    out.fixed_order = (n_mult > 0 && 2 * n_15 >= n_mult) ? 15 : 0;
+  }
   for (const Rec &rec : fused) {
     if (rec.type == TAG_DRIFT) info.n_drift_evals += 1;
     if (rec.type == TAG_MULT || rec.type == TAG_CMULT)
@@ -522,6 +531,7 @@ int xt::create_lattice(const void *packed, size_t nbytes, const PackOpts &po, xt
   lat->extended = img.extended;
   lat->mult_slot0 = img.mult_slot0;
   lat->mult_wf_off = img.mult_wf_off;
+  lat->fixed_order = img.fixed_order;
   lat->packed_host.assign(static_cast<const unsigned char *>(packed), static_cast<const unsigned char *>(packed) + nbytes);
 
   auto fail = [&](cudaError_t e, const char *what) {

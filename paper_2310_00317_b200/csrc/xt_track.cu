@@ -117,10 +117,10 @@ __device__ __forceinline__ double rcp_seed(double a) {
 
 constexpr int kPrefetch = 4;  // 16-byte slots of a record loaded ahead of its dispatch ...
 #ifndef XT_PF4
-#define XT_PF4 2
+#define XT_PF4 4
 #endif
 #ifndef XT_PF3
-#define XT_PF3 2
+#define XT_PF3 4
 #endif
 template <int P, bool REG>
 struct Prefetched {  // ... of which this many really are (the rest is read where it is used)
@@ -709,13 +709,14 @@ __device__ __forceinline__ void monitor_store(const Parts<P> &q, ColdT &cold, do
 // Push the P particles of this thread through every record of one staged chunk.
 // Returns the position just behind the chunk (where the next chunk of the image starts).
 //
-// Dispatch: a switch on type | flags | order of the (warp-uniform) tag.  The records a thin
-// drift-kick-drift lattice is made of -- order-15 multipoles (straight and curved) with the flag sets
-// none, POST, POST+POST2, PRE+POST+POST2 -- have handlers in which flags, curvature and order are
-// compile-time constants: no flag branches, no remainder branches, a fully unrolled Horner whose
-// coefficient loads all sit at immediate offsets.  Every other multipole takes the same code with
-// flags and order read at run time.
-template <int P, bool THICK, class ColdT>
+// Dispatch: a switch on type | flags [| order] of the (warp-uniform) tag.  The records a thin
+// drift-kick-drift lattice is made of -- multipoles (straight and curved) with the flag sets none, POST,
+// POST+POST2, PRE+POST+POST2 -- have handlers in which flags and curvature are compile-time constants.
+// Lattices whose multipoles are mostly of one order (the packer counts: order 15 in configs[2-4]) run the
+// NFIX instantiation, where that order is a compile-time constant too: no remainder branches, a fully
+// unrolled Horner whose coefficient loads all sit at immediate offsets.  Every other multipole takes the
+// same code with flags and order read at run time.
+template <int P, bool THICK, int NFIX, class ColdT>
 __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const unsigned char *rp, ColdT &cold,
                                                             int64_t turns_done, const TrackArgs &a) {
   uint32_t tag = reinterpret_cast<const RecHdr *>(rp)->next;  // chunk preamble
@@ -731,18 +732,11 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
     const double p0 = h.p0;
     const uint32_t elem = h.elem;
     rp += tag >> 16;  // record size in bytes
-#ifndef XT_FIXED_ORDER
-#define XT_FIXED_ORDER 15  // the multipole order with fully unrolled handlers (0: none, order always read at run time)
-#endif
-#if XT_FIXED_ORDER > 0
-    constexpr uint32_t kKeyMask = 0x7fffu;  // type | flags | order << 8
-    constexpr uint32_t kOrd = static_cast<uint32_t>(XT_FIXED_ORDER);
-    constexpr int kOrdT = XT_FIXED_ORDER;
-#else
-    constexpr uint32_t kKeyMask = 0xffu;  // type | flags
-    constexpr uint32_t kOrd = 0u;
-    constexpr int kOrdT = -1;
-#endif
+    // NFIX > 0: the multipole order with fully unrolled handlers (the switch key then includes the order);
+    // NFIX = 0: the flag sets are specialised, the order is read at run time.
+    constexpr uint32_t kKeyMask = NFIX > 0 ? 0x7fffu : 0xffu;  // type | flags [| order << 8]
+    constexpr uint32_t kOrd = NFIX > 0 ? static_cast<uint32_t>(NFIX) : 0u;
+    constexpr int kOrdT = NFIX > 0 ? NFIX : -1;
     switch (tag & kKeyMask) {
       case TAG_DRIFT:
       case TAG_DRIFT | TAG_POST: {
@@ -814,7 +808,8 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
       }
       default: {
         const uint32_t type = tag & TAG_TYPE_MASK;
-        if (type == TAG_MULT || type == TAG_CMULT) {  // any other order / flag set (misaligned magnets): run time
+        if (type == TAG_MULT || type == TAG_CMULT) {
+          // any other order or flag set (misaligned magnets): everything read at run time
           multipole_record<P, -1, -1, -1>(q, cold, slots, pf, tag, p0);
         } else if (THICK) {  // the extended maps: only lattices that contain them run these instantiations
           const int order = static_cast<int>((tag >> 8) & 0x7fu);
@@ -862,7 +857,7 @@ struct RegBudget {
 // the cold state lives in registers); then staging buffer 0 (and buffer 1 for multi-chunk lattices),
 // 128-byte aligned, and 64 spare bytes (the record prefetch and the run-time Horner loop read up to four
 // slots past the record they are in; the values are never used).
-template <int P, bool THICK, bool REG>
+template <int P, bool THICK, bool REG, int NFIX>
 __global__ void __maxnreg__((RegBudget<P, REG, THICK>::value)) xt_track_kernel(const TrackArgs a) {
   extern __shared__ __align__(128) unsigned char smem[];
   const uint32_t bar0 = smem_addr(smem);
@@ -964,7 +959,7 @@ __global__ void __maxnreg__((RegBudget<P, REG, THICK>::value)) xt_track_kernel(c
     if (warp_alive) {
       const int32_t n_sub = (c * m + m < a.n_chunks ? m : a.n_chunks - c * m);
       const unsigned char *rp = buf0 + static_cast<size_t>(cb) * stage_bytes;
-      for (int32_t k = 0; k < n_sub; ++k) rp = track_chunk<P, THICK>(q, rp, cold, turns_done, a);
+      for (int32_t k = 0; k < n_sub; ++k) rp = track_chunk<P, THICK, NFIX>(q, rp, cold, turns_done, a);
     }
     ++gidx;
     if (++c == n_stages) {
@@ -1017,7 +1012,7 @@ __global__ void xt_init_derived_kernel(xt_particles p, int64_t n, double beta0, 
 // L1 (every hot read is a shared-memory broadcast) and read the register count the occupancy rule below
 // needs.  (Round 1 made these three driver calls on every launch; xt_track_knobs launches once per turn.)
 constexpr int kMaxDevices = 64;
-template <int P, bool THICK, bool REG>
+template <int P, bool THICK, bool REG, int NFIX>
 int kernel_registers(int device, int *regs) {
   static std::atomic<int> cache[kMaxDevices];  // 0: not configured yet
   const int slot = (device >= 0 && device < kMaxDevices) ? device : -1;
@@ -1028,17 +1023,17 @@ int kernel_registers(int device, int *regs) {
       return XT_OK;
     }
   }
-  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P, THICK, REG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P, THICK, REG>, cudaFuncAttributePreferredSharedMemoryCarveout,
+  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P, THICK, REG, NFIX>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+  XT_CUDA(cudaFuncSetAttribute(xt_track_kernel<P, THICK, REG, NFIX>, cudaFuncAttributePreferredSharedMemoryCarveout,
                                cudaSharedmemCarveoutMaxShared));
   cudaFuncAttributes fa;
-  XT_CUDA(cudaFuncGetAttributes(&fa, xt_track_kernel<P, THICK, REG>));
+  XT_CUDA(cudaFuncGetAttributes(&fa, xt_track_kernel<P, THICK, REG, NFIX>));
   *regs = fa.numRegs > 0 ? fa.numRegs : 128;
   if (slot >= 0) cache[slot].store(*regs, std::memory_order_release);
   return XT_OK;
 }
 
-template <int P, bool THICK, bool REG>
+template <int P, bool THICK, bool REG, int NFIX>
 int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
   const size_t cold_bytes =
       (static_cast<size_t>(8 * Cold<P, REG>::kPitch) * block + 127) & ~static_cast<size_t>(127);
@@ -1052,7 +1047,7 @@ int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaSt
   // Staging depth: as many chunks per bulk copy (fewer CTA-wide barriers per turn) as shared memory
   // allows without taking a resident CTA away.
   int regs = 128;
-  const int rc = kernel_registers<P, THICK, REG>(lat->device, &regs);
+  const int rc = kernel_registers<P, THICK, REG, NFIX>(lat->device, &regs);
   if (rc != XT_OK) return rc;
   int64_t resident = 65536 / (static_cast<int64_t>(regs) * block);
   if (resident > grid / a.grid_quantum) resident = grid / a.grid_quantum;
@@ -1069,23 +1064,31 @@ int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaSt
     }
   }
   const size_t smem = smem_for(b.stage_chunks);
-  xt_track_kernel<P, THICK, REG><<<static_cast<unsigned>(grid), block, smem, st>>>(b);
+  xt_track_kernel<P, THICK, REG, NFIX><<<static_cast<unsigned>(grid), block, smem, st>>>(b);
   count_launch();
   XT_CUDA(cudaGetLastError());
   return XT_OK;
 }
 
-// Lattices with thick elements take the instantiation that has their maps compiled in.
+// Lattices with thick elements take the instantiation that has their maps compiled in; lattices full of
+// order-15 multipoles the one with the unrolled order-15 handlers (3 and 4 particles per thread: the
+// shapes large lattices run with).
+constexpr int kFixedOrder = 15;
 template <int P, bool REG>
 int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
-  return lat->extended ? launch_track_pt<P, true, REG>(a, lat, block, st)
-                       : launch_track_pt<P, false, REG>(a, lat, block, st);
+  if (P >= 3 && lat->fixed_order == kFixedOrder) {
+    constexpr int NF = P >= 3 ? kFixedOrder : 0;
+    return lat->extended ? launch_track_pt<P, true, REG, NF>(a, lat, block, st)
+                         : launch_track_pt<P, false, REG, NF>(a, lat, block, st);
+  }
+  return lat->extended ? launch_track_pt<P, true, REG, 0>(a, lat, block, st)
+                       : launch_track_pt<P, false, REG, 0>(a, lat, block, st);
 }
 
 }  // namespace
 
 // ppt: particles per thread (1, 2, 3, 4); cold_in_regs: the cold per-particle state in registers
-// instead of shared memory (instantiated for 2 and 3 particles per thread: the small-ensemble shapes).
+// instead of shared memory (instantiated for 3 particles per thread: the small-ensemble shape).
 int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, const int64_t *d_n_active,
                  int64_t n_turns, int block, int ppt, bool cold_in_regs, cudaStream_t st) {
   if (n_part <= 0 || n_turns <= 0) return XT_OK;
@@ -1105,9 +1108,8 @@ int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, c
   a.tib = lat->k.tib;
   a.igam2 = lat->k.igam2;
   if (cold_in_regs) {
-    if (ppt == 2) return launch_track_p<2, true>(a, lat, block, st);
     if (ppt == 3) return launch_track_p<3, true>(a, lat, block, st);
-    set_error("xt_track: cold_in_registers needs 2 or 3 particles per thread");
+    set_error("xt_track: cold_in_registers needs 3 particles per thread");
     return XT_ERR_INVALID_ARG;
   }
   switch (ppt) {
