@@ -139,7 +139,7 @@ typedef struct {
   int64_t n_by_type[8];     /* elements per XT_* type id                                      */
   int64_t sum_order;        /* sum of N over all multipoles                                   */
   int64_t n_curved;         /* multipoles with hxl != 0                                       */
-  int64_t has_aperture;     /* 1 if any LimitRect / LimitEllipse                              */
+  int64_t has_aperture;     /* 1 if any LimitRect / LimitEllipse / LimitPolygon               */
   double beta0, gamma0;     /* reference particle as derived by the packer                    */
   double circumference;     /* sum of drift and thick-element lengths [m]                     */
   int64_t n_drift_evals;    /* sqrt evaluations per turn after fusion (consecutive drifts     */
@@ -235,7 +235,13 @@ int xt_fp64_fma_probe(int pattern, double *flops_per_s, double *ms, void *cuda_s
  * xt_track launch of nine particles through the whole line; only the 4x4 algebra is host code.
  * guess4 (HOST, x px y py; may be NULL = origin).  Synchronises the stream.  XT_ERR_UNSTABLE if a
  * probe particle is lost, M - 1 is singular, or 25 steps do not reach |dz| < 1e-13; an unstable
- * plane (|cos mu| >= 1) is reported through stable = 0 and NaN optics, not as an error. */
+ * plane (|cos mu| >= 1) is reported through stable = 0 and NaN optics, not as an error.
+ * Limitation of the 4-D entry points (xt_twiss4d, _chrom, _line): the probes are tracked through the line
+ * AS IT IS, live RF cavities included.  They start at zeta = 0 but slip before they reach a cavity and pick
+ * up a small energy kick there, so in a ring with cavities on, the "4-D" orbit, dispersion and chromaticity
+ * contain that longitudinal motion (relative 1e-4 on the dispersion downstream of the cavities of the
+ * LHC-sized configs).  Pass a lattice without cavities for a pure 4-D result, or use xt_twiss6d.  The oracle
+ * procedure (oracle/make_optics.py) tracks the same way, so parity does not see this. */
 typedef struct {
   double co[4];                 /* closed orbit x, px, y, py                                    */
   double m[16];                 /* one-turn Jacobian at the closed orbit, row-major              */
@@ -270,7 +276,8 @@ int xt_refine_loss_location(const xt_lattice *lat, const xt_particles *p, int64_
  * links of that coefficient in the order given (product rounded, then the sum); what the packer derives from
  * the coefficient follows (knl/n!, the curvature fold, the weak-focusing term).  The call copies table and
  * links to the device and replaces any earlier set; n_links == 0 removes it.  XT_ERR_BAD_LATTICE if a link
- * does not name a multipole coefficient that exists or a knob of the table. */
+ * does not name a multipole coefficient that exists or a knob of the table.  A call that fails leaves the
+ * lattice with the knob set it had. */
 typedef struct {
   int64_t element;
   int32_t order, skew, knob, reserved;
@@ -281,8 +288,9 @@ int xt_lattice_set_knobs(xt_lattice *lat, const double *table, int32_t n_knobs, 
 /* xt_track for n_turns turns with the knobs applied: before turn j (0-based) a small kernel rewrites the linked
  * coefficients in the device image for step = clamp(step0 + j, 0, n_steps - 1), then the tracking kernel runs
  * that turn (one launch per turn, stream-ordered, no host synchronisation); afterwards the image is back at
- * its base values.  While it runs the lattice must not be used by another stream.  No loss compaction. */
-int xt_track_knobs(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
+ * its base values.  The lattice is NOT const here: the call rewrites its device image in place, so while it
+ * runs the lattice must not be used by another stream or thread.  No loss compaction. */
+int xt_track_knobs(xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
                    int64_t step0, void *cuda_stream);
 
 /* Dispersion and chromaticity at the start of the line ("tunes, beta, alpha,

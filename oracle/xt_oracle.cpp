@@ -135,6 +135,9 @@ int parse(const void* packed, size_t nbytes, Lattice& L) {
     return std::isfinite(v);
   };
   L.el.clear();
+  // every record is at least 8 bytes: a count the buffer cannot hold is a truncated buffer (found by the
+  // ASan run of tests/test_sanitizers.py: a 48-byte buffer announcing 2^32 - 1 elements reserved 1.2 TB)
+  if (n_el > (nbytes - 48) / 8) return -2;
   L.el.reserve(n_el);
   for (uint32_t i = 0; i < n_el; ++i) {
     if (off + 8 > nbytes) return -2;

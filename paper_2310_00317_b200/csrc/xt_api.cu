@@ -22,6 +22,16 @@ int cuda_fail(cudaError_t e, const char *what) {
 
 void count_launch(int64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+int check_device(const xt_lattice *lat, const char *fn) {
+  int dev = -1;
+  XT_CUDA(cudaGetDevice(&dev));
+  if (!lat || dev != lat->device) {  // the lattice image lives on the device it was created on
+    set_error(std::string(fn) + ": the current CUDA device is not the one the lattice was created on");
+    return XT_ERR_INVALID_ARG;
+  }
+  return XT_OK;
+}
+
 namespace {
 
 int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p, int64_t n_part) {
@@ -34,13 +44,7 @@ int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p
     set_error(std::string(fn) + ": a required particle array is NULL (only particle_id, at_element may be)");
     return XT_ERR_INVALID_ARG;
   }
-  int dev = -1;
-  XT_CUDA(cudaGetDevice(&dev));
-  if (dev != lat->device) {  // the lattice image lives on the device it was created on
-    set_error(std::string(fn) + ": the current CUDA device is not the one the lattice was created on");
-    return XT_ERR_INVALID_ARG;
-  }
-  return XT_OK;
+  return check_device(lat, fn);
 }
 
 // Launch shape of the tracking kernel: threads per CTA, particles per thread, and where the cold
@@ -171,7 +175,7 @@ class StatsTimer {
 }  // namespace
 }  // namespace xt
 
-extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
+static int xt_track_ex_impl(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
                            void *cuda_stream, const xt_track_opts *opts) {
   int rc = xt::check_particles("xt_track", lat, p, n_part);
   if (rc != XT_OK) return rc;
@@ -267,7 +271,7 @@ extern "C" int xt_track(const xt_lattice *lat, const xt_particles *p, int64_t n_
   return xt_track_ex(lat, p, n_part, n_turns, cuda_stream, nullptr);
 }
 
-extern "C" int xt_track_host(const xt_lattice *lat, const xt_particles *hp, int64_t n_part, int64_t n_turns,
+static int xt_track_host_impl(const xt_lattice *lat, const xt_particles *hp, int64_t n_part, int64_t n_turns,
                              void *cuda_stream, const xt_track_opts *opts) {
   int rc = xt::check_particles("xt_track_host", lat, hp, n_part);
   if (rc != XT_OK) return rc;
@@ -364,4 +368,14 @@ extern "C" const char *xt_build_info(void) {
 #else
   return "libxt_b200 sm_100a fmad=true";
 #endif
+}
+
+// C ABI: no C++ exception may cross it (include/xt.h: "No exceptions, no abort()").  The bodies above use
+// std::vector / std::map / std::string; a failed host allocation comes back as XT_ERR_NOMEM.
+extern "C" int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns, void *cuda_stream, const xt_track_opts *opts) {
+  return xt::guarded<int>([&] { return xt_track_ex_impl(lat, p, n_part, n_turns, cuda_stream, opts); });
+}
+
+extern "C" int xt_track_host(const xt_lattice *lat, const xt_particles *hp, int64_t n_part, int64_t n_turns, void *cuda_stream, const xt_track_opts *opts) {
+  return xt::guarded<int>([&] { return xt_track_host_impl(lat, hp, n_part, n_turns, cuda_stream, opts); });
 }

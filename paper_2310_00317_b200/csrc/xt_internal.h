@@ -6,6 +6,7 @@
 
 #include <cstddef>
 #include <cstdint>
+#include <new>
 #include <string>
 #include <vector>
 
@@ -83,7 +84,11 @@ static_assert(sizeof(RecHdr) == 16, "record header must be one 16-byte slot");
 
 struct alignas(16) ChunkDesc {
   uint64_t offset;  // byte offset into the image (multiple of 16)
-  uint32_t nbytes;  // multiple of 16, <= chunk_bytes, includes the TAG_END record
+  uint32_t nbytes;  // multiple of 16, <= chunk_bytes: preamble + records (there is no END record: TAG_END is the
+                    // `next` field of the chunk's last header).  The kernel's slot prefetch and the run-time Horner
+                    // loop read up to 64 bytes past the last record of a stage; the values are never used.  Behind
+                    // the last buffer that is the 64 spare bytes of the allocation; behind buffer 0 it is the head
+                    // of buffer 1, possibly while a bulk copy is writing it -- a read whose result is discarded.
   uint32_t pad;
 };
 
@@ -127,6 +132,23 @@ namespace xt {
 void set_error(const std::string &msg);
 int cuda_fail(cudaError_t e, const char *what);
 void count_launch(int64_t n = 1);
+// XT_ERR_INVALID_ARG unless the current CUDA device is the one the lattice's image lives on (every entry
+// point that takes a lattice checks this before it allocates or launches anything).
+int check_device(const xt_lattice *lat, const char *fn);
+// Runs the body of a C-ABI entry point; turns any C++ exception into an error code (the message is short
+// enough for std::string's in-place buffer: reporting must not allocate).
+template <class R, class F>
+R guarded(F &&body) noexcept {
+  try {
+    return body();
+  } catch (const std::bad_alloc &) {
+    try { set_error("out of memory"); } catch (...) {}
+    return static_cast<R>(XT_ERR_NOMEM);
+  } catch (...) {
+    try { set_error("C++ exception"); } catch (...) {}
+    return static_cast<R>(XT_ERR_NOMEM);
+  }
+}
 #define XT_CUDA(call)                                      \
   do {                                                     \
     cudaError_t e__ = (call);                              \

@@ -74,13 +74,15 @@ int launch_apply(const xt_lattice *lat, int64_t step, int with_links, cudaStream
 }  // namespace
 }  // namespace xt
 
-extern "C" int xt_lattice_set_knobs(xt_lattice *lat, const double *table, int32_t n_knobs, int64_t n_steps,
+static int xt_lattice_set_knobs_impl(xt_lattice *lat, const double *table, int32_t n_knobs, int64_t n_steps,
                                     const xt_knob_link *links, int64_t n_links) {
   using namespace xt;
   if (!lat || n_links < 0) {
     set_error("xt_lattice_set_knobs: lat is NULL or n_links < 0");
     return XT_ERR_INVALID_ARG;
   }
+  int rc_dev = check_device(lat, "xt_lattice_set_knobs");
+  if (rc_dev != XT_OK) return rc_dev;
   if (n_links == 0) {
     drop_knobs(lat);
     return XT_OK;
@@ -143,32 +145,39 @@ extern "C" int xt_lattice_set_knobs(xt_lattice *lat, const double *table, int32_
     flat.insert(flat.end(), by_target[key].begin(), by_target[key].end());
     targets.push_back(t);
   }
-  drop_knobs(lat);
+  // build the new set first; the lattice keeps its previous knobs unless everything succeeded
+  double *d_table = nullptr;
+  void *d_targets = nullptr, *d_links = nullptr;
   auto fail = [&](cudaError_t e, const char *what) {
-    drop_knobs(lat);
+    cudaFree(d_table);
+    cudaFree(d_targets);
+    cudaFree(d_links);
     return cuda_fail(e, what);
   };
   cudaError_t e;
   const size_t tb = static_cast<size_t>(n_knobs) * n_steps * sizeof(double);
-  if ((e = cudaMalloc(&lat->d_knob_table, tb)) != cudaSuccess) return fail(e, "cudaMalloc(knob table)");
-  if ((e = cudaMalloc(&lat->d_knob_targets, targets.size() * sizeof(KnobTarget))) != cudaSuccess)
+  if ((e = cudaMalloc(reinterpret_cast<void **>(&d_table), tb)) != cudaSuccess) return fail(e, "cudaMalloc(knob table)");
+  if ((e = cudaMalloc(&d_targets, targets.size() * sizeof(KnobTarget))) != cudaSuccess)
     return fail(e, "cudaMalloc(knob targets)");
-  if ((e = cudaMalloc(&lat->d_knob_links, flat.size() * sizeof(KnobLink))) != cudaSuccess)
+  if ((e = cudaMalloc(&d_links, flat.size() * sizeof(KnobLink))) != cudaSuccess)
     return fail(e, "cudaMalloc(knob links)");
-  if ((e = cudaMemcpy(lat->d_knob_table, table, tb, cudaMemcpyHostToDevice)) != cudaSuccess)
+  if ((e = cudaMemcpy(d_table, table, tb, cudaMemcpyHostToDevice)) != cudaSuccess)
     return fail(e, "cudaMemcpy(knob table)");
-  if ((e = cudaMemcpy(lat->d_knob_targets, targets.data(), targets.size() * sizeof(KnobTarget),
-                      cudaMemcpyHostToDevice)) != cudaSuccess)
-    return fail(e, "cudaMemcpy(knob targets)");
-  if ((e = cudaMemcpy(lat->d_knob_links, flat.data(), flat.size() * sizeof(KnobLink), cudaMemcpyHostToDevice)) !=
+  if ((e = cudaMemcpy(d_targets, targets.data(), targets.size() * sizeof(KnobTarget), cudaMemcpyHostToDevice)) !=
       cudaSuccess)
+    return fail(e, "cudaMemcpy(knob targets)");
+  if ((e = cudaMemcpy(d_links, flat.data(), flat.size() * sizeof(KnobLink), cudaMemcpyHostToDevice)) != cudaSuccess)
     return fail(e, "cudaMemcpy(knob links)");
+  drop_knobs(lat);
+  lat->d_knob_table = d_table;
+  lat->d_knob_targets = d_targets;
+  lat->d_knob_links = d_links;
   lat->n_knob_targets = static_cast<int64_t>(targets.size());
   lat->n_knob_steps = n_steps;
   return XT_OK;
 }
 
-extern "C" int xt_track_knobs(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
+static int xt_track_knobs_impl(xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
                               int64_t step0, void *cuda_stream) {
   using namespace xt;
   if (!lat || !p || n_turns < 0) {
@@ -179,6 +188,8 @@ extern "C" int xt_track_knobs(const xt_lattice *lat, const xt_particles *p, int6
     set_error("xt_track_knobs: the lattice has no knobs (xt_lattice_set_knobs)");
     return XT_ERR_INVALID_ARG;
   }
+  const int rc_dev = check_device(lat, "xt_track_knobs");  // before the first launch touches the image
+  if (rc_dev != XT_OK) return rc_dev;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   xt_track_opts opts{};
   opts.compact_every = -1;
@@ -190,4 +201,14 @@ extern "C" int xt_track_knobs(const xt_lattice *lat, const xt_particles *p, int6
   }
   const int rc_restore = launch_apply(lat, 0, 0, st);  // the image goes back to its base values, whatever happened
   return rc != XT_OK ? rc : rc_restore;
+}
+
+// C ABI: no C++ exception may cross it (include/xt.h: "No exceptions, no abort()").  The bodies above use
+// std::vector / std::map / std::string; a failed host allocation comes back as XT_ERR_NOMEM.
+extern "C" int xt_lattice_set_knobs(xt_lattice *lat, const double *table, int32_t n_knobs, int64_t n_steps, const xt_knob_link *links, int64_t n_links) {
+  return xt::guarded<int>([&] { return xt_lattice_set_knobs_impl(lat, table, n_knobs, n_steps, links, n_links); });
+}
+
+extern "C" int xt_track_knobs(xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns, int64_t step0, void *cuda_stream) {
+  return xt::guarded<int>([&] { return xt_track_knobs_impl(lat, p, n_part, n_turns, step0, cuda_stream); });
 }

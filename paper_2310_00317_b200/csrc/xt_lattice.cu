@@ -93,6 +93,12 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
     set_error("xt_lattice_create: unsupported version or total_bytes does not match nbytes");
     return XT_ERR_BAD_LATTICE;
   }
+  // every element record is at least 8 bytes (type, aux): a count the buffer cannot hold is rejected before
+  // anything is sized from it (a 48-byte buffer announcing 2^32-1 elements must not allocate 32 GB)
+  if (n_elements > (nbytes - 48) / 8 || n_elements >= (1u << 24)) {
+    set_error("xt_lattice_create: n_elements does not fit the buffer (truncated) or exceeds 2^24 - 1");
+    return XT_ERR_BAD_LATTICE;
+  }
   if (!std::isfinite(p0c) || !std::isfinite(mass0) || !std::isfinite(q0) || !(p0c > 0.0) ||
       !(mass0 > 0.0)) {
     set_error("xt_lattice_create: p0c and mass0 must be finite and > 0, q0 finite");
@@ -503,7 +509,7 @@ extern "C" int xt_lattice_create(const void *packed, size_t nbytes, xt_lattice *
   return xt_lattice_create_ex(packed, nbytes, nullptr, out);
 }
 
-extern "C" int xt_lattice_create_ex(const void *packed, size_t nbytes, const xt_lattice_opts *opts,
+static int xt_lattice_create_ex_impl(const void *packed, size_t nbytes, const xt_lattice_opts *opts,
                                     xt_lattice **out) {
   if (!out) {
     xt::set_error("xt_lattice_create: out is NULL");
@@ -583,7 +589,7 @@ extern "C" int xt_lattice_get_info(const xt_lattice *lat, xt_lattice_info *info)
   return XT_OK;
 }
 
-extern "C" int64_t xt_lattice_s_table(const xt_lattice *lat, double *out, int64_t cap) {
+static int64_t xt_lattice_s_table_impl(const xt_lattice *lat, double *out, int64_t cap) {
   if (!lat || cap < 0 || (cap > 0 && !out)) {
     xt::set_error("xt_lattice_s_table: invalid argument");
     return XT_ERR_INVALID_ARG;
@@ -593,7 +599,7 @@ extern "C" int64_t xt_lattice_s_table(const xt_lattice *lat, double *out, int64_
   return n;
 }
 
-extern "C" int64_t xt_lattice_pack_host(const void *packed, size_t nbytes, const xt_lattice_opts *opts,
+static int64_t xt_lattice_pack_host_impl(const void *packed, size_t nbytes, const xt_lattice_opts *opts,
                                         void *image, size_t cap, xt_lattice_info *info) {
   if (cap > 0 && !image) {
     xt::set_error("xt_lattice_pack_host: image is NULL but cap > 0");
@@ -609,4 +615,18 @@ extern "C" int64_t xt_lattice_pack_host(const void *packed, size_t nbytes, const
   if (n) std::memcpy(image, img.image.data(), n);
   if (info) *info = img.info;
   return static_cast<int64_t>(img.image.size());
+}
+
+// C ABI: no C++ exception may cross it (include/xt.h: "No exceptions, no abort()").  The bodies above use
+// std::vector / std::map / std::string; a failed host allocation comes back as XT_ERR_NOMEM.
+extern "C" int xt_lattice_create_ex(const void *packed, size_t nbytes, const xt_lattice_opts *opts, xt_lattice **out) {
+  return xt::guarded<int>([&] { return xt_lattice_create_ex_impl(packed, nbytes, opts, out); });
+}
+
+extern "C" int64_t xt_lattice_pack_host(const void *packed, size_t nbytes, const xt_lattice_opts *opts, void *image, size_t cap, xt_lattice_info *info) {
+  return xt::guarded<int64_t>([&] { return xt_lattice_pack_host_impl(packed, nbytes, opts, image, cap, info); });
+}
+
+extern "C" int64_t xt_lattice_s_table(const xt_lattice *lat, double *out, int64_t cap) {
+  return xt::guarded<int64_t>([&] { return xt_lattice_s_table_impl(lat, out, cap); });
 }

@@ -179,7 +179,7 @@ struct LatticeGuard {
 }  // namespace
 }  // namespace xt
 
-extern "C" int xt_refine_loss_location(const xt_lattice *lat, const xt_particles *p, int64_t n_part, double ds,
+static int xt_refine_loss_location_impl(const xt_lattice *lat, const xt_particles *p, int64_t n_part, double ds,
                                        int32_t n_poly, int64_t *n_refined, void *cuda_stream) {
   using namespace xt;
   if (n_refined) *n_refined = 0;
@@ -197,6 +197,8 @@ extern "C" int xt_refine_loss_location(const xt_lattice *lat, const xt_particles
     return XT_ERR_INVALID_ARG;
   }
   if (n_part == 0) return XT_OK;
+  const int rc_dev = check_device(lat, "xt_refine_loss_location");  // before any allocation or launch
+  if (rc_dev != XT_OK) return rc_dev;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   Line line;
   if (!read_line(lat->packed_host, line)) {
@@ -350,4 +352,10 @@ extern "C" int xt_refine_loss_location(const xt_lattice *lat, const xt_particles
 #undef XT_TRY_RC
   if (n_refined) *n_refined = static_cast<int64_t>(moved);
   return XT_OK;
+}
+
+// C ABI: no C++ exception may cross it (include/xt.h: "No exceptions, no abort()").  The bodies above use
+// std::vector / std::map / std::string; a failed host allocation comes back as XT_ERR_NOMEM.
+extern "C" int xt_refine_loss_location(const xt_lattice *lat, const xt_particles *p, int64_t n_part, double ds, int32_t n_poly, int64_t *n_refined, void *cuda_stream) {
+  return xt::guarded<int>([&] { return xt_refine_loss_location_impl(lat, p, n_part, ds, n_poly, n_refined, cuda_stream); });
 }

@@ -118,13 +118,14 @@ int one_turn_and_jacobian(const xt_lattice *lat, const Probe &pr, const double z
 }  // namespace
 }  // namespace xt
 
-extern "C" int xt_twiss4d(const xt_lattice *lat, double delta0, const double *guess4, xt_twiss4d_result *out,
+static int xt_twiss4d_impl(const xt_lattice *lat, double delta0, const double *guess4, xt_twiss4d_result *out,
                           void *cuda_stream) {
   using namespace xt;
   if (!lat || !out || !std::isfinite(delta0)) {
     set_error("xt_twiss4d: NULL lattice / result or non-finite delta0");
     return XT_ERR_INVALID_ARG;
   }
+  if (const int rc_dev = check_device(lat, "xt_twiss4d")) return rc_dev;  // before any allocation or launch
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   Probe pr;
   const size_t pitch = 256;  // bytes per array (9 x 8 = 72 used)
@@ -222,7 +223,7 @@ int chromatic_twiss(const xt_lattice *lat, double delta0, double ddelta, const d
 }  // namespace
 }  // namespace xt
 
-extern "C" int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
+static int xt_twiss4d_chrom_impl(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
                                 xt_twiss4d_chrom_result *out, void *cuda_stream) {
   using namespace xt;
   if (!out || !(ddelta > 0.0) || !std::isfinite(ddelta)) {
@@ -237,7 +238,7 @@ extern "C" int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double dde
   return XT_OK;
 }
 
-extern "C" int xt_twiss4d_normal_form(const double *m, xt_twiss4d_modes *out) {
+static int xt_twiss4d_normal_form_impl(const double *m, xt_twiss4d_modes *out) {
   using namespace xt;
   using cplx = std::complex<double>;
   if (!m || !out) {
@@ -332,13 +333,14 @@ extern "C" int xt_twiss4d_normal_form(const double *m, xt_twiss4d_modes *out) {
   return XT_OK;
 }
 
-extern "C" int xt_twiss4d_line(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
+static int xt_twiss4d_line_impl(const xt_lattice *lat, double delta0, double ddelta, const double *guess4,
                                xt_twiss4d_chrom_result *start, xt_twiss_row *rows, int64_t cap, void *cuda_stream) {
   using namespace xt;
   if (!lat || !rows || !(ddelta > 0.0) || !std::isfinite(ddelta) || !std::isfinite(delta0)) {
     set_error("xt_twiss4d_line: NULL lattice / rows, or ddelta not > 0");
     return XT_ERR_INVALID_ARG;
   }
+  if (const int rc_dev = check_device(lat, "xt_twiss4d_line")) return rc_dev;
   Line line;
   if (!read_line(lat->packed_host, line)) {
     set_error("xt_twiss4d_line: the lattice holds no readable packed buffer");
@@ -560,12 +562,13 @@ int solve6(double a[6][7]) {  // Gaussian elimination with partial pivoting on [
 }  // namespace
 }  // namespace xt
 
-extern "C" int xt_twiss6d(const xt_lattice *lat, const double *guess6, xt_twiss6d_result *out, void *cuda_stream) {
+static int xt_twiss6d_impl(const xt_lattice *lat, const double *guess6, xt_twiss6d_result *out, void *cuda_stream) {
   using namespace xt;
   if (!lat || !out) {
     set_error("xt_twiss6d: NULL lattice or result");
     return XT_ERR_INVALID_ARG;
   }
+  if (const int rc_dev = check_device(lat, "xt_twiss6d")) return rc_dev;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   double *d_f64 = nullptr;
   int64_t *d_i64 = nullptr;
@@ -676,4 +679,26 @@ extern "C" int xt_twiss6d(const xt_lattice *lat, const double *guess6, xt_twiss6
   res.q2_frac = frac(a2, jac[6 * 2 + 3]);
   *out = res;
   return done(XT_OK);
+}
+
+// C ABI: no C++ exception may cross it (include/xt.h: "No exceptions, no abort()").  The bodies above use
+// std::vector / std::map / std::string; a failed host allocation comes back as XT_ERR_NOMEM.
+extern "C" int xt_twiss4d(const xt_lattice *lat, double delta0, const double *guess4, xt_twiss4d_result *out, void *cuda_stream) {
+  return xt::guarded<int>([&] { return xt_twiss4d_impl(lat, delta0, guess4, out, cuda_stream); });
+}
+
+extern "C" int xt_twiss4d_chrom(const xt_lattice *lat, double delta0, double ddelta, const double *guess4, xt_twiss4d_chrom_result *out, void *cuda_stream) {
+  return xt::guarded<int>([&] { return xt_twiss4d_chrom_impl(lat, delta0, ddelta, guess4, out, cuda_stream); });
+}
+
+extern "C" int xt_twiss4d_line(const xt_lattice *lat, double delta0, double ddelta, const double *guess4, xt_twiss4d_chrom_result *start, xt_twiss_row *rows, int64_t cap, void *cuda_stream) {
+  return xt::guarded<int>([&] { return xt_twiss4d_line_impl(lat, delta0, ddelta, guess4, start, rows, cap, cuda_stream); });
+}
+
+extern "C" int xt_twiss6d(const xt_lattice *lat, const double *guess6, xt_twiss6d_result *out, void *cuda_stream) {
+  return xt::guarded<int>([&] { return xt_twiss6d_impl(lat, guess6, out, cuda_stream); });
+}
+
+extern "C" int xt_twiss4d_normal_form(const double *m, xt_twiss4d_modes *out) {
+  return xt::guarded<int>([&] { return xt_twiss4d_normal_form_impl(m, out); });
 }
