@@ -56,7 +56,10 @@ BENCH_TURNS = {4: 3000}        # configs[4] is 1e5 turns (hours): the bench line
 # Algorithmic FP64 flops per element visit (minimal arithmetic of the
 # canonical forms; FMA = 2, add/mul/sqrt/div = 1, compares = 0, sin = 1) ...
 FLOPS_MIN = dict(drift=17, mult_base=2, mult_per_order=8, curved_extra=7, cavity=19, srot=12,
-                 shift=2, rect=0, ellipse=5)
+                 shift=2, rect=0, ellipse=5,
+                 # thick maps, every operation of the canonical form counted once,
+                 # sincos = 2, cosh = sinh = sqrt = division = 1, FMA = 2
+                 thick_quad=66, thick_bend=68)
 # ... and FP64 flops as executed by the sm_100a kernel (counted in the SASS of
 # libxt_b200.so, profiles/r01_sass_fp64_counts.md): a drift is one evaluation of 1/pz and
 # 1/(pz + b) (13 FP64 instructions, 21 flops; consecutive drifts share it after fusion) plus
@@ -72,9 +75,10 @@ def flops_per_particle_turn(info: dict, table: dict) -> float:
         drifts = t[1] * table["drift"]
     else:
         drifts = t[1] * table["drift_apply"] + info["n_drift_evals"] * table["drift_eval"]
+    thick = info.get("n_thick_quad", 0) * table.get("thick_quad", 0) + info.get("n_thick_bend", 0) * table.get("thick_bend", 0)
     return (drifts + n_mult * table["mult_base"] + info["sum_order"] * table["mult_per_order"]
             + info["n_curved"] * table["curved_extra"] + t[3] * table["cavity"] + t[4] * table["srot"]
-            + t[5] * table["shift"] + t[6] * table["rect"] + t[7] * table["ellipse"])
+            + t[5] * table["shift"] + t[6] * table["rect"] + t[7] * table["ellipse"] + thick)
 
 
 class ClockSampler:
@@ -128,12 +132,15 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+THICK_COUNTS = {}     # thick elements of the lattice make_inputs built last (xt_lattice_info counts them together)
+
+
 def make_inputs(cfg: int, rank: int, workload: str = ""):
     """Seeded synthetic lattice + ensemble of config ``cfg``."""
-    els = C.lattice(cfg)
-    if workload == "thick":
-        els = C.thicken(els)
+    els = C.lattice_cfg2_thick() if workload == "thick" else C.lattice(cfg)
     buf = C.pack(els)
+    THICK_COUNTS.update(n_thick_quad=sum(type(e).__name__ == "Quadrupole" for e in els),
+                        n_thick_bend=sum(type(e).__name__ == "Bend" for e in els))
     if cfg in (0, 2, 3) and rank:
         coords = {0: C.particles_cfg0, 2: C.particles_cfg2, 3: C.particles_cfg3}[cfg](seed=1000 + cfg + 100 * rank)
     else:
@@ -329,7 +336,7 @@ def main():
     if args.particles:
         coords = C.subsample(coords, slice(0, args.particles))
     lat = X.xt_lattice_create_ex(buf, chunk_bytes=args.chunk) if args.chunk else X.xt_lattice_create(buf)
-    info = lat.info
+    info = dict(lat.info, **THICK_COUNTS)
     n_el = info["n_elements"]
     n_part = len(coords["x"])
     stream = torch.cuda.current_stream()
@@ -458,6 +465,7 @@ def main():
         if cfg == 3 and world == 1:
             b2, c2 = make_inputs(2, 0)
             l2 = X.xt_lattice_create(b2)
+            assert not THICK_COUNTS["n_thick_quad"]
             t2 = C.n_turns(2)
             n2 = len(c2["x"])
             r2 = time_workload(X, torch, l2, c2, t2, max(5, args.also_steps), 3, args, barrier)

@@ -2,10 +2,11 @@
 //
 // Aperture elements "stop the tracking for the particles found to be outside"
 // (PAPER.md:178).  A stopped particle is frozen, so it can be retired: every compact_every
-// turns the alive particles are packed to the front of a working SoA (stable partition:
-// warp ballot + popc, block scan, tile offsets) so that the tracking kernel's warps stay
-// full; each retired particle is written straight to its final place in the caller's
-// arrays through its origin index.  HBM-bound, 2 x n x 112 B per pass.
+// turns the alive particles are packed to the front of a working SoA (stable partition in ONE
+// kernel: warp ballot + popc, block scan, single-pass look-back scan over the tiles) so that the
+// tracking kernel's warps stay full; each retired particle is written straight to its final place
+// in the caller's arrays through its origin index.  HBM-bound, 2 x n x 112 B per pass; measured
+// 4.0-4.4 TB/s on 2e6 particles (profiles/r02_compaction_summary.md).
 #include "xt_internal.h"
 
 namespace xt {
@@ -30,82 +31,127 @@ __device__ __forceinline__ void copy_particle(const xt_particles &dst, int64_t j
   if (dst.at_element) dst.at_element[j] = src.at_element ? src.at_element[i] : 0;
 }
 
-// Pass 1: alive count per tile.
-__global__ void __launch_bounds__(kTile) count_alive_kernel(const int64_t *__restrict__ state,
-                                                            const int64_t *n_src_ptr, int64_t n_src_val,
-                                                            int64_t *tile_counts) {
-  const int64_t n_src = n_src_ptr ? *n_src_ptr : n_src_val;
-  const int64_t i = static_cast<int64_t>(blockIdx.x) * kTile + threadIdx.x;
-  const int alive = (i < n_src) && (state[i] == 1);
-  const int cnt = __syncthreads_count(alive);
-  if (threadIdx.x == 0) tile_counts[blockIdx.x] = cnt;
+// One pass, one kernel: stable partition with a single-pass ("decoupled look-back") scan over the tiles.
+// Every CTA takes a ticket (tiles are then processed in ticket order whatever order the hardware starts
+// CTAs in), counts its alive particles (ballot + popc), publishes the count, looks back over the tiles
+// before it until it meets one whose inclusive prefix is known, publishes its own inclusive prefix and
+// moves its particles: alive ones to dst[prefix + rank] (carrying their origin index), lost ones of a
+// working set straight to their final place user[origin].  The last tile writes the new alive count.
+// Status word of a tile: [epoch : 30][flag : 2][value : 32]; flag 1 = the tile's own count, 2 = inclusive
+// prefix; the epoch (one per pass) makes words of earlier passes read as "not ready", so the array is
+// cleared once per xt_track_ex call, not once per pass.  Reads 8 B (state) + 112 B per particle once,
+// writes 112 B per particle once: the 2 x n x 112 B of SURVEY.md 8(a) row C plus the state read it
+// repeats (the count must be known before the move).
+constexpr uint64_t kFlagAggregate = 1, kFlagPrefix = 2;
+__device__ __forceinline__ uint64_t pack_status(uint32_t epoch, uint64_t flag, uint32_t value) {
+  return (static_cast<uint64_t>(epoch) << 34) | (flag << 32) | value;
 }
 
-// Pass 2: exclusive scan of the tile counts in place (one CTA), total -> *n_dst.
-__global__ void __launch_bounds__(1024) scan_tiles_kernel(int64_t *tile_counts, int64_t n_tiles, int64_t *n_dst) {
-  __shared__ int64_t warp_sums[32];
-  __shared__ int64_t carry;
-  if (threadIdx.x == 0) carry = 0;
-  __syncthreads();
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  for (int64_t start = 0; start < n_tiles; start += 1024) {
-    const int64_t i = start + threadIdx.x;
-    const int64_t v = (i < n_tiles) ? tile_counts[i] : 0;
-    int64_t incl = v;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const int64_t t = __shfl_up_sync(0xffffffffu, incl, d);
-      if (lane >= d) incl += t;
-    }
-    if (lane == 31) warp_sums[warp] = incl;
-    __syncthreads();
-    if (warp == 0) {
-      int64_t w = warp_sums[lane];
-#pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {
-        const int64_t t = __shfl_up_sync(0xffffffffu, w, d);
-        if (lane >= d) w += t;
-      }
-      warp_sums[lane] = w;  // inclusive over warps
-    }
-    __syncthreads();
-    const int64_t before = carry + (warp ? warp_sums[warp - 1] : 0);
-    if (i < n_tiles) tile_counts[i] = before + incl - v;
-    __syncthreads();
-    if (threadIdx.x == 0) carry += warp_sums[31];
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) *n_dst = carry;
-}
-
-// Pass 3: move.  Alive entries go to dst[tile_offset + rank]; lost entries of a working set
-// retire to user[origin].
-__global__ void __launch_bounds__(kTile) partition_move_kernel(xt_particles src, const int64_t *src_origin,
-                                                               const int64_t *n_src_ptr, int64_t n_src_val,
-                                                               const int64_t *tile_offsets, xt_particles dst,
-                                                               int64_t *dst_origin, xt_particles user,
-                                                               int retire_lost) {
+__global__ void __launch_bounds__(kTile) partition_fused_kernel(xt_particles src, const int64_t *src_origin,
+                                                                const int64_t *n_src_ptr, int64_t n_src_val,
+                                                                xt_particles dst, int64_t *dst_origin,
+                                                                xt_particles user, int retire_lost,
+                                                                unsigned long long *status, unsigned int *ticket,
+                                                                uint32_t epoch, int64_t *n_dst) {
   __shared__ int warp_counts[kTile / 32];
+  __shared__ unsigned int s_tile;
+  __shared__ uint32_t s_excl;
+  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+  __syncthreads();
+  const unsigned int tile = s_tile;
   const int64_t n_src = n_src_ptr ? *n_src_ptr : n_src_val;
-  const int64_t i = static_cast<int64_t>(blockIdx.x) * kTile + threadIdx.x;
-  if (static_cast<int64_t>(blockIdx.x) * kTile >= n_src) return;
+  const int64_t n_tiles_used = n_src > 0 ? (n_src + kTile - 1) / kTile : 1;  // tile 0 always reports
+  if (static_cast<int64_t>(tile) >= n_tiles_used) {
+    if (tile == gridDim.x - 1 && threadIdx.x == 0) *ticket = 0;  // the last ticket holder resets the counter
+    return;
+  }
+  const int64_t i = static_cast<int64_t>(tile) * kTile + threadIdx.x;
   const bool in_range = i < n_src;
-  const bool alive = in_range && (src.state[i] == 1);
+  // the whole record goes into registers before the scan: the loads are in flight while the tile waits for
+  // its prefix
+  double f[10] = {};
+  int64_t at_turn = 0, state = 0, at_element = 0, origin = 0;
+  if (in_range) {
+    state = src.state[i];
+    f[0] = src.x[i];
+    f[1] = src.px[i];
+    f[2] = src.y[i];
+    f[3] = src.py[i];
+    f[4] = src.zeta[i];
+    f[5] = src.delta[i];
+    f[6] = src.ptau[i];
+    f[7] = src.rpp[i];
+    f[8] = src.rvv[i];
+    f[9] = src.s[i];
+    at_turn = src.at_turn[i];
+    at_element = src.at_element ? src.at_element[i] : 0;
+    origin = src_origin ? src_origin[i] : i;
+  }
+  const bool alive = in_range && (state == 1);
   const unsigned ballot = __ballot_sync(0xffffffffu, alive);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (lane == 0) warp_counts[warp] = __popc(ballot);
   __syncthreads();
-  int before = 0;
-  for (int w = 0; w < warp; ++w) before += warp_counts[w];
-  const int rank = before + __popc(ballot & ((1u << lane) - 1u));
-  const int64_t origin = in_range ? (src_origin ? src_origin[i] : i) : 0;
-  if (alive) {
-    const int64_t j = tile_offsets[blockIdx.x] + rank;
-    copy_particle(dst, j, src, i);
-    dst_origin[j] = origin;
-  } else if (in_range && retire_lost) {
-    copy_particle(user, origin, src, i);
+  int before = 0, total = 0;
+#pragma unroll
+  for (int w = 0; w < kTile / 32; ++w) {
+    const int c = warp_counts[w];
+    if (w < warp) before += c;
+    total += c;
   }
+  if (warp == 0) {
+    // publish the tile's own count, then look back (32 predecessors at a time)
+    uint32_t excl = 0;
+    if (tile == 0) {
+      if (lane == 0) atomicExch(&status[0], pack_status(epoch, kFlagPrefix, static_cast<uint32_t>(total)));
+    } else {
+      if (lane == 0) atomicExch(&status[tile], pack_status(epoch, kFlagAggregate, static_cast<uint32_t>(total)));
+      int64_t look = static_cast<int64_t>(tile) - 1;
+      bool done = false;
+      while (!done) {
+        const int64_t k = look - lane;
+        uint64_t w = 0;
+        uint64_t flag = kFlagPrefix;  // lanes before tile 0 read as a zero prefix
+        if (k >= 0) {
+          do {
+            w = atomicAdd(&status[k], 0ull);  // volatile read through L2
+            flag = ((w >> 34) == epoch) ? ((w >> 32) & 3u) : 0u;
+          } while (flag == 0);
+        }
+        const unsigned has_prefix = __ballot_sync(0xffffffffu, flag == kFlagPrefix);
+        const int first = __ffs(has_prefix) - 1;  // nearest tile with a known inclusive prefix (there is one if k < 0 anywhere)
+        const uint32_t v = (k >= 0 && (first < 0 || lane <= first)) ? static_cast<uint32_t>(w) : 0u;
+        excl += __reduce_add_sync(0xffffffffu, v);
+        if (first >= 0) done = true;
+        else look -= 32;
+      }
+      if (lane == 0) atomicExch(&status[tile], pack_status(epoch, kFlagPrefix, excl + static_cast<uint32_t>(total)));
+    }
+    if (lane == 0) {
+      s_excl = excl;
+      if (static_cast<int64_t>(tile) == n_tiles_used - 1) *n_dst = static_cast<int64_t>(excl) + total;
+      if (tile == gridDim.x - 1) *ticket = 0;
+    }
+  }
+  __syncthreads();
+  const int rank = before + __popc(ballot & ((1u << lane) - 1u));
+  if (!in_range || (!alive && !retire_lost)) return;
+  const xt_particles &o = alive ? dst : user;
+  const int64_t j = alive ? static_cast<int64_t>(s_excl) + rank : origin;
+  o.x[j] = f[0];
+  o.px[j] = f[1];
+  o.y[j] = f[2];
+  o.py[j] = f[3];
+  o.zeta[j] = f[4];
+  o.delta[j] = f[5];
+  o.ptau[j] = f[6];
+  o.rpp[j] = f[7];
+  o.rvv[j] = f[8];
+  o.s[j] = f[9];
+  o.at_turn[j] = at_turn;
+  o.state[j] = state;
+  if (o.at_element) o.at_element[j] = at_element;
+  if (alive) dst_origin[j] = origin;
 }
 
 __global__ void __launch_bounds__(kTile) scatter_back_kernel(xt_particles src, const int64_t *src_origin,
@@ -135,7 +181,11 @@ __global__ void __launch_bounds__(256) histogram_kernel(const int64_t *__restric
       if (q > n_bins - 1) q = n_bins - 1;
       b = static_cast<int>(q);
     }
-    atomicAdd(&sh[b], 1u);
+    // neighbouring particles of an amplitude scan mostly share a bin: one shared-memory atomic per
+    // distinct bin of the warp instead of one per particle
+    const unsigned active = __activemask();
+    const unsigned same = __match_any_sync(active, b);
+    if ((__ffs(same) - 1) == static_cast<int>(threadIdx.x & 31)) atomicAdd(&sh[b], static_cast<unsigned int>(__popc(same)));
   }
   __syncthreads();
   for (int b = threadIdx.x; b <= n_bins; b += blockDim.x)
@@ -179,29 +229,32 @@ void plan_compaction(void *ws, int64_t n_part, CompactPlan &plan) {
     plan.w[k].origin = static_cast<int64_t *>(take());
   }
   plan.n_tiles = (n_part + kTile - 1) / kTile;
-  plan.tile_counts = reinterpret_cast<int64_t *>(at);
+  plan.status = reinterpret_cast<unsigned long long *>(at);
   at += align256(static_cast<size_t>(plan.n_tiles) * 8);
-  plan.n_active = reinterpret_cast<int64_t *>(at);
+  plan.counter[0] = reinterpret_cast<int64_t *>(at);
+  plan.counter[1] = plan.counter[0] + 1;
+  plan.ticket = reinterpret_cast<unsigned int *>(plan.counter[0] + 2);
+  plan.n_active = plan.counter[0];
+  plan.epoch = 0;
 }
 
-int launch_partition(const CompactPlan &plan, const xt_particles &src, const int64_t *src_origin,
-                     bool src_is_user, int64_t n_part, const WorkSet &dst, const xt_particles &user,
-                     cudaStream_t st) {
+int launch_partition(CompactPlan &plan, const xt_particles &src, const int64_t *src_origin, bool src_is_user,
+                     int64_t n_part, const WorkSet &dst, const xt_particles &user, cudaStream_t st) {
   if (n_part <= 0) return XT_OK;
-  const unsigned grid = static_cast<unsigned>(plan.n_tiles);
-  const int64_t *n_ptr = src_is_user ? nullptr : plan.n_active;
-  count_alive_kernel<<<grid, kTile, 0, st>>>(src.state, n_ptr, n_part, plan.tile_counts);
+  if (plan.epoch == 0) {  // first pass of the call: the status words and the ticket start from zero
+    XT_CUDA(cudaMemsetAsync(plan.status, 0, static_cast<size_t>(plan.n_tiles) * 8, st));
+    XT_CUDA(cudaMemsetAsync(plan.counter[0], 0, 32, st));
+  }
+  plan.epoch += 1;
+  // the pass reads the extent of src from one counter and writes the new alive count to the other
+  int64_t *n_in = plan.n_active;
+  int64_t *n_out = (n_in == plan.counter[0]) ? plan.counter[1] : plan.counter[0];
+  partition_fused_kernel<<<static_cast<unsigned>(plan.n_tiles), kTile, 0, st>>>(
+      src, src_origin, src_is_user ? nullptr : n_in, n_part, dst.p, dst.origin, user, src_is_user ? 0 : 1,
+      plan.status, plan.ticket, plan.epoch, n_out);
   XT_CUDA(cudaGetLastError());
-  // scan_tiles overwrites the counter with the new alive count, but the move kernel still
-  // needs the old extent of src: keep it in the second counter slot.
-  int64_t *n_old = plan.n_active + 1;
-  if (!src_is_user) XT_CUDA(cudaMemcpyAsync(n_old, plan.n_active, 8, cudaMemcpyDeviceToDevice, st));
-  scan_tiles_kernel<<<1, 1024, 0, st>>>(plan.tile_counts, plan.n_tiles, plan.n_active);
-  XT_CUDA(cudaGetLastError());
-  partition_move_kernel<<<grid, kTile, 0, st>>>(src, src_origin, src_is_user ? nullptr : n_old, n_part,
-                                               plan.tile_counts, dst.p, dst.origin, user, src_is_user ? 0 : 1);
-  XT_CUDA(cudaGetLastError());
-  count_launch(3);
+  plan.n_active = n_out;
+  count_launch();
   return XT_OK;
 }
 
@@ -220,7 +273,7 @@ int launch_histogram(const int64_t *at_turn, const int64_t *state, int64_t n, in
   XT_CUDA(cudaMemsetAsync(hist, 0, static_cast<size_t>(n_bins + 1) * 8, st));
   if (n <= 0) return XT_OK;
   int64_t grid = (n + 255) / 256;
-  if (grid > 148 * 8) grid = 148 * 8;
+  if (grid > 148 * 2) grid = 148 * 2;  // few CTAs: the global atomics at the end all hit the same n_bins + 1 words
   histogram_kernel<<<static_cast<unsigned>(grid), 256, static_cast<size_t>(n_bins + 1) * 4, st>>>(
       at_turn, state, n, bin_width, static_cast<int>(n_bins), reinterpret_cast<unsigned long long *>(hist));
   XT_CUDA(cudaGetLastError());

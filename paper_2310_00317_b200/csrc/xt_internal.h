@@ -194,14 +194,18 @@ size_t compaction_workspace_bytes(int64_t n_part);
 // Carves two WorkSets + counters + tile scratch out of `ws` (256-byte aligned pieces).
 struct CompactPlan {
   WorkSet w[2];
-  int64_t *n_active = nullptr;   // device counter
-  int64_t *tile_counts = nullptr;
+  int64_t *n_active = nullptr;   // device counter holding the extent of the current working set
+  int64_t *counter[2] = {nullptr, nullptr};  // n_active alternates between the two (a pass reads one, writes the other)
+  unsigned long long *status = nullptr;      // per-tile status words of the single-pass scan
+  unsigned int *ticket = nullptr;            // tile ticket counter
+  uint32_t epoch = 0;                        // pass number of this call (tags the status words)
   int64_t n_tiles = 0;
 };
 void plan_compaction(void *ws, int64_t n_part, CompactPlan &plan);
 // dst <- alive entries of src (stable); lost entries of src are written to `user` at their
-// origin unless src_is_user.  n_src read from plan.n_active unless src_is_user (then n_part).
-int launch_partition(const CompactPlan &plan, const xt_particles &src, const int64_t *src_origin,
+// origin unless src_is_user.  The extent of src is read from plan.n_active unless src_is_user (then n_part);
+// afterwards plan.n_active points to the counter that holds the new alive count.
+int launch_partition(CompactPlan &plan, const xt_particles &src, const int64_t *src_origin,
                      bool src_is_user, int64_t n_part, const WorkSet &dst, const xt_particles &user,
                      cudaStream_t st);
 int launch_scatter_back(const CompactPlan &plan, const WorkSet &src, int64_t n_part,

@@ -463,12 +463,17 @@ __device__ __forceinline__ void multipole_record(Parts<P> &q, ColdT &cold, const
 struct Hot {
   double x, px, y, py, zeta;
 };
+// Inlined into the P-times unrolled callers the thick maps of a thread's P particles interleave (P independent
+// chains through sincos / cosh / sinh instead of one); -DXT_THICK_INLINE=__noinline__ keeps one copy out of line.
+#ifndef XT_THICK_INLINE
+#define XT_THICK_INLINE __forceinline__
+#endif
 
 // Thick quadrupole (reading A18): the exact flow of
 // H = (px^2 + py^2)/(2(1+delta)) + (k1/2)(x^2 - y^2) over the length.  With w = sqrt(|k1|/(1+delta))
 // the focusing plane turns by w L (cos, sin), the other follows cosh, sinh; the path length is
 // zeta += L g/((1+delta)((1+delta)+b)) - rv0v/(2(1+delta)^2) int (px^2 + py^2) ds (closed form below).
-__device__ __noinline__ Hot thick_quadrupole_one(Hot h, const double delta, const double opd2, const double b,
+__device__ XT_THICK_INLINE Hot thick_quadrupole_one(Hot h, const double delta, const double opd2, const double b,
                                                  const double g, const double rv0v, const double k1,
                                                  const double length) {
   const double opd = 1.0 + delta;
@@ -509,7 +514,7 @@ __device__ __noinline__ Hot thick_quadrupole_one(Hot h, const double delta, cons
 // Thick sector bend, 'expanded' model (reading A19):
 // the exact flow of H = (px^2 + py^2)/(2(1+delta)) - h x (1+delta) + k0 x + (k0 h/2) x^2, i.e. the
 // thin curved multipole of step M2 smeared over the arc length.  Same arithmetic as the oracle's.
-__device__ __noinline__ Hot thick_bend_one(Hot p, const double delta, const double opd2, const double b,
+__device__ XT_THICK_INLINE Hot thick_bend_one(Hot p, const double delta, const double opd2, const double b,
                                            const double g, const double rv, const double k0, const double h,
                                            const double length) {
   const double opd = 1.0 + delta;

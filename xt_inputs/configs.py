@@ -22,7 +22,7 @@ from typing import Dict, List, Optional, Tuple
 
 import numpy as np
 
-from .packed import (Cavity, Drift, LimitEllipse, LimitRect, Multipole, SRotation,
+from .packed import (Bend, Cavity, Drift, LimitEllipse, LimitRect, Multipole, Quadrupole, SRotation,
                      XYShift, pack_lattice)
 
 P0C = 450e9                 # eV, BASELINE.json configs[0]
@@ -105,11 +105,16 @@ def _with_errors(main_order: int, main_strength: float, rng: np.random.Generator
 def lhc_like_elements(k3l: float = 1.0, misalign: bool = False, errors: bool = True,
                       apertures: bool = True,
                       err_seed: int = 2002, mis_seed: int = 3003,
-                      n_halfcells: int = LHC_NHALF) -> List:
+                      n_halfcells: int = LHC_NHALF, thick: bool = False) -> List:
     """configs[2] (k3l=1), configs[3] (misalign=True), configs[4] (k3l=5).
 
     400 half-cells; each magnet (and cavity) sits mid-slot as [Drift(l/2), magnet, Drift(l/2)];
     a LimitEllipse(20 mm, 15 mm) follows every 10th element.
+
+    ``thick=True`` (the thick-map bench workload): every quadrupole becomes a thick
+    Quadrupole (length min(3.1 m, 0.8 slot), k1 = k1l/length) and every bend a thick sector Bend ('expanded';
+    length 0.8 slot, k0 = h = hxl/length), each taking its length out of the two drifts of its slot; thick
+    elements carry no multipole errors; sextupoles and octupoles stay thin with their order-15 errors.
     """
     rng = np.random.default_rng(err_seed)
     rng_mis = np.random.default_rng(mis_seed)
@@ -130,6 +135,8 @@ def lhc_like_elements(k3l: float = 1.0, misalign: bool = False, errors: bool = T
         sign = +1.0 if focusing else -1.0
         slots: List[List] = []
         quad = magnet(1, +LHC_KF if focusing else -LHC_KD)
+        if thick:
+            quad = ("quad", +LHC_KF if focusing else -LHC_KD)
         if misalign:
             dx, dy = rng_mis.normal(0.0, 1e-4, size=2)
             th = rng_mis.normal(0.0, 1e-4)
@@ -143,7 +150,8 @@ def lhc_like_elements(k3l: float = 1.0, misalign: bool = False, errors: bool = T
             slots.append([magnet(3, sign * k3l)])                        # O
         if arc:
             for b in range(4):
-                slots.append([magnet(0, hxl_bend, hxl=hxl_bend, length=LHC_BEND_LEN)])
+                slots.append([("bend", hxl_bend)] if thick else
+                             [magnet(0, hxl_bend, hxl=hxl_bend, length=LHC_BEND_LEN)])
                 if b == 1:
                     slots.append([magnet(2, k2l)])                       # S2 between bend pairs
         else:
@@ -152,9 +160,20 @@ def lhc_like_elements(k3l: float = 1.0, misalign: bool = False, errors: bool = T
                 slots.append([Cavity(1e6, 400e6, 180.0)])
         half = 0.5 * (LHC_LHALF / len(slots))
         for group in slots:
-            base.append(Drift(half))
+            taken = 0.0
+            for k, el in enumerate(group):
+                if isinstance(el, tuple):                      # thick stand-in: (kind, integrated strength)
+                    kind, strength = el
+                    if kind == "quad":
+                        length = min(3.1, 1.6 * half)
+                        group[k] = Quadrupole(strength / length, length)
+                    else:
+                        length = 1.6 * half
+                        group[k] = Bend(strength / length, strength / length, length)
+                    taken = length
+            base.append(Drift(half - 0.5 * taken))
             base.extend(group)
-            base.append(Drift(half))
+            base.append(Drift(half - 0.5 * taken))
     if not apertures:
         return base
     out: List = []
@@ -175,6 +194,11 @@ def lattice_cfg3() -> List:
 
 def lattice_cfg4() -> List:
     return lhc_like_elements(k3l=5.0)
+
+
+def lattice_cfg2_thick() -> List:
+    """configs[2] with thick quadrupoles and thick sector bends (bench.py --workload thick)."""
+    return lhc_like_elements(k3l=1.0, thick=True)
 
 
 def strip_cavities(elements: List) -> List:
