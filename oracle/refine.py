@@ -150,7 +150,7 @@ def sliced_elements(elements: Sequence, frames: Sequence, poly_u, poly_l, seg_le
                 elif isinstance(el, PK.Quadrupole):
                     out.append(PK.Quadrupole(el.k1, piece))
                 else:
-                    out.append(PK.Bend(el.k0, el.h, piece))
+                    out.append(PK.Bend(el.k0, el.h, piece, el.model))
                 sloc_of.append(sloc)
                 sloc = sloc + piece
                 lam = sloc / seg_len

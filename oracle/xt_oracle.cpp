@@ -79,8 +79,9 @@ struct Element {
   double a = 0.0, b = 0.0, a2 = 0.0, b2 = 0.0, a2b2 = 0.0;
   // QUADRUPOLE (thick): k1, length
   double k1 = 0.0;
-  // BEND (thick sector bend): k0, h, length
+  // BEND (thick sector bend): k0, h, length; model 0 = 'expanded', 1 = 'full'
   double k0 = 0.0, h = 0.0;
+  int model = 0;
   // LIMITPOLYGON: vertices (vx[i], vy[i]), closed
   std::vector<double> vx, vy;
   // RADMULTIPOLE: as MULTIPOLE (c[0] folded, wf from the raw knl[0]), plus krad = (2/3) r0 (beta0 gamma0)^3
@@ -207,6 +208,8 @@ int parse(const void* packed, size_t nbytes, Lattice& L) {
       case BEND:
         if (!rd(e.k0) || !rd(e.h) || !rd(e.length)) return -2;
         if (!(e.k0 * e.h > 0.0) || !(e.length > 0.0)) return -2;   // focusing strength k0 h must be > 0
+        if (aux > 1u) return -2;                                     // 0: 'expanded', 1: 'full'
+        e.model = static_cast<int>(aux);
         s = s + e.length;
         break;
       case RADMULTIPOLE: {
@@ -472,6 +475,44 @@ int xo_track(const void* packed, size_t nbytes, const xo_particles* P, int64_t n
           }
 
           case BEND: {
+            if (e.model == 1) {
+              // Thick sector bend, 'full' model ("a 'full' map, which is appropriate for small
+              // accelerators [12]"; reading A23): the exact map of a charge in the uniform field k0 seen from
+              // the frame that follows the arc of curvature h -- the helix, cut by the exit plane.  With
+              // pz = sqrt((1+delta)^2 - px^2 - py^2), theta = h L and C = pz - k0 (1/h + x):
+              //   px' = px cos(theta) + C sin(theta)
+              //   x'  = (h pz' - dpx'/ds - k0)/(h k0),  dpx'/ds = h (C cos(theta) - px sin(theta))
+              //   y'  = y + py (theta + D)/k0,  D = asin(px/ph) - asin(px'/ph),  ph^2 = (1+delta)^2 - py^2
+              //   zeta' = zeta + L - (1 + beta0 ptau)(theta + D)/k0          (path length (1+delta)(theta + D)/k0)
+              // evaluated in a form without cancellation (the reference particle of a matched bend has every
+              // term below exactly zero): pz - 1 = (delta(delta+2) - px^2 - py^2)/(pz + 1),
+              // C = (pz - 1) - (k0 - h)/h - k0 x,  1 - cos(theta) = 2 sin^2(theta/2),
+              // pz' - pz = -(px' - px)(px' + px)/(pz' + pz), which turn x' into
+              //   x' = x + [px sin + (1 - cos) C - (px' - px)(px + px')/(pz' + pz)]/k0
+              // and L - (1 + beta0 ptau) theta/k0 into ((k0 - h) - h beta0 ptau) L/k0.
+              const double t1 = px * px;
+              const double pxy2 = py * py + t1;
+              const double pz = std::sqrt(k.opd2 - pxy2);
+              const double dpz = (delta * (delta + 2.0) - pxy2) / (pz + 1.0);
+              const double eps = (e.k0 - e.h) / e.h;
+              const double cc = (dpz - eps) - e.k0 * x;
+              const double th = e.h * e.length;
+              const double sn = std::sin(th);
+              const double sh = std::sin(0.5 * th);
+              const double c1 = 2.0 * (sh * sh);
+              const double dpx = cc * sn - px * c1;
+              const double px1 = px + dpx;
+              const double ph2 = k.opd2 - py * py;
+              const double pz1 = std::sqrt(ph2 - px1 * px1);
+              const double num = (px * sn + c1 * cc) - (dpx * (px + px1)) / (pz1 + pz);
+              const double iph = 1.0 / std::sqrt(ph2);
+              const double dd = std::asin(px * iph) - std::asin(px1 * iph);
+              x = num / e.k0 + x;
+              y = (py * (th + dd)) / e.k0 + y;
+              zeta = (zeta + (((e.k0 - e.h) - e.h * (L.beta0 * ptau)) * e.length) / e.k0) - (k.b * dd) / e.k0;
+              px = px1;
+              break;
+            }
             // Thick sector bend, 'expanded' model ("the bend can be 'full' or 'expanded'";
             // reading A19): exact flow of
             //   H = (px^2 + py^2)/(2(1+delta)) - h x (1+delta) + k0 x + (k0 h/2) x^2

@@ -18,8 +18,9 @@ accelerator element".  Here that sequence is flattened into one little-endian,
     type 6 LIMITRECT     aux=0  min_x, max_x, min_y, max_y
     type 7 LIMITELLIPSE  aux=0  a, b
     type 8 QUADRUPOLE    aux=0  k1 [1/m^2], length [m]   (thick; k1 != 0, length > 0)
-    type 9 BEND          aux=0  k0 [1/m], h [1/m], length [m]   (thick sector bend, 'expanded' map,
-                                PAPER.md:72; k0*h > 0, length > 0; a pure sector bend has k0 = h)
+    type 9 BEND          aux=m  k0 [1/m], h [1/m], length [m]   (thick sector bend: m = 0 the
+                                'expanded' map, m = 1 the 'full' map; k0*h > 0, length > 0; a pure sector
+                                bend has k0 = h)
     type 10 LIMITPOLYGON aux=n  x[0..n), y[0..n)   (closed polygon, 3 <= n <= 256 vertices; PAPER.md:178
                                 "polygonal interpolation")
     type 12 RADMULTIPOLE aux=N  hxl, length, knl[0..N], ksl[0..N]   (thin multipole with "mean" synchrotron
@@ -115,11 +116,12 @@ class Quadrupole:
 
 @dataclass(frozen=True)
 class Bend:
-    """Thick sector bend ('expanded' model): dipole strength k0 = By/(P0/q0), curvature h
-    of the reference orbit, arc length."""
+    """Thick sector bend: dipole strength k0 = By/(P0/q0), curvature h of the reference
+    orbit, arc length; model 0 = the 'expanded' map, 1 = the 'full' map."""
     k0: float
     h: float
     length: float
+    model: int = 0
 
 
 @dataclass(frozen=True)
@@ -167,7 +169,7 @@ def _record(el) -> bytes:
     if isinstance(el, Quadrupole):
         return struct.pack("<II2d", 8, 0, el.k1, el.length)
     if isinstance(el, Bend):
-        return struct.pack("<II3d", 9, 0, el.k0, el.h, el.length)
+        return struct.pack("<II3d", 9, int(el.model), el.k0, el.h, el.length)
     if isinstance(el, LimitPolygon):
         assert len(el.x) == len(el.y)
         return struct.pack("<II%dd" % (2 * len(el.x)), 10, len(el.x), *el.x, *el.y)
@@ -223,7 +225,7 @@ def unpack_lattice(buf: bytes):
             out.append(Quadrupole(k1, length))
         elif t == 9:
             k0, h, length = struct.unpack_from("<3d", buf, off); off += 24
-            out.append(Bend(k0, h, length))
+            out.append(Bend(k0, h, length, aux))
         elif t == 12:
             m = aux + 1
             vals = struct.unpack_from("<%dd" % (2 + 2 * m), buf, off); off += 8 * (2 + 2 * m)
