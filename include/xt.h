@@ -54,8 +54,9 @@ enum {
   XT_LIMITELLIPSE = 7,/* a, b (edge inclusive)                                   (step A)   */
   XT_QUADRUPOLE = 8,  /* k1 [1/m^2], length [m]: thick quadrupole, k1 != 0, length > 0           */
                       /* (reading A18)             */
-  XT_BEND = 9,        /* k0 [1/m], h [1/m], length [m]: thick sector bend, 'expanded' model,     */
-                      /* k0*h > 0, length > 0 (reading A19)               */
+  XT_BEND = 9,        /* k0 [1/m], h [1/m], length [m]: thick sector bend, k0*h > 0, length > 0; */
+                      /* aux = 0: the 'expanded' map (reading A19), aux = 1: the 'full' */
+                      /* map, the exact helix in the uniform field (reading A23)    */
   XT_LIMITPOLYGON = 10,/* aux = n vertices (3..256); x[0..n), y[0..n): closed polygon, even-odd   */
                       /* rule, NaN lost ("polygonal"; reading A20)         */
                       /* 11 is reserved (internal)                                                */

@@ -166,6 +166,111 @@ def normal_form4(J):
     return out
 
 
+S6 = np.zeros((6, 6))
+for _k in range(3):
+    S6[2 * _k, 2 * _k + 1], S6[2 * _k + 1, 2 * _k] = 1.0, -1.0
+
+
+def normal_form6(J, rvv_co=1.0):
+    """Twiss steps 3 and 5 in six dimensions ("Linear Normal Form of the map from the
+    eigenvalues and eigenvectors of the Jacobian matrix", "Mais-Ripken").  J is the one-turn matrix in
+    (x, px, y, py, zeta, delta) as ``jac6`` gives it; rvv_co = beta/beta0 on the closed orbit turns it into
+    the canonical variables (..., zeta, pzeta = ptau/beta0): d pzeta = rvv d delta (dE = beta c dP).
+    numpy.linalg.eig; of each conjugate pair the eigenvector with v^H S v = +2i after scaling is kept; the
+    longitudinal mode (3) is the one with the smallest tune angle, of the other two mode 1 is the one with
+    the larger horizontal part; phase origin: the mode's own plane (x, y, zeta) real positive.
+    Mais-Ripken functions of mode k in plane u (x, y, zeta): beta_uk = |v_u|^2, alpha_uk = -Re(conj(v_u) v_pu).
+    Dispersion "from the eigenvectors" (step 5): the transverse part of the longitudinal mode per unit of its
+    momentum part, D_u = Re(v_u / v_pzeta) per pzeta, x rvv_co per delta.  Returns None if an eigenvalue is off
+    the unit circle or real."""
+    t = np.diag([1.0, 1.0, 1.0, 1.0, 1.0, rvv_co])
+    jc = t @ np.asarray(J, dtype=np.float64) @ np.linalg.inv(t)
+    lam, vec = np.linalg.eig(jc)
+    modes = []
+    for k in range(6):
+        if abs(abs(lam[k]) - 1.0) > 1e-5 or abs(lam[k].imag) < 1e-12:
+            return None
+        v = vec[:, k]
+        norm = (np.conj(v) @ S6 @ v).imag / 2.0
+        if norm > 0.0:
+            modes.append((lam[k], v / math.sqrt(norm)))
+    if len(modes) != 3:
+        return None
+    modes.sort(key=lambda m: abs(math.atan2(m[0].imag, m[0].real)))
+    longitudinal, rest = modes[0], modes[1:]
+    rest.sort(key=lambda m: -abs(m[1][0]) ** 2)
+    out = {}
+    for k, (lmb, v) in enumerate(rest + [longitudinal], start=1):
+        ref = v[2 * (k - 1)]
+        v = v * (abs(ref) / ref)
+        out["q%d_frac" % k] = (math.atan2(lmb.imag, lmb.real) / (2 * math.pi)) % 1.0
+        out["v%d" % k] = v
+        for name, i in (("x", 0), ("y", 2), ("z", 4)):
+            out["bet%s%d" % (name, k)] = abs(v[i]) ** 2
+            out["alf%s%d" % (name, k)] = -(np.conj(v[i]) * v[i + 1]).real
+    v3 = out["v3"]
+    for name, i in (("dx", 0), ("dpx", 1), ("dy", 2), ("dpy", 3)):
+        out[name] = (v3[i] / v3[5]).real * rvv_co
+    return out
+
+
+def optics6d_along(elements, p0c, mass0, q0, rows, guess=None):
+    """The six-dimensional optics carried along the line (steps 4-5: the eigenvectors are
+    propagated "to all other elements by tracking").  For every requested row i (the entrance of element i):
+    the 6x6 Jacobian J_i of the map from the start to row i by central differences around the 6-D closed
+    orbit (steps of ``jac6``), in canonical variables at both ends (rvv at the start and at the row), and the
+    three eigenvectors v_k(i) = J_i v_k(0): beta_uk = |v_u|^2, alpha_uk, the mode phases
+    mu_k = arg of the mode's own component (mod 2 pi), and the dispersion of the longitudinal mode.  Each row
+    is tracked through its own prefix line."""
+    from xt_inputs import packed as PK
+    buf = PK.pack_lattice(elements, p0c, mass0, q0)
+    on = optics6d_of(buf, guess)
+    z0 = on["co"]
+    beta0, _ = O.reference(buf)
+
+    def rvv_of(delta, ptau):
+        return (1.0 + delta) / (1.0 + beta0 * ptau)
+
+    def ptau_of(delta):
+        tt = delta * (delta + 2.0)
+        return tt / (math.sqrt(tt + 1.0 / beta0 ** 2) + 1.0 / beta0)
+
+    rvv0 = rvv_of(z0[5], ptau_of(z0[5]))
+    nf = normal_form6(on["m"], rvv0)
+    assert nf is not None
+    on.update(nf)
+    pts = np.tile(z0, (13, 1))
+    for i in range(6):
+        pts[1 + 2 * i, i] += H6[i]
+        pts[2 + 2 * i, i] -= H6[i]
+    out = []
+    for row in rows:
+        prefix = PK.pack_lattice(list(elements[:row]) or [PK.Marker()], p0c, mass0, q0)
+        p = O.new_particles(prefix, dict(x=pts[:, 0].copy(), px=pts[:, 1].copy(), y=pts[:, 2].copy(),
+                                         py=pts[:, 3].copy(), zeta=pts[:, 4].copy(), delta=pts[:, 5].copy()))
+        O.track(prefix, p, 1)
+        assert np.all(p["state"] == 1)
+        z = np.stack([p["x"], p["px"], p["y"], p["py"], p["zeta"], p["delta"]], axis=1)
+        J = np.zeros((6, 6))
+        for i in range(6):
+            J[:, i] = (z[1 + 2 * i] - z[2 + 2 * i]) / (2 * H6[i])
+        rvv1 = rvv_of(p["delta"][0], p["ptau"][0])
+        jc = np.diag([1, 1, 1, 1, 1, rvv1]) @ J @ np.diag([1, 1, 1, 1, 1, 1.0 / rvv0])
+        r = {"co": z[0].copy()}
+        for k in (1, 2, 3):
+            v = jc @ nf["v%d" % k]
+            for name, i in (("x", 0), ("y", 2), ("z", 4)):
+                r["bet%s%d" % (name, k)] = abs(v[i]) ** 2
+                r["alf%s%d" % (name, k)] = -(np.conj(v[i]) * v[i + 1]).real
+            own = v[2 * (k - 1)]
+            r["mu%d" % k] = math.atan2(own.imag, own.real) % (2 * math.pi)
+            if k == 3:
+                for name, i in (("dx", 0), ("dpx", 1), ("dy", 2), ("dpy", 3)):
+                    r[name] = (v[i] / v[5]).real * rvv1
+        out.append(r)
+    return on, out
+
+
 def chromatic_optics_of(buf, ddelta=1e-4, delta=0.0):
     """Dispersion and chromaticity at the start of the line (the optics "as a function of the
     momentum"): central differences in delta of the closed orbit and of the tunes, each from the three steps

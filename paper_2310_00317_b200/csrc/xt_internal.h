@@ -66,6 +66,7 @@ enum : uint32_t {
   TAG_BEND = 10,
   TAG_POLY = 11,
   TAG_RMULT = 13,  // radiating multipole: p0 = hxl; (c[n], s[n]) pairs n = N .. 0 (c[0] = knl[0] - hxl); {wf, length}; {krad, 0}
+  TAG_BENDF = 14,  // thick sector bend, 'full' map
   TAG_MON = 12,  // internal: store the coordinates of every alive particle into row p0 of the monitor buffer
   TAG_TYPE_MASK = 0xf,
   TAG_PRE = 0x10,   // a drift of length l_pre comes first

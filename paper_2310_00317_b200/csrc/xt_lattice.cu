@@ -258,8 +258,12 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
           set_error("xt_lattice_create: thick bend needs k0*h > 0 and length > 0");
           return XT_ERR_BAD_LATTICE;
         }
+        if (aux > 1u) {
+          set_error("xt_lattice_create: thick bend model (aux) must be 0 ('expanded') or 1 ('full')");
+          return XT_ERR_BAD_LATTICE;
+        }
         out.extended = true;
-        rec.type = TAG_BEND;
+        rec.type = aux == 1u ? TAG_BENDF : TAG_BEND;
         rec.p0 = k0;
         rec.slot(h, length);
         info.n_thick += 1;

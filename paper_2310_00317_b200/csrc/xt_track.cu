@@ -545,6 +545,54 @@ __device__ XT_THICK_INLINE Hot thick_bend_one(Hot p, const double delta, const d
   return o;
 }
 
+// Thick sector bend, 'full' model ("a 'full' map, which is appropriate for small accelerators";
+// DESIGN.md reading A23): the helix of a charge in the uniform field k0, cut by the exit plane of the frame
+// of curvature h, in the cancellation-free form of the oracle (same arithmetic order).
+__device__ XT_THICK_INLINE Hot thick_bend_full_one(Hot p, const double delta, const double opd2, const double b,
+                                                   const double ptau, const double beta0, const double k0,
+                                                   const double h, const double length) {
+  const double x = p.x, px = p.px, py = p.py;
+  const double t1 = XT_MUL(px, px);
+  const double pxy2 = XT_MADD(py, py, t1);
+  const double pz = sqrt(opd2 - pxy2);
+  const double dpz = XT_NMADD(1.0, pxy2, XT_MUL(delta, delta + 2.0)) / (pz + 1.0);  // pz - 1
+  const double eps = (k0 - h) / h;
+  const double cc = XT_NMADD(k0, x, dpz - eps);
+  const double th = XT_MUL(h, length);
+  const double sn = sin(th);
+  const double sh = sin(XT_MUL(0.5, th));
+  const double c1 = XT_MUL(2.0, XT_MUL(sh, sh));  // 1 - cos
+  const double dpx = XT_NMADD(px, c1, XT_MUL(cc, sn));
+  const double px1 = px + dpx;
+  const double ph2 = XT_NMADD(py, py, opd2);
+  const double pz1 = sqrt(XT_NMADD(px1, px1, ph2));
+  const double num = XT_MADD(px, sn, XT_MUL(c1, cc)) - XT_MUL(dpx, px + px1) / (pz1 + pz);
+  const double iph = 1.0 / sqrt(ph2);
+  const double dd = asin(XT_MUL(px, iph)) - asin(XT_MUL(px1, iph));
+  Hot o;
+  o.x = num / k0 + x;
+  o.y = XT_MUL(py, th + dd) / k0 + p.y;
+  o.zeta = (p.zeta + XT_MUL(XT_NMADD(h, XT_MUL(beta0, ptau), k0 - h), length) / k0) - XT_MUL(b, dd) / k0;
+  o.px = px1;
+  o.py = py;
+  return o;
+}
+
+template <int P, class ColdT>
+__device__ __forceinline__ void thick_bend_full(Parts<P> &q, ColdT &cold, const double k0, const double h,
+                                                const double length, const double beta0) {
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    const Hot o = thick_bend_full_one(Hot{q.x[j], q.px[j], q.y[j], q.py[j], q.zeta[j]}, cold.delta(j), cold.opd2(j),
+                                      cold.b(j), cold.ptau(j), beta0, k0, h, length);
+    q.x[j] = o.x;
+    q.px[j] = o.px;
+    q.y[j] = o.y;
+    q.py[j] = o.py;
+    q.zeta[j] = o.zeta;
+  }
+}
+
 template <int P, class ColdT>
 __device__ __forceinline__ void thick_quadrupole(Parts<P> &q, ColdT &cold, const double k1, const double length) {
 #pragma unroll
@@ -820,6 +868,7 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
           const int order = static_cast<int>((tag >> 8) & 0x7fu);
           if (type == TAG_QUAD) thick_quadrupole<P>(q, cold, p0, pf[0].x);                 // p0 = k1, {length, 0}
           else if (type == TAG_BEND) thick_bend<P>(q, cold, p0, pf[0].x, pf[0].y);         // p0 = k0, {h, length}
+          else if (type == TAG_BENDF) thick_bend_full<P>(q, cold, p0, pf[0].x, pf[0].y, a.beta0);
           else if (type == TAG_RMULT) rad_multipole<P>(q, cold, slots, order, p0, a);      // p0 = hxl
           else if (type == TAG_MON) monitor_store<P>(q, cold, p0, a);                      // p0 = row
           else if (type == TAG_POLY)  // (record bytes - header) / 16 vertices

@@ -1,6 +1,7 @@
-"""Thick sector bend ('expanded' model, reading A19) on the GPU path against the oracle: a
-ring of thick bends and thick quadrupoles with a cavity and apertures; 1 turn at 1e-12, 100 turns at
-1e-10, losses exact, every launch shape bit-identical."""
+"""Thick sector bend ('expanded' model, reading A19, and 'full' model, reading A23) on the GPU
+path against the oracle: a ring of thick bends and thick quadrupoles with a cavity and apertures; 1 turn
+at 1e-12, 100 turns at 1e-10, losses exact, every launch shape bit-identical; a small ring (rho = 3.8 m)
+of 'full' bends, where the two models differ visibly."""
 import numpy as np
 import pytest
 
@@ -23,10 +24,11 @@ def X():
     return X
 
 
-def ring(n_cells=16, aperture=0.04):
-    h = 2.0 * np.pi / (2 * n_cells * 6.0)                      # 2 bends of 6 m per cell close the ring
-    cell = [Quadrupole(+0.35, 0.6), Drift(0.5), Bend(h, h, 6.0), Drift(0.5), Multipole(knl=(0.0, 0.0, 0.3)),
-            Quadrupole(-0.35, 0.6), Drift(0.5), Bend(h * 1.0001, h, 6.0), Drift(0.5), LimitEllipse(aperture, aperture)]
+def ring(n_cells=16, aperture=0.04, model=0, bend_len=6.0):
+    h = 2.0 * np.pi / (2 * n_cells * bend_len)                 # 2 bends per cell close the ring
+    cell = [Quadrupole(+0.35, 0.6), Drift(0.5), Bend(h, h, bend_len, model), Drift(0.5),
+            Multipole(knl=(0.0, 0.0, 0.3)), Quadrupole(-0.35, 0.6), Drift(0.5),
+            Bend(h * 1.0001, h, bend_len, model), Drift(0.5), LimitEllipse(aperture, aperture)]
     return cell * n_cells + [Cavity(1e6, 200e6, 180.0)]
 
 
@@ -41,8 +43,9 @@ def close(got, ref, rtol, sel):
     H.assert_parity(got, ref, rtol, sel=sel, keys=KEYS)      # reading A8: per-coordinate floor
 
 
-def test_thick_bend_ring_parity(X):
-    buf = pack_lattice(ring(), P0C, MASS0, 1.0)
+@pytest.mark.parametrize("model,bend_len", [(0, 6.0), (1, 6.0), (1, 1.5)])
+def test_thick_bend_ring_parity(X, model, bend_len):
+    buf = pack_lattice(ring(model=model, bend_len=bend_len), P0C, MASS0, 1.0)
     co = ensemble(4000)
     lat = X.xt_lattice_create(buf)
     assert lat.info["n_thick"] == 64
@@ -59,8 +62,23 @@ def test_thick_bend_ring_parity(X):
     lat.close()
 
 
-def test_thick_bend_losses_and_shapes(X):
-    buf = pack_lattice(ring(aperture=0.003), P0C, MASS0, 1.0)
+def test_full_and_expanded_differ_in_a_small_ring(X):
+    """The two models are different maps (they agree to second order only): in the rho = 3.8 m ring the GPU
+    results differ by far more than the parity tolerance, each agreeing with its own oracle model."""
+    co = ensemble(500, scale=3.0)
+    out = []
+    for model in (0, 1):
+        lat = X.xt_lattice_create(pack_lattice(ring(model=model, bend_len=1.5), P0C, MASS0, 1.0))
+        p = X.new_particles(lat, co)
+        X.xt_track(lat, p, 1)
+        out.append(X.particles_to_host(p))
+        lat.close()
+    assert 1e-9 < np.max(np.abs(out[0]["x"] - out[1]["x"])) < 1e-4
+
+
+@pytest.mark.parametrize("model", [0, 1])
+def test_thick_bend_losses_and_shapes(X, model):
+    buf = pack_lattice(ring(aperture=0.003, model=model), P0C, MASS0, 1.0)
     co = ensemble(2500, scale=4.0)
     ref = O.new_particles(buf, co)
     mm = np.full(2500, np.inf)
@@ -83,7 +101,8 @@ def test_thick_bend_losses_and_shapes(X):
                 a, b = got[k], base[k]
                 assert ((a == b) | (np.isnan(a.astype(np.float64)) & np.isnan(b.astype(np.float64)))).all(), (ppt, k)
     lat.close()
-    for bad in (Bend(0.0, 1e-3, 1.0), Bend(1e-3, -1e-3, 1.0), Bend(1e-3, 1e-3, 0.0)):
+    for bad in (Bend(0.0, 1e-3, 1.0, model), Bend(1e-3, -1e-3, 1.0, model), Bend(1e-3, 1e-3, 0.0, model),
+                Bend(1e-3, 1e-3, 1.0, 2)):
         with pytest.raises(X.XtError) as e:
             X.xt_lattice_create(pack_lattice([bad], P0C, MASS0, 1.0))
         assert e.value.code == -2
