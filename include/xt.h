@@ -325,6 +325,45 @@ typedef struct {
 } xt_twiss6d_result;
 int xt_twiss6d(const xt_lattice *lat, const double *guess6, xt_twiss6d_result *out, void *cuda_stream);
 
+/* Linear normal form in six dimensions (Twiss steps 3-5).  Pure HOST
+ * arithmetic, no CUDA call.  m: the 6x6 one-turn matrix of xt_twiss6d_result (row-major, variables x, px, y,
+ * py, zeta, delta); rvv_co = beta/beta0 on the closed orbit, which turns delta into the canonical
+ * pzeta = ptau/beta0 (d pzeta = rvv d delta; 1 for delta = 0).  The three pairs of eigenvalues follow from the
+ * cubic of xt_twiss6d; the eigenvector of exp(i mu_k) is (M - conj(lambda_k)) prod_{j != k} (M^2 - u_j M + 1) w;
+ * of each conjugate pair the one with v^H S v = +2i is kept.  Mode 3 is the one with the smallest tune angle
+ * (longitudinal); of the other two, mode 1 has the larger horizontal part; phase origin: the mode's own plane
+ * (x, y, zeta) real positive.  bet[u][k], alf[u][k]: Mais-Ripken functions of mode k in plane u (0 x, 1 y,
+ * 2 zeta): |v_u|^2 and -Re(conj(v_u) v_pu).  disp: dispersion "from the eigenvectors", Re(v_u / v_pzeta) of
+ * the longitudinal mode per unit delta (dx, dpx, dy, dpy).  q_frac[k]: arg(lambda_k)/2 pi in [0, 1).
+ * stable = 0 (and NaN) if an eigenvalue leaves the unit circle; degenerate = 1 (and NaN) if two modes have the
+ * same tune within what a central-difference matrix resolves. */
+typedef struct {
+  double q_frac[3];
+  double bet[3][3], alf[3][3]; /* [plane][mode] */
+  double disp[4];
+  double v[3][12];             /* eigenvectors: (re, im) of x, px, y, py, zeta, pzeta */
+  int32_t stable, degenerate;
+} xt_twiss6d_modes;
+int xt_twiss6d_normal_form(const double *m, double rvv_co, xt_twiss6d_modes *out);
+
+/* The six-dimensional optics along the line (the eigenvectors are propagated "to all other
+ * elements by tracking").  xt_twiss6d at the start, its normal form, then ONE launch of thirteen probes (the
+ * closed orbit and +-h along the six coordinates) through a copy of the line with a monitor record in front of
+ * every element; per row the host forms the 6x6 Jacobian from the start (canonical variables at both ends) and
+ * carries the three eigenvectors through it.  rows (HOST, cap >= n_elements + 1): row i = the entrance of
+ * element i, the last row the end of the line.  mu[k]: phase of mode k's own component from the start,
+ * unwrapped (the betatron phases only grow; the synchrotron phase is counted in its own sense).  start,
+ * start_modes may be NULL.  Errors as xt_twiss6d; XT_ERR_UNSTABLE also for degenerate modes.  Synchronises. */
+typedef struct {
+  double s;
+  double co[6];                /* closed orbit: x, px, y, py, zeta, delta */
+  double bet[3][3], alf[3][3]; /* [plane][mode] */
+  double mu[3];
+  double disp[4];              /* dx, dpx, dy, dpy per unit delta, from the longitudinal eigenvector */
+} xt_twiss6d_row;
+int xt_twiss6d_line(const xt_lattice *lat, const double *guess6, xt_twiss6d_result *start,
+                    xt_twiss6d_modes *start_modes, xt_twiss6d_row *rows, int64_t cap, void *cuda_stream);
+
 /* Linear normal form of a 4x4 one-turn matrix with coupling (PAPER.md:98 step 3 "from the eigenvalues and
  * eigenvectors of the Jacobian matrix", step 5 "Mais-Ripken").  Pure HOST arithmetic,
  * no CUDA call.  m: row-major, e.g. xt_twiss4d_result.m.  The characteristic polynomial of a symplectic

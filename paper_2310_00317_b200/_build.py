@@ -14,7 +14,7 @@ from typing import Dict, List
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["xt_api.cu", "xt_lattice.cu", "xt_track.cu", "xt_compact.cu", "xt_peak.cu", "xt_twiss.cu", "xt_refine.cu", "xt_knobs.cu"]
+SOURCES = ["xt_api.cu", "xt_lattice.cu", "xt_track.cu", "xt_compact.cu", "xt_peak.cu", "xt_twiss.cu", "xt_twiss6d.cu", "xt_refine.cu", "xt_knobs.cu"]
 HEADERS = [os.path.join(CSRC, "xt_internal.h"), os.path.join(CSRC, "xt_line.h"),
            os.path.join(os.path.dirname(HERE), "include", "xt.h")]
 

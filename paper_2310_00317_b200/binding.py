@@ -80,6 +80,17 @@ class xt_twiss6d_result(ctypes.Structure):
                 ("reserved", ctypes.c_int32)]
 
 
+class xt_twiss6d_modes(ctypes.Structure):
+    _fields_ = [("q_frac", ctypes.c_double * 3), ("bet", (ctypes.c_double * 3) * 3), ("alf", (ctypes.c_double * 3) * 3),
+                ("disp", ctypes.c_double * 4), ("v", (ctypes.c_double * 12) * 3),
+                ("stable", ctypes.c_int32), ("degenerate", ctypes.c_int32)]
+
+
+class xt_twiss6d_row(ctypes.Structure):
+    _fields_ = [("s", ctypes.c_double), ("co", ctypes.c_double * 6), ("bet", (ctypes.c_double * 3) * 3),
+                ("alf", (ctypes.c_double * 3) * 3), ("mu", ctypes.c_double * 3), ("disp", ctypes.c_double * 4)]
+
+
 class xt_twiss_row(ctypes.Structure):
     _fields_ = [(k, ctypes.c_double) for k in ("s", "x", "px", "y", "py", "betx", "alfx", "mux", "bety", "alfy",
                                                 "muy", "dx", "dpx", "dy", "dpy", "betx1", "bety1", "betx2", "bety2",
@@ -140,6 +151,10 @@ SIGNATURES = {
     "xt_twiss4d_chrom": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
                                         ctypes.POINTER(xt_twiss4d_chrom_result), _VP]),
     "xt_twiss6d": (ctypes.c_int, [_VP, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(xt_twiss6d_result), _VP]),
+    "xt_twiss6d_normal_form": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double), ctypes.c_double,
+                                              ctypes.POINTER(xt_twiss6d_modes)]),
+    "xt_twiss6d_line": (ctypes.c_int, [_VP, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(xt_twiss6d_result),
+                                       ctypes.POINTER(xt_twiss6d_modes), ctypes.POINTER(xt_twiss6d_row), _I64, _VP]),
     "xt_twiss4d_normal_form": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(xt_twiss4d_modes)]),
     "xt_twiss4d_line": (ctypes.c_int, [_VP, ctypes.c_double, ctypes.c_double, ctypes.POINTER(ctypes.c_double),
                                        ctypes.POINTER(xt_twiss4d_chrom_result), ctypes.POINTER(xt_twiss_row), _I64,
@@ -487,6 +502,55 @@ def xt_twiss6d(lat: Lattice, guess6=None, stream=None) -> Dict:
     _check(lat._lib, lat._lib.xt_twiss6d(lat.handle, g, ctypes.byref(res), _stream_ptr(stream)))
     return dict(co=np.array(list(res.co)), m=np.array(list(res.m)).reshape(6, 6), q1_frac=res.q1_frac,
                 q2_frac=res.q2_frac, qs=res.qs, iterations=res.iterations)
+
+
+_PLANES = ("x", "y", "z")
+
+
+def _modes6_dict(res: "xt_twiss6d_modes") -> Dict:
+    out = {"stable": int(res.stable), "degenerate": int(res.degenerate)}
+    for k in range(3):
+        out["q%d_frac" % (k + 1)] = res.q_frac[k]
+        raw = np.array(list(res.v[k]))
+        out["v%d" % (k + 1)] = raw[0::2] + 1j * raw[1::2]
+        for u, name in enumerate(_PLANES):
+            out["bet%s%d" % (name, k + 1)] = res.bet[u][k]
+            out["alf%s%d" % (name, k + 1)] = res.alf[u][k]
+    out["dx"], out["dpx"], out["dy"], out["dpy"] = list(res.disp)
+    return out
+
+
+def xt_twiss6d_normal_form(m, rvv_co: float = 1.0, kind: str = "prod") -> Dict:
+    """Normal modes of a 6x6 one-turn matrix in (x, px, y, py, zeta, delta) (host arithmetic only; include/xt.h)."""
+    lib = load_library(kind)
+    a = np.ascontiguousarray(m, dtype=np.float64).reshape(36)
+    res = xt_twiss6d_modes()
+    _check(lib, lib.xt_twiss6d_normal_form(a.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), float(rvv_co),
+                                           ctypes.byref(res)))
+    return _modes6_dict(res)
+
+
+def xt_twiss6d_line(lat: Lattice, guess6=None, stream=None):
+    """(start dict, list of row dicts): the six-dimensional optics carried along the line (include/xt.h)."""
+    n = lat.info["n_elements"] + 1
+    rows = (xt_twiss6d_row * n)()
+    res, modes = xt_twiss6d_result(), xt_twiss6d_modes()
+    g = (ctypes.c_double * 6)(*[float(v) for v in guess6]) if guess6 is not None else None
+    _check(lat._lib, lat._lib.xt_twiss6d_line(lat.handle, g, ctypes.byref(res), ctypes.byref(modes), rows, n,
+                                              _stream_ptr(stream)))
+    start = dict(co=np.array(list(res.co)), m=np.array(list(res.m)).reshape(6, 6), qs=res.qs,
+                 iterations=res.iterations)
+    start.update(_modes6_dict(modes))          # q1_frac .. q3_frac of the normal form (arg(lambda)/2 pi)
+    out = []
+    for r in rows:
+        d = {"s": r.s, "co": np.array(list(r.co)), "dx": r.disp[0], "dpx": r.disp[1], "dy": r.disp[2], "dpy": r.disp[3]}
+        for k in range(3):
+            d["mu%d" % (k + 1)] = r.mu[k]
+            for u, name in enumerate(_PLANES):
+                d["bet%s%d" % (name, k + 1)] = r.bet[u][k]
+                d["alf%s%d" % (name, k + 1)] = r.alf[u][k]
+        out.append(d)
+    return start, out
 
 
 def xt_twiss4d_normal_form(m, kind: str = "prod") -> Dict:

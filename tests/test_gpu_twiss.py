@@ -275,3 +275,102 @@ def test_six_dimensional_twiss(X):
             X.xt_twiss6d(lat)
         assert e.value.code == -5
         lat.close()
+
+
+def test_six_dimensional_normal_form_along_the_line(X):
+    """xt_twiss6d_line (steps 3-5 in six dimensions): (a) the closed forms of pin P24 on the GPU
+    path -- the modes of an uncoupled FODO ring with a cavity are its planes (4-D Courant-Snyder values row by row,
+    kick-slip closed form of the longitudinal mode), the dispersion ring gives the periodic dispersion of the 3x3
+    matrices from the longitudinal eigenvector; (b) the oracle procedure (make_optics.optics6d_along) on every row
+    of a skew-coupled ring with bends and on sampled rows of the LHC-sized configs[2]."""
+    from xt_inputs.packed import Cavity
+    from oracle import oracle as O
+    two_pi = 2 * math.pi
+
+    def phase_close(a, b, tol):
+        d = (a - b) % two_pi
+        return min(d, two_pi - d) < tol
+
+    # (a) uncoupled FODO + cavity
+    p0c = 1.0e9
+    cell = [Multipole(knl=(0.0, 0.1)), Drift(2.0), Multipole(knl=(0.0, -0.095)), Drift(2.0)]
+    els = cell * 10 + [Cavity(1e5, 200e6, 0.0)]
+    buf = pack_lattice(els, p0c, MASS0, 1.0)
+    lat = X.xt_lattice_create(buf)
+    start, rows = X.xt_twiss6d_line(lat)
+    flat_lat = X.xt_lattice_create(pack_lattice(cell * 10, p0c, MASS0, 1.0))
+    _, cols4 = X.xt_twiss4d_line(flat_lat)
+    rows4 = [{k: v[i] for k, v in cols4.items()} for i in range(len(cols4["s"]))]
+    flat_lat.close()
+    lat.close()
+    assert len(rows) == len(els) + 1 and start["stable"] == 1
+    for r6, r4 in zip(rows[:len(cell) * 10 + 1], rows4):
+        assert abs(r6["betx1"] / r4["betx"] - 1) < 5e-6 and abs(r6["bety2"] / r4["bety"] - 1) < 5e-6
+        assert abs(r6["alfx1"] - r4["alfx"]) < 5e-6 and abs(r6["alfy2"] - r4["alfy"]) < 5e-6
+        assert r6["bety1"] < 1e-8 and r6["betx2"] < 1e-8 and r6["betx3"] < 1e-8 and r6["betz1"] < 1e-8
+        assert abs(r6["mu1"] - r4["mux"]) < 5e-6 and abs(r6["mu2"] - r4["muy"]) < 5e-6       # both unwrapped
+    beta0, gamma0 = O.reference(buf)
+    kz = two_pi * 200e6 / (beta0 * 299792458.0)
+    A, B = 40.0 / gamma0 ** 2, (1e5 / p0c) * kz / beta0
+    mu_s = math.acos(1.0 - A * B / 2.0)
+    assert abs(start["betz3"] / (A / math.sin(mu_s)) - 1) < 1e-5
+    assert abs(rows[-1]["mu3"] - mu_s) < 1e-6 and abs(rows[-1]["mu1"] / two_pi - round(rows[-1]["mu1"] / two_pi - start["q1_frac"]) - start["q1_frac"]) < 1e-6
+    # (a) dispersion ring of pin P18 / P24 with a weak cavity
+    th = two_pi / 16
+    bend = Multipole(knl=(th,), hxl=th, length=1.5)
+    dcell = [Multipole(knl=(0.0, 0.25)), Drift(3.0), bend, Drift(3.0), Multipole(knl=(0.0, -0.25)), Drift(3.0), bend, Drift(3.0)]
+    quad = lambda k: np.array([[1.0, 0.0, 0.0], [-k, 1.0, 0.0], [0.0, 0.0, 1.0]])
+    drift = np.array([[1.0, 3.0, 0.0], [0.0, 1.0, 0.0], [0.0, 0.0, 1.0]])
+    dip = np.array([[1.0, 0.0, 0.0], [-th * th / 1.5, 1.0, th], [0.0, 0.0, 1.0]])
+    mats = [quad(0.25), drift, dip, drift, quad(-0.25), drift, dip, drift]
+    m = np.eye(3)
+    for e in mats:
+        m = e @ m
+    d = np.append(np.linalg.solve(np.eye(2) - m[:2, :2], m[:2, 2]), 1.0)
+    lat = X.xt_lattice_create(pack_lattice(dcell * 8 + [Cavity(2e4, 50e6, 180.0)], P0C, MASS0, 1.0))
+    start, rows = X.xt_twiss6d_line(lat)
+    lat.close()
+    for i in range(9):
+        assert abs(rows[i]["dx"] / d[0] - 1.0) < 3e-4 and abs(rows[i]["dpx"] - d[1]) < 3e-4 * max(abs(d[1]), 0.1), i
+        assert abs(rows[i]["dy"]) < 1e-6
+        if i < 8:
+            d = mats[i] @ d
+    # (b) oracle procedure: a skew-coupled ring with curved dipoles, every row
+    ks = [Multipole(knl=(0.0, 0.0), ksl=(0.0, 0.03))]
+    coupled = (ks + dcell) * 8 + [Cavity(2e5, 100e6, 180.0)]
+    want_on, want = MO.optics6d_along(coupled, P0C, MASS0, 1.0, list(range(len(coupled) + 1)))
+    lat = X.xt_lattice_create(pack_lattice(coupled, P0C, MASS0, 1.0))
+    start, rows = X.xt_twiss6d_line(lat)
+    lat.close()
+    assert want_on["bety1"] > 1e-3 * want_on["betx1"]                                      # really coupled
+    scale = max(want_on["betx1"], want_on["bety2"])
+    for k in ("q1_frac", "q2_frac", "q3_frac"):
+        assert abs(start[k] - want_on[k]) < 1e-7, k
+    for r, w in zip(rows, want):
+        np.testing.assert_allclose(r["co"], w["co"], atol=1e-9)
+        for mode in (1, 2, 3):
+            for pl in ("x", "y"):
+                assert abs(r["bet%s%d" % (pl, mode)] - w["bet%s%d" % (pl, mode)]) < 2e-5 * scale
+                assert abs(r["alf%s%d" % (pl, mode)] - w["alf%s%d" % (pl, mode)]) < 2e-5 * max(1.0, scale / 10)
+            sense = -1.0 if (mode == 3 and start["q3_frac"] > 0.5) else 1.0
+            assert phase_close(sense * r["mu%d" % mode], w["mu%d" % mode], 2e-5), (mode, r["mu%d" % mode], w["mu%d" % mode])
+        assert abs(r["betz3"] / w["betz3"] - 1) < 1e-4
+        for k in ("dx", "dpx", "dy", "dpy"):
+            assert abs(r[k] - w[k]) < 1e-4 * max(1.0, abs(w[k])), (k, r[k], w[k])
+    # (b) configs[2], sampled rows
+    els2 = C.lattice(2)
+    sample = [0, 1, 7, 200, 1234, 4321, len(els2) - 3, len(els2)]
+    want_on, want = MO.optics6d_along(els2, P0C, MASS0, 1.0, sample)
+    lat = X.xt_lattice_create(C.pack(els2))
+    start, rows = X.xt_twiss6d_line(lat)
+    lat.close()
+    scale = max(want_on["betx1"], want_on["bety2"])
+    for i, w in zip(sample, want):
+        r = rows[i]
+        np.testing.assert_allclose(r["co"][:4], w["co"][:4], atol=1e-9)
+        for key in ("betx1", "bety1", "betx2", "bety2"):
+            assert abs(r[key] - w[key]) < 1e-4 * scale, (i, key, r[key], w[key])
+        for key in ("dx", "dy"):
+            assert abs(r[key] - w[key]) < 2e-3 * max(1.0, abs(w[key])), (i, key, r[key], w[key])
+    print("configs[2] 6-D: q = %.6f %.6f %.6f, betx1 %.2f bety2 %.2f betz3 %.1f, dx %.4f at the start"
+          % (start["q1_frac"], start["q2_frac"], start["q3_frac"], start["betx1"], start["bety2"], start["betz3"], start["dx"]))

@@ -425,6 +425,46 @@ def test_normal_form_matches_the_oracle_eigen_decomposition():
     assert X.load_library("prod").xt_twiss4d_normal_form(None, None) == -1
 
 
+def test_normal_form6_matches_the_oracle_eigen_decomposition():
+    """xt_twiss6d_normal_form (host arithmetic: cubic in u = lambda + 1/lambda, projector eigenvectors) against
+    oracle/make_optics.normal_form6 (numpy.linalg.eig) on 6x6 matrices the oracle tracker produced: a FODO ring
+    with a cavity, the same seen from a rotated frame, and the dispersion ring of pin P24 (synchrotron tune
+    1e-4: the longitudinal pair sits 5e-7 from u = 2, where the two methods split the 1e-6 asymplecticity of a
+    central-difference matrix differently)."""
+    from oracle import make_optics as MO
+    from xt_inputs.packed import Cavity, SRotation
+    cell = [Multipole(knl=(0.0, 0.1)), Drift(2.0), Multipole(knl=(0.0, -0.095)), Drift(2.0)]
+    fodo = cell * 10 + [Cavity(1e5, 200e6, 0.0)]
+    rot = [SRotation.from_angle(-0.3)] + fodo + [SRotation.from_angle(0.3)]
+    th = 2.0 * np.pi / 16
+    bend = Multipole(knl=(th,), hxl=th, length=1.5)
+    ring = [Multipole(knl=(0.0, 0.25)), Drift(3.0), bend, Drift(3.0), Multipole(knl=(0.0, -0.25)), Drift(3.0), bend,
+            Drift(3.0)] * 8 + [Cavity(2e4, 50e6, 180.0)]
+    for els, p0c, tol in ((fodo, 1e9, 2e-8), (rot, 1e9, 2e-8), (ring, P0C, 1e-4)):
+        m = MO.optics6d_of(pack_lattice(els, p0c, MASS0, 1.0))["m"]
+        want, got = MO.normal_form6(m, 1.0), X.xt_twiss6d_normal_form(m, 1.0)
+        assert got["stable"] == 1 and got["degenerate"] == 0
+        for k, w in want.items():
+            if k.startswith("v"):
+                assert np.max(np.abs(got[k] - w)) < tol * np.max(np.abs(w)), k
+            elif k.startswith("q"):
+                assert abs(got[k] - w) < tol, (k, got[k], w)
+            else:
+                scale = max(abs(want["betx1"]), abs(want["bety2"])) if k[:3] in ("bet", "alf") and k[3] != "z" else 1.0
+                assert abs(got[k] - w) < tol * max(abs(w), scale), (k, got[k], w)
+    # rvv_co rescales the longitudinal momentum only: beta_z3 scales by 1/rvv (zeta per unit pzeta)
+    a, b = X.xt_twiss6d_normal_form(m, 1.0), X.xt_twiss6d_normal_form(m, 1.0 + 1e-3)
+    assert abs(b["q3_frac"] - a["q3_frac"]) < 1e-12 and abs(b["betx1"] / a["betx1"] - 1) < 1e-9
+    assert abs(b["betz3"] / a["betz3"] * (1.0 + 1e-3) - 1.0) < 1e-6
+    bad = np.eye(6)
+    bad[0, 0], bad[1, 1] = 2.0, 0.5
+    got = X.xt_twiss6d_normal_form(bad)
+    assert got["stable"] == 0 and np.isnan(got["q1_frac"])
+    assert X.load_library("prod").xt_twiss6d_normal_form(None, 1.0, None) == -1
+    assert ctypes.sizeof(B.xt_twiss6d_modes) == 8 * (3 + 9 + 9 + 4 + 36) + 8
+    assert ctypes.sizeof(B.xt_twiss6d_row) == 8 * (1 + 6 + 9 + 9 + 3 + 4)
+
+
 def test_radiating_multipole_is_packed_unfused():
     from xt_inputs.packed import RadMultipole
     els = [Drift(1.0), RadMultipole(knl=(2e-3, 0.1, 6.0), ksl=(0.0, 0.01), hxl=1.5e-3, length=4.0), Drift(1.0)]
