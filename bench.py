@@ -74,7 +74,7 @@ def flops_per_particle_turn(info: dict, table: dict) -> float:
     if "drift" in table:
         drifts = t[1] * table["drift"]
     else:
-        drifts = t[1] * table["drift_apply"] + info["n_drift_evals"] * table["drift_eval"]
+        drifts = info.get("n_drift_applies", t[1]) * table["drift_apply"] + info["n_drift_evals"] * table["drift_eval"]
     thick = info.get("n_thick_quad", 0) * table.get("thick_quad", 0) + info.get("n_thick_bend", 0) * table.get("thick_bend", 0)
     return (drifts + n_mult * table["mult_base"] + info["sum_order"] * table["mult_per_order"]
             + info["n_curved"] * table["curved_extra"] + t[3] * table["cavity"] + t[4] * table["srot"]

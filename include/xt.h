@@ -146,6 +146,10 @@ typedef struct {
   int64_t n_drift_evals;    /* sqrt evaluations per turn after fusion (consecutive drifts     */
                             /* share one; equals the number of drifts when fuse is off)       */
   int64_t n_thick;          /* thick elements (XT_QUADRUPOLE, XT_BEND); not in n_by_type      */
+  int64_t n_drift_applies;  /* drift applications per turn: the number of drifts, minus what   */
+                            /* the production build saves by applying consecutive drifts as    */
+                            /* one drift of the summed length (exact composition; the          */
+                            /* validation build applies every drift)                           */
 } xt_lattice_info;
 
 /* Options of xt_lattice_create_ex.  Zero-initialise for the defaults.  Neither changes any

@@ -111,7 +111,8 @@ class xt_lattice_info(ctypes.Structure):
                 ("sum_order", ctypes.c_int64), ("n_curved", ctypes.c_int64),
                 ("has_aperture", ctypes.c_int64), ("beta0", ctypes.c_double),
                 ("gamma0", ctypes.c_double), ("circumference", ctypes.c_double),
-                ("n_drift_evals", ctypes.c_int64), ("n_thick", ctypes.c_int64)]
+                ("n_drift_evals", ctypes.c_int64), ("n_thick", ctypes.c_int64),
+                ("n_drift_applies", ctypes.c_int64)]
 
     def as_dict(self) -> Dict:
         d = {k: getattr(self, k) for k, _ in self._fields_ if k != "n_by_type"}

@@ -171,6 +171,7 @@ struct HostImage {
 struct PackOpts {
   uint32_t chunk_bytes = kDefaultChunkBytes;
   bool fuse = true;
+  bool merge_drifts = true;    // production build: consecutive drifts -> one drift of the summed length (pass 1b)
   bool allow_monitor = false;  // accept the internal element type kMonitorType (xt_twiss4d_line builds such lines)
 };
 constexpr uint32_t kMonitorType = 11;  // packed-buffer type id, internal: {row} -> TAG_MON record

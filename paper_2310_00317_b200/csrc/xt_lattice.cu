@@ -339,6 +339,28 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
   }
   info.circumference = s_pos;
 
+  // ---- pass 1b (production build only): consecutive drifts become ONE drift of the summed length.  px, py
+  // and delta do not change in a drift, so D(l1) D(l2) = D(l1 + l2) exactly; what differs is one rounding
+  // of x, y, zeta instead of two.  The validation build (--fmad=false) keeps every drift, as the oracle
+  // does, and stays bit-identical to it.  Done before (and whether or not) records are fused, so that the
+  // production results do not depend on the fusion option.
+  info.n_drift_applies = info.n_by_type[XT_DRIFT];
+#ifndef XT_FMAD_OFF
+  if (opts.merge_drifts) {
+    std::vector<Rec> merged;
+    merged.reserve(recs.size());
+    for (Rec &rec : recs) {
+      if (rec.type == TAG_DRIFT && !merged.empty() && merged.back().type == TAG_DRIFT) {
+        merged.back().p0 = merged.back().p0 + rec.p0;
+        info.n_drift_applies -= 1;
+      } else {
+        merged.push_back(std::move(rec));
+      }
+    }
+    recs.swap(merged);
+  }
+#endif
+
   // ---- pass 2: fuse.  A thin lattice is mostly drift - kick - drift, with
   // misaligned magnets wrapped in XYShift / SRotation.  A fused record applies
   // the same maps in the same order with the same arithmetic; what is shared is the dispatch

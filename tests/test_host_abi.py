@@ -58,7 +58,7 @@ def test_struct_layouts_match_the_header():
     assert ctypes.sizeof(B.xt_track_opts) == 56          # + workspace ptr, bytes, stats ptr, cold_in_registers
     assert ctypes.sizeof(B.xt_track_stats) == 7 * 8 + 3 * 8 * B.XT_STATS_MAX_PASSES
     assert ctypes.sizeof(B.xt_lattice_opts) == 16
-    assert ctypes.sizeof(B.xt_lattice_info) == 8 * (5 + 8 + 3) + 8 * 3 + 8 + 8
+    assert ctypes.sizeof(B.xt_lattice_info) == 8 * (5 + 8 + 3) + 8 * 3 + 8 + 8 + 8
 
 
 def test_compute_calls_validate_arguments_without_a_device():
@@ -217,10 +217,23 @@ ALL_TYPES = [Drift(1.5), XYShift(1e-4, -2e-4), SRotation.from_angle(1e-3),
 
 
 # ------------------------------------------------------------------------ step P
+def merge_drifts(maps):
+    """What the PRODUCTION packer encodes: consecutive drifts as one drift of the summed length (exact
+    composition; the validation build keeps every drift)."""
+    out = []
+    for m in maps:
+        if m[0] == "drift" and out and out[-1][0] == "drift":
+            out[-1] = ("drift", out[-1][1] + m[1])
+        else:
+            out.append(m)
+    return out
+
+
+@pytest.mark.parametrize("kind", ["nofma", "prod"])
 @pytest.mark.parametrize("fuse", [True, False])
-def test_packer_encodes_every_map_in_order_with_prescaled_coefficients(fuse):
+def test_packer_encodes_every_map_in_order_with_prescaled_coefficients(fuse, kind):
     buf = pack(ALL_TYPES)
-    img, info = X.xt_lattice_pack_host(buf, fuse=fuse)
+    img, info = X.xt_lattice_pack_host(buf, kind=kind, fuse=fuse)
     assert info["n_elements"] == len(ALL_TYPES) and info["image_bytes"] == len(img)
     assert info["n_by_type"] == [1, 8, 4, 1, 2, 2, 1, 1]
     assert info["sum_order"] == 3 + 1 + 2 + 0 and info["n_curved"] == 2 and info["has_aperture"] == 1
@@ -230,18 +243,25 @@ def test_packer_encodes_every_map_in_order_with_prescaled_coefficients(fuse):
     chunks = walk_image(img, info["chunk_bytes"])
     assert len(chunks) == info["n_chunks"] == 1
     assert sum(len(c) for c in chunks) == info["n_records"]
-    assert_same_maps(all_maps(img, info["chunk_bytes"]), expected_maps(ALL_TYPES, info["beta0"]))
+    want = expected_maps(ALL_TYPES, info["beta0"])
+    merged = kind == "prod"
+    assert_same_maps(all_maps(img, info["chunk_bytes"]), merge_drifts(want) if merged else want)
+    assert info["n_drift_applies"] == (5 if merged else 8)          # [0.25 0.75] and [3.0 0.5 0.125] become one each
     if fuse:
         # [D shift rot M rot shift D D], cavity, D, rect, [D M + ellipse], [M D D], [D M]
         assert info["n_records"] == 7
         assert chunks[0][4][1] == (F_PRE | F_APER)
         first = chunks[0][0]
-        assert first[0] == T_CMULT and first[1] == (F_PRE | F_POST | F_POST2 | F_MISAL) and first[3] == 3
-        assert info["n_drift_evals"] == 2 + 1 + 1 + 1 + 1           # pre + post, D, [D M], [M D D], [D M]
-    else:
+        flags = F_PRE | F_POST | F_MISAL | (0 if merged else F_POST2)
+        assert first[0] == T_CMULT and first[1] == flags and first[3] == 3
+        # pre + post, D, [D M], [M D D], [D M]; merged: the last three drifts are one, behind the first of the two magnets
+        assert info["n_drift_evals"] == (2 + 1 + 1 + 1 + 0 if merged else 2 + 1 + 1 + 1 + 1)
+    elif not merged:
         assert info["n_records"] == len(ALL_TYPES) - 1             # the marker has no record
         assert info["n_drift_evals"] == 8
         assert [r[3] for r in chunks[0]] == [i for i, e in enumerate(ALL_TYPES) if not isinstance(e, Marker)]
+    else:
+        assert info["n_records"] == len(ALL_TYPES) - 1 - 3 and info["n_drift_evals"] == 5
 
 
 def test_cavity_and_aperture_constants():
@@ -257,17 +277,21 @@ def test_cavity_and_aperture_constants():
     assert ell[4] == a2 * b2 and ell[5][:2] == (b2, a2) and ell[3] == 1
 
 
+@pytest.mark.parametrize("kind", ["nofma", "prod"])
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3])
-def test_config_lattices_chunking_and_fusion(cfg):
+def test_config_lattices_chunking_and_fusion(cfg, kind):
     els = C.lattice(cfg)
     buf = C.pack(els)
-    img, info = X.xt_lattice_pack_host(buf)
+    img, info = X.xt_lattice_pack_host(buf, kind=kind)
     want = expected_maps(els, info["beta0"])
-    assert_same_maps(all_maps(img, info["chunk_bytes"]), want)
     n_drifts = sum(1 for m in want if m[0] == "drift")
+    if kind == "prod":
+        want = merge_drifts(want)
+    assert_same_maps(all_maps(img, info["chunk_bytes"]), want)
     assert info["n_by_type"][1] == n_drifts and info["n_drift_evals"] <= n_drifts
+    assert info["n_drift_applies"] == sum(1 for m in want if m[0] == "drift")
     for kw in (dict(fuse=False), dict(chunk_bytes=1024), dict(chunk_bytes=65536, fuse=False)):
-        img2, info2 = X.xt_lattice_pack_host(buf, **kw)
+        img2, info2 = X.xt_lattice_pack_host(buf, kind=kind, **kw)
         assert info2["chunk_bytes"] == kw.get("chunk_bytes", 8192)
         chunks = walk_image(img2, info2["chunk_bytes"])
         assert len(chunks) == info2["n_chunks"] and sum(len(c) for c in chunks) == info2["n_records"]
@@ -276,6 +300,8 @@ def test_config_lattices_chunking_and_fusion(cfg):
     if cfg >= 2:                                             # multi-chunk, mostly fused
         assert info["n_chunks"] > 40 and info["n_records"] < 0.5 * info["n_elements"]
         assert info["n_drift_evals"] < 0.65 * n_drifts
+        if kind == "prod":                                   # [D M D][D M D]: every interior pair of drifts is one
+            assert info["n_drift_applies"] < 0.56 * n_drifts
 
 
 def test_empty_and_marker_only_lattices():
