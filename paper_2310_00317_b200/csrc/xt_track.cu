@@ -127,6 +127,20 @@ struct Prefetched {  // ... of which this many really are (the rest is read wher
   static constexpr int value = REG ? kPrefetch : (P >= 4 ? XT_PF4 : (P == 3 ? XT_PF3 : kPrefetch));
 };
 
+// Which flag sets beyond {none, POST} have specialised multipole handlers in the production build:
+// -1: not even the flag-less one, 0: none, 1: PRE+POST, 2: PRE+POST and PRE.  (A case label moved to an impossible key -- order bits that
+// cannot occur -- drops its handler from the instantiation.)
+#ifndef XT_SET_P4
+#define XT_SET_P4 0
+#endif
+#ifndef XT_SET_P3
+#define XT_SET_P3 1
+#endif
+template <int P, bool REG>
+struct HandlerSet {
+  static constexpr int value = P >= 4 ? XT_SET_P4 : XT_SET_P3;
+};
+
 // Hot per-thread state of P particles: what drifts and kicks touch at every element.
 template <int P>
 struct Parts {
@@ -806,10 +820,23 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
   case TAG_CMULT | (F) | ((N) << 8):                                           \
     multipole_record<P, (F), 1, (NT)>(q, cold, slots, pf, tag, p0);            \
     break;
+      // The flag sets a drift-kick-drift lattice produces.  In the validation build every drift arrives on its
+      // own (POST2 records); in the production build consecutive drifts arrive merged, and which of the
+      // remaining sets get a specialised handler is a per-shape choice measured on configs[2] / [3]
+      // (profiles/r02_shape_sweep.md): every extra handler lengthens the dispatch and the code.
+#ifdef XT_FMAD_OFF
       XT_MULT_CASE(0u, kOrd, kOrdT)
+#else
+      XT_MULT_CASE((HandlerSet<P, ColdT::kInRegs>::value >= 0 ? 0u : 0x7000u), kOrd, kOrdT)
+#endif
       XT_MULT_CASE(TAG_POST, kOrd, kOrdT)
+#ifdef XT_FMAD_OFF
       XT_MULT_CASE(TAG_POST | TAG_POST2, kOrd, kOrdT)
       XT_MULT_CASE(TAG_PRE | TAG_POST | TAG_POST2, kOrd, kOrdT)
+#else
+      XT_MULT_CASE(TAG_PRE | TAG_POST | (HandlerSet<P, ColdT::kInRegs>::value >= 1 ? 0u : 0x7000u), kOrd, kOrdT)
+      XT_MULT_CASE(TAG_PRE | (HandlerSet<P, ColdT::kInRegs>::value >= 2 ? 0u : 0x7000u), kOrd, kOrdT)
+#endif
 #undef XT_MULT_CASE
       case TAG_CAVITY: {
         const double2 kv = pf[0];  // (kz, vn)
