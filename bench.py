@@ -392,6 +392,8 @@ def main():
                                       n_sm, sm_max_hz),
         }
         line["roofline"]["kernel_ms_steps"] = r["kernel_ms_steps"]
+        if cfg == 4:      # with compaction the retired slots are not tracked at all: "every slot of the launch" has no meaning
+            line["roofline"]["frac_all_slots"] = None
         # DRAM bytes of one launch: not measurable inside the run (needs ncu); the number is the --set full
         # capture's dram__bytes_read + dram__bytes_write per particle scaled to this launch
         line["roofline"]["traffic"] = 76.9 * n_part if cfg == 3 else None
