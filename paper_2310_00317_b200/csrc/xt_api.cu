@@ -50,12 +50,13 @@ int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p
 // Launch shape of the tracking kernel: threads per CTA, particles per thread, and where the cold
 // per-particle state lives.  Auto rule (measured on B200, profiles/r02_shape_sweep.md): 128-thread CTAs.
 // Several waves of particles (>= 4096 per SM, configs[3]): 4 per thread, cold state in shared memory,
-// 4 CTAs per SM at <= 128 registers.  Ensembles that fit the SMs in one wave of two CTAs
-// (<= 768 per SM, configs[2]: 676): 3 per thread with the cold state in registers -- the register file
-// is half empty there and every LDS taken out of a record shortens what a warp waits for.  In
-// between: 3 per thread, cold state in shared memory.  Below ~100 particles per SM one per thread keeps
-// more warps alive.  The kernel hands the particles out in equal shares over a whole number of CTAs
-// per SM, so the shape only has to make enough CTAs.
+// 4 CTAs per SM at <= 128 registers.  Ensembles that fit the SMs in one wave (<= 768 per SM, configs[2]:
+// 676): 2 per thread with the cold state in registers -- the register file is half empty there, every LDS
+// taken out of a record shortens what a warp waits for, and three warps of two particles per scheduler
+// cover each other's latencies better than two warps of three (0.524 against 0.511).  In between: 3 per
+// thread, cold state in shared memory.  Below ~100 particles per SM one per thread keeps more warps
+// alive.  The kernel hands the particles out in equal shares over a whole number of CTAs per SM, so the
+// shape only has to make enough CTAs.
 struct Shape {
   int block, ppt;
   bool cold_in_regs;
@@ -64,6 +65,7 @@ int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part,
   const int64_t per_sm = n_part / (lat->n_sm > 0 ? lat->n_sm : 1);
   int auto_ppt = 4, auto_block = 128;
   if (per_sm < 4096) auto_ppt = 3;
+  if (per_sm <= 768) auto_ppt = 2;
   if (per_sm < 96) {
     auto_ppt = 1;
     auto_block = 32;
@@ -76,13 +78,13 @@ int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part,
   else if (want_regs < 0)
     sh->cold_in_regs = false;
   else
-    sh->cold_in_regs = (sh->ppt == 3 && per_sm >= 96 && per_sm <= 768);
+    sh->cold_in_regs = (sh->ppt <= 3 && per_sm >= 96 && per_sm <= 768);
   if (sh->ppt < 1 || sh->ppt > 4) {
     set_error("xt_track_ex: particles_per_thread must be 0 (auto), 1, 2, 3 or 4");
     return XT_ERR_INVALID_ARG;
   }
-  if (sh->cold_in_regs && sh->ppt != 3) {
-    set_error("xt_track_ex: cold_in_registers needs 3 particles per thread");
+  if (sh->cold_in_regs && sh->ppt > 3) {
+    set_error("xt_track_ex: cold_in_registers needs 1, 2 or 3 particles per thread");
     return XT_ERR_INVALID_ARG;
   }
   if (sh->block < 32 || sh->block > 256 || (sh->block % 32) != 0) {

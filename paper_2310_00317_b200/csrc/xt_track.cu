@@ -136,9 +136,12 @@ struct Prefetched {  // ... of which this many really are (the rest is read wher
 #ifndef XT_SET_P3
 #define XT_SET_P3 1
 #endif
+#ifndef XT_SET_P2
+#define XT_SET_P2 1
+#endif
 template <int P, bool REG>
 struct HandlerSet {
-  static constexpr int value = P >= 4 ? XT_SET_P4 : XT_SET_P3;
+  static constexpr int value = P >= 4 ? XT_SET_P4 : (P == 3 ? XT_SET_P3 : XT_SET_P2);
 };
 
 // Hot per-thread state of P particles: what drifts and kicks touch at every element.
@@ -930,7 +933,7 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
 // state (at 64 / 80 registers they spilled ~100 values around every call).
 template <int P, bool REG, bool THICK>
 struct RegBudget {
-  static constexpr int value = REG ? (P == 3 ? XT_REGS3R : 255)
+  static constexpr int value = REG ? (P == 3 ? XT_REGS3R : (P == 2 ? 168 : 96))
                                    : (P == 1 ? (THICK ? 96 : 64) : (P == 2 ? (THICK ? 128 : 80) : (P == 3 ? XT_REGS3 : XT_REGS4)));
 };
 
@@ -1157,8 +1160,9 @@ int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaSt
 constexpr int kFixedOrder = 15;
 template <int P, bool REG>
 int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
-  if (P >= 3 && lat->fixed_order == kFixedOrder) {
-    constexpr int NF = P >= 3 ? kFixedOrder : 0;
+  constexpr bool kHasFixed = (P >= 3) || REG;  // which shapes exist with the unrolled order-15 handlers
+  if (kHasFixed && lat->fixed_order == kFixedOrder) {
+    constexpr int NF = kHasFixed ? kFixedOrder : 0;
     return lat->extended ? launch_track_pt<P, true, REG, NF>(a, lat, block, st)
                          : launch_track_pt<P, false, REG, NF>(a, lat, block, st);
   }
@@ -1189,8 +1193,10 @@ int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, c
   a.tib = lat->k.tib;
   a.igam2 = lat->k.igam2;
   if (cold_in_regs) {
+    if (ppt == 1) return launch_track_p<1, true>(a, lat, block, st);
+    if (ppt == 2) return launch_track_p<2, true>(a, lat, block, st);
     if (ppt == 3) return launch_track_p<3, true>(a, lat, block, st);
-    set_error("xt_track: cold_in_registers needs 3 particles per thread");
+    set_error("xt_track: cold_in_registers needs 1, 2 or 3 particles per thread");
     return XT_ERR_INVALID_ARG;
   }
   switch (ppt) {

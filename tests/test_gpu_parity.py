@@ -286,7 +286,7 @@ def test_launch_shape_fusion_and_chunk_size_do_not_change_results(X):
             p = X.new_particles(lat, coords)
             X.xt_track_ex(lat, p, 6, compact_every=-1, block_size=block, particles_per_thread=ppt)
             assert_bit_identical(X.particles_to_host(p), base)
-    for ppt, cold in ((3, 1), (2, -1), (3, -1)):      # cold per-particle state in registers / shared memory
+    for ppt, cold in ((1, 1), (2, 1), (3, 1), (2, -1), (3, -1)):      # cold per-particle state in registers / shared memory
         p = X.new_particles(lat, coords)
         X.xt_track_ex(lat, p, 6, compact_every=-1, block_size=64, particles_per_thread=ppt, cold_in_registers=cold)
         assert_bit_identical(X.particles_to_host(p), base)
