@@ -31,16 +31,21 @@ namespace xt {
 // follows it and vice versa (TAG_POST: second slot).  The maps are applied in element order
 // with unchanged arithmetic; the dispatch is shared, and so is what two consecutive drifts
 // would both compute from the unchanged (px, py).  Slots of a multipole record, in order:
-//   the N+1 coefficient pairs (the kernel prefetches the first slots behind every header);
-//   {wf, 0} if TAG_CMULT; {l_pre, l_post} if PRE|POST; {l_post2, 0} if POST2;
-//   {dx, dy}, {cos, sin}, {cos', sin'}, {dx', dy'} if MISAL.
+//   {l_pre, l_post}; {l_post2, wf}   -- always present (zero where unused), so that every slot of the
+//                                       record sits at an offset the handlers know at compile time;
+//   {dx, dy}, {cos, sin}, {cos', sin'}, {dx', dy'} if MISAL;
+//   the N+1 coefficient pairs (c[n], s[n]), n = N .. 0 (Horner order).
+// The kernel loads the first four slots behind every header before the dispatch resolves: the extras
+// and, without misalignment, the two leading pairs.
+// In the production build consecutive drifts reach the fusion pass already merged into one drift of the
+// summed length (xt_lattice.cu pass 1b), so TAG_POST2 only occurs in the validation build.
 // A multipole or drift record may also end with the LimitEllipse that follows it (TAG_APER):
 // its last two slots are then {b2, a2}, {a2*b2, element index of the aperture}.
 // Unfused records:
 //
 //   TAG_DRIFT    p0 = length; {l_2nd, 0} with TAG_POST                           16 B (32 B)
-//   TAG_MULT     p0 unused; (c[n], s[n]) pairs, n = N .. 0 (Horner order)        16 + 16(N+1)
-//   TAG_CMULT    p0 = hxl;  pairs as above (c[0] = knl[0] - hxl); {wf, 0}         32 + 16(N+1)
+//   TAG_MULT     p0 unused; two extras slots; (c[n], s[n]) pairs, n = N .. 0     48 + 16(N+1)
+//   TAG_CMULT    p0 = hxl;  as above with c[0] = knl[0] - hxl and wf in the extras 48 + 16(N+1)
 //   TAG_CAVITY   p0 = lag_rad; {kz, vn}                                          32 B
 //   TAG_SROT     p0 unused; {cos_z, sin_z}                                       32 B
 //   TAG_SHIFT    p0 unused; {dx, dy}                                             32 B

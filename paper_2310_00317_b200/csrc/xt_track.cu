@@ -9,22 +9,32 @@
 // streamed chunk by chunk from L2 into shared memory with 1-D TMA bulk copies
 // (cp.async.bulk + mbarrier complete_tx), double-buffered; every thread of the CTA reads the
 // same record, so each LDS.128 is a broadcast.  Dispatch is a switch on a value all lanes
-// share (warp-uniform); a record is usually a fused [drift] kick [drift drift] group
+// share (warp-uniform); a record is usually a fused [drift] kick [drift] group
 // (xt_internal.h).  Multipoles are a complex Horner recurrence of FMAs.
+//
+// Instantiations xt_track_kernel<P, THICK, REG, NFIX>: P particles per thread; THICK = the extended
+// maps (thick elements, polygons, radiation, monitors) compiled in; REG = the cold per-particle state
+// (functions of delta, ptau) in registers instead of shared memory (small ensembles); NFIX = 15: the
+// handlers of order-15 multipoles fully unrolled (lattices the packer finds full of them).
 //
 // Why P > 1 (profiles/r01b_track_p1_summary.md): with one particle per thread 58 % of the
 // issued warp instructions were not FP64 (dispatch, LDS, branches, the slow-path guards of
 // sqrt and /) and the FP64 pipe sat at 49 %.  P particles per thread share every one of those
 // instructions and give each warp P independent FP64 chains.
 //
+// What bounds it (profiles/r02_dfma_peak_sweep.md): an FP64 instruction costs max(2, number of
+// vector-register source operands) cycles of its scheduler's FP64 pipe, and nearly every DFMA of this
+// arithmetic has three (re x + t; x += px lpz; c - im y with c loaded from shared memory).
+//
 // Arithmetic.  The maps are written in the canonical order of DESIGN.md section 5 through
 // XT_MADD / XT_NMADD / XT_MUL.  The validation build (--fmad=false, XT_FMAD_OFF) evaluates
 // exactly those trees with IEEE sqrt and division and is bit-identical to the oracle on
 // cavity-free lattices.  The production build fuses every a*b + c into one DFMA (explicitly,
-// so that results do not depend on the launch shape) and replaces the drift's sqrt + division
+// so that results do not depend on the launch shape), replaces the drift's sqrt + division
 // by branch-free Newton sequences on the MUFU.RSQ64H / MUFU.RCP64H seeds (DESIGN.md section
-// 6.3): same formula, <= 2 ulp on the increments; the measured distance to the oracle is set by
-// FMA fusion, not by this block (<= 0.5 of the 1e-12 bar either way).
+// 6.3: same formula, <= 2 ulp on the increments) and receives consecutive drifts merged into one
+// (xt_lattice.cu pass 1b); the measured distance to the oracle is set by FMA fusion (<= 0.2 of the
+// 1e-12 bar in x, y; 0.03 in zeta).
 #include <atomic>
 
 #include "xt_internal.h"
