@@ -509,7 +509,21 @@ __device__ XT_THICK_INLINE Hot thick_quadrupole_one(Hot h, const double delta, c
   const double wl = XT_MUL(w, length);
   double sn, cs;
   sincos(wl, &sn, &cs);
+#ifdef XT_FMAD_OFF
   const double ch = cosh(wl), sh = sinh(wl);
+  const double h2w = 0.5 / w;
+#define XT_OVER_W(a) ((a) / w)
+#else
+  // production: cosh and sinh from one expm1 (wl >= 0; sinh = (e - 1 + (e - 1)/e)/2 keeps its accuracy for
+  // small arguments), and the divisions by w as multiplications by 1/w: ~2 ulp, far inside the 1e-12 bar
+  const double em1 = expm1(wl);
+  const double ep = em1 + 1.0;
+  const double en = 1.0 / ep;
+  const double ch = XT_MUL(0.5, ep + en), sh = XT_MUL(0.5, fma(em1, en, em1));
+  const double rw = 1.0 / w;
+  const double h2w = XT_MUL(0.5, rw);
+#define XT_OVER_W(a) XT_MUL((a), rw)
+#endif
   const double ow = XT_MUL(opd, w);
   const double iw = 1.0 / ow;
   const bool focus_x = rk > 0.0;
@@ -522,12 +536,12 @@ __device__ XT_THICK_INLINE Hot thick_quadrupole_one(Hot h, const double delta, c
   const double v1 = XT_MADD(v, ch, XT_MUL(XT_MUL(pv, iw), sh));
   const double pv1 = XT_MADD(pv, ch, XT_MUL(av, sh));
   const double hl = XT_MUL(0.5, length);
-  const double h2w = 0.5 / w;
   const double pu2 = XT_MUL(pu, pu), au2 = XT_MUL(au, au), pv2 = XT_MUL(pv, pv), av2 = XT_MUL(av, av);
   const double i_f = XT_MADD(pu2 + au2, hl, XT_MUL(XT_MUL(pu2 - au2, XT_MUL(sn, cs)), h2w)) -
-                     XT_MUL(XT_MUL(au, pu), XT_MUL(sn, sn)) / w;
+                     XT_OVER_W(XT_MUL(XT_MUL(au, pu), XT_MUL(sn, sn)));
   const double i_d = XT_MADD(pv2 - av2, hl, XT_MUL(XT_MUL(pv2 + av2, XT_MUL(sh, ch)), h2w)) +
-                     XT_MUL(XT_MUL(av, pv), XT_MUL(sh, sh)) / w;
+                     XT_OVER_W(XT_MUL(XT_MUL(av, pv), XT_MUL(sh, sh)));
+#undef XT_OVER_W
   const double slip = XT_MUL(length, g / XT_MUL(opd, opd + b));
   Hot o;
   o.zeta = (h.zeta + slip) - XT_MUL(rv0v / XT_MUL(2.0, opd2), i_f + i_d);
@@ -540,7 +554,8 @@ __device__ XT_THICK_INLINE Hot thick_quadrupole_one(Hot h, const double delta, c
 
 // Thick sector bend, 'expanded' model (reading A19):
 // the exact flow of H = (px^2 + py^2)/(2(1+delta)) - h x (1+delta) + k0 x + (k0 h/2) x^2, i.e. the
-// thin curved multipole of step M2 smeared over the arc length.  Same arithmetic as the oracle's.
+// thin curved multipole of step M2 smeared over the arc length.  The validation build evaluates the oracle's
+// expression tree; the production build multiplies by reciprocals where that tree divides repeatedly.
 __device__ XT_THICK_INLINE Hot thick_bend_one(Hot p, const double delta, const double opd2, const double b,
                                            const double g, const double rv, const double k0, const double h,
                                            const double length) {
@@ -551,16 +566,29 @@ __device__ XT_THICK_INLINE Hot thick_bend_one(Hot p, const double delta, const d
   sincos(wl, &sn, &cs);
   const double c1 = 1.0 - cs;
   const double ow = XT_MUL(opd, w);
-  const double fw = XT_NMADD(1.0, k0, XT_MUL(h, opd)) / w;  // (h (1+delta) - k0)/w
+#ifdef XT_FMAD_OFF
+#define XT_OVER_W(a) ((a) / w)
+#define XT_OVER_OW(a) ((a) / ow)
+  const double h2w = 0.5 / w;
+#else
+  // production: the nine divisions by w and by (1+delta) w as multiplications by two reciprocals (~2 ulp)
+  const double rw = 1.0 / w, row = 1.0 / ow;
+#define XT_OVER_W(a) XT_MUL((a), rw)
+#define XT_OVER_OW(a) XT_MUL((a), row)
+  const double h2w = XT_MUL(0.5, rw);
+#endif
+  const double fw = XT_OVER_W(XT_NMADD(1.0, k0, XT_MUL(h, opd)));  // (h (1+delta) - k0)/w
   const double x = p.x, px = p.px, py = p.py;
   const double a = XT_MADD(ow, x, -fw);
-  const double pw = px / ow;
-  const double x1 = XT_MADD(x, cs, XT_MUL(pw, sn)) + XT_MUL(fw, c1) / ow;
+  const double pw = XT_OVER_OW(px);
+  const double x1 = XT_MADD(x, cs, XT_MUL(pw, sn)) + XT_OVER_OW(XT_MUL(fw, c1));
   const double px1 = XT_NMADD(a, sn, XT_MUL(px, cs));
-  const double ix = (XT_MUL(x, sn) / w + XT_MUL(pw, c1) / w) + XT_MUL(fw / ow, length - sn / w);
+  const double ix = (XT_OVER_W(XT_MUL(x, sn)) + XT_OVER_W(XT_MUL(pw, c1))) + XT_MUL(XT_OVER_OW(fw), length - XT_OVER_W(sn));
   const double px2 = XT_MUL(px, px), a2 = XT_MUL(a, a);
-  const double ip = XT_MADD(px2 + a2, XT_MUL(0.5, length), XT_MUL(XT_MUL(px2 - a2, XT_MUL(sn, cs)), 0.5 / w)) -
-                    XT_MUL(XT_MUL(a, px), XT_MUL(sn, sn)) / w;
+  const double ip = XT_MADD(px2 + a2, XT_MUL(0.5, length), XT_MUL(XT_MUL(px2 - a2, XT_MUL(sn, cs)), h2w)) -
+                    XT_OVER_W(XT_MUL(XT_MUL(a, px), XT_MUL(sn, sn)));
+#undef XT_OVER_W
+#undef XT_OVER_OW
   const double slip = XT_MUL(length, g / XT_MUL(opd, opd + b));
   Hot o;
   o.zeta = ((p.zeta + slip) - XT_MUL(XT_MUL(rv, h), ix)) -
