@@ -314,6 +314,42 @@ def test_multi_chunk_compaction_cfg4(X):
     lat.close()
 
 
+def test_caller_workspace_and_stats(X):
+    """xt_track_opts.workspace (the caller may own the scratch of step C) and .stats (CUDA-event
+    record of the call): results are bit-identical to the library-allocated, untimed call; the record counts
+    launches and passes and its pass sizes are the alive counts; a workspace that is too small is refused."""
+    import torch
+    full = C.particles(4)
+    idx = np.linspace(0, len(full["x"]) - 1, 5003).astype(np.int64)
+    coords = C.subsample(full, idx)
+    lat = X.xt_lattice_create(packed(4))
+    a = X.new_particles(lat, coords)
+    X.xt_track_ex(lat, a, 12, compact_every=4)
+    ha = X.particles_to_host(a)
+    need = X.xt_track_workspace_bytes(len(idx))
+    assert need >= 2 * 14 * 8 * len(idx)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    ws.fill_(0xAB)                                                  # stale bytes must not matter
+    b = X.new_particles(lat, coords)
+    st = X.xt_track_ex(lat, b, 12, compact_every=4, workspace=ws, stats=True)
+    assert_bit_identical(X.particles_to_host(b), ha)
+    assert st["n_track_launches"] == 3 and st["n_passes"] == 3      # initial partition + 2 between the launches
+    assert st["pass_n_in"][0] == len(idx) and st["pass_n_in"][1] == st["pass_n_out"][0]
+    assert st["pass_n_in"][2] == st["pass_n_out"][1] and st["pass_n_out"][0] >= st["pass_n_out"][1] >= st["pass_n_out"][2]
+    n_alive_before_last_launch = st["pass_n_out"][2]
+    assert n_alive_before_last_launch >= int((ha["state"] == 1).sum()) > 0
+    assert st["track_ms"] > 0 and st["compact_ms"] > 0 and st["scatter_ms"] > 0
+    assert st["compact_bytes"] == 2 * 112.0 * sum(st["pass_n_in"])
+    c = X.new_particles(lat, coords)
+    st2 = X.xt_track_ex(lat, c, 12, compact_every=-1, stats=True)   # no compaction: one launch, no pass
+    assert st2["n_track_launches"] == 1 and st2["n_passes"] == 0
+    assert_bit_identical(X.particles_to_host(c), ha)
+    with pytest.raises(X.XtError) as e:
+        X.xt_track_ex(lat, X.new_particles(lat, coords), 12, compact_every=4, workspace=ws[:need // 2])
+    assert e.value.code == -1
+    lat.close()
+
+
 def test_permutation_invariance_and_frozen_lost(X):
     coords = C.subsample(C.particles_cfg1(sigma=1e-3), slice(0, None, 503))
     n = len(coords["x"])
