@@ -110,7 +110,16 @@ class StatsTimer {
   void begin() {
     if (!stats_) return;
     Span s{};
-    if (cudaEventCreate(&s.a) != cudaSuccess || cudaEventCreate(&s.b) != cudaSuccess) return;
+    s.kind = -1;  // until its end is recorded
+    if (cudaEventCreate(&s.a) != cudaSuccess) {
+      failed_ = true;
+      return;
+    }
+    if (cudaEventCreate(&s.b) != cudaSuccess) {
+      cudaEventDestroy(s.a);
+      failed_ = true;
+      return;
+    }
     cudaEventRecord(s.a, st_);
     ev_.push_back(s);
   }
@@ -120,6 +129,10 @@ class StatsTimer {
   int finish(int64_t n_part) {
     if (!stats_) return XT_OK;
     XT_CUDA(cudaStreamSynchronize(st_));
+    if (failed_) {  // an event could not be created: the tracking itself is complete, the record is not
+      set_error("xt_track_ex: could not create the CUDA events of xt_track_stats");
+      return XT_ERR_CUDA;
+    }
     xt_track_stats &o = *stats_;
     o = xt_track_stats{};
     std::vector<int64_t> log(n_pass_);
@@ -157,7 +170,7 @@ class StatsTimer {
     int kind;
   };
   void end(int kind, const int64_t *d_n_active) {
-    if (!stats_ || ev_.empty()) return;
+    if (!stats_ || failed_ || ev_.empty() || ev_.back().kind != -1) return;
     ev_.back().kind = kind;
     cudaEventRecord(ev_.back().b, st_);
     if (kind == 1 && d_n_active) {
@@ -172,6 +185,7 @@ class StatsTimer {
   std::vector<Span> ev_;
   int64_t *d_log_ = nullptr;
   int n_pass_ = 0;
+  bool failed_ = false;
 };
 
 }  // namespace
