@@ -845,7 +845,8 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
     constexpr uint32_t kKeyMask = NFIX > 0 ? 0x7fffu : 0xffu;  // type | flags [| order << 8]
     constexpr uint32_t kOrd = NFIX > 0 ? static_cast<uint32_t>(NFIX) : 0u;
     constexpr int kOrdT = NFIX > 0 ? NFIX : -1;
-    switch (tag & kKeyMask) {
+    const uint32_t key = tag & kKeyMask;
+    switch (key) {
       case TAG_DRIFT:
       case TAG_DRIFT | TAG_POST: {
         DriftCoef<P> d;
