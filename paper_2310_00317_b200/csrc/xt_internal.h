@@ -118,7 +118,8 @@ struct xt_lattice {
   std::vector<double> s_table_host;
   std::vector<unsigned char> packed_host;  // the buffer the lattice was created from (xt_refine.cu re-reads it)
   bool extended = false;                   // thick maps or polygon apertures: the THICK kernels
-  int fixed_order = 0;                     // 15 if most multipole records are of order 15 (unrolled handlers), else 0
+  int fixed_order = 0;                     // which orders have unrolled handlers: 15 (most multipoles of order 15),
+                                           // 1 | 2 << 5 (most of order 1 or 2), else 0
   std::vector<uint64_t> mult_slot0;        // per element: image offset of a multipole's first coefficient pair
   std::vector<uint64_t> mult_wf_off;       // per element: image offset of a multipole's weak-focusing term
   // time functions (xt_knobs.cu); all device memory, owned

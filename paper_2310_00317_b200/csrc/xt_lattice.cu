@@ -445,14 +445,18 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
     fused.swap(merged);
   }
   info.n_records = static_cast<int64_t>(fused.size());
-  {  // which instantiation of the tracking kernel suits the lattice: is it full of order-15 multipoles?
-    int64_t n_mult = 0, n_15 = 0;
+  {  // which instantiation of the tracking kernel suits the lattice: full of order-15 multipoles (errors on
+     // every magnet), or of thin quadrupoles and sextupoles (orders 1 and 2)?
+    int64_t n_mult = 0, n_15 = 0, n_low = 0;
     for (const Rec &rec : fused) {
       if (rec.type != TAG_MULT && rec.type != TAG_CMULT) continue;
       ++n_mult;
       if (rec.order == 15) ++n_15;
+      if (rec.order == 1 || rec.order == 2) ++n_low;
     }
-    out.fixed_order = (n_mult > 0 && 2 * n_15 >= n_mult) ? 15 : 0;
+    out.fixed_order = 0;
+    if (n_mult > 0 && 2 * n_15 >= n_mult) out.fixed_order = 15;
+    else if (n_mult > 0 && 2 * n_low >= n_mult) out.fixed_order = 1 | (2 << 5);
   }
   for (const Rec &rec : fused) {
     if (rec.type == TAG_DRIFT) info.n_drift_evals += 1;

@@ -840,11 +840,14 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
     const double p0 = h.p0;
     const uint32_t elem = h.elem;
     rp += tag >> 16;  // record size in bytes
-    // NFIX > 0: the multipole order with fully unrolled handlers (the switch key then includes the order);
-    // NFIX = 0: the flag sets are specialised, the order is read at run time.
+    // NFIX > 0: the multipole order(s) with fully unrolled handlers, first | second << 5 (the switch key then
+    // includes the order); NFIX = 0: the flag sets are specialised, the order is read at run time.
     constexpr uint32_t kKeyMask = NFIX > 0 ? 0x7fffu : 0xffu;  // type | flags [| order << 8]
-    constexpr uint32_t kOrd = NFIX > 0 ? static_cast<uint32_t>(NFIX) : 0u;
-    constexpr int kOrdT = NFIX > 0 ? NFIX : -1;
+    constexpr uint32_t kOrd = NFIX > 0 ? static_cast<uint32_t>(NFIX & 31) : 0u;
+    constexpr int kOrdT = NFIX > 0 ? (NFIX & 31) : -1;
+    constexpr uint32_t kOrdB = static_cast<uint32_t>(NFIX >> 5);          // second fixed order, 0: none
+    constexpr int kOrdBT = (NFIX >> 5) > 0 ? (NFIX >> 5) : 1;
+    constexpr uint32_t kNoB = (NFIX >> 5) > 0 ? 0u : 0x6000u;             // parks the second order's labels
     const uint32_t key = tag & kKeyMask;
     switch (key) {
       case TAG_DRIFT:
@@ -872,6 +875,8 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
       XT_MULT_CASE((HandlerSet<P, ColdT::kInRegs>::value >= 0 ? 0u : 0x7000u), kOrd, kOrdT)
 #endif
       XT_MULT_CASE(TAG_POST, kOrd, kOrdT)
+      XT_MULT_CASE(kNoB, kOrdB, kOrdBT)  // the second fixed order (lattices of thin quadrupoles and sextupoles)
+      XT_MULT_CASE(TAG_POST | kNoB, kOrdB, kOrdBT)
 #ifdef XT_FMAD_OFF
       XT_MULT_CASE(TAG_POST | TAG_POST2, kOrd, kOrdT)
       XT_MULT_CASE(TAG_PRE | TAG_POST | TAG_POST2, kOrd, kOrdT)
@@ -1196,12 +1201,18 @@ int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaSt
 // Lattices with thick elements take the instantiation that has their maps compiled in; lattices full of
 // order-15 multipoles the one with the unrolled order-15 handlers (3 and 4 particles per thread: the
 // shapes large lattices run with).
-constexpr int kFixedOrder = 15;
+constexpr int kFixedOrder = 15;       // configs[2-4]: every magnet carries errors up to order 15
+constexpr int kFixedLow = 1 | (2 << 5);  // thin quadrupoles and sextupoles (configs[0], [1]): orders 1 and 2
 template <int P, bool REG>
 int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
   constexpr bool kHasFixed = (P >= 3) || REG;  // which shapes exist with the unrolled order-15 handlers
   if (kHasFixed && lat->fixed_order == kFixedOrder) {
     constexpr int NF = kHasFixed ? kFixedOrder : 0;
+    return lat->extended ? launch_track_pt<P, true, REG, NF>(a, lat, block, st)
+                         : launch_track_pt<P, false, REG, NF>(a, lat, block, st);
+  }
+  if (!REG && lat->fixed_order == kFixedLow) {
+    constexpr int NF = REG ? 0 : kFixedLow;
     return lat->extended ? launch_track_pt<P, true, REG, NF>(a, lat, block, st)
                          : launch_track_pt<P, false, REG, NF>(a, lat, block, st);
   }
