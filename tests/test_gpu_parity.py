@@ -301,6 +301,30 @@ def test_launch_shape_fusion_and_chunk_size_do_not_change_results(X):
         lat2.close()
 
 
+def test_launch_shapes_on_a_quadrupole_sextupole_lattice(X):
+    """configs[1b] (orders 1 and 2 only: the kernels with those two orders fixed; single chunk, losses): every
+    launch shape and both homes of the cold state reproduce the default bit for bit, in both builds; the
+    validation build equals the oracle bit for bit on the cavity-stripped lattice."""
+    coords = C.subsample(C.particles_cfg1(sigma=1e-3), slice(0, None, 211))
+    for kind, strip in (("prod", False), ("nofma", True)):
+        buf = packed(1, strip=strip)
+        lat = X.xt_lattice_create(buf, kind=kind)
+        base = X.new_particles(lat, coords)
+        X.xt_track_ex(lat, base, 40)
+        base = X.particles_to_host(base)
+        assert 0.05 < (base["state"] == 0).mean() < 0.95
+        for ppt, block, cold in ((1, 32, -1), (2, 64, -1), (3, 96, -1), (4, 128, -1), (1, 64, 1), (2, 128, 1), (3, 32, 1)):
+            p = X.new_particles(lat, coords)
+            X.xt_track_ex(lat, p, 40, block_size=block, particles_per_thread=ppt, cold_in_registers=cold,
+                          compact_every=-1 if ppt % 2 else 7)
+            assert_bit_identical(X.particles_to_host(p), base)
+        lat.close()
+        if strip:
+            ref = O.new_particles(buf, coords)
+            O.track(buf, ref, 40, threads=THREADS)
+            assert_bit_identical(base, ref)
+
+
 def test_multi_chunk_compaction_cfg4(X):
     full = C.particles(4)
     idx = np.linspace(0, len(full["x"]) - 1, 3001).astype(np.int64)
