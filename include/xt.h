@@ -197,6 +197,27 @@ int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t n_part, in
  * counts, two counters): what xt_track_opts.workspace must provide. */
 uint64_t xt_track_workspace_bytes(int64_t n_part);
 
+/* xt_track_ex for callers that cannot allocate (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): the same steps with the same results (bit-identical to
+ * xt_track_ex in the same build), but the scratch of step C (particles stopped by
+ * an aperture are retired, the alive ones packed) is a fixed array in the library's device image
+ * instead of a stream-ordered allocation.  The call makes no cudaMalloc / cudaFree /
+ * cudaMallocAsync and calls no allocating library routine.
+ *   - n_part <= XT_TRACK_STATIC_MAX_PARTICLES, else XT_ERR_INVALID_ARG (xt_last_error names the
+ *     limit).  The array is 7.0 MiB (xt_track_workspace_bytes of the limit); every GPU that
+ *     loads the library holds it until the process exits.
+ *   - opts may be NULL; opts->workspace, ->workspace_bytes and ->stats must be 0 / NULL (the
+ *     stats record creates events and allocates): XT_ERR_INVALID_ARG otherwise.
+ *   - p: DEVICE arrays, the caller's inputs and outputs as in xt_track_ex; nothing else is kept.
+ *   - ALL calls on a device share the one array, which keeps the previous call's bytes (the
+ *     call clears what must start at zero itself).  Two xt_track_static calls whose GPU work can
+ *     overlap (different streams, or graphs launched concurrently) RACE on it: order them on one
+ *     stream or with events.  Calls on different devices do not interact.
+ *   - Lattices without apertures, compact_every < 0 or n_turns <= the period never touch it. */
+#define XT_TRACK_STATIC_MAX_PARTICLES 32768
+int xt_track_static(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
+                    void *cuda_stream, const xt_track_opts *opts);
+
 /* End-to-end variant: the SAME call with HOST arrays.  Copies the ensemble to the device
  * (stream-ordered allocation), tracks, copies everything back and synchronises the stream.
  * Pinned host memory makes the copies asynchronous; pageable memory also works. */

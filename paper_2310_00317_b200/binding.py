@@ -134,6 +134,8 @@ SIGNATURES = {
     "xt_track": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _VP]),
     "xt_track_ex": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _VP,
                                    ctypes.POINTER(xt_track_opts)]),
+    "xt_track_static": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _VP,
+                                       ctypes.POINTER(xt_track_opts)]),
     "xt_track_host": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _I64, _VP,
                                      ctypes.POINTER(xt_track_opts)]),
     "xt_particles_init_derived": (ctypes.c_int, [_VP, ctypes.POINTER(xt_particles), _I64, _VP]),
@@ -406,6 +408,20 @@ def xt_track_ex(lat: Lattice, p: Dict, n_turns: int, stream=None, *, turns_per_l
     _check(lat._lib, lat._lib.xt_track_ex(lat.handle, ctypes.byref(st), _n_part(p), int(n_turns),
                                           _stream_ptr(stream), ctypes.byref(o) if o else None))
     return _stats_dict(rec) if stats else None
+
+
+XT_TRACK_STATIC_MAX_PARTICLES = 32768
+
+
+def xt_track_static(lat: Lattice, p: Dict, n_turns: int, stream=None, *, turns_per_launch: int = 0,
+                    compact_every: int = 0, block_size: int = 0, particles_per_thread: int = 0,
+                    cold_in_registers: int = 0) -> None:
+    """xt_track_ex without any allocation: step C's scratch is the library's static device array
+    (at most XT_TRACK_STATIC_MAX_PARTICLES particles; calls that overlap on the GPU race, include/xt.h)."""
+    st = _struct_from_tensors(p)
+    o = _opts(turns_per_launch, compact_every, block_size, particles_per_thread, None, None, cold_in_registers)
+    _check(lat._lib, lat._lib.xt_track_static(lat.handle, ctypes.byref(st), _n_part(p), int(n_turns),
+                                              _stream_ptr(stream), ctypes.byref(o) if o else None))
 
 
 def xt_track_host(lat: Lattice, p_host: Dict, n_turns: int, stream=None, *, turns_per_launch: int = 0,

@@ -7,6 +7,9 @@
 // tracking kernel's warps stay full; each retired particle is written straight to its final place
 // in the caller's arrays through its origin index.  HBM-bound, 2 x n x 112 B per pass; measured
 // 4.0-4.4 TB/s on 2e6 particles (profiles/r02_compaction_summary.md).
+#include <atomic>
+#include <string>
+
 #include "xt_internal.h"
 
 namespace xt {
@@ -282,3 +285,85 @@ int launch_histogram(const int64_t *at_turn, const int64_t *state, int64_t n, in
 }
 
 }  // namespace xt
+
+// ------------------------------------------------------------------ xt_track_static (include/xt.h)
+// Tracking with loss compaction for callers that may not allocate (CUDA graph capture, serving loops,
+// harnesses that forbid cudaMalloc): the whole scratch of step C -- two working sets of 14 arrays, the tile
+// status words of the single-pass scan, the ticket and the two counters -- lives in ONE file-scope device
+// array of fixed size instead of a cudaMallocAsync block.  Every GPU that loads the library holds the
+// array (7.0 MiB) until the process exits.  All calls share it: it keeps the previous call's bytes, two
+// calls that overlap on the GPU race (see the header).  What must start at zero (status words, ticket,
+// counters) is cleared by the first pass of every call (launch_partition, plan.epoch == 0); the working
+// sets are written by a pass before anything reads them.
+namespace xt {
+namespace {
+
+constexpr int64_t kStaticMaxParticles = XT_TRACK_STATIC_MAX_PARTICLES;
+constexpr size_t up256(size_t v) { return (v + 255) & ~static_cast<size_t>(255); }
+constexpr size_t kStaticBytes = 2 * 14 * up256(static_cast<size_t>(kStaticMaxParticles) * 8) +
+                                up256(static_cast<size_t>((kStaticMaxParticles + kTile - 1) / kTile) * 8) + 256;
+static_assert(kStaticBytes <= (8u << 20), "the static workspace is meant to stay modest");
+
+static __device__ __align__(256) unsigned char g_static_workspace[kStaticBytes];
+
+// In host code `g_static_workspace` is only a handle of the symbol, not a device address: the address
+// comes from cudaGetSymbolAddress, once per device, with that device current.
+constexpr int kMaxDevices = 64;
+std::atomic<void *> g_static_address[kMaxDevices];
+
+int static_workspace_address(void **out) {
+  int dev = -1;
+  XT_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) {
+    set_error("xt_track_static: device ordinal out of range");
+    return XT_ERR_INVALID_ARG;
+  }
+  void *ptr = g_static_address[dev].load(std::memory_order_acquire);
+  if (!ptr) {
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_workspace);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(static workspace)");
+    if (!ptr || (reinterpret_cast<uintptr_t>(ptr) & 255u)) {
+      set_error("xt_track_static: the static workspace has no 256-byte aligned device address");
+      return XT_ERR_CUDA;
+    }
+    g_static_address[dev].store(ptr, std::memory_order_release);
+  }
+  *out = ptr;
+  return XT_OK;
+}
+
+}  // namespace
+}  // namespace xt
+
+extern "C" int xt_track_static(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
+                               void *cuda_stream, const xt_track_opts *opts) {
+  return xt::guarded<int>([&] {
+    if (!lat || !p) {
+      xt::set_error("xt_track_static: NULL lattice or particles");
+      return static_cast<int>(XT_ERR_INVALID_ARG);
+    }
+    if (n_part > xt::kStaticMaxParticles) {
+      xt::set_error("xt_track_static: n_part = " + std::to_string(n_part) + " exceeds XT_TRACK_STATIC_MAX_PARTICLES = " +
+                    std::to_string(xt::kStaticMaxParticles) +
+                    ", all the static device workspace holds; use xt_track_ex with xt_track_opts.workspace");
+      return static_cast<int>(XT_ERR_INVALID_ARG);
+    }
+    if (opts && (opts->workspace || opts->workspace_bytes || opts->stats)) {
+      xt::set_error("xt_track_static: xt_track_opts.workspace / .stats must be NULL (the workspace is the library's "
+                    "static array; the stats record allocates)");
+      return static_cast<int>(XT_ERR_INVALID_ARG);
+    }
+    int rc = xt::check_device(lat, "xt_track_static");
+    if (rc != XT_OK) return rc;
+    if (xt::compaction_workspace_bytes(xt::kStaticMaxParticles) > xt::kStaticBytes) {
+      xt::set_error("xt_track_static: internal error, the static workspace is smaller than step C needs");
+      return static_cast<int>(XT_ERR_CUDA);
+    }
+    void *ws = nullptr;
+    if ((rc = xt::static_workspace_address(&ws)) != XT_OK) return rc;
+    xt_track_opts o = opts ? *opts : xt_track_opts{};
+    o.workspace = ws;  // a device address; the partition and tracking kernels receive pointers cut from it
+    o.workspace_bytes = xt::kStaticBytes;
+    return xt_track_ex(lat, p, n_part, n_turns, cuda_stream, &o);
+  });
+}
