@@ -396,8 +396,8 @@ def main():
             line["roofline"]["frac_all_slots"] = None
         # DRAM bytes of one launch: not measurable inside the run (needs ncu); the number is the --set full
         # capture's dram__bytes_read + dram__bytes_write per particle scaled to this launch
-        line["roofline"]["traffic"] = 76.9 * n_part if cfg == 3 else None
-        line["roofline"]["traffic_source"] = ("ncu capture profiles/r01m_track_cfg3_summary.md: 76.9 B per particle "
+        line["roofline"]["traffic"] = 78.0 * n_part if cfg == 3 else None
+        line["roofline"]["traffic_source"] = ("ncu capture profiles/r02c_track_cfg3_summary.md: 78 B per particle "
                                               "(reads + writes of one launch), scaled by n_part; not measured in "
                                               "this run") if cfg == 3 else None
         line["roofline"]["operand_pattern_ceilings_tflops"] = probe
