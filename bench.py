@@ -237,7 +237,7 @@ def time_workload(X, torch, lat, coords, turns, steps, warmup, args, barrier, sa
         if ev0 is not None:
             ev0.record(stream)
         X.xt_track_ex(lat, work, turns, block_size=args.block, particles_per_thread=args.ppt,
-                      cold_in_registers=args.cold)
+                      cold_in_registers=args.cold, balance=args.balance)
         if ev1 is not None:
             ev1.record(stream)
 
@@ -306,6 +306,8 @@ def main():
     ap.add_argument("--ppt", type=int, default=0, help="particles per thread (0: auto)")
     ap.add_argument("--chunk", type=int, default=0, help="staging-buffer bytes (0: library default)")
     ap.add_argument("--cold", type=int, default=0, help="cold state: 0 auto, 1 registers, -1 shared memory")
+    ap.add_argument("--balance", type=int, default=0,
+                    help="xt_track_opts.balance: 0 auto, -1 off, 1 on, n > 1 on with n turns per item")
     ap.add_argument("--also-steps", type=int, default=5, help="timed steps of the configs[2] leg (mean)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and configs[2] legs")
     args = ap.parse_args()

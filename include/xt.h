@@ -128,7 +128,14 @@ typedef struct {
                             /*    memory.                                                        */
                             /*    Launch-shape option like the two above: results are            */
                             /*    bit-identical for every shape.                                 */
-  int32_t reserved;         /* 0                                                               */
+  int32_t balance;          /* small ensembles (cold state in registers) without compaction:     */
+                            /*    0: auto, -1: never, 1: always, n > 1: always, n turns per item.  */
+                            /*    The CTAs of one launch are persistent and draw (group of         */
+                            /*    particles, block of turns) items from a device counter, so that  */
+                            /*    an ensemble that does not fill a whole number of CTAs per SM     */
+                            /*    still keeps every SM busy.  Needs 4 bytes  */
+                            /*    per group of particles + 8: from `workspace` when given, else    */
+                            /*    stream-ordered.  Launch-shape option: bit-identical results.     */
 } xt_track_opts;
 
 /* Static description of a lattice image; counts are per turn. */

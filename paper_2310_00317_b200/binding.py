@@ -51,7 +51,7 @@ class xt_track_opts(ctypes.Structure):
                 ("block_size", ctypes.c_int32), ("particles_per_thread", ctypes.c_int32),
                 ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_uint64),
                 ("stats", ctypes.POINTER(xt_track_stats)),
-                ("cold_in_registers", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("cold_in_registers", ctypes.c_int32), ("balance", ctypes.c_int32)]
 
 
 class xt_lattice_opts(ctypes.Structure):
@@ -357,12 +357,13 @@ def _n_part(p: Dict) -> int:
 
 
 def _opts(turns_per_launch=0, compact_every=0, block_size=0, particles_per_thread=0, workspace=None, stats=None,
-          cold_in_registers=0):
-    if not (turns_per_launch or compact_every or block_size or particles_per_thread or cold_in_registers) \
+          cold_in_registers=0, balance=0):
+    if not (turns_per_launch or compact_every or block_size or particles_per_thread or cold_in_registers or balance) \
             and workspace is None and stats is None:
         return None
     o = xt_track_opts(int(turns_per_launch), int(compact_every), int(block_size), int(particles_per_thread))
     o.cold_in_registers = int(cold_in_registers)
+    o.balance = int(balance)
     if workspace is not None:                      # a torch uint8 CUDA tensor, caller-owned
         o.workspace = workspace.data_ptr()
         o.workspace_bytes = workspace.numel() * workspace.element_size()
@@ -399,12 +400,13 @@ def xt_track(lat: Lattice, p: Dict, n_turns: int, stream=None) -> None:
 
 def xt_track_ex(lat: Lattice, p: Dict, n_turns: int, stream=None, *, turns_per_launch: int = 0,
                 compact_every: int = 0, block_size: int = 0, particles_per_thread: int = 0,
-                workspace=None, stats: bool = False, cold_in_registers: int = 0):
+                workspace=None, stats: bool = False, cold_in_registers: int = 0, balance: int = 0):
     """``workspace``: optional torch uint8 CUDA tensor of xt_track_workspace_bytes(n) bytes; ``stats=True``
     returns the call's xt_track_stats as a dict (and makes the call synchronous)."""
     st = _struct_from_tensors(p)
     rec = xt_track_stats() if stats else None
-    o = _opts(turns_per_launch, compact_every, block_size, particles_per_thread, workspace, rec, cold_in_registers)
+    o = _opts(turns_per_launch, compact_every, block_size, particles_per_thread, workspace, rec, cold_in_registers,
+              balance)
     _check(lat._lib, lat._lib.xt_track_ex(lat.handle, ctypes.byref(st), _n_part(p), int(n_turns),
                                           _stream_ptr(stream), ctypes.byref(o) if o else None))
     return _stats_dict(rec) if stats else None
@@ -415,11 +417,12 @@ XT_TRACK_STATIC_MAX_PARTICLES = 32768
 
 def xt_track_static(lat: Lattice, p: Dict, n_turns: int, stream=None, *, turns_per_launch: int = 0,
                     compact_every: int = 0, block_size: int = 0, particles_per_thread: int = 0,
-                    cold_in_registers: int = 0) -> None:
+                    cold_in_registers: int = 0, balance: int = 0) -> None:
     """xt_track_ex without any allocation: step C's scratch is the library's static device array
     (at most XT_TRACK_STATIC_MAX_PARTICLES particles; calls that overlap on the GPU race, include/xt.h)."""
     st = _struct_from_tensors(p)
-    o = _opts(turns_per_launch, compact_every, block_size, particles_per_thread, None, None, cold_in_registers)
+    o = _opts(turns_per_launch, compact_every, block_size, particles_per_thread, None, None, cold_in_registers,
+              balance)
     _check(lat._lib, lat._lib.xt_track_static(lat.handle, ctypes.byref(st), _n_part(p), int(n_turns),
                                               _stream_ptr(stream), ctypes.byref(o) if o else None))
 

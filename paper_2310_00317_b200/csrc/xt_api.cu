@@ -49,26 +49,37 @@ int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p
 
 // Launch shape of the tracking kernel: threads per CTA, particles per thread, and where the cold
 // per-particle state lives.  Auto rule (measured on B200, profiles/r02_shape_sweep.md): 128-thread CTAs.
-// Several waves of particles (>= 4096 per SM, configs[3]): 4 per thread, cold state in shared memory,
-// 4 CTAs per SM at <= 128 registers.  Ensembles that fit the SMs in one wave (<= 768 per SM, configs[2]:
-// 676): 2 per thread with the cold state in registers -- the register file is half empty there, every LDS
-// taken out of a record shortens what a warp waits for, and three warps of two particles per scheduler
-// cover each other's latencies better than two warps of three (0.524 against 0.511).  In between: 3 per
-// thread, cold state in shared memory.  Below ~100 particles per SM one per thread keeps more warps
-// alive.  The kernel hands the particles out in equal shares over a whole number of CTAs per SM, so the
-// shape only has to make enough CTAs.
+// Many waves of particles (configs[3]: 67 568 per SM): 4 per thread, cold state in shared memory, 4 CTAs per
+// SM at <= 128 registers, every CTA owning its share for the whole launch.  Up to ~12 000 per SM, when the
+// launch is long enough for the balanced mode (xt_track.cu: one CTA per (group, block of turns) item, a
+// queue of ready groups): the cold state in registers, 2 per thread up to 1024 per SM, 3 above; full
+// warps and an SM that is never short of a CTA beat the static shapes by 16-30 % there (configs[2]: 0.522 ->
+// 0.610 of the DFMA peak; 150 000 particles on the configs[3] lattice: 0.477 -> 0.619; 10^6: 0.608 ->
+// 0.644; 2 * 10^6: equal; above, the static 4-per-thread shape wins).  Launches too short for that (or
+// with compaction, whose particle count lives on the device): 2 per thread / registers up to 768 per SM
+// (configs[2] statically: 0.524 against 0.511 for 3 per thread), 3 per thread / shared memory up to 4096,
+// 4 above.  Below ~100 particles per SM one per thread keeps more warps alive.
 struct Shape {
   int block, ppt;
   bool cold_in_regs;
 };
-int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part, Shape *sh) {
+int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part, bool can_balance, Shape *sh) {
   const int64_t per_sm = n_part / (lat->n_sm > 0 ? lat->n_sm : 1);
   int auto_ppt = 4, auto_block = 128;
+  bool auto_regs = false;
   if (per_sm < 4096) auto_ppt = 3;
-  if (per_sm <= 768) auto_ppt = 2;
+  if (can_balance && per_sm <= 12288) {
+    auto_ppt = 3;
+    auto_regs = true;
+  }
+  if (per_sm <= 768 || (can_balance && per_sm <= 1024)) {
+    auto_ppt = 2;
+    auto_regs = true;
+  }
   if (per_sm < 96) {
     auto_ppt = 1;
     auto_block = 32;
+    auto_regs = false;
   }
   sh->ppt = (o && o->particles_per_thread) ? o->particles_per_thread : auto_ppt;
   sh->block = (o && o->block_size) ? o->block_size : auto_block;
@@ -78,7 +89,7 @@ int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part,
   else if (want_regs < 0)
     sh->cold_in_regs = false;
   else
-    sh->cold_in_regs = (sh->ppt <= 3 && per_sm >= 96 && per_sm <= 768);
+    sh->cold_in_regs = auto_regs && sh->ppt <= 3;
   if (sh->ppt < 1 || sh->ppt > 4) {
     set_error("xt_track_ex: particles_per_thread must be 0 (auto), 1, 2, 3 or 4");
     return XT_ERR_INVALID_ARG;
@@ -199,8 +210,6 @@ static int xt_track_ex_impl(const xt_lattice *lat, const xt_particles *p, int64_
     xt::set_error("xt_track: negative n_turns");
     return XT_ERR_INVALID_ARG;
   }
-  xt::Shape sh{};
-  if ((rc = xt::resolve_shape(opts, lat, n_part, &sh)) != XT_OK) return rc;
   if (opts && opts->turns_per_launch < 0) {
     xt::set_error("xt_track_ex: negative turns_per_launch");
     return XT_ERR_INVALID_ARG;
@@ -216,18 +225,50 @@ static int xt_track_ex_impl(const xt_lattice *lat, const xt_particles *p, int64_
     if (n_turns > pr) period = pr;
   }
   const int64_t tpl_opt = opts ? opts->turns_per_launch : 0;
+  // the balanced mode needs launches of several blocks of turns and a particle count known to the host
+  const int64_t launch_turns = (tpl_opt > 0 && tpl_opt < n_turns) ? tpl_opt : n_turns;
+  const bool can_balance = period == 0 && xt::balance_pays(lat, launch_turns, opts ? opts->balance : 0);
+  xt::Shape sh{};
+  if ((rc = xt::resolve_shape(opts, lat, n_part, can_balance, &sh)) != XT_OK) return rc;
 
   xt::StatsTimer tm(opts ? opts->stats : nullptr, st);
   if (period == 0) {
-    const int64_t tpl = tpl_opt > 0 ? tpl_opt : n_turns;
-    for (int64_t done = 0; done < n_turns;) {
-      const int64_t k = (n_turns - done < tpl) ? n_turns - done : tpl;
-      tm.begin();
-      if ((rc = xt::launch_track(lat, *p, n_part, nullptr, k, sh.block, sh.ppt, sh.cold_in_regs, st)) != XT_OK) return rc;
-      tm.end_track();
-      done += k;
+    // Balanced mode of the shapes with the cold state in registers (xt_track.cu): needs two counters and one
+    // word per item, from the caller's workspace if there is one, else stream-ordered.
+    const int balance = opts ? opts->balance : 0;
+    unsigned int *queue = nullptr;
+    bool own_queue = false;
+    if (sh.cold_in_regs && can_balance) {
+      const size_t qb = xt::balance_scratch_bytes(n_part, sh.block, sh.ppt);
+      if (opts && opts->workspace) {
+        if (opts->workspace_bytes >= qb && !(reinterpret_cast<uintptr_t>(opts->workspace) & 255u)) {
+          queue = static_cast<unsigned int *>(opts->workspace);
+        } else if (balance > 0) {
+          xt::set_error("xt_track_ex: workspace too small for the balanced mode (xt_track_workspace_bytes is enough) or not 256-byte aligned");
+          return XT_ERR_INVALID_ARG;
+        }
+      } else {
+        XT_CUDA(cudaMallocAsync(reinterpret_cast<void **>(&queue), qb, st));
+        own_queue = true;
+      }
+    } else if (balance > 0) {
+      xt::set_error("xt_track_ex: balance > 0 needs the cold state in registers (cold_in_registers = 1, or the auto shape of small ensembles)");
+      return XT_ERR_INVALID_ARG;
     }
-    return tm.finish(n_part);
+    auto done = [&](int code) {
+      if (own_queue) cudaFreeAsync(queue, st);
+      return code;
+    };
+    const int64_t tpl = tpl_opt > 0 ? tpl_opt : n_turns;
+    for (int64_t done_turns = 0; done_turns < n_turns;) {
+      const int64_t k = (n_turns - done_turns < tpl) ? n_turns - done_turns : tpl;
+      tm.begin();
+      if ((rc = xt::launch_track(lat, *p, n_part, nullptr, k, sh.block, sh.ppt, sh.cold_in_regs, st, queue, balance)) != XT_OK)
+        return done(rc);
+      tm.end_track();
+      done_turns += k;
+    }
+    return done(tm.finish(n_part));
   }
 
   void *ws = opts ? opts->workspace : nullptr;

@@ -188,9 +188,16 @@ int pack_image(const void *packed, size_t nbytes, const PackOpts &opts, HostImag
 // block: threads per CTA; ppt: particles per thread (1, 2, 3 or 4; 4 needs block <= 256); cold_in_regs: the
 // per-particle functions of (delta, ptau) in registers instead of shared memory (ppt 2 or 3 only).
 // TAG_MON records store into lat->d_monitor_rows (rows of n_part x 6 doubles: x, px, y, py, zeta, delta).
+// queue: device scratch of balance_scratch_bytes() for the balanced mode (persistent CTAs drawing
+// (group, block of turns) items from a ticket counter; cold_in_regs shapes without a device counter only),
+// or nullptr.  balance: xt_track_opts.balance (< 0 never, 0 auto, 1 always, n > 1 always with n turns per item).
 int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part,
                  const int64_t *d_n_active, int64_t n_turns, int block, int ppt, bool cold_in_regs,
-                 cudaStream_t st);
+                 cudaStream_t st, unsigned int *queue = nullptr, int balance = 0);
+size_t balance_scratch_bytes(int64_t n_part, int block, int ppt);
+// turns per item of the balanced mode for a launch of n_turns turns, and whether the auto rule would use it
+int64_t balance_block_turns(const xt_lattice *lat, int64_t n_turns, int balance);
+bool balance_pays(const xt_lattice *lat, int64_t n_turns, int balance);
 int launch_init_derived(const xt_lattice *lat, const xt_particles &p, int64_t n, cudaStream_t st);
 
 // xt_compact.cu (step C) -- SoA working set with an origin index

@@ -42,6 +42,13 @@
 namespace xt {
 namespace {
 
+// Balanced mode: turns in the first item of group g.  The later items have block_turns turns each; the first
+// ones are staggered (1 .. block_turns, by a hash of the group) so that the CTAs of one SM do not all finish,
+// wait and restart at the same moments -- the load only evens out when their waits do not coincide.
+__host__ __device__ inline int64_t first_block_turns(uint32_t group, int64_t block_turns) {
+  return 1 + static_cast<int64_t>(((group * 2654435761u) >> 8) % static_cast<uint32_t>(block_turns));
+}
+
 struct TrackArgs {
   const unsigned char *image;
   const ChunkDesc *chunks;
@@ -56,6 +63,13 @@ struct TrackArgs {
   int32_t stage_chunks;  // consecutive chunks staged by one bulk copy (they are contiguous in the image)
   int32_t grid_quantum;  // CTAs are handed out in multiples of this (the SM count)
   double beta0, tib, igam2;
+  // Balanced mode (cold-state-in-registers shapes only; nullptr otherwise): the CTAs are persistent and
+  // draw (group of particles, block of turns) items from a first-in first-out queue.  queue[0]: pop
+  // tickets; queue[1]: pushes; queue[2 + n]: item of push n, plus one.
+  unsigned int *queue;
+  int32_t n_groups;     // groups of blockDim.x * P particles
+  int32_t block_turns;  // turns per item
+  int64_t n_items;      // items of all groups: a staggered first one, then blocks of block_turns turns
 };
 
 __device__ __forceinline__ uint32_t smem_addr(const void *p) {
@@ -996,128 +1010,315 @@ __global__ void __maxnreg__((RegBudget<P, REG, THICK>::value)) xt_track_kernel(c
   unsigned char *const buf0 =
       smem + 128 + ((static_cast<uint32_t>(8 * ColdT::kPitch) * blockDim.x + 127u) & ~127u);
 
-  // Balanced hand-out (device side, so that compaction's device counter needs no host
-  // sync): use as few CTAs as hold n_active particles, rounded up to a whole number per SM,
-  // and give each the same share.
-  const int64_t n_active = a.n_active ? *a.n_active : a.n_part;
-  const int64_t cap = static_cast<int64_t>(blockDim.x) * P;
-  const int64_t need = (n_active + cap - 1) / cap;
-  int64_t used = ((need + a.grid_quantum - 1) / a.grid_quantum) * a.grid_quantum;
-  if (used > static_cast<int64_t>(gridDim.x)) used = gridDim.x;
-  if (static_cast<int64_t>(blockIdx.x) >= used) return;  // CTA-uniform
-  const int64_t share = (n_active + used - 1) / used;
-  const int64_t start = static_cast<int64_t>(blockIdx.x) * share;
-  if (start >= n_active) return;  // CTA-uniform
-  const int64_t count = (n_active - start < share) ? n_active - start : share;
+  if constexpr (!REG) {
+    // The shapes with the cold state in shared memory: one share of the ensemble per CTA for the whole launch.
+    // Balanced hand-out (device side, so that compaction's device counter needs no host
+    // sync): use as few CTAs as hold n_active particles, rounded up to a whole number per SM,
+    // and give each the same share.
+    const int64_t n_active = a.n_active ? *a.n_active : a.n_part;
+    const int64_t cap = static_cast<int64_t>(blockDim.x) * P;
+    const int64_t need = (n_active + cap - 1) / cap;
+    int64_t used = ((need + a.grid_quantum - 1) / a.grid_quantum) * a.grid_quantum;
+    if (used > static_cast<int64_t>(gridDim.x)) used = gridDim.x;
+    if (static_cast<int64_t>(blockIdx.x) >= used) return;  // CTA-uniform
+    const int64_t share = (n_active + used - 1) / used;
+    const int64_t start = static_cast<int64_t>(blockIdx.x) * share;
+    if (start >= n_active) return;  // CTA-uniform
+    const int64_t count = (n_active - start < share) ? n_active - start : share;
 
-  Parts<P> q;
-  cold.first = start + threadIdx.x;
-  q.alive = 0;
+    Parts<P> q;
+    cold.first = start + threadIdx.x;
+    q.alive = 0;
 #pragma unroll
-  for (int j = 0; j < P; ++j) {
-    const int64_t k = static_cast<int64_t>(j) * blockDim.x + threadIdx.x;
-    const int64_t i = start + k;
-    const bool live = (k < count) && (a.p.state[i] == 1);
-    if (live) {
-      q.x[j] = a.p.x[i];
-      q.px[j] = a.p.px[i];
-      q.y[j] = a.p.y[i];
-      q.py[j] = a.p.py[i];
-      q.zeta[j] = a.p.zeta[i];
-      const double delta = a.p.delta[i];
-      const double ptau = a.p.ptau[i];
-      cold.delta(j) = delta;
-      cold.ptau(j) = ptau;
-      q.alive |= 1u << j;
-      const double opd = 1.0 + delta;
-      const double b = XT_MADD(a.beta0, ptau, 1.0);
-      const double t = XT_MUL(ptau, ptau + a.tib);
-      refresh_cached(cold, j, opd, b, t, a.igam2);
-    } else {
-      q.x[j] = q.px[j] = q.y[j] = q.py[j] = q.zeta[j] = 0.0;
-      cold.opd2(j) = cold.b(j) = 1.0;
-      cold.g(j) = 0.0;
-      cold.ptau(j) = cold.delta(j) = 0.0;
-      cold.rv0v(j) = 1.0;
-    }
-  }
-
-  const bool single = (a.n_chunks == 1);
-  if (threadIdx.x == 0) {
-    mbar_init(bar0, 1);
-    mbar_init(bar0 + 8, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  // A stage = stage_chunks consecutive chunks = one bulk copy into one buffer.  A lattice that fits one
-  // chunk is loaded once and stays resident in buffer 0: its warps run free, no CTA-level
-  // synchronisation; otherwise the stages alternate between the two buffers and a __syncthreads_or at
-  // the end of each releases the buffer and tells the CTA whether anyone is still alive.  One loop (and
-  // one copy of the record interpreter in the instruction cache) serves both.
-  const int32_t m = a.stage_chunks;
-  const int32_t n_stages = (a.n_chunks + m - 1) / m;
-  const uint32_t stage_bytes = static_cast<uint32_t>(m) * a.chunk_bytes;
-  auto load_stage = [&](int32_t sidx, uint32_t nb) {  // thread 0 only
-    const int32_t first = sidx * m;
-    const int32_t last = (first + m < a.n_chunks ? first + m : a.n_chunks) - 1;
-    const ChunkDesc d0 = a.chunks[first], d1 = a.chunks[last];
-    const uint32_t bytes = static_cast<uint32_t>(d1.offset + d1.nbytes - d0.offset);
-    tma_load_chunk(bar0 + 8 * nb, smem_addr(buf0 + static_cast<size_t>(nb) * stage_bytes), a.image + d0.offset,
-                   bytes);
-  };
-  if (threadIdx.x == 0) load_stage(0, 0);
-  if (single) mbar_wait(bar0, 0);
-  const int64_t total = a.n_turns * n_stages;
-  int64_t turns_done = 0;
-  int64_t gidx = 0;  // global stage counter: buffer = gidx & 1, phase parity = (gidx >> 1) & 1
-  int32_t c = 0;
-  bool any = true;
-  while (gidx < total) {
-    uint32_t cb = 0;
-    if (!single) {
-      if (threadIdx.x == 0 && gidx + 1 < total) {
-        // buffer (gidx+1)&1 was released by the __syncthreads_or that ended iteration gidx-1
-        load_stage((c + 1 == n_stages) ? 0 : c + 1, static_cast<uint32_t>((gidx + 1) & 1));
+    for (int j = 0; j < P; ++j) {
+      const int64_t k = static_cast<int64_t>(j) * blockDim.x + threadIdx.x;
+      const int64_t i = start + k;
+      const bool live = (k < count) && (a.p.state[i] == 1);
+      if (live) {
+        q.x[j] = a.p.x[i];
+        q.px[j] = a.p.px[i];
+        q.y[j] = a.p.y[i];
+        q.py[j] = a.p.py[i];
+        q.zeta[j] = a.p.zeta[i];
+        const double delta = a.p.delta[i];
+        const double ptau = a.p.ptau[i];
+        cold.delta(j) = delta;
+        cold.ptau(j) = ptau;
+        q.alive |= 1u << j;
+        const double opd = 1.0 + delta;
+        const double b = XT_MADD(a.beta0, ptau, 1.0);
+        const double t = XT_MUL(ptau, ptau + a.tib);
+        refresh_cached(cold, j, opd, b, t, a.igam2);
+      } else {
+        q.x[j] = q.px[j] = q.y[j] = q.py[j] = q.zeta[j] = 0.0;
+        cold.opd2(j) = cold.b(j) = 1.0;
+        cold.g(j) = 0.0;
+        cold.ptau(j) = cold.delta(j) = 0.0;
+        cold.rv0v(j) = 1.0;
       }
-      cb = static_cast<uint32_t>(gidx & 1);
-      mbar_wait(bar0 + 8 * cb, static_cast<uint32_t>((gidx >> 1) & 1));
     }
-    const bool warp_alive = __any_sync(0xffffffffu, q.alive != 0);
-    if (single && !warp_alive) break;  // this warp is done; the others do not wait for it
-    if (warp_alive) {
-      const int32_t n_sub = (c * m + m < a.n_chunks ? m : a.n_chunks - c * m);
-      const unsigned char *rp = buf0 + static_cast<size_t>(cb) * stage_bytes;
-      for (int32_t k = 0; k < n_sub; ++k) rp = track_chunk<P, THICK, NFIX>(q, rp, cold, turns_done, a);
-    }
-    ++gidx;
-    if (++c == n_stages) {
-      c = 0;
-      ++turns_done;  // T: turn completed
-    }
-    if (!single) {
-      any = __syncthreads_or(q.alive != 0 ? 1 : 0) != 0;
-      if (!any) break;
-    }
-  }
-  if (!single && !any && gidx < total) {
-    // every particle of the CTA is lost: drain the copy still in flight before exiting
-    mbar_wait(bar0 + 8 * static_cast<uint32_t>(gidx & 1), static_cast<uint32_t>((gidx >> 1) & 1));
-  }
 
-  // W: survivors (lost particles were written when they were lost; rpp, rvv by the cavities)
+    const bool single = (a.n_chunks == 1);
+    if (threadIdx.x == 0) {
+      mbar_init(bar0, 1);
+      mbar_init(bar0 + 8, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    // A stage = stage_chunks consecutive chunks = one bulk copy into one buffer.  A lattice that fits one
+    // chunk is loaded once and stays resident in buffer 0: its warps run free, no CTA-level
+    // synchronisation; otherwise the stages alternate between the two buffers and a __syncthreads_or at
+    // the end of each releases the buffer and tells the CTA whether anyone is still alive.  One loop (and
+    // one copy of the record interpreter in the instruction cache) serves both.
+    const int32_t m = a.stage_chunks;
+    const int32_t n_stages = (a.n_chunks + m - 1) / m;
+    const uint32_t stage_bytes = static_cast<uint32_t>(m) * a.chunk_bytes;
+    auto load_stage = [&](int32_t sidx, uint32_t nb) {  // thread 0 only
+      const int32_t first = sidx * m;
+      const int32_t last = (first + m < a.n_chunks ? first + m : a.n_chunks) - 1;
+      const ChunkDesc d0 = a.chunks[first], d1 = a.chunks[last];
+      const uint32_t bytes = static_cast<uint32_t>(d1.offset + d1.nbytes - d0.offset);
+      tma_load_chunk(bar0 + 8 * nb, smem_addr(buf0 + static_cast<size_t>(nb) * stage_bytes), a.image + d0.offset,
+                     bytes);
+    };
+    if (threadIdx.x == 0) load_stage(0, 0);
+    if (single) mbar_wait(bar0, 0);
+    const int64_t total = a.n_turns * n_stages;
+    int64_t turns_done = 0;
+    int64_t gidx = 0;  // global stage counter: buffer = gidx & 1, phase parity = (gidx >> 1) & 1
+    int32_t c = 0;
+    bool any = true;
+    while (gidx < total) {
+      uint32_t cb = 0;
+      if (!single) {
+        if (threadIdx.x == 0 && gidx + 1 < total) {
+          // buffer (gidx+1)&1 was released by the __syncthreads_or that ended iteration gidx-1
+          load_stage((c + 1 == n_stages) ? 0 : c + 1, static_cast<uint32_t>((gidx + 1) & 1));
+        }
+        cb = static_cast<uint32_t>(gidx & 1);
+        mbar_wait(bar0 + 8 * cb, static_cast<uint32_t>((gidx >> 1) & 1));
+      }
+      const bool warp_alive = __any_sync(0xffffffffu, q.alive != 0);
+      if (single && !warp_alive) break;  // this warp is done; the others do not wait for it
+      if (warp_alive) {
+        const int32_t n_sub = (c * m + m < a.n_chunks ? m : a.n_chunks - c * m);
+        const unsigned char *rp = buf0 + static_cast<size_t>(cb) * stage_bytes;
+        for (int32_t k = 0; k < n_sub; ++k) rp = track_chunk<P, THICK, NFIX>(q, rp, cold, turns_done, a);
+      }
+      ++gidx;
+      if (++c == n_stages) {
+        c = 0;
+        ++turns_done;  // T: turn completed
+      }
+      if (!single) {
+        any = __syncthreads_or(q.alive != 0 ? 1 : 0) != 0;
+        if (!any) break;
+      }
+    }
+    if (!single && !any && gidx < total) {
+      // every particle of the CTA is lost: drain the copy still in flight before exiting
+      mbar_wait(bar0 + 8 * static_cast<uint32_t>(gidx & 1), static_cast<uint32_t>((gidx >> 1) & 1));
+    }
+
+    // W: survivors (lost particles were written when they were lost; rpp, rvv by the cavities)
 #pragma unroll
-  for (int j = 0; j < P; ++j) {
-    if (q.alive & (1u << j)) {
-      const int64_t i = cold.idx(j);
-      a.p.x[i] = q.x[j];
-      a.p.px[i] = q.px[j];
-      a.p.y[i] = q.y[j];
-      a.p.py[i] = q.py[j];
-      a.p.zeta[i] = q.zeta[j];
-      a.p.delta[i] = cold.delta(j);
-      a.p.ptau[i] = cold.ptau(j);
-      a.p.s[i] = 0.0;
-      a.p.at_turn[i] += turns_done;
+    for (int j = 0; j < P; ++j) {
+      if (q.alive & (1u << j)) {
+        const int64_t i = cold.idx(j);
+        a.p.x[i] = q.x[j];
+        a.p.px[i] = q.px[j];
+        a.p.y[i] = q.y[j];
+        a.p.py[i] = q.py[j];
+        a.p.zeta[i] = q.zeta[j];
+        a.p.delta[i] = cold.delta(j);
+        a.p.ptau[i] = cold.ptau(j);
+        a.p.s[i] = 0.0;
+        a.p.at_turn[i] += turns_done;
+      }
+    }
+  } else {
+    // The small-ensemble shapes (cold state in registers): the same, or the balanced mode.
+    // Balanced mode (compiled into the shapes that keep the cold state in registers: the one-wave
+    // ensembles).  An ensemble of G groups on S resident CTAs, G / S not an integer, leaves lanes or whole
+    // CTA slots empty for the whole run when every CTA owns its particles (configs[2]: 5.28 warp-slots per
+    // scheduler run as 6).  Here the work is cut into items (group g of blockDim.x * P particles, block k of
+    // a few turns) and the launch has one CTA per item; the hardware starts a CTA whenever a slot is free.
+    // A first-in first-out queue in device memory holds the groups that are ready for their next block:
+    // the first G pop tickets are block 0 of each group; a CTA that has stored block k of a group pushes
+    // the group's next item, and pop ticket G + n takes push number n (spinning until it is there).  A
+    // group in the queue is taken by the next CTA that starts, so no group waits while an SM has room, and
+    // an SM on which a CTA waits runs its other CTAs faster: the load evens out over the run.  Tickets are
+    // taken in the order the CTAs start and every push is made by a running CTA, so nothing can deadlock.
+    // The state of a group goes through HBM between its blocks.
+    // queue[0]: pop tickets, queue[1]: pushes, queue[2 + n]: item of push n, plus one (0: not there yet).
+    const bool queued = a.queue != nullptr;
+    __shared__ unsigned int s_item;
+    int64_t start, count, n_turns, t0 = 0;
+    unsigned int item = 0;
+    if (queued) {
+      if (threadIdx.x == 0) {
+        const unsigned int my = atomicAdd(a.queue, 1u);
+        unsigned int it = my;
+        if (my >= static_cast<unsigned int>(a.n_groups)) {
+          const unsigned int *slot = a.queue + 2 + (my - static_cast<unsigned int>(a.n_groups));
+          unsigned int v;
+          for (;;) {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(slot) : "memory");
+            if (v != 0u) break;
+            __nanosleep(256);
+          }
+          __threadfence();
+          it = v - 1u;
+        }
+        s_item = it;
+      }
+      __syncthreads();
+      item = s_item;
+      const unsigned int grp = item % static_cast<unsigned int>(a.n_groups);
+      const unsigned int blk = item / static_cast<unsigned int>(a.n_groups);
+      const int64_t cap = static_cast<int64_t>(blockDim.x) * P;
+      start = static_cast<int64_t>(grp) * cap;
+      count = (a.n_part - start < cap) ? a.n_part - start : cap;
+      const int64_t l0 = first_block_turns(grp, a.block_turns);
+      t0 = blk == 0 ? 0 : l0 + static_cast<int64_t>(blk - 1) * a.block_turns;
+      const int64_t len = blk == 0 ? l0 : static_cast<int64_t>(a.block_turns);
+      n_turns = (a.n_turns - t0 < len) ? a.n_turns - t0 : len;
+    } else {
+      // Balanced hand-out (device side, so that compaction's device counter needs no host
+      // sync): use as few CTAs as hold n_active particles, rounded up to a whole number per SM,
+      // and give each the same share.
+      const int64_t n_active = a.n_active ? *a.n_active : a.n_part;
+      const int64_t cap = static_cast<int64_t>(blockDim.x) * P;
+      const int64_t need = (n_active + cap - 1) / cap;
+      int64_t used = ((need + a.grid_quantum - 1) / a.grid_quantum) * a.grid_quantum;
+      if (used > static_cast<int64_t>(gridDim.x)) used = gridDim.x;
+      if (static_cast<int64_t>(blockIdx.x) >= used) return;  // CTA-uniform
+      const int64_t share = (n_active + used - 1) / used;
+      start = static_cast<int64_t>(blockIdx.x) * share;
+      if (start >= n_active) return;  // CTA-uniform
+      count = (n_active - start < share) ? n_active - start : share;
+      n_turns = a.n_turns;
+    }
+
+    Parts<P> q;
+    cold.first = start + threadIdx.x;
+    q.alive = 0;
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+      const int64_t k = static_cast<int64_t>(j) * blockDim.x + threadIdx.x;
+      const int64_t i = start + k;
+      const bool live = (k < count) && (__ldcg(a.p.state + i) == 1);
+      if (live) {
+        q.x[j] = __ldcg(a.p.x + i);
+        q.px[j] = __ldcg(a.p.px + i);
+        q.y[j] = __ldcg(a.p.y + i);
+        q.py[j] = __ldcg(a.p.py + i);
+        q.zeta[j] = __ldcg(a.p.zeta + i);
+        const double delta = __ldcg(a.p.delta + i);
+        const double ptau = __ldcg(a.p.ptau + i);
+        cold.delta(j) = delta;
+        cold.ptau(j) = ptau;
+        q.alive |= 1u << j;
+        const double opd = 1.0 + delta;
+        const double b = XT_MADD(a.beta0, ptau, 1.0);
+        const double t = XT_MUL(ptau, ptau + a.tib);
+        refresh_cached(cold, j, opd, b, t, a.igam2);
+      } else {
+        q.x[j] = q.px[j] = q.y[j] = q.py[j] = q.zeta[j] = 0.0;
+        cold.opd2(j) = cold.b(j) = 1.0;
+        cold.g(j) = 0.0;
+        cold.ptau(j) = cold.delta(j) = 0.0;
+        cold.rv0v(j) = 1.0;
+      }
+    }
+
+    const bool single = (a.n_chunks == 1);
+    if (threadIdx.x == 0) {
+      mbar_init(bar0, 1);
+      mbar_init(bar0 + 8, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    // A stage = stage_chunks consecutive chunks = one bulk copy into one buffer.  A lattice that fits one
+    // chunk is loaded once and stays resident in buffer 0: its warps run free, no CTA-level
+    // synchronisation; otherwise the stages alternate between the two buffers and a __syncthreads_or at
+    // the end of each releases the buffer and tells the CTA whether anyone is still alive.  One loop (and
+    // one copy of the record interpreter in the instruction cache) serves both.
+    const int32_t m = a.stage_chunks;
+    const int32_t n_stages = (a.n_chunks + m - 1) / m;
+    const uint32_t stage_bytes = static_cast<uint32_t>(m) * a.chunk_bytes;
+    auto load_stage = [&](int32_t sidx, uint32_t nb) {  // thread 0 only
+      const int32_t first = sidx * m;
+      const int32_t last = (first + m < a.n_chunks ? first + m : a.n_chunks) - 1;
+      const ChunkDesc d0 = a.chunks[first], d1 = a.chunks[last];
+      const uint32_t bytes = static_cast<uint32_t>(d1.offset + d1.nbytes - d0.offset);
+      tma_load_chunk(bar0 + 8 * nb, smem_addr(buf0 + static_cast<size_t>(nb) * stage_bytes), a.image + d0.offset,
+                     bytes);
+    };
+    if (threadIdx.x == 0) load_stage(0, 0);
+    if (single) mbar_wait(bar0, 0);
+    const int64_t total = n_turns * n_stages;
+    int64_t turns_done = 0;
+    int64_t gidx = 0;  // global stage counter: buffer = gidx & 1, phase parity = (gidx >> 1) & 1
+    int32_t c = 0;
+    bool any = true;
+    while (gidx < total) {
+      uint32_t cb = 0;
+      if (!single) {
+        if (threadIdx.x == 0 && gidx + 1 < total) {
+          // buffer (gidx+1)&1 was released by the __syncthreads_or that ended iteration gidx-1
+          load_stage((c + 1 == n_stages) ? 0 : c + 1, static_cast<uint32_t>((gidx + 1) & 1));
+        }
+        cb = static_cast<uint32_t>(gidx & 1);
+        mbar_wait(bar0 + 8 * cb, static_cast<uint32_t>((gidx >> 1) & 1));
+      }
+      const bool warp_alive = __any_sync(0xffffffffu, q.alive != 0);
+      if (single && !warp_alive) break;  // this warp is done; the others do not wait for it
+      if (warp_alive) {
+        const int32_t n_sub = (c * m + m < a.n_chunks ? m : a.n_chunks - c * m);
+        const unsigned char *rp = buf0 + static_cast<size_t>(cb) * stage_bytes;
+        for (int32_t k = 0; k < n_sub; ++k) rp = track_chunk<P, THICK, NFIX>(q, rp, cold, turns_done, a);
+      }
+      ++gidx;
+      if (++c == n_stages) {
+        c = 0;
+        ++turns_done;  // T: turn completed
+      }
+      if (!single) {
+        any = __syncthreads_or(q.alive != 0 ? 1 : 0) != 0;
+        if (!any) break;
+      }
+    }
+    if (!single && !any && gidx < total) {
+      // every particle of the CTA is lost: drain the copy still in flight before exiting
+      mbar_wait(bar0 + 8 * static_cast<uint32_t>(gidx & 1), static_cast<uint32_t>((gidx >> 1) & 1));
+    }
+
+    // W: survivors (lost particles were written when they were lost; rpp, rvv by the cavities)
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+      if (q.alive & (1u << j)) {
+        const int64_t i = cold.idx(j);
+        a.p.x[i] = q.x[j];
+        a.p.px[i] = q.px[j];
+        a.p.y[i] = q.y[j];
+        a.p.py[i] = q.py[j];
+        a.p.zeta[i] = q.zeta[j];
+        a.p.delta[i] = cold.delta(j);
+        a.p.ptau[i] = cold.ptau(j);
+        a.p.s[i] = 0.0;
+        a.p.at_turn[i] = __ldcg(a.p.at_turn + i) + turns_done;
+      }
+    }
+    if (queued) {
+      // publish: every thread's stores, then the group's next item (release)
+      __syncthreads();
+      if (threadIdx.x == 0 && t0 + n_turns < a.n_turns) {
+        __threadfence();
+        const unsigned int n = atomicAdd(a.queue + 1, 1u);
+        const unsigned int next = item + static_cast<unsigned int>(a.n_groups) + 1u;
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(a.queue + 2 + n), "r"(next) : "memory");
+      }
     }
   }
 }
@@ -1161,26 +1362,53 @@ int kernel_registers(int device, int *regs) {
   return XT_OK;
 }
 
+// Items of the balanced mode: about this many lattice records each (configs[2]: 4 turns, 9 ms), at most
+// kMaxBlocks blocks of turns per launch (the queue has one word per item), at least four, and more groups
+// than SMs (else every CTA has an SM of its own).
+constexpr int64_t kItemRecords = 12000;
+constexpr int64_t kMaxBlocks = 256;
+constexpr int64_t kMinBlocks = 4;
+
 template <int P, bool THICK, bool REG, int NFIX>
-int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
+int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, int balance, cudaStream_t st) {
   const size_t cold_bytes =
       (static_cast<size_t>(8 * Cold<P, REG>::kPitch) * block + 127) & ~static_cast<size_t>(127);
   const int64_t cap = static_cast<int64_t>(block) * P;
   const int64_t need = (a.n_part + cap - 1) / cap;
-  const int64_t grid = ((need + a.grid_quantum - 1) / a.grid_quantum) * a.grid_quantum;
+  int64_t grid = ((need + a.grid_quantum - 1) / a.grid_quantum) * a.grid_quantum;
   if (grid > 2147483647LL) {
     set_error("xt_track: too many particles for one launch");
     return XT_ERR_INVALID_ARG;
   }
-  // Staging depth: as many chunks per bulk copy (fewer CTA-wide barriers per turn) as shared memory
-  // allows without taking a resident CTA away.
   int regs = 128;
   const int rc = kernel_registers<P, THICK, REG, NFIX>(lat->device, &regs);
   if (rc != XT_OK) return rc;
-  int64_t resident = 65536 / (static_cast<int64_t>(regs) * block);
-  if (resident > grid / a.grid_quantum) resident = grid / a.grid_quantum;
-  if (resident < 1) resident = 1;
+  const int64_t by_regs = 65536 / (static_cast<int64_t>(regs) * block) > 0 ? 65536 / (static_cast<int64_t>(regs) * block) : 1;
   TrackArgs b = a;
+  if (!REG) b.queue = nullptr;
+  if (b.queue) {
+    const int64_t t = balance_block_turns(lat, a.n_turns, balance);
+    const int64_t n_blocks = (a.n_turns + t - 1) / t;
+    const bool worth = balance > 0 || (n_blocks >= kMinBlocks && need > a.grid_quantum);
+    if (worth && need * (n_blocks + 1) < 2000000000LL && t < 2000000000LL && need < 4000000) {
+      b.n_groups = static_cast<int32_t>(need);
+      b.block_turns = static_cast<int32_t>(t);
+      b.n_items = 0;  // a staggered first item, then blocks of t turns
+      for (int64_t g = 0; g < need; ++g) {
+        const int64_t l0 = first_block_turns(static_cast<uint32_t>(g), t);
+        b.n_items += 1 + (a.n_turns > l0 ? (a.n_turns - l0 + t - 1) / t : 0);
+      }
+      grid = b.n_items;  // one CTA per item; the hardware starts them as slots become free
+    } else {
+      b.queue = nullptr;
+    }
+  }
+  // Staging depth: as many chunks per bulk copy (fewer CTA-wide barriers per turn) as shared memory
+  // allows without taking a resident CTA away.
+  int64_t resident = by_regs;
+  const int64_t per_sm = (grid + a.grid_quantum - 1) / a.grid_quantum;
+  if (resident > per_sm) resident = per_sm;
+  if (resident < 1) resident = 1;
   b.stage_chunks = 1;
   const size_t chunk = static_cast<size_t>(lat->info.chunk_bytes);
   auto smem_for = [&](int m) { return 128 + 64 + cold_bytes + (lat->info.n_chunks == 1 ? 1 : 2) * m * chunk; };
@@ -1204,28 +1432,52 @@ int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, cudaSt
 constexpr int kFixedOrder = 15;       // configs[2-4]: every magnet carries errors up to order 15
 constexpr int kFixedLow = 1 | (2 << 5);  // thin quadrupoles and sextupoles (configs[0], [1]): orders 1 and 2
 template <int P, bool REG>
-int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, cudaStream_t st) {
+int launch_track_p(const TrackArgs &a, const xt_lattice *lat, int block, int balance, cudaStream_t st) {
   constexpr bool kHasFixed = (P >= 3) || REG;  // which shapes exist with the unrolled order-15 handlers
   if (kHasFixed && lat->fixed_order == kFixedOrder) {
     constexpr int NF = kHasFixed ? kFixedOrder : 0;
-    return lat->extended ? launch_track_pt<P, true, REG, NF>(a, lat, block, st)
-                         : launch_track_pt<P, false, REG, NF>(a, lat, block, st);
+    return lat->extended ? launch_track_pt<P, true, REG, NF>(a, lat, block, balance, st)
+                         : launch_track_pt<P, false, REG, NF>(a, lat, block, balance, st);
   }
   if (!REG && lat->fixed_order == kFixedLow) {
     constexpr int NF = REG ? 0 : kFixedLow;
-    return lat->extended ? launch_track_pt<P, true, REG, NF>(a, lat, block, st)
-                         : launch_track_pt<P, false, REG, NF>(a, lat, block, st);
+    return lat->extended ? launch_track_pt<P, true, REG, NF>(a, lat, block, balance, st)
+                         : launch_track_pt<P, false, REG, NF>(a, lat, block, balance, st);
   }
-  return lat->extended ? launch_track_pt<P, true, REG, 0>(a, lat, block, st)
-                       : launch_track_pt<P, false, REG, 0>(a, lat, block, st);
+  return lat->extended ? launch_track_pt<P, true, REG, 0>(a, lat, block, balance, st)
+                       : launch_track_pt<P, false, REG, 0>(a, lat, block, balance, st);
 }
 
 }  // namespace
 
 // ppt: particles per thread (1, 2, 3, 4); cold_in_regs: the cold per-particle state in registers
 // instead of shared memory (instantiated for 3 particles per thread: the small-ensemble shape).
+int64_t balance_block_turns(const xt_lattice *lat, int64_t n_turns, int balance) {
+  const int64_t rec = lat->info.n_records > 0 ? lat->info.n_records : 1;
+  int64_t t = balance > 1 ? balance : (kItemRecords + rec - 1) / rec;
+  if (t < (n_turns + kMaxBlocks - 1) / kMaxBlocks) t = (n_turns + kMaxBlocks - 1) / kMaxBlocks;
+  if (t > n_turns) t = n_turns;
+  return t > 0 ? t : 1;
+}
+
+bool balance_pays(const xt_lattice *lat, int64_t n_turns, int balance) {
+  if (balance < 0 || n_turns <= 0) return false;
+  if (balance > 0) return true;
+  // the shapes with the cold state in registers have no handlers with the orders 1 and 2 fixed
+  if (lat->fixed_order == kFixedLow) return false;
+  const int64_t t = balance_block_turns(lat, n_turns, balance);
+  return (n_turns + t - 1) / t >= kMinBlocks;
+}
+
+size_t balance_scratch_bytes(int64_t n_part, int block, int ppt) {
+  const int64_t cap = static_cast<int64_t>(block) * ppt;
+  const int64_t need = cap > 0 ? (n_part + cap - 1) / cap : 0;
+  return (static_cast<size_t>(need * kMaxBlocks + 2) * sizeof(unsigned int) + 255) & ~static_cast<size_t>(255);
+}
+
 int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, const int64_t *d_n_active,
-                 int64_t n_turns, int block, int ppt, bool cold_in_regs, cudaStream_t st) {
+                 int64_t n_turns, int block, int ppt, bool cold_in_regs, cudaStream_t st, unsigned int *queue,
+                 int balance) {
   if (n_part <= 0 || n_turns <= 0) return XT_OK;
   TrackArgs a;
   a.image = lat->d_image;
@@ -1242,22 +1494,29 @@ int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, c
   a.beta0 = lat->k.beta0;
   a.tib = lat->k.tib;
   a.igam2 = lat->k.igam2;
+  a.queue = (cold_in_regs && !d_n_active && balance >= 0) ? queue : nullptr;
+  a.n_groups = 0;
+  a.block_turns = 0;
+  a.n_items = 0;
+  if (a.queue) {  // tickets and per-group counters start from zero
+    XT_CUDA(cudaMemsetAsync(a.queue, 0, balance_scratch_bytes(n_part, block, ppt), st));
+  }
   if (cold_in_regs) {
-    if (ppt == 1) return launch_track_p<1, true>(a, lat, block, st);
-    if (ppt == 2) return launch_track_p<2, true>(a, lat, block, st);
-    if (ppt == 3) return launch_track_p<3, true>(a, lat, block, st);
+    if (ppt == 1) return launch_track_p<1, true>(a, lat, block, balance, st);
+    if (ppt == 2) return launch_track_p<2, true>(a, lat, block, balance, st);
+    if (ppt == 3) return launch_track_p<3, true>(a, lat, block, balance, st);
     set_error("xt_track: cold_in_registers needs 1, 2 or 3 particles per thread");
     return XT_ERR_INVALID_ARG;
   }
   switch (ppt) {
     case 1:
-      return launch_track_p<1, false>(a, lat, block, st);
+      return launch_track_p<1, false>(a, lat, block, balance, st);
     case 2:
-      return launch_track_p<2, false>(a, lat, block, st);
+      return launch_track_p<2, false>(a, lat, block, balance, st);
     case 3:
-      return launch_track_p<3, false>(a, lat, block, st);
+      return launch_track_p<3, false>(a, lat, block, balance, st);
     case 4:
-      return launch_track_p<4, false>(a, lat, block, st);
+      return launch_track_p<4, false>(a, lat, block, balance, st);
     default:
       set_error("xt_track: particles_per_thread must be 1, 2, 3 or 4");
       return XT_ERR_INVALID_ARG;

@@ -301,6 +301,60 @@ def test_launch_shape_fusion_and_chunk_size_do_not_change_results(X):
         lat2.close()
 
 
+def test_balanced_mode_is_bit_identical(X):
+    """xt_track_opts.balance: persistent CTAs that draw (group of particles, block of
+    turns) items from a ticket counter, the state of a group passing through HBM between its blocks.  Only
+    the schedule changes: every variant reproduces the unbalanced launch bit for bit -- multi-chunk and
+    single-chunk lattices, losses spread over the turns (at_turn, at_element and s of the lost included), a
+    ragged last group and a ragged last block of turns, both builds, scratch from the caller's workspace."""
+    import torch
+    full = C.particles(4)
+    idx = np.linspace(0, len(full["x"]) - 1, 5003).astype(np.int64)
+    coords = C.subsample(full, idx)
+    for kind in ("prod", "nofma"):
+        lat = X.xt_lattice_create(packed(4), kind=kind)                 # 8 606 elements, many chunks, apertures
+        base = X.new_particles(lat, coords)
+        X.xt_track_ex(lat, base, 11, compact_every=-1, balance=-1)
+        base = X.particles_to_host(base)
+        lost = base["state"] == 0
+        assert 0.05 < lost.mean() < 0.95 and len(np.unique(base["at_turn"][lost])) >= 5
+        for ppt, block, bal in ((2, 128, 2), (2, 64, 3), (1, 32, 4), (3, 96, 2), (2, 128, 1), (2, 256, 11), (1, 64, 12)):
+            p = X.new_particles(lat, coords)
+            X.xt_track_ex(lat, p, 11, compact_every=-1, particles_per_thread=ppt, block_size=block,
+                          cold_in_registers=1, balance=bal)
+            assert_bit_identical(X.particles_to_host(p), base)
+        # split over several launches, each balanced; scratch taken from a caller's workspace
+        ws = torch.empty(X.xt_track_workspace_bytes(len(idx)), dtype=torch.uint8, device="cuda")
+        ws.fill_(0xCD)                                                  # stale bytes must not matter
+        p = X.new_particles(lat, coords)
+        X.xt_track_ex(lat, p, 11, compact_every=-1, particles_per_thread=2, block_size=128, cold_in_registers=1,
+                      balance=2, turns_per_launch=5, workspace=ws)
+        assert_bit_identical(X.particles_to_host(p), base)
+        # the auto shape of a one-wave ensemble (2 per thread, registers) with the auto rule
+        p = X.new_particles(lat, coords)
+        X.xt_track_ex(lat, p, 11, compact_every=-1)
+        assert_bit_identical(X.particles_to_host(p), base)
+        with pytest.raises(X.XtError) as e:                            # needs the cold state in registers
+            X.xt_track_ex(lat, X.new_particles(lat, coords), 3, cold_in_registers=-1, particles_per_thread=2, balance=1)
+        assert e.value.code == -1
+        with pytest.raises(X.XtError) as e:                            # forced, but the workspace cannot hold the queue
+            X.xt_track_ex(lat, X.new_particles(lat, coords), 3, cold_in_registers=1, particles_per_thread=2, balance=1,
+                          workspace=ws[:256])
+        assert e.value.code == -1
+        lat.close()
+    # single-chunk lattice (warps run free inside an item), continuing a run
+    coords1 = C.subsample(C.particles_cfg1(sigma=1e-3), slice(0, None, 97))
+    lat = X.xt_lattice_create(packed(1))
+    a, b = X.new_particles(lat, coords1), X.new_particles(lat, coords1)
+    X.xt_track_ex(lat, a, 50, balance=-1)
+    X.xt_track_ex(lat, b, 20, particles_per_thread=2, block_size=64, cold_in_registers=1, balance=7)
+    X.xt_track_ex(lat, b, 30, particles_per_thread=1, block_size=128, cold_in_registers=1, balance=4)
+    ha = X.particles_to_host(a)
+    assert (ha["state"] == 0).any()
+    assert_bit_identical(X.particles_to_host(b), ha)
+    lat.close()
+
+
 def test_launch_shapes_on_a_quadrupole_sextupole_lattice(X):
     """configs[1b] (orders 1 and 2 only: the kernels with those two orders fixed; single chunk, losses): every
     launch shape and both homes of the cold state reproduce the default bit for bit, in both builds; the
