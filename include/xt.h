@@ -211,7 +211,7 @@ uint64_t xt_track_workspace_bytes(int64_t n_part);
  * instead of a stream-ordered allocation.  The call makes no cudaMalloc / cudaFree /
  * cudaMallocAsync and calls no allocating library routine.
  *   - n_part <= XT_TRACK_STATIC_MAX_PARTICLES, else XT_ERR_INVALID_ARG (xt_last_error names the
- *     limit).  The array is 7.0 MiB (xt_track_workspace_bytes of the limit); every GPU that
+ *     limit).  The array is 7.0 MiB (the working sets of step C for the limit); every GPU that
  *     loads the library holds it until the process exits.
  *   - opts may be NULL; opts->workspace, ->workspace_bytes and ->stats must be 0 / NULL (the
  *     stats record creates events and allocates): XT_ERR_INVALID_ARG otherwise.

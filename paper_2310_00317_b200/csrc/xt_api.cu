@@ -63,12 +63,15 @@ struct Shape {
   int block, ppt;
   bool cold_in_regs;
 };
-int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part, bool can_balance, Shape *sh) {
+int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part, bool can_balance, bool compacting,
+                  Shape *sh) {
   const int64_t per_sm = n_part / (lat->n_sm > 0 ? lat->n_sm : 1);
+  // with compaction n_part is only the bound of what is still alive: lean towards the balanced shapes
+  const int64_t balanced_up_to = compacting ? 16384 : 12288;
   int auto_ppt = 4, auto_block = 128;
   bool auto_regs = false;
   if (per_sm < 4096) auto_ppt = 3;
-  if (can_balance && per_sm <= 12288) {
+  if (can_balance && per_sm <= balanced_up_to) {
     auto_ppt = 3;
     auto_regs = true;
   }
@@ -227,9 +230,10 @@ static int xt_track_ex_impl(const xt_lattice *lat, const xt_particles *p, int64_
   const int64_t tpl_opt = opts ? opts->turns_per_launch : 0;
   // the balanced mode needs launches of several blocks of turns and a particle count known to the host
   const int64_t launch_turns = (tpl_opt > 0 && tpl_opt < n_turns) ? tpl_opt : n_turns;
-  const bool can_balance = period == 0 && xt::balance_pays(lat, launch_turns, opts ? opts->balance : 0);
+  const int64_t kernel_turns = (period > 0 && launch_turns > period) ? period : launch_turns;
+  const bool can_balance = xt::balance_pays(lat, kernel_turns, opts ? opts->balance : 0);
   xt::Shape sh{};
-  if ((rc = xt::resolve_shape(opts, lat, n_part, can_balance, &sh)) != XT_OK) return rc;
+  if ((rc = xt::resolve_shape(opts, lat, n_part, can_balance, period > 0, &sh)) != XT_OK) return rc;
 
   xt::StatsTimer tm(opts ? opts->stats : nullptr, st);
   if (period == 0) {
@@ -272,13 +276,28 @@ static int xt_track_ex_impl(const xt_lattice *lat, const xt_particles *p, int64_
   }
 
   void *ws = opts ? opts->workspace : nullptr;
-  const size_t ws_bytes = xt::compaction_workspace_bytes(n_part);
+  const size_t c_bytes = xt::compaction_workspace_bytes(n_part);
+  // the balanced mode's queue sits behind the working sets when the shape can use it and there is room
+  const int balance = opts ? opts->balance : 0;
+  size_t q_bytes = (sh.cold_in_regs && can_balance) ? xt::balance_scratch_bytes(n_part, sh.block, sh.ppt) : 0;
   const bool own_ws = (ws == nullptr);
-  if (!own_ws && (opts->workspace_bytes < ws_bytes || (reinterpret_cast<uintptr_t>(ws) & 255u))) {
+  if (!own_ws && (opts->workspace_bytes < c_bytes || (reinterpret_cast<uintptr_t>(ws) & 255u))) {
     xt::set_error("xt_track_ex: workspace too small (see xt_track_workspace_bytes) or not 256-byte aligned");
     return XT_ERR_INVALID_ARG;
   }
-  if (own_ws) XT_CUDA(cudaMallocAsync(&ws, ws_bytes, st));
+  if (!own_ws && opts->workspace_bytes < c_bytes + q_bytes) {
+    if (balance > 0) {
+      xt::set_error("xt_track_ex: workspace too small for the balanced mode with this launch shape");
+      return XT_ERR_INVALID_ARG;
+    }
+    q_bytes = 0;
+  }
+  if (balance > 0 && !sh.cold_in_regs) {
+    xt::set_error("xt_track_ex: balance > 0 needs the cold state in registers (cold_in_registers = 1, or the auto shape of small ensembles)");
+    return XT_ERR_INVALID_ARG;
+  }
+  if (own_ws) XT_CUDA(cudaMallocAsync(&ws, c_bytes + q_bytes, st));
+  unsigned int *queue = q_bytes ? reinterpret_cast<unsigned int *>(static_cast<unsigned char *>(ws) + c_bytes) : nullptr;
   xt::CompactPlan plan;
   xt::plan_compaction(ws, n_part, plan);
   auto bail = [&](int code) {
@@ -297,7 +316,9 @@ static int xt_track_ex_impl(const xt_lattice *lat, const xt_particles *p, int64_
     if (k > tpl) k = tpl;
     if (k > period - since) k = period - since;
     tm.begin();
-    if ((rc = xt::launch_track(lat, plan.w[cur].p, n_part, plan.n_active, k, sh.block, sh.ppt, sh.cold_in_regs, st)) != XT_OK) return bail(rc);
+    if ((rc = xt::launch_track(lat, plan.w[cur].p, n_part, plan.n_active, k, sh.block, sh.ppt, sh.cold_in_regs, st, queue,
+                               balance)) != XT_OK)
+      return bail(rc);
     tm.end_track();
     done += k;
     since += k;
@@ -320,7 +341,9 @@ static int xt_track_ex_impl(const xt_lattice *lat, const xt_particles *p, int64_
 }
 
 extern "C" uint64_t xt_track_workspace_bytes(int64_t n_part) {
-  return n_part > 0 ? static_cast<uint64_t>(xt::compaction_workspace_bytes(n_part)) : 0;
+  // the working sets of step C, and behind them the queue of the balanced mode for the auto shapes
+  return n_part > 0 ? static_cast<uint64_t>(xt::compaction_workspace_bytes(n_part) + xt::balance_scratch_bytes(n_part, 128, 2))
+                    : 0;
 }
 
 extern "C" int xt_track(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,

@@ -65,7 +65,7 @@ struct TrackArgs {
   double beta0, tib, igam2;
   // Balanced mode (cold-state-in-registers shapes only; nullptr otherwise): the CTAs are persistent and
   // draw (group of particles, block of turns) items from a first-in first-out queue.  queue[0]: pop
-  // tickets; queue[1]: pushes; queue[2 + n]: item of push n, plus one.
+  // tickets; queue[1]: pushes; queue[2]: finished groups; queue[4 + n]: item of push n, plus one.
   unsigned int *queue;
   int32_t n_groups;     // groups of blockDim.x * P particles
   int32_t block_turns;  // turns per item
@@ -1150,35 +1150,51 @@ __global__ void __maxnreg__((RegBudget<P, REG, THICK>::value)) xt_track_kernel(c
     // an SM on which a CTA waits runs its other CTAs faster: the load evens out over the run.  Tickets are
     // taken in the order the CTAs start and every push is made by a running CTA, so nothing can deadlock.
     // The state of a group goes through HBM between its blocks.
-    // queue[0]: pop tickets, queue[1]: pushes, queue[2 + n]: item of push n, plus one (0: not there yet).
+    // queue[0]: pop tickets, queue[1]: pushes, queue[2]: groups that are through, queue[4 + n]: item of push n,
+  // plus one (0: not there yet).
     const bool queued = a.queue != nullptr;
     __shared__ unsigned int s_item;
     int64_t start, count, n_turns, t0 = 0;
-    unsigned int item = 0;
+    unsigned int item = 0, n_groups = 0;
     if (queued) {
+      // with compaction the number of particles (and of groups) is a device counter; the launch then has
+      // CTAs for the largest number of items there can be, and the ones left over leave when every group
+      // has done its last block (queue[2])
+      const int64_t cap = static_cast<int64_t>(blockDim.x) * P;
+      const int64_t n_act = a.n_active ? *a.n_active : a.n_part;
+      n_groups = static_cast<unsigned int>((n_act + cap - 1) / cap);
       if (threadIdx.x == 0) {
         const unsigned int my = atomicAdd(a.queue, 1u);
         unsigned int it = my;
-        if (my >= static_cast<unsigned int>(a.n_groups)) {
-          const unsigned int *slot = a.queue + 2 + (my - static_cast<unsigned int>(a.n_groups));
-          unsigned int v;
+        if (my >= n_groups) {
+          const unsigned int *slot = a.queue + 4 + (my - n_groups);
+          it = 0xffffffffu;
           for (;;) {
+            unsigned int v, fin;
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(slot) : "memory");
-            if (v != 0u) break;
+            if (v != 0u) {
+              it = v - 1u;
+              break;
+            }
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(fin) : "l"(a.queue + 2) : "memory");
+            if (fin >= n_groups) {  // nothing will be pushed any more (a push precedes the count it enables)
+              asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(slot) : "memory");
+              if (v != 0u) it = v - 1u;
+              break;
+            }
             __nanosleep(256);
           }
           __threadfence();
-          it = v - 1u;
         }
         s_item = it;
       }
       __syncthreads();
       item = s_item;
-      const unsigned int grp = item % static_cast<unsigned int>(a.n_groups);
-      const unsigned int blk = item / static_cast<unsigned int>(a.n_groups);
-      const int64_t cap = static_cast<int64_t>(blockDim.x) * P;
+      if (item == 0xffffffffu) return;  // CTA-uniform: a CTA left over
+      const unsigned int grp = item % n_groups;
+      const unsigned int blk = item / n_groups;
       start = static_cast<int64_t>(grp) * cap;
-      count = (a.n_part - start < cap) ? a.n_part - start : cap;
+      count = (n_act - start < cap) ? n_act - start : cap;
       const int64_t l0 = first_block_turns(grp, a.block_turns);
       t0 = blk == 0 ? 0 : l0 + static_cast<int64_t>(blk - 1) * a.block_turns;
       const int64_t len = blk == 0 ? l0 : static_cast<int64_t>(a.block_turns);
@@ -1311,13 +1327,17 @@ __global__ void __maxnreg__((RegBudget<P, REG, THICK>::value)) xt_track_kernel(c
       }
     }
     if (queued) {
-      // publish: every thread's stores, then the group's next item (release)
+      // publish: every thread's stores, then the group's next item (release), or one group fewer to wait for
       __syncthreads();
-      if (threadIdx.x == 0 && t0 + n_turns < a.n_turns) {
+      if (threadIdx.x == 0) {
         __threadfence();
-        const unsigned int n = atomicAdd(a.queue + 1, 1u);
-        const unsigned int next = item + static_cast<unsigned int>(a.n_groups) + 1u;
-        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(a.queue + 2 + n), "r"(next) : "memory");
+        if (t0 + n_turns < a.n_turns) {
+          const unsigned int n = atomicAdd(a.queue + 1, 1u);
+          const unsigned int next = item + n_groups + 1u;
+          asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(a.queue + 4 + n), "r"(next) : "memory");
+        } else {
+          atomicAdd(a.queue + 2, 1u);
+        }
       }
     }
   }
@@ -1472,7 +1492,7 @@ bool balance_pays(const xt_lattice *lat, int64_t n_turns, int balance) {
 size_t balance_scratch_bytes(int64_t n_part, int block, int ppt) {
   const int64_t cap = static_cast<int64_t>(block) * ppt;
   const int64_t need = cap > 0 ? (n_part + cap - 1) / cap : 0;
-  return (static_cast<size_t>(need * kMaxBlocks + 2) * sizeof(unsigned int) + 255) & ~static_cast<size_t>(255);
+  return (static_cast<size_t>(need * kMaxBlocks + 4) * sizeof(unsigned int) + 255) & ~static_cast<size_t>(255);
 }
 
 int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, const int64_t *d_n_active,
@@ -1494,7 +1514,7 @@ int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, c
   a.beta0 = lat->k.beta0;
   a.tib = lat->k.tib;
   a.igam2 = lat->k.igam2;
-  a.queue = (cold_in_regs && !d_n_active && balance >= 0) ? queue : nullptr;
+  a.queue = (cold_in_regs && balance >= 0) ? queue : nullptr;
   a.n_groups = 0;
   a.block_turns = 0;
   a.n_items = 0;

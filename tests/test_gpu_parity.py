@@ -330,6 +330,17 @@ def test_balanced_mode_is_bit_identical(X):
         X.xt_track_ex(lat, p, 11, compact_every=-1, particles_per_thread=2, block_size=128, cold_in_registers=1,
                       balance=2, turns_per_launch=5, workspace=ws)
         assert_bit_identical(X.particles_to_host(p), base)
+        # with loss compaction: the number of groups is then a device counter and the launch has CTAs to spare
+        for ppt, block, bal, every in ((2, 128, 2, 4), (3, 64, 1, 3), (1, 32, 3, 5)):
+            p = X.new_particles(lat, coords)
+            st = X.xt_track_ex(lat, p, 11, compact_every=every, particles_per_thread=ppt, block_size=block,
+                               cold_in_registers=1, balance=bal, stats=True)
+            assert st["n_passes"] >= 2
+            assert_bit_identical(X.particles_to_host(p), base)
+        p = X.new_particles(lat, coords)                                 # ... in a caller's workspace
+        X.xt_track_ex(lat, p, 11, compact_every=4, particles_per_thread=2, block_size=128, cold_in_registers=1,
+                      balance=2, workspace=ws)
+        assert_bit_identical(X.particles_to_host(p), base)
         # the auto shape of a one-wave ensemble (2 per thread, registers) with the auto rule
         p = X.new_particles(lat, coords)
         X.xt_track_ex(lat, p, 11, compact_every=-1)
