@@ -119,8 +119,8 @@ typedef struct {
   int32_t particles_per_thread; /* 0: auto; else 1, 2, 3 or 4                                 */
   void *workspace;          /* DEVICE scratch for compaction, caller-owned, or NULL: the      */
   uint64_t workspace_bytes; /*    library then uses cudaMallocAsync / cudaFreeAsync on the    */
-                            /*    stream.  Needs xt_track_workspace_bytes(n_part) bytes,      */
-                            /*    256-byte aligned; too small: XT_ERR_INVALID_ARG.  With it   */
+                            /*    stream.  xt_track_workspace_bytes(n_part) bytes, 256-byte   */
+                            /*    aligned; too small for step C: XT_ERR_INVALID_ARG.  With it */
                             /*    xt_track_ex allocates nothing.                              */
   xt_track_stats *stats;    /* HOST, optional: see xt_track_stats (makes the call synchronous) */
   int32_t cold_in_registers;/* 0: auto; 1: keep the per-particle functions of (delta, ptau) in   */
@@ -200,8 +200,10 @@ int xt_track(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64
 int xt_track_ex(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
                 void *cuda_stream, const xt_track_opts *opts);
 
-/* Bytes of device scratch step C needs for n_part particles (two working sets of 14 arrays, tile
- * counts, two counters): what xt_track_opts.workspace must provide. */
+/* Bytes of device scratch for n_part particles: what step C needs (two working sets of 14 arrays, tile
+ * counts, two counters) and, behind it, the queue of the balanced mode for the auto launch shapes.
+ * xt_track_opts.workspace should provide this much; one that only holds step C's part is accepted and
+ * the balanced mode is then not used with compaction. */
 uint64_t xt_track_workspace_bytes(int64_t n_part);
 
 /* xt_track_ex for callers that cannot allocate (code under CUDA graph capture, serving loops,
@@ -220,7 +222,8 @@ uint64_t xt_track_workspace_bytes(int64_t n_part);
  *     call clears what must start at zero itself).  Two xt_track_static calls whose GPU work can
  *     overlap (different streams, or graphs launched concurrently) RACE on it: order them on one
  *     stream or with events.  Calls on different devices do not interact.
- *   - Lattices without apertures, compact_every < 0 or n_turns <= the period never touch it. */
+ *   - Runs without compaction use at most the first bytes of it (the queue of the balanced mode,
+ *     xt_track_opts.balance) or nothing at all. */
 #define XT_TRACK_STATIC_MAX_PARTICLES 32768
 int xt_track_static(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
                     void *cuda_stream, const xt_track_opts *opts);

@@ -1383,11 +1383,11 @@ int kernel_registers(int device, int *regs) {
 }
 
 // Items of the balanced mode: about this many lattice records each (configs[2]: 4 turns, 9 ms), at most
-// kMaxBlocks blocks of turns per launch (the queue has one word per item), at least four, and more groups
+// kMaxBlocks blocks of turns per launch (the queue has one word per item), at least six, and more groups
 // than SMs (else every CTA has an SM of its own).
 constexpr int64_t kItemRecords = 12000;
 constexpr int64_t kMaxBlocks = 256;
-constexpr int64_t kMinBlocks = 4;
+constexpr int64_t kMinBlocks = 6;
 
 template <int P, bool THICK, bool REG, int NFIX>
 int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, int balance, cudaStream_t st) {
