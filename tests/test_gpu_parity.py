@@ -366,6 +366,32 @@ def test_balanced_mode_is_bit_identical(X):
     lat.close()
 
 
+def test_balanced_mode_random_shapes(X):
+    """Seeded sweep of the balanced mode over ensemble sizes (from a single particle), launch lengths (from one
+    turn), item lengths, launch shapes and compaction periods, on a lattice cut into many small chunks: every
+    run reproduces the static launch of the same length bit for bit (and terminates)."""
+    rng = np.random.default_rng(20231000)
+    full = C.particles(4)
+    lat = X.xt_lattice_create_ex(packed(4), chunk_bytes=4096)
+    cases = [(1, 1, 1, 32, 1, -1), (1, 9, 2, 128, 2, 3), (33, 1, 3, 32, 5, -1), (257, 2, 2, 128, 1, -1),
+             (384, 7, 3, 128, 7, 2), (385, 13, 3, 128, 2, 5)]
+    for _ in range(10):
+        cases.append((int(rng.integers(2, 3000)), int(rng.integers(1, 30)), int(rng.integers(1, 4)),
+                      int(rng.choice([32, 64, 128, 256])), int(rng.integers(1, 10)), int(rng.choice([-1, 3, 7]))))
+    for n, turns, ppt, block, bal, every in cases:
+        idx = np.sort(rng.choice(len(full["x"]), size=n, replace=False))
+        coords = C.subsample(full, idx)
+        a, b = X.new_particles(lat, coords), X.new_particles(lat, coords)
+        X.xt_track_ex(lat, a, turns, compact_every=-1, balance=-1)
+        X.xt_track_ex(lat, b, turns, compact_every=every, particles_per_thread=ppt, block_size=block,
+                      cold_in_registers=1, balance=bal)
+        try:
+            assert_bit_identical(X.particles_to_host(b), X.particles_to_host(a))
+        except AssertionError as e:
+            raise AssertionError("case %r: %s" % ((n, turns, ppt, block, bal, every), e))
+    lat.close()
+
+
 def test_launch_shapes_on_a_quadrupole_sextupole_lattice(X):
     """configs[1b] (orders 1 and 2 only: the kernels with those two orders fixed; single chunk, losses): every
     launch shape and both homes of the cold state reproduce the default bit for bit, in both builds; the
