@@ -1169,20 +1169,22 @@ __global__ void __maxnreg__((RegBudget<P, REG, THICK>::value)) xt_track_kernel(c
         if (my >= n_groups) {
           const unsigned int *slot = a.queue + 4 + (my - n_groups);
           it = 0xffffffffu;
-          for (;;) {
+          for (unsigned int spin = 0;; ++spin) {
             unsigned int v, fin;
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(slot) : "memory");
             if (v != 0u) {
               it = v - 1u;
               break;
             }
-            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(fin) : "l"(a.queue + 2) : "memory");
-            if (fin >= n_groups) {  // nothing will be pushed any more (a push precedes the count it enables)
-              asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(slot) : "memory");
-              if (v != 0u) it = v - 1u;
-              break;
+            if ((spin & 7u) == 7u) {  // now and then: is everything through?
+              asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(fin) : "l"(a.queue + 2) : "memory");
+              if (fin >= n_groups) {  // nothing will be pushed any more (a push precedes the count it enables)
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(slot) : "memory");
+                if (v != 0u) it = v - 1u;
+                break;
+              }
             }
-            __nanosleep(256);
+            __nanosleep(1000);  // an item lasts milliseconds
           }
           __threadfence();
         }
