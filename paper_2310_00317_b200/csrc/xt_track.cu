@@ -67,9 +67,7 @@ struct TrackArgs {
   // draw (group of particles, block of turns) items from a first-in first-out queue.  queue[0]: pop
   // tickets; queue[1]: pushes; queue[2]: finished groups; queue[4 + n]: item of push n, plus one.
   unsigned int *queue;
-  int32_t n_groups;     // groups of blockDim.x * P particles
-  int32_t block_turns;  // turns per item
-  int64_t n_items;      // items of all groups: a staggered first one, then blocks of block_turns turns
+  int32_t block_turns;  // turns per item (the first item of a group: first_block_turns)
 };
 
 __device__ __forceinline__ uint32_t smem_addr(const void *p) {
@@ -1413,14 +1411,10 @@ int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, int ba
     const int64_t n_blocks = (a.n_turns + t - 1) / t;
     const bool worth = balance > 0 || (n_blocks >= kMinBlocks && need > a.grid_quantum);
     if (worth && need * (n_blocks + 1) < 2000000000LL && t < 2000000000LL && need < 4000000) {
-      b.n_groups = static_cast<int32_t>(need);
       b.block_turns = static_cast<int32_t>(t);
-      b.n_items = 0;  // a staggered first item, then blocks of t turns
-      for (int64_t g = 0; g < need; ++g) {
-        const int64_t l0 = first_block_turns(static_cast<uint32_t>(g), t);
-        b.n_items += 1 + (a.n_turns > l0 ? (a.n_turns - l0 + t - 1) / t : 0);
-      }
-      grid = b.n_items;  // one CTA per item; the hardware starts them as slots become free
+      // one CTA per item, the hardware starts them as slots become free: a first item of 1 .. t turns per
+      // group, then blocks of t turns (an upper bound: the CTAs left over leave when every group is through)
+      grid = need * (1 + (a.n_turns - 1 + t - 1) / t);
     } else {
       b.queue = nullptr;
     }
@@ -1517,9 +1511,7 @@ int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, c
   a.tib = lat->k.tib;
   a.igam2 = lat->k.igam2;
   a.queue = (cold_in_regs && balance >= 0) ? queue : nullptr;
-  a.n_groups = 0;
   a.block_turns = 0;
-  a.n_items = 0;
   if (a.queue) {  // tickets and per-group counters start from zero
     XT_CUDA(cudaMemsetAsync(a.queue, 0, balance_scratch_bytes(n_part, block, ppt), st));
   }
