@@ -128,14 +128,17 @@ typedef struct {
                             /*    memory.                                                        */
                             /*    Launch-shape option like the two above: results are            */
                             /*    bit-identical for every shape.                                 */
-  int32_t balance;          /* small ensembles (cold state in registers) without compaction:     */
-                            /*    0: auto, -1: never, 1: always, n > 1: always, n turns per item.  */
-                            /*    The CTAs of one launch are persistent and draw (group of         */
-                            /*    particles, block of turns) items from a device counter, so that  */
-                            /*    an ensemble that does not fill a whole number of CTAs per SM     */
-                            /*    still keeps every SM busy.  Needs 4 bytes  */
-                            /*    per group of particles + 8: from `workspace` when given, else    */
-                            /*    stream-ordered.  Launch-shape option: bit-identical results.     */
+  int32_t balance;          /* launch shapes with the cold state in registers (the auto shapes  */
+                            /*    up to ~2 million particles):                                  */
+                            /*    0: auto, -1: never, 1: always, n > 1: always, n turns per item. */
+                            /*    The launch has one CTA per (group of particles, block of      */
+                            /*    turns) item and a queue of ready groups in device memory, so    */
+                            /*    that an ensemble that does not fill a whole number of CTAs per  */
+                            /*    SM still keeps every SM busy with full warps (DESIGN.md section */
+                            /*    6.2b).  Needs 4 bytes per item + 16: from `workspace` when      */
+                            /*    given, else stream-ordered.  Launch-shape option: bit-identical */
+                            /*    results.  > 0 with a shape that keeps the cold state in shared  */
+                            /*    memory: XT_ERR_INVALID_ARG.                                     */
 } xt_track_opts;
 
 /* Static description of a lattice image; counts are per turn. */
