@@ -1421,8 +1421,10 @@ int launch_track_pt(const TrackArgs &a, const xt_lattice *lat, int block, int ba
   }
   // Staging depth: as many chunks per bulk copy (fewer CTA-wide barriers per turn) as shared memory
   // allows without taking a resident CTA away.
+  // (In the balanced mode no more CTAs of an SM run at a time than there are groups per SM: configs[2] has
+  // 2.64, three resident CTAs with four chunks per stage do better than four with two, 0.612 against 0.603.)
   int64_t resident = by_regs;
-  const int64_t per_sm = (grid + a.grid_quantum - 1) / a.grid_quantum;
+  const int64_t per_sm = ((b.queue ? need : grid) + a.grid_quantum - 1) / a.grid_quantum;
   if (resident > per_sm) resident = per_sm;
   if (resident < 1) resident = 1;
   b.stage_chunks = 1;
