@@ -55,10 +55,27 @@ def test_library_loads_and_exports_every_declared_symbol(kind):
 def test_struct_layouts_match_the_header():
     # sizes the C compiler gives the public structs (LP64): 14 pointers; 2 x i64 + 2 x i32; ...
     assert ctypes.sizeof(B.xt_particles) == 14 * 8
-    assert ctypes.sizeof(B.xt_track_opts) == 56          # + workspace ptr, bytes, stats ptr, cold_in_registers
+    assert ctypes.sizeof(B.xt_track_opts) == 56          # + workspace ptr, bytes, stats ptr, cold_in_registers, balance
     assert ctypes.sizeof(B.xt_track_stats) == 7 * 8 + 3 * 8 * B.XT_STATS_MAX_PASSES
     assert ctypes.sizeof(B.xt_lattice_opts) == 16
     assert ctypes.sizeof(B.xt_lattice_info) == 8 * (5 + 8 + 3) + 8 * 3 + 8 + 8 + 8
+
+
+def test_track_workspace_bytes_holds_step_c_and_the_queue():
+    """xt_track_workspace_bytes (host arithmetic, no device): two working sets of 14 arrays for step C, and
+    behind them the queue of the balanced mode for the auto shapes (one word per item: up to 256 blocks of
+    turns per group of 256 particles); 256-byte granular, monotonic, 0 for an empty ensemble."""
+    for kind in ("prod", "nofma"):
+        assert X.xt_track_workspace_bytes(0, kind) == 0 and X.xt_track_workspace_bytes(-5, kind) == 0
+        last = 0
+        for n in (1, 31, 256, 257, 5003, 32768, 100000, 2000400, 10 ** 7):
+            b = X.xt_track_workspace_bytes(n, kind)
+            groups = -(-n // 256)
+            assert b % 256 == 0 and b >= last
+            assert b >= 2 * 14 * 8 * n + 8 * (-(-n // 256)) + 4 * 256 * groups
+            assert b <= 2 * 14 * (8 * n + 256) + 8 * groups + 4 * 256 * groups + 2048
+            last = b
+    assert X.xt_track_workspace_bytes(X.XT_TRACK_STATIC_MAX_PARTICLES) <= 8 << 20
 
 
 def test_compute_calls_validate_arguments_without_a_device():
