@@ -124,7 +124,7 @@ typedef struct {
                             /*    xt_track_ex allocates nothing.                              */
   xt_track_stats *stats;    /* HOST, optional: see xt_track_stats (makes the call synchronous) */
   int32_t cold_in_registers;/* 0: auto; 1: keep the per-particle functions of (delta, ptau) in   */
-                            /*    registers (1, 2 or 3 particles per thread); -1: in shared      */
+                            /*    registers; -1: in shared                                         */
                             /*    memory.                                                        */
                             /*    Launch-shape option like the two above: results are            */
                             /*    bit-identical for every shape.                                 */

@@ -72,7 +72,7 @@ int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part,
   bool auto_regs = false;
   if (per_sm < 4096) auto_ppt = 3;
   if (can_balance && per_sm <= balanced_up_to) {
-    auto_ppt = 3;
+    auto_ppt = 3;  // (4 per thread / registers: +2 % on the configs[3] lattice, -0.7 % on configs[4]; by option)
     auto_regs = true;
   }
   if (per_sm <= 768 || (can_balance && per_sm <= 1024)) {
@@ -92,13 +92,9 @@ int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part,
   else if (want_regs < 0)
     sh->cold_in_regs = false;
   else
-    sh->cold_in_regs = auto_regs && sh->ppt <= 3;
+    sh->cold_in_regs = auto_regs;
   if (sh->ppt < 1 || sh->ppt > 4) {
     set_error("xt_track_ex: particles_per_thread must be 0 (auto), 1, 2, 3 or 4");
-    return XT_ERR_INVALID_ARG;
-  }
-  if (sh->cold_in_regs && sh->ppt > 3) {
-    set_error("xt_track_ex: cold_in_registers needs 1, 2 or 3 particles per thread");
     return XT_ERR_INVALID_ARG;
   }
   if (sh->block < 32 || sh->block > 256 || (sh->block % 32) != 0) {

@@ -989,7 +989,7 @@ __device__ __forceinline__ const unsigned char *track_chunk(Parts<P> &q, const u
 // state (at 64 / 80 registers they spilled ~100 values around every call).
 template <int P, bool REG, bool THICK>
 struct RegBudget {
-  static constexpr int value = REG ? (P == 3 ? XT_REGS3R : (P == 2 ? 168 : 96))
+  static constexpr int value = REG ? (P == 4 ? 168 : (P == 3 ? XT_REGS3R : (P == 2 ? 168 : 96)))
                                    : (P == 1 ? (THICK ? 96 : 64) : (P == 2 ? (THICK ? 128 : 80) : (P == 3 ? XT_REGS3 : XT_REGS4)));
 };
 
@@ -1521,7 +1521,8 @@ int launch_track(const xt_lattice *lat, const xt_particles &p, int64_t n_part, c
     if (ppt == 1) return launch_track_p<1, true>(a, lat, block, balance, st);
     if (ppt == 2) return launch_track_p<2, true>(a, lat, block, balance, st);
     if (ppt == 3) return launch_track_p<3, true>(a, lat, block, balance, st);
-    set_error("xt_track: cold_in_registers needs 1, 2 or 3 particles per thread");
+    if (ppt == 4) return launch_track_p<4, true>(a, lat, block, balance, st);
+    set_error("xt_track: particles_per_thread must be 1, 2, 3 or 4");
     return XT_ERR_INVALID_ARG;
   }
   switch (ppt) {

@@ -286,12 +286,12 @@ def test_launch_shape_fusion_and_chunk_size_do_not_change_results(X):
             p = X.new_particles(lat, coords)
             X.xt_track_ex(lat, p, 6, compact_every=-1, block_size=block, particles_per_thread=ppt)
             assert_bit_identical(X.particles_to_host(p), base)
-    for ppt, cold in ((1, 1), (2, 1), (3, 1), (2, -1), (3, -1)):      # cold per-particle state in registers / shared memory
+    for ppt, cold in ((1, 1), (2, 1), (3, 1), (4, 1), (2, -1), (3, -1)):   # cold per-particle state in registers / shared memory
         p = X.new_particles(lat, coords)
         X.xt_track_ex(lat, p, 6, compact_every=-1, block_size=64, particles_per_thread=ppt, cold_in_registers=cold)
         assert_bit_identical(X.particles_to_host(p), base)
     with pytest.raises(X.XtError):
-        X.xt_track_ex(lat, X.new_particles(lat, coords), 1, particles_per_thread=4, cold_in_registers=1)
+        X.xt_track_ex(lat, X.new_particles(lat, coords), 1, particles_per_thread=5, cold_in_registers=1)
     lat.close()
     for kw in (dict(fuse=False), dict(chunk_bytes=1024), dict(chunk_bytes=65536), dict(chunk_bytes=4224, fuse=False)):
         lat2 = X.xt_lattice_create_ex(buf, **kw)
@@ -318,7 +318,7 @@ def test_balanced_mode_is_bit_identical(X):
         base = X.particles_to_host(base)
         lost = base["state"] == 0
         assert 0.05 < lost.mean() < 0.95 and len(np.unique(base["at_turn"][lost])) >= 5
-        for ppt, block, bal in ((2, 128, 2), (2, 64, 3), (1, 32, 4), (3, 96, 2), (2, 128, 1), (2, 256, 11), (1, 64, 12)):
+        for ppt, block, bal in ((2, 128, 2), (2, 64, 3), (1, 32, 4), (3, 96, 2), (4, 128, 3), (2, 128, 1), (2, 256, 11), (1, 64, 12)):
             p = X.new_particles(lat, coords)
             X.xt_track_ex(lat, p, 11, compact_every=-1, particles_per_thread=ppt, block_size=block,
                           cold_in_registers=1, balance=bal)
@@ -376,7 +376,7 @@ def test_balanced_mode_random_shapes(X):
     cases = [(1, 1, 1, 32, 1, -1), (1, 9, 2, 128, 2, 3), (33, 1, 3, 32, 5, -1), (257, 2, 2, 128, 1, -1),
              (384, 7, 3, 128, 7, 2), (385, 13, 3, 128, 2, 5)]
     for _ in range(10):
-        cases.append((int(rng.integers(2, 3000)), int(rng.integers(1, 30)), int(rng.integers(1, 4)),
+        cases.append((int(rng.integers(2, 3000)), int(rng.integers(1, 30)), int(rng.integers(1, 5)),
                       int(rng.choice([32, 64, 128, 256])), int(rng.integers(1, 10)), int(rng.choice([-1, 3, 7]))))
     for n, turns, ppt, block, bal, every in cases:
         idx = np.sort(rng.choice(len(full["x"]), size=n, replace=False))
