@@ -226,7 +226,9 @@ uint64_t xt_track_workspace_bytes(int64_t n_part);
  *     overlap (different streams, or graphs launched concurrently) RACE on it: order them on one
  *     stream or with events.  Calls on different devices do not interact.
  *   - Runs without compaction use at most the first bytes of it (the queue of the balanced mode,
- *     xt_track_opts.balance) or nothing at all. */
+ *     xt_track_opts.balance) or nothing at all.  With compaction the queue only fits behind the
+ *     working sets of smaller ensembles: otherwise the balanced mode is not used (balance > 0:
+ *     XT_ERR_INVALID_ARG). */
 #define XT_TRACK_STATIC_MAX_PARTICLES 32768
 int xt_track_static(const xt_lattice *lat, const xt_particles *p, int64_t n_part, int64_t n_turns,
                     void *cuda_stream, const xt_track_opts *opts);
