@@ -398,9 +398,10 @@ def main():
             line["roofline"]["frac_all_slots"] = None
         # DRAM bytes of one launch: not measurable inside the run (needs ncu); the number is the --set full
         # capture's dram__bytes_read + dram__bytes_write per particle scaled to this launch
-        line["roofline"]["traffic"] = 78.0 * n_part if cfg == 3 else None
-        line["roofline"]["traffic_source"] = ("ncu capture profiles/r02c_track_cfg3_summary.md: 78 B per particle "
-                                              "(reads + writes of one launch), scaled by n_part; not measured in "
+        line["roofline"]["traffic"] = 45.9 * n_part * turns if cfg == 3 else None
+        line["roofline"]["traffic_source"] = ("ncu capture profiles/r02i_track_cfg3_balanced_summary.md: 45.9 B per "
+                                              "particle-turn (reads + writes; the state of a group of particles passes "
+                                              "through HBM every four turns), scaled to the launch; not measured in "
                                               "this run") if cfg == 3 else None
         line["roofline"]["operand_pattern_ceilings_tflops"] = probe
         line["roofline"]["peak_sweep"] = {"best": best, "rows": sweep,

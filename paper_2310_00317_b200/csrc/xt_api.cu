@@ -49,14 +49,14 @@ int check_particles(const char *fn, const xt_lattice *lat, const xt_particles *p
 
 // Launch shape of the tracking kernel: threads per CTA, particles per thread, and where the cold
 // per-particle state lives.  Auto rule (measured on B200, profiles/r02_shape_sweep.md): 128-thread CTAs.
-// Many waves of particles (configs[3]: 67 568 per SM): 4 per thread, cold state in shared memory, 4 CTAs per
+// The static shape for many waves of particles: 4 per thread, cold state in shared memory, 4 CTAs per
 // SM at <= 128 registers, every CTA owning its share for the whole launch.  Up to ~12 000 per SM, when the
 // launch is long enough for the balanced mode (xt_track.cu: one CTA per (group, block of turns) item, a
 // queue of ready groups): the cold state in registers, 2 per thread up to 1024 per SM, 3 above; full
 // warps and an SM that is never short of a CTA beat the static shapes by 16-30 % there (configs[2]: 0.522 ->
 // 0.610 of the DFMA peak; 150 000 particles on the configs[3] lattice: 0.477 -> 0.619; 10^6: 0.608 ->
-// 0.644; 2 * 10^6: equal; above, the static 4-per-thread shape wins).  Launches too short for that (or
-// with compaction, whose particle count lives on the device): 2 per thread / registers up to 768 per SM
+// 0.644; 2 * 10^6: equal).  Beyond that, on thin lattices: 4 per thread in registers at a 168-register cap,
+// still balanced (configs[3]: 0.659 -> 0.662).  Launches too short for that: 2 per thread / registers up to 768 per SM
 // (configs[2] statically: 0.524 against 0.511 for 3 per thread), 3 per thread / shared memory up to 4096,
 // 4 above.  Below ~100 particles per SM one per thread keeps more warps alive.
 struct Shape {
@@ -71,6 +71,7 @@ int resolve_shape(const xt_track_opts *o, const xt_lattice *lat, int64_t n_part,
   int auto_ppt = 4, auto_block = 128;
   bool auto_regs = false;
   if (per_sm < 4096) auto_ppt = 3;
+  if (can_balance && per_sm > balanced_up_to && !lat->extended) auto_regs = true;  // 4 per thread, balanced
   if (can_balance && per_sm <= balanced_up_to) {
     auto_ppt = 3;  // (4 per thread / registers: +2 % on the configs[3] lattice, -0.7 % on configs[4]; by option)
     auto_regs = true;
